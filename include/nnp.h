@@ -1,0 +1,161 @@
+/* nnp.h -- C ABI of libnnp_b200: Behler-Parrinello neural-network-potential (NNP)
+ * energy + force evaluation on one NVIDIA B200 (sm_100a).
+ *
+ * What it computes: the per-timestep NNP kernel of arXiv 2002.00054 section 3.1,
+ * Fig. 1(b): step 1 atom-centred symmetry functions ("Gaussian
+ * functions of neighbor distances with radial or angular character", L34), step 2
+ * one small feed-forward network per atom giving the atomic energy, step 3 forces
+ * from the gradient of the network w.r.t. the descriptors times the gradient of the
+ * descriptors w.r.t. coordinates, with dG/dr recomputed instead of stored (L56-58,
+ * L98, L124), preceded by a periodic cell-list neighbour build (L48, L116).
+ * The paper prints no formulas; the exact definitions used (cosine cutoff, n2p2
+ * type-2 radial and type-3 "narrow" angular functions, softplus networks) are listed
+ * in DESIGN.md "Readings" and restated at nnp_sf below.
+ *
+ * Conventions
+ *   - units: Angstrom, eV (whatever the weights encode); all floating point is FP64.
+ *   - "device" pointers are CUDA device memory on the model's device; "host" pointers
+ *     are ordinary (preferably pinned) host memory.
+ *   - nothing here allocates per call except nnp_compute_host (library-owned, cached).
+ *   - every function returns an nnp_status; no exceptions, no abort() across the ABI.
+ *     Argument errors are returned synchronously.  Errors detected on the device
+ *     (neighbour overflow, non-finite input) are reported by nnp_sync_status().
+ *   - nnp_compute enqueues work on the caller's stream and returns without
+ *     synchronising.  There is no CPU fallback: without a CUDA device every entry
+ *     point that needs one returns NNP_ERR_CUDA.
+ *   - a model is not thread-safe; use one model per host thread / stream.
+ */
+#ifndef NNP_H_
+#define NNP_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nnp_model nnp_model; /* opaque, owned by the library */
+
+typedef enum {
+    NNP_OK = 0,
+    NNP_ERR_INVALID_ARG = 1,       /* null pointer, bad size, unsupported SF parameter */
+    NNP_ERR_BOX_TOO_SMALL = 2,     /* some box length < 2*rc (minimum image would be ambiguous) */
+    NNP_ERR_TYPE_RANGE = 3,        /* an atom type outside [0, n_elem)  (device-detected) */
+    NNP_ERR_NEIGHBOR_OVERFLOW = 4, /* an atom has more neighbours than max_neighbors (device-detected) */
+    NNP_ERR_WORKSPACE = 5,         /* workspace pointer null / misaligned / too small */
+    NNP_ERR_CUDA = 6,              /* CUDA runtime error; see nnp_last_error */
+    NNP_ERR_NONFINITE = 7          /* NaN/Inf in positions (device-detected) */
+} nnp_status;
+
+/* One symmetry function of central element `central` (n2p2 numbering, C2-C5).
+ *   kind 2 (radial):  G = sum_{j in N(i), t_j = e1} exp(-eta (r_ij - rs)^2) fc(r_ij)
+ *   kind 3 (angular, narrow): with a=r_ij, b=r_ik, c=r_jk, cos = u.v/(ab),
+ *       G = 2^(1-zeta) sum_{j<k in N(i), {t_j,t_k} = {e1,e2}, c < rc}
+ *               (1 + lambda cos)^zeta  exp(-eta (a^2+b^2+c^2))  fc(a) fc(b) fc(c)
+ *   fc(r) = (cos(pi r / rc) + 1)/2 for r < rc, else 0;  N(i) = { j != i : r_ij^2 < rc^2 }.
+ * Constraints (else NNP_ERR_INVALID_ARG): eta >= 0; kind 3 needs lambda = +1 or -1 and
+ * zeta an integer in [1, 64]; rs is used by kind 2 only.  The order of the entries with
+ * equal `central` is the order of that element's descriptor vector G (= network input). */
+typedef struct {
+    int32_t central;
+    int32_t kind;
+    int32_t e1, e2;
+    double eta, rs, lambda, zeta;
+} nnp_sf;
+
+/* Create a model on CUDA device `cuda_device`.
+ *   n_elem        number of elements (1..4); atom types are indices into elem_names.
+ *   elem_names    [n_elem] NUL-terminated names (copied; informational).
+ *   rc            cutoff radius (> 0), one for all symmetry functions.
+ *   sf            [n_sf] symmetry functions, all elements together (copied).
+ *   n_layers      [n_elem] number of weight layers of each element's network (>= 1).
+ *   layer_sizes   [n_elem] -> [n_layers[e]+1] sizes; first = number of SFs with central == e,
+ *                 last = 1.  Hidden widths <= 256.
+ *   weights       [n_elem] -> flat row-major  W1[out][in], b1[out], W2, b2, ...  (copied).
+ *                 Hidden layers use softplus log(1+e^x); the output layer is linear.
+ * All inputs are host memory and are not referenced after return. */
+nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* const* elem_names, double rc,
+                      int32_t n_sf, const nnp_sf* sf, const int32_t* n_layers,
+                      const int32_t* const* layer_sizes, const double* const* weights,
+                      int32_t cuda_device);
+
+/* Free the model and everything the library allocated for it.  NULL is allowed. */
+void nnp_destroy(nnp_model* m);
+
+/* Upper bound on neighbours per atom the kernels provision for (default 160; the
+ * water-like workloads average 91, Poisson tail < 150 at 2.1 M atoms).  Range 32..255. */
+nnp_status nnp_set_max_neighbors(nnp_model* m, int32_t max_neighbors);
+
+/* Bytes of device workspace nnp_compute needs for n_atoms (0 on error). */
+size_t nnp_workspace_bytes(const nnp_model* m, int64_t n_atoms);
+
+/* One energy + force evaluation (Fig. 1(b) steps 1-3 after the neighbour build).
+ *   d_pos        [n_atoms][3] device, any real coordinates (wrapped into the box internally)
+ *   d_type       [n_atoms]    device, element index per atom
+ *   box          [3] HOST, orthorhombic box lengths, origin 0; each must be >= 2*rc
+ *   d_e_atom     [n_atoms]    device out, atomic energies E_i, caller's atom order
+ *   d_e_total    [1]          device out, E = sum_i E_i (deterministic summation order)
+ *   d_force      [n_atoms][3] device out, F_m = - sum_i sum_s dE_i/dG_is * dG_is/dr_m
+ *   d_workspace  device, 256-byte aligned, >= nnp_workspace_bytes(m, n_atoms); owned by the
+ *                caller; it also holds the neighbour list / G read by the nnp_get_* calls, so
+ *                keep it alive until those are done.
+ *   cuda_stream  a cudaStream_t (NULL = default stream); all work is enqueued there.
+ * n_atoms == 0 is allowed (writes e_total = 0). */
+nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d_pos, const int32_t* d_type,
+                       const double box[3], double* d_e_atom, double* d_e_total, double* d_force,
+                       void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* Same evaluation with HOST buffers: copies pos/type to the device, runs nnp_compute on an
+ * internal stream with library-owned (cached) device buffers, copies e_atom / e_total / force
+ * back and synchronises.  Returns device-detected errors too. */
+nnp_status nnp_compute_host(nnp_model* m, int64_t n_atoms, const double* h_pos, const int32_t* h_type,
+                            const double box[3], double* h_e_atom, double* h_e_total, double* h_force);
+
+/* Synchronise the stream of the last nnp_compute and return its device-side status. */
+nnp_status nnp_sync_status(nnp_model* m);
+
+/* Debug / parity exports of the LAST nnp_compute (they synchronise its stream first).
+ * Atom indices and row order are the CALLER's; all pointers are device memory.
+ *   nnp_get_neighbor_counts: d_counts[n_atoms] = |N(i)|.
+ *   nnp_get_neighbors: d_offsets[n_atoms+1] (exclusive prefix sum of the counts) and
+ *                      d_idx[total] with every row sorted ascending.  d_idx may be NULL to get
+ *                      offsets only; `idx_capacity` = number of int32 entries d_idx can hold.
+ *   nnp_get_sf / nnp_get_dedg: [n_atoms][g_stride] with g_stride = nnp_g_stride(m)
+ *                      (= max SFs per element; unused tail entries are 0). */
+nnp_status nnp_get_neighbor_counts(nnp_model* m, int32_t* d_counts);
+nnp_status nnp_get_neighbors(nnp_model* m, int64_t* d_offsets, int32_t* d_idx, int64_t idx_capacity);
+nnp_status nnp_get_sf(nnp_model* m, double* d_G);
+nnp_status nnp_get_dedg(nnp_model* m, double* d_dEdG);
+int32_t nnp_g_stride(const nnp_model* m);
+
+/* Per-stage device times of nnp_compute.  Off by default (no events recorded).
+ * ms[NNP_N_STAGES]: 0 wrap+bin+sort, 1 neighbour list, 2 symmetry functions,
+ * 3 networks fwd+bwd, 4 forces, 5 reduce+un-permute.  Synchronises the stream. */
+#define NNP_N_STAGES 6
+nnp_status nnp_set_timing(nnp_model* m, int32_t enabled);
+nnp_status nnp_get_timings(nnp_model* m, double* ms);
+
+/* Number of kernels the last nnp_compute launched (for launch accounting). */
+int32_t nnp_last_launch_count(const nnp_model* m);
+
+/* 1 if the model's angular symmetry functions run on a specialised kernel, 0 if on the
+ * generic (slower, any-table) kernel. */
+int32_t nnp_uses_fast_path(const nnp_model* m);
+
+/* Measure the FP64 FMA issue rate of the device (independent DFMA chains on every SM):
+ * thread-level DFMA instructions per second, *dfma_per_s = best 10-launch burst,
+ * *dfma_per_s_sustained (may be NULL) = mean over the whole `seconds`.  Roofline denominator. */
+nnp_status nnp_measure_fp64_peak(int32_t cuda_device, double seconds, double* dfma_per_s,
+                                 double* dfma_per_s_sustained);
+
+/* Last error text for this model (never NULL).  nnp_create failures: pass NULL. */
+const char* nnp_last_error(const nnp_model* m);
+
+/* "major.minor" of this library. */
+const char* nnp_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NNP_H_ */

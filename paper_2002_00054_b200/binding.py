@@ -1,0 +1,261 @@
+"""Thin ctypes binding of libnnp_b200.so (C ABI: include/nnp.h).  Argument marshalling
+only -- every step of the path runs in the CUDA kernels.  PyTorch is used for device
+memory and streams.  There is no CPU fallback: if the library is missing or there is no
+CUDA device the calls raise."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libnnp_b200.so")
+
+NNP_OK = 0
+STATUS_NAMES = {0: "NNP_OK", 1: "NNP_ERR_INVALID_ARG", 2: "NNP_ERR_BOX_TOO_SMALL", 3: "NNP_ERR_TYPE_RANGE",
+                4: "NNP_ERR_NEIGHBOR_OVERFLOW", 5: "NNP_ERR_WORKSPACE", 6: "NNP_ERR_CUDA", 7: "NNP_ERR_NONFINITE"}
+N_STAGES = 6
+STAGE_NAMES = ("sort", "neighbors", "symmetry_functions", "networks", "forces", "finalize")
+
+# every symbol include/nnp.h declares
+EXPORTS = ("nnp_create", "nnp_destroy", "nnp_set_max_neighbors", "nnp_workspace_bytes", "nnp_compute",
+           "nnp_compute_host", "nnp_sync_status", "nnp_get_neighbor_counts", "nnp_get_neighbors", "nnp_get_sf",
+           "nnp_get_dedg", "nnp_g_stride", "nnp_set_timing", "nnp_get_timings", "nnp_last_launch_count",
+           "nnp_uses_fast_path", "nnp_measure_fp64_peak", "nnp_last_error", "nnp_version")
+
+
+class NNPError(RuntimeError):
+    def __init__(self, status, msg=""):
+        self.status = status
+        super().__init__("%s: %s" % (STATUS_NAMES.get(status, status), msg))
+
+
+class _SF(C.Structure):
+    _fields_ = [("central", C.c_int32), ("kind", C.c_int32), ("e1", C.c_int32), ("e2", C.c_int32),
+                ("eta", C.c_double), ("rs", C.c_double), ("lam", C.c_double), ("zeta", C.c_double)]
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree library (fails loudly if it has not been built)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise OSError("libnnp_b200.so is not built: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                      "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    L.nnp_create.restype = C.c_int
+    L.nnp_create.argtypes = [C.POINTER(vp), i32, C.POINTER(C.c_char_p), dbl, i32, vp, vp, C.POINTER(vp),
+                             C.POINTER(vp), i32]
+    L.nnp_destroy.restype = None
+    L.nnp_destroy.argtypes = [vp]
+    L.nnp_set_max_neighbors.restype = C.c_int
+    L.nnp_set_max_neighbors.argtypes = [vp, i32]
+    L.nnp_workspace_bytes.restype = C.c_size_t
+    L.nnp_workspace_bytes.argtypes = [vp, i64]
+    L.nnp_compute.restype = C.c_int
+    L.nnp_compute.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), vp, vp, vp, vp, C.c_size_t, vp]
+    L.nnp_compute_host.restype = C.c_int
+    L.nnp_compute_host.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), vp, vp, vp]
+    L.nnp_sync_status.restype = C.c_int
+    L.nnp_sync_status.argtypes = [vp]
+    L.nnp_get_neighbor_counts.restype = C.c_int
+    L.nnp_get_neighbor_counts.argtypes = [vp, vp]
+    L.nnp_get_neighbors.restype = C.c_int
+    L.nnp_get_neighbors.argtypes = [vp, vp, vp, i64]
+    L.nnp_get_sf.restype = C.c_int
+    L.nnp_get_sf.argtypes = [vp, vp]
+    L.nnp_get_dedg.restype = C.c_int
+    L.nnp_get_dedg.argtypes = [vp, vp]
+    L.nnp_g_stride.restype = i32
+    L.nnp_g_stride.argtypes = [vp]
+    L.nnp_set_timing.restype = C.c_int
+    L.nnp_set_timing.argtypes = [vp, i32]
+    L.nnp_get_timings.restype = C.c_int
+    L.nnp_get_timings.argtypes = [vp, C.POINTER(dbl)]
+    L.nnp_last_launch_count.restype = i32
+    L.nnp_last_launch_count.argtypes = [vp]
+    L.nnp_uses_fast_path.restype = i32
+    L.nnp_uses_fast_path.argtypes = [vp]
+    L.nnp_measure_fp64_peak.restype = C.c_int
+    L.nnp_measure_fp64_peak.argtypes = [i32, dbl, C.POINTER(dbl), C.POINTER(dbl)]
+    L.nnp_last_error.restype = C.c_char_p
+    L.nnp_last_error.argtypes = [vp]
+    L.nnp_version.restype = C.c_char_p
+    L.nnp_version.argtypes = []
+    _lib = L
+    return L
+
+
+def measure_fp64_peak(device: int = 0, seconds: float = 0.5):
+    """-> (burst, sustained) thread-level DFMA instructions per second."""
+    L = load_library()
+    a, b = C.c_double(0.0), C.c_double(0.0)
+    st = L.nnp_measure_fp64_peak(device, seconds, C.byref(a), C.byref(b))
+    if st != NNP_OK:
+        raise NNPError(st, "nnp_measure_fp64_peak")
+    return a.value, b.value
+
+
+class NNP:
+    """nnp_create / nnp_compute with torch tensors as device buffers.
+
+    elements: names; rc: cutoff; sf: structured array (central, kind, e1, e2, eta, rs, lam, zeta);
+    layer_sizes / weights: per element (see include/nnp.h)."""
+
+    def __init__(self, elements, rc, sf, layer_sizes, weights, device: int = 0):
+        import torch  # device memory + streams only
+        self._torch = torch
+        self._L = load_library()
+        self._h = C.c_void_p(None)
+        self.device = int(device)
+        sf = np.ascontiguousarray(sf)
+        if sf.dtype.itemsize != C.sizeof(_SF):
+            raise ValueError("sf must have 48-byte records")
+        n_elem = len(elements)
+        names = (C.c_char_p * n_elem)(*[str(e).encode() for e in elements])
+        n_layers = np.array([len(ls) - 1 for ls in layer_sizes], dtype=np.int32)
+        ls_arrays = [np.ascontiguousarray(ls, dtype=np.int32) for ls in layer_sizes]
+        w_arrays = [np.ascontiguousarray(w, dtype=np.float64) for w in weights]
+        ls_ptrs = (C.c_void_p * n_elem)(*[a.ctypes.data for a in ls_arrays])
+        w_ptrs = (C.c_void_p * n_elem)(*[a.ctypes.data for a in w_arrays])
+        st = self._L.nnp_create(C.byref(self._h), n_elem, names, float(rc), int(sf.shape[0]),
+                                sf.ctypes.data_as(C.c_void_p), n_layers.ctypes.data_as(C.c_void_p),
+                                ls_ptrs, w_ptrs, self.device)
+        if st != NNP_OK:
+            msg = self._L.nnp_last_error(None).decode()
+            self._h = C.c_void_p(None)
+            raise NNPError(st, msg)
+        self.n_elem = n_elem
+        self.rc = float(rc)
+        self.g_stride = int(self._L.nnp_g_stride(self._h))
+        self._ws = None
+        self._ws_n = -1
+
+    @classmethod
+    def from_model(cls, model, device: int = 0):
+        """model: any object with .elements .rc .sf .layer_sizes .weights (e.g. workloads.Model)."""
+        return cls(model.elements, model.rc, model.sf, model.layer_sizes, model.weights, device)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._L.nnp_destroy(self._h)
+            self._h = C.c_void_p(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st):
+        if st != NNP_OK:
+            raise NNPError(st, self._L.nnp_last_error(self._h).decode())
+
+    # ---- configuration -------------------------------------------------------------------
+    def set_max_neighbors(self, k: int):
+        self._check(self._L.nnp_set_max_neighbors(self._h, int(k)))
+        self._ws = None
+        self._ws_n = -1
+
+    def set_timing(self, on: bool):
+        self._check(self._L.nnp_set_timing(self._h, 1 if on else 0))
+
+    def uses_fast_path(self) -> bool:
+        return bool(self._L.nnp_uses_fast_path(self._h))
+
+    def workspace_bytes(self, n_atoms: int) -> int:
+        return int(self._L.nnp_workspace_bytes(self._h, int(n_atoms)))
+
+    # ---- the hot path ----------------------------------------------------------------------
+    def compute(self, pos, types, box, out=None, sync=True):
+        """pos [N,3] f64 cuda tensor, types [N] i32 cuda tensor, box 3 floats (host).
+        -> (e_atom [N], e_total [1], force [N,3]) cuda tensors.  Enqueued on torch's current stream."""
+        torch = self._torch
+        n = int(pos.shape[0])
+        assert pos.is_cuda and pos.dtype == torch.float64 and pos.is_contiguous()
+        assert types.is_cuda and types.dtype == torch.int32 and types.is_contiguous()
+        dev = pos.device
+        if self._ws is None or self._ws_n != n:
+            nbytes = self.workspace_bytes(n)
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev)
+            self._ws_n = n
+        ws_ptr = (self._ws.data_ptr() + 255) // 256 * 256
+        if out is None:
+            e_atom = torch.empty(n, dtype=torch.float64, device=dev)
+            e_total = torch.empty(1, dtype=torch.float64, device=dev)
+            force = torch.empty((n, 3), dtype=torch.float64, device=dev)
+        else:
+            e_atom, e_total, force = out
+        boxc = (C.c_double * 3)(*[float(b) for b in box])
+        stream = torch.cuda.current_stream(dev).cuda_stream
+        st = self._L.nnp_compute(self._h, n, C.c_void_p(pos.data_ptr()), C.c_void_p(types.data_ptr()), boxc,
+                                 C.c_void_p(e_atom.data_ptr()), C.c_void_p(e_total.data_ptr()),
+                                 C.c_void_p(force.data_ptr()), C.c_void_p(ws_ptr),
+                                 self._ws.numel() - (ws_ptr - self._ws.data_ptr()), C.c_void_p(stream))
+        self._check(st)
+        if sync:
+            self.sync_status()
+        return e_atom, e_total, force
+
+    def compute_host(self, pos, types, box, out=None):
+        """Same evaluation with HOST numpy / pinned-torch buffers (copies inside the call)."""
+        def ptr(a):
+            return C.c_void_p(a.data_ptr()) if hasattr(a, "data_ptr") else a.ctypes.data_as(C.c_void_p)
+        n = int(pos.shape[0])
+        if out is None:
+            e_atom = np.empty(n, dtype=np.float64)
+            e_total = np.empty(1, dtype=np.float64)
+            force = np.empty((n, 3), dtype=np.float64)
+        else:
+            e_atom, e_total, force = out
+        boxc = (C.c_double * 3)(*[float(b) for b in box])
+        st = self._L.nnp_compute_host(self._h, n, ptr(pos), ptr(types), boxc, ptr(e_atom), ptr(e_total), ptr(force))
+        self._check(st)
+        return e_atom, e_total, force
+
+    def sync_status(self):
+        self._check(self._L.nnp_sync_status(self._h))
+
+    def last_launch_count(self) -> int:
+        return int(self._L.nnp_last_launch_count(self._h))
+
+    def timings_ms(self):
+        ms = (C.c_double * N_STAGES)()
+        self._check(self._L.nnp_get_timings(self._h, ms))
+        return dict(zip(STAGE_NAMES, [float(x) for x in ms]))
+
+    # ---- debug / parity exports of the last compute ----------------------------------------------
+    def neighbors(self, n_atoms: int):
+        """-> (offsets int64[N+1], idx int32[total]) cuda tensors; caller's atom ids, rows ascending."""
+        torch = self._torch
+        dev = torch.device("cuda", self.device)
+        off = torch.empty(n_atoms + 1, dtype=torch.int64, device=dev)
+        self._check(self._L.nnp_get_neighbors(self._h, C.c_void_p(off.data_ptr()), None, 0))
+        total = int(off[-1].item()) if n_atoms > 0 else 0
+        idx = torch.empty(max(total, 1), dtype=torch.int32, device=dev)
+        self._check(self._L.nnp_get_neighbors(self._h, C.c_void_p(off.data_ptr()), C.c_void_p(idx.data_ptr()), total))
+        return off, idx[:total]
+
+    def neighbor_counts(self, n_atoms: int):
+        torch = self._torch
+        c = torch.empty(max(n_atoms, 1), dtype=torch.int32, device=torch.device("cuda", self.device))
+        self._check(self._L.nnp_get_neighbor_counts(self._h, C.c_void_p(c.data_ptr())))
+        return c[:n_atoms]
+
+    def symmetry_functions(self, n_atoms: int):
+        torch = self._torch
+        g = torch.empty((max(n_atoms, 1), self.g_stride), dtype=torch.float64, device=torch.device("cuda", self.device))
+        self._check(self._L.nnp_get_sf(self._h, C.c_void_p(g.data_ptr())))
+        return g[:n_atoms]
+
+    def dedg(self, n_atoms: int):
+        torch = self._torch
+        g = torch.empty((max(n_atoms, 1), self.g_stride), dtype=torch.float64, device=torch.device("cuda", self.device))
+        self._check(self._L.nnp_get_dedg(self._h, C.c_void_p(g.data_ptr())))
+        return g[:n_atoms]

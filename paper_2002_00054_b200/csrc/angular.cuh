@@ -1,0 +1,176 @@
+// angular.cuh -- pieces shared by the symmetry-function kernel (k_sf.cu) and the force kernel
+// (k_force.cu): compile-time descriptions of angular pair groups, per-warp shared-memory
+// layout of a centre's neighbourhood, and the triplet enumeration with warp compaction.
+//
+// Design: one warp owns one centre atom.  Its neighbours are staged once
+// in shared memory (min-image vectors, 1/r, cutoff values, per-eta Gaussians); candidate
+// (j,k) pairs are enumerated in "tournament" order (round r pairs slot j with slot j+r), the
+// cheap r_jk < rc test is ballot-compacted into a small queue, and the expensive per-triplet
+// work runs only on full batches of 32 contributing triplets -> no idle lanes in the hot loop
+// even though only ~47 % of the enumerated pairs contribute.
+#pragma once
+#include "nnp_internal.h"
+
+namespace nnp {
+
+// ---------------------------------------------------------------- compile-time group specs
+// A specialised group is: NETA distinct etas with eta_e = eta_{RBASE(e)} * RATIO(e) (integer
+// ratios -> exp(-eta_e x) is a short multiplication chain of exp(-eta_0 x)), and per eta a
+// bit mask of (lambda, zeta) menu entries: bit b (0..6) = lambda +1, zeta 2^b; bit 8+b =
+// lambda -1, zeta 2^b.
+
+struct SpecGeneric {
+    static constexpr int ID = ANG_GENERIC;
+    static constexpr int NETA = 0;
+    static constexpr int MAXBIT = 0;
+    static constexpr int NACC = 0;
+    __host__ __device__ static constexpr unsigned mask(int) { return 0u; }
+    __host__ __device__ static constexpr int ratio(int) { return 1; }
+    __host__ __device__ static constexpr int rbase(int) { return 0; }
+};
+
+// BASELINE.json base set (reading C8): eta0 x {+-1} x {1,2,4,16}  +  10*eta0 x {+1} x {1,2,4,16}
+struct SpecBase12 {
+    static constexpr int ID = ANG_BASE12;
+    static constexpr int NETA = 2;
+    static constexpr int MAXBIT = 4;
+    static constexpr int NACC = 12;
+    __host__ __device__ static constexpr unsigned mask(int e) { return e == 0 ? 0x1717u : (e == 1 ? 0x0017u : 0u); }
+    __host__ __device__ static constexpr int ratio(int e) { return e == 1 ? 10 : 1; }
+    __host__ __device__ static constexpr int rbase(int) { return 0; }
+};
+
+// wide set (reading C9): eta0 x {1,3,10,30}, each x {+-1} x {1,2,4,16}
+struct SpecWide32 {
+    static constexpr int ID = ANG_WIDE32;
+    static constexpr int NETA = 4;
+    static constexpr int MAXBIT = 4;
+    static constexpr int NACC = 32;
+    __host__ __device__ static constexpr unsigned mask(int e) { return e < 4 ? 0x1717u : 0u; }
+    __host__ __device__ static constexpr int ratio(int e) { return e == 1 ? 3 : (e == 2 ? 10 : (e == 3 ? 3 : 1)); }
+    __host__ __device__ static constexpr int rbase(int e) { return e == 3 ? 2 : 0; }
+};
+
+// accumulator slot of menu entry (e, bit) = number of set menu bits before it
+template <class Spec>
+__host__ __device__ constexpr int acc_index(int e, int bit) {
+    int n = 0;
+    for (int ee = 0; ee < Spec::NETA; ++ee)
+        for (int b = 0; b < 16; ++b) {
+            if (ee == e && b == bit) return n;
+            if (Spec::mask(ee) >> b & 1u) ++n;
+        }
+    return n;
+}
+
+template <int K>
+__device__ __forceinline__ double ipow(double x) {
+    if constexpr (K <= 1) return x;
+    else if constexpr (K % 2 == 0) { const double h = ipow<K / 2>(x); return h * h; }
+    else return x * ipow<K - 1>(x);
+}
+
+// E[e] = exp(-eta_e * x) for all etas of the spec from ONE exp() and multiplication chains
+template <class Spec>
+__device__ __forceinline__ void eta_chain(double x, double eta0, double* E) {
+    E[0] = exp(-eta0 * x);
+    if constexpr (Spec::NETA > 1) E[1] = ipow<Spec::ratio(1)>(E[Spec::rbase(1)]);
+    if constexpr (Spec::NETA > 2) E[2] = ipow<Spec::ratio(2)>(E[Spec::rbase(2)]);
+    if constexpr (Spec::NETA > 3) E[3] = ipow<Spec::ratio(3)>(E[Spec::rbase(3)]);
+}
+
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+    return v;
+}
+
+// ---------------------------------------------------------------- per-warp neighbourhood in smem
+// Slot m (0..n-1) of the centre's neighbour row, grouped by element.  Packed as double2 so the
+// per-triplet gathers are 128-bit shared loads.
+struct Nbh {
+    double2* p0;   // (ux, uy)
+    double2* p1;   // (uz, 1/a)
+    double2* p2;   // (fc(a), a) in the SF kernel; (fc(a), fc'(a)/a) in the force kernel
+    double* pe;    // [slot * NETA + e]: SF kernel: exp(-eta_e a^2) * fc(a); force kernel: exp(-eta_e a^2)
+};
+
+// ---------------------------------------------------------------- triplet enumeration
+// Calls f(j, k, active) for batches of 32 contributing pairs (c^2 < rc2).  `queue` is 64 uint16
+// per warp.  Pairs inside one segment [s, s+ns) use the tournament order: round r = 1..ns/2 pairs
+// slot j with (j + r) mod ns, which visits each unordered pair once and keeps the j's (and the
+// k's) of one round all distinct -- the force kernel relies on that to keep shared-memory
+// atomic conflicts rare.
+struct PairQueue {
+    uint16_t* q;
+    int n;
+};
+
+template <class F>
+__device__ __forceinline__ void push_and_drain(PairQueue& Q, bool pass, int j, int k, int lane, F& f) {
+    const unsigned m = __ballot_sync(0xffffffffu, pass);
+    if (pass) Q.q[Q.n + __popc(m & ((1u << lane) - 1u))] = (uint16_t)((j << 8) | k);
+    Q.n += __popc(m);
+    __syncwarp();
+    if (Q.n >= 32) {
+        const unsigned e = Q.q[Q.n - 32 + lane];
+        Q.n -= 32;
+        __syncwarp();
+        f((int)(e >> 8), (int)(e & 255u), true);
+    }
+}
+
+template <class F>
+__device__ __forceinline__ void drain_tail(PairQueue& Q, int lane, F& f) {
+    if (Q.n > 0) {
+        const bool act = lane < Q.n;
+        const unsigned e = Q.q[act ? lane : 0];
+        Q.n = 0;
+        __syncwarp();
+        f((int)(e >> 8), (int)(e & 255u), act);
+    }
+    __syncwarp();
+}
+
+__device__ __forceinline__ bool pair_close(const Nbh& nb, int j, int k, double rc2) {
+    const double2 a0 = nb.p0[j], b0 = nb.p0[k];
+    const double az = nb.p1[j].x, bz = nb.p1[k].x;
+    const double wx = b0.x - a0.x, wy = b0.y - a0.y, wz = bz - az;
+    return wx * wx + wy * wy + wz * wz < rc2;
+}
+
+// all unordered pairs inside segment [s, s+ns)
+template <class F>
+__device__ __forceinline__ void enum_within(const Nbh& nb, int s, int ns, double rc2, PairQueue& Q, int lane, F& f) {
+    const int rounds = ns / 2;                 // r = 1..rounds; for even ns the last round is half
+    for (int r = 1; r <= rounds; ++r) {
+        const int lim = (2 * r == ns) ? ns / 2 : ns;
+        for (int j0 = 0; j0 < lim; j0 += 32) {
+            const int jj = j0 + lane;
+            int kk = jj + r;
+            if (kk >= ns) kk -= ns;
+            const bool valid = jj < lim;
+            const bool pass = valid && pair_close(nb, s + jj, s + kk, rc2);
+            push_and_drain(Q, pass, s + jj, s + kk, lane, f);
+        }
+    }
+}
+
+// all pairs (j in [s1, s1+n1), k in [s2, s2+n2)), disjoint segments
+template <class F>
+__device__ __forceinline__ void enum_between(const Nbh& nb, int s1, int n1, int s2, int n2, double rc2, PairQueue& Q,
+                                             int lane, F& f) {
+    if (n1 == 0 || n2 == 0) return;
+    for (int j0 = 0; j0 < n1; j0 += 32) {
+        const int jj = j0 + lane;
+        const bool valid = jj < n1;
+        int kk = jj % n2;                      // start of this lane's diagonal
+        for (int r = 0; r < n2; ++r) {
+            const bool pass = valid && pair_close(nb, s1 + jj, s2 + kk, rc2);
+            push_and_drain(Q, pass, s1 + jj, s2 + kk, lane, f);
+            if (++kk == n2) kk = 0;
+        }
+    }
+}
+
+}  // namespace nnp

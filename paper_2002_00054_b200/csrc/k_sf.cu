@@ -1,0 +1,265 @@
+// k_sf.cu -- S2: atom-centred symmetry functions G_i (PAPER.md L40 step 1: radial descriptors,
+// plus "a similar angular computation with one extra loop over neighbors of neighbors";
+// formulas: include/nnp.h at nnp_sf, readings 2-4).
+//
+// One warp per centre.  Radial and angular parts share the staged neighbourhood, so they are
+// ONE kernel here (the paper splits them, L98, because its parallel_for has no shared staging).
+// FP64-ALU bound: ~93 FP64 instructions per contributing triplet, ~1,940 triplets per atom.
+#include "angular.cuh"
+#include "geometry.cuh"
+
+namespace nnp {
+
+constexpr int SF_WARPS = 4;
+
+struct SfParams {
+    int64_t n;
+    int n_elem, ncell, stride, cap, g_stride;
+    double rc, rc2, inv_rc;
+    double box[3], half[3];
+    const double *sx, *sy, *sz;
+    const int32_t *cell_start, *nbr, *nbr_cnt;
+    double* G;
+    const ElemProgram* prog[MAX_ELEM];
+    int variant[MAX_ELEM];
+};
+
+template <class Spec>
+__host__ __device__ constexpr size_t sf_warp_smem(int cap) {
+    // p0, p1, p2 (double2 each) + pe (NETA doubles) per slot, queue (64 x u16), generic accumulators
+    return (size_t)cap * (48 + 8 * Spec::NETA) + 128 + (Spec::ID == ANG_GENERIC ? 64 * 8 : 0);
+}
+
+// ---- per-triplet work, specialised groups -------------------------------------------------
+template <class Spec>
+struct SfTripletFast {
+    const Nbh& nb;
+    double eta0, inv_rc;
+    double acc[Spec::NACC > 0 ? Spec::NACC : 1];
+
+    __device__ __forceinline__ SfTripletFast(const Nbh& nb_, double eta0_, double inv_rc_)
+        : nb(nb_), eta0(eta0_), inv_rc(inv_rc_) {
+#pragma unroll
+        for (int a = 0; a < Spec::NACC; ++a) acc[a] = 0.0;
+    }
+
+    __device__ __forceinline__ void operator()(int j, int k, bool active) {
+        const double2 j0 = nb.p0[j], j1 = nb.p1[j], k0 = nb.p0[k], k1 = nb.p1[k];
+        const double wx = k0.x - j0.x, wy = k0.y - j0.y, wz = k1.x - j1.x;
+        const double c2 = wx * wx + wy * wy + wz * wz;
+        const double c = sqrt(c2);
+        double fcc = 0.5 * cospi(c * inv_rc) + 0.5;
+        if (!active) fcc = 0.0;
+        double Ec[Spec::NETA];
+        eta_chain<Spec>(c2, eta0, Ec);
+        const double cosv = (j0.x * k0.x + j0.y * k0.y + j1.x * k1.x) * (j1.y * k1.y);
+        double pw[2][Spec::MAXBIT + 1];
+        pw[0][0] = 1.0 + cosv;
+        pw[1][0] = 1.0 - cosv;
+#pragma unroll
+        for (int b = 1; b <= Spec::MAXBIT; ++b) {
+            pw[0][b] = pw[0][b - 1] * pw[0][b - 1];
+            pw[1][b] = pw[1][b - 1] * pw[1][b - 1];
+        }
+#pragma unroll
+        for (int e = 0; e < Spec::NETA; ++e) {
+            const double xc = (nb.pe[j * Spec::NETA + e] * nb.pe[k * Spec::NETA + e]) * (Ec[e] * fcc);
+#pragma unroll
+            for (int b = 0; b <= Spec::MAXBIT; ++b) {
+                if (Spec::mask(e) >> b & 1u) acc[acc_index<Spec>(e, b)] = fma(pw[0][b], xc, acc[acc_index<Spec>(e, b)]);
+                if (Spec::mask(e) >> (8 + b) & 1u)
+                    acc[acc_index<Spec>(e, 8 + b)] = fma(pw[1][b], xc, acc[acc_index<Spec>(e, 8 + b)]);
+            }
+        }
+    }
+};
+
+// ---- per-triplet work, generic group: walk the SF list, reduce each value over the batch -----
+struct SfTripletGeneric {
+    const Nbh& nb;
+    const AngularSF* sf;
+    int nsf;
+    double inv_rc;
+    double* gacc;     // [64] per warp, shared memory
+    int lane;
+
+    __device__ __forceinline__ void operator()(int j, int k, bool active) {
+        const double2 j0 = nb.p0[j], j1 = nb.p1[j], j2 = nb.p2[j];
+        const double2 k0 = nb.p0[k], k1 = nb.p1[k], k2 = nb.p2[k];
+        const double wx = k0.x - j0.x, wy = k0.y - j0.y, wz = k1.x - j1.x;
+        const double c2 = wx * wx + wy * wy + wz * wz;
+        const double c = sqrt(c2);
+        double C = j2.x * k2.x * (0.5 * cospi(c * inv_rc) + 0.5);
+        if (!active) C = 0.0;
+        const double cosv = (j0.x * k0.x + j0.y * k0.y + j1.x * k1.x) * (j1.y * k1.y);
+        const double r2sum = j2.y * j2.y + k2.y * k2.y + c2;
+        for (int s = 0; s < nsf; ++s) {
+            const AngularSF f = sf[s];
+            const double base = 1.0 + (double)f.lam * cosv;
+            double pw = 1.0, bb = base;
+            for (int z = f.izeta; z > 0; z >>= 1) {
+                if (z & 1) pw *= bb;
+                bb *= bb;
+            }
+            double v = f.coef * pw * exp(-f.eta * r2sum) * C;
+            v = warp_sum(v);
+            if (lane == 0) gacc[s] += v;
+        }
+        __syncwarp();
+    }
+};
+
+template <class Spec>
+__global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ SfParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const int64_t i = (int64_t)blockIdx.x * SF_WARPS + wid;
+    if (i >= p.n) return;
+    int tc = 0;
+    for (int e = 1; e < p.n_elem; ++e)
+        if (i >= p.cell_start[(size_t)e * p.ncell]) tc = e;
+    if (p.variant[tc] != Spec::ID) return;
+    const ElemProgram* __restrict__ prog = p.prog[tc];
+
+    unsigned char* base = smem_raw + (size_t)wid * sf_warp_smem<Spec>(p.cap);
+    Nbh nb;
+    nb.p0 = reinterpret_cast<double2*>(base);
+    nb.p1 = nb.p0 + p.cap;
+    nb.p2 = nb.p1 + p.cap;
+    nb.pe = reinterpret_cast<double*>(nb.p2 + p.cap);
+    PairQueue Q;
+    Q.q = reinterpret_cast<uint16_t*>(nb.pe + (size_t)p.cap * Spec::NETA);
+    Q.n = 0;
+    double* gacc = reinterpret_cast<double*>(Q.q + 64);
+
+    // segment boundaries of the neighbour row (grouped by element)
+    int seg[MAX_ELEM + 1];
+    seg[0] = 0;
+#pragma unroll
+    for (int e = 0; e < MAX_ELEM; ++e) seg[e + 1] = seg[e] + p.nbr_cnt[(size_t)i * MAX_ELEM + e];
+    const int ntot = seg[MAX_ELEM];
+
+    // ---- stage the neighbourhood -------------------------------------------------------------
+    const double xi = p.sx[i], yi = p.sy[i], zi = p.sz[i];
+    const int32_t* row = p.nbr + (size_t)i * p.stride;
+    double eta0 = 0.0;
+    if constexpr (Spec::NETA > 0) eta0 = prog->ang_eta[0];
+    for (int m = lane; m < ntot; m += 32) {
+        const int j = row[m];
+        const double dx = min_image_1d(xi, p.sx[j], p.box[0], p.half[0]);
+        const double dy = min_image_1d(yi, p.sy[j], p.box[1], p.half[1]);
+        const double dz = min_image_1d(zi, p.sz[j], p.box[2], p.half[2]);
+        const double a2 = dx * dx + dy * dy + dz * dz;
+        const double a = sqrt(a2);
+        const double ia = 1.0 / a;
+        const double fa = 0.5 * cospi(a * p.inv_rc) + 0.5;
+        nb.p0[m] = make_double2(dx, dy);
+        nb.p1[m] = make_double2(dz, ia);
+        nb.p2[m] = make_double2(fa, a);
+        if constexpr (Spec::NETA > 0) {
+            double E[Spec::NETA];
+            eta_chain<Spec>(a2, eta0, E);
+#pragma unroll
+            for (int e = 0; e < Spec::NETA; ++e) nb.pe[m * Spec::NETA + e] = E[e] * fa;
+        }
+    }
+    __syncwarp();
+
+    double* Grow = p.G + (size_t)i * p.g_stride;
+    for (int s = prog->n_sf + lane; s < p.g_stride; s += 32) Grow[s] = 0.0;
+
+    // ---- radial: G = sum_j exp(-eta (a - rs)^2) fc(a) over the neighbours of element e ----------
+    for (int e = 0; e < p.n_elem; ++e) {
+        const int nr = prog->n_rad[e], off = prog->rad_off[e];
+        for (int r = 0; r < nr; ++r) {
+            const RadialSF f = prog->rad[off + r];
+            double acc = 0.0;
+            for (int m = seg[e] + lane; m < seg[e + 1]; m += 32) {
+                const double2 q = nb.p2[m];
+                const double d = q.y - f.rs;
+                acc = fma(exp(-f.eta * d * d), q.x, acc);
+            }
+            acc = warp_sum(acc);
+            if (lane == 0) Grow[f.g] = acc;
+        }
+    }
+
+    // ---- angular groups -----------------------------------------------------------------------
+    for (int e1 = 0; e1 < p.n_elem; ++e1)
+        for (int e2 = e1; e2 < p.n_elem; ++e2) {
+            const int pr = pair_index(e1, e2, p.n_elem);
+            const int na = prog->n_ang[pr];
+            if (na == 0) continue;
+            if constexpr (Spec::ID != ANG_GENERIC) {
+                SfTripletFast<Spec> f(nb, eta0, p.inv_rc);
+                if (e1 == e2) enum_within(nb, seg[e1], seg[e1 + 1] - seg[e1], p.rc2, Q, lane, f);
+                else enum_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], p.rc2, Q, lane, f);
+                drain_tail(Q, lane, f);
+#pragma unroll
+                for (int e = 0; e < Spec::NETA; ++e)
+#pragma unroll
+                    for (int b = 0; b < 16; ++b)
+                        if (Spec::mask(e) >> b & 1u) {
+                            const double tot = warp_sum(f.acc[acc_index<Spec>(e, b)]);
+                            const int zeta = 1 << (b & 7);
+                            const double coef = exp2((double)(1 - zeta));
+                            const int g = prog->ang_g[pr][e][b];
+                            if (lane == 0 && g >= 0) Grow[g] = coef * tot;
+                        }
+            } else {
+                for (int s = lane; s < na; s += 32) gacc[s] = 0.0;
+                __syncwarp();
+                SfTripletGeneric f{nb, prog->ang + prog->ang_off[pr], na, p.inv_rc, gacc, lane};
+                if (e1 == e2) enum_within(nb, seg[e1], seg[e1 + 1] - seg[e1], p.rc2, Q, lane, f);
+                else enum_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], p.rc2, Q, lane, f);
+                drain_tail(Q, lane, f);
+                for (int s = lane; s < na; s += 32) Grow[prog->ang[prog->ang_off[pr] + s].g] = gacc[s];
+                __syncwarp();
+            }
+        }
+}
+
+template <class Spec>
+static int launch_one(const SfParams& p, cudaStream_t st) {
+    const size_t smem = SF_WARPS * sf_warp_smem<Spec>(p.cap);
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(k_sf<Spec>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        configured = true;
+    }
+    const unsigned nb = (unsigned)((p.n + SF_WARPS - 1) / SF_WARPS);
+    k_sf<Spec><<<nb, SF_WARPS * 32, smem, st>>>(p);
+    return 1;
+}
+
+size_t sf_smem_bytes(int variant, int cap) {
+    switch (variant) {
+        case ANG_BASE12: return SF_WARPS * sf_warp_smem<SpecBase12>(cap);
+        case ANG_WIDE32: return SF_WARPS * sf_warp_smem<SpecWide32>(cap);
+        default: return SF_WARPS * sf_warp_smem<SpecGeneric>(cap);
+    }
+}
+
+int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
+              const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st) {
+    if (n == 0) return 0;
+    SfParams p;
+    p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride;
+    p.rc = rc; p.rc2 = rc * rc; p.inv_rc = 1.0 / rc;
+    for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
+    p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
+    p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.G = w.G;
+    bool use[3] = {false, false, false};
+    for (int e = 0; e < MAX_ELEM; ++e) {
+        p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
+        p.variant[e] = e < n_elem ? variant[e] : -1;
+        if (e < n_elem) use[variant[e]] = true;
+    }
+    int launches = 0;
+    if (use[ANG_BASE12]) launches += launch_one<SpecBase12>(p, st);
+    if (use[ANG_WIDE32]) launches += launch_one<SpecWide32>(p, st);
+    if (use[ANG_GENERIC]) launches += launch_one<SpecGeneric>(p, st);
+    return launches;
+}
+
+}  // namespace nnp

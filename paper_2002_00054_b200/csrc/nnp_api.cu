@@ -1,0 +1,561 @@
+// nnp_api.cu -- the C ABI of libnnp_b200 (include/nnp.h): model construction, workspace layout,
+// the nnp_compute pipeline S0..S5, the host-buffer entry point and the debug exports.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "angular.cuh"
+#include "nnp_internal.h"
+
+using namespace nnp;
+
+struct nnp_model {
+    int n_elem = 0;
+    std::vector<std::string> names;
+    double rc = 0.0;
+    int device = 0;
+    int max_nbr = 160;
+    int g_stride = 0;
+    int n_sf_elem[MAX_ELEM] = {0, 0, 0, 0};
+    ElemProgram* d_prog[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
+    int variant[MAX_ELEM] = {0, 0, 0, 0};
+    NetDesc nets[MAX_ELEM];
+    double* d_weights[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
+    // last nnp_compute (for the exports)
+    Workspace ws;
+    bool have_ws = false;
+    int64_t last_n = 0;
+    cudaStream_t last_stream = nullptr;
+    int last_launches = 0;
+    int32_t* h_status = nullptr;   // pinned
+    // timing
+    bool timing = false;
+    bool timing_valid = false;
+    cudaEvent_t ev[NNP_N_STAGES + 1];
+    bool ev_created = false;
+    // host-buffer path
+    cudaStream_t hstream = nullptr;
+    void* h_ws = nullptr;
+    size_t h_ws_bytes = 0;
+    int64_t h_cap = 0;
+    double *hd_pos = nullptr, *hd_e = nullptr, *hd_f = nullptr, *hd_etot = nullptr;
+    int32_t* hd_type = nullptr;
+    std::string err;
+};
+
+static std::string g_create_err = "";
+
+static nnp_status fail(nnp_model* m, nnp_status s, const std::string& msg) {
+    if (m) m->err = msg;
+    else g_create_err = msg;
+    return s;
+}
+
+#define NNP_CUDA(m, expr)                                                                       \
+    do {                                                                                        \
+        cudaError_t e__ = (expr);                                                               \
+        if (e__ != cudaSuccess)                                                                 \
+            return fail(m, NNP_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e__)); \
+    } while (0)
+
+struct DeviceGuard {
+    int prev = -1;
+    bool ok;
+    explicit DeviceGuard(int dev) {
+        ok = cudaGetDevice(&prev) == cudaSuccess && cudaSetDevice(dev) == cudaSuccess;
+    }
+    ~DeviceGuard() {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+// ---------------------------------------------------------------- workspace layout
+
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+static size_t ws_layout(Workspace* w, void* base, int64_t n, int n_elem, int stride, int g_stride) {
+    size_t off = 0;
+    auto take = [&](size_t bytes) -> void* {
+        void* p = base ? (void*)((char*)base + off) : nullptr;
+        off = align_up(off + bytes, 256);
+        return p;
+    };
+    const size_t N = (size_t)(n > 0 ? n : 1);
+    w->sx = (double*)take(N * 8); w->sy = (double*)take(N * 8); w->sz = (double*)take(N * 8);
+    w->tx = (double*)take(N * 8); w->ty = (double*)take(N * 8); w->tz = (double*)take(N * 8);
+    w->perm = (int32_t*)take(N * 4); w->tperm = (int32_t*)take(N * 4);
+    w->key = (int32_t*)take(N * 4); w->rank = (int32_t*)take(N * 4); w->tkey = (int32_t*)take(N * 4);
+    w->n_keys_cap = (int64_t)n_elem * (2 * (int64_t)N + 64) + 1;
+    w->cell_start = (int32_t*)take((size_t)w->n_keys_cap * 4);
+    w->scan_tmp_len = w->n_keys_cap / 2048 + 16384;
+    w->scan_tmp = (int32_t*)take((size_t)w->scan_tmp_len * 4);
+    w->nbr = (int32_t*)take(N * (size_t)stride * 4);
+    w->nbr_cnt = (int32_t*)take(N * MAX_ELEM * 4);
+    w->G = (double*)take(N * (size_t)g_stride * 8);
+    w->dEdG = (double*)take(N * (size_t)g_stride * 8);
+    w->e_sorted = (double*)take(N * 8);
+    w->f_sorted = (double*)take(N * 3 * 8);
+    w->n_partial = (int64_t)(N + 255) / 256 + 1;
+    w->partial = (double*)take((size_t)w->n_partial * 8);
+    w->status = (int32_t*)take(64);
+    w->bytes = off;
+    return off;
+}
+
+static bool make_grid(Grid* g, const double box[3], double rc, int64_t n) {
+    const double cs_min = rc * (1.0 + 1e-9);   // margin: a cell index rounded the wrong way must not hide a neighbour
+    int64_t limit = 2 * (n > 0 ? n : 1) + 64;
+    double nc[3];
+    for (int c = 0; c < 3; ++c) {
+        nc[c] = std::floor(box[c] / cs_min);
+        if (nc[c] < 1.0) nc[c] = 1.0;
+    }
+    while (nc[0] * nc[1] * nc[2] > (double)limit) {
+        const double s = std::cbrt((double)limit / (nc[0] * nc[1] * nc[2])) * 0.999;
+        for (int c = 0; c < 3; ++c) nc[c] = std::fmax(1.0, std::floor(nc[c] * s));
+    }
+    for (int c = 0; c < 3; ++c) {
+        g->box[c] = box[c];
+        g->half[c] = 0.5 * box[c];
+        g->nc[c] = (int)nc[c];
+        g->inv_cs[c] = nc[c] / box[c];
+        g->span[c] = g->nc[c] >= 3 ? 1 : 0;
+    }
+    g->ncell = g->nc[0] * g->nc[1] * g->nc[2];
+    return true;
+}
+
+// ---------------------------------------------------------------- create / destroy
+
+// try to express the angular groups of one element on a specialised variant
+template <class Spec>
+static bool match_spec(const std::vector<std::vector<AngularSF>>& groups, ElemProgram* P) {
+    std::vector<double> etas;
+    for (const auto& grp : groups)
+        for (const auto& f : grp) {
+            bool seen = false;
+            for (double e : etas) seen |= (e == f.eta);
+            if (!seen) etas.push_back(f.eta);
+        }
+    if ((int)etas.size() != Spec::NETA) return false;
+    for (size_t a = 0; a < etas.size(); ++a)
+        for (size_t b = a + 1; b < etas.size(); ++b)
+            if (etas[b] < etas[a]) std::swap(etas[a], etas[b]);
+    if (!(etas[0] > 0.0)) return false;
+    for (int e = 1; e < Spec::NETA; ++e) {
+        const double want = etas[Spec::rbase(e)] * Spec::ratio(e);
+        if (std::fabs(etas[e] - want) > 1e-12 * want) return false;
+    }
+    for (int e = 0; e < MAX_ETA; ++e) P->ang_eta[e] = e < Spec::NETA ? etas[e] : 0.0;
+    for (size_t p = 0; p < groups.size(); ++p) {
+        for (int e = 0; e < MAX_ETA; ++e)
+            for (int b = 0; b < 16; ++b) P->ang_g[p][e][b] = -1;
+        if (groups[p].empty()) continue;
+        unsigned seen[MAX_ETA] = {0, 0, 0, 0};
+        for (const auto& f : groups[p]) {
+            int e = -1;
+            for (int q = 0; q < Spec::NETA; ++q)
+                if (etas[q] == f.eta) e = q;
+            int bit = -1;
+            for (int b = 0; b < 7; ++b)
+                if (f.izeta == (1 << b)) bit = b;
+            if (e < 0 || bit < 0) return false;
+            if (f.lam < 0) bit += 8;
+            if (!(Spec::mask(e) >> bit & 1u) || (seen[e] >> bit & 1u)) return false;
+            seen[e] |= 1u << bit;
+            P->ang_g[p][e][bit] = (int16_t)f.g;
+        }
+        for (int e = 0; e < Spec::NETA; ++e)
+            if (seen[e] != Spec::mask(e)) return false;
+    }
+    return true;
+}
+
+extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* const* elem_names, double rc,
+                                 int32_t n_sf, const nnp_sf* sf, const int32_t* n_layers,
+                                 const int32_t* const* layer_sizes, const double* const* weights,
+                                 int32_t cuda_device) {
+    if (!out) return fail(nullptr, NNP_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (n_elem < 1 || n_elem > MAX_ELEM) return fail(nullptr, NNP_ERR_INVALID_ARG, "n_elem must be 1..4");
+    if (!(rc > 0.0) || !std::isfinite(rc)) return fail(nullptr, NNP_ERR_INVALID_ARG, "rc must be > 0");
+    if (n_sf < 1 || !sf || !n_layers || !layer_sizes || !weights)
+        return fail(nullptr, NNP_ERR_INVALID_ARG, "null table");
+
+    std::vector<ElemProgram> progs(n_elem);
+    std::vector<std::vector<std::vector<AngularSF>>> ang(n_elem);   // [central][pair] -> list
+    std::vector<std::vector<std::vector<RadialSF>>> rad(n_elem);    // [central][nbr element] -> list
+    int npair = n_elem * (n_elem + 1) / 2;
+    int count[MAX_ELEM] = {0, 0, 0, 0};
+    for (int c = 0; c < n_elem; ++c) { ang[c].resize(npair); rad[c].resize(n_elem); }
+    for (int q = 0; q < n_sf; ++q) {
+        const nnp_sf& f = sf[q];
+        if (f.central < 0 || f.central >= n_elem) return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.central out of range");
+        if (!(f.eta >= 0.0) || !std::isfinite(f.eta)) return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.eta must be >= 0");
+        const int g = count[f.central]++;
+        if (f.kind == 2) {
+            if (f.e1 < 0 || f.e1 >= n_elem) return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.e1 out of range");
+            if (!std::isfinite(f.rs)) return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.rs not finite");
+            rad[f.central][f.e1].push_back(RadialSF{f.eta, f.rs, g, 0});
+        } else if (f.kind == 3) {
+            if (f.e1 < 0 || f.e1 >= n_elem || f.e2 < 0 || f.e2 >= n_elem)
+                return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.e1/e2 out of range");
+            if (!(f.lambda == 1.0 || f.lambda == -1.0))
+                return fail(nullptr, NNP_ERR_INVALID_ARG, "angular lambda must be +1 or -1");
+            const int iz = (int)f.zeta;
+            if ((double)iz != f.zeta || iz < 1 || iz > 64)
+                return fail(nullptr, NNP_ERR_INVALID_ARG, "angular zeta must be an integer in [1, 64]");
+            const int a = f.e1 < f.e2 ? f.e1 : f.e2, b = f.e1 < f.e2 ? f.e2 : f.e1;
+            ang[f.central][pair_index(a, b, n_elem)].push_back(
+                AngularSF{f.eta, std::exp2(1.0 - f.zeta), g, iz, f.lambda > 0 ? 1 : -1, 0});
+        } else {
+            return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.kind must be 2 (radial) or 3 (angular narrow)");
+        }
+    }
+
+    nnp_model* m = new nnp_model();
+    m->n_elem = n_elem;
+    m->rc = rc;
+    m->device = cuda_device;
+    for (int c = 0; c < n_elem; ++c) m->names.push_back(elem_names && elem_names[c] ? elem_names[c] : "?");
+    auto bail = [&](nnp_status s, const std::string& msg) {
+        g_create_err = msg;
+        nnp_destroy(m);
+        return s;
+    };
+
+    for (int c = 0; c < n_elem; ++c) {
+        ElemProgram& P = progs[c];
+        std::memset(&P, 0, sizeof(P));
+        P.n_sf = count[c];
+        P.n_elem = n_elem;
+        m->n_sf_elem[c] = count[c];
+        if (count[c] < 1) return bail(NNP_ERR_INVALID_ARG, "an element has no symmetry functions");
+        if (count[c] > m->g_stride) m->g_stride = count[c];
+        int ro = 0;
+        for (int e = 0; e < n_elem; ++e) {
+            P.n_rad[e] = (int)rad[c][e].size();
+            P.rad_off[e] = ro;
+            if (ro + P.n_rad[e] > MAX_RAD_TOTAL) return bail(NNP_ERR_INVALID_ARG, "too many radial SFs (max 128 per element)");
+            for (const auto& f : rad[c][e]) P.rad[ro++] = f;
+        }
+        int ao = 0;
+        for (int p = 0; p < npair; ++p) {
+            P.n_ang[p] = (int)ang[c][p].size();
+            P.ang_off[p] = ao;
+            if (ao + P.n_ang[p] > MAX_ANG_TOTAL) return bail(NNP_ERR_INVALID_ARG, "too many angular SFs (max 512 per element)");
+            for (const auto& f : ang[c][p]) P.ang[ao++] = f;
+        }
+        bool any_ang = ao > 0;
+        P.variant = ANG_GENERIC;
+        if (any_ang) {
+            if (match_spec<SpecBase12>(ang[c], &P)) P.variant = ANG_BASE12;
+            else if (match_spec<SpecWide32>(ang[c], &P)) P.variant = ANG_WIDE32;
+            else {
+                for (int p = 0; p < npair; ++p)
+                    if (P.n_ang[p] > 64)
+                        return bail(NNP_ERR_INVALID_ARG, "generic angular path supports <= 64 SFs per pair group");
+            }
+        }
+        m->variant[c] = P.variant;
+    }
+
+    // networks: validate and pack everything on the host first, upload afterwards
+    std::vector<std::vector<double>> packed_all(n_elem);
+    for (int c = 0; c < n_elem; ++c) {
+        const int L = n_layers[c];
+        if (L < 1 || L > MAX_LAYERS) return bail(NNP_ERR_INVALID_ARG, "n_layers must be 1..8");
+        const int32_t* sz = layer_sizes[c];
+        if (!sz || !weights[c]) return bail(NNP_ERR_INVALID_ARG, "null layer_sizes/weights");
+        if (sz[0] != count[c]) return bail(NNP_ERR_INVALID_ARG, "first layer size must equal the element's SF count");
+        if (sz[L] != 1) return bail(NNP_ERR_INVALID_ARG, "last layer size must be 1");
+        NetDesc& nd = m->nets[c];
+        std::memset(&nd, 0, sizeof(nd));
+        nd.n_layers = L;
+        for (int l = 0; l <= L; ++l) {
+            if (sz[l] < 1 || (l > 0 && l < L && sz[l] > MAX_WIDTH)) return bail(NNP_ERR_INVALID_ARG, "bad layer width (hidden <= 256)");
+            nd.sizes[l] = sz[l];
+        }
+        auto r4 = [](int x) { return (x + 3) & ~3; };
+        size_t tot = 0;
+        for (int l = 0; l < L; ++l) {
+            nd.wt_off[l] = (int)tot; tot += (size_t)sz[l] * r4(sz[l + 1]);
+            nd.w_off[l] = (int)tot; tot += (size_t)sz[l + 1] * r4(sz[l]);
+            nd.b_off[l] = (int)tot; tot += (size_t)r4(sz[l + 1]);
+        }
+        std::vector<double> packed(tot, 0.0);
+        const double* src = weights[c];
+        for (int l = 0; l < L; ++l) {
+            const int nin = sz[l], nout = sz[l + 1];
+            const double* W = src;
+            const double* B = src + (size_t)nin * nout;
+            src = B + nout;
+            for (int o = 0; o < nout; ++o)
+                for (int i = 0; i < nin; ++i) {
+                    const double v = W[(size_t)o * nin + i];
+                    if (!std::isfinite(v)) return bail(NNP_ERR_INVALID_ARG, "non-finite weight");
+                    packed[nd.wt_off[l] + (size_t)i * r4(nout) + o] = v;
+                    packed[nd.w_off[l] + (size_t)o * r4(nin) + i] = v;
+                }
+            for (int o = 0; o < nout; ++o) packed[nd.b_off[l] + o] = B[o];
+        }
+        if (mlp_smem_bytes(nd, 8) > 200 * 1024) return bail(NNP_ERR_INVALID_ARG, "network too large for the shared-memory tile");
+        packed_all[c].swap(packed);
+    }
+    for (int c = 0; c < n_elem; ++c) {
+        NetDesc& nd = m->nets[c];
+        const std::vector<double>& packed = packed_all[c];
+        const size_t tot = packed.size();
+        DeviceGuard dg(cuda_device);
+        if (!dg.ok) return bail(NNP_ERR_CUDA, "cudaSetDevice failed (no CUDA device?)");
+        cudaError_t e = cudaMalloc(&m->d_weights[c], tot * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemcpy(m->d_weights[c], packed.data(), tot * sizeof(double), cudaMemcpyHostToDevice);
+        if (e == cudaSuccess) e = cudaMalloc(&m->d_prog[c], sizeof(ElemProgram));
+        if (e == cudaSuccess) e = cudaMemcpy(m->d_prog[c], &progs[c], sizeof(ElemProgram), cudaMemcpyHostToDevice);
+        if (e != cudaSuccess) return bail(NNP_ERR_CUDA, std::string("model upload: ") + cudaGetErrorString(e));
+        nd.weights = m->d_weights[c];
+    }
+    {
+        DeviceGuard dg(cuda_device);
+        if (cudaMallocHost(&m->h_status, 64) != cudaSuccess) return bail(NNP_ERR_CUDA, "cudaMallocHost failed");
+        std::memset(m->h_status, 0, 64);
+    }
+    *out = m;
+    return NNP_OK;
+}
+
+extern "C" void nnp_destroy(nnp_model* m) {
+    if (!m) return;
+    DeviceGuard dg(m->device);
+    for (int c = 0; c < MAX_ELEM; ++c) {
+        if (m->d_prog[c]) cudaFree(m->d_prog[c]);
+        if (m->d_weights[c]) cudaFree(m->d_weights[c]);
+    }
+    if (m->h_status) cudaFreeHost(m->h_status);
+    if (m->ev_created)
+        for (int k = 0; k <= NNP_N_STAGES; ++k) cudaEventDestroy(m->ev[k]);
+    if (m->h_ws) cudaFree(m->h_ws);
+    if (m->hd_pos) cudaFree(m->hd_pos);
+    if (m->hd_type) cudaFree(m->hd_type);
+    if (m->hd_e) cudaFree(m->hd_e);
+    if (m->hd_f) cudaFree(m->hd_f);
+    if (m->hd_etot) cudaFree(m->hd_etot);
+    if (m->hstream) cudaStreamDestroy(m->hstream);
+    delete m;
+}
+
+extern "C" nnp_status nnp_set_max_neighbors(nnp_model* m, int32_t max_neighbors) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    if (max_neighbors < 32 || max_neighbors > 255) return fail(m, NNP_ERR_INVALID_ARG, "max_neighbors must be 32..255");
+    m->max_nbr = max_neighbors;
+    m->have_ws = false;
+    return NNP_OK;
+}
+
+static int row_stride(const nnp_model* m) { return (m->max_nbr + 7) & ~7; }
+
+extern "C" size_t nnp_workspace_bytes(const nnp_model* m, int64_t n_atoms) {
+    if (!m || n_atoms < 0) return 0;
+    Workspace w;
+    return ws_layout(&w, nullptr, n_atoms, m->n_elem, row_stride(m), m->g_stride);
+}
+
+extern "C" int32_t nnp_g_stride(const nnp_model* m) { return m ? m->g_stride : 0; }
+extern "C" int32_t nnp_last_launch_count(const nnp_model* m) { return m ? m->last_launches : 0; }
+extern "C" int32_t nnp_uses_fast_path(const nnp_model* m) {
+    if (!m) return 0;
+    for (int c = 0; c < m->n_elem; ++c)
+        if (m->variant[c] == ANG_GENERIC) return 0;
+    return 1;
+}
+extern "C" const char* nnp_last_error(const nnp_model* m) { return m ? m->err.c_str() : g_create_err.c_str(); }
+extern "C" const char* nnp_version(void) { return "0.1"; }
+
+// ---------------------------------------------------------------- compute
+
+extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d_pos, const int32_t* d_type,
+                                  const double box[3], double* d_e_atom, double* d_e_total, double* d_force,
+                                  void* d_workspace, size_t workspace_bytes, void* cuda_stream) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    if (n_atoms < 0 || n_atoms > 0x7fffffffLL / 4) return fail(m, NNP_ERR_INVALID_ARG, "n_atoms out of range");
+    if (!box || !d_e_total) return fail(m, NNP_ERR_INVALID_ARG, "box / d_e_total is NULL");
+    if (n_atoms > 0 && (!d_pos || !d_type || !d_e_atom || !d_force)) return fail(m, NNP_ERR_INVALID_ARG, "null array");
+    for (int c = 0; c < 3; ++c) {
+        if (!std::isfinite(box[c]) || !(box[c] > 0.0)) return fail(m, NNP_ERR_INVALID_ARG, "box length must be finite and > 0");
+        if (box[c] < 2.0 * m->rc) return fail(m, NNP_ERR_BOX_TOO_SMALL, "box length < 2*rc");
+    }
+    const int stride = row_stride(m);
+    Workspace w;
+    const size_t need = ws_layout(&w, d_workspace, n_atoms, m->n_elem, stride, m->g_stride);
+    if (!d_workspace || ((uintptr_t)d_workspace & 255u) || workspace_bytes < need)
+        return fail(m, NNP_ERR_WORKSPACE, "workspace null, misaligned or too small");
+    DeviceGuard dg(m->device);
+    if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    Grid g;
+    make_grid(&g, box, m->rc, n_atoms);
+    if (m->timing && !m->ev_created) {
+        for (int k = 0; k <= NNP_N_STAGES; ++k) NNP_CUDA(m, cudaEventCreate(&m->ev[k]));
+        m->ev_created = true;
+    }
+    auto mark = [&](int k) {
+        if (m->timing) cudaEventRecord(m->ev[k], st);
+    };
+    int launches = 0;
+    mark(0);
+    launches += launch_sort(w, g, n_atoms, m->n_elem, d_pos, d_type, st);
+    mark(1);
+    launches += launch_neighbors(w, g, n_atoms, m->n_elem, m->rc * m->rc, stride, m->max_nbr, st);
+    mark(2);
+    launches += launch_sf(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->rc, stride, m->max_nbr, m->g_stride, st);
+    mark(3);
+    launches += launch_mlp(w, n_atoms, m->n_elem, g.ncell, m->nets, m->g_stride, st);
+    mark(4);
+    launches += launch_force(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->rc, stride, m->max_nbr, m->g_stride, st);
+    mark(5);
+    launches += launch_finalize(w, n_atoms, d_e_atom, d_e_total, d_force, st);
+    mark(6);
+    m->timing_valid = m->timing;
+    m->ws = w;
+    m->have_ws = true;
+    m->last_n = n_atoms;
+    m->last_stream = st;
+    m->last_launches = launches;
+    NNP_CUDA(m, cudaGetLastError());
+    return NNP_OK;
+}
+
+extern "C" nnp_status nnp_sync_status(nnp_model* m) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    if (!m->have_ws) return NNP_OK;
+    DeviceGuard dg(m->device);
+    NNP_CUDA(m, cudaMemcpyAsync(m->h_status, m->ws.status, sizeof(int32_t), cudaMemcpyDeviceToHost, m->last_stream));
+    NNP_CUDA(m, cudaStreamSynchronize(m->last_stream));
+    const int s = m->h_status[0];
+    if (s & ST_NONFINITE) return fail(m, NNP_ERR_NONFINITE, "non-finite position");
+    if (s & ST_TYPE_RANGE) return fail(m, NNP_ERR_TYPE_RANGE, "atom type out of range");
+    if (s & ST_NBR_OVERFLOW) return fail(m, NNP_ERR_NEIGHBOR_OVERFLOW, "an atom has more than max_neighbors neighbours");
+    return NNP_OK;
+}
+
+extern "C" nnp_status nnp_compute_host(nnp_model* m, int64_t n, const double* h_pos, const int32_t* h_type,
+                                       const double box[3], double* h_e_atom, double* h_e_total, double* h_force) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    if (n < 0) return fail(m, NNP_ERR_INVALID_ARG, "n_atoms < 0");
+    if (!h_e_total || (n > 0 && (!h_pos || !h_type || !h_e_atom || !h_force))) return fail(m, NNP_ERR_INVALID_ARG, "null array");
+    DeviceGuard dg(m->device);
+    if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
+    if (!m->hstream) NNP_CUDA(m, cudaStreamCreateWithFlags(&m->hstream, cudaStreamNonBlocking));
+    const size_t need = nnp_workspace_bytes(m, n);
+    if (need > m->h_ws_bytes) {
+        if (m->h_ws) cudaFree(m->h_ws);
+        m->h_ws = nullptr; m->h_ws_bytes = 0;
+        NNP_CUDA(m, cudaMalloc(&m->h_ws, need));
+        m->h_ws_bytes = need;
+    }
+    if (n > m->h_cap || !m->hd_etot) {
+        if (m->hd_pos) cudaFree(m->hd_pos);
+        if (m->hd_type) cudaFree(m->hd_type);
+        if (m->hd_e) cudaFree(m->hd_e);
+        if (m->hd_f) cudaFree(m->hd_f);
+        if (m->hd_etot) cudaFree(m->hd_etot);
+        m->hd_pos = m->hd_e = m->hd_f = m->hd_etot = nullptr; m->hd_type = nullptr; m->h_cap = 0;
+        const size_t N = (size_t)(n > 0 ? n : 1);
+        NNP_CUDA(m, cudaMalloc(&m->hd_pos, N * 24));
+        NNP_CUDA(m, cudaMalloc(&m->hd_type, N * 4));
+        NNP_CUDA(m, cudaMalloc(&m->hd_e, N * 8));
+        NNP_CUDA(m, cudaMalloc(&m->hd_f, N * 24));
+        NNP_CUDA(m, cudaMalloc(&m->hd_etot, 8));
+        m->h_cap = (int64_t)N;
+    }
+    if (n > 0) {
+        NNP_CUDA(m, cudaMemcpyAsync(m->hd_pos, h_pos, (size_t)n * 24, cudaMemcpyHostToDevice, m->hstream));
+        NNP_CUDA(m, cudaMemcpyAsync(m->hd_type, h_type, (size_t)n * 4, cudaMemcpyHostToDevice, m->hstream));
+    }
+    nnp_status s = nnp_compute(m, n, m->hd_pos, m->hd_type, box, m->hd_e, m->hd_etot, m->hd_f, m->h_ws, m->h_ws_bytes,
+                               (void*)m->hstream);
+    if (s != NNP_OK) return s;
+    if (n > 0) {
+        NNP_CUDA(m, cudaMemcpyAsync(h_e_atom, m->hd_e, (size_t)n * 8, cudaMemcpyDeviceToHost, m->hstream));
+        NNP_CUDA(m, cudaMemcpyAsync(h_force, m->hd_f, (size_t)n * 24, cudaMemcpyDeviceToHost, m->hstream));
+    }
+    NNP_CUDA(m, cudaMemcpyAsync(h_e_total, m->hd_etot, 8, cudaMemcpyDeviceToHost, m->hstream));
+    return nnp_sync_status(m);
+}
+
+// ---------------------------------------------------------------- timing
+
+extern "C" nnp_status nnp_set_timing(nnp_model* m, int32_t enabled) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    m->timing = enabled != 0;
+    if (!m->timing) m->timing_valid = false;
+    return NNP_OK;
+}
+
+extern "C" nnp_status nnp_get_timings(nnp_model* m, double* ms) {
+    if (!m || !ms) return NNP_ERR_INVALID_ARG;
+    if (!m->timing_valid) return fail(m, NNP_ERR_INVALID_ARG, "timing not enabled for the last nnp_compute");
+    DeviceGuard dg(m->device);
+    NNP_CUDA(m, cudaEventSynchronize(m->ev[NNP_N_STAGES]));
+    for (int k = 0; k < NNP_N_STAGES; ++k) {
+        float t = 0.f;
+        NNP_CUDA(m, cudaEventElapsedTime(&t, m->ev[k], m->ev[k + 1]));
+        ms[k] = t;
+    }
+    return NNP_OK;
+}
+
+// ---------------------------------------------------------------- exports
+
+extern "C" nnp_status nnp_get_neighbor_counts(nnp_model* m, int32_t* d_counts) {
+    if (!m || !d_counts) return NNP_ERR_INVALID_ARG;
+    if (!m->have_ws) return fail(m, NNP_ERR_INVALID_ARG, "no nnp_compute yet");
+    DeviceGuard dg(m->device);
+    launch_export_counts(m->ws, m->last_n, m->n_elem, d_counts, m->last_stream);
+    NNP_CUDA(m, cudaStreamSynchronize(m->last_stream));
+    return NNP_OK;
+}
+
+extern "C" nnp_status nnp_get_neighbors(nnp_model* m, int64_t* d_offsets, int32_t* d_idx, int64_t idx_capacity) {
+    if (!m || !d_offsets) return NNP_ERR_INVALID_ARG;
+    if (!m->have_ws) return fail(m, NNP_ERR_INVALID_ARG, "no nnp_compute yet");
+    DeviceGuard dg(m->device);
+    const int64_t n = m->last_n;
+    int32_t* d_counts = nullptr;
+    int64_t* d_tmp = nullptr;
+    NNP_CUDA(m, cudaMalloc(&d_counts, sizeof(int32_t) * (size_t)(n + 1)));
+    cudaError_t e = cudaMalloc(&d_tmp, sizeof(int64_t) * (size_t)(n / 2048 + 16384));
+    if (e != cudaSuccess) { cudaFree(d_counts); return fail(m, NNP_ERR_CUDA, cudaGetErrorString(e)); }
+    launch_export_counts(m->ws, n, m->n_elem, d_counts, m->last_stream);
+    launch_scan_i64_from_i32(d_counts, n, d_offsets, d_tmp, m->last_stream);
+    if (d_idx) launch_export_neighbors(m->ws, n, m->n_elem, row_stride(m), d_offsets, d_idx, idx_capacity, m->last_stream);
+    e = cudaStreamSynchronize(m->last_stream);
+    cudaFree(d_counts);
+    cudaFree(d_tmp);
+    if (e != cudaSuccess) return fail(m, NNP_ERR_CUDA, cudaGetErrorString(e));
+    return NNP_OK;
+}
+
+static nnp_status export_rows(nnp_model* m, const double* src, double* dst) {
+    if (!m || !dst) return NNP_ERR_INVALID_ARG;
+    if (!m->have_ws) return fail(m, NNP_ERR_INVALID_ARG, "no nnp_compute yet");
+    DeviceGuard dg(m->device);
+    launch_export_rows(m->ws, m->last_n, m->g_stride, src, dst, m->last_stream);
+    NNP_CUDA(m, cudaStreamSynchronize(m->last_stream));
+    return NNP_OK;
+}
+
+extern "C" nnp_status nnp_get_sf(nnp_model* m, double* d_G) { return export_rows(m, m ? m->ws.G : nullptr, d_G); }
+extern "C" nnp_status nnp_get_dedg(nnp_model* m, double* d) { return export_rows(m, m ? m->ws.dEdG : nullptr, d); }
+
+extern "C" nnp_status nnp_measure_fp64_peak(int32_t cuda_device, double seconds, double* dfma_per_s,
+                                            double* dfma_per_s_sustained) {
+    if (!dfma_per_s) return NNP_ERR_INVALID_ARG;
+    DeviceGuard dg(cuda_device);
+    if (!dg.ok) return NNP_ERR_CUDA;
+    cudaError_t e;
+    *dfma_per_s = fp64_peak(cuda_device, seconds, dfma_per_s_sustained, &e);
+    return e == cudaSuccess ? NNP_OK : NNP_ERR_CUDA;
+}

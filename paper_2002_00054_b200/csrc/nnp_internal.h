@@ -1,0 +1,137 @@
+// nnp_internal.h -- structures shared by the CUDA translation units of libnnp_b200.
+// Not part of the public ABI (that is include/nnp.h).  Shares nothing with oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstddef>
+#include <cstdint>
+
+#include "nnp.h"
+
+namespace nnp {
+
+constexpr int MAX_ELEM = 4;
+constexpr int MAX_PAIR = MAX_ELEM * (MAX_ELEM + 1) / 2;   // unordered neighbour-element pairs
+constexpr int MAX_ETA = 4;        // distinct angular etas on the specialised path
+constexpr int MAX_RAD_TOTAL = 128;  // radial SFs per central element (all neighbour elements)
+constexpr int MAX_ANG_TOTAL = 512;  // angular SFs per central element (all pairs)
+constexpr int MAX_LAYERS = 8;
+constexpr int MAX_WIDTH = 256;
+
+// Device-detected status bits (Workspace::status[0] is an OR of these)
+enum : int { ST_TYPE_RANGE = 1, ST_NBR_OVERFLOW = 2, ST_NONFINITE = 4 };
+
+// index of the unordered element pair (a <= b) among E elements
+__host__ __device__ inline int pair_index(int a, int b, int n_elem) {
+    return a * n_elem - (a * (a - 1)) / 2 + (b - a);
+}
+
+struct RadialSF {
+    double eta, rs;
+    int32_t g;       // position in the element's G vector
+    int32_t pad;
+};
+
+struct AngularSF {
+    double eta;
+    double coef;     // 2^(1-zeta)
+    int32_t g;
+    int32_t izeta;   // integer zeta
+    int32_t lam;     // +1 / -1
+    int32_t pad;
+};
+
+// Angular kernel variants.  Specialised variants bake the (eta ratio, lambda, zeta) structure
+// of a pair group into the kernel; ANG_GENERIC walks the AngularSF list (any table).
+enum AngVariant : int { ANG_GENERIC = 0, ANG_BASE12 = 1, ANG_WIDE32 = 2 };
+
+// Symmetry-function program of ONE central element; lives in device memory (model-owned).
+struct ElemProgram {
+    int32_t n_sf;
+    int32_t n_elem;
+    int32_t variant;                 // AngVariant
+    int32_t pad0;
+    int32_t n_rad[MAX_ELEM];         // radial SFs for neighbour element e
+    int32_t rad_off[MAX_ELEM];       // first index into rad[]
+    int32_t n_ang[MAX_PAIR];         // angular SFs of pair group p
+    int32_t ang_off[MAX_PAIR];       // first index into ang[]
+    // specialised path: eta values (shared by all groups of the element) and, per group,
+    // the G index of menu entry (eta slot e, bit b): bits 0..6 lambda=+1 zeta=2^b, 8..14 lambda=-1
+    double ang_eta[MAX_ETA];
+    int16_t ang_g[MAX_PAIR][MAX_ETA][16];
+    RadialSF rad[MAX_RAD_TOTAL];
+    AngularSF ang[MAX_ANG_TOTAL];
+};
+
+// One element's network in device memory.  `weights` holds, per layer l (all blocks padded to
+// multiples of 4 doubles, zero filled): WT_l [n_in][round4(n_out)] (transposed, forward pass),
+// W_l [n_out][round4(n_in)] (backward pass), b_l [round4(n_out)].
+struct NetDesc {
+    int32_t n_layers;                // weight layers
+    int32_t sizes[MAX_LAYERS + 1];
+    int32_t wt_off[MAX_LAYERS];
+    int32_t w_off[MAX_LAYERS];
+    int32_t b_off[MAX_LAYERS];
+    const double* weights;           // device
+};
+
+// Cell grid of one nnp_compute call (host-built, passed by value).
+struct Grid {
+    double box[3], half[3], inv_cs[3];
+    int32_t nc[3];
+    int32_t ncell;
+    int32_t span[3];                 // stencil half-width clipped: 1 if nc>=3 (3 cells), else visit all nc cells
+};
+
+struct Workspace {
+    double *sx, *sy, *sz;            // [N] wrapped coordinates, sorted by (element, cell, original index)
+    double *tx, *ty, *tz;            // [N] staging for the sort
+    int32_t *perm, *tperm;           // [N] sorted position -> original index
+    int32_t *key, *rank, *tkey;      // [N]
+    int32_t *cell_start;             // [n_elem * ncell + 1]
+    int32_t *scan_tmp;               // block sums of the scans
+    int32_t *nbr;                    // [N][stride] neighbour positions (sorted space), grouped by element
+    int32_t *nbr_cnt;                // [N][MAX_ELEM] neighbours of each element
+    double *G, *dEdG;                // [N][g_stride], sorted order
+    double *e_sorted;                // [N]
+    double *f_sorted;                // [N][3]
+    double *partial;                 // [n_partial] block sums of the energy
+    int32_t *status;                 // [4]
+    int64_t n_keys_cap;
+    int64_t scan_tmp_len;
+    int64_t n_partial;
+    size_t bytes;
+};
+
+// ---- launchers (each enqueues on `st`; returns the number of kernels launched) ----------
+int launch_sort(const Workspace& w, const Grid& g, int64_t n, int n_elem, const double* d_pos,
+                const int32_t* d_type, cudaStream_t st);
+int launch_neighbors(const Workspace& w, const Grid& g, int64_t n, int n_elem, double rc2, int stride,
+                     int max_nbr, cudaStream_t st);
+int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
+              const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st);
+int launch_mlp(const Workspace& w, int64_t n, int n_elem, int ncell, const NetDesc* nets, int g_stride,
+               cudaStream_t st);
+int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
+                 const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st);
+int launch_finalize(const Workspace& w, int64_t n, double* d_e_atom, double* d_e_total, double* d_force,
+                    cudaStream_t st);
+
+// exports
+int launch_export_counts(const Workspace& w, int64_t n, int n_elem, int32_t* d_counts, cudaStream_t st);
+int launch_export_neighbors(const Workspace& w, int64_t n, int n_elem, int stride, const int64_t* d_offsets,
+                            int32_t* d_idx, int64_t cap, cudaStream_t st);
+int launch_export_rows(const Workspace& w, int64_t n, int g_stride, const double* src_sorted, double* dst,
+                       cudaStream_t st);
+int launch_scan_i64_from_i32(const int32_t* d_in, int64_t n, int64_t* d_out /* n+1 */, int64_t* d_tmp,
+                             cudaStream_t st);
+void exclusive_scan_i32(int32_t* d_data, int64_t n, int32_t* d_tmp, cudaStream_t st, int* launches);
+
+size_t mlp_smem_bytes(const NetDesc& net, int ta);
+size_t sf_smem_bytes(int variant, int cap);
+size_t force_smem_bytes(int variant, int cap, int g_stride);
+
+double fp64_peak(int device, double seconds, double* sustained, cudaError_t* err);
+
+}  // namespace nnp

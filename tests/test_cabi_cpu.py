@@ -1,0 +1,100 @@
+"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/nnp.h declares,
+and rejects bad arguments synchronously (no compute calls -- there is no GPU here)."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    import __graft_entry__ as g
+    from paper_2002_00054_b200 import build as b
+    if not os.path.exists(b.LIB):
+        g.build()
+    from paper_2002_00054_b200 import load_library
+    return load_library()
+
+
+def test_exports_match_header(lib):
+    from paper_2002_00054_b200 import EXPORTS
+    hdr = open(os.path.join(ROOT, "include", "nnp.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(nnp_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(EXPORTS)
+    for name in declared:
+        assert getattr(lib, name) is not None
+    assert lib.nnp_version().decode() == "0.1"
+
+
+def _create(lib, model, n_elem=None, rc=None, sf=None, layer_sizes=None, weights=None):
+    from paper_2002_00054_b200.binding import _SF
+    n_elem = len(model.elements) if n_elem is None else n_elem
+    sf = np.ascontiguousarray(model.sf if sf is None else sf)
+    assert sf.dtype.itemsize == C.sizeof(_SF)
+    layer_sizes = model.layer_sizes if layer_sizes is None else layer_sizes
+    weights = model.weights if weights is None else weights
+    names = (C.c_char_p * len(model.elements))(*[e.encode() for e in model.elements])
+    nl = np.array([len(ls) - 1 for ls in layer_sizes], dtype=np.int32)
+    lsa = [np.ascontiguousarray(ls, dtype=np.int32) for ls in layer_sizes]
+    wa = [np.ascontiguousarray(w, dtype=np.float64) for w in weights]
+    lsp = (C.c_void_p * len(lsa))(*[a.ctypes.data for a in lsa])
+    wp = (C.c_void_p * len(wa))(*[a.ctypes.data for a in wa])
+    h = C.c_void_p(None)
+    st = lib.nnp_create(C.byref(h), n_elem, names, float(model.rc if rc is None else rc), int(sf.shape[0]),
+                        sf.ctypes.data_as(C.c_void_p), nl.ctypes.data_as(C.c_void_p), lsp, wp, 0)
+    return st, h
+
+
+def test_create_rejects_bad_arguments(lib):
+    model = W.make_model(False)
+    INVALID = 1
+    assert _create(lib, model, n_elem=0)[0] == INVALID
+    assert _create(lib, model, n_elem=5)[0] == INVALID
+    assert _create(lib, model, rc=-1.0)[0] == INVALID
+    sf = model.sf.copy(); sf["kind"][3] = 7
+    assert _create(lib, model, sf=sf)[0] == INVALID
+    sf = model.sf.copy(); sf["zeta"][20] = 2.5           # non-integer zeta
+    assert _create(lib, model, sf=sf)[0] == INVALID
+    assert b"zeta" in lib.nnp_last_error(None)
+    sf = model.sf.copy(); sf["lam"][20] = 0.5
+    assert _create(lib, model, sf=sf)[0] == INVALID
+    sf = model.sf.copy(); sf["e1"][0] = 2
+    assert _create(lib, model, sf=sf)[0] == INVALID
+    sf = model.sf.copy(); sf["central"][0] = -1
+    assert _create(lib, model, sf=sf)[0] == INVALID
+    ls = [list(x) for x in model.layer_sizes]; ls[0][0] = 51
+    assert _create(lib, model, layer_sizes=ls)[0] == INVALID
+    ls = [list(x) for x in model.layer_sizes]; ls[1][-1] = 2
+    assert _create(lib, model, layer_sizes=ls)[0] == INVALID
+
+
+def test_create_without_gpu_reports_cuda_error(lib):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    st, h = _create(lib, W.make_model(False))
+    assert st == 6 and not h.value          # NNP_ERR_CUDA: no CPU fallback
+    assert len(lib.nnp_last_error(None)) > 0
+
+
+def test_null_model_calls_are_safe(lib):
+    assert lib.nnp_workspace_bytes(None, 100) == 0
+    assert lib.nnp_sync_status(None) == 1
+    assert lib.nnp_g_stride(None) == 0
+    lib.nnp_destroy(None)
+
+
+def test_binding_fails_loudly_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_2002_00054_b200 import NNP, NNPError
+    with pytest.raises(NNPError):
+        NNP.from_model(W.make_model(False))

@@ -1,0 +1,274 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Tolerances (BASELINE.json north_star):
+  neighbour sets bit-exact (sorted index lists); total energy relative 1e-10;
+  force components absolute 1e-8 eV/A; e_atom abs 1e-10*max|E_i|; G abs 1e-11*max(1,|G|)."""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+import workloads as W
+from conftest import tiny_model
+
+pytestmark = pytest.mark.gpu
+
+E_REL = 1e-10
+F_ABS = 1e-8
+
+
+def _dev():
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device (no CPU fallback exists)"
+    return torch.device("cuda", 0)
+
+
+def _run(nnp, pos, types, box):
+    dev = _dev()
+    p = torch.tensor(np.ascontiguousarray(pos), dtype=torch.float64, device=dev)
+    t = torch.tensor(np.ascontiguousarray(types), dtype=torch.int32, device=dev)
+    e_atom, e_total, force = nnp.compute(p, t, box)
+    torch.cuda.synchronize()
+    return e_atom.cpu().numpy(), float(e_total.item()), force.cpu().numpy()
+
+
+def _check_full(model, sysm, max_neighbors=None):
+    """Whole-system comparison: neighbours, G, dE/dG, e_atom, E, F."""
+    from paper_2002_00054_b200 import NNP
+    nnp = NNP.from_model(model)
+    if max_neighbors:
+        nnp.set_max_neighbors(max_neighbors)
+    n = sysm.n_atoms
+    e_atom, e_total, force = _run(nnp, sysm.pos, sysm.types, sysm.box)
+    om = oracle.OracleModel(model)
+    ref = oracle.compute(om, sysm.pos, sysm.types, sysm.box)
+    # neighbour sets: bit-exact
+    off, idx = nnp.neighbors(n)
+    roff, ridx = oracle.neighbor_list(sysm.pos, sysm.box, model.rc)
+    assert np.array_equal(off.cpu().numpy(), roff)
+    assert np.array_equal(idx.cpu().numpy(), ridx)
+    assert np.array_equal(nnp.neighbor_counts(n).cpu().numpy(), np.diff(roff))
+    # descriptors and network gradients
+    G = nnp.symmetry_functions(n).cpu().numpy()
+    assert np.all(np.abs(G - ref.G) <= 1e-11 * np.maximum(1.0, np.abs(ref.G)))
+    B = nnp.dedg(n).cpu().numpy()
+    assert np.all(np.abs(B - ref.dEdG) <= 1e-11 * np.maximum(1.0, np.abs(ref.dEdG)))
+    # energies and forces
+    assert np.all(np.abs(e_atom - ref.e_atom) <= 1e-10 * np.abs(ref.e_atom).max())
+    assert abs(e_total - ref.e_total) <= E_REL * abs(ref.e_total)
+    assert abs(e_total - e_atom.sum()) <= 1e-12 * np.abs(e_atom).sum()
+    assert np.abs(force - ref.F).max() <= F_ABS
+    assert np.all(np.abs(force.sum(axis=0)) < 1e-8)
+    nnp.close()
+    return ref
+
+
+def test_config0_tiny_full_parity():
+    # configs[0]: 288 atoms, L = 14.2 -> only 2 cells per dimension (periodic stencil de-dup)
+    sysm, model = W.build(W.CONFIGS[0])
+    ref = _check_full(model, sysm)
+    assert abs(ref.e_total) > 1e-3 * np.abs(ref.e_atom).sum()     # no cancellation (reading C16)
+
+
+def test_mid_size_several_cells_ragged():
+    # 700 molecules -> 2100 atoms, L = 27.5 A: 4 cells per dimension, last CTAs/warps ragged
+    sysm = W.make_water(700, 4242)
+    _check_full(W.make_model(False), sysm)
+
+
+def test_orthorhombic_box_2_3_5_cells():
+    # box 12.6 x 18.7 x 31 -> 2, 3 and 5 cells: every stencil de-dup branch at once
+    box = np.array([12.6, 18.7, 31.0])
+    n_mol = 245
+    base = W.make_water(n_mol, 77, L=1.0)
+    sysm = W.WaterSystem(pos=base.pos * 0 + _uniform_in(box, 3 * n_mol, 77), types=base.types, box=box, seed=77)
+    _check_full(W.make_model(False), sysm)
+
+
+def _uniform_in(box, n, seed):
+    from workloads import rng
+    k = rng.stream_key(seed, 999)
+    u = rng.uniform(k, np.arange(3 * n, dtype=np.uint64)).reshape(n, 3)
+    return u * box
+
+
+def test_wide_model_small_system():
+    sysm = W.make_water(150, 31, L=15.3)
+    _check_full(W.make_model(True), sysm)
+
+
+def test_generic_table_three_elements():
+    # irregular table: zeta = 3, Rs != 0, a missing pair group, an element with few SFs,
+    # different hidden sizes -> the generic angular kernel and the generic network tiles
+    rows = []
+    for c in range(3):
+        for e1 in range(3):
+            rows.append((c, 2, e1, 0, 0.05 + 0.01 * c, 0.5 * e1, 0.0, 0.0))
+            rows.append((c, 2, e1, 0, 0.3, 1.0, 0.0, 0.0))
+        for (e1, e2) in ((0, 0), (0, 1), (1, 2), (2, 2)):      # (0,2) and (1,1) absent
+            rows.append((c, 3, e1, e2, 0.002, 1.0, 3.0))
+            rows.append((c, 3, e2, e1, 0.013, -1.0, 1.0))
+            rows.append((c, 3, e1, e2, 0.002, -1.0, 6.0))
+    rows = [r if len(r) == 8 else (r[0], r[1], r[2], r[3], r[4], 0.0, r[5], r[6]) for r in rows]
+    model = tiny_model(rows, n_elem=3, hidden=(7, 5, 3), seed=11)
+    sysm = W.make_water(120, 5, L=13.0)
+    sysm.types = (np.arange(sysm.n_atoms) % 3).astype(np.int32)
+    from paper_2002_00054_b200 import NNP
+    nnp = NNP.from_model(model)
+    assert not nnp.uses_fast_path()
+    nnp.close()
+    _check_full(model, sysm)
+
+
+def test_single_element_radial_only():
+    model = tiny_model([(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0), (0, 2, 0, 0, 0.4, 2.0, 0.0, 0.0)], hidden=(4,))
+    sysm = W.make_water(60, 3, L=12.4)
+    sysm.types[:] = 0
+    _check_full(model, sysm)
+
+
+@pytest.mark.parametrize("k", [1, 2, 3, 4])
+def test_full_size_configs_sampled(k):
+    """configs[1..4] at full size, in the launch configuration bench.py times: sampled outputs the
+    oracle can compute one by one (neighbour rows, G_i, E_i, F_m) + properties that hold at any size."""
+    from paper_2002_00054_b200 import NNP
+    cfg = W.CONFIGS[k]
+    sysm, model = W.build(cfg)
+    nnp = NNP.from_model(model)
+    n = sysm.n_atoms
+    e_atom, e_total, force = _run(nnp, sysm.pos, sysm.types, sysm.box)
+    n_samples = {1: 12, 2: 8, 3: 5, 4: 4}[k]
+    rs = np.random.RandomState(1000 + k)
+    samples = np.sort(rs.choice(n, n_samples, replace=False))
+    om = oracle.OracleModel(model)
+    ref = oracle.forces_on(om, sysm.pos, sysm.types, sysm.box, samples)
+    off, idx = nnp.neighbors(n)
+    off = off.cpu().numpy(); idx = idx.cpu().numpy()
+    G = nnp.symmetry_functions(n)[torch.tensor(samples, device=_dev())].cpu().numpy()
+    emax = np.abs(e_atom).max()
+    for q, m in enumerate(samples):
+        assert np.array_equal(idx[off[m]:off[m + 1]], ref.rows[q])          # bit-exact neighbour set
+        assert np.all(np.abs(G[q] - ref.G[q]) <= 1e-11 * np.maximum(1.0, np.abs(ref.G[q])))
+        assert abs(e_atom[m] - ref.e_atom[q]) <= 1e-10 * emax
+        assert np.abs(force[m] - ref.F[q]).max() <= F_ABS
+    # properties at full size
+    assert abs(e_total - e_atom.sum()) <= 1e-11 * np.abs(e_atom).sum()
+    assert np.all(np.abs(force.sum(axis=0)) < 1e-7)
+    cnt = np.diff(off)
+    assert 85 < cnt.mean() < 97 and cnt.max() < 160
+    # neighbour symmetry j in N(i) <=> i in N(j) on a sample of rows
+    for m in samples[:3]:
+        for j in idx[off[m]:off[m + 1]][:10]:
+            assert m in idx[off[j]:off[j + 1]]
+    nnp.close()
+
+
+def test_config1_displacement_sequence():
+    """configs[1]: repeated evaluations with cumulative sigma = 0.01 A kicks (reading C15); positions
+    drift out of the box and are re-wrapped by the library.  Parity at calls 0, 1, 50, 99 (sampled)."""
+    from paper_2002_00054_b200 import NNP
+    cfg = W.CONFIGS[1]
+    sysm, model = W.build(cfg)
+    nnp = NNP.from_model(model)
+    om = oracle.OracleModel(model)
+    pos = sysm.pos.copy()
+    samples = np.array([5, 7777, 24575])
+    for call in range(100):
+        if call >= 1:
+            pos = pos + W.displacement(sysm.n_atoms, cfg.seed_disp, call)
+        if call in (0, 1, 50, 99):
+            e_atom, e_total, force = _run(nnp, pos, sysm.types, sysm.box)
+            ref = oracle.forces_on(om, pos, sysm.types, sysm.box, samples)
+            off, idx = nnp.neighbors(sysm.n_atoms)
+            off = off.cpu().numpy(); idx = idx.cpu().numpy()
+            for q, m in enumerate(samples):
+                assert np.array_equal(idx[off[m]:off[m + 1]], ref.rows[q])
+                assert abs(e_atom[m] - ref.e_atom[q]) <= 1e-10 * np.abs(e_atom).max()
+                assert np.abs(force[m] - ref.F[q]).max() <= F_ABS
+    nnp.close()
+
+
+# ------------------------------------------------------------------------ edge cases
+
+def test_empty_and_tiny_inputs():
+    from paper_2002_00054_b200 import NNP
+    model = W.make_model(False)
+    nnp = NNP.from_model(model)
+    om = oracle.OracleModel(model)
+    box = np.array([20.0, 20.0, 20.0])
+    e_atom, e_total, force = _run(nnp, np.zeros((0, 3)), np.zeros(0, dtype=np.int32), box)
+    assert e_total == 0.0 and e_atom.shape == (0,) and force.shape == (0, 3)
+    # one atom: no neighbours, E = NN(0)
+    pos = np.array([[3.0, 4.0, 5.0]])
+    typ = np.array([1], dtype=np.int32)
+    e_atom, e_total, force = _run(nnp, pos, typ, box)
+    ref = oracle.compute(om, pos, typ, box)
+    assert abs(e_total - ref.e_total) <= 1e-12 * abs(ref.e_total) and np.all(force == 0.0)
+    # two atoms through the periodic boundary, one of them far outside the box
+    pos = np.array([[0.4, 1.0, 1.0], [19.5 + 40.0, 1.0 - 20.0, 1.0]])
+    typ = np.array([1, 0], dtype=np.int32)
+    e_atom, e_total, force = _run(nnp, pos, typ, box)
+    ref = oracle.compute(om, pos, typ, box)
+    assert abs(e_total - ref.e_total) <= E_REL * abs(ref.e_total)
+    assert np.abs(force - ref.F).max() <= F_ABS
+    assert np.abs(force).max() > 1e-6
+    nnp.close()
+
+
+def test_error_codes():
+    from paper_2002_00054_b200 import NNP, NNPError
+    model = W.make_model(False)
+    nnp = NNP.from_model(model)
+    dev = _dev()
+    sysm = W.make_water(50, 1, L=13.0)
+    pos = torch.tensor(sysm.pos, device=dev)
+    typ = torch.tensor(sysm.types, device=dev)
+    with pytest.raises(NNPError) as ei:
+        nnp.compute(pos, typ, [11.9, 13.0, 13.0])
+    assert ei.value.status == 2                       # NNP_ERR_BOX_TOO_SMALL
+    bad = typ.clone(); bad[3] = 2
+    with pytest.raises(NNPError) as ei:
+        nnp.compute(pos, bad, sysm.box)
+    assert ei.value.status == 3                       # NNP_ERR_TYPE_RANGE
+    badp = pos.clone(); badp[10, 1] = float("nan")
+    with pytest.raises(NNPError) as ei:
+        nnp.compute(badp, typ, sysm.box)
+    assert ei.value.status == 7                       # NNP_ERR_NONFINITE
+    # neighbour overflow: 150 atoms in 13^3 have ~60 neighbours each; allow only 32
+    nnp.set_max_neighbors(32)
+    with pytest.raises(NNPError) as ei:
+        nnp.compute(pos, typ, sysm.box)
+    assert ei.value.status == 4                       # NNP_ERR_NEIGHBOR_OVERFLOW
+    nnp.set_max_neighbors(160)
+    nnp.compute(pos, typ, sysm.box)                   # recovers
+    nnp.close()
+
+
+def test_dense_cluster_near_max_neighbors():
+    # 240 atoms in a 12.2 A box: ~115 neighbours per atom (close to the 160 cap)
+    sysm = W.make_water(80, 21, L=12.2)
+    _check_full(W.make_model(False), sysm)
+
+
+def test_host_buffer_entry_point_and_determinism():
+    from paper_2002_00054_b200 import NNP
+    sysm, model = W.build(W.CONFIGS[0])
+    nnp = NNP.from_model(model)
+    e1, E1, f1 = _run(nnp, sysm.pos, sysm.types, sysm.box)
+    e2, E2, f2 = _run(nnp, sysm.pos, sysm.types, sysm.box)
+    assert E1 == E2 and np.array_equal(e1, e2)        # fixed summation order for energies
+    assert np.abs(f1 - f2).max() < 1e-12              # forces: FP64 atomics, order may vary
+    eh, Eh, fh = nnp.compute_host(sysm.pos, sysm.types, sysm.box)
+    assert Eh[0] == E1 and np.array_equal(eh, e1) and np.abs(fh - f1).max() < 1e-12
+    nnp.close()
+
+
+def test_timings_and_launch_count():
+    from paper_2002_00054_b200 import NNP
+    sysm, model = W.build(W.CONFIGS[0])
+    nnp = NNP.from_model(model)
+    nnp.set_timing(True)
+    _run(nnp, sysm.pos, sysm.types, sysm.box)
+    t = nnp.timings_ms()
+    assert set(t) == {"sort", "neighbors", "symmetry_functions", "networks", "forces", "finalize"}
+    assert all(v >= 0.0 for v in t.values()) and t["forces"] > 0.0
+    assert nnp.last_launch_count() >= 9
+    nnp.close()
