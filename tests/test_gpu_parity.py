@@ -78,8 +78,8 @@ def test_orthorhombic_box_2_3_5_cells():
     # box 12.6 x 18.7 x 31 -> 2, 3 and 5 cells: every stencil de-dup branch at once
     box = np.array([12.6, 18.7, 31.0])
     n_mol = 245
-    base = W.make_water(n_mol, 77, L=1.0)
-    sysm = W.WaterSystem(pos=base.pos * 0 + _uniform_in(box, 3 * n_mol, 77), types=base.types, box=box, seed=77)
+    types = np.tile(np.array([W.TYPE_O, W.TYPE_H, W.TYPE_H], dtype=np.int32), n_mol)
+    sysm = W.WaterSystem(pos=_uniform_in(box, 3 * n_mol, 77), types=types, box=box, seed=77)
     _check_full(W.make_model(False), sysm)
 
 
