@@ -1,0 +1,345 @@
+"""bench.py -- NNP energy+force throughput on B200 (BASELINE.json metric: atom-steps/s + roofline fraction).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config k] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (S0 sort .. S5 reduce, neighbour list rebuilt every
+call) over one synthetic water-like system.  Default workload = BASELINE.json configs[3]
+(2,097,153 atoms, base-52 model): the configuration the north-star target is quoted on; it fits
+one GPU.  N > 1 (torchrun): the path does not shard in this build ("replicas only", DESIGN.md
+section 8(e)) -> every rank evaluates the same system on its own GPU, value = N * atoms * K / max time.
+
+One JSON line on stdout (rank 0).  Extra keys: roofline (dominant kernel k_force, FP64-ALU bound),
+cpu_baseline (the oracle on a bounded sample of centres of the same system), e2e (host buffers
+through nnp_compute_host), clocks, gpu_launches, stage_ms.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+METRIC = "nnp_energy_force_atom_steps_per_sec"
+UNIT = "atom-steps/s"
+
+# Algorithmic FP64-pipe thread-instructions per atom-step (
+# SURVEY.md 8(d)): minimal per-centre evaluation, water-like workload statistics
+# (91 neighbours, 4,141 enumerated (j,k), 1,941 contributing triplets per atom).
+FP64_INSTR_PER_ATOM = {
+    False: {"sf": 230e3, "mlp": 7e3, "force": 400e3},     # base-52 model
+    True: {"sf": 368e3, "mlp": 33e3, "force": 586e3},      # wide-128 model
+}
+# FP64 pipe peak derived from unit counts and clocks: 148 SMs x 64 DFMA lanes/clk x clocks.max.sm
+FP64_LANES_PER_SM = 64
+N_SM = 148
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return json.load(open(p))
+    except Exception:
+        return {}
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.rows = []
+        self.proc = None
+        self.thread = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+            return
+        def pump():
+            for line in self.proc.stdout:
+                self.rows.append(line.strip())
+        self.thread = threading.Thread(target=pump, daemon=True)
+        self.thread.start()
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for k, nm in enumerate(names):
+                if f[3 + k].lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(power)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def oracle_sample(cfg_index: int, n_centres: int, seed: int = 12345):
+    """Time the CPU oracle, as it stands, on `n_centres` randomly chosen centres of the workload:
+    brute-force neighbour search + SFs + network + force contributions of each centre
+    (= n_centres atom-steps).  -> (seconds, seconds in the neighbour search, cores)."""
+    import oracle
+    import workloads as W
+    sysm, model = W.build(W.CONFIGS[cfg_index])
+    om = oracle.OracleModel(model)
+    rs = np.random.RandomState(seed)
+    sel = np.sort(rs.choice(sysm.n_atoms, min(n_centres, sysm.n_atoms), replace=False)).astype(np.int64)
+    t0 = time.perf_counter()
+    r = oracle.centres(om, sysm.pos, sysm.types, sysm.box, sel, forces=True, want_g=False)
+    dt = time.perf_counter() - t0
+    return dt, float(r.timing[0]), 1, int(sel.size)
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    import workloads as W
+    cfg = W.CONFIGS[args.config]
+    sysm, model = W.build(cfg)
+    om = oracle.OracleModel(model)
+    # ~50 ms per centre at 2.1 M atoms (O(N) neighbour scan each): keep the whole run to a few minutes
+    per_step = args.ref_centres
+    if per_step <= 0:
+        budget_s = 120.0
+        est = 2.5e-8 * sysm.n_atoms + 1.2e-2
+        per_step = int(max(4, min(512, budget_s / ((args.steps + args.warmup) * est))))
+    rs = np.random.RandomState(777)
+
+    def step():
+        sel = np.sort(rs.choice(sysm.n_atoms, min(per_step, sysm.n_atoms), replace=False)).astype(np.int64)
+        oracle.centres(om, sysm.pos, sysm.types, sysm.box, sel, forces=True, want_g=False)
+        return sel.size
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    done = 0
+    for _ in range(args.steps):
+        done += step()
+    dt = time.perf_counter() - t0
+    value = done / dt
+    sample = "%d randomly chosen centres of %s per step (brute-force neighbours + SF + MLP + forces each)" % (
+        per_step, cfg.name)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "n_atoms": sysm.n_atoms, "model": model.name,
+                   "parallelism": "1 host core (single-threaded oracle)"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="index into BASELINE.json configs (default 3 = 2.1 M atoms)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--ref-centres", type=int, default=0, help="--impl reference: centres per step (0 = auto)")
+    ap.add_argument("--cpu-centres", type=int, default=400, help="oracle sample size of the cpu_baseline leg (0 = skip)")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-probe", action="store_true", help="skip the DFMA issue-rate probe (for ncu runs)")
+    args = ap.parse_args()
+    if args.warmup < 3:
+        args.warmup = 3
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+
+    import workloads as W
+    from paper_2002_00054_b200 import NNP, measure_fp64_peak
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    cfg = W.CONFIGS[args.config]
+    sysm, model = W.build(cfg)
+    n = sysm.n_atoms
+    nnp = NNP.from_model(model, device=local)
+    pos = torch.tensor(sysm.pos, dtype=torch.float64, device=dev)
+    typ = torch.tensor(sysm.types, dtype=torch.int32, device=dev)
+    out = (torch.empty(n, dtype=torch.float64, device=dev), torch.empty(1, dtype=torch.float64, device=dev),
+           torch.empty((n, 3), dtype=torch.float64, device=dev))
+    # configs[1]: small random displacements between calls (cumulative, applied on the device copy)
+    disp = None
+    if cfg.seed_disp is not None:
+        disp = [torch.tensor(W.displacement(n, cfg.seed_disp, c + 1), device=dev) for c in range(4)]
+
+    def step(i):
+        if disp is not None:
+            pos.add_(disp[i % len(disp)])
+        nnp.compute(pos, typ, sysm.box, out=out, sync=False)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # FP64 issue-rate probe (roofline context), before the timed region
+    dfma_burst, dfma_sust = (float("nan"), float("nan")) if args.no_probe else measure_fp64_peak(local, 0.5)
+
+    for i in range(args.warmup):
+        step(i)
+    nnp.sync_status()
+    nnp.set_timing(True)
+    stage_ms = np.zeros(6)
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    barrier()
+    e0 = torch.cuda.Event(enable_timing=True)
+    e1 = torch.cuda.Event(enable_timing=True)
+    launches = 0
+    e0.record()
+    for i in range(args.steps):
+        step(i)
+        launches += nnp.last_launch_count()
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    # stage times of the LAST timed step (events recorded on the stream inside nnp_compute)
+    t_last = nnp.timings_ms()
+    clocks = sampler.stop() if rank == 0 else None
+    nnp.sync_status()
+    nnp.set_timing(False)
+    if world > 1:
+        t = torch.tensor([ms], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+
+    # per-stage average over K more (untimed for the headline) steps, events inside nnp_compute
+    nnp.set_timing(True)
+    for i in range(args.steps):
+        step(i)
+        tm = nnp.timings_ms()
+        stage_ms += np.array([tm[k] for k in ("sort", "neighbors", "symmetry_functions", "networks", "forces", "finalize")])
+    stage_ms /= args.steps
+    nnp.set_timing(False)
+
+    # end to end: HOST buffers through nnp_compute_host (h2d + compute + d2h inside the call)
+    e2e = None
+    if not args.no_e2e:
+        hp = torch.tensor(sysm.pos, dtype=torch.float64).pin_memory()
+        ht = torch.tensor(sysm.types, dtype=torch.int32).pin_memory()
+        he = torch.empty(n, dtype=torch.float64).pin_memory()
+        hE = torch.empty(1, dtype=torch.float64).pin_memory()
+        hf = torch.empty((n, 3), dtype=torch.float64).pin_memory()
+        for _ in range(2):
+            nnp.compute_host(hp, ht, sysm.box, out=(he, hE, hf))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            nnp.compute_host(hp, ht, sysm.box, out=(he, hE, hf))
+        dt = time.perf_counter() - t0
+        if world > 1:
+            t = torch.tensor([dt], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            dt = float(t.item())
+        e2e = {"value": world * n * args.steps / dt, "unit": UNIT, "h2d_bytes_per_step": n * 28,
+               "d2h_bytes_per_step": n * 32 + 8, "ms_per_step": 1e3 * dt / args.steps,
+               "api": "nnp_compute_host (pinned host buffers)"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    peaks = _peaks()
+    sm_max = float(peaks.get("sm_max_mhz", 1965.0))
+    peak_alu = N_SM * FP64_LANES_PER_SM * sm_max * 1e6
+    instr = FP64_INSTR_PER_ATOM[cfg.wide]
+    force_ms = float(stage_ms[4])
+    achieved = instr["force"] * n / (force_ms * 1e-3)
+    total_instr = sum(instr.values()) * n
+    hbm_bytes_per_atom = 2.8e3 if not cfg.wide else 5.2e3
+    roofline = {
+        "bound": "alu", "kernel": "k_force", "achieved": achieved / 1e12, "peak": peak_alu / 1e12,
+        "unit": "T FP64 instr/s", "frac": achieved / peak_alu, "traffic": None,
+        "peak_source": "derived: 148 SMs x 64 FP64 lanes x %.0f MHz (clocks.max.sm); DFMA probe in this run: "
+                       "burst %.2f, sustained %.2f T instr/s" % (sm_max, dfma_burst / 1e12, dfma_sust / 1e12),
+        "frac_of_measured_dfma": achieved / dfma_burst,
+        "algorithmic_instr_per_launch": instr["force"] * n,
+        "kernel_ms": force_ms,
+        "whole_step": {"fp64_instr": total_instr, "frac": total_instr / (ms / args.steps * 1e-3) / peak_alu,
+                       "hbm_bytes": hbm_bytes_per_atom * n,
+                       "hbm_frac": hbm_bytes_per_atom * n / (ms / args.steps * 1e-3) / (peaks.get("hbm_gbs", 6650.0) * 1e9)},
+    }
+
+    cpu = None
+    if args.cpu_centres > 0:
+        dt, t_nbr, cores, ns = oracle_sample(args.config, args.cpu_centres)
+        cpu = {"value": ns / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "%d randomly chosen centres of %s, each: O(N) brute-force neighbour scan + SFs + MLP + "
+                         "force contributions; %.1f s total, %.1f s of it in the neighbour scan" % (ns, cfg.name, dt, t_nbr)}
+
+    line = {
+        "metric": METRIC, "value": world * n * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "n_atoms": n, "model": model.name, "box": float(sysm.box[0]),
+                   "neighbor_rebuild": "every call", "parallelism": "replicas x%d" % world,
+                   "l2": ("working set per step (%.2f GB workspace) %s the 126 MB L2; no flush between steps"
+                          % (nnp.workspace_bytes(n) / 1e9, "exceeds" if nnp.workspace_bytes(n) > 126e6 else "FITS IN"))},
+        "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks, "gpu_launches": launches,
+        "stage_ms": dict(zip(("sort", "neighbors", "symmetry_functions", "networks", "forces", "finalize"),
+                             [float(x) for x in stage_ms])),
+        "stage_ms_last_timed_step": t_last,
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

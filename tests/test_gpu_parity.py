@@ -109,7 +109,7 @@ def test_generic_table_three_elements():
             rows.append((c, 3, e1, e2, 0.002, -1.0, 6.0))
     rows = [r if len(r) == 8 else (r[0], r[1], r[2], r[3], r[4], 0.0, r[5], r[6]) for r in rows]
     model = tiny_model(rows, n_elem=3, hidden=(7, 5, 3), seed=11)
-    sysm = W.make_water(120, 5, L=13.0)
+    sysm = W.make_water(120, 5, L=15.0)
     sysm.types = (np.arange(sysm.n_atoms) % 3).astype(np.int32)
     from paper_2002_00054_b200 import NNP
     nnp = NNP.from_model(model)
