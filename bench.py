@@ -51,6 +51,23 @@ def _peaks():
         return {}
 
 
+def max_over_ranks(x: float, device=None) -> float:
+    """MAX of a per-rank scalar over the process group (identity when not initialised)."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+        return float(x)
+    t = torch.tensor([float(x)], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(n_atoms: int, steps: int, world: int, ms_max: float) -> float:
+    """Whole-job atom-steps/s of `world` independent replicas ("replicas only"):
+    every rank evaluates n_atoms atoms `steps` times; the job ends when the slowest rank ends."""
+    return world * n_atoms * steps / (ms_max * 1e-3)
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
 
@@ -252,10 +269,7 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     nnp.sync_status()
     nnp.set_timing(False)
-    if world > 1:
-        t = torch.tensor([ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
+    ms = max_over_ranks(ms, dev)
 
     # per-stage average over K more (untimed for the headline) steps, events inside nnp_compute
     nnp.set_timing(True)
@@ -281,11 +295,8 @@ def main():
         for _ in range(args.steps):
             nnp.compute_host(hp, ht, sysm.box, out=(he, hE, hf))
         dt = time.perf_counter() - t0
-        if world > 1:
-            t = torch.tensor([dt], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            dt = float(t.item())
-        e2e = {"value": world * n * args.steps / dt, "unit": UNIT, "h2d_bytes_per_step": n * 28,
+        dt = max_over_ranks(dt, dev)
+        e2e = {"value": job_value(n, args.steps, world, dt * 1e3), "unit": UNIT, "h2d_bytes_per_step": n * 28,
                "d2h_bytes_per_step": n * 32 + 8, "ms_per_step": 1e3 * dt / args.steps,
                "api": "nnp_compute_host (pinned host buffers)"}
 
@@ -323,7 +334,7 @@ def main():
                          "force contributions; %.1f s total, %.1f s of it in the neighbour scan" % (ns, cfg.name, dt, t_nbr)}
 
     line = {
-        "metric": METRIC, "value": world * n * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+        "metric": METRIC, "value": job_value(n, args.steps, world, ms), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg.name, "n_atoms": n, "model": model.name, "box": float(sysm.box[0]),
