@@ -4,11 +4,12 @@
 //
 // Design: one warp owns one centre atom.  Its neighbours are staged once
 // in shared memory (min-image vectors, 1/r, cutoff values, per-eta Gaussians); candidate
-// (j,k) pairs are enumerated in "tournament" order (round r pairs slot j with slot j+r), the
-// cheap r_jk < rc test is ballot-compacted into a small queue, and the expensive per-triplet
-// work runs only on full batches of 32 contributing triplets -> no idle lanes in the hot loop
+// (j,k) pairs are enumerated in rounds (round r pairs slot j with slot j+r), the cheap
+// r_jk < rc test is ballot-compacted into a small FIFO, and the expensive per-triplet work
+// runs only on full batches of 32 contributing triplets -> no idle lanes in the hot loop
 // even though only ~47 % of the enumerated pairs contribute.
 #pragma once
+#include "mathfn.cuh"
 #include "nnp_internal.h"
 
 namespace nnp {
@@ -73,7 +74,7 @@ __device__ __forceinline__ double ipow(double x) {
 // E[e] = exp(-eta_e * x) for all etas of the spec from ONE exp() and multiplication chains
 template <class Spec>
 __device__ __forceinline__ void eta_chain(double x, double eta0, double* E) {
-    E[0] = exp(-eta0 * x);
+    E[0] = exp_small(-eta0 * x);    // nnp_create admits a Spec only if eta_max * 3 rc^2 <= 700
     if constexpr (Spec::NETA > 1) E[1] = ipow<Spec::ratio(1)>(E[Spec::rbase(1)]);
     if constexpr (Spec::NETA > 2) E[2] = ipow<Spec::ratio(2)>(E[Spec::rbase(2)]);
     if constexpr (Spec::NETA > 3) E[3] = ipow<Spec::ratio(3)>(E[Spec::rbase(3)]);
@@ -92,31 +93,38 @@ struct Nbh {
     double2* p0;   // (ux, uy)
     double2* p1;   // (uz, 1/a)
     double2* p2;   // (fc(a), a) in the SF kernel; (fc(a), fc'(a)/a) in the force kernel
+                   // fc(a) = C^2, fc'(a)/a = -2 k2 C S with z = k2 a^2, k2 = (pi/(2 rc))^2 (mathfn.cuh)
     double* pe;    // [slot * NETA + e]: SF kernel: exp(-eta_e a^2) * fc(a); force kernel: exp(-eta_e a^2)
 };
 
 // ---------------------------------------------------------------- triplet enumeration
-// Calls f(j, k, active) for batches of 32 contributing pairs (c^2 < rc2).  `queue` is 64 uint16
-// per warp.  Pairs inside one segment [s, s+ns) use the tournament order: round r = 1..ns/2 pairs
-// slot j with (j + r) mod ns, which visits each unordered pair once and keeps the j's (and the
-// k's) of one round all distinct -- the force kernel relies on that to keep shared-memory
-// atomic conflicts rare.
+// Calls f(j, k, colour, active) for batches of 32 contributing pairs (c^2 < rc2).
+//
+// Pairs are enumerated in ROUNDS; inside one round every slot appears at most once as j and at
+// most once as k (within a segment: round r pairs slot j with (j + r) mod ns -- the "tournament"
+// order; between two segments: round r pairs slot s of the smaller segment with slot (s + r) mod
+// n_big of the bigger one).  The round number travels with the pair through the compaction queue
+// as its COLOUR: entries of equal colour never share a j or a k, which lets the force kernel
+// accumulate per-slot forces with plain shared-memory read-modify-writes, one colour at a time,
+// instead of FP64 shared atomics (CAS loops -- ncu showed them to be >35 % of the stall samples).
+// The queue is a 64-entry FIFO ring per warp, so a batch holds 2-4 consecutive colours.
 struct PairQueue {
-    uint16_t* q;
-    int n;
+    uint32_t* q;    // [64] (colour << 16) | (j << 8) | k
+    int head, n;
 };
 
 template <class F>
-__device__ __forceinline__ void push_and_drain(PairQueue& Q, bool pass, int j, int k, int lane, F& f) {
+__device__ __forceinline__ void push_and_drain(PairQueue& Q, bool pass, int j, int k, int col, int lane, F& f) {
     const unsigned m = __ballot_sync(0xffffffffu, pass);
-    if (pass) Q.q[Q.n + __popc(m & ((1u << lane) - 1u))] = (uint16_t)((j << 8) | k);
+    if (pass) Q.q[(Q.head + Q.n + __popc(m & ((1u << lane) - 1u))) & 63] = ((unsigned)col << 16) | (unsigned)((j << 8) | k);
     Q.n += __popc(m);
     __syncwarp();
     if (Q.n >= 32) {
-        const unsigned e = Q.q[Q.n - 32 + lane];
+        const unsigned e = Q.q[(Q.head + lane) & 63];
+        Q.head = (Q.head + 32) & 63;
         Q.n -= 32;
         __syncwarp();
-        f((int)(e >> 8), (int)(e & 255u), true);
+        f((int)((e >> 8) & 255u), (int)(e & 255u), (int)(e >> 16), true);
     }
 }
 
@@ -124,10 +132,11 @@ template <class F>
 __device__ __forceinline__ void drain_tail(PairQueue& Q, int lane, F& f) {
     if (Q.n > 0) {
         const bool act = lane < Q.n;
-        const unsigned e = Q.q[act ? lane : 0];
+        const unsigned e = Q.q[(Q.head + (act ? lane : 0)) & 63];
         Q.n = 0;
+        Q.head = 0;
         __syncwarp();
-        f((int)(e >> 8), (int)(e & 255u), act);
+        f((int)((e >> 8) & 255u), (int)(e & 255u), (int)(e >> 16), act);
     }
     __syncwarp();
 }
@@ -139,7 +148,7 @@ __device__ __forceinline__ bool pair_close(const Nbh& nb, int j, int k, double r
     return wx * wx + wy * wy + wz * wz < rc2;
 }
 
-// all unordered pairs inside segment [s, s+ns)
+// all unordered pairs inside segment [s, s+ns); colours 1..ns/2
 template <class F>
 __device__ __forceinline__ void enum_within(const Nbh& nb, int s, int ns, double rc2, PairQueue& Q, int lane, F& f) {
     const int rounds = ns / 2;                 // r = 1..rounds; for even ns the last round is half
@@ -151,24 +160,29 @@ __device__ __forceinline__ void enum_within(const Nbh& nb, int s, int ns, double
             if (kk >= ns) kk -= ns;
             const bool valid = jj < lim;
             const bool pass = valid && pair_close(nb, s + jj, s + kk, rc2);
-            push_and_drain(Q, pass, s + jj, s + kk, lane, f);
+            push_and_drain(Q, pass, s + jj, s + kk, r, lane, f);
         }
     }
 }
 
-// all pairs (j in [s1, s1+n1), k in [s2, s2+n2)), disjoint segments
+// all pairs (j in [s1, s1+n1), k in [s2, s2+n2)), disjoint segments; colours 0..max(n1,n2)-1
 template <class F>
 __device__ __forceinline__ void enum_between(const Nbh& nb, int s1, int n1, int s2, int n2, double rc2, PairQueue& Q,
                                              int lane, F& f) {
     if (n1 == 0 || n2 == 0) return;
-    for (int j0 = 0; j0 < n1; j0 += 32) {
-        const int jj = j0 + lane;
-        const bool valid = jj < n1;
-        int kk = jj % n2;                      // start of this lane's diagonal
-        for (int r = 0; r < n2; ++r) {
-            const bool pass = valid && pair_close(nb, s1 + jj, s2 + kk, rc2);
-            push_and_drain(Q, pass, s1 + jj, s2 + kk, lane, f);
-            if (++kk == n2) kk = 0;
+    const bool swap = n1 < n2;                 // lanes walk the smaller segment
+    const int ss = swap ? s1 : s2, ns = swap ? n1 : n2;      // small
+    const int sb = swap ? s2 : s1, nbig = swap ? n2 : n1;    // big
+    for (int r = 0; r < nbig; ++r) {
+        for (int q0 = 0; q0 < ns; q0 += 32) {
+            const int qs = q0 + lane;
+            int qb = qs + r;
+            if (qb >= nbig) qb -= nbig;        // qs < ns <= nbig and r < nbig: one wrap is enough
+            const bool valid = qs < ns;
+            const int j = swap ? ss + qs : sb + qb;           // j from segment 1, k from segment 2
+            const int k = swap ? sb + qb : ss + qs;
+            const bool pass = valid && pair_close(nb, j, k, rc2);
+            push_and_drain(Q, pass, j, k, r, lane, f);
         }
     }
 }

@@ -3,12 +3,17 @@
 // move as little data as possible, recomputing where necessary", L98, L124).  This holds "the
 // dominant angular force loop" (L116) and is the hottest kernel of the path.
 //
-// One warp per centre i, same staging / tournament enumeration / compaction as k_sf.cu.  For a
+// One warp per centre i, same staging / round enumeration / compaction as k_sf.cu.  For a
 // triplet (i; j,k) with u = r_j - r_i, v = r_k - r_i, w = v - u the beta-weighted gradient is
 //     dg/du = f_uu u + f_uv v - f_w w,      dg/dv = f_vv v + f_uv u + f_w w
-// (DESIGN.md "Force algebra"); the forces on j and k are accumulated per neighbour SLOT in shared
-// memory (FP64 atomicAdd = CAS loop; the tournament order keeps same-address collisions inside a
-// batch to <= 2-3), and each slot is flushed ONCE per centre with global FP64 atomics.
+// (DESIGN.md "Force algebra"), so  F_j = -s1 u + s3 v,  F_k = -s2 v + s3 u  with
+// s1 = f_uu + f_w, s2 = f_vv + f_w, s3 = f_w - f_uv.  Per neighbour SLOT the kernel accumulates
+// the scalar A = sum s1 and the vector V = sum s3 (partner vector) in shared memory and forms
+// F_slot = V - A u once per centre; the slot forces are flushed with one global FP64 RED per
+// component per neighbour.  Slot accumulation is a plain read-modify-write done one COLOUR at
+// a time (angular.cuh): pairs of equal colour never share a slot, and a warp owns its slots, so
+// no shared-memory atomics are needed (the first version's FP64 shared atomicAdd = CAS loops
+// took >35 % of the stall samples and ran 2.8 iterations on average; profiles/r1_*).
 #include "angular.cuh"
 #include "geometry.cuh"
 
@@ -20,7 +25,7 @@ constexpr double PI_D = 3.14159265358979323846;
 struct ForceParams {
     int64_t n;
     int n_elem, ncell, stride, cap, g_stride;
-    double rc, rc2, inv_rc;
+    double rc, rc2, inv_rc, k2;          // k2 = (pi / (2 rc))^2
     double box[3], half[3];
     const double *sx, *sy, *sz;
     const int32_t *cell_start, *nbr, *nbr_cnt;
@@ -32,67 +37,86 @@ struct ForceParams {
 
 template <class Spec>
 __host__ __device__ constexpr size_t force_warp_smem(int cap, int g_stride) {
-    // p0,p1,p2 + pe per slot + slot forces (3 doubles) ; queue ; beta row ; per-group coefficient tables
-    size_t b = (size_t)cap * (48 + 8 * Spec::NETA + 24) + 128 + (size_t)g_stride * 8;
-    b += (size_t)2 * Spec::NACC * 8;
+    // per slot: p0,p1,p2 (48 B) + pe (8*NETA) + accumulators (A,Vx),(Vy,Vz) (32 B);
+    // queue (64 x u32); beta row; per-group coefficient table (double2 per menu entry)
+    size_t b = (size_t)cap * (48 + 8 * Spec::NETA + 32) + 256 + (size_t)g_stride * 8;
+    b += (size_t)Spec::NACC * 16;
     return (b + 15) / 16 * 16;
 }
 
-// shared "slot force" accumulators
-struct SlotF {
-    double *x, *y, *z;
+// shared per-slot accumulators: F_slot = V - A * u
+struct SlotAcc {
+    double2* av;   // (A, Vx)
+    double2* yz;   // (Vy, Vz)
 };
 
-// common tail of the per-triplet work: from Z0 = sum beta P Y, Z1 = sum beta P' Y, Z2 = sum eta beta P Y
-// (Y = product of the three bare Gaussians) to the two slot forces.
+// From Z0 = sum beta P Y, Z1 = sum beta P' Y, Z2 = sum eta beta P Y  (Y = product of the three
+// bare Gaussians) to the slot updates.  fcc = fc(c), dfc = fc'(c)/c.
 __device__ __forceinline__ void triplet_forces(const double2 j0, const double2 j1, const double2 j2, const double2 k0,
                                                const double2 k1, const double2 k2, double fcc, double dfc, double cosv,
-                                               double Z0, double Z1, double Z2, const SlotF& sf, int j, int k, bool active) {
+                                               double iab, double Z0, double Z1, double Z2, const SlotAcc& acc, int j,
+                                               int k, int col, bool active) {
     const double fa = j2.x, dfa = j2.y, fb = k2.x, dfb = k2.y, ia = j1.y, ib = k1.y;
     const double fab = fa * fb;
     const double C = fab * fcc;
-    const double t2 = 2.0 * C * Z2;
-    const double f_w = (fab * dfc) * Z0 - t2;
+    const double t2 = (C + C) * Z2;
+    const double f_w = fma(fab * dfc, Z0, -t2);
     const double q = Z1 * C;
     const double qc = q * cosv;
-    const double f_uu = (dfa * fb * fcc) * Z0 - t2 - qc * (ia * ia);
-    const double f_vv = (fa * dfb * fcc) * Z0 - t2 - qc * (ib * ib);
-    const double f_uv = q * (ia * ib);
-    const double s1 = f_uu + f_w, s2 = f_vv + f_w, s3 = f_w - f_uv;
-    // F_j = -dg/du = -s1 u + s3 v ;  F_k = -dg/dv = -s2 v + s3 u
-    if (!active) return;
-    atomicAdd(&sf.x[j], s3 * k0.x - s1 * j0.x);
-    atomicAdd(&sf.y[j], s3 * k0.y - s1 * j0.y);
-    atomicAdd(&sf.z[j], s3 * k1.x - s1 * j1.x);
-    atomicAdd(&sf.x[k], s3 * j0.x - s2 * k0.x);
-    atomicAdd(&sf.y[k], s3 * j0.y - s2 * k0.y);
-    atomicAdd(&sf.z[k], s3 * j1.x - s2 * k1.x);
+    const double f_uu = fma(-qc, ia * ia, fma((dfa * fb) * fcc, Z0, -t2));
+    const double f_vv = fma(-qc, ib * ib, fma((fa * dfb) * fcc, Z0, -t2));
+    const double s1 = f_uu + f_w, s2 = f_vv + f_w, s3 = fma(-q, iab, f_w);
+    // colour passes: entries of one colour have pairwise distinct j and pairwise distinct k
+    unsigned pend = __ballot_sync(0xffffffffu, active);
+    while (pend) {
+        const int c = __shfl_sync(0xffffffffu, col, __ffs(pend) - 1);
+        const bool mine = active && col == c;
+        if (mine) {
+            double2 a = acc.av[j], b = acc.yz[j];
+            a.x += s1;
+            a.y = fma(s3, k0.x, a.y);
+            b.x = fma(s3, k0.y, b.x);
+            b.y = fma(s3, k1.x, b.y);
+            acc.av[j] = a;
+            acc.yz[j] = b;
+        }
+        __syncwarp();
+        if (mine) {
+            double2 a = acc.av[k], b = acc.yz[k];
+            a.x += s2;
+            a.y = fma(s3, j0.x, a.y);
+            b.x = fma(s3, j0.y, b.x);
+            b.y = fma(s3, j1.x, b.y);
+            acc.av[k] = a;
+            acc.yz[k] = b;
+        }
+        __syncwarp();
+        pend &= ~__ballot_sync(0xffffffffu, mine);
+    }
 }
 
 template <class Spec>
 struct ForceTripletFast {
     const Nbh& nb;
-    SlotF sf;
-    const double* bt0;   // [NACC] beta * 2^(1-zeta)                      (this group)
-    const double* bt1;   // [NACC] beta * 2^(1-zeta) * zeta * lambda
+    SlotAcc acc;
+    const double2* bt;   // [NACC] (beta 2^(1-zeta), beta 2^(1-zeta) zeta lambda) of this group
     double etas[Spec::NETA > 0 ? Spec::NETA : 1];
-    double inv_rc;
+    double k2;
 
-    __device__ __forceinline__ void operator()(int j, int k, bool active) {
+    __device__ __forceinline__ void operator()(int j, int k, int col, bool active) {
         const double2 j0 = nb.p0[j], j1 = nb.p1[j], j2 = nb.p2[j];
-        const double2 k0 = nb.p0[k], k1 = nb.p1[k], k2 = nb.p2[k];
+        const double2 k0 = nb.p0[k], k1 = nb.p1[k], kk2 = nb.p2[k];
         const double wx = k0.x - j0.x, wy = k0.y - j0.y, wz = k1.x - j1.x;
-        const double c2 = wx * wx + wy * wy + wz * wz;
-        const double ic = rsqrt(c2);
-        const double c = c2 * ic;
-        double sn, cs;
-        sincospi(c * inv_rc, &sn, &cs);
-        double fcc = 0.5 * cs + 0.5;
-        double dfc = (-0.5 * PI_D * inv_rc) * sn * ic;          // fc'(c)/c
+        const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
+        double Cc, Sc;
+        cos_sinc(c2 * k2, Cc, Sc);
+        double fcc = Cc * Cc;                       // fc(c)
+        double dfc = (-2.0 * k2) * (Cc * Sc);       // fc'(c)/c
         if (!active) { fcc = 0.0; dfc = 0.0; }
         double Ec[Spec::NETA];
         eta_chain<Spec>(c2, etas[0], Ec);
-        const double cosv = (j0.x * k0.x + j0.y * k0.y + j1.x * k1.x) * (j1.y * k1.y);
+        const double iab = j1.y * k1.y;
+        const double cosv = fma(j0.x, k0.x, fma(j0.y, k0.y, j1.x * k1.x)) * iab;
         // pw[l][b] = (1 +- cos)^(2^b) ; pd[l][b] = (1 +- cos)^(2^b - 1)
         double pw[2][Spec::MAXBIT + 1], pd[2][Spec::MAXBIT + 1];
         pw[0][0] = 1.0 + cosv; pw[1][0] = 1.0 - cosv;
@@ -114,41 +138,41 @@ struct ForceTripletFast {
 #pragma unroll
                 for (int l = 0; l < 2; ++l)
                     if (Spec::mask(e) >> (8 * l + b) & 1u) {
-                        const int a = acc_index<Spec>(e, 8 * l + b);
-                        T0 = fma(bt0[a], pw[l][b], T0);
-                        T1 = fma(bt1[a], pd[l][b], T1);
+                        const double2 c = bt[acc_index<Spec>(e, 8 * l + b)];
+                        T0 = fma(c.x, pw[l][b], T0);
+                        T1 = fma(c.y, pd[l][b], T1);
                     }
             }
             const double Y = (nb.pe[j * Spec::NETA + e] * nb.pe[k * Spec::NETA + e]) * Ec[e];
-            Z0 = fma(T0, Y, Z0);
+            const double A = T0 * Y;
+            Z0 += A;
             Z1 = fma(T1, Y, Z1);
-            Z2 = fma(etas[e] * T0, Y, Z2);
+            Z2 = fma(etas[e], A, Z2);
         }
-        triplet_forces(j0, j1, j2, k0, k1, k2, fcc, dfc, cosv, Z0, Z1, Z2, sf, j, k, active);
+        triplet_forces(j0, j1, j2, k0, k1, kk2, fcc, dfc, cosv, iab, Z0, Z1, Z2, acc, j, k, col, active);
     }
 };
 
 struct ForceTripletGeneric {
     const Nbh& nb;
-    SlotF sf;
+    SlotAcc acc;
     const AngularSF* list;
     int nsf;
     const double* brow;   // beta row of the centre (shared memory)
-    double inv_rc;
+    double k2;
 
-    __device__ __forceinline__ void operator()(int j, int k, bool active) {
+    __device__ __forceinline__ void operator()(int j, int k, int col, bool active) {
         const double2 j0 = nb.p0[j], j1 = nb.p1[j], j2 = nb.p2[j];
-        const double2 k0 = nb.p0[k], k1 = nb.p1[k], k2 = nb.p2[k];
+        const double2 k0 = nb.p0[k], k1 = nb.p1[k], kk2 = nb.p2[k];
         const double wx = k0.x - j0.x, wy = k0.y - j0.y, wz = k1.x - j1.x;
-        const double c2 = wx * wx + wy * wy + wz * wz;
-        const double ic = rsqrt(c2);
-        const double c = c2 * ic;
-        double sn, cs;
-        sincospi(c * inv_rc, &sn, &cs);
-        double fcc = 0.5 * cs + 0.5;
-        double dfc = (-0.5 * PI_D * inv_rc) * sn * ic;
+        const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
+        double Cc, Sc;
+        cos_sinc(c2 * k2, Cc, Sc);
+        double fcc = Cc * Cc;
+        double dfc = (-2.0 * k2) * (Cc * Sc);
         if (!active) { fcc = 0.0; dfc = 0.0; }
-        const double cosv = (j0.x * k0.x + j0.y * k0.y + j1.x * k1.x) * (j1.y * k1.y);
+        const double iab = j1.y * k1.y;
+        const double cosv = fma(j0.x, k0.x, fma(j0.y, k0.y, j1.x * k1.x)) * iab;
         const double a2 = 1.0 / (j1.y * j1.y), b2 = 1.0 / (k1.y * k1.y);
         const double r2sum = a2 + b2 + c2;
         double Z0 = 0.0, Z1 = 0.0, Z2 = 0.0;
@@ -168,7 +192,7 @@ struct ForceTripletGeneric {
             Z1 = fma(bc * (double)(f.izeta * f.lam) * pd, Y, Z1);
             Z2 = fma(f.eta * bc * pwv, Y, Z2);
         }
-        triplet_forces(j0, j1, j2, k0, k1, k2, fcc, dfc, cosv, Z0, Z1, Z2, sf, j, k, active);
+        triplet_forces(j0, j1, j2, k0, k1, kk2, fcc, dfc, cosv, iab, Z0, Z1, Z2, acc, j, k, col, active);
     }
 };
 
@@ -189,16 +213,15 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
     nb.p0 = reinterpret_cast<double2*>(base);
     nb.p1 = nb.p0 + p.cap;
     nb.p2 = nb.p1 + p.cap;
-    nb.pe = reinterpret_cast<double*>(nb.p2 + p.cap);
-    SlotF sf;
-    sf.x = nb.pe + (size_t)p.cap * Spec::NETA;
-    sf.y = sf.x + p.cap;
-    sf.z = sf.y + p.cap;
-    double* brow = sf.z + p.cap;
-    double* bt0 = brow + p.g_stride;
-    double* bt1 = bt0 + Spec::NACC;
+    SlotAcc acc;
+    acc.av = nb.p2 + p.cap;
+    acc.yz = acc.av + p.cap;
+    double2* bt = acc.yz + p.cap;
+    nb.pe = reinterpret_cast<double*>(bt + Spec::NACC);
+    double* brow = nb.pe + (size_t)p.cap * Spec::NETA;
     PairQueue Q;
-    Q.q = reinterpret_cast<uint16_t*>(bt1 + Spec::NACC);
+    Q.q = reinterpret_cast<uint32_t*>(brow + p.g_stride);
+    Q.head = 0;
     Q.n = 0;
 
     int seg[MAX_ELEM + 1];
@@ -210,7 +233,7 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
     for (int s = lane; s < p.g_stride; s += 32) brow[s] = p.dEdG[(size_t)i * p.g_stride + s];
     __syncwarp();
 
-    // ---- stage the neighbourhood; radial forces go straight into the slot accumulators ----------
+    // ---- stage the neighbourhood; the radial force  F_j = -R u  seeds the scalar accumulator A ---
     const double xi = p.sx[i], yi = p.sy[i], zi = p.sz[i];
     const int32_t* row = p.nbr + (size_t)i * p.stride;
     double eta0 = 0.0;
@@ -222,33 +245,32 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
             const double dx = min_image_1d(xi, p.sx[j], p.box[0], p.half[0]);
             const double dy = min_image_1d(yi, p.sy[j], p.box[1], p.half[1]);
             const double dz = min_image_1d(zi, p.sz[j], p.box[2], p.half[2]);
-            const double a2 = dx * dx + dy * dy + dz * dz;
+            const double a2 = fma(dx, dx, fma(dy, dy, dz * dz));
             const double ia = rsqrt(a2);
             const double a = a2 * ia;
-            double sn, cs;
-            sincospi(a * p.inv_rc, &sn, &cs);
-            const double fa = 0.5 * cs + 0.5;
-            const double dfa_r = (-0.5 * PI_D * p.inv_rc) * sn;   // fc'(a)
+            double Ca, Sa;
+            cos_sinc(a2 * p.k2, Ca, Sa);
+            const double fa = Ca * Ca;                          // fc(a)
+            const double dfa_a = (-2.0 * p.k2) * (Ca * Sa);     // fc'(a)/a
             nb.p0[m] = make_double2(dx, dy);
             nb.p1[m] = make_double2(dz, ia);
-            nb.p2[m] = make_double2(fa, dfa_r * ia);
+            nb.p2[m] = make_double2(fa, dfa_a);
             if constexpr (Spec::NETA > 0) {
                 double E[Spec::NETA];
                 eta_chain<Spec>(a2, eta0, E);
 #pragma unroll
                 for (int q = 0; q < Spec::NETA; ++q) nb.pe[m * Spec::NETA + q] = E[q];
             }
-            // R = sum_r beta_r exp(-eta d^2) (fc' - 2 eta d fc) / a ;  F_j = -R u
+            // R = sum_r beta_r exp(-eta d^2) (fc'(a) - 2 eta d fc(a)) / a,  d = a - rs
             double R = 0.0;
             for (int r = 0; r < nr; ++r) {
                 const RadialSF f = prog->rad[off + r];
                 const double d = a - f.rs;
-                R = fma(brow[f.g] * exp(-f.eta * d * d), dfa_r - 2.0 * f.eta * d * fa, R);
+                const double ex = exp_small(fmax(-f.eta * d * d, -700.0));
+                R = fma(brow[f.g] * ex, fma(-2.0 * f.eta * d, fa * ia, dfa_a), R);
             }
-            R *= ia;
-            sf.x[m] = -R * dx;
-            sf.y[m] = -R * dy;
-            sf.z[m] = -R * dz;
+            acc.av[m] = make_double2(R, 0.0);
+            acc.yz[m] = make_double2(0.0, 0.0);
         }
     }
     __syncwarp();
@@ -260,7 +282,7 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
             const int na = prog->n_ang[pr];
             if (na == 0) continue;
             if constexpr (Spec::ID != ANG_GENERIC) {
-                // coefficient tables of this group
+                // coefficient table of this group
                 if (lane < 16) {
 #pragma unroll
                     for (int e = 0; e < Spec::NETA; ++e) {
@@ -275,20 +297,19 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
                                 if (ee < e) a += __popc(mk);
                                 else if (ee == e) a += __popc(mk & ((1u << lane) - 1u));
                             }
-                            bt0[a] = bc;
-                            bt1[a] = bc * (double)zeta * lam;
+                            bt[a] = make_double2(bc, bc * (double)zeta * lam);
                         }
                     }
                 }
                 __syncwarp();
-                ForceTripletFast<Spec> f{nb, sf, bt0, bt1, {}, p.inv_rc};
+                ForceTripletFast<Spec> f{nb, acc, bt, {}, p.k2};
 #pragma unroll
                 for (int e = 0; e < Spec::NETA; ++e) f.etas[e] = prog->ang_eta[e];
                 if (e1 == e2) enum_within(nb, seg[e1], seg[e1 + 1] - seg[e1], p.rc2, Q, lane, f);
                 else enum_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], p.rc2, Q, lane, f);
                 drain_tail(Q, lane, f);
             } else {
-                ForceTripletGeneric f{nb, sf, prog->ang + prog->ang_off[pr], na, brow, p.inv_rc};
+                ForceTripletGeneric f{nb, acc, prog->ang + prog->ang_off[pr], na, brow, p.k2};
                 if (e1 == e2) enum_within(nb, seg[e1], seg[e1 + 1] - seg[e1], p.rc2, Q, lane, f);
                 else enum_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], p.rc2, Q, lane, f);
                 drain_tail(Q, lane, f);
@@ -296,11 +317,13 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
         }
     __syncwarp();
 
-    // ---- flush: one global FP64 atomic per neighbour component; the centre gets minus the sum ----
+    // ---- flush: F_slot = V - A u; one global FP64 RED per component; the centre gets minus the sum
     double fx = 0.0, fy = 0.0, fz = 0.0;
     for (int m = lane; m < ntot; m += 32) {
         const int j = row[m];
-        const double ax = sf.x[m], ay = sf.y[m], az = sf.z[m];
+        const double2 u0 = nb.p0[m], av = acc.av[m], yz = acc.yz[m];
+        const double uz = nb.p1[m].x;
+        const double ax = fma(-av.x, u0.x, av.y), ay = fma(-av.x, u0.y, yz.x), az = fma(-av.x, uz, yz.y);
         atomicAdd(&p.f_sorted[3 * (size_t)j + 0], ax);
         atomicAdd(&p.f_sorted[3 * (size_t)j + 1], ay);
         atomicAdd(&p.f_sorted[3 * (size_t)j + 2], az);
@@ -340,7 +363,7 @@ int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const
     if (n == 0) return 0;
     ForceParams p;
     p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride;
-    p.rc = rc; p.rc2 = rc * rc; p.inv_rc = 1.0 / rc;
+    p.rc = rc; p.rc2 = rc * rc; p.inv_rc = 1.0 / rc; p.k2 = (PI_D / (2.0 * rc)) * (PI_D / (2.0 * rc));
     for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.dEdG = w.dEdG; p.f_sorted = w.f_sorted;

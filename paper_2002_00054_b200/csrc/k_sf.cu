@@ -15,7 +15,7 @@ constexpr int SF_WARPS = 4;
 struct SfParams {
     int64_t n;
     int n_elem, ncell, stride, cap, g_stride;
-    double rc, rc2, inv_rc;
+    double rc, rc2, inv_rc, k2;          // k2 = (pi / (2 rc))^2
     double box[3], half[3];
     const double *sx, *sy, *sz;
     const int32_t *cell_start, *nbr, *nbr_cnt;
@@ -26,33 +26,33 @@ struct SfParams {
 
 template <class Spec>
 __host__ __device__ constexpr size_t sf_warp_smem(int cap) {
-    // p0, p1, p2 (double2 each) + pe (NETA doubles) per slot, queue (64 x u16), generic accumulators
-    return (size_t)cap * (48 + 8 * Spec::NETA) + 128 + (Spec::ID == ANG_GENERIC ? 64 * 8 : 0);
+    // p0, p1, p2 (double2 each) + pe (NETA doubles) per slot, queue (64 x u32), generic accumulators
+    return (size_t)cap * (48 + 8 * Spec::NETA) + 256 + (Spec::ID == ANG_GENERIC ? 64 * 8 : 0);
 }
 
 // ---- per-triplet work, specialised groups -------------------------------------------------
 template <class Spec>
 struct SfTripletFast {
     const Nbh& nb;
-    double eta0, inv_rc;
+    double eta0, k2;
     double acc[Spec::NACC > 0 ? Spec::NACC : 1];
 
-    __device__ __forceinline__ SfTripletFast(const Nbh& nb_, double eta0_, double inv_rc_)
-        : nb(nb_), eta0(eta0_), inv_rc(inv_rc_) {
+    __device__ __forceinline__ SfTripletFast(const Nbh& nb_, double eta0_, double k2_)
+        : nb(nb_), eta0(eta0_), k2(k2_) {
 #pragma unroll
         for (int a = 0; a < Spec::NACC; ++a) acc[a] = 0.0;
     }
 
-    __device__ __forceinline__ void operator()(int j, int k, bool active) {
+    __device__ __forceinline__ void operator()(int j, int k, int, bool active) {
         const double2 j0 = nb.p0[j], j1 = nb.p1[j], k0 = nb.p0[k], k1 = nb.p1[k];
         const double wx = k0.x - j0.x, wy = k0.y - j0.y, wz = k1.x - j1.x;
-        const double c2 = wx * wx + wy * wy + wz * wz;
-        const double c = sqrt(c2);
-        double fcc = 0.5 * cospi(c * inv_rc) + 0.5;
+        const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
+        const double Cc = cos_only(c2 * k2);
+        double fcc = Cc * Cc;                       // fc(c) = cos^2(pi c / (2 rc))
         if (!active) fcc = 0.0;
         double Ec[Spec::NETA];
         eta_chain<Spec>(c2, eta0, Ec);
-        const double cosv = (j0.x * k0.x + j0.y * k0.y + j1.x * k1.x) * (j1.y * k1.y);
+        const double cosv = fma(j0.x, k0.x, fma(j0.y, k0.y, j1.x * k1.x)) * (j1.y * k1.y);
         double pw[2][Spec::MAXBIT + 1];
         pw[0][0] = 1.0 + cosv;
         pw[1][0] = 1.0 - cosv;
@@ -79,20 +79,20 @@ struct SfTripletGeneric {
     const Nbh& nb;
     const AngularSF* sf;
     int nsf;
-    double inv_rc;
+    double k2;
     double* gacc;     // [64] per warp, shared memory
     int lane;
 
-    __device__ __forceinline__ void operator()(int j, int k, bool active) {
+    __device__ __forceinline__ void operator()(int j, int k, int, bool active) {
         const double2 j0 = nb.p0[j], j1 = nb.p1[j], j2 = nb.p2[j];
-        const double2 k0 = nb.p0[k], k1 = nb.p1[k], k2 = nb.p2[k];
+        const double2 k0 = nb.p0[k], k1 = nb.p1[k], kq = nb.p2[k];
         const double wx = k0.x - j0.x, wy = k0.y - j0.y, wz = k1.x - j1.x;
-        const double c2 = wx * wx + wy * wy + wz * wz;
-        const double c = sqrt(c2);
-        double C = j2.x * k2.x * (0.5 * cospi(c * inv_rc) + 0.5);
+        const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
+        const double Cc = cos_only(c2 * k2);
+        double C = j2.x * kq.x * (Cc * Cc);
         if (!active) C = 0.0;
         const double cosv = (j0.x * k0.x + j0.y * k0.y + j1.x * k1.x) * (j1.y * k1.y);
-        const double r2sum = j2.y * j2.y + k2.y * k2.y + c2;
+        const double r2sum = j2.y * j2.y + kq.y * kq.y + c2;
         for (int s = 0; s < nsf; ++s) {
             const AngularSF f = sf[s];
             const double base = 1.0 + (double)f.lam * cosv;
@@ -128,7 +128,8 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
     nb.p2 = nb.p1 + p.cap;
     nb.pe = reinterpret_cast<double*>(nb.p2 + p.cap);
     PairQueue Q;
-    Q.q = reinterpret_cast<uint16_t*>(nb.pe + (size_t)p.cap * Spec::NETA);
+    Q.q = reinterpret_cast<uint32_t*>(nb.pe + (size_t)p.cap * Spec::NETA);
+    Q.head = 0;
     Q.n = 0;
     double* gacc = reinterpret_cast<double*>(Q.q + 64);
 
@@ -149,10 +150,11 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
         const double dx = min_image_1d(xi, p.sx[j], p.box[0], p.half[0]);
         const double dy = min_image_1d(yi, p.sy[j], p.box[1], p.half[1]);
         const double dz = min_image_1d(zi, p.sz[j], p.box[2], p.half[2]);
-        const double a2 = dx * dx + dy * dy + dz * dz;
-        const double a = sqrt(a2);
-        const double ia = 1.0 / a;
-        const double fa = 0.5 * cospi(a * p.inv_rc) + 0.5;
+        const double a2 = fma(dx, dx, fma(dy, dy, dz * dz));
+        const double ia = rsqrt(a2);
+        const double a = a2 * ia;
+        const double Ca = cos_only(a2 * p.k2);
+        const double fa = Ca * Ca;                  // fc(a)
         nb.p0[m] = make_double2(dx, dy);
         nb.p1[m] = make_double2(dz, ia);
         nb.p2[m] = make_double2(fa, a);
@@ -177,7 +179,7 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
             for (int m = seg[e] + lane; m < seg[e + 1]; m += 32) {
                 const double2 q = nb.p2[m];
                 const double d = q.y - f.rs;
-                acc = fma(exp(-f.eta * d * d), q.x, acc);
+                acc = fma(exp_small(fmax(-f.eta * d * d, -700.0)), q.x, acc);
             }
             acc = warp_sum(acc);
             if (lane == 0) Grow[f.g] = acc;
@@ -191,7 +193,7 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
             const int na = prog->n_ang[pr];
             if (na == 0) continue;
             if constexpr (Spec::ID != ANG_GENERIC) {
-                SfTripletFast<Spec> f(nb, eta0, p.inv_rc);
+                SfTripletFast<Spec> f(nb, eta0, p.k2);
                 if (e1 == e2) enum_within(nb, seg[e1], seg[e1 + 1] - seg[e1], p.rc2, Q, lane, f);
                 else enum_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], p.rc2, Q, lane, f);
                 drain_tail(Q, lane, f);
@@ -209,7 +211,7 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
             } else {
                 for (int s = lane; s < na; s += 32) gacc[s] = 0.0;
                 __syncwarp();
-                SfTripletGeneric f{nb, prog->ang + prog->ang_off[pr], na, p.inv_rc, gacc, lane};
+                SfTripletGeneric f{nb, prog->ang + prog->ang_off[pr], na, p.k2, gacc, lane};
                 if (e1 == e2) enum_within(nb, seg[e1], seg[e1 + 1] - seg[e1], p.rc2, Q, lane, f);
                 else enum_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], p.rc2, Q, lane, f);
                 drain_tail(Q, lane, f);
@@ -246,6 +248,7 @@ int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const El
     SfParams p;
     p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride;
     p.rc = rc; p.rc2 = rc * rc; p.inv_rc = 1.0 / rc;
+    p.k2 = (3.14159265358979323846 / (2.0 * rc)) * (3.14159265358979323846 / (2.0 * rc));
     for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.G = w.G;

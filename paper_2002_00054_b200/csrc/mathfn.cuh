@@ -1,0 +1,53 @@
+// mathfn.cuh -- the CUDA path's own FP64 special functions for the symmetry-function kernels.
+//
+// Why not libdevice exp / sincospi / sqrt here: ncu (profiles/r1_*) shows the hot loops are
+// issue-bound, not FP64-pipe bound, and ~25 % of the issued instructions were UMOV / IMAD.MOV
+// pairs materialising libdevice's 64-bit polynomial constants as immediates plus the
+// BSSY/BSYNC/FSEL scaffolding of its special-case paths.  Here the coefficients live in the
+// constant bank (DFMA takes c[bank][offset] operands directly), arguments are known to be
+// in range, and the cosine cutoff is evaluated as a function of c^2 -- no sqrt, no rsqrt, no
+// sincospi per triplet:
+//     z = (pi c / (2 rc))^2 ,  C = cos(sqrt z) ,  S = sin(sqrt z)/sqrt z     (entire in z)
+//     fc(c)    = (cos(pi c / rc) + 1)/2 = C^2
+//     fc'(c)/c = -2 (pi/(2 rc))^2 C S
+// Coefficients: coeffs.inc, written by gen_coeffs.py (Chebyshev-node fits, errors < 6e-17).
+#pragma once
+
+namespace nnp {
+
+#include "coeffs.inc"
+
+// exp(y) for y in [-700, 0.35]  (callers guarantee the range; no overflow / denormal handling).
+__device__ __forceinline__ double exp_small(double y) {
+    const double MAGIC = 6755399441055744.0;                 // 1.5 * 2^52: round-to-nearest-integer trick
+    const double t = fma(y, 1.4426950408889634, MAGIC);      // y * log2(e)
+    const int k = __double2loint(t);
+    const double kf = t - MAGIC;
+    double r = fma(kf, -6.93147180369123816490e-01, y);      // ln2 hi
+    r = fma(kf, -1.90821492927058770002e-10, r);             // ln2 lo
+    double p = EXPC[11];
+#pragma unroll
+    for (int q = 10; q >= 0; --q) p = fma(p, r, EXPC[q]);
+    return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
+}
+
+// C = cos(sqrt z), S = sin(sqrt z)/sqrt z for z in [0, (pi/2)^2]
+__device__ __forceinline__ void cos_sinc(double z, double& C, double& S) {
+    double c = COSC[8], s = SNCC[8];
+#pragma unroll
+    for (int q = 7; q >= 0; --q) {
+        c = fma(c, z, COSC[q]);
+        s = fma(s, z, SNCC[q]);
+    }
+    C = c;
+    S = s;
+}
+
+__device__ __forceinline__ double cos_only(double z) {
+    double c = COSC[8];
+#pragma unroll
+    for (int q = 7; q >= 0; --q) c = fma(c, z, COSC[q]);
+    return c;
+}
+
+}  // namespace nnp

@@ -251,8 +251,13 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
         bool any_ang = ao > 0;
         P.variant = ANG_GENERIC;
         if (any_ang) {
-            if (match_spec<SpecBase12>(ang[c], &P)) P.variant = ANG_BASE12;
-            else if (match_spec<SpecWide32>(ang[c], &P)) P.variant = ANG_WIDE32;
+            // the specialised kernels use exp_small() unclamped: its argument -eta (a^2+b^2+c^2) must stay > -700
+            double eta_max = 0.0;
+            for (int p = 0; p < npair; ++p)
+                for (const auto& f : ang[c][p]) eta_max = std::fmax(eta_max, f.eta);
+            const bool in_range = eta_max * 3.0 * rc * rc <= 700.0;
+            if (in_range && match_spec<SpecBase12>(ang[c], &P)) P.variant = ANG_BASE12;
+            else if (in_range && match_spec<SpecWide32>(ang[c], &P)) P.variant = ANG_WIDE32;
             else {
                 for (int p = 0; p < npair; ++p)
                     if (P.n_ang[p] > 64)
@@ -404,6 +409,13 @@ extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d
         if (m->timing) cudaEventRecord(m->ev[k], st);
     };
     int launches = 0;
+    if (n_atoms == 0) {   // nothing to launch: E = 0
+        NNP_CUDA(m, cudaMemsetAsync(d_e_total, 0, sizeof(double), st));
+        NNP_CUDA(m, cudaMemsetAsync(w.status, 0, sizeof(int32_t) * 4, st));
+        m->timing_valid = false;
+        m->ws = w; m->have_ws = true; m->last_n = 0; m->last_stream = st; m->last_launches = 0;
+        return NNP_OK;
+    }
     mark(0);
     launches += launch_sort(w, g, n_atoms, m->n_elem, d_pos, d_type, st);
     mark(1);
