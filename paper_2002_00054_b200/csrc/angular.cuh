@@ -88,103 +88,124 @@ __device__ __forceinline__ double warp_sum(double v) {
 
 // ---------------------------------------------------------------- per-warp neighbourhood in smem
 // Slot m (0..n-1) of the centre's neighbour row, grouped by element.  Packed as double2 so the
-// per-triplet gathers are 128-bit shared loads.
+// per-triplet gathers are 128-bit shared loads.  A second, FP32 copy of the min-image vectors
+// feeds the candidate screening (below): 12 B per slot instead of 24 B, FP32 pipe instead of FP64.
 struct Nbh {
     double2* p0;   // (ux, uy)
     double2* p1;   // (uz, 1/a)
-    double2* p2;   // (fc(a), a) in the SF kernel; (fc(a), fc'(a)/a) in the force kernel
+    double2* p2;   // SF kernel: (exp(-eta_0 a^2), fc(a));  force kernel: (fc(a), fc'(a)/a)
                    // fc(a) = C^2, fc'(a)/a = -2 k2 C S with z = k2 a^2, k2 = (pi/(2 rc))^2 (mathfn.cuh)
-    double* pe;    // [slot * NETA + e]: SF kernel: exp(-eta_e a^2) * fc(a); force kernel: exp(-eta_e a^2)
+    double2* p3;   // force kernel only: (exp(-eta_0 a^2), unused)
+    float2* fxy;   // (float ux, float uy)
+    float* fz;     // float uz
 };
 
 // ---------------------------------------------------------------- triplet enumeration
-// Calls f(j, k, colour, active) for batches of 32 contributing pairs (c^2 < rc2).
+// Calls f(j, k, colour, active) for batches of 32 candidate pairs that passed the SCREEN
+//     |u_k - u_j|^2 < rc^2 (1 + 1e-5)      evaluated in FP32 on the FP32 copies
+// (FP32 error of that expression is < 1e-6 rc^2, so no contributing pair is ever dropped); the
+// functor applies the exact FP64 test c^2 < rc^2 itself and zeroes fc(c) otherwise.  ncu on the first
+// version (profiles/r1_k_force_k_sf_summary.md) showed the FP64 pair test with four shared loads per
+// candidate to be 35 % of the instructions and 20 % of the shared-memory wavefronts of k_force.
 //
-// Pairs are enumerated in ROUNDS; inside one round every slot appears at most once as j and at
-// most once as k (within a segment: round r pairs slot j with (j + r) mod ns -- the "tournament"
-// order; between two segments: round r pairs slot s of the smaller segment with slot (s + r) mod
-// n_big of the bigger one).  The round number travels with the pair through the compaction queue
-// as its COLOUR: entries of equal colour never share a j or a k, which lets the force kernel
-// accumulate per-slot forces with plain shared-memory read-modify-writes, one colour at a time,
-// instead of FP64 shared atomics (CAS loops -- ncu showed them to be >35 % of the stall samples).
-// The queue is a 64-entry FIFO ring per warp, so a batch holds 2-4 consecutive colours.
+// Pairs are visited in ROUNDS flattened into one index p so that all 32 lanes stay busy: within
+// a segment of ns slots, p = (r-1) ns + j pairs slot j with slot (j + r) mod ns, r = 1..ns/2 (the
+// last round of an even ns is half) -- inside one round every slot appears at most once as j and
+// at most once as k.  Between two segments, p = r n_small + s pairs slot s of the smaller segment
+// with slot (s + r) mod n_big of the bigger one.  The round number travels with the pair through
+// the compaction queue as its COLOUR: entries of equal colour never share a j or a k, which lets
+// the force kernel accumulate per-slot forces with plain shared-memory read-modify-writes, one
+// colour at a time, instead of FP64 shared atomics (CAS loops).  The queue is a 64-entry FIFO
+// ring per warp.
 struct PairQueue {
     uint32_t* q;    // [64] (colour << 16) | (j << 8) | k
     int head, n;
 };
 
-template <class F>
-__device__ __forceinline__ void push_and_drain(PairQueue& Q, bool pass, int j, int k, int col, int lane, F& f) {
+__device__ __forceinline__ void q_push(PairQueue& Q, bool pass, int j, int k, int col, int lane) {
     const unsigned m = __ballot_sync(0xffffffffu, pass);
     if (pass) Q.q[(Q.head + Q.n + __popc(m & ((1u << lane) - 1u))) & 63] = ((unsigned)col << 16) | (unsigned)((j << 8) | k);
     Q.n += __popc(m);
     __syncwarp();
-    if (Q.n >= 32) {
-        const unsigned e = Q.q[(Q.head + lane) & 63];
-        Q.head = (Q.head + 32) & 63;
-        Q.n -= 32;
-        __syncwarp();
-        f((int)((e >> 8) & 255u), (int)(e & 255u), (int)(e >> 16), true);
-    }
 }
 
+// pop min(32, n) entries (n >= 1) and hand them to f; idle lanes replay entry 0 with active = false
 template <class F>
-__device__ __forceinline__ void drain_tail(PairQueue& Q, int lane, F& f) {
-    if (Q.n > 0) {
-        const bool act = lane < Q.n;
-        const unsigned e = Q.q[(Q.head + (act ? lane : 0)) & 63];
-        Q.n = 0;
-        Q.head = 0;
-        __syncwarp();
-        f((int)((e >> 8) & 255u), (int)(e & 255u), (int)(e >> 16), act);
-    }
+__device__ __forceinline__ void q_pop(PairQueue& Q, int lane, F& f) {
+    const int cnt = Q.n < 32 ? Q.n : 32;
+    const bool act = lane < cnt;
+    const unsigned e = Q.q[(Q.head + (act ? lane : 0)) & 63];
+    Q.head = (Q.head + cnt) & 63;
+    Q.n -= cnt;
     __syncwarp();
+    f((int)((e >> 8) & 255u), (int)(e & 255u), (int)(e >> 16), act);
 }
 
-__device__ __forceinline__ bool pair_close(const Nbh& nb, int j, int k, double rc2) {
-    const double2 a0 = nb.p0[j], b0 = nb.p0[k];
-    const double az = nb.p1[j].x, bz = nb.p1[k].x;
-    const double wx = b0.x - a0.x, wy = b0.y - a0.y, wz = bz - az;
-    return wx * wx + wy * wy + wz * wz < rc2;
+__device__ __forceinline__ bool pair_close32(const Nbh& nb, int j, int k, float rc2f) {
+    const float2 a = nb.fxy[j], b = nb.fxy[k];
+    const float wx = b.x - a.x, wy = b.y - a.y, wz = nb.fz[k] - nb.fz[j];
+    return fmaf(wx, wx, fmaf(wy, wy, wz * wz)) < rc2f;
 }
 
-// all unordered pairs inside segment [s, s+ns); colours 1..ns/2
+// all unordered pairs inside segment [s, s+ns); colours 1..ns/2; the queue is empty on return
 template <class F>
-__device__ __forceinline__ void enum_within(const Nbh& nb, int s, int ns, double rc2, PairQueue& Q, int lane, F& f) {
-    const int rounds = ns / 2;                 // r = 1..rounds; for even ns the last round is half
-    for (int r = 1; r <= rounds; ++r) {
-        const int lim = (2 * r == ns) ? ns / 2 : ns;
-        for (int j0 = 0; j0 < lim; j0 += 32) {
-            const int jj = j0 + lane;
+__device__ __forceinline__ void pairs_within(const Nbh& nb, int s, int ns, float rc2f, PairQueue& Q, int lane, F& f) {
+    const int P = ns * (ns - 1) / 2;
+    if (P <= 0) return;
+    int jj = lane, r = 1;
+    while (jj >= ns) { jj -= ns; ++r; }
+    int p0 = 0;
+    while (true) {
+        if (p0 < P) {
+            bool pass = false;
             int kk = jj + r;
-            if (kk >= ns) kk -= ns;
-            const bool valid = jj < lim;
-            const bool pass = valid && pair_close(nb, s + jj, s + kk, rc2);
-            push_and_drain(Q, pass, s + jj, s + kk, r, lane, f);
+            if (p0 + lane < P) {                    // r <= ns/2 here, so one wrap is enough
+                if (kk >= ns) kk -= ns;
+                pass = pair_close32(nb, s + jj, s + kk, rc2f);
+            }
+            q_push(Q, pass, s + jj, s + kk, r, lane);
+            p0 += 32;
+            jj += 32;
+            while (jj >= ns) { jj -= ns; ++r; }
         }
+        if (Q.n >= 32 || (p0 >= P && Q.n > 0)) q_pop(Q, lane, f);
+        else if (p0 >= P) break;
     }
 }
 
 // all pairs (j in [s1, s1+n1), k in [s2, s2+n2)), disjoint segments; colours 0..max(n1,n2)-1
 template <class F>
-__device__ __forceinline__ void enum_between(const Nbh& nb, int s1, int n1, int s2, int n2, double rc2, PairQueue& Q,
-                                             int lane, F& f) {
+__device__ __forceinline__ void pairs_between(const Nbh& nb, int s1, int n1, int s2, int n2, float rc2f, PairQueue& Q,
+                                              int lane, F& f) {
     if (n1 == 0 || n2 == 0) return;
-    const bool swap = n1 < n2;                 // lanes walk the smaller segment
+    const bool swap = n1 < n2;                 // the fast index walks the smaller segment
     const int ss = swap ? s1 : s2, ns = swap ? n1 : n2;      // small
     const int sb = swap ? s2 : s1, nbig = swap ? n2 : n1;    // big
-    for (int r = 0; r < nbig; ++r) {
-        for (int q0 = 0; q0 < ns; q0 += 32) {
-            const int qs = q0 + lane;
-            int qb = qs + r;
-            if (qb >= nbig) qb -= nbig;        // qs < ns <= nbig and r < nbig: one wrap is enough
-            const bool valid = qs < ns;
-            const int j = swap ? ss + qs : sb + qb;           // j from segment 1, k from segment 2
-            const int k = swap ? sb + qb : ss + qs;
-            const bool pass = valid && pair_close(nb, j, k, rc2);
-            push_and_drain(Q, pass, j, k, r, lane, f);
+    const int P = ns * nbig;
+    int qs = lane, r = 0;
+    while (qs >= ns) { qs -= ns; ++r; }
+    int p0 = 0;
+    while (true) {
+        if (p0 < P) {
+            bool pass = false;
+            int qb = qs + r, j = 0, k = 0;
+            if (p0 + lane < P) {                    // r < nbig and qs < ns <= nbig: one wrap is enough
+                if (qb >= nbig) qb -= nbig;
+                j = swap ? ss + qs : sb + qb;       // j from segment 1, k from segment 2
+                k = swap ? sb + qb : ss + qs;
+                pass = pair_close32(nb, j, k, rc2f);
+            }
+            q_push(Q, pass, j, k, r, lane);
+            p0 += 32;
+            qs += 32;
+            while (qs >= ns) { qs -= ns; ++r; }
         }
+        if (Q.n >= 32 || (p0 >= P && Q.n > 0)) q_pop(Q, lane, f);
+        else if (p0 >= P) break;
     }
 }
+
+// screening threshold (see above)
+__device__ __forceinline__ float screen_rc2(double rc2) { return (float)(rc2 * (1.0 + 1e-5)); }
 
 }  // namespace nnp

@@ -35,12 +35,20 @@ struct ForceParams {
     int variant[MAX_ELEM];
 };
 
+// per-warp shared-memory footprint (bytes): six double2 planes (geometry, cutoff, Gaussian, two
+// accumulators), the FP32 screening copy, the coefficient tables of all pair groups, and the beta row
+// which later doubles as the 64-entry pair queue
 template <class Spec>
-__host__ __device__ constexpr size_t force_warp_smem(int cap, int g_stride) {
-    // per slot: p0,p1,p2 (48 B) + pe (8*NETA) + accumulators (A,Vx),(Vy,Vz) (32 B);
-    // queue (64 x u32); beta row; per-group coefficient table (double2 per menu entry)
-    size_t b = (size_t)cap * (48 + 8 * Spec::NETA + 32) + 256 + (size_t)g_stride * 8;
-    b += (size_t)Spec::NACC * 16;
+__host__ __device__ constexpr int bt_stride() { return Spec::NACC + 1; }   // +1: groups land on different banks
+
+template <class Spec>
+__host__ __device__ constexpr size_t force_warp_smem(int cap, int g_stride, int n_elem) {
+    const size_t capa = (size_t)((cap + 3) & ~3);
+    const size_t npair = (size_t)n_elem * (n_elem + 1) / 2;
+    size_t b = capa * (6 * 16 + 12);
+    b += npair * bt_stride<Spec>() * 16;
+    const size_t rowq = (size_t)g_stride * 8 > 256 ? (size_t)g_stride * 8 : 256;
+    b += rowq;
     return (b + 15) / 16 * 16;
 }
 
@@ -99,22 +107,31 @@ template <class Spec>
 struct ForceTripletFast {
     const Nbh& nb;
     SlotAcc acc;
-    const double2* bt;   // [NACC] (beta 2^(1-zeta), beta 2^(1-zeta) zeta lambda) of this group
-    double etas[Spec::NETA > 0 ? Spec::NETA : 1];
-    double k2;
+    const double2* bt;   // [pair group][bt_stride]: (beta 2^(1-zeta), beta 2^(1-zeta) zeta lambda)
+    double eta0, eta[Spec::NETA > 0 ? Spec::NETA : 1];
+    double k2, rc2;
+    int sg1, sg2, sg3, n_elem;     // first slot of neighbour element 1, 2, 3
 
     __device__ __forceinline__ void operator()(int j, int k, int col, bool active) {
-        const double2 j0 = nb.p0[j], j1 = nb.p1[j], j2 = nb.p2[j];
-        const double2 k0 = nb.p0[k], k1 = nb.p1[k], kk2 = nb.p2[k];
+        const double2 j0 = nb.p0[j], j1 = nb.p1[j], j2 = nb.p2[j], j3 = nb.p3[j];
+        const double2 k0 = nb.p0[k], k1 = nb.p1[k], kk2 = nb.p2[k], k3 = nb.p3[k];
+        // pair group of (element of j, element of k)
+        const int ej = (j >= sg1) + (j >= sg2) + (j >= sg3), ek = (k >= sg1) + (k >= sg2) + (k >= sg3);
+        const int ea = min(ej, ek), eb = max(ej, ek);
+        const double2* btg = bt + (ea * n_elem - (ea * (ea - 1)) / 2 + (eb - ea)) * bt_stride<Spec>();
         const double wx = k0.x - j0.x, wy = k0.y - j0.y, wz = k1.x - j1.x;
         const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
         double Cc, Sc;
         cos_sinc(c2 * k2, Cc, Sc);
         double fcc = Cc * Cc;                       // fc(c)
         double dfc = (-2.0 * k2) * (Cc * Sc);       // fc'(c)/c
-        if (!active) { fcc = 0.0; dfc = 0.0; }
-        double Ec[Spec::NETA];
-        eta_chain<Spec>(c2, etas[0], Ec);
+        if (!active || !(c2 < rc2)) { fcc = 0.0; dfc = 0.0; }   // exact cutoff (the queue was screened in FP32)
+        // Y_e = exp(-eta_e (a^2 + b^2 + c^2)): one exp, then integer powers
+        double Y[Spec::NETA];
+        Y[0] = (j3.x * k3.x) * exp_small(-eta0 * c2);
+        if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
+        if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
+        if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
         const double iab = j1.y * k1.y;
         const double cosv = fma(j0.x, k0.x, fma(j0.y, k0.y, j1.x * k1.x)) * iab;
         // pw[l][b] = (1 +- cos)^(2^b) ; pd[l][b] = (1 +- cos)^(2^b - 1)
@@ -138,16 +155,15 @@ struct ForceTripletFast {
 #pragma unroll
                 for (int l = 0; l < 2; ++l)
                     if (Spec::mask(e) >> (8 * l + b) & 1u) {
-                        const double2 c = bt[acc_index<Spec>(e, 8 * l + b)];
+                        const double2 c = btg[acc_index<Spec>(e, 8 * l + b)];
                         T0 = fma(c.x, pw[l][b], T0);
                         T1 = fma(c.y, pd[l][b], T1);
                     }
             }
-            const double Y = (nb.pe[j * Spec::NETA + e] * nb.pe[k * Spec::NETA + e]) * Ec[e];
-            const double A = T0 * Y;
+            const double A = T0 * Y[e];
             Z0 += A;
-            Z1 = fma(T1, Y, Z1);
-            Z2 = fma(etas[e], A, Z2);
+            Z1 = fma(T1, Y[e], Z1);
+            Z2 = fma(eta[e], A, Z2);
         }
         triplet_forces(j0, j1, j2, k0, k1, kk2, fcc, dfc, cosv, iab, Z0, Z1, Z2, acc, j, k, col, active);
     }
@@ -159,7 +175,7 @@ struct ForceTripletGeneric {
     const AngularSF* list;
     int nsf;
     const double* brow;   // beta row of the centre (shared memory)
-    double k2;
+    double k2, rc2;
 
     __device__ __forceinline__ void operator()(int j, int k, int col, bool active) {
         const double2 j0 = nb.p0[j], j1 = nb.p1[j], j2 = nb.p2[j];
@@ -170,7 +186,7 @@ struct ForceTripletGeneric {
         cos_sinc(c2 * k2, Cc, Sc);
         double fcc = Cc * Cc;
         double dfc = (-2.0 * k2) * (Cc * Sc);
-        if (!active) { fcc = 0.0; dfc = 0.0; }
+        if (!active || !(c2 < rc2)) { fcc = 0.0; dfc = 0.0; }
         const double iab = j1.y * k1.y;
         const double cosv = fma(j0.x, k0.x, fma(j0.y, k0.y, j1.x * k1.x)) * iab;
         const double a2 = 1.0 / (j1.y * j1.y), b2 = 1.0 / (k1.y * k1.y);
@@ -208,19 +224,23 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
     if (p.variant[tc] != Spec::ID) return;
     const ElemProgram* __restrict__ prog = p.prog[tc];
 
-    unsigned char* base = smem_raw + (size_t)wid * force_warp_smem<Spec>(p.cap, p.g_stride);
+    const int capa = (p.cap + 3) & ~3;
+    const int npair = p.n_elem * (p.n_elem + 1) / 2;
+    unsigned char* base = smem_raw + (size_t)wid * force_warp_smem<Spec>(p.cap, p.g_stride, p.n_elem);
     Nbh nb;
     nb.p0 = reinterpret_cast<double2*>(base);
-    nb.p1 = nb.p0 + p.cap;
-    nb.p2 = nb.p1 + p.cap;
+    nb.p1 = nb.p0 + capa;
+    nb.p2 = nb.p1 + capa;
+    nb.p3 = nb.p2 + capa;
     SlotAcc acc;
-    acc.av = nb.p2 + p.cap;
-    acc.yz = acc.av + p.cap;
-    double2* bt = acc.yz + p.cap;
-    nb.pe = reinterpret_cast<double*>(bt + Spec::NACC);
-    double* brow = nb.pe + (size_t)p.cap * Spec::NETA;
+    acc.av = nb.p3 + capa;
+    acc.yz = acc.av + capa;
+    double2* bt = acc.yz + capa;
+    nb.fxy = reinterpret_cast<float2*>(bt + npair * bt_stride<Spec>());
+    nb.fz = reinterpret_cast<float*>(nb.fxy + capa);
+    double* brow = reinterpret_cast<double*>(nb.fz + capa);
     PairQueue Q;
-    Q.q = reinterpret_cast<uint32_t*>(brow + p.g_stride);
+    Q.q = reinterpret_cast<uint32_t*>(brow);   // the beta row is dead once the tables are built
     Q.head = 0;
     Q.n = 0;
 
@@ -255,12 +275,9 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
             nb.p0[m] = make_double2(dx, dy);
             nb.p1[m] = make_double2(dz, ia);
             nb.p2[m] = make_double2(fa, dfa_a);
-            if constexpr (Spec::NETA > 0) {
-                double E[Spec::NETA];
-                eta_chain<Spec>(a2, eta0, E);
-#pragma unroll
-                for (int q = 0; q < Spec::NETA; ++q) nb.pe[m * Spec::NETA + q] = E[q];
-            }
+            nb.fxy[m] = make_float2((float)dx, (float)dy);
+            nb.fz[m] = (float)dz;
+            if constexpr (Spec::NETA > 0) nb.p3[m] = make_double2(exp_small(-eta0 * a2), 0.0);
             // R = sum_r beta_r exp(-eta d^2) (fc'(a) - 2 eta d fc(a)) / a,  d = a - rs
             double R = 0.0;
             for (int r = 0; r < nr; ++r) {
@@ -275,46 +292,56 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
     }
     __syncwarp();
 
-    // ---- angular groups -----------------------------------------------------------------------
-    for (int e1 = 0; e1 < p.n_elem; ++e1)
-        for (int e2 = e1; e2 < p.n_elem; ++e2) {
-            const int pr = pair_index(e1, e2, p.n_elem);
-            const int na = prog->n_ang[pr];
-            if (na == 0) continue;
-            if constexpr (Spec::ID != ANG_GENERIC) {
-                // coefficient table of this group
-                if (lane < 16) {
+    // ---- angular part ---------------------------------------------------------------------------
+    const float rc2f = screen_rc2(p.rc2);
+    if constexpr (Spec::ID != ANG_GENERIC) {
+        // coefficient tables of all pair groups, then ONE sweep over all unordered neighbour pairs:
+        // the pair group is looked up per triplet, so a round (= colour class) spans the whole row
+        bool any = false;
+        for (int pr = 0; pr < npair; ++pr) {
+            any |= prog->n_ang[pr] > 0;
+            if (lane < 16) {
 #pragma unroll
-                    for (int e = 0; e < Spec::NETA; ++e) {
-                        if (Spec::mask(e) >> lane & 1u) {
-                            const int g = prog->ang_g[pr][e][lane];
-                            const int zeta = 1 << (lane & 7);
-                            const double lam = lane < 8 ? 1.0 : -1.0;
-                            const double bc = g >= 0 ? brow[g] * exp2((double)(1 - zeta)) : 0.0;
-                            int a = 0;   // accumulator slot = set bits before (e, lane)
-                            for (int ee = 0; ee < Spec::NETA; ++ee) {
-                                const unsigned mk = Spec::mask(ee);
-                                if (ee < e) a += __popc(mk);
-                                else if (ee == e) a += __popc(mk & ((1u << lane) - 1u));
-                            }
-                            bt[a] = make_double2(bc, bc * (double)zeta * lam);
+                for (int e = 0; e < Spec::NETA; ++e) {
+                    if (Spec::mask(e) >> lane & 1u) {
+                        const int g = prog->ang_g[pr][e][lane];
+                        const int zeta = 1 << (lane & 7);
+                        const double lam = lane < 8 ? 1.0 : -1.0;
+                        const double bc = g >= 0 ? brow[g] * exp2((double)(1 - zeta)) : 0.0;
+                        int a = 0;   // accumulator slot = set bits before (e, lane)
+                        for (int ee = 0; ee < Spec::NETA; ++ee) {
+                            const unsigned mk = Spec::mask(ee);
+                            if (ee < e) a += __popc(mk);
+                            else if (ee == e) a += __popc(mk & ((1u << lane) - 1u));
                         }
+                        bt[pr * bt_stride<Spec>() + a] = make_double2(bc, bc * (double)zeta * lam);
                     }
                 }
-                __syncwarp();
-                ForceTripletFast<Spec> f{nb, acc, bt, {}, p.k2};
-#pragma unroll
-                for (int e = 0; e < Spec::NETA; ++e) f.etas[e] = prog->ang_eta[e];
-                if (e1 == e2) enum_within(nb, seg[e1], seg[e1 + 1] - seg[e1], p.rc2, Q, lane, f);
-                else enum_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], p.rc2, Q, lane, f);
-                drain_tail(Q, lane, f);
-            } else {
-                ForceTripletGeneric f{nb, acc, prog->ang + prog->ang_off[pr], na, brow, p.k2};
-                if (e1 == e2) enum_within(nb, seg[e1], seg[e1 + 1] - seg[e1], p.rc2, Q, lane, f);
-                else enum_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], p.rc2, Q, lane, f);
-                drain_tail(Q, lane, f);
             }
         }
+        __syncwarp();        // tables written, beta row dead -> its memory becomes the pair queue
+        if (any) {
+            ForceTripletFast<Spec> f{nb, acc, bt, eta0, {}, p.k2, p.rc2, seg[1],
+                                     p.n_elem > 2 ? seg[2] : 0x7fffffff, p.n_elem > 3 ? seg[3] : 0x7fffffff, p.n_elem};
+            if (p.n_elem < 2) f.sg1 = 0x7fffffff;
+#pragma unroll
+            for (int e = 0; e < Spec::NETA; ++e) f.eta[e] = prog->ang_eta[e];
+            pairs_within(nb, 0, ntot, rc2f, Q, lane, f);
+        }
+    } else {
+        // generic tables: per pair group, walking the SF list; the beta row stays live, so the queue
+        // sits in the (unused) p3 plane
+        Q.q = reinterpret_cast<uint32_t*>(nb.p3);
+        for (int e1 = 0; e1 < p.n_elem; ++e1)
+            for (int e2 = e1; e2 < p.n_elem; ++e2) {
+                const int pr = pair_index(e1, e2, p.n_elem);
+                const int na = prog->n_ang[pr];
+                if (na == 0) continue;
+                ForceTripletGeneric f{nb, acc, prog->ang + prog->ang_off[pr], na, brow, p.k2, p.rc2};
+                if (e1 == e2) pairs_within(nb, seg[e1], seg[e1 + 1] - seg[e1], rc2f, Q, lane, f);
+                else pairs_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], rc2f, Q, lane, f);
+            }
+    }
     __syncwarp();
 
     // ---- flush: F_slot = V - A u; one global FP64 RED per component; the centre gets minus the sum
@@ -339,7 +366,7 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
 
 template <class Spec>
 static int launch_one(const ForceParams& p, cudaStream_t st) {
-    const size_t smem = FC_WARPS * force_warp_smem<Spec>(p.cap, p.g_stride);
+    const size_t smem = FC_WARPS * force_warp_smem<Spec>(p.cap, p.g_stride, p.n_elem);
     static bool configured = false;
     if (!configured) {
         cudaFuncSetAttribute(k_force<Spec>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -350,11 +377,11 @@ static int launch_one(const ForceParams& p, cudaStream_t st) {
     return 1;
 }
 
-size_t force_smem_bytes(int variant, int cap, int g_stride) {
+size_t force_smem_bytes(int variant, int cap, int g_stride, int n_elem) {
     switch (variant) {
-        case ANG_BASE12: return FC_WARPS * force_warp_smem<SpecBase12>(cap, g_stride);
-        case ANG_WIDE32: return FC_WARPS * force_warp_smem<SpecWide32>(cap, g_stride);
-        default: return FC_WARPS * force_warp_smem<SpecGeneric>(cap, g_stride);
+        case ANG_BASE12: return FC_WARPS * force_warp_smem<SpecBase12>(cap, g_stride, n_elem);
+        case ANG_WIDE32: return FC_WARPS * force_warp_smem<SpecWide32>(cap, g_stride, n_elem);
+        default: return FC_WARPS * force_warp_smem<SpecGeneric>(cap, g_stride, n_elem);
     }
 }
 

@@ -26,32 +26,39 @@ struct SfParams {
 
 template <class Spec>
 __host__ __device__ constexpr size_t sf_warp_smem(int cap) {
-    // p0, p1, p2 (double2 each) + pe (NETA doubles) per slot, queue (64 x u32), generic accumulators
-    return (size_t)cap * (48 + 8 * Spec::NETA) + 256 + (Spec::ID == ANG_GENERIC ? 64 * 8 : 0);
+    // p0, p1, p2 (double2 each), a (double), FP32 screening copy (12 B) per slot; queue (64 x u32);
+    // generic accumulators
+    const size_t capa = (size_t)((cap + 3) & ~3);
+    return capa * (48 + 8 + 12) + 256 + (Spec::ID == ANG_GENERIC ? 64 * 8 : 0);
 }
 
 // ---- per-triplet work, specialised groups -------------------------------------------------
 template <class Spec>
 struct SfTripletFast {
     const Nbh& nb;
-    double eta0, k2;
+    double eta0, k2, rc2;
     double acc[Spec::NACC > 0 ? Spec::NACC : 1];
 
-    __device__ __forceinline__ SfTripletFast(const Nbh& nb_, double eta0_, double k2_)
-        : nb(nb_), eta0(eta0_), k2(k2_) {
+    __device__ __forceinline__ SfTripletFast(const Nbh& nb_, double eta0_, double k2_, double rc2_)
+        : nb(nb_), eta0(eta0_), k2(k2_), rc2(rc2_) {
 #pragma unroll
         for (int a = 0; a < Spec::NACC; ++a) acc[a] = 0.0;
     }
 
     __device__ __forceinline__ void operator()(int j, int k, int, bool active) {
-        const double2 j0 = nb.p0[j], j1 = nb.p1[j], k0 = nb.p0[k], k1 = nb.p1[k];
+        const double2 j0 = nb.p0[j], j1 = nb.p1[j], j2 = nb.p2[j];
+        const double2 k0 = nb.p0[k], k1 = nb.p1[k], k2v = nb.p2[k];
         const double wx = k0.x - j0.x, wy = k0.y - j0.y, wz = k1.x - j1.x;
         const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
         const double Cc = cos_only(c2 * k2);
-        double fcc = Cc * Cc;                       // fc(c) = cos^2(pi c / (2 rc))
-        if (!active) fcc = 0.0;
-        double Ec[Spec::NETA];
-        eta_chain<Spec>(c2, eta0, Ec);
+        double C = (j2.y * k2v.y) * (Cc * Cc);      // fc(a) fc(b) fc(c), fc(c) = cos^2(pi c / (2 rc))
+        if (!active || !(c2 < rc2)) C = 0.0;        // exact cutoff (the queue was screened in FP32)
+        // Y_e = exp(-eta_e (a^2 + b^2 + c^2)): one exp, then integer powers
+        double Y[Spec::NETA];
+        Y[0] = (j2.x * k2v.x) * exp_small(-eta0 * c2);
+        if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
+        if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
+        if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
         const double cosv = fma(j0.x, k0.x, fma(j0.y, k0.y, j1.x * k1.x)) * (j1.y * k1.y);
         double pw[2][Spec::MAXBIT + 1];
         pw[0][0] = 1.0 + cosv;
@@ -63,7 +70,7 @@ struct SfTripletFast {
         }
 #pragma unroll
         for (int e = 0; e < Spec::NETA; ++e) {
-            const double xc = (nb.pe[j * Spec::NETA + e] * nb.pe[k * Spec::NETA + e]) * (Ec[e] * fcc);
+            const double xc = Y[e] * C;
 #pragma unroll
             for (int b = 0; b <= Spec::MAXBIT; ++b) {
                 if (Spec::mask(e) >> b & 1u) acc[acc_index<Spec>(e, b)] = fma(pw[0][b], xc, acc[acc_index<Spec>(e, b)]);
@@ -79,7 +86,8 @@ struct SfTripletGeneric {
     const Nbh& nb;
     const AngularSF* sf;
     int nsf;
-    double k2;
+    double k2, rc2;
+    const double* ra; // [slot] distance a
     double* gacc;     // [64] per warp, shared memory
     int lane;
 
@@ -89,10 +97,11 @@ struct SfTripletGeneric {
         const double wx = k0.x - j0.x, wy = k0.y - j0.y, wz = k1.x - j1.x;
         const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
         const double Cc = cos_only(c2 * k2);
-        double C = j2.x * kq.x * (Cc * Cc);
-        if (!active) C = 0.0;
+        double C = j2.y * kq.y * (Cc * Cc);
+        if (!active || !(c2 < rc2)) C = 0.0;
         const double cosv = (j0.x * k0.x + j0.y * k0.y + j1.x * k1.x) * (j1.y * k1.y);
-        const double r2sum = j2.y * j2.y + kq.y * kq.y + c2;
+        const double aj = ra[j], ak = ra[k];
+        const double r2sum = aj * aj + ak * ak + c2;
         for (int s = 0; s < nsf; ++s) {
             const AngularSF f = sf[s];
             const double base = 1.0 + (double)f.lam * cosv;
@@ -121,14 +130,18 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
     if (p.variant[tc] != Spec::ID) return;
     const ElemProgram* __restrict__ prog = p.prog[tc];
 
+    const int capa = (p.cap + 3) & ~3;
     unsigned char* base = smem_raw + (size_t)wid * sf_warp_smem<Spec>(p.cap);
     Nbh nb;
     nb.p0 = reinterpret_cast<double2*>(base);
-    nb.p1 = nb.p0 + p.cap;
-    nb.p2 = nb.p1 + p.cap;
-    nb.pe = reinterpret_cast<double*>(nb.p2 + p.cap);
+    nb.p1 = nb.p0 + capa;
+    nb.p2 = nb.p1 + capa;
+    nb.p3 = nullptr;
+    double* ra = reinterpret_cast<double*>(nb.p2 + capa);
+    nb.fxy = reinterpret_cast<float2*>(ra + capa);
+    nb.fz = reinterpret_cast<float*>(nb.fxy + capa);
     PairQueue Q;
-    Q.q = reinterpret_cast<uint32_t*>(nb.pe + (size_t)p.cap * Spec::NETA);
+    Q.q = reinterpret_cast<uint32_t*>(nb.fz + capa);
     Q.head = 0;
     Q.n = 0;
     double* gacc = reinterpret_cast<double*>(Q.q + 64);
@@ -152,18 +165,15 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
         const double dz = min_image_1d(zi, p.sz[j], p.box[2], p.half[2]);
         const double a2 = fma(dx, dx, fma(dy, dy, dz * dz));
         const double ia = rsqrt(a2);
-        const double a = a2 * ia;
         const double Ca = cos_only(a2 * p.k2);
-        const double fa = Ca * Ca;                  // fc(a)
+        double E0 = 0.0;
+        if constexpr (Spec::NETA > 0) E0 = exp_small(-eta0 * a2);
         nb.p0[m] = make_double2(dx, dy);
         nb.p1[m] = make_double2(dz, ia);
-        nb.p2[m] = make_double2(fa, a);
-        if constexpr (Spec::NETA > 0) {
-            double E[Spec::NETA];
-            eta_chain<Spec>(a2, eta0, E);
-#pragma unroll
-            for (int e = 0; e < Spec::NETA; ++e) nb.pe[m * Spec::NETA + e] = E[e] * fa;
-        }
+        nb.p2[m] = make_double2(E0, Ca * Ca);       // (exp(-eta_0 a^2), fc(a))
+        ra[m] = a2 * ia;
+        nb.fxy[m] = make_float2((float)dx, (float)dy);
+        nb.fz[m] = (float)dz;
     }
     __syncwarp();
 
@@ -177,9 +187,8 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
             const RadialSF f = prog->rad[off + r];
             double acc = 0.0;
             for (int m = seg[e] + lane; m < seg[e + 1]; m += 32) {
-                const double2 q = nb.p2[m];
-                const double d = q.y - f.rs;
-                acc = fma(exp_small(fmax(-f.eta * d * d, -700.0)), q.x, acc);
+                const double d = ra[m] - f.rs;
+                acc = fma(exp_small(fmax(-f.eta * d * d, -700.0)), nb.p2[m].y, acc);
             }
             acc = warp_sum(acc);
             if (lane == 0) Grow[f.g] = acc;
@@ -187,16 +196,16 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
     }
 
     // ---- angular groups -----------------------------------------------------------------------
+    const float rc2f = screen_rc2(p.rc2);
     for (int e1 = 0; e1 < p.n_elem; ++e1)
         for (int e2 = e1; e2 < p.n_elem; ++e2) {
             const int pr = pair_index(e1, e2, p.n_elem);
             const int na = prog->n_ang[pr];
             if (na == 0) continue;
             if constexpr (Spec::ID != ANG_GENERIC) {
-                SfTripletFast<Spec> f(nb, eta0, p.k2);
-                if (e1 == e2) enum_within(nb, seg[e1], seg[e1 + 1] - seg[e1], p.rc2, Q, lane, f);
-                else enum_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], p.rc2, Q, lane, f);
-                drain_tail(Q, lane, f);
+                SfTripletFast<Spec> f(nb, eta0, p.k2, p.rc2);
+                if (e1 == e2) pairs_within(nb, seg[e1], seg[e1 + 1] - seg[e1], rc2f, Q, lane, f);
+                else pairs_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], rc2f, Q, lane, f);
 #pragma unroll
                 for (int e = 0; e < Spec::NETA; ++e)
 #pragma unroll
@@ -211,10 +220,10 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
             } else {
                 for (int s = lane; s < na; s += 32) gacc[s] = 0.0;
                 __syncwarp();
-                SfTripletGeneric f{nb, prog->ang + prog->ang_off[pr], na, p.k2, gacc, lane};
-                if (e1 == e2) enum_within(nb, seg[e1], seg[e1 + 1] - seg[e1], p.rc2, Q, lane, f);
-                else enum_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], p.rc2, Q, lane, f);
-                drain_tail(Q, lane, f);
+                SfTripletGeneric f{nb, prog->ang + prog->ang_off[pr], na, p.k2, p.rc2, ra, gacc, lane};
+                if (e1 == e2) pairs_within(nb, seg[e1], seg[e1 + 1] - seg[e1], rc2f, Q, lane, f);
+                else pairs_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], rc2f, Q, lane, f);
+                __syncwarp();
                 for (int s = lane; s < na; s += 32) Grow[prog->ang[prog->ang_off[pr] + s].g] = gacc[s];
                 __syncwarp();
             }
