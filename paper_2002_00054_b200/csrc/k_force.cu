@@ -14,6 +14,8 @@
 // a time (angular.cuh): pairs of equal colour never share a slot, and a warp owns its slots, so
 // no shared-memory atomics are needed (the first version's FP64 shared atomicAdd = CAS loops
 // took >35 % of the stall samples and ran 2.8 iterations on average; profiles/r1_*).
+#include <cstdlib>
+
 #include "angular.cuh"
 #include "geometry.cuh"
 
@@ -402,8 +404,13 @@ int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const
     }
     cudaMemsetAsync(w.f_sorted, 0, sizeof(double) * 3 * (size_t)n, st);
     int launches = 0;
-    if (use[ANG_BASE12]) launches += launch_one<SpecBase12>(p, st);
-    if (use[ANG_WIDE32]) launches += launch_one<SpecWide32>(p, st);
+    static const bool queue_design = getenv("NNP_QUEUE_DESIGN") != nullptr;   // A/B switch while both designs exist
+    if (queue_design) {
+        if (use[ANG_BASE12]) launches += launch_one<SpecBase12>(p, st);
+        if (use[ANG_WIDE32]) launches += launch_one<SpecWide32>(p, st);
+    } else if (use[ANG_BASE12] || use[ANG_WIDE32]) {
+        launches += launch_force2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, st);
+    }
     if (use[ANG_GENERIC]) launches += launch_one<SpecGeneric>(p, st);
     return launches;
 }

@@ -1,0 +1,418 @@
+// k_force2.cu -- S4 fast path (specialised pair groups): forces F_m = - sum_i sum_s beta_is dG_is/dr_m
+// with dG/dr RECOMPUTED, never stored (PAPER.md L40 step 3, L56-58, L98, L124); "the dominant
+// angular force loop" (L116).  Lane-owned design (stream.cuh): one CTA of WPC warps per centre i; the
+// centre's contributing triplets (i; j,k) are split evenly over the threads; a lane keeps neighbour j
+// in registers, gathers only the partner k, accumulates the force on j in registers and the force on
+// k in its warp's per-slot shared-memory accumulator (lanes of a warp that hit the same slot take
+// turns; the turn order comes from match.any, issued early so that its latency hides).
+//
+// Per triplet, with u = r_j - r_i, v = r_k - r_i, w = v - u, the beta-weighted gradient is
+//     dg/du = f_uu u + f_uv v - f_w w,      dg/dv = f_vv v + f_uv u + f_w w
+// so  F_j = -s1 u + s3 v,  F_k = -s2 v + s3 u  with s1 = f_uu + f_w, s2 = f_vv + f_w, s3 = f_w - f_uv.
+// The force on j is kept as (A = sum s1, V = sum s3 v) in registers while the lane owns j and folded
+// into the slot accumulator as V - A u when the lane leaves j; the force on k goes straight into the
+// slot accumulator (three doubles per slot).  F_slot - R u (R = radial part) is flushed with one global
+// FP64 RED per component per neighbour; the centre receives minus the sum.
+//
+// Coefficients: the lane keeps c_b = beta_b 2^(1-zeta_b) of its current pair group in registers
+// (NACC <= 12) -- per-lane table loads from shared memory cost 4 wavefronts each (ncu, r1b) -- and gets
+// dP/dcos from the SAME coefficients with pre-scaled powers zeta (1 +- cos)^(zeta-1): the factor zeta =
+// 2^b is an integer add on the exponent field, the factor lambda a negated operand.
+#include "angular.cuh"
+#include "geometry.cuh"
+#include "stream.cuh"
+
+namespace nnp {
+
+struct Force2Params {
+    int64_t n;
+    int n_elem, ncell, stride, cap, g_stride;
+    double rc, rc2, k2;                  // k2 = (pi / (2 rc))^2
+    double box[3], half[3];
+    const double *sx, *sy, *sz;
+    const int32_t *cell_start, *nbr, *nbr_cnt;
+    const double* dEdG;
+    double* f_sorted;
+    const ElemProgram* prog[MAX_ELEM];
+    int variant[MAX_ELEM];
+};
+
+template <class Spec>
+__host__ __device__ constexpr int bt2_stride() { return Spec::NACC + 1; }   // +1: groups land on different banks
+
+// shared memory of one centre (= one CTA of WPC warps): planes p0,p1,p2 (double2), WPC accumulator
+// sets fxy (double2), fz (double) [+ 8 B pad; the FP32 screening copy and the prefix array alias set 0],
+// e0, rad (double), coefficient tables, group table, beta row, scratch, masks
+template <class Spec>
+__host__ __device__ constexpr size_t force2_smem(int cap, int g_stride, int n_elem, int wpc) {
+    const size_t capa = (size_t)((cap + 3) & ~3);
+    const size_t npair = (size_t)n_elem * (n_elem + 1) / 2;
+    size_t b = capa * (3 * 16 + 2 * 8 + (size_t)wpc * 32);
+    b += npair * bt2_stride<Spec>() * 16;
+    b += npair * sizeof(GroupTab);
+    b += (size_t)g_stride * 8 + 64;
+    b += (size_t)mask_words_cap(cap, n_elem) * 4;
+    return (b + 15) / 16 * 16;
+}
+
+struct SlotAcc2 {
+    double2* fxy;  // (Fx, Fy)
+    double* fz;    // Fz
+};
+
+// rank of the lane among the lanes of its warp that target the same slot (inactive lanes: 0)
+__device__ __forceinline__ int conflict_rank(int slot, bool act, int lane) {
+    const unsigned peers = __match_any_sync(FULL, act ? slot : -1 - lane);
+    return __popc(peers & ((1u << lane) - 1u));
+}
+
+// acc[slot] += (x, y, z) for the lanes with act; lanes that target the same slot take turns
+__device__ __forceinline__ void slot_add(const SlotAcc2& acc, int slot, bool act, int rank, double x, double y, double z) {
+    for (int pass = 0; __any_sync(FULL, act && rank >= pass); ++pass) {
+        if (act && rank == pass) {
+            double2 p = acc.fxy[slot];
+            double q = acc.fz[slot];
+            p.x += x; p.y += y; q += z;
+            acc.fxy[slot] = p;
+            acc.fz[slot] = q;
+        }
+        __syncwarp();
+    }
+}
+
+// x * 2^b for b >= 0 by an integer add on the exponent field (x >= 0 finite, far from overflow; x = 0
+// becomes 2^(b-1023), which is harmless where it is used)
+__device__ __forceinline__ double scale2(double x, int b) {
+    return __hiloint2double(__double2hiint(x) + (b << 20), __double2loint(x));
+}
+
+// data of the lane's owner slot j, in registers
+struct JData {
+    double ux, uy, uz, ia, fa, dfa, e0;
+};
+
+template <class Spec, int WPC>
+__global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_constant__ Force2Params p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int NT = WPC * 32;
+    constexpr bool REGC = Spec::NACC <= 12;          // coefficients of the current group in registers
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int64_t i = blockIdx.x;
+    int tc = 0;
+    for (int e = 1; e < p.n_elem; ++e)
+        if (i >= p.cell_start[(size_t)e * p.ncell]) tc = e;
+    if (p.variant[tc] != Spec::ID) return;          // uniform per CTA
+    const ElemProgram* __restrict__ prog = p.prog[tc];
+
+    const int capa = (p.cap + 3) & ~3;
+    const int npair = p.n_elem * (p.n_elem + 1) / 2;
+    double2* p0 = reinterpret_cast<double2*>(smem_raw);     // (ux, uy)
+    double2* p1 = p0 + capa;                                // (uz, 1/a)
+    double2* p2 = p1 + capa;                                // (fc(a), fc'(a)/a)
+    double2* acc0 = p2 + capa;                              // WPC x (fxy[capa] double2, fz[capa] double, pad)
+    SlotAcc2 acc;
+    acc.fxy = acc0 + (size_t)wid * 2 * capa;
+    acc.fz = reinterpret_cast<double*>(acc.fxy + capa);
+    double* e0 = reinterpret_cast<double*>(acc0 + (size_t)WPC * 2 * capa);   // exp(-eta_0 a^2)
+    double* rad = e0 + capa;                                  // radial scalar R
+    double2* bt = reinterpret_cast<double2*>(rad + capa);     // [pair][bt2_stride]: (beta 2^(1-zeta), beta 2^(1-zeta) zeta lambda)
+    double* btc = reinterpret_cast<double*>(bt);              // register-coefficient path: [pair][2 * bt2_stride] doubles, c_b only
+    GroupTab* tab = reinterpret_cast<GroupTab*>(bt + npair * bt2_stride<Spec>());
+    double* brow = reinterpret_cast<double*>(tab + npair);
+    int* wsum = reinterpret_cast<int*>(brow + p.g_stride);    // 16 ints of scratch
+    uint32_t* masks = reinterpret_cast<uint32_t*>(wsum + 16);
+    float4* f32 = reinterpret_cast<float4*>(acc0);            // alias: screening copy (dead before the accumulators are zeroed)
+    uint16_t* C = reinterpret_cast<uint16_t*>(acc0 + capa);   // alias: prefix of the mask popcounts
+
+    int seg[MAX_ELEM + 1];
+    seg[0] = 0;
+#pragma unroll
+    for (int e = 0; e < MAX_ELEM; ++e) seg[e + 1] = seg[e] + p.nbr_cnt[(size_t)i * MAX_ELEM + e];
+    const int ntot = seg[MAX_ELEM];
+
+    for (int s = tid; s < p.g_stride; s += NT) brow[s] = p.dEdG[(size_t)i * p.g_stride + s];
+    __syncthreads();
+
+    // ---- stage the neighbourhood; radial part R = sum_r beta_r exp(-eta d^2) (fc'(a) - 2 eta d fc(a)) / a
+    const double xi = p.sx[i], yi = p.sy[i], zi = p.sz[i];
+    const int32_t* row = p.nbr + (size_t)i * p.stride;
+    const double eta0 = prog->ang_eta[0];
+    for (int e = 0; e < p.n_elem; ++e) {
+        const int nr = prog->n_rad[e], off = prog->rad_off[e];
+        for (int m = seg[e] + tid; m < seg[e + 1]; m += NT) {
+            const int j = row[m];
+            const double dx = min_image_1d(xi, p.sx[j], p.box[0], p.half[0]);
+            const double dy = min_image_1d(yi, p.sy[j], p.box[1], p.half[1]);
+            const double dz = min_image_1d(zi, p.sz[j], p.box[2], p.half[2]);
+            const double a2 = fma(dx, dx, fma(dy, dy, dz * dz));
+            const double ia = rsqrt(a2);
+            const double a = a2 * ia;
+            double Ca, Sa;
+            cos_sinc(a2 * p.k2, Ca, Sa);
+            const double fa = Ca * Ca;                          // fc(a)
+            const double dfa_a = (-2.0 * p.k2) * (Ca * Sa);     // fc'(a)/a
+            p0[m] = make_double2(dx, dy);
+            p1[m] = make_double2(dz, ia);
+            p2[m] = make_double2(fa, dfa_a);
+            e0[m] = exp_small(-eta0 * a2);
+            f32[m] = make_float4((float)dx, (float)dy, (float)dz, 0.f);
+            double R = 0.0;
+            for (int r = 0; r < nr; ++r) {
+                const RadialSF f = prog->rad[off + r];
+                const double d = a - f.rs;
+                const double ex = exp_small(fmax(-f.eta * d * d, -700.0));
+                R = fma(brow[f.g] * ex, fma(-2.0 * f.eta * d, fa * ia, dfa_a), R);
+            }
+            rad[m] = R;
+        }
+    }
+    // coefficient tables of all pair groups
+    if (tid < 16) {
+        for (int pr = 0; pr < npair; ++pr) {
+#pragma unroll
+            for (int e = 0; e < Spec::NETA; ++e) {
+                if (Spec::mask(e) >> tid & 1u) {
+                    const int g = prog->ang_g[pr][e][tid];
+                    const int zeta = 1 << (tid & 7);
+                    const double lam = tid < 8 ? 1.0 : -1.0;
+                    const double bc = g >= 0 ? brow[g] * exp2((double)(1 - zeta)) : 0.0;
+                    int a = 0;   // accumulator slot = set bits before (e, tid)
+                    for (int ee = 0; ee < Spec::NETA; ++ee) {
+                        const unsigned mk = Spec::mask(ee);
+                        if (ee < e) a += __popc(mk);
+                        else if (ee == e) a += __popc(mk & ((1u << tid) - 1u));
+                    }
+                    if constexpr (REGC) btc[pr * 2 * bt2_stride<Spec>() + a] = bc;
+                    else bt[pr * bt2_stride<Spec>() + a] = make_double2(bc, bc * (double)zeta * lam);
+                }
+            }
+        }
+    }
+    int NW = 0;
+    const int ng = build_groups<true>(seg, p.n_elem, prog->n_ang, tab, tid, NW);
+    __syncthreads();
+
+    // ---- screening -> masks; prefix; even split of the triplet stream over the NT threads ------------
+    const float rc2f = (float)(p.rc2 * (1.0 + 1e-5));
+    for (int g = 0; g < ng; ++g) screen_group(tab[g], f32, masks, rc2f, tid, NT);
+    __syncthreads();
+    const int T = mask_prefix(masks, C, NW, tid, NT, wsum);
+    __syncthreads();
+    const int quota = (T + NT - 1) / NT;
+    Walker wk;
+    wk.masks = masks; wk.tab = tab;
+    wk.cnt = max(0, min(quota, T - tid * quota));
+    wk.m = 0u; wk.idx = 0; wk.j = 0; wk.w = 0; wk.g = 0;
+    wk.jbeg = wk.jend = wk.kbase = wk.ns = wk.pair = wk.gfirst = 0; wk.W = 1; wk.last = 1;
+    if (wk.cnt > 0) wk.seek(C, NW, ng, tid * quota);
+    __syncthreads();
+    for (int m = tid; m < WPC * 2 * capa; m += NT) acc0[m] = make_double2(0.0, 0.0);   // the aliases are dead
+    __syncthreads();
+
+    // ---- angular part: every lane walks its range of the stream ---------------------------------------
+    double eta[Spec::NETA];
+#pragma unroll
+    for (int e = 0; e < Spec::NETA; ++e) eta[e] = prog->ang_eta[e];
+    JData J;
+    J.ux = J.uy = J.uz = 1.0; J.ia = 1.0; J.fa = 0.0; J.dfa = 0.0; J.e0 = 1.0;
+    int jcur = -1, paircur = -1;
+    double Aj = 0.0, Vx = 0.0, Vy = 0.0, Vz = 0.0;
+    double cf[REGC ? Spec::NACC : 1];                 // c_b of the lane's current pair group
+#pragma unroll
+    for (int a = 0; a < (REGC ? Spec::NACC : 1); ++a) cf[a] = 0.0;
+    for (int it = 0; it < quota; ++it) {
+        const bool active = wk.cnt > 0;
+        wk.advance();
+        // Owner slot changed: fold the j-side sums into the slot accumulator and load the new j.  No
+        // conflict is possible inside the loop: the stream is j-major, so the lanes that share a slot j
+        // are consecutive and only the last of them leaves j before its range ends (the others flush
+        // after the loop).
+        if (active && wk.j != jcur) {
+            if (jcur >= 0) {
+                double2 a = acc.fxy[jcur];
+                double b = acc.fz[jcur];
+                a.x += fma(-Aj, J.ux, Vx); a.y += fma(-Aj, J.uy, Vy); b += fma(-Aj, J.uz, Vz);
+                acc.fxy[jcur] = a;
+                acc.fz[jcur] = b;
+            }
+            jcur = wk.j;
+            const double2 a0 = p0[jcur], a1 = p1[jcur], a2 = p2[jcur];
+            J.ux = a0.x; J.uy = a0.y; J.uz = a1.x; J.ia = a1.y; J.fa = a2.x; J.dfa = a2.y; J.e0 = e0[jcur];
+            Aj = 0.0; Vx = 0.0; Vy = 0.0; Vz = 0.0;
+        }
+        if constexpr (REGC) {
+            if (active && wk.pair != paircur) {
+                paircur = wk.pair;
+                const double2* src = reinterpret_cast<const double2*>(btc + paircur * 2 * bt2_stride<Spec>());
+#pragma unroll
+                for (int a = 0; a < Spec::NACC / 2; ++a) {
+                    const double2 c = src[a];
+                    cf[2 * a] = c.x; cf[2 * a + 1] = c.y;
+                }
+                if constexpr (Spec::NACC & 1) cf[Spec::NACC - 1] = btc[paircur * 2 * bt2_stride<Spec>() + Spec::NACC - 1];
+            }
+        }
+        __syncwarp();
+        const double2* btg = bt + wk.pair * bt2_stride<Spec>();
+        const int k = active ? wk.pop() : max(jcur, 0);
+        const int rank = conflict_rank(k, active, lane);       // issued early: its latency hides behind the FP64 work
+        const double2 k0 = p0[k], k1 = p1[k], k2v = p2[k];
+        const double ek = e0[k];
+        const double wx = k0.x - J.ux, wy = k0.y - J.uy, wz = k1.x - J.uz;
+        const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
+        double Cc, Sc;
+        cos_sinc(c2 * p.k2, Cc, Sc);
+        double fcc = Cc * Cc;                          // fc(c)
+        double dfc = (-2.0 * p.k2) * (Cc * Sc);        // fc'(c)/c
+        if (!active || !(c2 < p.rc2)) { fcc = 0.0; dfc = 0.0; }   // exact cutoff (the masks were screened in FP32)
+        double Y[Spec::NETA];
+        Y[0] = (J.e0 * ek) * exp_small(-eta0 * c2);
+        if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
+        if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
+        if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
+        const double iab = J.ia * k1.y;
+        const double cosv = fma(J.ux, k0.x, fma(J.uy, k0.y, J.uz * k1.x)) * iab;
+        // pw[l][b] = (1 +- cos)^(2^b) ; pd[l][b] = (1 +- cos)^(2^b - 1)  (REGC: times zeta = 2^b)
+        double pw[2][Spec::MAXBIT + 1], pd[2][Spec::MAXBIT + 1];
+        pw[0][0] = 1.0 + cosv; pw[1][0] = 1.0 - cosv;
+        pd[0][0] = 1.0; pd[1][0] = 1.0;
+#pragma unroll
+        for (int b = 1; b <= Spec::MAXBIT; ++b) {
+#pragma unroll
+            for (int l = 0; l < 2; ++l) {
+                pw[l][b] = pw[l][b - 1] * pw[l][b - 1];
+                pd[l][b] = pd[l][b - 1] * pw[l][b - 1];
+            }
+        }
+        if constexpr (REGC) {
+#pragma unroll
+            for (int b = 1; b <= Spec::MAXBIT; ++b) {
+                pd[0][b] = scale2(pd[0][b], b);
+                pd[1][b] = scale2(pd[1][b], b);
+            }
+        }
+        double Z0 = 0.0, Z1 = 0.0, Z2 = 0.0;
+#pragma unroll
+        for (int e = 0; e < Spec::NETA; ++e) {
+            double T0 = 0.0, T1 = 0.0;
+#pragma unroll
+            for (int b = 0; b <= Spec::MAXBIT; ++b) {
+#pragma unroll
+                for (int l = 0; l < 2; ++l)
+                    if (Spec::mask(e) >> (8 * l + b) & 1u) {
+                        if constexpr (REGC) {
+                            const double c = cf[acc_index<Spec>(e, 8 * l + b)];
+                            T0 = fma(c, pw[l][b], T0);
+                            T1 = l == 0 ? fma(c, pd[l][b], T1) : fma(-c, pd[l][b], T1);
+                        } else {
+                            const double2 c = btg[acc_index<Spec>(e, 8 * l + b)];
+                            T0 = fma(c.x, pw[l][b], T0);
+                            T1 = fma(c.y, pd[l][b], T1);
+                        }
+                    }
+            }
+            const double A = T0 * Y[e];
+            Z0 += A;
+            Z1 = fma(T1, Y[e], Z1);
+            Z2 = fma(eta[e], A, Z2);
+        }
+        // slot scalars
+        const double fab = J.fa * k2v.x;
+        const double Cf = fab * fcc;
+        const double t2 = (Cf + Cf) * Z2;
+        const double f_w = fma(fab * dfc, Z0, -t2);
+        const double q = Z1 * Cf;
+        const double qc = q * cosv;
+        const double f_uu = fma(-qc, J.ia * J.ia, fma((J.dfa * k2v.x) * fcc, Z0, -t2));
+        const double f_vv = fma(-qc, k1.y * k1.y, fma((J.fa * k2v.y) * fcc, Z0, -t2));
+        const double s1 = f_uu + f_w, s2 = f_vv + f_w, s3 = fma(-q, iab, f_w);
+        Aj += s1;
+        Vx = fma(s3, k0.x, Vx);
+        Vy = fma(s3, k0.y, Vy);
+        Vz = fma(s3, k1.x, Vz);
+        // F_k = s3 u - s2 v
+        slot_add(acc, k, active, rank, fma(s3, J.ux, -s2 * k0.x), fma(s3, J.uy, -s2 * k0.y), fma(s3, J.uz, -s2 * k1.x));
+    }
+    // the lanes whose ranges end inside the same slot j fold it in here, one after the other
+    slot_add(acc, jcur, jcur >= 0, conflict_rank(jcur, jcur >= 0, lane), fma(-Aj, J.ux, Vx), fma(-Aj, J.uy, Vy),
+             fma(-Aj, J.uz, Vz));
+    __syncthreads();
+
+    // ---- flush: F_slot - R u; one global FP64 RED per component; the centre gets minus the sum -------
+    double fx = 0.0, fy = 0.0, fz = 0.0;
+    for (int m = tid; m < ntot; m += NT) {
+        const int j = row[m];
+        const double2 u0 = p0[m];
+        const double uz = p1[m].x;
+        double2 fxy = acc0[m];
+        double fzz = reinterpret_cast<const double*>(acc0 + capa)[m];
+#pragma unroll
+        for (int w = 1; w < WPC; ++w) {
+            const double2 a = acc0[(size_t)w * 2 * capa + m];
+            fxy.x += a.x; fxy.y += a.y;
+            fzz += reinterpret_cast<const double*>(acc0 + (size_t)w * 2 * capa + capa)[m];
+        }
+        const double R = rad[m];
+        const double ax = fma(-R, u0.x, fxy.x), ay = fma(-R, u0.y, fxy.y), az = fma(-R, uz, fzz);
+        atomicAdd(&p.f_sorted[3 * (size_t)j + 0], ax);
+        atomicAdd(&p.f_sorted[3 * (size_t)j + 1], ay);
+        atomicAdd(&p.f_sorted[3 * (size_t)j + 2], az);
+        fx -= ax; fy -= ay; fz -= az;
+    }
+    fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
+    if (lane == 0) {
+        atomicAdd(&p.f_sorted[3 * (size_t)i + 0], fx);
+        atomicAdd(&p.f_sorted[3 * (size_t)i + 1], fy);
+        atomicAdd(&p.f_sorted[3 * (size_t)i + 2], fz);
+    }
+}
+
+#ifndef NNP_F2_WPC
+#define NNP_F2_WPC 2
+#endif
+constexpr int F2_WPC = NNP_F2_WPC;
+
+template <class Spec>
+static int launch_one2(const Force2Params& p, cudaStream_t st) {
+    const size_t smem = force2_smem<Spec>(p.cap, p.g_stride, p.n_elem, F2_WPC);
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(k_force2<Spec, F2_WPC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        configured = true;
+    }
+    k_force2<Spec, F2_WPC><<<(unsigned)p.n, F2_WPC * 32, smem, st>>>(p);
+    return 1;
+}
+
+size_t force2_smem_bytes(int variant, int cap, int g_stride, int n_elem) {
+    switch (variant) {
+        case ANG_BASE12: return force2_smem<SpecBase12>(cap, g_stride, n_elem, F2_WPC);
+        case ANG_WIDE32: return force2_smem<SpecWide32>(cap, g_stride, n_elem, F2_WPC);
+        default: return 0;
+    }
+}
+
+// launches the fast kernels for the specialised variants in use; the caller has zeroed f_sorted
+int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
+                  const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st) {
+    if (n == 0) return 0;
+    Force2Params p;
+    p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride;
+    p.rc = rc; p.rc2 = rc * rc;
+    p.k2 = (3.14159265358979323846 / (2.0 * rc)) * (3.14159265358979323846 / (2.0 * rc));
+    for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
+    p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
+    p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.dEdG = w.dEdG; p.f_sorted = w.f_sorted;
+    bool use[3] = {false, false, false};
+    for (int e = 0; e < MAX_ELEM; ++e) {
+        p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
+        p.variant[e] = e < n_elem ? variant[e] : -1;
+        if (e < n_elem) use[variant[e]] = true;
+    }
+    int launches = 0;
+    if (use[ANG_BASE12]) launches += launch_one2<SpecBase12>(p, st);
+    if (use[ANG_WIDE32]) launches += launch_one2<SpecWide32>(p, st);
+    return launches;
+}
+
+}  // namespace nnp
