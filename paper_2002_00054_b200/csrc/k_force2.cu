@@ -40,18 +40,21 @@ struct Force2Params {
 template <class Spec>
 __host__ __device__ constexpr int bt2_stride() { return Spec::NACC + 1; }   // +1: groups land on different banks
 
-// shared memory of one centre (= one CTA of WPC warps): planes p0,p1,p2 (double2), WPC accumulator
-// sets fxy (double2), fz (double) [+ 8 B pad; the FP32 screening copy and the prefix array alias set 0],
-// e0, rad (double), coefficient tables, group table, beta row, scratch, masks
+// Shared memory of one centre (= one CTA of WPC warps).  CAPA (slot capacity) is a template parameter so
+// that every array of the hot loop sits at a compile-time offset (ncu r1b: with run-time plane offsets
+// the loop spent ~40 of its ~380 instructions re-deriving shared-memory addresses):
+//   planes p0,p1,p2 (double2[CAPA]) | WPC accumulator sets: fxy double2[CAPA], fz double[CAPA], 8 B pad
+//   (the FP32 screening copy and the prefix array alias set 0) | e0, rad double[CAPA] |
+//   then, at run-time offsets: group table, coefficient tables, scratch, beta row, and the mask words
+//   (mask + descriptor, uint2[mask_words_cap(CAPA, n_elem)])
 template <class Spec>
-__host__ __device__ constexpr size_t force2_smem(int cap, int g_stride, int n_elem, int wpc) {
-    const size_t capa = (size_t)((cap + 3) & ~3);
+__host__ __device__ constexpr size_t force2_smem(int capa, int g_stride, int n_elem, int wpc) {
     const size_t npair = (size_t)n_elem * (n_elem + 1) / 2;
-    size_t b = capa * (3 * 16 + 2 * 8 + (size_t)wpc * 32);
-    b += npair * bt2_stride<Spec>() * 16;
+    size_t b = (size_t)capa * (3 * 16 + 2 * 8 + (size_t)wpc * 32);
     b += npair * sizeof(GroupTab);
-    b += (size_t)g_stride * 8 + 64;
-    b += (size_t)mask_words_cap(cap, n_elem) * 4;
+    b += npair * bt2_stride<Spec>() * 16;
+    b += 64 + (size_t)((g_stride + 1) & ~1) * 8;
+    b += (size_t)mask_words_cap(capa, n_elem) * 8;
     return (b + 15) / 16 * 16;
 }
 
@@ -91,7 +94,7 @@ struct JData {
     double ux, uy, uz, ia, fa, dfa, e0;
 };
 
-template <class Spec, int WPC>
+template <class Spec, int WPC, int CAPA>
 __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_constant__ Force2Params p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NT = WPC * 32;
@@ -104,7 +107,7 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
     if (p.variant[tc] != Spec::ID) return;          // uniform per CTA
     const ElemProgram* __restrict__ prog = p.prog[tc];
 
-    const int capa = (p.cap + 3) & ~3;
+    constexpr int capa = CAPA;
     const int npair = p.n_elem * (p.n_elem + 1) / 2;
     double2* p0 = reinterpret_cast<double2*>(smem_raw);     // (ux, uy)
     double2* p1 = p0 + capa;                                // (uz, 1/a)
@@ -115,12 +118,12 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
     acc.fz = reinterpret_cast<double*>(acc.fxy + capa);
     double* e0 = reinterpret_cast<double*>(acc0 + (size_t)WPC * 2 * capa);   // exp(-eta_0 a^2)
     double* rad = e0 + capa;                                  // radial scalar R
-    double2* bt = reinterpret_cast<double2*>(rad + capa);     // [pair][bt2_stride]: (beta 2^(1-zeta), beta 2^(1-zeta) zeta lambda)
+    GroupTab* tab = reinterpret_cast<GroupTab*>(rad + capa);
+    double2* bt = reinterpret_cast<double2*>(tab + npair);    // [pair][bt2_stride]: (beta 2^(1-zeta), beta 2^(1-zeta) zeta lambda)
     double* btc = reinterpret_cast<double*>(bt);              // register-coefficient path: [pair][2 * bt2_stride] doubles, c_b only
-    GroupTab* tab = reinterpret_cast<GroupTab*>(bt + npair * bt2_stride<Spec>());
-    double* brow = reinterpret_cast<double*>(tab + npair);
-    int* wsum = reinterpret_cast<int*>(brow + p.g_stride);    // 16 ints of scratch
-    uint32_t* masks = reinterpret_cast<uint32_t*>(wsum + 16);
+    int* wsum = reinterpret_cast<int*>(bt + npair * bt2_stride<Spec>());   // 16 ints of scratch
+    double* brow = reinterpret_cast<double*>(wsum + 16);
+    uint2* words = reinterpret_cast<uint2*>(brow + ((p.g_stride + 1) & ~1));   // (mask, descriptor)
     float4* f32 = reinterpret_cast<float4*>(acc0);            // alias: screening copy (dead before the accumulators are zeroed)
     uint16_t* C = reinterpret_cast<uint16_t*>(acc0 + capa);   // alias: prefix of the mask popcounts
 
@@ -194,17 +197,16 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
 
     // ---- screening -> masks; prefix; even split of the triplet stream over the NT threads ------------
     const float rc2f = (float)(p.rc2 * (1.0 + 1e-5));
-    for (int g = 0; g < ng; ++g) screen_group(tab[g], f32, masks, rc2f, tid, NT);
+    for (int g = 0; g < ng; ++g) screen_group(tab[g], f32, words, rc2f, tid, NT);
     __syncthreads();
-    const int T = mask_prefix(masks, C, NW, tid, NT, wsum);
+    const int T = mask_prefix(words, C, NW, tid, NT, wsum);
     __syncthreads();
     const int quota = (T + NT - 1) / NT;
     Walker wk;
-    wk.masks = masks; wk.tab = tab;
+    wk.words = words;
     wk.cnt = max(0, min(quota, T - tid * quota));
-    wk.m = 0u; wk.idx = 0; wk.j = 0; wk.w = 0; wk.g = 0;
-    wk.jbeg = wk.jend = wk.kbase = wk.ns = wk.pair = wk.gfirst = 0; wk.W = 1; wk.last = 1;
-    if (wk.cnt > 0) wk.seek(C, NW, ng, tid * quota);
+    wk.m = 1u; wk.d = 0u; wk.idx = 0;
+    if (wk.cnt > 0) wk.seek(C, NW, tid * quota);
     __syncthreads();
     for (int m = tid; m < WPC * 2 * capa; m += NT) acc0[m] = make_double2(0.0, 0.0);   // the aliases are dead
     __syncthreads();
@@ -220,40 +222,46 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
     double cf[REGC ? Spec::NACC : 1];                 // c_b of the lane's current pair group
 #pragma unroll
     for (int a = 0; a < (REGC ? Spec::NACC : 1); ++a) cf[a] = 0.0;
+    uint32_t dcur = 0xffffffffu;
     for (int it = 0; it < quota; ++it) {
         const bool active = wk.cnt > 0;
         wk.advance();
-        // Owner slot changed: fold the j-side sums into the slot accumulator and load the new j.  No
-        // conflict is possible inside the loop: the stream is j-major, so the lanes that share a slot j
-        // are consecutive and only the last of them leaves j before its range ends (the others flush
-        // after the loop).
-        if (active && wk.j != jcur) {
-            if (jcur >= 0) {
-                double2 a = acc.fxy[jcur];
-                double b = acc.fz[jcur];
-                a.x += fma(-Aj, J.ux, Vx); a.y += fma(-Aj, J.uy, Vy); b += fma(-Aj, J.uz, Vz);
-                acc.fxy[jcur] = a;
-                acc.fz[jcur] = b;
-            }
-            jcur = wk.j;
-            const double2 a0 = p0[jcur], a1 = p1[jcur], a2 = p2[jcur];
-            J.ux = a0.x; J.uy = a0.y; J.uz = a1.x; J.ia = a1.y; J.fa = a2.x; J.dfa = a2.y; J.e0 = e0[jcur];
-            Aj = 0.0; Vx = 0.0; Vy = 0.0; Vz = 0.0;
-        }
-        if constexpr (REGC) {
-            if (active && wk.pair != paircur) {
-                paircur = wk.pair;
-                const double2* src = reinterpret_cast<const double2*>(btc + paircur * 2 * bt2_stride<Spec>());
-#pragma unroll
-                for (int a = 0; a < Spec::NACC / 2; ++a) {
-                    const double2 c = src[a];
-                    cf[2 * a] = c.x; cf[2 * a + 1] = c.y;
+        // New mask word: maybe a new owner slot (fold the j-side sums into the slot accumulator, load the
+        // new j) and maybe a new pair group (reload the coefficients).  No conflict is possible inside the
+        // loop: the stream is j-major, so the lanes that share a slot j are consecutive and only the last
+        // of them leaves j before its range ends (the others flush after the loop).
+        if (active && wk.d != dcur) {
+            dcur = wk.d;
+            const int jn = wk.j();
+            if (jn != jcur) {
+                if (jcur >= 0) {
+                    double2 a = acc.fxy[jcur];
+                    double b = acc.fz[jcur];
+                    a.x += fma(-Aj, J.ux, Vx); a.y += fma(-Aj, J.uy, Vy); b += fma(-Aj, J.uz, Vz);
+                    acc.fxy[jcur] = a;
+                    acc.fz[jcur] = b;
                 }
-                if constexpr (Spec::NACC & 1) cf[Spec::NACC - 1] = btc[paircur * 2 * bt2_stride<Spec>() + Spec::NACC - 1];
+                jcur = jn;
+                const double2 a0 = p0[jcur], a1 = p1[jcur], a2 = p2[jcur];
+                J.ux = a0.x; J.uy = a0.y; J.uz = a1.x; J.ia = a1.y; J.fa = a2.x; J.dfa = a2.y; J.e0 = e0[jcur];
+                Aj = 0.0; Vx = 0.0; Vy = 0.0; Vz = 0.0;
+            }
+            const int pr = pair_of_slots(jn, wk.first_partner(), seg, p.n_elem);
+            if (pr != paircur) {
+                paircur = pr;
+                if constexpr (REGC) {
+                    const double2* src = reinterpret_cast<const double2*>(btc + pr * 2 * bt2_stride<Spec>());
+#pragma unroll
+                    for (int a = 0; a < Spec::NACC / 2; ++a) {
+                        const double2 c = src[a];
+                        cf[2 * a] = c.x; cf[2 * a + 1] = c.y;
+                    }
+                    if constexpr (Spec::NACC & 1) cf[Spec::NACC - 1] = btc[pr * 2 * bt2_stride<Spec>() + Spec::NACC - 1];
+                }
             }
         }
         __syncwarp();
-        const double2* btg = bt + wk.pair * bt2_stride<Spec>();
+        const double2* btg = bt + max(paircur, 0) * bt2_stride<Spec>();
         const int k = active ? wk.pop() : max(jcur, 0);
         const int rank = conflict_rank(k, active, lane);       // issued early: its latency hides behind the FP64 work
         const double2 k0 = p0[k], k1 = p1[k], k2v = p2[k];
@@ -372,24 +380,24 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
 #endif
 constexpr int F2_WPC = NNP_F2_WPC;
 
-template <class Spec>
-static int launch_one2(const Force2Params& p, cudaStream_t st) {
-    const size_t smem = force2_smem<Spec>(p.cap, p.g_stride, p.n_elem, F2_WPC);
+template <class Spec, int CAPA>
+static int launch_capa(const Force2Params& p, cudaStream_t st) {
+    const size_t smem = force2_smem<Spec>(CAPA, p.g_stride, p.n_elem, F2_WPC);
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_force2<Spec, F2_WPC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaFuncSetAttribute(k_force2<Spec, F2_WPC, CAPA>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         configured = true;
     }
-    k_force2<Spec, F2_WPC><<<(unsigned)p.n, F2_WPC * 32, smem, st>>>(p);
+    k_force2<Spec, F2_WPC, CAPA><<<(unsigned)p.n, F2_WPC * 32, smem, st>>>(p);
     return 1;
 }
 
-size_t force2_smem_bytes(int variant, int cap, int g_stride, int n_elem) {
-    switch (variant) {
-        case ANG_BASE12: return force2_smem<SpecBase12>(cap, g_stride, n_elem, F2_WPC);
-        case ANG_WIDE32: return force2_smem<SpecWide32>(cap, g_stride, n_elem, F2_WPC);
-        default: return 0;
-    }
+// slot capacity = smallest instantiated CAPA that holds max_neighbors (nnp_set_max_neighbors: 32..255)
+template <class Spec>
+static int launch_one2(const Force2Params& p, cudaStream_t st) {
+    if (p.cap <= 128) return launch_capa<Spec, 128>(p, st);
+    if (p.cap <= 160) return launch_capa<Spec, 160>(p, st);
+    return launch_capa<Spec, 256>(p, st);
 }
 
 // launches the fast kernels for the specialised variants in use; the caller has zeroed f_sorted

@@ -5,6 +5,8 @@
 // One warp per centre.  Radial and angular parts share the staged neighbourhood, so they are
 // ONE kernel here (the paper splits them, L98, because its parallel_for has no shared staging).
 // FP64-ALU bound: ~93 FP64 instructions per contributing triplet, ~1,940 triplets per atom.
+#include <cstdlib>
+
 #include "angular.cuh"
 #include "geometry.cuh"
 
@@ -268,8 +270,13 @@ int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const El
         if (e < n_elem) use[variant[e]] = true;
     }
     int launches = 0;
-    if (use[ANG_BASE12]) launches += launch_one<SpecBase12>(p, st);
-    if (use[ANG_WIDE32]) launches += launch_one<SpecWide32>(p, st);
+    static const bool queue_design = getenv("NNP_QUEUE_DESIGN") != nullptr;   // A/B switch while both designs exist
+    if (queue_design) {
+        if (use[ANG_BASE12]) launches += launch_one<SpecBase12>(p, st);
+        if (use[ANG_WIDE32]) launches += launch_one<SpecWide32>(p, st);
+    } else if (use[ANG_BASE12] || use[ANG_WIDE32]) {
+        launches += launch_sf2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, st);
+    }
     if (use[ANG_GENERIC]) launches += launch_one<SpecGeneric>(p, st);
     return launches;
 }

@@ -1,0 +1,264 @@
+// k_sf2.cu -- S2 fast path (specialised pair groups): atom-centred symmetry functions G_i, radial
+// G2 and angular G3 (PAPER.md L40 step 1; formulas: include/nnp.h at nnp_sf, readings 2-4).
+// Lane-owned design (stream.cuh), same staging / screening / stream split as k_force2.cu: one CTA of
+// WPC warps per centre; a lane keeps neighbour j in registers and gathers only the partner k.  The
+// stream is GROUP-major here, so a lane changes pair group at most (#groups - 1) times per centre: it
+// accumulates the NACC values of its current group in registers and hands them over (shared-memory
+// atomics, rare) when its group changes; at the end the lanes of a warp are reduced per group.
+#include "angular.cuh"
+#include "geometry.cuh"
+#include "stream.cuh"
+
+namespace nnp {
+
+struct Sf2Params {
+    int64_t n;
+    int n_elem, ncell, stride, cap, g_stride;
+    double rc, rc2, k2;                  // k2 = (pi / (2 rc))^2
+    double box[3], half[3];
+    const double *sx, *sy, *sz;
+    const int32_t *cell_start, *nbr, *nbr_cnt;
+    double* G;
+    const ElemProgram* prog[MAX_ELEM];
+    int variant[MAX_ELEM];
+};
+
+// Shared memory of one centre: planes p0 (ux,uy), p1 (uz,1/a), p2 (exp(-eta0 a^2), fc(a)) double2[CAPA];
+// ra (a) double[CAPA]; FP32 screening copy float4[CAPA] (the prefix array aliases it afterwards);
+// then group table, G accumulators [npair][NACC], scratch, mask words (mask + descriptor)
+template <class Spec>
+__host__ __device__ constexpr size_t sf2_smem(int capa, int n_elem) {
+    const size_t npair = (size_t)n_elem * (n_elem + 1) / 2;
+    size_t b = (size_t)capa * (3 * 16 + 8 + 16);
+    b += npair * sizeof(GroupTab);
+    b += npair * Spec::NACC * 8;
+    b += 64;
+    b += (size_t)mask_words_cap(capa, n_elem) * 8;
+    return (b + 15) / 16 * 16;
+}
+
+template <class Spec, int WPC, int CAPA>
+__global__ void __launch_bounds__(WPC * 32, 16 / WPC) k_sf2(const __grid_constant__ Sf2Params p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int NT = WPC * 32;
+    constexpr int NACC = Spec::NACC;
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int64_t i = blockIdx.x;
+    int tc = 0;
+    for (int e = 1; e < p.n_elem; ++e)
+        if (i >= p.cell_start[(size_t)e * p.ncell]) tc = e;
+    if (p.variant[tc] != Spec::ID) return;          // uniform per CTA
+    const ElemProgram* __restrict__ prog = p.prog[tc];
+
+    constexpr int capa = CAPA;
+    const int npair = p.n_elem * (p.n_elem + 1) / 2;
+    double2* p0 = reinterpret_cast<double2*>(smem_raw);     // (ux, uy)
+    double2* p1 = p0 + capa;                                // (uz, 1/a)
+    double2* p2 = p1 + capa;                                // (exp(-eta_0 a^2), fc(a))
+    double* ra = reinterpret_cast<double*>(p2 + capa);      // a
+    float4* f32 = reinterpret_cast<float4*>(ra + capa);     // screening copy
+    uint16_t* C = reinterpret_cast<uint16_t*>(f32);         // alias: prefix of the mask popcounts (after screening)
+    GroupTab* tab = reinterpret_cast<GroupTab*>(f32 + capa);
+    double* gacc = reinterpret_cast<double*>(tab + npair);  // [pair][NACC]
+    int* wsum = reinterpret_cast<int*>(gacc + npair * NACC);
+    uint2* words = reinterpret_cast<uint2*>(wsum + 16);     // (mask, descriptor)
+
+    int seg[MAX_ELEM + 1];
+    seg[0] = 0;
+#pragma unroll
+    for (int e = 0; e < MAX_ELEM; ++e) seg[e + 1] = seg[e] + p.nbr_cnt[(size_t)i * MAX_ELEM + e];
+    const int ntot = seg[MAX_ELEM];
+
+    // ---- stage the neighbourhood -------------------------------------------------------------------
+    const double xi = p.sx[i], yi = p.sy[i], zi = p.sz[i];
+    const int32_t* row = p.nbr + (size_t)i * p.stride;
+    const double eta0 = prog->ang_eta[0];
+    for (int m = tid; m < ntot; m += NT) {
+        const int j = row[m];
+        const double dx = min_image_1d(xi, p.sx[j], p.box[0], p.half[0]);
+        const double dy = min_image_1d(yi, p.sy[j], p.box[1], p.half[1]);
+        const double dz = min_image_1d(zi, p.sz[j], p.box[2], p.half[2]);
+        const double a2 = fma(dx, dx, fma(dy, dy, dz * dz));
+        const double ia = rsqrt(a2);
+        const double Ca = cos_only(a2 * p.k2);
+        p0[m] = make_double2(dx, dy);
+        p1[m] = make_double2(dz, ia);
+        p2[m] = make_double2(exp_small(-eta0 * a2), Ca * Ca);
+        ra[m] = a2 * ia;
+        f32[m] = make_float4((float)dx, (float)dy, (float)dz, 0.f);
+    }
+    for (int s = tid; s < npair * NACC; s += NT) gacc[s] = 0.0;
+    int NW = 0;
+    const int ng = build_groups<false>(seg, p.n_elem, prog->n_ang, tab, tid, NW);
+    __syncthreads();
+
+    double* Grow = p.G + (size_t)i * p.g_stride;
+    for (int s = prog->n_sf + tid; s < p.g_stride; s += NT) Grow[s] = 0.0;
+
+    // ---- radial: G = sum_j exp(-eta (a - rs)^2) fc(a) over the neighbours of element e; one warp per SF
+    for (int e = 0; e < p.n_elem; ++e) {
+        const int nr = prog->n_rad[e], off = prog->rad_off[e];
+        for (int r = wid; r < nr; r += WPC) {
+            const RadialSF f = prog->rad[off + r];
+            double acc = 0.0;
+            for (int m = seg[e] + lane; m < seg[e + 1]; m += 32) {
+                const double d = ra[m] - f.rs;
+                acc = fma(exp_small(fmax(-f.eta * d * d, -700.0)), p2[m].y, acc);
+            }
+            acc = warp_sum(acc);
+            if (lane == 0) Grow[f.g] = acc;
+        }
+    }
+
+    // ---- screening -> masks; prefix; even split of the triplet stream over the NT threads ------------
+    const float rc2f = (float)(p.rc2 * (1.0 + 1e-5));
+    for (int g = 0; g < ng; ++g) screen_group(tab[g], f32, words, rc2f, tid, NT);
+    __syncthreads();
+    const int T = mask_prefix(words, C, NW, tid, NT, wsum);
+    __syncthreads();
+    const int quota = (T + NT - 1) / NT;
+    Walker wk;
+    wk.words = words;
+    wk.cnt = max(0, min(quota, T - tid * quota));
+    wk.m = 1u; wk.d = 0u; wk.idx = 0;
+    if (wk.cnt > 0) wk.seek(C, NW, tid * quota);
+
+    // ---- angular part: every lane walks its range of the stream ---------------------------------------
+    double jx = 1.0, jy = 1.0, jz = 1.0, jia = 1.0, je0 = 1.0, jfa = 0.0;
+    int jcur = -1, paircur = -1;
+    uint32_t dcur = 0xffffffffu;
+    double acc[NACC];
+#pragma unroll
+    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    for (int it = 0; it < quota; ++it) {
+        const bool active = wk.cnt > 0;
+        wk.advance();
+        if (active && wk.d != dcur) {
+            dcur = wk.d;
+            const int jn = wk.j();
+            if (jn != jcur) {
+                jcur = jn;
+                const double2 a0 = p0[jcur], a1 = p1[jcur], a2 = p2[jcur];
+                jx = a0.x; jy = a0.y; jz = a1.x; jia = a1.y; je0 = a2.x; jfa = a2.y;
+            }
+            const int pr = pair_of_slots(jn, wk.first_partner(), seg, p.n_elem);
+            if (pr != paircur) {
+                // the lane enters another pair group (at most #groups - 1 times per centre): hand the sums over
+                if (paircur >= 0) {
+#pragma unroll
+                    for (int a = 0; a < NACC; ++a) {
+                        atomicAdd(&gacc[paircur * NACC + a], acc[a]);
+                        acc[a] = 0.0;
+                    }
+                }
+                paircur = pr;
+            }
+        }
+        const int k = active ? wk.pop() : max(jcur, 0);
+        const double2 k0 = p0[k], k1 = p1[k], k2v = p2[k];
+        const double wx = k0.x - jx, wy = k0.y - jy, wz = k1.x - jz;
+        const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
+        const double Cc = cos_only(c2 * p.k2);
+        double Cf = (jfa * k2v.y) * (Cc * Cc);      // fc(a) fc(b) fc(c), fc(c) = cos^2(pi c / (2 rc))
+        if (!active || !(c2 < p.rc2)) Cf = 0.0;     // exact cutoff (the masks were screened in FP32)
+        double Y[Spec::NETA];
+        Y[0] = (je0 * k2v.x) * exp_small(-eta0 * c2);
+        if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
+        if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
+        if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
+        const double cosv = fma(jx, k0.x, fma(jy, k0.y, jz * k1.x)) * (jia * k1.y);
+        double pw[2][Spec::MAXBIT + 1];
+        pw[0][0] = 1.0 + cosv;
+        pw[1][0] = 1.0 - cosv;
+#pragma unroll
+        for (int b = 1; b <= Spec::MAXBIT; ++b) {
+            pw[0][b] = pw[0][b - 1] * pw[0][b - 1];
+            pw[1][b] = pw[1][b - 1] * pw[1][b - 1];
+        }
+#pragma unroll
+        for (int e = 0; e < Spec::NETA; ++e) {
+            const double xc = Y[e] * Cf;
+#pragma unroll
+            for (int b = 0; b <= Spec::MAXBIT; ++b) {
+                if (Spec::mask(e) >> b & 1u) acc[acc_index<Spec>(e, b)] = fma(pw[0][b], xc, acc[acc_index<Spec>(e, b)]);
+                if (Spec::mask(e) >> (8 + b) & 1u)
+                    acc[acc_index<Spec>(e, 8 + b)] = fma(pw[1][b], xc, acc[acc_index<Spec>(e, 8 + b)]);
+            }
+        }
+    }
+    // ---- reduce: per pair group present in the warp, sum the lanes that ended in it -------------------
+    for (int pr = 0; pr < npair; ++pr) {
+        if (!__any_sync(FULL, paircur == pr)) continue;
+#pragma unroll
+        for (int a = 0; a < NACC; ++a) {
+            const double v = warp_sum(paircur == pr ? acc[a] : 0.0);
+            if (lane == 0) atomicAdd(&gacc[pr * NACC + a], v);
+        }
+    }
+    __syncthreads();
+    // ---- G = 2^(1-zeta) * sum ---------------------------------------------------------------------------
+    for (int s = tid; s < npair * 16 * Spec::NETA; s += NT) {
+        const int pr = s / (16 * Spec::NETA), rem = s - pr * 16 * Spec::NETA;
+        const int e = rem >> 4, b = rem & 15;
+        bool on = false;
+        int a = 0;
+#pragma unroll
+        for (int ee = 0; ee < Spec::NETA; ++ee) {
+            const unsigned mk = Spec::mask(ee);
+            if (ee < e) a += __popc(mk);
+            else if (ee == e) { a += __popc(mk & ((1u << b) - 1u)); on = (mk >> b) & 1u; }
+        }
+        if (!on || prog->n_ang[pr] == 0) continue;
+        const int g = prog->ang_g[pr][e][b];
+        if (g >= 0) Grow[g] = exp2((double)(1 - (1 << (b & 7)))) * gacc[pr * NACC + a];
+    }
+}
+
+#ifndef NNP_SF2_WPC
+#define NNP_SF2_WPC 2
+#endif
+constexpr int SF2_WPC = NNP_SF2_WPC;
+
+template <class Spec, int CAPA>
+static int launch_capa_sf(const Sf2Params& p, cudaStream_t st) {
+    const size_t smem = sf2_smem<Spec>(CAPA, p.n_elem);
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(k_sf2<Spec, SF2_WPC, CAPA>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        configured = true;
+    }
+    k_sf2<Spec, SF2_WPC, CAPA><<<(unsigned)p.n, SF2_WPC * 32, smem, st>>>(p);
+    return 1;
+}
+
+template <class Spec>
+static int launch_one_sf2(const Sf2Params& p, cudaStream_t st) {
+    if (p.cap <= 128) return launch_capa_sf<Spec, 128>(p, st);
+    if (p.cap <= 160) return launch_capa_sf<Spec, 160>(p, st);
+    return launch_capa_sf<Spec, 256>(p, st);
+}
+
+// launches the fast kernels for the specialised variants in use
+int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
+               const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st) {
+    if (n == 0) return 0;
+    Sf2Params p;
+    p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride;
+    p.rc = rc; p.rc2 = rc * rc;
+    p.k2 = (3.14159265358979323846 / (2.0 * rc)) * (3.14159265358979323846 / (2.0 * rc));
+    for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
+    p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
+    p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.G = w.G;
+    bool use[3] = {false, false, false};
+    for (int e = 0; e < MAX_ELEM; ++e) {
+        p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
+        p.variant[e] = e < n_elem ? variant[e] : -1;
+        if (e < n_elem) use[variant[e]] = true;
+    }
+    int launches = 0;
+    if (use[ANG_BASE12]) launches += launch_one_sf2<SpecBase12>(p, st);
+    if (use[ANG_WIDE32]) launches += launch_one_sf2<SpecWide32>(p, st);
+    return launches;
+}
+
+}  // namespace nnp

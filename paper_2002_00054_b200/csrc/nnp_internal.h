@@ -115,6 +115,9 @@ int launch_mlp(const Workspace& w, int64_t n, int n_elem, int ncell, const NetDe
                cudaStream_t st);
 int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
                  const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st);
+// fast path of S2 (lane-owned design, k_sf2.cu): specialised variants only
+int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
+               const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st);
 // fast path of S4 (lane-owned design, k_force2.cu): specialised variants only; f_sorted already zeroed
 int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
                   const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st);

@@ -13,6 +13,11 @@
 //     so every lane evaluates ceil(T/NT) triplets whatever the pass rate is;
 //   * a lane walks its range bit by bit: j stays in registers until the mask of the next j starts
 //     (data of j reloaded, j-side force sum flushed), only the partner k is gathered.
+// Every mask word carries a 32-bit DESCRIPTOR (owner slot j, first partner slot, wrap bound and
+// modulus), so that walking needs no group table: with 32 lanes on 32 different ranges, SOME lane
+// moves to its next word or its next j in almost every iteration, and such a rare-per-lane step costs
+// the whole warp its instructions (ncu r1b: ~100 of ~220 instructions per iteration of the first
+// version were this bookkeeping).
 // A pair group is either WITHIN one element segment (tournament: bit r-1 of slot j pairs it with
 // slot (j + r) mod ns, r = 1..ns/2, each unordered pair once) or BETWEEN two segments (bit q of
 // slot j of the first pairs it with slot q of the second).
@@ -44,8 +49,10 @@ struct GroupTab {
 };
 
 // upper bound of the mask words of one centre with at most `cap` neighbours of `n_elem` elements:
-// within: ns * ceil(floor(ns/2)/32) <= ns (ns/64 + 1); between: n1 * ceil(n2/32) <= n1 (n2/32 + 1)
-__host__ __device__ constexpr int mask_words_cap(int cap, int n_elem) { return cap * cap / 64 + cap * n_elem + 8; }
+// within: ns * ceil(floor(ns/2)/32) <= ns (ns/64 + 1); between: n1 * ceil(n2/32) <= n1 (n2/32 + 1);
+// summed over the groups: <= n^2/64 + n * n_elem.  (The u16 prefix array of the kernels aliases a
+// 16 B-per-slot region: 2 * (n^2/64 + 4 n) <= 16 * capacity holds for n <= 255.)
+__host__ __device__ constexpr int mask_words_cap(int cap, int n_elem) { return cap * cap / 64 + cap * n_elem; }
 
 // Builds the group table of the centre (uniform code; every thread computes the same, thread 0 stores).
 // n_ang[pr] != 0 marks pair groups that have angular symmetry functions.  Returns #groups; NW out.
@@ -89,11 +96,22 @@ __device__ __forceinline__ bool close32(const float4 a, const float4 b, float rc
     return fmaf(wx, wx, fmaf(wy, wy, wz * wz)) < rc2f;
 }
 
+// descriptor of mask word w of owner slot j = jbeg + jl:  j | first partner << 8 | wrap bound << 16 | modulus << 24;
+// bit b of the word pairs j with slot k = first + b, minus the modulus if k >= wrap bound
+__device__ __forceinline__ uint32_t word_desc(const GroupTab& g, int jl, int w) {
+    if (g.ns > 0) {
+        int kb = jl + 32 * w + 1;
+        if (kb >= g.ns) kb -= g.ns;
+        return (uint32_t)(g.jbeg + jl) | (uint32_t)(g.jbeg + kb) << 8 | (uint32_t)(g.jbeg + g.ns) << 16 | (uint32_t)g.ns << 24;
+    }
+    return (uint32_t)(g.jbeg + jl) | (uint32_t)(g.kbase + 32 * w) << 8 | 255u << 16;
+}
+
 // Screening of one group: FP32 test |u_k - u_j|^2 < rc^2 (1 + 1e-5) (never drops a contributing pair; the
-// evaluation applies the exact FP64 test) -> masks[woff + (j - jbeg) stride + word].  Thread t owns slot
-// j = jbeg + t (+nt, ...) in registers; within a group its partner walks (j + r) mod ns (distinct
-// consecutive addresses), between groups all lanes test the same partner (broadcast load).
-__device__ __forceinline__ void screen_group(const GroupTab g, const float4* f32, uint32_t* masks, float rc2f, int tid,
+// evaluation applies the exact FP64 test) -> words[woff + (j - jbeg) stride + w] = (mask, descriptor).
+// Thread t owns slot j = jbeg + t (+nt, ...) in registers; within a group its partner walks (j + r) mod ns
+// (distinct consecutive addresses), between groups all lanes test the same partner (broadcast load).
+__device__ __forceinline__ void screen_group(const GroupTab g, const float4* f32, uint2* words, float rc2f, int tid,
                                              int nt) {
     const int nj = g.jend - g.jbeg;
     const int R = g.nk;
@@ -101,7 +119,7 @@ __device__ __forceinline__ void screen_group(const GroupTab g, const float4* f32
         const int jl = jb + (tid & 31);
         const bool vj = jl < nj;
         const float4 a = f32[g.jbeg + (vj ? jl : 0)];
-        uint32_t* dst = masks + g.woff + jl * g.stride;
+        uint2* dst = words + g.woff + jl * g.stride;
         uint32_t word = 0, bit = 1u;
         if (g.ns > 0) {
             // tournament inside the segment: round t pairs j with (j + t + 1) mod ns; with an even ns the
@@ -116,7 +134,7 @@ __device__ __forceinline__ void screen_group(const GroupTab g, const float4* f32
                 if (close32(a, src[kl], rc2f)) word |= bit;
                 bit <<= 1;
                 if ((t & 31) == 31) {
-                    if (vj) dst[t >> 5] = word;
+                    if (vj) dst[t >> 5] = make_uint2(word, word_desc(g, jl, t >> 5));
                     word = 0; bit = 1u;
                 }
             }
@@ -125,31 +143,30 @@ __device__ __forceinline__ void screen_group(const GroupTab g, const float4* f32
                 if (kl >= ns) kl -= ns;
                 if (jl < R && close32(a, src[kl], rc2f)) word |= bit;
             }
-            if (vj && (R & 31) != 0) dst[(R - 1) >> 5] = word;
-            else if (vj && Rfull < R) dst[(R - 1) >> 5] = word;
+            if (vj && ((R & 31) != 0 || Rfull < R)) dst[(R - 1) >> 5] = make_uint2(word, word_desc(g, jl, (R - 1) >> 5));
         } else {
             const float4* src = f32 + g.kbase;
             for (int t = 0; t < R; ++t) {
                 if (close32(a, src[t], rc2f)) word |= bit;       // uniform address: broadcast
                 bit <<= 1;
                 if ((t & 31) == 31) {
-                    if (vj) dst[t >> 5] = word;
+                    if (vj) dst[t >> 5] = make_uint2(word, word_desc(g, jl, t >> 5));
                     word = 0; bit = 1u;
                 }
             }
-            if (vj && (R & 31) != 0) dst[(R - 1) >> 5] = word;
+            if (vj && (R & 31) != 0) dst[(R - 1) >> 5] = make_uint2(word, word_desc(g, jl, (R - 1) >> 5));
         }
     }
 }
 
 // Exclusive prefix of the mask popcounts -> C[0..NW) (u16; T <= 255*254/2 fits); returns T.
 // Block-wide: nt = 32 * nwarp threads; wsum = nwarp ints of shared scratch.  Contains __syncthreads.
-__device__ __forceinline__ int mask_prefix(const uint32_t* masks, uint16_t* C, int NW, int tid, int nt, int* wsum) {
+__device__ __forceinline__ int mask_prefix(const uint2* words, uint16_t* C, int NW, int tid, int nt, int* wsum) {
     const int lane = tid & 31, wid = tid >> 5, nwarp = nt >> 5;
     const int chunk = (NW + nt - 1) / nt;
     const int beg = min(tid * chunk, NW), end = min(beg + chunk, NW);
     int s = 0;
-    for (int x = beg; x < end; ++x) s += __popc(masks[x]);
+    for (int x = beg; x < end; ++x) s += __popc(words[x].x);
     int incl = s;
 #pragma unroll
     for (int d = 1; d < 32; d <<= 1) {
@@ -167,85 +184,62 @@ __device__ __forceinline__ int mask_prefix(const uint32_t* masks, uint16_t* C, i
     int run = base + incl - s;
     for (int x = beg; x < end; ++x) {
         C[x] = (uint16_t)run;
-        run += __popc(masks[x]);
+        run += __popc(words[x].x);
     }
     return total;
 }
 
 // A lane's position in the triplet stream.
 struct Walker {
-    const uint32_t* masks;
-    const GroupTab* tab;
-    int idx, j, w, g;                  // current mask word: index, owner slot, word-in-group, group
-    int jbeg, jend, kbase, ns, W, pair, gfirst, last;
-    uint32_t m;                        // bits of the current word not yet visited
-    int cnt;                           // triplets left for this lane
+    const uint2* words;
+    int idx;          // current word
+    uint32_t m;       // bits of the current word not yet visited (kept non-zero once the lane is done)
+    uint32_t d;       // descriptor of the current word
+    int cnt;          // triplets left for this lane
 
-    __device__ __forceinline__ void load_group() {
-        const int4 a = reinterpret_cast<const int4*>(tab + g)[0];
-        const int4 b = reinterpret_cast<const int4*>(tab + g)[1];
-        const int4 c = reinterpret_cast<const int4*>(tab + g)[2];
-        jbeg = a.x; jend = a.y; kbase = a.z; ns = a.w; W = b.x; pair = b.y; gfirst = c.y; last = c.z;
-    }
+    __device__ __forceinline__ int j() const { return (int)(d & 255u); }
+    __device__ __forceinline__ int first_partner() const { return (int)((d >> 8) & 255u); }
 
     // position the lane at triplet number S of the stream (cnt > 0 required)
-    __device__ __forceinline__ void seek(const uint16_t* C, int NW, int ng, int S) {
+    __device__ __forceinline__ void seek(const uint16_t* C, int NW, int S) {
         int lo = 0, hi = NW - 1;                   // largest idx with C[idx] <= S
         while (lo < hi) {
             const int mid = (lo + hi + 1) >> 1;
             if ((int)C[mid] <= S) lo = mid; else hi = mid - 1;
         }
         idx = lo;
-        m = masks[idx];
+        const uint2 w = words[idx];
+        m = w.x;
+        d = w.y;
         for (int s = S - (int)C[idx]; s > 0; --s) m &= m - 1;
-        int g0 = 0;                                // block: last block head whose first word is <= idx
-        for (int t = 1; t < ng; ++t)
-            if (tab[t].gfirst == t && tab[t].woff <= idx) g0 = t;
-        const int base = tab[g0].woff, stride = tab[g0].stride;
-        const int rel = idx - base;
-        const int jl = rel / stride;
-        const int r2 = rel - jl * stride;
-        g = g0;                                    // group inside the block: last one starting at or before r2
-        for (int t = g0 + 1; t < ng; ++t)
-            if (tab[t].gfirst == g0 && tab[t].woff - base <= r2) g = t;
-        load_group();
-        w = r2 - (tab[g].woff - base);
-        j = jbeg + jl;
     }
 
-    // move the lane, if it has run out of bits and still has triplets to do, to its next non-empty
-    // word (plain divergent loop: no warp-synchronous operation inside)
+    // move the lane to its next non-empty word if it has run out of bits (plain divergent loop)
     __device__ __forceinline__ void advance() {
-        if (cnt > 0) {
-            while (m == 0u) {
-                ++idx; ++w;
-                if (w == W) {
-                    w = 0;
-                    if (!last) { ++g; load_group(); }            // same j, next group of the block
-                    else {
-                        ++j;
-                        if (j == jend) { ++g; load_group(); j = jbeg; }      // next block
-                        else if (g != gfirst) { g = gfirst; load_group(); }  // next j, first group of the block
-                    }
-                }
-                m = masks[idx];
-            }
+        while (m == 0u) {
+            ++idx;
+            const uint2 w = words[idx];
+            m = w.x;
+            d = w.y;
         }
     }
 
-    // pop the next triplet of the lane: partner slot k (m != 0 required)
+    // pop the next triplet of the lane: partner slot k
     __device__ __forceinline__ int pop() {
         const int b = __ffs(m) - 1;
         m &= m - 1;
-        --cnt;
-        const int t = (w << 5) + b;
-        if (ns > 0) {
-            int kl = j - jbeg + t + 1;
-            if (kl >= ns) kl -= ns;
-            return jbeg + kl;
-        }
-        return kbase + t;
+        if (--cnt == 0) m = 1u;                    // done: never advance past the lane's range
+        int k = (int)((d >> 8) & 255u) + b;
+        if (k >= (int)((d >> 16) & 255u)) k -= (int)(d >> 24);
+        return k;
     }
 };
+
+// pair-group index of (owner slot j, partner slot k) from the segment boundaries (element of j <= element of k)
+__device__ __forceinline__ int pair_of_slots(int j, int k, const int* seg, int n_elem) {
+    const int ej = (j >= seg[1]) + (j >= seg[2]) + (j >= seg[3]);
+    const int ek = (k >= seg[1]) + (k >= seg[2]) + (k >= seg[3]);
+    return pair_index(ej, ek, n_elem);
+}
 
 }  // namespace nnp
