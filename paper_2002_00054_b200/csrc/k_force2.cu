@@ -246,7 +246,7 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
                 J.ux = a0.x; J.uy = a0.y; J.uz = a1.x; J.ia = a1.y; J.fa = a2.x; J.dfa = a2.y; J.e0 = e0[jcur];
                 Aj = 0.0; Vx = 0.0; Vy = 0.0; Vz = 0.0;
             }
-            const int pr = pair_of_slots(jn, wk.first_partner(), seg, p.n_elem);
+            const int pr = p.n_elem <= 2 ? wk.pair2() : pair_of_slots(jn, wk.first_partner(), seg, p.n_elem);
             if (pr != paircur) {
                 paircur = pr;
                 if constexpr (REGC) {

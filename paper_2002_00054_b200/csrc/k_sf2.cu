@@ -27,11 +27,11 @@ struct Sf2Params {
 // ra (a) double[CAPA]; FP32 screening copy float4[CAPA] (the prefix array aliases it afterwards);
 // then group table, G accumulators [npair][NACC], scratch, mask words (mask + descriptor)
 template <class Spec>
-__host__ __device__ constexpr size_t sf2_smem(int capa, int n_elem) {
+__host__ __device__ constexpr size_t sf2_smem(int capa, int n_elem, int wpc) {
     const size_t npair = (size_t)n_elem * (n_elem + 1) / 2;
     size_t b = (size_t)capa * (3 * 16 + 8 + 16);
     b += npair * sizeof(GroupTab);
-    b += npair * Spec::NACC * 8;
+    b += (size_t)(wpc + 1) * npair * Spec::NACC * 8;
     b += 64;
     b += (size_t)mask_words_cap(capa, n_elem) * 8;
     return (b + 15) / 16 * 16;
@@ -59,8 +59,11 @@ __global__ void __launch_bounds__(WPC * 32, 16 / WPC) k_sf2(const __grid_constan
     float4* f32 = reinterpret_cast<float4*>(ra + capa);     // screening copy
     uint16_t* C = reinterpret_cast<uint16_t*>(f32);         // alias: prefix of the mask popcounts (after screening)
     GroupTab* tab = reinterpret_cast<GroupTab*>(f32 + capa);
-    double* gacc = reinterpret_cast<double*>(tab + npair);  // [pair][NACC]
-    int* wsum = reinterpret_cast<int*>(gacc + npair * NACC);
+    // [WPC + 1][pair][NACC]: set 0 = sums handed over by the one lane that leaves a group inside its range,
+    // set 1 + w = sums of the lanes of warp w that end in the group; added in this fixed order (the energies
+    // must not depend on scheduling)
+    double* gacc = reinterpret_cast<double*>(tab + npair);
+    int* wsum = reinterpret_cast<int*>(gacc + (WPC + 1) * npair * NACC);
     uint2* words = reinterpret_cast<uint2*>(wsum + 16);     // (mask, descriptor)
 
     int seg[MAX_ELEM + 1];
@@ -87,7 +90,7 @@ __global__ void __launch_bounds__(WPC * 32, 16 / WPC) k_sf2(const __grid_constan
         ra[m] = a2 * ia;
         f32[m] = make_float4((float)dx, (float)dy, (float)dz, 0.f);
     }
-    for (int s = tid; s < npair * NACC; s += NT) gacc[s] = 0.0;
+    for (int s = tid; s < (WPC + 1) * npair * NACC; s += NT) gacc[s] = 0.0;
     int NW = 0;
     const int ng = build_groups<false>(seg, p.n_elem, prog->n_ang, tab, tid, NW);
     __syncthreads();
@@ -141,13 +144,15 @@ __global__ void __launch_bounds__(WPC * 32, 16 / WPC) k_sf2(const __grid_constan
                 const double2 a0 = p0[jcur], a1 = p1[jcur], a2 = p2[jcur];
                 jx = a0.x; jy = a0.y; jz = a1.x; jia = a1.y; je0 = a2.x; jfa = a2.y;
             }
-            const int pr = pair_of_slots(jn, wk.first_partner(), seg, p.n_elem);
+            const int pr = p.n_elem <= 2 ? wk.pair2() : pair_of_slots(jn, wk.first_partner(), seg, p.n_elem);
             if (pr != paircur) {
-                // the lane enters another pair group (at most #groups - 1 times per centre): hand the sums over
+                // The lane enters another pair group: hand the sums over.  Only ONE lane of the CTA leaves a
+                // given group inside its range (the group-major stream is split into contiguous ranges),
+                // so this is a plain store.
                 if (paircur >= 0) {
 #pragma unroll
                     for (int a = 0; a < NACC; ++a) {
-                        atomicAdd(&gacc[paircur * NACC + a], acc[a]);
+                        gacc[paircur * NACC + a] = acc[a];
                         acc[a] = 0.0;
                     }
                 }
@@ -192,7 +197,7 @@ __global__ void __launch_bounds__(WPC * 32, 16 / WPC) k_sf2(const __grid_constan
 #pragma unroll
         for (int a = 0; a < NACC; ++a) {
             const double v = warp_sum(paircur == pr ? acc[a] : 0.0);
-            if (lane == 0) atomicAdd(&gacc[pr * NACC + a], v);
+            if (lane == 0) gacc[((1 + wid) * npair + pr) * NACC + a] = v;
         }
     }
     __syncthreads();
@@ -210,7 +215,12 @@ __global__ void __launch_bounds__(WPC * 32, 16 / WPC) k_sf2(const __grid_constan
         }
         if (!on || prog->n_ang[pr] == 0) continue;
         const int g = prog->ang_g[pr][e][b];
-        if (g >= 0) Grow[g] = exp2((double)(1 - (1 << (b & 7)))) * gacc[pr * NACC + a];
+        if (g >= 0) {
+            double tot = gacc[pr * NACC + a];
+#pragma unroll
+            for (int w = 0; w < WPC; ++w) tot += gacc[((1 + w) * npair + pr) * NACC + a];
+            Grow[g] = exp2((double)(1 - (1 << (b & 7)))) * tot;
+        }
     }
 }
 
@@ -221,7 +231,7 @@ constexpr int SF2_WPC = NNP_SF2_WPC;
 
 template <class Spec, int CAPA>
 static int launch_capa_sf(const Sf2Params& p, cudaStream_t st) {
-    const size_t smem = sf2_smem<Spec>(CAPA, p.n_elem);
+    const size_t smem = sf2_smem<Spec>(CAPA, p.n_elem, SF2_WPC);
     static bool configured = false;
     if (!configured) {
         cudaFuncSetAttribute(k_sf2<Spec, SF2_WPC, CAPA>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);

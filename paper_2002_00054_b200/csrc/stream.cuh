@@ -96,15 +96,22 @@ __device__ __forceinline__ bool close32(const float4 a, const float4 b, float rc
     return fmaf(wx, wx, fmaf(wy, wy, wz * wz)) < rc2f;
 }
 
-// descriptor of mask word w of owner slot j = jbeg + jl:  j | first partner << 8 | wrap bound << 16 | modulus << 24;
-// bit b of the word pairs j with slot k = first + b, minus the modulus if k >= wrap bound
+// Descriptor of mask word w of owner slot j = jbeg + jl:
+//     j | first << 8 | alt << 16 | bw << 24 | pair << 30
+// Bit b of the word pairs j with slot  k = (b + (b < bw ? first : alt)) & 255:  `first` is the partner of
+// bit 0, bw the first bit that wraps round the end of the segment (32 = none) and alt = segment start - bw
+// (mod 256).  The pair-group index fits the two spare bits when there are at most two elements (three
+// groups); with more elements the kernels derive it from the slots (pair_of_slots).
 __device__ __forceinline__ uint32_t word_desc(const GroupTab& g, int jl, int w) {
+    const uint32_t hi = (uint32_t)(g.pair & 3) << 30;
     if (g.ns > 0) {
         int kb = jl + 32 * w + 1;
         if (kb >= g.ns) kb -= g.ns;
-        return (uint32_t)(g.jbeg + jl) | (uint32_t)(g.jbeg + kb) << 8 | (uint32_t)(g.jbeg + g.ns) << 16 | (uint32_t)g.ns << 24;
+        const int bw = min(g.ns - kb, 32);
+        return (uint32_t)(g.jbeg + jl) | (uint32_t)(g.jbeg + kb) << 8 | (uint32_t)((g.jbeg - bw) & 255) << 16 |
+               (uint32_t)bw << 24 | hi;
     }
-    return (uint32_t)(g.jbeg + jl) | (uint32_t)(g.kbase + 32 * w) << 8 | 255u << 16;
+    return (uint32_t)(g.jbeg + jl) | (uint32_t)(g.kbase + 32 * w) << 8 | 32u << 24 | hi;
 }
 
 // Screening of one group: FP32 test |u_k - u_j|^2 < rc^2 (1 + 1e-5) (never drops a contributing pair; the
@@ -199,6 +206,7 @@ struct Walker {
 
     __device__ __forceinline__ int j() const { return (int)(d & 255u); }
     __device__ __forceinline__ int first_partner() const { return (int)((d >> 8) & 255u); }
+    __device__ __forceinline__ int pair2() const { return (int)(d >> 30); }     // valid when n_elem <= 2
 
     // position the lane at triplet number S of the stream (cnt > 0 required)
     __device__ __forceinline__ void seek(const uint16_t* C, int NW, int S) {
@@ -229,9 +237,8 @@ struct Walker {
         const int b = __ffs(m) - 1;
         m &= m - 1;
         if (--cnt == 0) m = 1u;                    // done: never advance past the lane's range
-        int k = (int)((d >> 8) & 255u) + b;
-        if (k >= (int)((d >> 16) & 255u)) k -= (int)(d >> 24);
-        return k;
+        const uint32_t sel = b < (int)((d >> 24) & 63u) ? d >> 8 : d >> 16;
+        return (int)((sel + (uint32_t)b) & 255u);
     }
 };
 
