@@ -86,6 +86,49 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
+// Sum N (power of two, <= 32) per-lane values over the warp with N - 1 + log2(32 / N) 64-bit shuffles
+// instead of 5 N: at every step a lane keeps one half of its values and hands the other half to its
+// partner.  On return s[0] of lane l holds the total of value index  vi = sum_t bit_(4-t)(l) * (N >> (t+1))
+// (warp_reduce_index), in every lane of the group that shares those bits.  Fixed order -> deterministic.
+template <int N>
+__device__ __forceinline__ void warp_reduce_multi(double (&s)[N], int lane) {
+    static_assert(N == 1 || N == 2 || N == 4 || N == 8 || N == 16 || N == 32, "N must be a power of two");
+    int width = N, delta = 16;
+#pragma unroll
+    for (int step = 0; step < 5; ++step) {
+        if (width > 1) {
+            const int half = width >> 1;
+            const bool hi = (lane & delta) != 0;
+#pragma unroll
+            for (int t = 0; t < N / 2; ++t) {
+                if (t < half) {
+                    const double mine = hi ? s[half + t] : s[t];
+                    const double other = hi ? s[t] : s[half + t];
+                    s[t] = mine + __shfl_xor_sync(0xffffffffu, other, delta);
+                }
+            }
+            width = half;
+        } else {
+            s[0] += __shfl_xor_sync(0xffffffffu, s[0], delta);
+        }
+        delta >>= 1;
+    }
+}
+
+template <int N>
+__device__ __forceinline__ int warp_reduce_index(int lane) {
+    int vi = 0, width = N, delta = 16;
+#pragma unroll
+    for (int step = 0; step < 5; ++step) {
+        if (width > 1) {
+            width >>= 1;
+            if (lane & delta) vi += width;
+        }
+        delta >>= 1;
+    }
+    return vi;
+}
+
 // ---------------------------------------------------------------- per-warp neighbourhood in smem
 // Slot m (0..n-1) of the centre's neighbour row, grouped by element.  Packed as double2 so the
 // per-triplet gathers are 128-bit shared loads.  A second, FP32 copy of the min-image vectors

@@ -38,7 +38,7 @@ __host__ __device__ constexpr size_t sf2_smem(int capa, int n_elem, int wpc) {
 }
 
 template <class Spec, int WPC, int CAPA>
-__global__ void __launch_bounds__(WPC * 32, 16 / WPC) k_sf2(const __grid_constant__ Sf2Params p) {
+__global__ void __launch_bounds__(WPC * 32, (Spec::NACC <= 12 ? 24 : 16) / WPC) k_sf2(const __grid_constant__ Sf2Params p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NT = WPC * 32;
     constexpr int NACC = Spec::NACC;
@@ -192,13 +192,15 @@ __global__ void __launch_bounds__(WPC * 32, 16 / WPC) k_sf2(const __grid_constan
         }
     }
     // ---- reduce: per pair group present in the warp, sum the lanes that ended in it -------------------
+    constexpr int NR = NACC <= 16 ? 16 : 32;
     for (int pr = 0; pr < npair; ++pr) {
         if (!__any_sync(FULL, paircur == pr)) continue;
+        double v[NR];
 #pragma unroll
-        for (int a = 0; a < NACC; ++a) {
-            const double v = warp_sum(paircur == pr ? acc[a] : 0.0);
-            if (lane == 0) gacc[((1 + wid) * npair + pr) * NACC + a] = v;
-        }
+        for (int a = 0; a < NR; ++a) v[a] = (a < NACC && paircur == pr) ? acc[a < NACC ? a : 0] : 0.0;
+        warp_reduce_multi<NR>(v, lane);
+        const int a = warp_reduce_index<NR>(lane);
+        if ((lane & (32 / NR - 1)) == 0 && a < NACC) gacc[((1 + wid) * npair + pr) * NACC + a] = v[0];
     }
     __syncthreads();
     // ---- G = 2^(1-zeta) * sum ---------------------------------------------------------------------------
