@@ -33,6 +33,9 @@ struct Force2Params {
     const int32_t *cell_start, *nbr, *nbr_cnt;
     const double* dEdG;
     double* f_sorted;
+    const int64_t* word_off;             // masks from the SF kernel (see Workspace::gmask)
+    const uint32_t* gmask;
+    int64_t gmask_cap;
     const ElemProgram* prog[MAX_ELEM];
     int variant[MAX_ELEM];
 };
@@ -134,6 +137,15 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
     const int ntot = seg[MAX_ELEM];
 
     for (int s = tid; s < p.g_stride; s += NT) brow[s] = p.dEdG[(size_t)i * p.g_stride + s];
+    // The SF kernel has screened this centre already (Workspace::gmask): fetch its mask words now, so that
+    // the global-memory latency hides behind the staging below (consumed after the group table exists).
+    constexpr int NPRE = 6;                                   // words per thread kept in registers
+    const int64_t moff = p.word_off[i];
+    const int nwg = (int)(p.word_off[i + 1] - moff);
+    const bool have_masks = moff + nwg <= p.gmask_cap;
+    uint32_t pre[NPRE];
+#pragma unroll
+    for (int r = 0; r < NPRE; ++r) pre[r] = (have_masks && tid + r * NT < nwg) ? p.gmask[moff + tid + r * NT] : 0u;
     __syncthreads();
 
     // ---- stage the neighbourhood; radial part R = sum_r beta_r exp(-eta d^2) (fc'(a) - 2 eta d fc(a)) / a
@@ -197,7 +209,25 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
 
     // ---- screening -> masks; prefix; even split of the triplet stream over the NT threads ------------
     const float rc2f = (float)(p.rc2 * (1.0 + 1e-5));
-    for (int g = 0; g < ng; ++g) screen_group(tab[g], f32, words, rc2f, tid, NT);
+    if (have_masks) {
+        // masks arrive in the SF kernel's group-major order; place them j-major and rebuild the descriptors
+#pragma unroll
+        for (int r = 0; r < NPRE; ++r) {
+            const int y = tid + r * NT;
+            if (y < NW) {
+                int g, jl, w;
+                decode_gmajor(tab, ng, y, g, jl, w);
+                words[tab[g].woff + jl * tab[g].stride + w] = make_uint2(pre[r], word_desc(tab[g], jl, w));
+            }
+        }
+        for (int y = tid + NPRE * NT; y < NW; y += NT) {
+            int g, jl, w;
+            decode_gmajor(tab, ng, y, g, jl, w);
+            words[tab[g].woff + jl * tab[g].stride + w] = make_uint2(p.gmask[moff + y], word_desc(tab[g], jl, w));
+        }
+    } else {
+        for (int g = 0; g < ng; ++g) screen_group(tab[g], f32, words, rc2f, tid, NT);
+    }
     __syncthreads();
     const int T = mask_prefix(words, C, NW, tid, NT, wsum);
     __syncthreads();
@@ -411,6 +441,7 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
     for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.dEdG = w.dEdG; p.f_sorted = w.f_sorted;
+    p.word_off = w.word_off; p.gmask = w.gmask; p.gmask_cap = w.gmask_cap;
     bool use[3] = {false, false, false};
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;

@@ -19,6 +19,9 @@ struct Sf2Params {
     const double *sx, *sy, *sz;
     const int32_t *cell_start, *nbr, *nbr_cnt;
     double* G;
+    const int64_t* word_off;             // mask export (see Workspace::gmask)
+    uint32_t* gmask;
+    int64_t gmask_cap;
     const ElemProgram* prog[MAX_ELEM];
     int variant[MAX_ELEM];
 };
@@ -117,6 +120,12 @@ __global__ void __launch_bounds__(WPC * 32, (Spec::NACC <= 12 ? 24 : 16) / WPC) 
     const float rc2f = (float)(p.rc2 * (1.0 + 1e-5));
     for (int g = 0; g < ng; ++g) screen_group(tab[g], f32, words, rc2f, tid, NT);
     __syncthreads();
+    // hand the masks to the force kernel (this kernel's group-major order), if they fit the budget
+    {
+        const int64_t off = p.word_off[i];
+        if (off + NW <= p.gmask_cap)
+            for (int x = tid; x < NW; x += NT) p.gmask[off + x] = words[x].x;
+    }
     const int T = mask_prefix(words, C, NW, tid, NT, wsum);
     __syncthreads();
     const int quota = (T + NT - 1) / NT;
@@ -226,6 +235,34 @@ __global__ void __launch_bounds__(WPC * 32, (Spec::NACC <= 12 ? 24 : 16) / WPC) 
     }
 }
 
+// ---- mask words per centre and their prefix -----------------------------------------------------------
+__global__ void __launch_bounds__(256)
+k_count_words(int64_t n, int n_elem, int ncell, const int32_t* __restrict__ cell_start,
+              const int32_t* __restrict__ nbr_cnt, const ElemProgram* p0, const ElemProgram* p1, const ElemProgram* p2,
+              const ElemProgram* p3, int32_t* __restrict__ nw) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    int tc = 0;
+    for (int e = 1; e < n_elem; ++e)
+        if (i >= cell_start[(size_t)e * ncell]) tc = e;
+    const ElemProgram* prog = tc == 0 ? p0 : (tc == 1 ? p1 : (tc == 2 ? p2 : p3));
+    int seg[MAX_ELEM + 1];
+    seg[0] = 0;
+#pragma unroll
+    for (int e = 0; e < MAX_ELEM; ++e) seg[e + 1] = seg[e] + nbr_cnt[(size_t)i * MAX_ELEM + e];
+    nw[i] = count_words(seg, n_elem, prog->n_ang);
+}
+
+int launch_word_offsets(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
+                        cudaStream_t st) {
+    if (n == 0) return 0;
+    const ElemProgram* pr[MAX_ELEM];
+    for (int e = 0; e < MAX_ELEM; ++e) pr[e] = e < n_elem ? d_prog[e] : nullptr;
+    k_count_words<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, n_elem, g.ncell, w.cell_start, w.nbr_cnt, pr[0], pr[1],
+                                                                pr[2], pr[3], w.nw);
+    return 1 + launch_scan_i64_from_i32(w.nw, n, w.word_off, w.word_tmp, st);
+}
+
 #ifndef NNP_SF2_WPC
 #define NNP_SF2_WPC 2
 #endif
@@ -261,6 +298,7 @@ int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const E
     for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.G = w.G;
+    p.word_off = w.word_off; p.gmask = w.gmask; p.gmask_cap = w.gmask_cap;
     bool use[3] = {false, false, false};
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;

@@ -97,6 +97,11 @@ static size_t ws_layout(Workspace* w, void* base, int64_t n, int n_elem, int str
     w->dEdG = (double*)take(N * (size_t)g_stride * 8);
     w->e_sorted = (double*)take(N * 8);
     w->f_sorted = (double*)take(N * 3 * 8);
+    w->nw = (int32_t*)take(N * 4);
+    w->word_off = (int64_t*)take((N + 1) * 8);
+    w->word_tmp = (int64_t*)take(((N + 1) / 4096 + 2 * 4096 + 16) * 8);
+    w->gmask_cap = (int64_t)N * WORD_BUDGET;
+    w->gmask = (uint32_t*)take((size_t)w->gmask_cap * 4);
     w->n_partial = (int64_t)(N + 255) / 256 + 1;
     w->partial = (double*)take((size_t)w->n_partial * 8);
     w->status = (int32_t*)take(64);
@@ -421,6 +426,7 @@ extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d
     mark(1);
     launches += launch_neighbors(w, g, n_atoms, m->n_elem, m->rc * m->rc, stride, m->max_nbr, st);
     mark(2);
+    launches += launch_word_offsets(w, g, n_atoms, m->n_elem, m->d_prog, st);
     launches += launch_sf(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->rc, stride, m->max_nbr, m->g_stride, st);
     mark(3);
     launches += launch_mlp(w, n_atoms, m->n_elem, g.ncell, m->nets, m->g_stride, st);

@@ -96,6 +96,14 @@ struct Workspace {
     double *G, *dEdG;                // [N][g_stride], sorted order
     double *e_sorted;                // [N]
     double *f_sorted;                // [N][3]
+    // masks handed from the symmetry-function kernel to the force kernel (fast paths): the SF kernel
+    // screens the (j,k) candidates of every centre anyway; it stores the mask words of centre i in the
+    // force kernel's (j-major) order at gmask[word_off[i] ..), if they fit the budget
+    int32_t *nw;                     // [N] mask words of centre i
+    int64_t *word_off;               // [N+1] exclusive prefix of nw
+    int64_t *word_tmp;               // scan scratch
+    uint32_t *gmask;                 // [gmask_cap]
+    int64_t gmask_cap;
     double *partial;                 // [n_partial] block sums of the energy
     int32_t *status;                 // [4]
     int64_t n_keys_cap;
@@ -115,6 +123,10 @@ int launch_mlp(const Workspace& w, int64_t n, int n_elem, int ncell, const NetDe
                cudaStream_t st);
 int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
                  const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st);
+// mask words per centre + their prefix (k_sf2.cu); before launch_sf
+constexpr int WORD_BUDGET = 320;     // gmask capacity = N * WORD_BUDGET words (a water-like centre with 91 neighbours has 152)
+int launch_word_offsets(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
+                        cudaStream_t st);
 // fast path of S2 (lane-owned design, k_sf2.cu): specialised variants only
 int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
                const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st);

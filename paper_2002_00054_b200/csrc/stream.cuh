@@ -45,7 +45,7 @@ struct GroupTab {
     int stride;       // words from (j, w) to (j + 1, w)
     int gfirst;       // first group of the block this group belongs to
     int last;         // 1 if this is the last group of its block
-    int pad;
+    int gmoff;        // index of this group's first word in GROUP-major order (the order of the exported masks)
 };
 
 // upper bound of the mask words of one centre with at most `cap` neighbours of `n_elem` elements:
@@ -59,7 +59,7 @@ __host__ __device__ constexpr int mask_words_cap(int cap, int n_elem) { return c
 template <bool JMAJOR>
 __device__ __forceinline__ int build_groups(const int* seg, int n_elem, const int32_t* n_ang, GroupTab* tab, int tid,
                                             int& NW) {
-    int ng = 0, woff = 0;
+    int ng = 0, woff = 0, gm = 0;
     for (int e1 = 0; e1 < n_elem; ++e1) {
         const int n1 = seg[e1 + 1] - seg[e1];
         const int gfirst = ng;
@@ -69,11 +69,13 @@ __device__ __forceinline__ int build_groups(const int* seg, int n_elem, const in
             if (n_ang[pr] == 0) continue;
             const int n2 = seg[e2 + 1] - seg[e2];
             GroupTab g;
-            g.jbeg = seg[e1]; g.jend = seg[e1 + 1]; g.pair = pr; g.pad = 0;
+            g.jbeg = seg[e1]; g.jend = seg[e1 + 1]; g.pair = pr;
             if (e1 == e2) { g.kbase = g.jbeg; g.ns = n1; g.nk = n1 / 2; }
             else { g.kbase = seg[e2]; g.ns = 0; g.nk = n1 > 0 ? n2 : 0; }
             g.W = (g.nk + 31) >> 5;
             if (g.W == 0) continue;
+            g.gmoff = gm;
+            gm += n1 * g.W;
             if (JMAJOR) { g.woff = woff + wsum; g.gfirst = gfirst; g.stride = 0; g.last = 0; wsum += g.W; }
             else { g.woff = woff; g.gfirst = ng; g.stride = g.W; g.last = 1; woff += n1 * g.W; }
             if (tid == 0) tab[ng] = g;
@@ -89,6 +91,30 @@ __device__ __forceinline__ int build_groups(const int* seg, int n_elem, const in
     }
     NW = woff;
     return ng;
+}
+
+// number of mask words of a centre (= NW of build_groups, either order)
+__device__ __forceinline__ int count_words(const int* seg, int n_elem, const int32_t* n_ang) {
+    int nw = 0;
+    for (int e1 = 0; e1 < n_elem; ++e1) {
+        const int n1 = seg[e1 + 1] - seg[e1];
+        for (int e2 = e1; e2 < n_elem; ++e2) {
+            if (n_ang[pair_index(e1, e2, n_elem)] == 0) continue;
+            const int nk = e1 == e2 ? n1 / 2 : (n1 > 0 ? seg[e2 + 1] - seg[e2] : 0);
+            nw += n1 * ((nk + 31) >> 5);
+        }
+    }
+    return nw;
+}
+
+// group-major word index y -> (group, local owner index, word)
+__device__ __forceinline__ void decode_gmajor(const GroupTab* tab, int ng, int y, int& g, int& jl, int& w) {
+    g = 0;
+    for (int t = 1; t < ng; ++t)
+        if (tab[t].gmoff <= y) g = t;
+    const int rel = y - tab[g].gmoff, W = tab[g].W;
+    jl = W == 1 ? rel : (W == 2 ? rel >> 1 : rel / W);
+    w = rel - jl * W;
 }
 
 __device__ __forceinline__ bool close32(const float4 a, const float4 b, float rc2f) {
