@@ -8,7 +8,7 @@ call) over one synthetic water-like system.  Default workload = BASELINE.json co
 one GPU.  N > 1 (torchrun): the path does not shard in this build ("replicas only", DESIGN.md
 section 8(e)) -> every rank evaluates the same system on its own GPU, value = N * atoms * K / max time.
 
-One JSON line on stdout (rank 0).  Extra keys: roofline (dominant kernel k_force, FP64-ALU bound),
+One JSON line on stdout (rank 0).  Extra keys: roofline (dominant kernel k_force2, FP64-ALU bound),
 cpu_baseline (the oracle on a bounded sample of centres of the same system), e2e (host buffers
 through nnp_compute_host), clocks, gpu_launches, stage_ms.
 """
@@ -314,7 +314,7 @@ def main():
     total_instr = sum(instr.values()) * n
     hbm_bytes_per_atom = 2.8e3 if not cfg.wide else 5.2e3
     roofline = {
-        "bound": "alu", "kernel": "k_force", "achieved": achieved / 1e12, "peak": peak_alu / 1e12,
+        "bound": "alu", "kernel": "k_force2", "achieved": achieved / 1e12, "peak": peak_alu / 1e12,
         "unit": "T FP64 instr/s", "frac": achieved / peak_alu, "traffic": None,
         "peak_source": "derived: 148 SMs x 64 FP64 lanes x %.0f MHz (clocks.max.sm); DFMA probe in this run: "
                        "burst %.2f, sustained %.2f T instr/s" % (sm_max, dfma_burst / 1e12, dfma_sust / 1e12),

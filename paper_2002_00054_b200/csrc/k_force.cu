@@ -3,6 +3,8 @@
 // move as little data as possible, recomputing where necessary", L98, L124).  This holds "the
 // dominant angular force loop" (L116) and is the hottest kernel of the path.
 //
+// GENERIC path: any symmetry-function table.  Tables with the structure of a compile-time Spec
+// (angular.cuh) run on the lane-owned fast path, k_force2.cu.
 // One warp per centre i, same staging / round enumeration / compaction as k_sf.cu.  For a
 // triplet (i; j,k) with u = r_j - r_i, v = r_k - r_i, w = v - u the beta-weighted gradient is
 //     dg/du = f_uu u + f_uv v - f_w w,      dg/dv = f_vv v + f_uv u + f_w w
@@ -14,8 +16,6 @@
 // a time (angular.cuh): pairs of equal colour never share a slot, and a warp owns its slots, so
 // no shared-memory atomics are needed (the first version's FP64 shared atomicAdd = CAS loops
 // took >35 % of the stall samples and ran 2.8 iterations on average; profiles/r1_*).
-#include <cstdlib>
-
 #include "angular.cuh"
 #include "geometry.cuh"
 
@@ -104,72 +104,6 @@ __device__ __forceinline__ void triplet_forces(const double2 j0, const double2 j
         pend &= ~__ballot_sync(0xffffffffu, mine);
     }
 }
-
-template <class Spec>
-struct ForceTripletFast {
-    const Nbh& nb;
-    SlotAcc acc;
-    const double2* bt;   // [pair group][bt_stride]: (beta 2^(1-zeta), beta 2^(1-zeta) zeta lambda)
-    double eta0, eta[Spec::NETA > 0 ? Spec::NETA : 1];
-    double k2, rc2;
-    int sg1, sg2, sg3, n_elem;     // first slot of neighbour element 1, 2, 3
-
-    __device__ __forceinline__ void operator()(int j, int k, int col, bool active) {
-        const double2 j0 = nb.p0[j], j1 = nb.p1[j], j2 = nb.p2[j], j3 = nb.p3[j];
-        const double2 k0 = nb.p0[k], k1 = nb.p1[k], kk2 = nb.p2[k], k3 = nb.p3[k];
-        // pair group of (element of j, element of k)
-        const int ej = (j >= sg1) + (j >= sg2) + (j >= sg3), ek = (k >= sg1) + (k >= sg2) + (k >= sg3);
-        const int ea = min(ej, ek), eb = max(ej, ek);
-        const double2* btg = bt + (ea * n_elem - (ea * (ea - 1)) / 2 + (eb - ea)) * bt_stride<Spec>();
-        const double wx = k0.x - j0.x, wy = k0.y - j0.y, wz = k1.x - j1.x;
-        const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
-        double Cc, Sc;
-        cos_sinc(c2 * k2, Cc, Sc);
-        double fcc = Cc * Cc;                       // fc(c)
-        double dfc = (-2.0 * k2) * (Cc * Sc);       // fc'(c)/c
-        if (!active || !(c2 < rc2)) { fcc = 0.0; dfc = 0.0; }   // exact cutoff (the queue was screened in FP32)
-        // Y_e = exp(-eta_e (a^2 + b^2 + c^2)): one exp, then integer powers
-        double Y[Spec::NETA];
-        Y[0] = (j3.x * k3.x) * exp_small(-eta0 * c2);
-        if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
-        if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
-        if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
-        const double iab = j1.y * k1.y;
-        const double cosv = fma(j0.x, k0.x, fma(j0.y, k0.y, j1.x * k1.x)) * iab;
-        // pw[l][b] = (1 +- cos)^(2^b) ; pd[l][b] = (1 +- cos)^(2^b - 1)
-        double pw[2][Spec::MAXBIT + 1], pd[2][Spec::MAXBIT + 1];
-        pw[0][0] = 1.0 + cosv; pw[1][0] = 1.0 - cosv;
-        pd[0][0] = 1.0; pd[1][0] = 1.0;
-#pragma unroll
-        for (int b = 1; b <= Spec::MAXBIT; ++b) {
-#pragma unroll
-            for (int l = 0; l < 2; ++l) {
-                pw[l][b] = pw[l][b - 1] * pw[l][b - 1];
-                pd[l][b] = pd[l][b - 1] * pw[l][b - 1];
-            }
-        }
-        double Z0 = 0.0, Z1 = 0.0, Z2 = 0.0;
-#pragma unroll
-        for (int e = 0; e < Spec::NETA; ++e) {
-            double T0 = 0.0, T1 = 0.0;
-#pragma unroll
-            for (int b = 0; b <= Spec::MAXBIT; ++b) {
-#pragma unroll
-                for (int l = 0; l < 2; ++l)
-                    if (Spec::mask(e) >> (8 * l + b) & 1u) {
-                        const double2 c = btg[acc_index<Spec>(e, 8 * l + b)];
-                        T0 = fma(c.x, pw[l][b], T0);
-                        T1 = fma(c.y, pd[l][b], T1);
-                    }
-            }
-            const double A = T0 * Y[e];
-            Z0 += A;
-            Z1 = fma(T1, Y[e], Z1);
-            Z2 = fma(eta[e], A, Z2);
-        }
-        triplet_forces(j0, j1, j2, k0, k1, kk2, fcc, dfc, cosv, iab, Z0, Z1, Z2, acc, j, k, col, active);
-    }
-};
 
 struct ForceTripletGeneric {
     const Nbh& nb;
@@ -296,41 +230,7 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
 
     // ---- angular part ---------------------------------------------------------------------------
     const float rc2f = screen_rc2(p.rc2);
-    if constexpr (Spec::ID != ANG_GENERIC) {
-        // coefficient tables of all pair groups, then ONE sweep over all unordered neighbour pairs:
-        // the pair group is looked up per triplet, so a round (= colour class) spans the whole row
-        bool any = false;
-        for (int pr = 0; pr < npair; ++pr) {
-            any |= prog->n_ang[pr] > 0;
-            if (lane < 16) {
-#pragma unroll
-                for (int e = 0; e < Spec::NETA; ++e) {
-                    if (Spec::mask(e) >> lane & 1u) {
-                        const int g = prog->ang_g[pr][e][lane];
-                        const int zeta = 1 << (lane & 7);
-                        const double lam = lane < 8 ? 1.0 : -1.0;
-                        const double bc = g >= 0 ? brow[g] * exp2((double)(1 - zeta)) : 0.0;
-                        int a = 0;   // accumulator slot = set bits before (e, lane)
-                        for (int ee = 0; ee < Spec::NETA; ++ee) {
-                            const unsigned mk = Spec::mask(ee);
-                            if (ee < e) a += __popc(mk);
-                            else if (ee == e) a += __popc(mk & ((1u << lane) - 1u));
-                        }
-                        bt[pr * bt_stride<Spec>() + a] = make_double2(bc, bc * (double)zeta * lam);
-                    }
-                }
-            }
-        }
-        __syncwarp();        // tables written, beta row dead -> its memory becomes the pair queue
-        if (any) {
-            ForceTripletFast<Spec> f{nb, acc, bt, eta0, {}, p.k2, p.rc2, seg[1],
-                                     p.n_elem > 2 ? seg[2] : 0x7fffffff, p.n_elem > 3 ? seg[3] : 0x7fffffff, p.n_elem};
-            if (p.n_elem < 2) f.sg1 = 0x7fffffff;
-#pragma unroll
-            for (int e = 0; e < Spec::NETA; ++e) f.eta[e] = prog->ang_eta[e];
-            pairs_within(nb, 0, ntot, rc2f, Q, lane, f);
-        }
-    } else {
+    {
         // generic tables: per pair group, walking the SF list; the beta row stays live, so the queue
         // sits in the (unused) p3 plane
         Q.q = reinterpret_cast<uint32_t*>(nb.p3);
@@ -404,13 +304,8 @@ int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const
     }
     cudaMemsetAsync(w.f_sorted, 0, sizeof(double) * 3 * (size_t)n, st);
     int launches = 0;
-    static const bool queue_design = getenv("NNP_QUEUE_DESIGN") != nullptr;   // A/B switch while both designs exist
-    if (queue_design) {
-        if (use[ANG_BASE12]) launches += launch_one<SpecBase12>(p, st);
-        if (use[ANG_WIDE32]) launches += launch_one<SpecWide32>(p, st);
-    } else if (use[ANG_BASE12] || use[ANG_WIDE32]) {
+    if (use[ANG_BASE12] || use[ANG_WIDE32])     // specialised tables: lane-owned design (k_force2.cu)
         launches += launch_force2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, st);
-    }
     if (use[ANG_GENERIC]) launches += launch_one<SpecGeneric>(p, st);
     return launches;
 }

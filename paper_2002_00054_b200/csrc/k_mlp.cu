@@ -157,8 +157,9 @@ int launch_mlp(const Workspace& w, int64_t n, int n_elem, int ncell, const NetDe
         p.elem_end = w.cell_start + (size_t)(e + 1) * ncell;
         p.G = w.G; p.dEdG = w.dEdG; p.e_sorted = w.e_sorted; p.g_stride = g_stride;
         const size_t budget = 100 * 1024;
-        if (mlp_smem_bytes(p.net, 64) <= budget) launch_ta<64>(p, n, mlp_smem_bytes(p.net, 64), st);
-        else if (mlp_smem_bytes(p.net, 32) <= budget) launch_ta<32>(p, n, mlp_smem_bytes(p.net, 32), st);
+        // 32 atoms per CTA: 8 thread groups cover the 7 output blocks of a 25-wide layer in one round
+        // (measured 4.6 ms against 6.5 ms with 64 atoms / 4 groups at 2.1 M atoms)
+        if (mlp_smem_bytes(p.net, 32) <= budget) launch_ta<32>(p, n, mlp_smem_bytes(p.net, 32), st);
         else if (mlp_smem_bytes(p.net, 16) <= 2 * budget) launch_ta<16>(p, n, mlp_smem_bytes(p.net, 16), st);
         else launch_ta<8>(p, n, mlp_smem_bytes(p.net, 8), st);
         ++launches;

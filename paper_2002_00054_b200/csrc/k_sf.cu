@@ -2,11 +2,10 @@
 // plus "a similar angular computation with one extra loop over neighbors of neighbors";
 // formulas: include/nnp.h at nnp_sf, readings 2-4).
 //
+// GENERIC path: any symmetry-function table (walks the SF list per triplet).  Tables with the
+// structure of a compile-time Spec (angular.cuh) run on the lane-owned fast path, k_sf2.cu.
 // One warp per centre.  Radial and angular parts share the staged neighbourhood, so they are
 // ONE kernel here (the paper splits them, L98, because its parallel_for has no shared staging).
-// FP64-ALU bound: ~93 FP64 instructions per contributing triplet, ~1,940 triplets per atom.
-#include <cstdlib>
-
 #include "angular.cuh"
 #include "geometry.cuh"
 
@@ -33,55 +32,6 @@ __host__ __device__ constexpr size_t sf_warp_smem(int cap) {
     const size_t capa = (size_t)((cap + 3) & ~3);
     return capa * (48 + 8 + 12) + 256 + (Spec::ID == ANG_GENERIC ? 64 * 8 : 0);
 }
-
-// ---- per-triplet work, specialised groups -------------------------------------------------
-template <class Spec>
-struct SfTripletFast {
-    const Nbh& nb;
-    double eta0, k2, rc2;
-    double acc[Spec::NACC > 0 ? Spec::NACC : 1];
-
-    __device__ __forceinline__ SfTripletFast(const Nbh& nb_, double eta0_, double k2_, double rc2_)
-        : nb(nb_), eta0(eta0_), k2(k2_), rc2(rc2_) {
-#pragma unroll
-        for (int a = 0; a < Spec::NACC; ++a) acc[a] = 0.0;
-    }
-
-    __device__ __forceinline__ void operator()(int j, int k, int, bool active) {
-        const double2 j0 = nb.p0[j], j1 = nb.p1[j], j2 = nb.p2[j];
-        const double2 k0 = nb.p0[k], k1 = nb.p1[k], k2v = nb.p2[k];
-        const double wx = k0.x - j0.x, wy = k0.y - j0.y, wz = k1.x - j1.x;
-        const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
-        const double Cc = cos_only(c2 * k2);
-        double C = (j2.y * k2v.y) * (Cc * Cc);      // fc(a) fc(b) fc(c), fc(c) = cos^2(pi c / (2 rc))
-        if (!active || !(c2 < rc2)) C = 0.0;        // exact cutoff (the queue was screened in FP32)
-        // Y_e = exp(-eta_e (a^2 + b^2 + c^2)): one exp, then integer powers
-        double Y[Spec::NETA];
-        Y[0] = (j2.x * k2v.x) * exp_small(-eta0 * c2);
-        if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
-        if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
-        if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
-        const double cosv = fma(j0.x, k0.x, fma(j0.y, k0.y, j1.x * k1.x)) * (j1.y * k1.y);
-        double pw[2][Spec::MAXBIT + 1];
-        pw[0][0] = 1.0 + cosv;
-        pw[1][0] = 1.0 - cosv;
-#pragma unroll
-        for (int b = 1; b <= Spec::MAXBIT; ++b) {
-            pw[0][b] = pw[0][b - 1] * pw[0][b - 1];
-            pw[1][b] = pw[1][b - 1] * pw[1][b - 1];
-        }
-#pragma unroll
-        for (int e = 0; e < Spec::NETA; ++e) {
-            const double xc = Y[e] * C;
-#pragma unroll
-            for (int b = 0; b <= Spec::MAXBIT; ++b) {
-                if (Spec::mask(e) >> b & 1u) acc[acc_index<Spec>(e, b)] = fma(pw[0][b], xc, acc[acc_index<Spec>(e, b)]);
-                if (Spec::mask(e) >> (8 + b) & 1u)
-                    acc[acc_index<Spec>(e, 8 + b)] = fma(pw[1][b], xc, acc[acc_index<Spec>(e, 8 + b)]);
-            }
-        }
-    }
-};
 
 // ---- per-triplet work, generic group: walk the SF list, reduce each value over the batch -----
 struct SfTripletGeneric {
@@ -204,22 +154,7 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
             const int pr = pair_index(e1, e2, p.n_elem);
             const int na = prog->n_ang[pr];
             if (na == 0) continue;
-            if constexpr (Spec::ID != ANG_GENERIC) {
-                SfTripletFast<Spec> f(nb, eta0, p.k2, p.rc2);
-                if (e1 == e2) pairs_within(nb, seg[e1], seg[e1 + 1] - seg[e1], rc2f, Q, lane, f);
-                else pairs_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], rc2f, Q, lane, f);
-#pragma unroll
-                for (int e = 0; e < Spec::NETA; ++e)
-#pragma unroll
-                    for (int b = 0; b < 16; ++b)
-                        if (Spec::mask(e) >> b & 1u) {
-                            const double tot = warp_sum(f.acc[acc_index<Spec>(e, b)]);
-                            const int zeta = 1 << (b & 7);
-                            const double coef = exp2((double)(1 - zeta));
-                            const int g = prog->ang_g[pr][e][b];
-                            if (lane == 0 && g >= 0) Grow[g] = coef * tot;
-                        }
-            } else {
+            {
                 for (int s = lane; s < na; s += 32) gacc[s] = 0.0;
                 __syncwarp();
                 SfTripletGeneric f{nb, prog->ang + prog->ang_off[pr], na, p.k2, p.rc2, ra, gacc, lane};
@@ -270,13 +205,8 @@ int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const El
         if (e < n_elem) use[variant[e]] = true;
     }
     int launches = 0;
-    static const bool queue_design = getenv("NNP_QUEUE_DESIGN") != nullptr;   // A/B switch while both designs exist
-    if (queue_design) {
-        if (use[ANG_BASE12]) launches += launch_one<SpecBase12>(p, st);
-        if (use[ANG_WIDE32]) launches += launch_one<SpecWide32>(p, st);
-    } else if (use[ANG_BASE12] || use[ANG_WIDE32]) {
+    if (use[ANG_BASE12] || use[ANG_WIDE32])     // specialised tables: lane-owned design (k_sf2.cu)
         launches += launch_sf2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, st);
-    }
     if (use[ANG_GENERIC]) launches += launch_one<SpecGeneric>(p, st);
     return launches;
 }

@@ -243,9 +243,20 @@ def test_error_codes():
 
 
 def test_dense_cluster_near_max_neighbors():
-    # 240 atoms in a 12.2 A box: ~115 neighbours per atom (close to the 160 cap)
+    # 240 atoms in a 12.2 A box: ~115 neighbours per atom (close to the 160 cap).  Such a centre has
+    # ~346 mask words, more than the workspace budget of 320 per atom: the last centres do not fit the
+    # mask hand-over from k_sf2 to k_force2, so this case runs BOTH the hand-over and the force kernel's
+    # own screening.
     sysm = W.make_water(80, 21, L=12.2)
     _check_full(W.make_model(False), sysm)
+
+
+@pytest.mark.parametrize("max_neighbors", [128, 200])
+def test_slot_capacity_variants(max_neighbors):
+    # the fast kernels are instantiated for slot capacities 128 / 160 / 256 (shared-memory layout at
+    # compile-time offsets); 160 is the default, these are the other two
+    sysm, model = W.build(W.CONFIGS[0])
+    _check_full(model, sysm, max_neighbors=max_neighbors)
 
 
 def test_host_buffer_entry_point_and_determinism():
