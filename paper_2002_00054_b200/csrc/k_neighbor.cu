@@ -1,7 +1,7 @@
 // k_neighbor.cu -- S1: full neighbour list N(i) = { j != i : |r_j - r_i|_min-image^2 < rc^2 }
 // from the (element, cell)-sorted SoA positions ("neighbor list", L116 "random
-// access (neighbor list)").  One warp per atom; lanes sweep the contiguous x-runs of the
-// 3x3(x3) cell stencil, ballot-compact the hits and write the row coalesced.  Rows hold
+// access (neighbor list)").  One warp per atom; the <= 18 contiguous x-runs of the 3x3(x3) cell
+// stencil are walked as one flat candidate range, hits are ballot-compacted and the row written coalesced.  Rows hold
 // positions in the SORTED order, grouped by neighbour element (all of element 0, then 1, ...),
 // which is what lets the symmetry-function kernels run type-homogeneous segments.
 #include "geometry.cuh"
@@ -48,32 +48,52 @@ k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
 
     int32_t* row = nbr + (size_t)i * stride;
     int cnt = 0;
+    const int nrun = nz * ny * nxr;                     // <= 18 contiguous runs of candidates per element
     for (int e = 0; e < n_elem; ++e) {
         const int32_t* cs = cell_start + (size_t)e * g.ncell;
         const int cnt_before = cnt;
-        for (int a = 0; a < nz; ++a)
-            for (int b = 0; b < ny; ++b) {
-                const int rowbase = (zs[a] * g.nc[1] + ys[b]) * g.nc[0];
-                for (int r = 0; r < nxr; ++r) {
-                    const int j0 = cs[rowbase + xr0[r]], j1 = cs[rowbase + xr1[r] + 1];
-                    for (int jb = j0; jb < j1; jb += 32) {
-                        const int j = jb + lane;
-                        bool hit = false;
-                        if (j < j1 && j != i) {
-                            const double dx = min_image_1d(xi, sx[j], g.box[0], g.half[0]);
-                            const double dy = min_image_1d(yi, sy[j], g.box[1], g.half[1]);
-                            const double dz = min_image_1d(zi, sz[j], g.box[2], g.half[2]);
-                            hit = dist2_exact(dx, dy, dz) < rc2;
-                        }
-                        const unsigned m = __ballot_sync(0xffffffffu, hit);
-                        if (hit) {
-                            const int p = cnt + __popc(m & ((1u << lane) - 1u));
-                            if (p < max_nbr) row[p] = j;
-                        }
-                        cnt += __popc(m);
-                    }
-                }
+        // run table: lane r owns run r (its bounds come in ONE round trip instead of one per run), then the
+        // candidates of all runs are walked as one flat index space -> full chunks of 32 whatever the run lengths
+        int j0 = 0, len = 0;
+        if (lane < nrun) {
+            const int r = lane % nxr, ab = lane / nxr;
+            const int b = ab % ny, a = ab / ny;
+            const int rowbase = (zs[a] * g.nc[1] + ys[b]) * g.nc[0];
+            j0 = cs[rowbase + xr0[r]];
+            len = cs[rowbase + xr1[r] + 1] - j0;
+        }
+        int incl = len;
+#pragma unroll
+        for (int d = 1; d < 32; d <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, incl, d);
+            if (lane >= d) incl += t;
+        }
+        const int P = incl - len;                       // first flat index of run `lane`
+        const int total = __shfl_sync(0xffffffffu, incl, 31);
+        for (int f0 = 0; f0 < total; f0 += 32) {
+            const int f = f0 + lane;
+            int lo = 0, hi = 31;                        // largest run r with P[r] <= f
+#pragma unroll
+            for (int step = 0; step < 5; ++step) {
+                const int mid = (lo + hi + 1) >> 1;
+                const int pm = __shfl_sync(0xffffffffu, P, mid);
+                if (pm <= f) lo = mid; else hi = mid - 1;
             }
+            const int j = __shfl_sync(0xffffffffu, j0, lo) + (f - __shfl_sync(0xffffffffu, P, lo));
+            bool hit = false;
+            if (f < total && j != i) {
+                const double dx = min_image_1d(xi, sx[j], g.box[0], g.half[0]);
+                const double dy = min_image_1d(yi, sy[j], g.box[1], g.half[1]);
+                const double dz = min_image_1d(zi, sz[j], g.box[2], g.half[2]);
+                hit = dist2_exact(dx, dy, dz) < rc2;
+            }
+            const unsigned m = __ballot_sync(0xffffffffu, hit);
+            if (hit) {
+                const int p = cnt + __popc(m & ((1u << lane) - 1u));
+                if (p < max_nbr) row[p] = j;
+            }
+            cnt += __popc(m);
+        }
         if (lane == 0) nbr_cnt[(size_t)i * MAX_ELEM + e] = min(cnt, max_nbr) - min(cnt_before, max_nbr);
     }
     if (lane == 0) {
