@@ -38,6 +38,9 @@ FP64_INSTR_PER_ATOM = {
     False: {"sf": 230e3, "mlp": 7e3, "force": 400e3},     # base-52 model
     True: {"sf": 368e3, "mlp": 33e3, "force": 586e3},      # wide-128 model
 }
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_force2 launch, from the ncu captures under profiles/
+# (r1b_launches_config3.csv for configs[3], r1b_ncu_k_sf2_k_force2.md for configs[2]); null where not captured
+NCU_DRAM_BYTES_K_FORCE2 = {3: 3619019008 + 103957248, 2: 338736896 + 9724160}
 # FP64 pipe peak derived from unit counts and clocks: 148 SMs x 64 DFMA lanes/clk x clocks.max.sm
 FP64_LANES_PER_SM = 64
 N_SM = 148
@@ -315,7 +318,7 @@ def main():
     hbm_bytes_per_atom = 2.8e3 if not cfg.wide else 5.2e3
     roofline = {
         "bound": "alu", "kernel": "k_force2", "achieved": achieved / 1e12, "peak": peak_alu / 1e12,
-        "unit": "T FP64 instr/s", "frac": achieved / peak_alu, "traffic": None,
+        "unit": "T FP64 instr/s", "frac": achieved / peak_alu, "traffic": NCU_DRAM_BYTES_K_FORCE2.get(args.config),
         "peak_source": "derived: 148 SMs x 64 FP64 lanes x %.0f MHz (clocks.max.sm); DFMA probe in this run: "
                        "burst %.2f, sustained %.2f T instr/s" % (sm_max, dfma_burst / 1e12, dfma_sust / 1e12),
         "frac_of_measured_dfma": achieved / dfma_burst,
