@@ -118,6 +118,20 @@ def test_generic_table_three_elements():
     _check_full(model, sysm)
 
 
+@pytest.mark.parametrize("elements", [("X",), ("A", "B", "C")])
+def test_fast_path_one_and_three_elements(elements):
+    # the base-12 table on 1 and 3 elements: the lane-owned kernels with a single tournament segment
+    # (1 group) and with 6 pair groups (pair index derived from the slots, not from the descriptor bits)
+    model = W.make_model(False, seed=77, elements=elements, hidden=(9, 6))
+    sysm = W.make_water(120, 9, L=15.0)
+    sysm.types = (np.arange(sysm.n_atoms) % len(elements)).astype(np.int32)
+    from paper_2002_00054_b200 import NNP
+    nnp = NNP.from_model(model)
+    assert nnp.uses_fast_path()
+    nnp.close()
+    _check_full(model, sysm)
+
+
 def test_single_element_radial_only():
     model = tiny_model([(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0), (0, 2, 0, 0, 0.4, 2.0, 0.0, 0.0)], hidden=(4,))
     sysm = W.make_water(60, 3, L=12.4)
