@@ -299,8 +299,8 @@ int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const
     bool use[3] = {false, false, false};
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
-        p.variant[e] = e < n_elem ? variant[e] : -1;
-        if (e < n_elem) use[variant[e]] = true;
+        p.variant[e] = e < n_elem ? (variant[e] & 255) : -1;      // bit 8 = tiny_exp flag (fast launchers)
+        if (e < n_elem) use[variant[e] & 255] = true;
     }
     cudaMemsetAsync(w.f_sorted, 0, sizeof(double) * 3 * (size_t)n, st);
     int launches = 0;

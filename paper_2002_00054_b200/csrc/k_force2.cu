@@ -97,7 +97,7 @@ struct JData {
     double ux, uy, uz, ia, fa, dfa, e0;
 };
 
-template <class Spec, int WPC, int CAPA>
+template <class Spec, int WPC, int CAPA, bool TINY>
 __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_constant__ Force2Params p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NT = WPC * 32;
@@ -152,6 +152,8 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
     const double xi = p.sx[i], yi = p.sy[i], zi = p.sz[i];
     const int32_t* row = p.nbr + (size_t)i * p.stride;
     const double eta0 = prog->ang_eta[0];
+    constexpr bool tiny = TINY;                      // exp(-eta_0 r^2) without range reduction (mathfn.cuh exp_tiny)
+    if ((prog->tiny_exp != 0) != TINY) return;       // uniform per CTA: the other instantiation owns this element
     for (int e = 0; e < p.n_elem; ++e) {
         const int nr = prog->n_rad[e], off = prog->rad_off[e];
         for (int m = seg[e] + tid; m < seg[e + 1]; m += NT) {
@@ -169,7 +171,7 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
             p0[m] = make_double2(dx, dy);
             p1[m] = make_double2(dz, ia);
             p2[m] = make_double2(fa, dfa_a);
-            e0[m] = exp_small(-eta0 * a2);
+            e0[m] = (tiny ? exp_tiny(-eta0 * a2) : exp_small(-eta0 * a2));
             f32[m] = make_float4((float)dx, (float)dy, (float)dz, 0.f);
             double R = 0.0;
             for (int r = 0; r < nr; ++r) {
@@ -304,7 +306,7 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
         double dfc = (-2.0 * p.k2) * (Cc * Sc);        // fc'(c)/c
         if (!active || !(c2 < p.rc2)) { fcc = 0.0; dfc = 0.0; }   // exact cutoff (the masks were screened in FP32)
         double Y[Spec::NETA];
-        Y[0] = (J.e0 * ek) * exp_small(-eta0 * c2);
+        Y[0] = (J.e0 * ek) * (tiny ? exp_tiny(-eta0 * c2) : exp_small(-eta0 * c2));
         if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
         if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
         if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
@@ -410,24 +412,24 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
 #endif
 constexpr int F2_WPC = NNP_F2_WPC;
 
-template <class Spec, int CAPA>
+template <class Spec, int CAPA, bool TINY>
 static int launch_capa(const Force2Params& p, cudaStream_t st) {
     const size_t smem = force2_smem<Spec>(CAPA, p.g_stride, p.n_elem, F2_WPC);
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_force2<Spec, F2_WPC, CAPA>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaFuncSetAttribute(k_force2<Spec, F2_WPC, CAPA, TINY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         configured = true;
     }
-    k_force2<Spec, F2_WPC, CAPA><<<(unsigned)p.n, F2_WPC * 32, smem, st>>>(p);
+    k_force2<Spec, F2_WPC, CAPA, TINY><<<(unsigned)p.n, F2_WPC * 32, smem, st>>>(p);
     return 1;
 }
 
 // slot capacity = smallest instantiated CAPA that holds max_neighbors (nnp_set_max_neighbors: 32..255)
-template <class Spec>
+template <class Spec, bool TINY>
 static int launch_one2(const Force2Params& p, cudaStream_t st) {
-    if (p.cap <= 128) return launch_capa<Spec, 128>(p, st);
-    if (p.cap <= 160) return launch_capa<Spec, 160>(p, st);
-    return launch_capa<Spec, 256>(p, st);
+    if (p.cap <= 128) return launch_capa<Spec, 128, TINY>(p, st);
+    if (p.cap <= 160) return launch_capa<Spec, 160, TINY>(p, st);
+    return launch_capa<Spec, 256, TINY>(p, st);
 }
 
 // launches the fast kernels for the specialised variants in use; the caller has zeroed f_sorted
@@ -442,15 +444,17 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.dEdG = w.dEdG; p.f_sorted = w.f_sorted;
     p.word_off = w.word_off; p.gmask = w.gmask; p.gmask_cap = w.gmask_cap;
-    bool use[3] = {false, false, false};
+    bool use[3][2] = {{false, false}, {false, false}, {false, false}};   // [variant][tiny_exp]
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
-        p.variant[e] = e < n_elem ? variant[e] : -1;
-        if (e < n_elem) use[variant[e]] = true;
+        p.variant[e] = e < n_elem ? (variant[e] & 255) : -1;                 // bit 8 of variant[] = tiny_exp of the element
+        if (e < n_elem) use[variant[e] & 255][(variant[e] >> 8) & 1] = true;
     }
     int launches = 0;
-    if (use[ANG_BASE12]) launches += launch_one2<SpecBase12>(p, st);
-    if (use[ANG_WIDE32]) launches += launch_one2<SpecWide32>(p, st);
+    if (use[ANG_BASE12][1]) launches += launch_one2<SpecBase12, true>(p, st);
+    if (use[ANG_BASE12][0]) launches += launch_one2<SpecBase12, false>(p, st);
+    if (use[ANG_WIDE32][1]) launches += launch_one2<SpecWide32, true>(p, st);
+    if (use[ANG_WIDE32][0]) launches += launch_one2<SpecWide32, false>(p, st);
     return launches;
 }
 

@@ -201,8 +201,8 @@ int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const El
     bool use[3] = {false, false, false};
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
-        p.variant[e] = e < n_elem ? variant[e] : -1;
-        if (e < n_elem) use[variant[e]] = true;
+        p.variant[e] = e < n_elem ? (variant[e] & 255) : -1;      // bit 8 = tiny_exp flag (fast launchers)
+        if (e < n_elem) use[variant[e] & 255] = true;
     }
     int launches = 0;
     if (use[ANG_BASE12] || use[ANG_WIDE32])     // specialised tables: lane-owned design (k_sf2.cu)

@@ -40,7 +40,7 @@ __host__ __device__ constexpr size_t sf2_smem(int capa, int n_elem, int wpc) {
     return (b + 15) / 16 * 16;
 }
 
-template <class Spec, int WPC, int CAPA>
+template <class Spec, int WPC, int CAPA, bool TINY>
 __global__ void __launch_bounds__(WPC * 32, (Spec::NACC <= 12 ? 24 : 16) / WPC) k_sf2(const __grid_constant__ Sf2Params p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NT = WPC * 32;
@@ -79,6 +79,8 @@ __global__ void __launch_bounds__(WPC * 32, (Spec::NACC <= 12 ? 24 : 16) / WPC) 
     const double xi = p.sx[i], yi = p.sy[i], zi = p.sz[i];
     const int32_t* row = p.nbr + (size_t)i * p.stride;
     const double eta0 = prog->ang_eta[0];
+    constexpr bool tiny = TINY;                      // exp(-eta_0 r^2) without range reduction (mathfn.cuh exp_tiny)
+    if ((prog->tiny_exp != 0) != TINY) return;       // uniform per CTA: the other instantiation owns this element
     for (int m = tid; m < ntot; m += NT) {
         const int j = row[m];
         const double dx = min_image_1d(xi, p.sx[j], p.box[0], p.half[0]);
@@ -89,7 +91,7 @@ __global__ void __launch_bounds__(WPC * 32, (Spec::NACC <= 12 ? 24 : 16) / WPC) 
         const double Ca = cos_only(a2 * p.k2);
         p0[m] = make_double2(dx, dy);
         p1[m] = make_double2(dz, ia);
-        p2[m] = make_double2(exp_small(-eta0 * a2), Ca * Ca);
+        p2[m] = make_double2((tiny ? exp_tiny(-eta0 * a2) : exp_small(-eta0 * a2)), Ca * Ca);
         ra[m] = a2 * ia;
         f32[m] = make_float4((float)dx, (float)dy, (float)dz, 0.f);
     }
@@ -176,7 +178,7 @@ __global__ void __launch_bounds__(WPC * 32, (Spec::NACC <= 12 ? 24 : 16) / WPC) 
         double Cf = (jfa * k2v.y) * (Cc * Cc);      // fc(a) fc(b) fc(c), fc(c) = cos^2(pi c / (2 rc))
         if (!active || !(c2 < p.rc2)) Cf = 0.0;     // exact cutoff (the masks were screened in FP32)
         double Y[Spec::NETA];
-        Y[0] = (je0 * k2v.x) * exp_small(-eta0 * c2);
+        Y[0] = (je0 * k2v.x) * (tiny ? exp_tiny(-eta0 * c2) : exp_small(-eta0 * c2));
         if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
         if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
         if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
@@ -268,23 +270,23 @@ int launch_word_offsets(const Workspace& w, const Grid& g, int64_t n, int n_elem
 #endif
 constexpr int SF2_WPC = NNP_SF2_WPC;
 
-template <class Spec, int CAPA>
+template <class Spec, int CAPA, bool TINY>
 static int launch_capa_sf(const Sf2Params& p, cudaStream_t st) {
     const size_t smem = sf2_smem<Spec>(CAPA, p.n_elem, SF2_WPC);
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_sf2<Spec, SF2_WPC, CAPA>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaFuncSetAttribute(k_sf2<Spec, SF2_WPC, CAPA, TINY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         configured = true;
     }
-    k_sf2<Spec, SF2_WPC, CAPA><<<(unsigned)p.n, SF2_WPC * 32, smem, st>>>(p);
+    k_sf2<Spec, SF2_WPC, CAPA, TINY><<<(unsigned)p.n, SF2_WPC * 32, smem, st>>>(p);
     return 1;
 }
 
-template <class Spec>
+template <class Spec, bool TINY>
 static int launch_one_sf2(const Sf2Params& p, cudaStream_t st) {
-    if (p.cap <= 128) return launch_capa_sf<Spec, 128>(p, st);
-    if (p.cap <= 160) return launch_capa_sf<Spec, 160>(p, st);
-    return launch_capa_sf<Spec, 256>(p, st);
+    if (p.cap <= 128) return launch_capa_sf<Spec, 128, TINY>(p, st);
+    if (p.cap <= 160) return launch_capa_sf<Spec, 160, TINY>(p, st);
+    return launch_capa_sf<Spec, 256, TINY>(p, st);
 }
 
 // launches the fast kernels for the specialised variants in use
@@ -299,15 +301,17 @@ int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const E
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.G = w.G;
     p.word_off = w.word_off; p.gmask = w.gmask; p.gmask_cap = w.gmask_cap;
-    bool use[3] = {false, false, false};
+    bool use[3][2] = {{false, false}, {false, false}, {false, false}};   // [variant][tiny_exp]
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
-        p.variant[e] = e < n_elem ? variant[e] : -1;
-        if (e < n_elem) use[variant[e]] = true;
+        p.variant[e] = e < n_elem ? (variant[e] & 255) : -1;                 // bit 8 of variant[] = tiny_exp of the element
+        if (e < n_elem) use[variant[e] & 255][(variant[e] >> 8) & 1] = true;
     }
     int launches = 0;
-    if (use[ANG_BASE12]) launches += launch_one_sf2<SpecBase12>(p, st);
-    if (use[ANG_WIDE32]) launches += launch_one_sf2<SpecWide32>(p, st);
+    if (use[ANG_BASE12][1]) launches += launch_one_sf2<SpecBase12, true>(p, st);
+    if (use[ANG_BASE12][0]) launches += launch_one_sf2<SpecBase12, false>(p, st);
+    if (use[ANG_WIDE32][1]) launches += launch_one_sf2<SpecWide32, true>(p, st);
+    if (use[ANG_WIDE32][0]) launches += launch_one_sf2<SpecWide32, false>(p, st);
     return launches;
 }
 

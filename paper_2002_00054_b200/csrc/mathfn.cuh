@@ -31,6 +31,15 @@ __device__ __forceinline__ double exp_small(double y) {
     return __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
 }
 
+// exp(y) for y in [-0.05, 0]: no range reduction, degree 6.  The triplet Gaussian exp(-eta_0 c^2) of a
+// model with eta_0 rc^2 <= 0.05 (the water-like models: 0.001 * 36) never leaves this interval.
+__device__ __forceinline__ double exp_tiny(double y) {
+    double p = EXPT[6];
+#pragma unroll
+    for (int q = 5; q >= 0; --q) p = fma(p, y, EXPT[q]);
+    return p;
+}
+
 // C = cos(sqrt z), S = sin(sqrt z)/sqrt z for z in [0, (pi/2)^2]
 __device__ __forceinline__ void cos_sinc(double z, double& C, double& S) {
     double c = COSC[8], s = SNCC[8];

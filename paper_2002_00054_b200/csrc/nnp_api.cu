@@ -269,7 +269,8 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
                         return bail(NNP_ERR_INVALID_ARG, "generic angular path supports <= 64 SFs per pair group");
             }
         }
-        m->variant[c] = P.variant;
+        P.tiny_exp = (P.variant != ANG_GENERIC && P.ang_eta[0] * rc * rc * (1.0 + 1e-5) <= 0.05) ? 1 : 0;
+        m->variant[c] = P.variant | (P.tiny_exp << 8);      // bit 8: host-side copy of tiny_exp for the launchers
     }
 
     // networks: validate and pack everything on the host first, upload afterwards
@@ -377,7 +378,7 @@ extern "C" int32_t nnp_last_launch_count(const nnp_model* m) { return m ? m->las
 extern "C" int32_t nnp_uses_fast_path(const nnp_model* m) {
     if (!m) return 0;
     for (int c = 0; c < m->n_elem; ++c)
-        if (m->variant[c] == ANG_GENERIC) return 0;
+        if ((m->variant[c] & 255) == ANG_GENERIC) return 0;
     return 1;
 }
 extern "C" const char* nnp_last_error(const nnp_model* m) { return m ? m->err.c_str() : g_create_err.c_str(); }

@@ -51,7 +51,7 @@ struct ElemProgram {
     int32_t n_sf;
     int32_t n_elem;
     int32_t variant;                 // AngVariant
-    int32_t pad0;
+    int32_t tiny_exp;                // specialised path: eta_0 rc^2 <= 0.05 -> exp_tiny() for exp(-eta_0 r^2)
     int32_t n_rad[MAX_ELEM];         // radial SFs for neighbour element e
     int32_t rad_off[MAX_ELEM];       // first index into rad[]
     int32_t n_ang[MAX_PAIR];         // angular SFs of pair group p

@@ -132,6 +132,14 @@ def test_fast_path_one_and_three_elements(elements):
     _check_full(model, sysm)
 
 
+def test_fast_path_large_cutoff_general_exp():
+    # rc = 8 A: eta_0 rc^2 = 0.064 > 0.05, so the fast kernels take the range-reduced exp (the water-like
+    # configs, rc = 6 A, run on the small-argument polynomial exp_tiny)
+    model = W.make_model(False, seed=5, rc=8.0)
+    sysm = W.make_water(80, 13, L=16.5)
+    _check_full(model, sysm)
+
+
 def test_single_element_radial_only():
     model = tiny_model([(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0), (0, 2, 0, 0, 0.4, 2.0, 0.0, 0.0)], hidden=(4,))
     sysm = W.make_water(60, 3, L=12.4)
