@@ -198,6 +198,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--ref-centres", type=int, default=0, help="--impl reference: centres per step (0 = auto)")
     ap.add_argument("--cpu-centres", type=int, default=400, help="oracle sample size of the cpu_baseline leg (0 = skip)")
+    ap.add_argument("--md", action="store_true",
+                    help="time velocity-Verlet MD steps (nnp_md_run: kick+drift, the whole path, kick) instead of bare evaluations")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-probe", action="store_true", help="skip the DFMA issue-rate probe (for ncu runs)")
     args = ap.parse_args()
@@ -235,7 +237,16 @@ def main():
     if cfg.seed_disp is not None:
         disp = [torch.tensor(W.displacement(n, cfg.seed_disp, c + 1), device=dev) for c in range(4)]
 
+    vel = None
+    if args.md:     # thermal-ish velocities (sigma 0.005 A/fs), masses of H and O; forces of the start positions
+        g = torch.Generator(device=dev).manual_seed(1234)
+        vel = 0.005 * torch.randn((n, 3), dtype=torch.float64, device=dev, generator=g)
+        nnp.compute(pos, typ, sysm.box, out=out, sync=True)
+
     def step(i):
+        if args.md:
+            nnp.md_run(1, 0.25, (1.008, 15.999), pos, vel, typ, sysm.box, out, sync=False)
+            return
         if disp is not None:
             pos.add_(disp[i % len(disp)])
         nnp.compute(pos, typ, sysm.box, out=out, sync=False)
@@ -341,7 +352,7 @@ def main():
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": cfg.name, "n_atoms": n, "model": model.name, "box": float(sysm.box[0]),
-                   "neighbor_rebuild": "every call", "parallelism": "replicas x%d" % world,
+                   "neighbor_rebuild": "every call", "md": bool(args.md), "parallelism": "replicas x%d" % world,
                    "l2": ("working set per step (%.2f GB workspace) %s the 126 MB L2; no flush between steps"
                           % (nnp.workspace_bytes(n) / 1e9, "exceeds" if nnp.workspace_bytes(n) > 126e6 else "FITS IN"))},
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks, "gpu_launches": launches,

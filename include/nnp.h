@@ -112,6 +112,29 @@ nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d_pos, const
 nnp_status nnp_compute_host(nnp_model* m, int64_t n_atoms, const double* h_pos, const int32_t* h_type,
                             const double box[3], double* h_e_atom, double* h_e_total, double* h_force);
 
+/* ---- MD loop around the path (the implementation is checked by energy
+ * conservation in an NVE run).  Velocity Verlet, everything on the device:
+ *     v += (dt/2) F/m ;  x += dt v ;  F = nnp_compute(x) ;  v += (dt/2) F/m
+ * Units: A, eV, amu, fs  (1 eV/(A amu) = NNP_ACC_UNIT A/fs^2).
+ *
+ * nnp_md_run advances n_steps steps.  On entry d_force must hold the forces of d_pos (call nnp_compute
+ * first); on return d_pos / d_vel / d_force / d_e_atom / d_e_total belong to the last step.  Positions are
+ * NOT wrapped (nnp_compute wraps internally).  The neighbour list is rebuilt every step.
+ *   h_mass   [n_elem] HOST, masses in amu, by element index
+ *   d_vel    [n_atoms][3] device, in/out, A/fs
+ * Everything is enqueued on cuda_stream; no synchronisation inside.
+ * nnp_md_kinetic_energy: *d_ekin (device, [1]) = sum_i m_i |v_i|^2 / (2 NNP_ACC_UNIT) in eV, deterministic
+ * summation order; d_workspace as for nnp_compute (only its energy-partials scratch is touched, the exports of
+ * the last nnp_compute stay valid). */
+#define NNP_ACC_UNIT 9.648533215665327e-3 /* (1.602176634e-19 J/eV) / (1.66053906660e-27 kg/amu) * 1e-10, CODATA 2018 */
+nnp_status nnp_md_run(nnp_model* m, int32_t n_steps, double dt_fs, const double* h_mass, int64_t n_atoms,
+                      double* d_pos, double* d_vel, const int32_t* d_type, const double box[3],
+                      double* d_e_atom, double* d_e_total, double* d_force,
+                      void* d_workspace, size_t workspace_bytes, void* cuda_stream);
+nnp_status nnp_md_kinetic_energy(nnp_model* m, const double* h_mass, int64_t n_atoms, const double* d_vel,
+                                 const int32_t* d_type, double* d_ekin, void* d_workspace, size_t workspace_bytes,
+                                 void* cuda_stream);
+
 /* Synchronise the stream of the last nnp_compute and return its device-side status. */
 nnp_status nnp_sync_status(nnp_model* m);
 

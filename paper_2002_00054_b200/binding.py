@@ -20,7 +20,7 @@ STAGE_NAMES = ("sort", "neighbors", "symmetry_functions", "networks", "forces", 
 
 # every symbol include/nnp.h declares
 EXPORTS = ("nnp_create", "nnp_destroy", "nnp_set_max_neighbors", "nnp_workspace_bytes", "nnp_compute",
-           "nnp_compute_host", "nnp_sync_status", "nnp_get_neighbor_counts", "nnp_get_neighbors", "nnp_get_sf",
+           "nnp_compute_host", "nnp_md_run", "nnp_md_kinetic_energy", "nnp_sync_status", "nnp_get_neighbor_counts", "nnp_get_neighbors", "nnp_get_sf",
            "nnp_get_dedg", "nnp_g_stride", "nnp_set_timing", "nnp_get_timings", "nnp_last_launch_count",
            "nnp_uses_fast_path", "nnp_measure_fp64_peak", "nnp_last_error", "nnp_version")
 
@@ -62,6 +62,11 @@ def load_library():
     L.nnp_compute.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), vp, vp, vp, vp, C.c_size_t, vp]
     L.nnp_compute_host.restype = C.c_int
     L.nnp_compute_host.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), vp, vp, vp]
+    L.nnp_md_run.restype = C.c_int
+    L.nnp_md_run.argtypes = [vp, i32, dbl, C.POINTER(dbl), i64, vp, vp, vp, C.POINTER(dbl), vp, vp, vp, vp,
+                             C.c_size_t, vp]
+    L.nnp_md_kinetic_energy.restype = C.c_int
+    L.nnp_md_kinetic_energy.argtypes = [vp, C.POINTER(dbl), i64, vp, vp, vp, vp, C.c_size_t, vp]
     L.nnp_sync_status.restype = C.c_int
     L.nnp_sync_status.argtypes = [vp]
     L.nnp_get_neighbor_counts.restype = C.c_int
@@ -202,6 +207,44 @@ class NNP:
         if sync:
             self.sync_status()
         return e_atom, e_total, force
+
+    # ---- MD loop around the path (velocity Verlet, NVE) ---------------------------------------------
+    def _ws_ptr(self, n, dev):
+        torch = self._torch
+        if self._ws is None or self._ws_n != n:
+            self._ws = torch.empty(self.workspace_bytes(n) + 256, dtype=torch.uint8, device=dev)
+            self._ws_n = n
+        ptr = (self._ws.data_ptr() + 255) // 256 * 256
+        return ptr, self._ws.numel() - (ptr - self._ws.data_ptr())
+
+    def md_run(self, n_steps, dt_fs, masses, pos, vel, types, box, state, sync=True):
+        """n_steps velocity-Verlet steps in place on pos / vel (cuda f64 [N,3]); `state` = (e_atom, e_total,
+        force) from a compute() of pos (the forces are read on entry, everything is updated)."""
+        n = int(pos.shape[0])
+        e_atom, e_total, force = state
+        ws_ptr, ws_len = self._ws_ptr(n, pos.device)
+        m = (C.c_double * len(masses))(*[float(x) for x in masses])
+        boxc = (C.c_double * 3)(*[float(b) for b in box])
+        stream = self._torch.cuda.current_stream(pos.device).cuda_stream
+        st = self._L.nnp_md_run(self._h, int(n_steps), float(dt_fs), m, n, C.c_void_p(pos.data_ptr()),
+                                C.c_void_p(vel.data_ptr()), C.c_void_p(types.data_ptr()), boxc,
+                                C.c_void_p(e_atom.data_ptr()), C.c_void_p(e_total.data_ptr()),
+                                C.c_void_p(force.data_ptr()), C.c_void_p(ws_ptr), ws_len, C.c_void_p(stream))
+        self._check(st)
+        if sync:
+            self.sync_status()
+
+    def kinetic_energy(self, masses, vel, types):
+        """sum m v^2 / 2 in eV -> cuda f64 [1]."""
+        n = int(vel.shape[0])
+        out = self._torch.empty(1, dtype=self._torch.float64, device=vel.device)
+        ws_ptr, ws_len = self._ws_ptr(n, vel.device)
+        m = (C.c_double * len(masses))(*[float(x) for x in masses])
+        stream = self._torch.cuda.current_stream(vel.device).cuda_stream
+        self._check(self._L.nnp_md_kinetic_energy(self._h, m, n, C.c_void_p(vel.data_ptr()),
+                                                  C.c_void_p(types.data_ptr()), C.c_void_p(out.data_ptr()),
+                                                  C.c_void_p(ws_ptr), ws_len, C.c_void_p(stream)))
+        return out
 
     def compute_host(self, pos, types, box, out=None):
         """Same evaluation with HOST numpy / pinned-torch buffers (copies inside the call)."""

@@ -446,6 +446,51 @@ extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d
     return NNP_OK;
 }
 
+extern "C" nnp_status nnp_md_run(nnp_model* m, int32_t n_steps, double dt_fs, const double* h_mass, int64_t n_atoms,
+                                 double* d_pos, double* d_vel, const int32_t* d_type, const double box[3],
+                                 double* d_e_atom, double* d_e_total, double* d_force, void* d_workspace,
+                                 size_t workspace_bytes, void* cuda_stream) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    if (n_steps < 0 || !h_mass || !(dt_fs > 0.0) || !std::isfinite(dt_fs)) return fail(m, NNP_ERR_INVALID_ARG, "n_steps / dt / masses");
+    for (int e = 0; e < m->n_elem; ++e)
+        if (!(h_mass[e] > 0.0) || !std::isfinite(h_mass[e])) return fail(m, NNP_ERR_INVALID_ARG, "mass must be finite and > 0");
+    if (n_atoms > 0 && (!d_pos || !d_vel || !d_type || !d_force)) return fail(m, NNP_ERR_INVALID_ARG, "null array");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int launches = 0;
+    for (int s = 0; s < n_steps; ++s) {
+        {
+            DeviceGuard dg(m->device);
+            if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
+            launches += launch_vv(n_atoms, m->n_elem, h_mass, d_type, d_force, d_vel, d_pos, dt_fs, true, st);
+        }
+        const nnp_status rc = nnp_compute(m, n_atoms, d_pos, d_type, box, d_e_atom, d_e_total, d_force, d_workspace,
+                                          workspace_bytes, cuda_stream);
+        if (rc != NNP_OK) return rc;
+        launches += m->last_launches;
+        DeviceGuard dg(m->device);
+        launches += launch_vv(n_atoms, m->n_elem, h_mass, d_type, d_force, d_vel, d_pos, dt_fs, false, st);
+    }
+    m->last_launches = launches;
+    NNP_CUDA(m, cudaGetLastError());
+    return NNP_OK;
+}
+
+extern "C" nnp_status nnp_md_kinetic_energy(nnp_model* m, const double* h_mass, int64_t n_atoms, const double* d_vel,
+                                            const int32_t* d_type, double* d_ekin, void* d_workspace,
+                                            size_t workspace_bytes, void* cuda_stream) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    if (!h_mass || !d_ekin || n_atoms < 0 || (n_atoms > 0 && (!d_vel || !d_type))) return fail(m, NNP_ERR_INVALID_ARG, "null array");
+    Workspace w;
+    const size_t need = ws_layout(&w, d_workspace, n_atoms, m->n_elem, row_stride(m), m->g_stride);
+    if (!d_workspace || ((uintptr_t)d_workspace & 255u) || workspace_bytes < need)
+        return fail(m, NNP_ERR_WORKSPACE, "workspace null, misaligned or too small");
+    DeviceGuard dg(m->device);
+    if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
+    launch_ekin(n_atoms, m->n_elem, h_mass, d_type, d_vel, w.partial, d_ekin, (cudaStream_t)cuda_stream);   // the energy partials are scratch between calls
+    NNP_CUDA(m, cudaGetLastError());
+    return NNP_OK;
+}
+
 extern "C" nnp_status nnp_sync_status(nnp_model* m) {
     if (!m) return NNP_ERR_INVALID_ARG;
     if (!m->have_ws) return NNP_OK;

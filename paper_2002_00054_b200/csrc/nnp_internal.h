@@ -136,6 +136,12 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
 int launch_finalize(const Workspace& w, int64_t n, double* d_e_atom, double* d_e_total, double* d_force,
                     cudaStream_t st);
 
+// MD loop (k_md.cu)
+int launch_vv(int64_t n, int n_elem, const double* h_mass, const int32_t* d_type, const double* d_force, double* d_vel,
+              double* d_pos, double dt, bool drift, cudaStream_t st);
+int launch_ekin(int64_t n, int n_elem, const double* h_mass, const int32_t* d_type, const double* d_vel, double* d_part,
+                double* d_out, cudaStream_t st);
+
 // exports
 int launch_export_counts(const Workspace& w, int64_t n, int n_elem, int32_t* d_counts, cudaStream_t st);
 int launch_export_neighbors(const Workspace& w, int64_t n, int n_elem, int stride, const int64_t* d_offsets,
