@@ -39,8 +39,8 @@ FP64_INSTR_PER_ATOM = {
     True: {"sf": 368e3, "mlp": 33e3, "force": 586e3},      # wide-128 model
 }
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_force2 launch, from the ncu captures under profiles/
-# (r1b_launches_config3.csv for configs[3], r1b_ncu_k_sf2_k_force2.md for configs[2]); null where not captured
-NCU_DRAM_BYTES_K_FORCE2 = {3: 3619019008 + 103957248, 2: 338736896 + 9724160}
+# (r1c_launches_config3.csv for configs[3], r1b_ncu_k_sf2_k_force2.md for configs[2]); null where not captured
+NCU_DRAM_BYTES_K_FORCE2 = {3: 3617511680 + 103882496, 2: 338736896 + 9724160}
 # FP64 pipe peak derived from unit counts and clocks: 148 SMs x 64 DFMA lanes/clk x clocks.max.sm
 FP64_LANES_PER_SM = 64
 N_SM = 148
