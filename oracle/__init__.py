@@ -23,7 +23,8 @@ class _SF(C.Structure):
 class _Model(C.Structure):
     _fields_ = [("n_elem", C.c_int32), ("rc", C.c_double), ("n_sf", C.c_int32),
                 ("sf", C.c_void_p), ("n_layers", C.c_void_p), ("layer_sizes", C.c_void_p),
-                ("weights", C.c_void_p)]
+                ("weights", C.c_void_p), ("sf_shift", C.c_void_p), ("sf_scale", C.c_void_p),
+                ("activation", C.c_int32)]
 
 
 def lib():
@@ -66,8 +67,14 @@ class OracleModel:
         self.n_sf_per_elem = [int(np.sum(sf["central"] == e)) for e in range(self.n_elem)]
         self.g_stride = max(self.n_sf_per_elem)
         self.rc = float(model.rc)
+        # model generality: optional affine SF scaling and tanh activation
+        sc = getattr(model, "sf_scaling", None)
+        self.sf_shift = None if sc is None else np.ascontiguousarray(np.concatenate([np.asarray(a, dtype=np.float64) for a, _ in sc]))
+        self.sf_scale = None if sc is None else np.ascontiguousarray(np.concatenate([np.asarray(b, dtype=np.float64) for _, b in sc]))
+        self.activation = {"softplus": 0, "tanh": 1}[getattr(model, "activation", "softplus")]
         self.c = _Model(self.n_elem, self.rc, sf.shape[0], _ptr(sf), _ptr(self.n_layers),
-                        _ptr(self.layer_sizes), _ptr(self.weights))
+                        _ptr(self.layer_sizes), _ptr(self.weights), _ptr(self.sf_shift), _ptr(self.sf_scale),
+                        self.activation)
 
 
 def fc(r, rc):

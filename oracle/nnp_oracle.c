@@ -54,6 +54,12 @@ typedef struct {
     const int32_t* n_layers;      /* [n_elem] number of weight layers (3 for in-25-25-1) */
     const int32_t* layer_sizes;   /* concatenated, n_layers[e]+1 entries per element     */
     const double* weights;        /* concatenated per element: W1[out][in], b1, W2, b2, ... */
+    /* model generality (n2p2 scales / centres its symmetry functions and offers tanh):
+     * network input x_s = sf_scale_s * (G_s - sf_shift_s); both concatenated per element in G order,
+     * NULL = identity.  activation: 0 softplus (BASELINE.json), 1 tanh; output layer linear. */
+    const double* sf_shift;
+    const double* sf_scale;
+    int32_t activation;
 } oracle_model;
 
 static double now_s(void) {
@@ -222,14 +228,22 @@ static void sf_centre(const oracle_model* M, int tc, int nn, const double* u, co
 static double softplus(double x) { return fmax(x, 0.0) + log1p(exp(-fabs(x))); }
 static double sigmoid(double x) { return 1.0 / (1.0 + exp(-x)); }
 
-void oracle_mlp(int32_t n_layers, const int32_t* sizes, const double* wts, const double* G,
-                double* e_out, double* beta /* may be NULL */) {
+static double act_f(int kind, double z) { return kind == 1 ? tanh(z) : softplus(z); }
+static double act_d(int kind, double z) {
+    if (kind == 1) { const double t = tanh(z); return 1.0 - t * t; }
+    return sigmoid(z);
+}
+
+/* E = NN(x), x_s = scale_s (G_s - shift_s);  beta_s = dE/dG_s = scale_s dE/dx_s */
+void oracle_mlp2(int32_t n_layers, const int32_t* sizes, const double* wts, const double* G,
+                 const double* shift /* may be NULL */, const double* scale /* may be NULL */, int32_t activation,
+                 double* e_out, double* beta /* may be NULL */) {
     int maxw = 0;
     for (int l = 0; l <= n_layers; ++l)
         if (sizes[l] > maxw) maxw = sizes[l];
     double* act = (double*)calloc((size_t)(n_layers + 1) * maxw, sizeof(double)); /* activations */
     double* pre = (double*)calloc((size_t)(n_layers + 1) * maxw, sizeof(double)); /* pre-activations */
-    for (int i = 0; i < sizes[0]; ++i) act[i] = G[i];
+    for (int i = 0; i < sizes[0]; ++i) act[i] = (scale ? scale[i] : 1.0) * (G[i] - (shift ? shift[i] : 0.0));
     const double* p = wts;
     for (int l = 0; l < n_layers; ++l) {
         int nin = sizes[l], nout = sizes[l + 1];
@@ -240,7 +254,7 @@ void oracle_mlp(int32_t n_layers, const int32_t* sizes, const double* wts, const
             double z = b[o];
             for (int i = 0; i < nin; ++i) z += W[(size_t)o * nin + i] * act[(size_t)l * maxw + i];
             pre[(size_t)(l + 1) * maxw + o] = z;
-            act[(size_t)(l + 1) * maxw + o] = (l == n_layers - 1) ? z : softplus(z);
+            act[(size_t)(l + 1) * maxw + o] = (l == n_layers - 1) ? z : act_f(activation, z);
         }
     }
     *e_out = act[(size_t)n_layers * maxw + 0];
@@ -260,15 +274,21 @@ void oracle_mlp(int32_t n_layers, const int32_t* sizes, const double* wts, const
             int nin = sizes[l], nout = sizes[l + 1];
             for (int i = 0; i < nin; ++i) gp[i] = 0.0;
             for (int o = 0; o < nout; ++o) {
-                double dz = g[o] * ((l == n_layers - 1) ? 1.0 : sigmoid(pre[(size_t)(l + 1) * maxw + o]));
+                double dz = g[o] * ((l == n_layers - 1) ? 1.0 : act_d(activation, pre[(size_t)(l + 1) * maxw + o]));
                 for (int i = 0; i < nin; ++i) gp[i] += Wl[l][(size_t)o * nin + i] * dz;
             }
             for (int i = 0; i < nin; ++i) g[i] = gp[i];
         }
-        for (int i = 0; i < sizes[0]; ++i) beta[i] = g[i];
+        for (int i = 0; i < sizes[0]; ++i) beta[i] = (scale ? scale[i] : 1.0) * g[i];
         free(g); free(gp); free(Wl);
     }
     free(act); free(pre);
+}
+
+/* the BASELINE.json network: softplus, unscaled input */
+void oracle_mlp(int32_t n_layers, const int32_t* sizes, const double* wts, const double* G,
+                double* e_out, double* beta /* may be NULL */) {
+    oracle_mlp2(n_layers, sizes, wts, G, NULL, NULL, 0, e_out, beta);
 }
 
 static void element_net(const oracle_model* M, int e, int32_t* n_layers, const int32_t** sizes,
@@ -336,7 +356,10 @@ int32_t oracle_centres(const oracle_model* M, int64_t n, const double* pos, cons
         int32_t nl; const int32_t* sizes; const double* wts;
         element_net(M, tc, &nl, &sizes, &wts);
         double e;
-        oracle_mlp(nl, sizes, wts, Gi, &e, bi);
+        int sf_off = 0;                       /* this element's slice of sf_shift / sf_scale */
+        for (int q2 = 0; q2 < tc; ++q2) sf_off += oracle_n_sf_of(M, q2);
+        oracle_mlp2(nl, sizes, wts, Gi, M->sf_shift ? M->sf_shift + sf_off : NULL,
+                    M->sf_scale ? M->sf_scale + sf_off : NULL, M->activation, &e, bi);
         if (e_atom) e_atom[q] = e;
         if (G) for (int s = 0; s < nsf; ++s) G[q * g_stride + s] = Gi[s];
         if (dEdG) for (int s = 0; s < nsf; ++s) dEdG[q * g_stride + s] = bi[s];

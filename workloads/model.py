@@ -44,6 +44,10 @@ class Model:
     weights: list              # per element: flat f64 [W1(out x in), b1, W2, b2, ..., W_last, b_last]
     name: str = ""
     n_sf_per_elem: list = field(default_factory=list)
+    # model generality: per element (shift[n_sf], scale[n_sf]) with network input
+    # x = scale * (G - shift), or None; hidden activation "softplus" (BASELINE.json) or "tanh"
+    sf_scaling: list | None = None
+    activation: str = "softplus"
 
 
 def radial_etas(n: int) -> np.ndarray:
