@@ -112,6 +112,17 @@ nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d_pos, const
 nnp_status nnp_compute_host(nnp_model* m, int64_t n_atoms, const double* h_pos, const int32_t* h_type,
                             const double box[3], double* h_e_atom, double* h_e_total, double* h_force);
 
+/* ---- model generality (n2p2 models scale / centre their symmetry functions and may use
+ * tanh).  Both settings apply to the following nnp_compute calls; defaults: no scaling, softplus.
+ * nnp_set_sf_scaling: the network of element `elem` reads x_s = h_scale[s] * (G_s - h_shift[s]) instead of G_s
+ *   (HOST arrays of the element's symmetry-function count, in G order; both NULL = back to identity).
+ *   nnp_get_sf still returns the unscaled G, nnp_get_dedg returns dE/dG (= scale * dE/dx).  Synchronises the device.
+ * nnp_set_activation: hidden-layer activation of every element; the output layer stays linear. */
+#define NNP_ACT_SOFTPLUS 0
+#define NNP_ACT_TANH 1
+nnp_status nnp_set_sf_scaling(nnp_model* m, int32_t elem, const double* h_shift, const double* h_scale);
+nnp_status nnp_set_activation(nnp_model* m, int32_t kind);
+
 /* ---- MD loop around the path (the implementation is checked by energy
  * conservation in an NVE run).  Velocity Verlet, everything on the device:
  *     v += (dt/2) F/m ;  x += dt v ;  F = nnp_compute(x) ;  v += (dt/2) F/m

@@ -20,7 +20,7 @@ STAGE_NAMES = ("sort", "neighbors", "symmetry_functions", "networks", "forces", 
 
 # every symbol include/nnp.h declares
 EXPORTS = ("nnp_create", "nnp_destroy", "nnp_set_max_neighbors", "nnp_workspace_bytes", "nnp_compute",
-           "nnp_compute_host", "nnp_md_run", "nnp_md_kinetic_energy", "nnp_sync_status", "nnp_get_neighbor_counts", "nnp_get_neighbors", "nnp_get_sf",
+           "nnp_compute_host", "nnp_set_sf_scaling", "nnp_set_activation", "nnp_md_run", "nnp_md_kinetic_energy", "nnp_sync_status", "nnp_get_neighbor_counts", "nnp_get_neighbors", "nnp_get_sf",
            "nnp_get_dedg", "nnp_g_stride", "nnp_set_timing", "nnp_get_timings", "nnp_last_launch_count",
            "nnp_uses_fast_path", "nnp_measure_fp64_peak", "nnp_last_error", "nnp_version")
 
@@ -62,6 +62,10 @@ def load_library():
     L.nnp_compute.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), vp, vp, vp, vp, C.c_size_t, vp]
     L.nnp_compute_host.restype = C.c_int
     L.nnp_compute_host.argtypes = [vp, i64, vp, vp, C.POINTER(dbl), vp, vp, vp]
+    L.nnp_set_sf_scaling.restype = C.c_int
+    L.nnp_set_sf_scaling.argtypes = [vp, i32, vp, vp]
+    L.nnp_set_activation.restype = C.c_int
+    L.nnp_set_activation.argtypes = [vp, i32]
     L.nnp_md_run.restype = C.c_int
     L.nnp_md_run.argtypes = [vp, i32, dbl, C.POINTER(dbl), i64, vp, vp, vp, C.POINTER(dbl), vp, vp, vp, vp,
                              C.c_size_t, vp]
@@ -145,7 +149,13 @@ class NNP:
     @classmethod
     def from_model(cls, model, device: int = 0):
         """model: any object with .elements .rc .sf .layer_sizes .weights (e.g. workloads.Model)."""
-        return cls(model.elements, model.rc, model.sf, model.layer_sizes, model.weights, device)
+        obj = cls(model.elements, model.rc, model.sf, model.layer_sizes, model.weights, device)
+        if getattr(model, "sf_scaling", None) is not None:
+            for e, (shift, scale) in enumerate(model.sf_scaling):
+                obj.set_sf_scaling(e, shift, scale)
+        if getattr(model, "activation", "softplus") != "softplus":
+            obj.set_activation(model.activation)
+        return obj
 
     def close(self):
         if getattr(self, "_h", None) is not None and self._h.value:
@@ -207,6 +217,20 @@ class NNP:
         if sync:
             self.sync_status()
         return e_atom, e_total, force
+
+    # ---- model generality ------------------------------------------------------------
+    def set_sf_scaling(self, elem, shift, scale):
+        """Network input of element `elem`: x = scale * (G - shift); None, None switches it off."""
+        if shift is None:
+            self._check(self._L.nnp_set_sf_scaling(self._h, int(elem), None, None))
+            return
+        a = np.ascontiguousarray(shift, dtype=np.float64)
+        b = np.ascontiguousarray(scale, dtype=np.float64)
+        self._check(self._L.nnp_set_sf_scaling(self._h, int(elem), a.ctypes.data_as(C.c_void_p),
+                                               b.ctypes.data_as(C.c_void_p)))
+
+    def set_activation(self, name):
+        self._check(self._L.nnp_set_activation(self._h, {"softplus": 0, "tanh": 1}[name]))
 
     # ---- MD loop around the path (velocity Verlet, NVE) ---------------------------------------------
     def _ws_ptr(self, n, dev):

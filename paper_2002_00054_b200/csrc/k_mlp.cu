@@ -29,6 +29,11 @@ struct MlpParams {
 
 __device__ __forceinline__ double softplus_d(double x) { return fmax(x, 0.0) + log1p(exp(-fabs(x))); }
 __device__ __forceinline__ double sigmoid_d(double x) { return 1.0 / (1.0 + exp(-x)); }
+// hidden activation and its derivative: kind 0 softplus (BASELINE.json), 1 tanh
+__device__ __forceinline__ void activate(int kind, double z, double& h, double& dh) {
+    if (kind == 1) { h = tanh(z); dh = fma(-h, h, 1.0); }
+    else { h = softplus_d(z); dh = sigmoid_d(z); }
+}
 
 __host__ __device__ inline int round4(int x) { return (x + 3) & ~3; }
 
@@ -61,7 +66,9 @@ __global__ void __launch_bounds__(MLP_THREADS) k_mlp(const __grid_constant__ Mlp
 
     for (int idx = t; idx < TA * n_in; idx += MLP_THREADS) {
         const int aa = idx / n_in, s = idx - aa * n_in;
-        X0[s * TAP + aa] = aa < na ? p.G[(size_t)(start + aa) * gs + s] : 0.0;
+        double x = aa < na ? p.G[(size_t)(start + aa) * gs + s] : 0.0;
+        if (net.sf_scale) x = net.sf_scale[s] * (x - net.sf_shift[s]);      // affine SF scaling (8(f)4)
+        X0[s * TAP + aa] = x;
     }
     if (t < TA) Al[L][t] = 1.0;
     __syncthreads();
@@ -88,8 +95,10 @@ __global__ void __launch_bounds__(MLP_THREADS) k_mlp(const __grid_constant__ Mlp
 #pragma unroll
                 for (int k = 0; k < 4; ++k)
                     if (ob + k < nout) {
-                        Al[l + 1][(ob + k) * TAP + a] = softplus_d(z[k]);
-                        Dl[l + 1][(ob + k) * TAP + a] = sigmoid_d(z[k]);
+                        double h, dh;
+                        activate(net.activation, z[k], h, dh);
+                        Al[l + 1][(ob + k) * TAP + a] = h;
+                        Dl[l + 1][(ob + k) * TAP + a] = dh;
                     }
             } else if (ob == 0 && a < na) {
                 p.e_sorted[start + a] = z0;
@@ -125,7 +134,9 @@ __global__ void __launch_bounds__(MLP_THREADS) k_mlp(const __grid_constant__ Mlp
 
     for (int idx = t; idx < na * gs; idx += MLP_THREADS) {
         const int aa = idx / gs, s = idx - aa * gs;
-        p.dEdG[(size_t)(start + aa) * gs + s] = s < n_in ? X0[s * TAP + aa] : 0.0;
+        double b = s < n_in ? X0[s * TAP + aa] : 0.0;
+        if (net.sf_scale && s < n_in) b *= net.sf_scale[s];                 // dE/dG = scale * dE/dx
+        p.dEdG[(size_t)(start + aa) * gs + s] = b;
     }
 }
 

@@ -23,6 +23,7 @@ struct nnp_model {
     int variant[MAX_ELEM] = {0, 0, 0, 0};
     NetDesc nets[MAX_ELEM];
     double* d_weights[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
+    double* d_scaling[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};   // [2][n_sf]: shift, scale (or null)
     // last nnp_compute (for the exports)
     Workspace ws;
     bool have_ws = false;
@@ -343,6 +344,7 @@ extern "C" void nnp_destroy(nnp_model* m) {
     for (int c = 0; c < MAX_ELEM; ++c) {
         if (m->d_prog[c]) cudaFree(m->d_prog[c]);
         if (m->d_weights[c]) cudaFree(m->d_weights[c]);
+        if (m->d_scaling[c]) cudaFree(m->d_scaling[c]);
     }
     if (m->h_status) cudaFreeHost(m->h_status);
     if (m->ev_created)
@@ -355,6 +357,35 @@ extern "C" void nnp_destroy(nnp_model* m) {
     if (m->hd_etot) cudaFree(m->hd_etot);
     if (m->hstream) cudaStreamDestroy(m->hstream);
     delete m;
+}
+
+extern "C" nnp_status nnp_set_sf_scaling(nnp_model* m, int32_t elem, const double* h_shift, const double* h_scale) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    if (elem < 0 || elem >= m->n_elem) return fail(m, NNP_ERR_INVALID_ARG, "element index out of range");
+    if ((h_shift == nullptr) != (h_scale == nullptr)) return fail(m, NNP_ERR_INVALID_ARG, "shift and scale go together");
+    DeviceGuard dg(m->device);
+    if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
+    NNP_CUDA(m, cudaDeviceSynchronize());          // the old arrays may still be in use
+    NetDesc& nd = m->nets[elem];
+    if (m->d_scaling[elem]) { cudaFree(m->d_scaling[elem]); m->d_scaling[elem] = nullptr; }
+    nd.sf_shift = nd.sf_scale = nullptr;
+    if (!h_shift) return NNP_OK;
+    const int n = m->n_sf_elem[elem];
+    for (int s = 0; s < n; ++s)
+        if (!std::isfinite(h_shift[s]) || !std::isfinite(h_scale[s])) return fail(m, NNP_ERR_INVALID_ARG, "non-finite scaling");
+    NNP_CUDA(m, cudaMalloc(&m->d_scaling[elem], 2 * (size_t)n * sizeof(double)));
+    NNP_CUDA(m, cudaMemcpy(m->d_scaling[elem], h_shift, n * sizeof(double), cudaMemcpyHostToDevice));
+    NNP_CUDA(m, cudaMemcpy(m->d_scaling[elem] + n, h_scale, n * sizeof(double), cudaMemcpyHostToDevice));
+    nd.sf_shift = m->d_scaling[elem];
+    nd.sf_scale = m->d_scaling[elem] + n;
+    return NNP_OK;
+}
+
+extern "C" nnp_status nnp_set_activation(nnp_model* m, int32_t kind) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    if (kind != NNP_ACT_SOFTPLUS && kind != NNP_ACT_TANH) return fail(m, NNP_ERR_INVALID_ARG, "unknown activation");
+    for (int c = 0; c < m->n_elem; ++c) m->nets[c].activation = kind;
+    return NNP_OK;
 }
 
 extern "C" nnp_status nnp_set_max_neighbors(nnp_model* m, int32_t max_neighbors) {

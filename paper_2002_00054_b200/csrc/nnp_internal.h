@@ -74,6 +74,11 @@ struct NetDesc {
     int32_t w_off[MAX_LAYERS];
     int32_t b_off[MAX_LAYERS];
     const double* weights;           // device
+    // model generality: network input x_s = sf_scale[s] * (G_s - sf_shift[s]); device arrays
+    // [sizes[0]] or nullptr (identity); activation 0 = softplus, 1 = tanh (hidden layers; output linear)
+    const double* sf_shift;
+    const double* sf_scale;
+    int32_t activation;
 };
 
 // Cell grid of one nnp_compute call (host-built, passed by value).

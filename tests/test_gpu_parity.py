@@ -140,6 +140,28 @@ def test_fast_path_large_cutoff_general_exp():
     _check_full(model, sysm)
 
 
+@pytest.mark.parametrize("activation", ["softplus", "tanh"])
+def test_sf_scaling_and_activation(activation):
+    # model generality: affine SF scaling in front of the networks, tanh hidden layers
+    import copy
+    model = copy.deepcopy(W.make_model(False))
+    rng = np.random.default_rng(3)
+    model.sf_scaling = [(rng.uniform(0.0, 0.5, n), rng.uniform(0.2, 3.0, n)) for n in model.n_sf_per_elem]
+    model.activation = activation
+    sysm = W.make_water(150, 31, L=15.3)
+    _check_full(model, sysm)
+    # switching the scaling off again restores the plain model
+    from paper_2002_00054_b200 import NNP
+    nnp = NNP.from_model(model)
+    for e in range(len(model.elements)):
+        nnp.set_sf_scaling(e, None, None)
+    nnp.set_activation("softplus")
+    _, E, _ = _run(nnp, sysm.pos, sysm.types, sysm.box)
+    ref = oracle.compute(oracle.OracleModel(W.make_model(False)), sysm.pos, sysm.types, sysm.box)
+    assert abs(E - ref.e_total) <= E_REL * abs(ref.e_total)
+    nnp.close()
+
+
 def test_single_element_radial_only():
     model = tiny_model([(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0), (0, 2, 0, 0, 0.4, 2.0, 0.0, 0.0)], hidden=(4,))
     sysm = W.make_water(60, 3, L=12.4)
