@@ -202,6 +202,11 @@ def test_full_size_configs_sampled(k):
     for m in samples[:3]:
         for j in idx[off[m]:off[m + 1]][:10]:
             assert m in idx[off[j]:off[j + 1]]
+    # repeatability at full size (a shared-memory race in the lane-owned kernels would show up as a run-to-run
+    # difference well above the reordering noise of the FP64 global atomics; compute-sanitizer is closed on this pool)
+    e_atom2, e_total2, force2 = _run(nnp, sysm.pos, sysm.types, sysm.box)
+    assert e_total2 == e_total and np.array_equal(e_atom2, e_atom)
+    assert np.abs(force2 - force).max() < 1e-11
     nnp.close()
 
 
