@@ -37,6 +37,9 @@ UNIT = "atom-steps/s"
 FP64_INSTR_PER_ATOM = {
     False: {"sf": 230e3, "mlp": 7e3, "force": 400e3},     # base-52 model
     True: {"sf": 368e3, "mlp": 33e3, "force": 586e3},      # wide-128 model
+    # Ni-like metal (not a BASELINE.json config): 18 neighbours, 153 enumerated (j,k), 60 contributing
+    # triplets per atom, same per-unit costs: SF 18*230 + 153*7 + 60*93, force 18*264 + 153*7 + 60*179, MLP 20-30-30-1
+    "metal": {"sf": 10.8e3, "mlp": 3.3e3, "force": 16.6e3},
 }
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_force2 launch, from the ncu captures under profiles/
 # (r1c_launches_config3.csv for configs[3], r1b_ncu_k_sf2_k_force2.md for configs[2]); null where not captured
@@ -228,6 +231,8 @@ def main():
     sysm, model = W.build(cfg)
     n = sysm.n_atoms
     nnp = NNP.from_model(model, device=local)
+    if cfg.kind == "metal":
+        nnp.set_max_neighbors(48)      # 18 neighbours per atom: the 64-slot, one-warp-per-centre kernels
     pos = torch.tensor(sysm.pos, dtype=torch.float64, device=dev)
     typ = torch.tensor(sysm.types, dtype=torch.int32, device=dev)
     out = (torch.empty(n, dtype=torch.float64, device=dev), torch.empty(1, dtype=torch.float64, device=dev),
@@ -322,11 +327,11 @@ def main():
     peaks = _peaks()
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     peak_alu = N_SM * FP64_LANES_PER_SM * sm_max * 1e6
-    instr = FP64_INSTR_PER_ATOM[cfg.wide]
+    instr = FP64_INSTR_PER_ATOM["metal" if cfg.kind == "metal" else cfg.wide]
     force_ms = float(stage_ms[4])
     achieved = instr["force"] * n / (force_ms * 1e-3)
     total_instr = sum(instr.values()) * n
-    hbm_bytes_per_atom = 2.8e3 if not cfg.wide else 5.2e3
+    hbm_bytes_per_atom = 1.0e3 if cfg.kind == "metal" else (2.8e3 if not cfg.wide else 5.2e3)
     roofline = {
         "bound": "alu", "kernel": "k_force2", "achieved": achieved / 1e12, "peak": peak_alu / 1e12,
         "unit": "T FP64 instr/s", "frac": achieved / peak_alu, "traffic": NCU_DRAM_BYTES_K_FORCE2.get(args.config),

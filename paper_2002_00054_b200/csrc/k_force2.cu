@@ -412,21 +412,23 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
 #endif
 constexpr int F2_WPC = NNP_F2_WPC;
 
-template <class Spec, int CAPA, bool TINY>
+template <class Spec, int CAPA, bool TINY, int WPC = F2_WPC>
 static int launch_capa(const Force2Params& p, cudaStream_t st) {
-    const size_t smem = force2_smem<Spec>(CAPA, p.g_stride, p.n_elem, F2_WPC);
+    const size_t smem = force2_smem<Spec>(CAPA, p.g_stride, p.n_elem, WPC);
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_force2<Spec, F2_WPC, CAPA, TINY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaFuncSetAttribute(k_force2<Spec, WPC, CAPA, TINY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         configured = true;
     }
-    k_force2<Spec, F2_WPC, CAPA, TINY><<<(unsigned)p.n, F2_WPC * 32, smem, st>>>(p);
+    k_force2<Spec, WPC, CAPA, TINY><<<(unsigned)p.n, WPC * 32, smem, st>>>(p);
     return 1;
 }
 
 // slot capacity = smallest instantiated CAPA that holds max_neighbors (nnp_set_max_neighbors: 32..255)
 template <class Spec, bool TINY>
 static int launch_one2(const Force2Params& p, cudaStream_t st) {
+    // small neighbourhoods (metals: ~20 neighbours, ~60 triplets per centre): 64 slots, ONE warp per centre
+    if (p.cap <= 64) return launch_capa<Spec, 64, TINY, 1>(p, st);
     if (p.cap <= 128) return launch_capa<Spec, 128, TINY>(p, st);
     if (p.cap <= 160) return launch_capa<Spec, 160, TINY>(p, st);
     return launch_capa<Spec, 256, TINY>(p, st);

@@ -270,20 +270,22 @@ int launch_word_offsets(const Workspace& w, const Grid& g, int64_t n, int n_elem
 #endif
 constexpr int SF2_WPC = NNP_SF2_WPC;
 
-template <class Spec, int CAPA, bool TINY>
+template <class Spec, int CAPA, bool TINY, int WPC = SF2_WPC>
 static int launch_capa_sf(const Sf2Params& p, cudaStream_t st) {
-    const size_t smem = sf2_smem<Spec>(CAPA, p.n_elem, SF2_WPC);
+    const size_t smem = sf2_smem<Spec>(CAPA, p.n_elem, WPC);
     static bool configured = false;
     if (!configured) {
-        cudaFuncSetAttribute(k_sf2<Spec, SF2_WPC, CAPA, TINY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaFuncSetAttribute(k_sf2<Spec, WPC, CAPA, TINY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         configured = true;
     }
-    k_sf2<Spec, SF2_WPC, CAPA, TINY><<<(unsigned)p.n, SF2_WPC * 32, smem, st>>>(p);
+    k_sf2<Spec, WPC, CAPA, TINY><<<(unsigned)p.n, WPC * 32, smem, st>>>(p);
     return 1;
 }
 
 template <class Spec, bool TINY>
 static int launch_one_sf2(const Sf2Params& p, cudaStream_t st) {
+    // small neighbourhoods (metals: ~20 neighbours, ~60 triplets per centre): 64 slots, ONE warp per centre
+    if (p.cap <= 64) return launch_capa_sf<Spec, 64, TINY, 1>(p, st);
     if (p.cap <= 128) return launch_capa_sf<Spec, 128, TINY>(p, st);
     if (p.cap <= 160) return launch_capa_sf<Spec, 160, TINY>(p, st);
     return launch_capa_sf<Spec, 256, TINY>(p, st);

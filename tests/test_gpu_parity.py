@@ -162,6 +162,14 @@ def test_sf_scaling_and_activation(activation):
     nnp.close()
 
 
+def test_metal_like_small_neighbourhoods():
+    # Ni-like fcc metal, rc = 3.9 A, 18 neighbours per atom -> with max_neighbors <= 64 the
+    # 64-slot, one-warp-per-centre instantiation of the lane-owned kernels
+    sysm, model = W.build(W.Config("fcc6", 6, False, 1, 11, 12, None, "metal"))
+    _check_full(model, sysm, max_neighbors=48)
+    _check_full(model, sysm)                       # and the default 160-slot kernels on the same system
+
+
 def test_single_element_radial_only():
     model = tiny_model([(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0), (0, 2, 0, 0, 0.4, 2.0, 0.0, 0.0)], hidden=(4,))
     sysm = W.make_water(60, 3, L=12.4)
