@@ -5,6 +5,9 @@
 //   hidden: h = softplus(W h_prev + b) = max(x,0) + log1p(exp(-|x|)),  softplus' = 1/(1+exp(-x));
 //   output layer linear (readings 5, C12).
 //
+// Two kernels: k_mlp_reg (below) for small networks -- n_in -> n1 -> n2 -> 1 with n1, n2 <= 32, the paper's
+// "~30 x 2" (L40) and BASELINE.json's 25-25 -- with the weights in the kernel parameter block, and the tiled
+// k_mlp<TA> for everything else (the 64-64 networks of the wide config, other depths).
 // The paper calls this "a minor portion of the overall computation" (L40, L90); here it is ~1 %
 // (base) to ~3 % (wide) of the FP64 work, so it runs on plain DFMA: a tile of TA atoms per CTA,
 // activations in shared memory as [neuron][atom] (conflict-free, stride TA+1), each thread owns
@@ -140,6 +143,121 @@ __global__ void __launch_bounds__(MLP_THREADS) k_mlp(const __grid_constant__ Mlp
     }
 }
 
+// ---- register kernel for small networks (n_in -> n1 -> n2 -> 1, n1, n2 <= 32, n_in <= 80) ----------------
+// One thread per atom, every activation in registers, the weights in the kernel PARAMETER block: their
+// index is warp-uniform, so they arrive through the constant cache in uniform registers (LDCU) and the
+// FP64 FMAs take them as operands -- no shared-memory or L1 operand traffic at all.  The tiled kernel above
+// is bound by exactly that traffic (3 loads per 4 FMAs): 4.6 ms at 2.1 M atoms against ~1 ms of FP64 work.
+struct MlpRegParams {
+    MlpRegWeights W;
+    const int32_t* elem_begin;
+    const int32_t* elem_end;
+    const double* G;
+    double* dEdG;
+    double* e_sorted;
+    const double* sf_shift;
+    const double* sf_scale;
+    int g_stride, activation;
+};
+static_assert(sizeof(MlpRegParams) <= 32000, "kernel parameter block limit (32,764 B)");
+
+constexpr int MLP_REG_THREADS = 64;
+
+// Loops are ROLLED over the input index (run-time, warp-uniform -> LDCU weight loads) and UNROLLED over the
+// 32 outputs held in registers; per-thread hidden activations / derivatives sit in shared memory as
+// [neuron][thread] columns (conflict-free), so no register array is ever indexed dynamically.
+__global__ void __launch_bounds__(MLP_REG_THREADS) k_mlp_reg(const __grid_constant__ MlpRegParams p) {
+    constexpr int H = MLP_REG_H, NT = MLP_REG_THREADS;
+    __shared__ double sh_h[H][NT];               // h1, later delta_1
+    __shared__ double sh_s[H][NT];               // act'(z1)
+    const int t = threadIdx.x;
+    const int begin = *p.elem_begin, end = *p.elem_end;
+    const int64_t a = (int64_t)begin + (int64_t)blockIdx.x * NT + t;
+    if (a >= end) return;                        // no barrier below: a thread only touches its own column
+    const int n_in = p.W.n_in, n1 = p.W.n1, n2 = p.W.n2, gs = p.g_stride;
+    const double* W1 = p.W.w;                    // [n_in][H]
+    const double* B1 = W1 + n_in * H;
+    const double* W2 = B1 + H;                   // [H][H], input-major
+    const double* B2 = W2 + H * H;
+    const double* W3 = B2 + H;
+    const double* Grow = p.G + (size_t)a * gs;
+    double* Brow = p.dEdG + (size_t)a * gs;
+
+    double acc[H];
+    // ---- forward, layer 1: z1 = b1 + W1^T x
+#pragma unroll
+    for (int o = 0; o < H; ++o) acc[o] = B1[o];
+#pragma unroll 1
+    for (int i = 0; i < n_in; ++i) {
+        double x = Grow[i];
+        if (p.sf_scale) x = p.sf_scale[i] * (x - p.sf_shift[i]);
+#pragma unroll
+        for (int o = 0; o < H; ++o) acc[o] = fma(W1[i * H + o], x, acc[o]);
+    }
+#pragma unroll
+    for (int o = 0; o < H; ++o) sh_h[o][t] = acc[o];
+#pragma unroll 1
+    for (int o = 0; o < n1; ++o) {               // rolled: ONE copy of the activation code
+        double h, d;
+        activate(p.activation, sh_h[o][t], h, d);
+        sh_h[o][t] = h;
+        sh_s[o][t] = d;
+    }
+    // ---- layer 2: z2 = b2 + W2^T h1
+#pragma unroll
+    for (int o = 0; o < H; ++o) acc[o] = B2[o];
+#pragma unroll 1
+    for (int i = 0; i < n1; ++i) {
+        const double x = sh_h[i][t];
+#pragma unroll
+        for (int o = 0; o < H; ++o) acc[o] = fma(W2[i * H + o], x, acc[o]);
+    }
+    double e = W3[H];                            // b3
+#pragma unroll
+    for (int o = 0; o < H; ++o) sh_h[o][t] = acc[o];      // h1 is dead: its columns take z2, then delta_2
+#pragma unroll 1
+    for (int o = 0; o < n2; ++o) {
+        double h, d;
+        activate(p.activation, sh_h[o][t], h, d);
+        e = fma(W3[o], h, e);
+        sh_h[o][t] = W3[o] * d;                  // delta_2[o] = w3[o] act'(z2[o])
+    }
+#pragma unroll
+    for (int o = 0; o < H; ++o) acc[o] = o < n2 ? sh_h[o][t] : 0.0;
+    p.e_sorted[a] = e;
+    // ---- backward: delta_1[i] = act'(z1[i]) sum_o W2[i][o] delta_2[o]   (delta_2 in registers)
+#pragma unroll 1
+    for (int i = 0; i < n1; ++i) {
+        double g0 = 0.0, g1 = 0.0, g2 = 0.0, g3 = 0.0;
+#pragma unroll
+        for (int o = 0; o < H; o += 4) {
+            g0 = fma(W2[i * H + o], acc[o], g0);
+            g1 = fma(W2[i * H + o + 1], acc[o + 1], g1);
+            g2 = fma(W2[i * H + o + 2], acc[o + 2], g2);
+            g3 = fma(W2[i * H + o + 3], acc[o + 3], g3);
+        }
+        sh_h[i][t] = sh_s[i][t] * ((g0 + g1) + (g2 + g3));
+    }
+    // ---- beta_k = dE/dG_k = scale_k sum_i W1[k][i] delta_1[i]   (delta_1 into registers)
+#pragma unroll
+    for (int i = 0; i < H; ++i) acc[i] = i < n1 ? sh_h[i][t] : 0.0;
+#pragma unroll 1
+    for (int k = 0; k < n_in; ++k) {
+        double g0 = 0.0, g1 = 0.0, g2 = 0.0, g3 = 0.0;
+#pragma unroll
+        for (int i = 0; i < H; i += 4) {
+            g0 = fma(W1[k * H + i], acc[i], g0);
+            g1 = fma(W1[k * H + i + 1], acc[i + 1], g1);
+            g2 = fma(W1[k * H + i + 2], acc[i + 2], g2);
+            g3 = fma(W1[k * H + i + 3], acc[i + 3], g3);
+        }
+        double b = (g0 + g1) + (g2 + g3);
+        if (p.sf_scale) b *= p.sf_scale[k];
+        Brow[k] = b;
+    }
+    for (int k = n_in; k < gs; ++k) Brow[k] = 0.0;
+}
+
 size_t mlp_smem_bytes(const NetDesc& net, int TA) {
     size_t rows = net.sizes[0] + 1;
     for (int l = 1; l < net.n_layers; ++l) rows += 2 * (size_t)net.sizes[l];
@@ -167,6 +285,17 @@ int launch_mlp(const Workspace& w, int64_t n, int n_elem, int ncell, const NetDe
         p.elem_begin = w.cell_start + (size_t)e * ncell;
         p.elem_end = w.cell_start + (size_t)(e + 1) * ncell;
         p.G = w.G; p.dEdG = w.dEdG; p.e_sorted = w.e_sorted; p.g_stride = g_stride;
+        if (nets[e].reg) {          // small network: register kernel, weights in the parameter block
+            MlpRegParams q;
+            q.W = *nets[e].reg;
+            q.elem_begin = p.elem_begin; q.elem_end = p.elem_end;
+            q.G = w.G; q.dEdG = w.dEdG; q.e_sorted = w.e_sorted;
+            q.sf_shift = nets[e].sf_shift; q.sf_scale = nets[e].sf_scale;
+            q.g_stride = g_stride; q.activation = nets[e].activation;
+            k_mlp_reg<<<(unsigned)((n + MLP_REG_THREADS - 1) / MLP_REG_THREADS), MLP_REG_THREADS, 0, st>>>(q);
+            ++launches;
+            continue;
+        }
         const size_t budget = 100 * 1024;
         // 32 atoms per CTA: 8 thread groups cover the 7 output blocks of a 25-wide layer in one round
         // (measured 4.6 ms against 6.5 ms with 64 atoms / 4 groups at 2.1 M atoms)

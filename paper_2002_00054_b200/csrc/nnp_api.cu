@@ -23,7 +23,8 @@ struct nnp_model {
     int variant[MAX_ELEM] = {0, 0, 0, 0};
     NetDesc nets[MAX_ELEM];
     double* d_weights[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
-    double* d_scaling[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};   // [2][n_sf]: shift, scale (or null)
+    double* d_scaling[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
+    MlpRegWeights* reg_w[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};   // host, see NetDesc::reg   // [2][n_sf]: shift, scale (or null)
     // last nnp_compute (for the exports)
     Workspace ws;
     bool have_ws = false;
@@ -314,6 +315,36 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
             for (int o = 0; o < nout; ++o) packed[nd.b_off[l] + o] = B[o];
         }
         if (mlp_smem_bytes(nd, 8) > 200 * 1024) return bail(NNP_ERR_INVALID_ARG, "network too large for the shared-memory tile");
+        // parameter-block copy for the register kernel: n_in -> n1 -> n2 -> 1 with n1, n2 <= 32
+        if (L == 3 && sz[1] <= MLP_REG_H && sz[2] <= MLP_REG_H &&
+            (size_t)sz[0] * MLP_REG_H + 2 * MLP_REG_H + MLP_REG_H * MLP_REG_H + MLP_REG_H + 1 <= (size_t)MLP_REG_MAXW) {
+            MlpRegWeights* R = new MlpRegWeights();
+            std::memset(R, 0, sizeof(*R));
+            R->n_in = sz[0]; R->n1 = sz[1]; R->n2 = sz[2];
+            const int H = MLP_REG_H;
+            const double* W1 = weights[c];
+            const double* B1 = W1 + (size_t)sz[1] * sz[0];
+            const double* W2 = B1 + sz[1];
+            const double* B2 = W2 + (size_t)sz[2] * sz[1];
+            const double* W3 = B2 + sz[2];
+            const double* B3 = W3 + sz[2];
+            double* q = R->w;
+            for (int o = 0; o < sz[1]; ++o)
+                for (int i = 0; i < sz[0]; ++i) q[(size_t)i * H + o] = W1[(size_t)o * sz[0] + i];
+            q += (size_t)sz[0] * H;
+            for (int o = 0; o < sz[1]; ++o) q[o] = B1[o];
+            q += H;
+            for (int o = 0; o < sz[2]; ++o)
+                for (int i = 0; i < sz[1]; ++i) q[(size_t)i * H + o] = W2[(size_t)o * sz[1] + i];
+            q += (size_t)H * H;
+            for (int o = 0; o < sz[2]; ++o) q[o] = B2[o];
+            q += H;
+            for (int o = 0; o < sz[2]; ++o) q[o] = W3[o];
+            q += H;
+            q[0] = B3[0];
+            m->reg_w[c] = R;
+            nd.reg = R;
+        }
         packed_all[c].swap(packed);
     }
     for (int c = 0; c < n_elem; ++c) {
@@ -345,6 +376,7 @@ extern "C" void nnp_destroy(nnp_model* m) {
         if (m->d_prog[c]) cudaFree(m->d_prog[c]);
         if (m->d_weights[c]) cudaFree(m->d_weights[c]);
         if (m->d_scaling[c]) cudaFree(m->d_scaling[c]);
+        delete m->reg_w[c];
     }
     if (m->h_status) cudaFreeHost(m->h_status);
     if (m->ev_created)

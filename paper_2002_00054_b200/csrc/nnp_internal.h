@@ -64,6 +64,16 @@ struct ElemProgram {
     AngularSF ang[MAX_ANG_TOTAL];
 };
 
+// Small networks (two hidden layers of width <= 32, <= 80 inputs) also travel in the KERNEL PARAMETER block
+// (k_mlp_reg, k_mlp.cu): warp-uniform weights then come through the constant cache into uniform registers
+// instead of through the load/store pipe.  Hidden widths are padded to 32 with zero weights.
+constexpr int MLP_REG_H = 32;
+constexpr int MLP_REG_MAXW = 3700;
+struct MlpRegWeights {
+    int32_t n_in, n1, n2, pad;
+    double w[MLP_REG_MAXW];          // W1[n_in][32] | b1[32] | W2[32][32] (input-major) | b2[32] | w3[32] | b3
+};
+
 // One element's network in device memory.  `weights` holds, per layer l (all blocks padded to
 // multiples of 4 doubles, zero filled): WT_l [n_in][round4(n_out)] (transposed, forward pass),
 // W_l [n_out][round4(n_in)] (backward pass), b_l [round4(n_out)].
@@ -79,6 +89,7 @@ struct NetDesc {
     const double* sf_shift;
     const double* sf_scale;
     int32_t activation;
+    const MlpRegWeights* reg;        // HOST memory (model-owned) or nullptr: parameter-block copy for k_mlp_reg
 };
 
 // Cell grid of one nnp_compute call (host-built, passed by value).
