@@ -15,7 +15,8 @@
 // FP64 RED per component per neighbour; the centre receives minus the sum.
 //
 // Coefficients: the lane keeps c_b = beta_b 2^(1-zeta_b) of its current pair group in registers
-// (NACC <= 12) -- per-lane table loads from shared memory cost 4 wavefronts each (ncu, r1b) -- and gets
+// (NACC <= 12; larger sets load them per eta as 128-bit pairs) -- per-lane table loads from shared memory
+// cost 4 wavefronts each (ncu, r1b) -- and gets
 // dP/dcos from the SAME coefficients with pre-scaled powers zeta (1 +- cos)^(zeta-1): the factor zeta =
 // 2^b is an integer add on the exponent field, the factor lambda a negated operand.
 #include "angular.cuh"
@@ -199,8 +200,8 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
                         if (ee < e) a += __popc(mk);
                         else if (ee == e) a += __popc(mk & ((1u << tid) - 1u));
                     }
-                    if constexpr (REGC) btc[pr * 2 * bt2_stride<Spec>() + a] = bc;
-                    else bt[pr * bt2_stride<Spec>() + a] = make_double2(bc, bc * (double)zeta * lam);
+                    btc[pr * 2 * bt2_stride<Spec>() + a] = bc;
+                    (void)zeta; (void)lam;
                 }
             }
         }
@@ -293,6 +294,7 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
             }
         }
         __syncwarp();
+        // c_b of the lane's pair group: registers (REGC) or, for the large sets, 128-bit loads of c pairs per eta
         const double2* btg = bt + max(paircur, 0) * bt2_stride<Spec>();
         const int k = active ? wk.pop() : max(jcur, 0);
         const int rank = conflict_rank(k, active, lane);       // issued early: its latency hides behind the FP64 work
@@ -324,31 +326,38 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_cons
                 pd[l][b] = pd[l][b - 1] * pw[l][b - 1];
             }
         }
-        if constexpr (REGC) {
 #pragma unroll
-            for (int b = 1; b <= Spec::MAXBIT; ++b) {
-                pd[0][b] = scale2(pd[0][b], b);
-                pd[1][b] = scale2(pd[1][b], b);
-            }
+        for (int b = 1; b <= Spec::MAXBIT; ++b) {       // times zeta = 2^b: dP/dcos comes from the SAME coefficients
+            pd[0][b] = scale2(pd[0][b], b);
+            pd[1][b] = scale2(pd[1][b], b);
         }
         double Z0 = 0.0, Z1 = 0.0, Z2 = 0.0;
 #pragma unroll
         for (int e = 0; e < Spec::NETA; ++e) {
             double T0 = 0.0, T1 = 0.0;
+            // the coefficients of eta_e sit at consecutive (even-aligned) accumulator indices
+            constexpr int NE = 16;
+            double ce[REGC ? 1 : NE];
+            if constexpr (!REGC) {
+                const int base = acc_index<Spec>(e, 0) & ~1;
+#pragma unroll
+                for (int q = 0; q < NE / 2; ++q) {
+                    if (base + 2 * q < acc_index<Spec>(e + 1, 0)) {          // folds after unrolling: only this eta's pairs
+                        const double2 v = btg[(base >> 1) + q];
+                        ce[2 * q] = v.x; ce[2 * q + 1] = v.y;
+                    } else { ce[2 * q] = 0.0; ce[2 * q + 1] = 0.0; }
+                }
+            }
 #pragma unroll
             for (int b = 0; b <= Spec::MAXBIT; ++b) {
 #pragma unroll
                 for (int l = 0; l < 2; ++l)
                     if (Spec::mask(e) >> (8 * l + b) & 1u) {
-                        if constexpr (REGC) {
-                            const double c = cf[acc_index<Spec>(e, 8 * l + b)];
-                            T0 = fma(c, pw[l][b], T0);
-                            T1 = l == 0 ? fma(c, pd[l][b], T1) : fma(-c, pd[l][b], T1);
-                        } else {
-                            const double2 c = btg[acc_index<Spec>(e, 8 * l + b)];
-                            T0 = fma(c.x, pw[l][b], T0);
-                            T1 = fma(c.y, pd[l][b], T1);
-                        }
+                        double c;
+                        if constexpr (REGC) c = cf[acc_index<Spec>(e, 8 * l + b)];
+                        else c = ce[acc_index<Spec>(e, 8 * l + b) - (acc_index<Spec>(e, 0) & ~1)];
+                        T0 = fma(c, pw[l][b], T0);
+                        T1 = l == 0 ? fma(c, pd[l][b], T1) : fma(-c, pd[l][b], T1);
                     }
             }
             const double A = T0 * Y[e];
