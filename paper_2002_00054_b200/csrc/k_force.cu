@@ -279,14 +279,6 @@ static int launch_one(const ForceParams& p, cudaStream_t st) {
     return 1;
 }
 
-size_t force_smem_bytes(int variant, int cap, int g_stride, int n_elem) {
-    switch (variant) {
-        case ANG_BASE12: return FC_WARPS * force_warp_smem<SpecBase12>(cap, g_stride, n_elem);
-        case ANG_WIDE32: return FC_WARPS * force_warp_smem<SpecWide32>(cap, g_stride, n_elem);
-        default: return FC_WARPS * force_warp_smem<SpecGeneric>(cap, g_stride, n_elem);
-    }
-}
-
 int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
                  const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st) {
     if (n == 0) return 0;

@@ -180,14 +180,6 @@ static int launch_one(const SfParams& p, cudaStream_t st) {
     return 1;
 }
 
-size_t sf_smem_bytes(int variant, int cap) {
-    switch (variant) {
-        case ANG_BASE12: return SF_WARPS * sf_warp_smem<SpecBase12>(cap);
-        case ANG_WIDE32: return SF_WARPS * sf_warp_smem<SpecWide32>(cap);
-        default: return SF_WARPS * sf_warp_smem<SpecGeneric>(cap);
-    }
-}
-
 int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
               const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st) {
     if (n == 0) return 0;

@@ -169,8 +169,6 @@ int launch_scan_i64_from_i32(const int32_t* d_in, int64_t n, int64_t* d_out /* n
 void exclusive_scan_i32(int32_t* d_data, int64_t n, int32_t* d_tmp, cudaStream_t st, int* launches);
 
 size_t mlp_smem_bytes(const NetDesc& net, int ta);
-size_t sf_smem_bytes(int variant, int cap);
-size_t force_smem_bytes(int variant, int cap, int g_stride, int n_elem);
 
 double fp64_peak(int device, double seconds, double* sustained, cudaError_t* err);
 
