@@ -46,6 +46,13 @@ k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
     else if (cx == g.nc[0] - 1) { xr0[0] = 0; xr1[0] = 0; xr0[1] = cx - 1; xr1[1] = cx; nxr = 2; }
     else { xr0[0] = cx - 1; xr1[0] = cx + 1; nxr = 1; }
 
+    // An atom of an interior cell (and >= 4 cells along the dimension) never needs the +-L of the minimum
+    // image: its candidates are less than two cell widths <= L/2 away, so both conditions of min_image_1d
+    // are false and the raw difference IS the result (same bits).  Warp-uniform -> 12 instructions fewer
+    // per chunk of candidates for ~87 % of the atoms (the kernel is issue-bound: ncu, 83 % issue slots).
+    const bool wx = !(g.nc[0] >= 4 && cx >= 1 && cx <= g.nc[0] - 2);
+    const bool wy = !(g.nc[1] >= 4 && cy >= 1 && cy <= g.nc[1] - 2);
+    const bool wz = !(g.nc[2] >= 4 && cz >= 1 && cz <= g.nc[2] - 2);
     int32_t* row = nbr + (size_t)i * stride;
     int cnt = 0;
     const int nrun = nz * ny * nxr;                     // <= 18 contiguous runs of candidates per element
@@ -82,9 +89,9 @@ k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
             const int j = __shfl_sync(0xffffffffu, j0, lo) + (f - __shfl_sync(0xffffffffu, P, lo));
             bool hit = false;
             if (f < total && j != i) {
-                const double dx = min_image_1d(xi, sx[j], g.box[0], g.half[0]);
-                const double dy = min_image_1d(yi, sy[j], g.box[1], g.half[1]);
-                const double dz = min_image_1d(zi, sz[j], g.box[2], g.half[2]);
+                const double dx = wx ? min_image_1d(xi, sx[j], g.box[0], g.half[0]) : __dsub_rn(sx[j], xi);
+                const double dy = wy ? min_image_1d(yi, sy[j], g.box[1], g.half[1]) : __dsub_rn(sy[j], yi);
+                const double dz = wz ? min_image_1d(zi, sz[j], g.box[2], g.half[2]) : __dsub_rn(sz[j], zi);
                 hit = dist2_exact(dx, dy, dz) < rc2;
             }
             const unsigned m = __ballot_sync(0xffffffffu, hit);
