@@ -10,7 +10,8 @@
 //     z = (pi c / (2 rc))^2 ,  C = cos(sqrt z) ,  S = sin(sqrt z)/sqrt z     (entire in z)
 //     fc(c)    = (cos(pi c / rc) + 1)/2 = C^2
 //     fc'(c)/c = -2 (pi/(2 rc))^2 C S
-// Coefficients: coeffs.inc, written by gen_coeffs.py (Chebyshev-node fits, errors < 6e-17).
+// Coefficients: coeffs.inc, written by gen_coeffs.py (Chebyshev-node fits; exp 1.2e-17, cos 2.0e-15 and
+// sinc 1.4e-16 absolute -- degree 7 for the cutoff pair: four orders below the 1e-11 tolerance on G).
 #pragma once
 
 namespace nnp {
@@ -42,9 +43,9 @@ __device__ __forceinline__ double exp_tiny(double y) {
 
 // C = cos(sqrt z), S = sin(sqrt z)/sqrt z for z in [0, (pi/2)^2]
 __device__ __forceinline__ void cos_sinc(double z, double& C, double& S) {
-    double c = COSC[8], s = SNCC[8];
+    double c = COSC[7], s = SNCC[7];
 #pragma unroll
-    for (int q = 7; q >= 0; --q) {
+    for (int q = 6; q >= 0; --q) {
         c = fma(c, z, COSC[q]);
         s = fma(s, z, SNCC[q]);
     }
@@ -53,9 +54,9 @@ __device__ __forceinline__ void cos_sinc(double z, double& C, double& S) {
 }
 
 __device__ __forceinline__ double cos_only(double z) {
-    double c = COSC[8];
+    double c = COSC[7];
 #pragma unroll
-    for (int q = 7; q >= 0; --q) c = fma(c, z, COSC[q]);
+    for (int q = 6; q >= 0; --q) c = fma(c, z, COSC[q]);
     return c;
 }
 
