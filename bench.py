@@ -42,8 +42,8 @@ FP64_INSTR_PER_ATOM = {
     "metal": {"sf": 10.8e3, "mlp": 3.3e3, "force": 16.6e3},
 }
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_force2 launch, from the ncu captures under profiles/
-# (r1e_launches_config3.csv for configs[3], r1b_ncu_k_sf2_k_force2.md for configs[2]); null where not captured
-NCU_DRAM_BYTES_K_FORCE2 = {3: 3617511680 + 103882496, 2: 338736896 + 9724160}
+# (r1f_launches_config3.csv for configs[3], r1b_ncu_k_sf2_k_force2.md for configs[2]); null where not captured
+NCU_DRAM_BYTES_K_FORCE2 = {3: 3617708288 + 103256064, 2: 338736896 + 9724160}
 # FP64 pipe peak derived from unit counts and clocks: 148 SMs x 64 DFMA lanes/clk x clocks.max.sm
 FP64_LANES_PER_SM = 64
 N_SM = 148
