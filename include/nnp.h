@@ -133,7 +133,9 @@ nnp_status nnp_set_activation(nnp_model* m, int32_t kind);
  * NOT wrapped (nnp_compute wraps internally).  The neighbour list is rebuilt every step.
  *   h_mass   [n_elem] HOST, masses in amu, by element index
  *   d_vel    [n_atoms][3] device, in/out, A/fs
- * Everything is enqueued on cuda_stream; no synchronisation inside.
+ * Everything is enqueued on cuda_stream; no synchronisation inside (except once at the start if the graph of a
+ * previous run is still alive).  With n_steps >= 4, a non-NULL stream and per-stage timing off, steps 2..n are
+ * replayed from a CUDA graph of one step captured on that stream (small systems are launch-latency bound).
  * nnp_md_kinetic_energy: *d_ekin (device, [1]) = sum_i m_i |v_i|^2 / (2 NNP_ACC_UNIT) in eV, deterministic
  * summation order; d_workspace as for nnp_compute (only its energy-partials scratch is touched, the exports of
  * the last nnp_compute stay valid). */

@@ -24,7 +24,9 @@ struct nnp_model {
     NetDesc nets[MAX_ELEM];
     double* d_weights[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
     double* d_scaling[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
-    MlpRegWeights* reg_w[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};   // host, see NetDesc::reg   // [2][n_sf]: shift, scale (or null)
+    MlpRegWeights* reg_w[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};   // host, see NetDesc::reg
+    cudaGraphExec_t md_exec = nullptr;     // graph of one MD step of the last nnp_md_run (kept until the next run)
+    cudaStream_t md_exec_stream = nullptr;   // [2][n_sf]: shift, scale (or null)
     // last nnp_compute (for the exports)
     Workspace ws;
     bool have_ws = false;
@@ -387,6 +389,7 @@ extern "C" void nnp_destroy(nnp_model* m) {
     if (m->hd_e) cudaFree(m->hd_e);
     if (m->hd_f) cudaFree(m->hd_f);
     if (m->hd_etot) cudaFree(m->hd_etot);
+    if (m->md_exec) { cudaStreamSynchronize(m->md_exec_stream); cudaGraphExecDestroy(m->md_exec); }
     if (m->hstream) cudaStreamDestroy(m->hstream);
     delete m;
 }
@@ -520,7 +523,7 @@ extern "C" nnp_status nnp_md_run(nnp_model* m, int32_t n_steps, double dt_fs, co
     if (n_atoms > 0 && (!d_pos || !d_vel || !d_type || !d_force)) return fail(m, NNP_ERR_INVALID_ARG, "null array");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     int launches = 0;
-    for (int s = 0; s < n_steps; ++s) {
+    auto one_step = [&]() -> nnp_status {
         {
             DeviceGuard dg(m->device);
             if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
@@ -532,6 +535,51 @@ extern "C" nnp_status nnp_md_run(nnp_model* m, int32_t n_steps, double dt_fs, co
         launches += m->last_launches;
         DeviceGuard dg(m->device);
         launches += launch_vv(n_atoms, m->n_elem, h_mass, d_type, d_force, d_vel, d_pos, dt_fs, false, st);
+        return NNP_OK;
+    };
+    if (m->md_exec) {       // the graph of the previous run may still be executing
+        DeviceGuard dg(m->device);
+        cudaStreamSynchronize(m->md_exec_stream);
+        cudaGraphExecDestroy(m->md_exec);
+        m->md_exec = nullptr;
+    }
+    int done = 0;
+    // A step is 16 launches with fixed arguments: for small systems it is launch-bound (configs[0]: 0.24 ms per
+    // step, of which the kernels need a third), so steps 2..n are replayed from a CUDA graph captured on the
+    // caller's stream.  Needs a real (capturable) stream and no per-stage timing; step 1 runs plainly so that
+    // every kernel attribute is configured outside the capture.
+    if (n_steps >= 4 && st != nullptr && !m->timing && n_atoms > 0) {
+        nnp_status rc = one_step();
+        if (rc != NNP_OK) return rc;
+        done = 1;
+        DeviceGuard dg(m->device);
+        if (cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            const int before = launches;
+            rc = one_step();
+            cudaGraph_t graph = nullptr;
+            const cudaError_t ce = cudaStreamEndCapture(st, &graph);
+            const int per_step = launches - before;
+            launches = before;
+            if (rc == NNP_OK && ce == cudaSuccess && graph &&
+                cudaGraphInstantiate(&m->md_exec, graph, 0) == cudaSuccess) {
+                m->md_exec_stream = st;
+                for (; done < n_steps; ++done) {
+                    if (cudaGraphLaunch(m->md_exec, st) != cudaSuccess) break;
+                    launches += per_step;
+                }
+            } else {
+                cudaGetLastError();     // capture refused: fall back to plain launches below
+                m->md_exec = nullptr;
+            }
+            if (graph) cudaGraphDestroy(graph);
+            if (rc != NNP_OK) return rc;
+        } else {
+            cudaGetLastError();
+        }
+    }
+    for (; done < n_steps; ++done) {
+        const nnp_status rc = one_step();
+        if (rc != NNP_OK) return rc;
     }
     m->last_launches = launches;
     NNP_CUDA(m, cudaGetLastError());
