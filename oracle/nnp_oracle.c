@@ -38,6 +38,7 @@
 
 /* One symmetry function (own declaration; memory layout documented for ctypes).
  * kind 2: radial  G = sum_j exp(-eta (r_ij - rs)^2) fc(r_ij),   t_j = e1
+ * kind 9: angular WIDE, as kind 3 without the r_jk terms (see sf_centre)
  * kind 3: angular G = 2^(1-zeta) sum_{j<k} (1 + lambda cos th)^zeta
  *                       exp(-eta (a^2+b^2+c^2)) fc(a) fc(b) fc(c),  {t_j,t_k} = {e1,e2}, c < rc
  * (n2p2 numbering, readings C2-C5). */
@@ -175,7 +176,10 @@ static void sf_centre(const oracle_model* M, int tc, int nn, const double* u, co
                     }
                 }
             }
-        } else { /* kind 3 */
+        } else { /* kind 3 (angular narrow) or kind 9 (angular WIDE, n2p2 numbering):
+                  *   G = 2^(1-zeta) sum_{j<k} (1 + lambda cos)^zeta exp(-eta (a^2 + b^2)) fc(a) fc(b)
+                  * -- no r_jk term and no r_jk cutoff: every pair of neighbours of the two elements counts */
+            const int wide = (f->kind == 9);
             double pref = pow(2.0, 1.0 - f->zeta);
             for (int j = 0; j < nn; ++j)
                 for (int k = j + 1; k < nn; ++k) {
@@ -188,24 +192,25 @@ static void sf_centre(const oracle_model* M, int tc, int nn, const double* u, co
                     double b2 = vv[0] * vv[0] + vv[1] * vv[1] + vv[2] * vv[2];
                     double c2 = ww[0] * ww[0] + ww[1] * ww[1] + ww[2] * ww[2];
                     double a = sqrt(a2), b = sqrt(b2), c = sqrt(c2);
-                    if (!(c < rc)) continue;                      /* narrow: needs r_jk < rc */
+                    if (!wide && !(c < rc)) continue;             /* narrow: needs r_jk < rc */
                     double ct = (uu[0] * vv[0] + uu[1] * vv[1] + uu[2] * vv[2]) / (a * b);
                     double base = 1.0 + f->lambda * ct;
                     double P = pref * pow(base, f->zeta);
-                    double X = exp(-f->eta * (a2 + b2 + c2));
-                    double fa = oracle_fc(a, rc), fb = oracle_fc(b, rc), fcc = oracle_fc(c, rc);
+                    double X = exp(-f->eta * (wide ? a2 + b2 : a2 + b2 + c2));
+                    double fa = oracle_fc(a, rc), fb = oracle_fc(b, rc), fcc = wide ? 1.0 : oracle_fc(c, rc);
                     double C = fa * fb * fcc;
                     acc += P * X * C;
                     if (beta) {
                         double dP = pref * f->zeta * f->lambda * pow(base, f->zeta - 1.0); /* dP/dcos */
-                        double dfa = oracle_dfc(a, rc), dfb = oracle_dfc(b, rc), dfc = oracle_dfc(c, rc);
+                        double dfa = oracle_dfc(a, rc), dfb = oracle_dfc(b, rc), dfc = wide ? 0.0 : oracle_dfc(c, rc);
+                        const double wq = wide ? 0.0 : 1.0;       /* weight of the c^2 term in the exponent */
                         for (int x = 0; x < 3; ++x) {
                             /* cos = u.v/(ab) */
                             double dct_du = vv[x] / (a * b) - ct * uu[x] / a2;
                             double dct_dv = uu[x] / (a * b) - ct * vv[x] / b2;
                             /* X = exp(-eta(a2+b2+c2)), c2 = |v-u|^2 */
-                            double dX_du = X * (-f->eta) * (2.0 * uu[x] - 2.0 * ww[x]);
-                            double dX_dv = X * (-f->eta) * (2.0 * vv[x] + 2.0 * ww[x]);
+                            double dX_du = X * (-f->eta) * (2.0 * uu[x] - wq * 2.0 * ww[x]);
+                            double dX_dv = X * (-f->eta) * (2.0 * vv[x] + wq * 2.0 * ww[x]);
                             /* C = fc(a) fc(b) fc(c) */
                             double dC_du = dfa * (uu[x] / a) * fb * fcc + fa * fb * dfc * (-ww[x] / c);
                             double dC_dv = fa * dfb * (vv[x] / b) * fcc + fa * fb * dfc * (ww[x] / c);
