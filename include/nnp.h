@@ -53,8 +53,11 @@ typedef enum {
  *   kind 3 (angular, narrow): with a=r_ij, b=r_ik, c=r_jk, cos = u.v/(ab),
  *       G = 2^(1-zeta) sum_{j<k in N(i), {t_j,t_k} = {e1,e2}, c < rc}
  *               (1 + lambda cos)^zeta  exp(-eta (a^2+b^2+c^2))  fc(a) fc(b) fc(c)
+ *   kind 9 (angular, wide): the same without the r_jk terms,
+ *       G = 2^(1-zeta) sum_{j<k in N(i), {t_j,t_k} = {e1,e2}} (1 + lambda cos)^zeta  exp(-eta (a^2+b^2))  fc(a) fc(b)
+ *       (a table that contains kind 9 runs on the generic kernels)
  *   fc(r) = (cos(pi r / rc) + 1)/2 for r < rc, else 0;  N(i) = { j != i : r_ij^2 < rc^2 }.
- * Constraints (else NNP_ERR_INVALID_ARG): eta >= 0; kind 3 needs lambda = +1 or -1 and
+ * Constraints (else NNP_ERR_INVALID_ARG): eta >= 0; kinds 3 and 9 need lambda = +1 or -1 and
  * zeta an integer in [1, 64]; rs is used by kind 2 only.  The order of the entries with
  * equal `central` is the order of that element's descriptor vector G (= network input). */
 typedef struct {

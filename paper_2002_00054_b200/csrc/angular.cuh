@@ -251,4 +251,11 @@ __device__ __forceinline__ void pairs_between(const Nbh& nb, int s1, int n1, int
 // screening threshold (see above)
 __device__ __forceinline__ float screen_rc2(double rc2) { return (float)(rc2 * (1.0 + 1e-5)); }
 
+// whether a pair group's list holds a wide angular SF (kind 9): its triplets are not limited by r_jk
+__device__ __forceinline__ bool group_has_wide(const AngularSF* list, int n) {
+    bool w = false;
+    for (int s = 0; s < n; ++s) w |= list[s].wide != 0;
+    return w;
+}
+
 }  // namespace nnp

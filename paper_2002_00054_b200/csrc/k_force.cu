@@ -64,8 +64,8 @@ struct SlotAcc {
 // bare Gaussians) to the slot updates.  fcc = fc(c), dfc = fc'(c)/c.
 __device__ __forceinline__ void triplet_forces(const double2 j0, const double2 j1, const double2 j2, const double2 k0,
                                                const double2 k1, const double2 k2, double fcc, double dfc, double cosv,
-                                               double iab, double Z0, double Z1, double Z2, const SlotAcc& acc, int j,
-                                               int k, int col, bool active) {
+                                               double iab, double Z0, double Z1, double Z2, double W0, double W1,
+                                               double W2, const SlotAcc& acc, int j, int k, int col, bool active) {
     const double fa = j2.x, dfa = j2.y, fb = k2.x, dfb = k2.y, ia = j1.y, ib = k1.y;
     const double fab = fa * fb;
     const double C = fab * fcc;
@@ -75,7 +75,13 @@ __device__ __forceinline__ void triplet_forces(const double2 j0, const double2 j
     const double qc = q * cosv;
     const double f_uu = fma(-qc, ia * ia, fma((dfa * fb) * fcc, Z0, -t2));
     const double f_vv = fma(-qc, ib * ib, fma((fa * dfb) * fcc, Z0, -t2));
-    const double s1 = f_uu + f_w, s2 = f_vv + f_w, s3 = fma(-q, iab, f_w);
+    // wide SFs (kind 9): the same sums W0, W1, W2 over their own list, without any r_jk dependence
+    const double tw = (fab + fab) * W2;
+    const double qw = W1 * fab;
+    const double qwc = qw * cosv;
+    const double g_uu = fma(-qwc, ia * ia, fma(dfa * fb, W0, -tw));
+    const double g_vv = fma(-qwc, ib * ib, fma(fa * dfb, W0, -tw));
+    const double s1 = f_uu + f_w + g_uu, s2 = f_vv + f_w + g_vv, s3 = fma(-(q + qw), iab, f_w);
     // colour passes: entries of one colour have pairwise distinct j and pairwise distinct k
     unsigned pend = __ballot_sync(0xffffffffu, active);
     while (pend) {
@@ -126,8 +132,9 @@ struct ForceTripletGeneric {
         const double iab = j1.y * k1.y;
         const double cosv = fma(j0.x, k0.x, fma(j0.y, k0.y, j1.x * k1.x)) * iab;
         const double a2 = 1.0 / (j1.y * j1.y), b2 = 1.0 / (k1.y * k1.y);
-        const double r2sum = a2 + b2 + c2;
-        double Z0 = 0.0, Z1 = 0.0, Z2 = 0.0;
+        const double r2ab = a2 + b2;
+        const double r2sum = r2ab + c2;
+        double Z0 = 0.0, Z1 = 0.0, Z2 = 0.0, W0 = 0.0, W1 = 0.0, W2 = 0.0;
         for (int s = 0; s < nsf; ++s) {
             const AngularSF f = list[s];
             const double base = 1.0 + (double)f.lam * cosv;
@@ -138,13 +145,20 @@ struct ForceTripletGeneric {
                 bb *= bb;
             }
             const double pwv = pd * base;
-            const double Y = exp(-f.eta * r2sum);
+            const double Y = exp(-f.eta * (f.wide ? r2ab : r2sum));
             const double bc = brow[f.g] * f.coef;
-            Z0 = fma(bc * pwv, Y, Z0);
-            Z1 = fma(bc * (double)(f.izeta * f.lam) * pd, Y, Z1);
-            Z2 = fma(f.eta * bc * pwv, Y, Z2);
+            const double t0 = bc * pwv * Y, t1 = bc * (double)(f.izeta * f.lam) * pd * Y;
+            if (f.wide) {
+                W0 += t0;
+                W1 += t1;
+                W2 = fma(f.eta, t0, W2);
+            } else {
+                Z0 += t0;
+                Z1 += t1;
+                Z2 = fma(f.eta, t0, Z2);
+            }
         }
-        triplet_forces(j0, j1, j2, k0, k1, kk2, fcc, dfc, cosv, iab, Z0, Z1, Z2, acc, j, k, col, active);
+        triplet_forces(j0, j1, j2, k0, k1, kk2, fcc, dfc, cosv, iab, Z0, Z1, Z2, W0, W1, W2, acc, j, k, col, active);
     }
 };
 
@@ -240,8 +254,9 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
                 const int na = prog->n_ang[pr];
                 if (na == 0) continue;
                 ForceTripletGeneric f{nb, acc, prog->ang + prog->ang_off[pr], na, brow, p.k2, p.rc2};
-                if (e1 == e2) pairs_within(nb, seg[e1], seg[e1 + 1] - seg[e1], rc2f, Q, lane, f);
-                else pairs_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], rc2f, Q, lane, f);
+                const float rs = group_has_wide(prog->ang + prog->ang_off[pr], na) ? 3.0e38f : rc2f;   // wide SFs: no r_jk screen
+                if (e1 == e2) pairs_within(nb, seg[e1], seg[e1 + 1] - seg[e1], rs, Q, lane, f);
+                else pairs_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], rs, Q, lane, f);
             }
     }
     __syncwarp();

@@ -49,11 +49,14 @@ struct SfTripletGeneric {
         const double wx = k0.x - j0.x, wy = k0.y - j0.y, wz = k1.x - j1.x;
         const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
         const double Cc = cos_only(c2 * k2);
-        double C = j2.y * kq.y * (Cc * Cc);
+        double Cw = j2.y * kq.y;                    // wide SFs (kind 9): fc(a) fc(b), no r_jk cutoff
+        double C = Cw * (Cc * Cc);                  // narrow SFs: times fc(c), needs c < rc
+        if (!active) Cw = 0.0;
         if (!active || !(c2 < rc2)) C = 0.0;
         const double cosv = (j0.x * k0.x + j0.y * k0.y + j1.x * k1.x) * (j1.y * k1.y);
         const double aj = ra[j], ak = ra[k];
-        const double r2sum = aj * aj + ak * ak + c2;
+        const double r2ab = aj * aj + ak * ak;
+        const double r2sum = r2ab + c2;
         for (int s = 0; s < nsf; ++s) {
             const AngularSF f = sf[s];
             const double base = 1.0 + (double)f.lam * cosv;
@@ -62,7 +65,7 @@ struct SfTripletGeneric {
                 if (z & 1) pw *= bb;
                 bb *= bb;
             }
-            double v = f.coef * pw * exp(-f.eta * r2sum) * C;
+            double v = f.wide ? f.coef * pw * exp(-f.eta * r2ab) * Cw : f.coef * pw * exp(-f.eta * r2sum) * C;
             v = warp_sum(v);
             if (lane == 0) gacc[s] += v;
         }
@@ -158,8 +161,9 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
                 for (int s = lane; s < na; s += 32) gacc[s] = 0.0;
                 __syncwarp();
                 SfTripletGeneric f{nb, prog->ang + prog->ang_off[pr], na, p.k2, p.rc2, ra, gacc, lane};
-                if (e1 == e2) pairs_within(nb, seg[e1], seg[e1 + 1] - seg[e1], rc2f, Q, lane, f);
-                else pairs_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], rc2f, Q, lane, f);
+                const float rs = group_has_wide(prog->ang + prog->ang_off[pr], na) ? 3.0e38f : rc2f;   // wide SFs: no r_jk screen
+                if (e1 == e2) pairs_within(nb, seg[e1], seg[e1 + 1] - seg[e1], rs, Q, lane, f);
+                else pairs_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], rs, Q, lane, f);
                 __syncwarp();
                 for (int s = lane; s < na; s += 32) Grow[prog->ang[prog->ang_off[pr] + s].g] = gacc[s];
                 __syncwarp();

@@ -208,7 +208,7 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
             if (f.e1 < 0 || f.e1 >= n_elem) return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.e1 out of range");
             if (!std::isfinite(f.rs)) return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.rs not finite");
             rad[f.central][f.e1].push_back(RadialSF{f.eta, f.rs, g, 0});
-        } else if (f.kind == 3) {
+        } else if (f.kind == 3 || f.kind == 9) {
             if (f.e1 < 0 || f.e1 >= n_elem || f.e2 < 0 || f.e2 >= n_elem)
                 return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.e1/e2 out of range");
             if (!(f.lambda == 1.0 || f.lambda == -1.0))
@@ -218,9 +218,9 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
                 return fail(nullptr, NNP_ERR_INVALID_ARG, "angular zeta must be an integer in [1, 64]");
             const int a = f.e1 < f.e2 ? f.e1 : f.e2, b = f.e1 < f.e2 ? f.e2 : f.e1;
             ang[f.central][pair_index(a, b, n_elem)].push_back(
-                AngularSF{f.eta, std::exp2(1.0 - f.zeta), g, iz, f.lambda > 0 ? 1 : -1, 0});
+                AngularSF{f.eta, std::exp2(1.0 - f.zeta), g, iz, f.lambda > 0 ? 1 : -1, f.kind == 9 ? 1 : 0});
         } else {
-            return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.kind must be 2 (radial) or 3 (angular narrow)");
+            return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.kind must be 2 (radial), 3 (angular narrow) or 9 (angular wide)");
         }
     }
 
@@ -262,9 +262,10 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
         if (any_ang) {
             // the specialised kernels use exp_small() unclamped: its argument -eta (a^2+b^2+c^2) must stay > -700
             double eta_max = 0.0;
+            bool any_wide = false;           // wide angular SFs run on the generic kernels only
             for (int p = 0; p < npair; ++p)
-                for (const auto& f : ang[c][p]) eta_max = std::fmax(eta_max, f.eta);
-            const bool in_range = eta_max * 3.0 * rc * rc <= 700.0;
+                for (const auto& f : ang[c][p]) { eta_max = std::fmax(eta_max, f.eta); any_wide |= f.wide != 0; }
+            const bool in_range = !any_wide && eta_max * 3.0 * rc * rc <= 700.0;
             if (in_range && match_spec<SpecBase12>(ang[c], &P)) P.variant = ANG_BASE12;
             else if (in_range && match_spec<SpecWide32>(ang[c], &P)) P.variant = ANG_WIDE32;
             else {

@@ -39,7 +39,7 @@ struct AngularSF {
     int32_t g;
     int32_t izeta;   // integer zeta
     int32_t lam;     // +1 / -1
-    int32_t pad;
+    int32_t wide;    // 1: wide angular SF (n2p2 kind 9: no r_jk term, no r_jk cutoff); generic kernels only
 };
 
 // Angular kernel variants.  Specialised variants bake the (eta ratio, lambda, zeta) structure

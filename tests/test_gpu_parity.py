@@ -170,6 +170,27 @@ def test_metal_like_small_neighbourhoods():
     _check_full(model, sysm)                       # and the default 160-slot kernels on the same system
 
 
+def test_wide_angular_mixed_with_narrow():
+    # wide angular SFs (n2p2 kind 9: no r_jk term, no r_jk cutoff) next to narrow ones in the
+    # same pair group; a table that holds one runs on the generic kernels with the FP32 r_jk screen disabled
+    rows = []
+    for c in range(2):
+        for e1 in range(2):
+            rows.append((c, 2, e1, 0, 0.05, 0.0, 0.0, 0.0))
+        for (e1, e2) in ((0, 0), (0, 1), (1, 1)):
+            rows.append((c, 9, e1, e2, 0.004, 0.0, 1.0, 2.0))
+            rows.append((c, 9, e1, e2, 0.010, 0.0, -1.0, 1.0))
+            rows.append((c, 3, e1, e2, 0.004, 0.0, 1.0, 4.0))
+            rows.append((c, 9, e1, e2, 0.0, 0.0, 1.0, 16.0))
+    model = tiny_model(rows, n_elem=2, hidden=(5, 4), seed=21)
+    _check_full(model, W.make_water(150, 5, L=16.7))
+    # wide only, one element
+    rows = [(0, 2, 0, 0, 0.05, 0.0, 0.0, 0.0), (0, 9, 0, 0, 0.02, 0.0, -1.0, 3.0), (0, 9, 0, 0, 0.001, 0.0, 1.0, 1.0)]
+    sysm = W.make_water(60, 3, L=12.4)
+    sysm.types[:] = 0
+    _check_full(tiny_model(rows, hidden=(4,), seed=3), sysm)
+
+
 def test_single_element_radial_only():
     model = tiny_model([(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0), (0, 2, 0, 0, 0.4, 2.0, 0.0, 0.0)], hidden=(4,))
     sysm = W.make_water(60, 3, L=12.4)
