@@ -98,8 +98,11 @@ struct JData {
     double ux, uy, uz, ia, fa, dfa, e0;
 };
 
+#ifndef F2_MINB1
+#define F2_MINB1 20          // resident CTAs per SM asked of the one-warp-per-centre instantiation (metals: 5.2 vs 5.65 ms at 14)
+#endif
 template <class Spec, int WPC, int CAPA, bool TINY>
-__global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2(const __grid_constant__ Force2Params p) {
+__global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_force2(const __grid_constant__ Force2Params p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NT = WPC * 32;
     constexpr bool REGC = Spec::NACC <= 12;          // coefficients of the current group in registers

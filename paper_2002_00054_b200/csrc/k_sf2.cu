@@ -40,8 +40,11 @@ __host__ __device__ constexpr size_t sf2_smem(int capa, int n_elem, int wpc) {
     return (b + 15) / 16 * 16;
 }
 
+#ifndef S2_MINB1
+#define S2_MINB1 24          // resident CTAs per SM asked of the one-warp-per-centre instantiation (12 SFs per group)
+#endif
 template <class Spec, int WPC, int CAPA, bool TINY>
-__global__ void __launch_bounds__(WPC * 32, (Spec::NACC <= 12 ? 24 : 16) / WPC) k_sf2(const __grid_constant__ Sf2Params p) {
+__global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MINB1 : 16) : (Spec::NACC <= 12 ? 24 : 16) / WPC) k_sf2(const __grid_constant__ Sf2Params p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NT = WPC * 32;
     constexpr int NACC = Spec::NACC;
