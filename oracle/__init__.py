@@ -24,7 +24,7 @@ class _Model(C.Structure):
     _fields_ = [("n_elem", C.c_int32), ("rc", C.c_double), ("n_sf", C.c_int32),
                 ("sf", C.c_void_p), ("n_layers", C.c_void_p), ("layer_sizes", C.c_void_p),
                 ("weights", C.c_void_p), ("sf_shift", C.c_void_p), ("sf_scale", C.c_void_p),
-                ("activation", C.c_int32)]
+                ("activation", C.c_int32), ("sf_rc", C.c_void_p)]
 
 
 def lib():
@@ -72,9 +72,13 @@ class OracleModel:
         self.sf_shift = None if sc is None else np.ascontiguousarray(np.concatenate([np.asarray(a, dtype=np.float64) for a, _ in sc]))
         self.sf_scale = None if sc is None else np.ascontiguousarray(np.concatenate([np.asarray(b, dtype=np.float64) for _, b in sc]))
         self.activation = {"softplus": 0, "tanh": 1}[getattr(model, "activation", "softplus")]
+        # per-SF cutoff radii, in the order of model.sf (None: the global rc for all)
+        rcs = getattr(model, "sf_cutoffs", None)
+        self.sf_rc = None if rcs is None else np.ascontiguousarray(rcs, dtype=np.float64)
+        assert self.sf_rc is None or (self.sf_rc.shape == (sf.shape[0],) and np.all(self.sf_rc > 0) and np.all(self.sf_rc <= self.rc))
         self.c = _Model(self.n_elem, self.rc, sf.shape[0], _ptr(sf), _ptr(self.n_layers),
                         _ptr(self.layer_sizes), _ptr(self.weights), _ptr(self.sf_shift), _ptr(self.sf_scale),
-                        self.activation)
+                        self.activation, _ptr(self.sf_rc))
 
 
 def fc(r, rc):

@@ -61,6 +61,10 @@ typedef struct {
     const double* sf_shift;
     const double* sf_scale;
     int32_t activation;
+    /* per-SF cutoff radii (n2p2 gives every symmetry function its own rc): [n_sf] in the
+     * order of `sf`, each 0 < sf_rc[q] <= rc; NULL = the one global rc.  The neighbourhood N(i) is still
+     * the one of the global rc; an SF with a smaller rc simply has fc(r; sf_rc) = 0 beyond it. */
+    const double* sf_rc;
 } oracle_model;
 
 static double now_s(void) {
@@ -150,12 +154,12 @@ double oracle_dfc(double r, double rc) {
  * neighbours, F = - sum_s beta[s] * dG_s/dr   (reading 6). */
 static void sf_centre(const oracle_model* M, int tc, int nn, const double* u, const int32_t* tn,
                       double* G, const double* beta, double* fi, double* fn) {
-    const double rc = M->rc;
     int s = -1;
     for (int q = 0; q < M->n_sf; ++q) {
         const oracle_sf* f = &M->sf[q];
         if (f->central != tc) continue;
         ++s;
+        const double rc = M->sf_rc ? M->sf_rc[q] : M->rc;     /* this SF's cutoff radius */
         double acc = 0.0;
         if (f->kind == 2) {
             for (int j = 0; j < nn; ++j) {

@@ -48,6 +48,8 @@ class Model:
     # x = scale * (G - shift), or None; hidden activation "softplus" (BASELINE.json) or "tanh"
     sf_scaling: list | None = None
     activation: str = "softplus"
+    # per-SF cutoff radii in the order of `sf` (each <= rc), or None: one global rc
+    sf_cutoffs: list | None = None
 
 
 def radial_etas(n: int) -> np.ndarray:
