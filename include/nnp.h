@@ -120,11 +120,18 @@ nnp_status nnp_compute_host(nnp_model* m, int64_t n_atoms, const double* h_pos, 
  * nnp_set_sf_scaling: the network of element `elem` reads x_s = h_scale[s] * (G_s - h_shift[s]) instead of G_s
  *   (HOST arrays of the element's symmetry-function count, in G order; both NULL = back to identity).
  *   nnp_get_sf still returns the unscaled G, nnp_get_dedg returns dE/dG (= scale * dE/dx).  Synchronises the device.
- * nnp_set_activation: hidden-layer activation of every element; the output layer stays linear. */
+ * nnp_set_activation: hidden-layer activation of every element; the output layer stays linear.
+ * nnp_set_sf_cutoffs: per-SF cutoff radii (n2p2 gives every symmetry function its own rc): h_rc is a HOST array
+ *   of n_sf radii in the order of the `sf` table of nnp_create, each 0 < h_rc[s] <= rc (else NNP_ERR_INVALID_ARG);
+ *   SF s then uses fc(r; h_rc[s]) = (cos(pi r / h_rc[s]) + 1)/2 for r < h_rc[s], else 0 -- for r_ij, r_ik and, in
+ *   kind 3, for r_jk (which must be < h_rc[s]) -- on the neighbourhood of the global rc.  NULL = back to the one
+ *   global rc.  An element that has an SF with a radius other than rc runs on the generic kernels.
+ *   Synchronises the device. */
 #define NNP_ACT_SOFTPLUS 0
 #define NNP_ACT_TANH 1
 nnp_status nnp_set_sf_scaling(nnp_model* m, int32_t elem, const double* h_shift, const double* h_scale);
 nnp_status nnp_set_activation(nnp_model* m, int32_t kind);
+nnp_status nnp_set_sf_cutoffs(nnp_model* m, int32_t n_sf, const double* h_rc);
 
 /* ---- MD loop around the path (the implementation is checked by energy
  * conservation in an NVE run).  Velocity Verlet, everything on the device:

@@ -60,28 +60,9 @@ struct SlotAcc {
     double2* yz;   // (Vy, Vz)
 };
 
-// From Z0 = sum beta P Y, Z1 = sum beta P' Y, Z2 = sum eta beta P Y  (Y = product of the three
-// bare Gaussians) to the slot updates.  fcc = fc(c), dfc = fc'(c)/c.
-__device__ __forceinline__ void triplet_forces(const double2 j0, const double2 j1, const double2 j2, const double2 k0,
-                                               const double2 k1, const double2 k2, double fcc, double dfc, double cosv,
-                                               double iab, double Z0, double Z1, double Z2, double W0, double W1,
-                                               double W2, const SlotAcc& acc, int j, int k, int col, bool active) {
-    const double fa = j2.x, dfa = j2.y, fb = k2.x, dfb = k2.y, ia = j1.y, ib = k1.y;
-    const double fab = fa * fb;
-    const double C = fab * fcc;
-    const double t2 = (C + C) * Z2;
-    const double f_w = fma(fab * dfc, Z0, -t2);
-    const double q = Z1 * C;
-    const double qc = q * cosv;
-    const double f_uu = fma(-qc, ia * ia, fma((dfa * fb) * fcc, Z0, -t2));
-    const double f_vv = fma(-qc, ib * ib, fma((fa * dfb) * fcc, Z0, -t2));
-    // wide SFs (kind 9): the same sums W0, W1, W2 over their own list, without any r_jk dependence
-    const double tw = (fab + fab) * W2;
-    const double qw = W1 * fab;
-    const double qwc = qw * cosv;
-    const double g_uu = fma(-qwc, ia * ia, fma(dfa * fb, W0, -tw));
-    const double g_vv = fma(-qwc, ib * ib, fma(fa * dfb, W0, -tw));
-    const double s1 = f_uu + f_w + g_uu, s2 = f_vv + f_w + g_vv, s3 = fma(-(q + qw), iab, f_w);
+// One triplet's  F_j = -s1 u + s3 v  and  F_k = -s2 v + s3 u  into the shared slot accumulators (A, V).
+__device__ __forceinline__ void slot_updates(const double2 j0, const double2 j1, const double2 k0, const double2 k1, double s1,
+                                             double s2, double s3, const SlotAcc& acc, int j, int k, int col, bool active) {
     // colour passes: entries of one colour have pairwise distinct j and pairwise distinct k
     unsigned pend = __ballot_sync(0xffffffffu, active);
     while (pend) {
@@ -111,6 +92,31 @@ __device__ __forceinline__ void triplet_forces(const double2 j0, const double2 j
     }
 }
 
+// From Z0 = sum beta P Y, Z1 = sum beta P' Y, Z2 = sum eta beta P Y  (Y = product of the three
+// bare Gaussians) to the slot updates.  fcc = fc(c), dfc = fc'(c)/c.
+__device__ __forceinline__ void triplet_forces(const double2 j0, const double2 j1, const double2 j2, const double2 k0,
+                                               const double2 k1, const double2 k2, double fcc, double dfc, double cosv,
+                                               double iab, double Z0, double Z1, double Z2, double W0, double W1,
+                                               double W2, const SlotAcc& acc, int j, int k, int col, bool active) {
+    const double fa = j2.x, dfa = j2.y, fb = k2.x, dfb = k2.y, ia = j1.y, ib = k1.y;
+    const double fab = fa * fb;
+    const double C = fab * fcc;
+    const double t2 = (C + C) * Z2;
+    const double f_w = fma(fab * dfc, Z0, -t2);
+    const double q = Z1 * C;
+    const double qc = q * cosv;
+    const double f_uu = fma(-qc, ia * ia, fma((dfa * fb) * fcc, Z0, -t2));
+    const double f_vv = fma(-qc, ib * ib, fma((fa * dfb) * fcc, Z0, -t2));
+    // wide SFs (kind 9): the same sums W0, W1, W2 over their own list, without any r_jk dependence
+    const double tw = (fab + fab) * W2;
+    const double qw = W1 * fab;
+    const double qwc = qw * cosv;
+    const double g_uu = fma(-qwc, ia * ia, fma(dfa * fb, W0, -tw));
+    const double g_vv = fma(-qwc, ib * ib, fma(fa * dfb, W0, -tw));
+    const double s1 = f_uu + f_w + g_uu, s2 = f_vv + f_w + g_vv, s3 = fma(-(q + qw), iab, f_w);
+    slot_updates(j0, j1, k0, k1, s1, s2, s3, acc, j, k, col, active);
+}
+
 struct ForceTripletGeneric {
     const Nbh& nb;
     SlotAcc acc;
@@ -118,6 +124,7 @@ struct ForceTripletGeneric {
     int nsf;
     const double* brow;   // beta row of the centre (shared memory)
     double k2, rc2;
+    bool own;             // the SFs carry their own cutoff radii (ElemProgram::per_sf_rc)
 
     __device__ __forceinline__ void operator()(int j, int k, int col, bool active) {
         const double2 j0 = nb.p0[j], j1 = nb.p1[j], j2 = nb.p2[j];
@@ -134,6 +141,37 @@ struct ForceTripletGeneric {
         const double a2 = 1.0 / (j1.y * j1.y), b2 = 1.0 / (k1.y * k1.y);
         const double r2ab = a2 + b2;
         const double r2sum = r2ab + c2;
+        if (own) {
+            // every SF has its own fc(.; rc_s): no common cutoff factor to pull out, the three slot scalars are summed SF by SF
+            const double a2j = fma(j0.x, j0.x, fma(j0.y, j0.y, j1.x * j1.x)), a2k = fma(k0.x, k0.x, fma(k0.y, k0.y, k1.x * k1.x));
+            const double ia2 = j1.y * j1.y, ib2 = k1.y * k1.y;
+            double s1 = 0.0, s2 = 0.0, s3 = 0.0;
+            for (int s = 0; s < nsf; ++s) {
+                const AngularSF f = list[s];
+                const double base = 1.0 + (double)f.lam * cosv;
+                double pd = 1.0, bb = base;
+                for (int z = f.izeta - 1; z > 0; z >>= 1) {
+                    if (z & 1) pd *= bb;
+                    bb *= bb;
+                }
+                double fa, dfa, fb, dfb, fcs = 1.0, dfcs = 0.0;
+                fc_dfc_own(a2j, f.rc2, f.k2, fa, dfa);
+                fc_dfc_own(a2k, f.rc2, f.k2, fb, dfb);
+                if (!f.wide) fc_dfc_own(c2, f.rc2, f.k2, fcs, dfcs);
+                const double Y = exp(-f.eta * (f.wide ? a2j + a2k : a2j + a2k + c2));
+                const double bc = brow[f.g] * f.coef;
+                const double t0 = bc * (pd * base) * Y, t1 = bc * (double)(f.izeta * f.lam) * pd * Y;
+                const double fab = fa * fb, C = fab * fcs;
+                const double t2 = (C + C) * (f.eta * t0);
+                const double fw = f.wide ? 0.0 : fma(fab * dfcs, t0, -t2);
+                const double q = t1 * C, qc = q * cosv;
+                s1 += fma(-qc, ia2, fma((dfa * fb) * fcs, t0, -t2)) + fw;
+                s2 += fma(-qc, ib2, fma((fa * dfb) * fcs, t0, -t2)) + fw;
+                s3 += fma(-q, iab, fw);
+            }
+            slot_updates(j0, j1, k0, k1, s1, s2, s3, acc, j, k, col, active);
+            return;
+        }
         double Z0 = 0.0, Z1 = 0.0, Z2 = 0.0, W0 = 0.0, W1 = 0.0, W2 = 0.0;
         for (int s = 0; s < nsf; ++s) {
             const AngularSF f = list[s];
@@ -234,7 +272,9 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
                 const RadialSF f = prog->rad[off + r];
                 const double d = a - f.rs;
                 const double ex = exp_small(fmax(-f.eta * d * d, -700.0));
-                R = fma(brow[f.g] * ex, fma(-2.0 * f.eta * d, fa * ia, dfa_a), R);
+                double fs = fa, dfs = dfa_a;
+                if (prog->per_sf_rc) fc_dfc_own(a2, f.rc2, f.k2, fs, dfs);
+                R = fma(brow[f.g] * ex, fma(-2.0 * f.eta * d, fs * ia, dfs), R);
             }
             acc.av[m] = make_double2(R, 0.0);
             acc.yz[m] = make_double2(0.0, 0.0);
@@ -253,7 +293,7 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
                 const int pr = pair_index(e1, e2, p.n_elem);
                 const int na = prog->n_ang[pr];
                 if (na == 0) continue;
-                ForceTripletGeneric f{nb, acc, prog->ang + prog->ang_off[pr], na, brow, p.k2, p.rc2};
+                ForceTripletGeneric f{nb, acc, prog->ang + prog->ang_off[pr], na, brow, p.k2, p.rc2, prog->per_sf_rc != 0};
                 const float rs = group_has_wide(prog->ang + prog->ang_off[pr], na) ? 3.0e38f : rc2f;   // wide SFs: no r_jk screen
                 if (e1 == e2) pairs_within(nb, seg[e1], seg[e1 + 1] - seg[e1], rs, Q, lane, f);
                 else pairs_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], rs, Q, lane, f);

@@ -42,6 +42,7 @@ struct SfTripletGeneric {
     const double* ra; // [slot] distance a
     double* gacc;     // [64] per warp, shared memory
     int lane;
+    bool own;         // the SFs carry their own cutoff radii (ElemProgram::per_sf_rc)
 
     __device__ __forceinline__ void operator()(int j, int k, int, bool active) {
         const double2 j0 = nb.p0[j], j1 = nb.p1[j], j2 = nb.p2[j];
@@ -57,8 +58,13 @@ struct SfTripletGeneric {
         const double aj = ra[j], ak = ra[k];
         const double r2ab = aj * aj + ak * ak;
         const double r2sum = r2ab + c2;
+        const double a2j = fma(j0.x, j0.x, fma(j0.y, j0.y, j1.x * j1.x)), a2k = fma(k0.x, k0.x, fma(k0.y, k0.y, k1.x * k1.x));
         for (int s = 0; s < nsf; ++s) {
             const AngularSF f = sf[s];
+            if (own) {          // fc(.; rc_s) of this SF for a, b (and c)
+                Cw = active ? fc_own(a2j, f.rc2, f.k2) * fc_own(a2k, f.rc2, f.k2) : 0.0;
+                C = f.wide ? 0.0 : Cw * fc_own(c2, f.rc2, f.k2);
+            }
             const double base = 1.0 + (double)f.lam * cosv;
             double pw = 1.0, bb = base;
             for (int z = f.izeta; z > 0; z >>= 1) {
@@ -143,7 +149,13 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
             double acc = 0.0;
             for (int m = seg[e] + lane; m < seg[e + 1]; m += 32) {
                 const double d = ra[m] - f.rs;
-                acc = fma(exp_small(fmax(-f.eta * d * d, -700.0)), nb.p2[m].y, acc);
+                double fcv = nb.p2[m].y;
+                if (prog->per_sf_rc) {
+                    const double2 u0 = nb.p0[m];
+                    const double uz = nb.p1[m].x;
+                    fcv = fc_own(fma(u0.x, u0.x, fma(u0.y, u0.y, uz * uz)), f.rc2, f.k2);
+                }
+                acc = fma(exp_small(fmax(-f.eta * d * d, -700.0)), fcv, acc);
             }
             acc = warp_sum(acc);
             if (lane == 0) Grow[f.g] = acc;
@@ -160,7 +172,7 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
             {
                 for (int s = lane; s < na; s += 32) gacc[s] = 0.0;
                 __syncwarp();
-                SfTripletGeneric f{nb, prog->ang + prog->ang_off[pr], na, p.k2, p.rc2, ra, gacc, lane};
+                SfTripletGeneric f{nb, prog->ang + prog->ang_off[pr], na, p.k2, p.rc2, ra, gacc, lane, prog->per_sf_rc != 0};
                 const float rs = group_has_wide(prog->ang + prog->ang_off[pr], na) ? 3.0e38f : rc2f;   // wide SFs: no r_jk screen
                 if (e1 == e2) pairs_within(nb, seg[e1], seg[e1 + 1] - seg[e1], rs, Q, lane, f);
                 else pairs_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], rs, Q, lane, f);

@@ -60,4 +60,20 @@ __device__ __forceinline__ double cos_only(double z) {
     return c;
 }
 
+// Cutoff of an SF with its own radius rc_s (nnp_set_sf_cutoffs), from r^2: fc = cos^2(pi r / (2 rc_s)) for
+// r < rc_s, else 0; rc2 = rc_s^2, k2 = (pi / (2 rc_s))^2.  The polynomial argument is clamped to its range.
+__device__ __forceinline__ double fc_own(double r2, double rc2, double k2) {
+    const double C = cos_only(fmin(r2, rc2) * k2);
+    return r2 < rc2 ? C * C : 0.0;
+}
+
+// the same with df = fc'(r) / r
+__device__ __forceinline__ void fc_dfc_own(double r2, double rc2, double k2, double& f, double& df) {
+    double C, S;
+    cos_sinc(fmin(r2, rc2) * k2, C, S);
+    const bool in = r2 < rc2;
+    f = in ? C * C : 0.0;
+    df = in ? (-2.0 * k2) * (C * S) : 0.0;
+}
+
 }  // namespace nnp

@@ -20,6 +20,8 @@ struct nnp_model {
     int g_stride = 0;
     int n_sf_elem[MAX_ELEM] = {0, 0, 0, 0};
     ElemProgram* d_prog[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
+    std::vector<ElemProgram> h_prog;             // host copies as built by nnp_create (global rc, specialised variants)
+    std::vector<std::pair<int, int>> sf_loc;     // per SF of the nnp_create table: (central element, position in its G)
     int variant[MAX_ELEM] = {0, 0, 0, 0};
     NetDesc nets[MAX_ELEM];
     double* d_weights[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
@@ -50,6 +52,12 @@ struct nnp_model {
 };
 
 static std::string g_create_err = "";
+
+// (pi / (2 rc))^2, the argument scale of the cutoff polynomials (same arithmetic as the kernel launchers)
+static double k2_of(double rc) {
+    const double t = 3.14159265358979323846 / (2.0 * rc);
+    return t * t;
+}
 
 static nnp_status fail(nnp_model* m, nnp_status s, const std::string& msg) {
     if (m) m->err = msg;
@@ -207,7 +215,7 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
         if (f.kind == 2) {
             if (f.e1 < 0 || f.e1 >= n_elem) return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.e1 out of range");
             if (!std::isfinite(f.rs)) return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.rs not finite");
-            rad[f.central][f.e1].push_back(RadialSF{f.eta, f.rs, g, 0});
+            rad[f.central][f.e1].push_back(RadialSF{f.eta, f.rs, g, 0, rc * rc, k2_of(rc)});
         } else if (f.kind == 3 || f.kind == 9) {
             if (f.e1 < 0 || f.e1 >= n_elem || f.e2 < 0 || f.e2 >= n_elem)
                 return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.e1/e2 out of range");
@@ -218,7 +226,8 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
                 return fail(nullptr, NNP_ERR_INVALID_ARG, "angular zeta must be an integer in [1, 64]");
             const int a = f.e1 < f.e2 ? f.e1 : f.e2, b = f.e1 < f.e2 ? f.e2 : f.e1;
             ang[f.central][pair_index(a, b, n_elem)].push_back(
-                AngularSF{f.eta, std::exp2(1.0 - f.zeta), g, iz, f.lambda > 0 ? 1 : -1, f.kind == 9 ? 1 : 0});
+                AngularSF{f.eta, std::exp2(1.0 - f.zeta), g, iz, f.lambda > 0 ? 1 : -1, f.kind == 9 ? 1 : 0, rc * rc,
+                          k2_of(rc)});
         } else {
             return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.kind must be 2 (radial), 3 (angular narrow) or 9 (angular wide)");
         }
@@ -368,6 +377,11 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
         if (cudaMallocHost(&m->h_status, 64) != cudaSuccess) return bail(NNP_ERR_CUDA, "cudaMallocHost failed");
         std::memset(m->h_status, 0, 64);
     }
+    m->h_prog = progs;
+    {
+        int cnt[MAX_ELEM] = {0, 0, 0, 0};
+        for (int s = 0; s < n_sf; ++s) m->sf_loc.push_back({sf[s].central, cnt[sf[s].central]++});
+    }
     *out = m;
     return NNP_OK;
 }
@@ -393,6 +407,54 @@ extern "C" void nnp_destroy(nnp_model* m) {
     if (m->md_exec) { cudaStreamSynchronize(m->md_exec_stream); cudaGraphExecDestroy(m->md_exec); }
     if (m->hstream) cudaStreamDestroy(m->hstream);
     delete m;
+}
+
+extern "C" nnp_status nnp_set_sf_cutoffs(nnp_model* m, int32_t n_sf, const double* h_rc) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    if (h_rc && n_sf != (int32_t)m->sf_loc.size()) return fail(m, NNP_ERR_INVALID_ARG, "n_sf differs from the table of nnp_create");
+    std::vector<std::vector<double>> rcg(m->n_elem);
+    for (int c = 0; c < m->n_elem; ++c) rcg[c].assign(m->n_sf_elem[c], m->rc);
+    if (h_rc)
+        for (size_t s = 0; s < m->sf_loc.size(); ++s) {
+            if (!(h_rc[s] > 0.0) || !(h_rc[s] <= m->rc)) return fail(m, NNP_ERR_INVALID_ARG, "SF cutoff must be in (0, rc]");
+            rcg[m->sf_loc[s].first][m->sf_loc[s].second] = h_rc[s];
+        }
+    const int npair = m->n_elem * (m->n_elem + 1) / 2;
+    std::vector<ElemProgram> progs = m->h_prog;
+    for (int c = 0; c < m->n_elem; ++c) {
+        ElemProgram& P = progs[c];
+        bool own = false;
+        int nr = 0, na = 0;
+        for (int e = 0; e < m->n_elem; ++e) nr += P.n_rad[e];
+        for (int p = 0; p < npair; ++p) na += P.n_ang[p];
+        for (int r = 0; r < nr; ++r) {
+            const double x = rcg[c][P.rad[r].g];
+            P.rad[r].rc2 = x * x;
+            P.rad[r].k2 = k2_of(x);
+            own |= x != m->rc;
+        }
+        for (int a = 0; a < na; ++a) {
+            const double x = rcg[c][P.ang[a].g];
+            P.ang[a].rc2 = x * x;
+            P.ang[a].k2 = k2_of(x);
+            own |= x != m->rc;
+        }
+        if (own) {             // the specialised kernels stage ONE fc per neighbour: such an element runs on the generic ones
+            for (int p = 0; p < npair; ++p)
+                if (P.n_ang[p] > 64) return fail(m, NNP_ERR_INVALID_ARG, "generic angular path supports <= 64 SFs per pair group");
+            P.per_sf_rc = 1;
+            P.variant = ANG_GENERIC;
+            P.tiny_exp = 0;
+        }
+    }
+    DeviceGuard dg(m->device);
+    if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
+    NNP_CUDA(m, cudaDeviceSynchronize());          // the old tables may still be in use
+    for (int c = 0; c < m->n_elem; ++c) {
+        NNP_CUDA(m, cudaMemcpy(m->d_prog[c], &progs[c], sizeof(ElemProgram), cudaMemcpyHostToDevice));
+        m->variant[c] = progs[c].variant | (progs[c].tiny_exp << 8);
+    }
+    return NNP_OK;
 }
 
 extern "C" nnp_status nnp_set_sf_scaling(nnp_model* m, int32_t elem, const double* h_shift, const double* h_scale) {

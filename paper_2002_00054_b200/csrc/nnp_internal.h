@@ -31,6 +31,7 @@ struct RadialSF {
     double eta, rs;
     int32_t g;       // position in the element's G vector
     int32_t pad;
+    double rc2, k2;  // this SF's cutoff: rc_s^2 and (pi / (2 rc_s))^2 (read only when ElemProgram::per_sf_rc)
 };
 
 struct AngularSF {
@@ -40,6 +41,7 @@ struct AngularSF {
     int32_t izeta;   // integer zeta
     int32_t lam;     // +1 / -1
     int32_t wide;    // 1: wide angular SF (n2p2 kind 9: no r_jk term, no r_jk cutoff); generic kernels only
+    double rc2, k2;  // this SF's cutoff: rc_s^2 and (pi / (2 rc_s))^2 (read only when ElemProgram::per_sf_rc)
 };
 
 // Angular kernel variants.  Specialised variants bake the (eta ratio, lambda, zeta) structure
@@ -52,6 +54,8 @@ struct ElemProgram {
     int32_t n_elem;
     int32_t variant;                 // AngVariant
     int32_t tiny_exp;                // specialised path: eta_0 rc^2 <= 0.05 -> exp_tiny() for exp(-eta_0 r^2)
+    int32_t per_sf_rc;               // 1: some SF of this element has its own cutoff radius (nnp_set_sf_cutoffs); generic kernels
+    int32_t pad0;
     int32_t n_rad[MAX_ELEM];         // radial SFs for neighbour element e
     int32_t rad_off[MAX_ELEM];       // first index into rad[]
     int32_t n_ang[MAX_PAIR];         // angular SFs of pair group p

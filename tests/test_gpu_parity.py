@@ -191,6 +191,51 @@ def test_wide_angular_mixed_with_narrow():
     _check_full(tiny_model(rows, hidden=(4,), seed=3), sysm)
 
 
+def test_per_sf_cutoff_radii():
+    # every SF with its own cutoff radius (nnp_set_sf_cutoffs) on the rc = 6 neighbourhood;
+    # radial, narrow and wide angular SFs of several radii mixed in the same groups
+    rows, rcs = [], []
+    for c in range(2):
+        for e1 in range(2):
+            for rr in (6.0, 4.5, 3.0):
+                rows.append((c, 2, e1, 0, 0.08, 0.5, 0.0, 0.0)); rcs.append(rr)
+        for (e1, e2) in ((0, 0), (0, 1), (1, 1)):
+            rows.append((c, 3, e1, e2, 0.01, 0.0, 1.0, 2.0)); rcs.append(6.0)
+            rows.append((c, 3, e1, e2, 0.01, 0.0, -1.0, 1.0)); rcs.append(4.0)
+            rows.append((c, 9, e1, e2, 0.02, 0.0, 1.0, 4.0)); rcs.append(5.0)
+            rows.append((c, 9, e1, e2, 0.004, 0.0, -1.0, 2.0)); rcs.append(3.2)
+    model = tiny_model(rows, n_elem=2, hidden=(5, 4), seed=31)
+    model.sf_cutoffs = rcs
+    _check_full(model, W.make_water(150, 5, L=16.7))
+    # only ONE element of the base-52 model gets shorter radii: it moves to the generic kernels, the other
+    # stays on the lane-owned fast path; then back to the global rc: bit-identical to a fresh model
+    from paper_2002_00054_b200 import NNP
+    sysm, base = W.build(W.CONFIGS[0])
+    rc2 = np.where((base.sf["central"] == 1) & (np.arange(len(base.sf)) % 3 == 0), 0.8 * base.rc, base.rc)
+    base.sf_cutoffs = list(rc2)
+    _check_full(base, sysm)
+    nnp = NNP.from_model(base)
+    nnp.set_sf_cutoffs(None)
+    base.sf_cutoffs = None
+    ref = NNP.from_model(base)
+    a, b = _run(nnp, sysm.pos, sysm.types, sysm.box), _run(ref, sysm.pos, sysm.types, sysm.box)
+    assert np.array_equal(a[0], b[0])
+    nnp.close(); ref.close()
+
+
+def test_sf_cutoff_argument_errors():
+    from paper_2002_00054_b200 import NNP, NNPError
+    model = W.make_model(False)
+    nnp = NNP.from_model(model)
+    n = len(model.sf)
+    for bad in ([model.rc] * (n - 1), [model.rc] * (n - 1) + [model.rc * 1.01], [model.rc] * (n - 1) + [0.0],
+                [model.rc] * (n - 1) + [float("nan")]):
+        with pytest.raises(NNPError) as ei:
+            nnp.set_sf_cutoffs(bad)
+        assert ei.value.status == 1                   # NNP_ERR_INVALID_ARG
+    nnp.close()
+
+
 def test_single_element_radial_only():
     model = tiny_model([(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0), (0, 2, 0, 0, 0.4, 2.0, 0.0, 0.0)], hidden=(4,))
     sysm = W.make_water(60, 3, L=12.4)
