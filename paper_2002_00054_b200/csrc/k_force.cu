@@ -145,7 +145,7 @@ struct ForceTripletGeneric {
             // every SF has its own fc(.; rc_s): no common cutoff factor to pull out, the three slot scalars are summed SF by SF
             const double a2j = fma(j0.x, j0.x, fma(j0.y, j0.y, j1.x * j1.x)), a2k = fma(k0.x, k0.x, fma(k0.y, k0.y, k1.x * k1.x));
             const double ia2 = j1.y * j1.y, ib2 = k1.y * k1.y;
-            double s1 = 0.0, s2 = 0.0, s3 = 0.0;
+            double s1 = 0.0, s2 = 0.0, s3 = 0.0, en = -1.0, ew = -1.0, Yn = 0.0, Yw = 0.0;
             for (int s = 0; s < nsf; ++s) {
                 const AngularSF f = list[s];
                 const double base = 1.0 + (double)f.lam * cosv;
@@ -158,7 +158,14 @@ struct ForceTripletGeneric {
                 fc_dfc_own(a2j, f.rc2, f.k2, fa, dfa);
                 fc_dfc_own(a2k, f.rc2, f.k2, fb, dfb);
                 if (!f.wide) fc_dfc_own(c2, f.rc2, f.k2, fcs, dfcs);
-                const double Y = exp(-f.eta * (f.wide ? a2j + a2k : a2j + a2k + c2));
+                double Y;
+                if (f.wide) {
+                    if (f.eta != ew) { ew = f.eta; Yw = exp_small(fmax(-f.eta * (a2j + a2k), -700.0)); }
+                    Y = Yw;
+                } else {
+                    if (f.eta != en) { en = f.eta; Yn = exp_small(fmax(-f.eta * (a2j + a2k + c2), -700.0)); }
+                    Y = Yn;
+                }
                 const double bc = brow[f.g] * f.coef;
                 const double t0 = bc * (pd * base) * Y, t1 = bc * (double)(f.izeta * f.lam) * pd * Y;
                 const double fab = fa * fb, C = fab * fcs;
@@ -173,6 +180,7 @@ struct ForceTripletGeneric {
             return;
         }
         double Z0 = 0.0, Z1 = 0.0, Z2 = 0.0, W0 = 0.0, W1 = 0.0, W2 = 0.0;
+        double en = -1.0, ew = -1.0, Yn = 0.0, Yw = 0.0;
         for (int s = 0; s < nsf; ++s) {
             const AngularSF f = list[s];
             const double base = 1.0 + (double)f.lam * cosv;
@@ -183,7 +191,14 @@ struct ForceTripletGeneric {
                 bb *= bb;
             }
             const double pwv = pd * base;
-            const double Y = exp(-f.eta * (f.wide ? r2ab : r2sum));
+            double Y;           // exp(-eta r^2), shared by consecutive SFs of equal eta
+            if (f.wide) {
+                if (f.eta != ew) { ew = f.eta; Yw = exp_small(fmax(-f.eta * r2ab, -700.0)); }
+                Y = Yw;
+            } else {
+                if (f.eta != en) { en = f.eta; Yn = exp_small(fmax(-f.eta * r2sum, -700.0)); }
+                Y = Yn;
+            }
             const double bc = brow[f.g] * f.coef;
             const double t0 = bc * pwv * Y, t1 = bc * (double)(f.izeta * f.lam) * pd * Y;
             if (f.wide) {

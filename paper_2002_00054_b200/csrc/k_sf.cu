@@ -16,6 +16,7 @@ constexpr int SF_WARPS = 4;
 struct SfParams {
     int64_t n;
     int n_elem, ncell, stride, cap, g_stride;
+    int na_max;                          // largest angular pair group of the model (per-lane accumulators)
     double rc, rc2, inv_rc, k2;          // k2 = (pi / (2 rc))^2
     double box[3], half[3];
     const double *sx, *sy, *sz;
@@ -26,11 +27,11 @@ struct SfParams {
 };
 
 template <class Spec>
-__host__ __device__ constexpr size_t sf_warp_smem(int cap) {
+__host__ __device__ constexpr size_t sf_warp_smem(int cap, int na_max) {
     // p0, p1, p2 (double2 each), a (double), FP32 screening copy (12 B) per slot; queue (64 x u32);
-    // generic accumulators
+    // generic accumulators: one per (SF of the current pair group, lane)
     const size_t capa = (size_t)((cap + 3) & ~3);
-    return capa * (48 + 8 + 12) + 256 + (Spec::ID == ANG_GENERIC ? 64 * 8 : 0);
+    return capa * (48 + 8 + 12) + 256 + (Spec::ID == ANG_GENERIC ? (size_t)(na_max > 1 ? na_max : 1) * 32 * 8 : 0);
 }
 
 // ---- per-triplet work, generic group: walk the SF list, reduce each value over the batch -----
@@ -40,7 +41,7 @@ struct SfTripletGeneric {
     int nsf;
     double k2, rc2;
     const double* ra; // [slot] distance a
-    double* gacc;     // [64] per warp, shared memory
+    double* gacc;     // [nsf][32] per warp, shared memory: every lane sums its own triplets, reduced once per group
     int lane;
     bool own;         // the SFs carry their own cutoff radii (ElemProgram::per_sf_rc)
 
@@ -59,6 +60,8 @@ struct SfTripletGeneric {
         const double r2ab = aj * aj + ak * ak;
         const double r2sum = r2ab + c2;
         const double a2j = fma(j0.x, j0.x, fma(j0.y, j0.y, j1.x * j1.x)), a2k = fma(k0.x, k0.x, fma(k0.y, k0.y, k1.x * k1.x));
+        // exp(-eta r^2) is shared by consecutive SFs of equal eta (the usual order of a table)
+        double en = -1.0, ew = -1.0, Yn = 0.0, Yw = 0.0;
         for (int s = 0; s < nsf; ++s) {
             const AngularSF f = sf[s];
             if (own) {          // fc(.; rc_s) of this SF for a, b (and c)
@@ -71,9 +74,15 @@ struct SfTripletGeneric {
                 if (z & 1) pw *= bb;
                 bb *= bb;
             }
-            double v = f.wide ? f.coef * pw * exp(-f.eta * r2ab) * Cw : f.coef * pw * exp(-f.eta * r2sum) * C;
-            v = warp_sum(v);
-            if (lane == 0) gacc[s] += v;
+            double v;
+            if (f.wide) {
+                if (f.eta != ew) { ew = f.eta; Yw = exp_small(fmax(-f.eta * r2ab, -700.0)); }
+                v = f.coef * pw * Yw * Cw;
+            } else {
+                if (f.eta != en) { en = f.eta; Yn = exp_small(fmax(-f.eta * r2sum, -700.0)); }
+                v = f.coef * pw * Yn * C;
+            }
+            gacc[s * 32 + lane] += v;
         }
         __syncwarp();
     }
@@ -92,7 +101,7 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
     const ElemProgram* __restrict__ prog = p.prog[tc];
 
     const int capa = (p.cap + 3) & ~3;
-    unsigned char* base = smem_raw + (size_t)wid * sf_warp_smem<Spec>(p.cap);
+    unsigned char* base = smem_raw + (size_t)wid * sf_warp_smem<Spec>(p.cap, p.na_max);
     Nbh nb;
     nb.p0 = reinterpret_cast<double2*>(base);
     nb.p1 = nb.p0 + capa;
@@ -170,14 +179,17 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
             const int na = prog->n_ang[pr];
             if (na == 0) continue;
             {
-                for (int s = lane; s < na; s += 32) gacc[s] = 0.0;
+                for (int s = 0; s < na; ++s) gacc[s * 32 + lane] = 0.0;
                 __syncwarp();
                 SfTripletGeneric f{nb, prog->ang + prog->ang_off[pr], na, p.k2, p.rc2, ra, gacc, lane, prog->per_sf_rc != 0};
                 const float rs = group_has_wide(prog->ang + prog->ang_off[pr], na) ? 3.0e38f : rc2f;   // wide SFs: no r_jk screen
                 if (e1 == e2) pairs_within(nb, seg[e1], seg[e1 + 1] - seg[e1], rs, Q, lane, f);
                 else pairs_between(nb, seg[e1], seg[e1 + 1] - seg[e1], seg[e2], seg[e2 + 1] - seg[e2], rs, Q, lane, f);
                 __syncwarp();
-                for (int s = lane; s < na; s += 32) Grow[prog->ang[prog->ang_off[pr] + s].g] = gacc[s];
+                for (int s = 0; s < na; ++s) {
+                    const double v = warp_sum(gacc[s * 32 + lane]);
+                    if (lane == 0) Grow[prog->ang[prog->ang_off[pr] + s].g] = v;
+                }
                 __syncwarp();
             }
         }
@@ -185,7 +197,7 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
 
 template <class Spec>
 static int launch_one(const SfParams& p, cudaStream_t st) {
-    const size_t smem = SF_WARPS * sf_warp_smem<Spec>(p.cap);
+    const size_t smem = SF_WARPS * sf_warp_smem<Spec>(p.cap, p.na_max);
     static bool configured = false;
     if (!configured) {
         cudaFuncSetAttribute(k_sf<Spec>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -197,9 +209,10 @@ static int launch_one(const SfParams& p, cudaStream_t st) {
 }
 
 int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-              const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st) {
+              const int* variant, double rc, int stride, int max_nbr, int g_stride, int na_max, cudaStream_t st) {
     if (n == 0) return 0;
     SfParams p;
+    p.na_max = na_max;
     p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride;
     p.rc = rc; p.rc2 = rc * rc; p.inv_rc = 1.0 / rc;
     p.k2 = (3.14159265358979323846 / (2.0 * rc)) * (3.14159265358979323846 / (2.0 * rc));

@@ -18,6 +18,7 @@ struct nnp_model {
     int device = 0;
     int max_nbr = 160;
     int g_stride = 0;
+    int na_max = 0;                 // largest angular pair group (SF count) of any element
     int n_sf_elem[MAX_ELEM] = {0, 0, 0, 0};
     ElemProgram* d_prog[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
     std::vector<ElemProgram> h_prog;             // host copies as built by nnp_create (global rc, specialised variants)
@@ -262,6 +263,7 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
         int ao = 0;
         for (int p = 0; p < npair; ++p) {
             P.n_ang[p] = (int)ang[c][p].size();
+            if (P.n_ang[p] > m->na_max) m->na_max = P.n_ang[p];
             P.ang_off[p] = ao;
             if (ao + P.n_ang[p] > MAX_ANG_TOTAL) return bail(NNP_ERR_INVALID_ARG, "too many angular SFs (max 512 per element)");
             for (const auto& f : ang[c][p]) P.ang[ao++] = f;
@@ -557,7 +559,7 @@ extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d
     launches += launch_neighbors(w, g, n_atoms, m->n_elem, m->rc * m->rc, stride, m->max_nbr, st);
     mark(2);
     launches += launch_word_offsets(w, g, n_atoms, m->n_elem, m->d_prog, st);
-    launches += launch_sf(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->rc, stride, m->max_nbr, m->g_stride, st);
+    launches += launch_sf(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->rc, stride, m->max_nbr, m->g_stride, m->na_max, st);
     mark(3);
     launches += launch_mlp(w, n_atoms, m->n_elem, g.ncell, m->nets, m->g_stride, st);
     mark(4);

@@ -138,7 +138,7 @@ int launch_sort(const Workspace& w, const Grid& g, int64_t n, int n_elem, const 
 int launch_neighbors(const Workspace& w, const Grid& g, int64_t n, int n_elem, double rc2, int stride,
                      int max_nbr, cudaStream_t st);
 int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-              const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st);
+              const int* variant, double rc, int stride, int max_nbr, int g_stride, int na_max, cudaStream_t st);
 int launch_mlp(const Workspace& w, int64_t n, int n_elem, int ncell, const NetDesc* nets, int g_stride,
                cudaStream_t st);
 int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
