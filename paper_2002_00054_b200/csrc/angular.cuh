@@ -25,6 +25,7 @@ struct SpecGeneric {
     static constexpr int NETA = 0;
     static constexpr int MAXBIT = 0;
     static constexpr int NACC = 0;
+    static constexpr bool FREE_ETA = false;
     __host__ __device__ static constexpr unsigned mask(int) { return 0u; }
     __host__ __device__ static constexpr int ratio(int) { return 1; }
     __host__ __device__ static constexpr int rbase(int) { return 0; }
@@ -36,6 +37,7 @@ struct SpecBase12 {
     static constexpr int NETA = 2;
     static constexpr int MAXBIT = 4;
     static constexpr int NACC = 12;
+    static constexpr bool FREE_ETA = false;
     __host__ __device__ static constexpr unsigned mask(int e) { return e == 0 ? 0x1717u : (e == 1 ? 0x0017u : 0u); }
     __host__ __device__ static constexpr int ratio(int e) { return e == 1 ? 10 : 1; }
     __host__ __device__ static constexpr int rbase(int) { return 0; }
@@ -47,9 +49,24 @@ struct SpecWide32 {
     static constexpr int NETA = 4;
     static constexpr int MAXBIT = 4;
     static constexpr int NACC = 32;
+    static constexpr bool FREE_ETA = false;
     __host__ __device__ static constexpr unsigned mask(int e) { return e < 4 ? 0x1717u : 0u; }
     __host__ __device__ static constexpr int ratio(int e) { return e == 1 ? 3 : (e == 2 ? 10 : (e == 3 ? 3 : 1)); }
     __host__ __device__ static constexpr int rbase(int e) { return e == 3 ? 2 : 0; }
+};
+
+// Any table with at most four distinct eta values (no ratio between them), lambda = +-1 and zeta in {1,2,4,16}: the
+// menu of SpecWide32 with entries allowed to be missing (coefficient 0 / no G index) and exp(-eta_e r^2) evaluated
+// per eta instead of as an integer power of the first -- the lane-owned kernels for models that are not BASELINE.json's.
+struct SpecFree32 {
+    static constexpr int ID = ANG_FREE32;
+    static constexpr int NETA = 4;
+    static constexpr int MAXBIT = 4;
+    static constexpr int NACC = 32;
+    static constexpr bool FREE_ETA = true;
+    __host__ __device__ static constexpr unsigned mask(int e) { return e < 4 ? 0x1717u : 0u; }
+    __host__ __device__ static constexpr int ratio(int) { return 1; }
+    __host__ __device__ static constexpr int rbase(int) { return 0; }
 };
 
 // accumulator slot of menu entry (e, bit) = number of set menu bits before it

@@ -358,7 +358,7 @@ int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const
     for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.dEdG = w.dEdG; p.f_sorted = w.f_sorted;
-    bool use[3] = {false, false, false};
+    bool use[ANG_NVARIANT] = {};
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
         p.variant[e] = e < n_elem ? (variant[e] & 255) : -1;      // bit 8 = tiny_exp flag (fast launchers)
@@ -366,7 +366,7 @@ int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const
     }
     cudaMemsetAsync(w.f_sorted, 0, sizeof(double) * 3 * (size_t)n, st);
     int launches = 0;
-    if (use[ANG_BASE12] || use[ANG_WIDE32])     // specialised tables: lane-owned design (k_force2.cu)
+    if (use[ANG_BASE12] || use[ANG_WIDE32] || use[ANG_FREE32])     // specialised tables: lane-owned design (k_force2.cu)
         launches += launch_force2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, st);
     if (use[ANG_GENERIC]) launches += launch_one<SpecGeneric>(p, st);
     return launches;

@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_fo
             p0[m] = make_double2(dx, dy);
             p1[m] = make_double2(dz, ia);
             p2[m] = make_double2(fa, dfa_a);
-            e0[m] = (tiny ? exp_tiny(-eta0 * a2) : exp_small(-eta0 * a2));
+            e0[m] = Spec::FREE_ETA ? a2 : (tiny ? exp_tiny(-eta0 * a2) : exp_small(-eta0 * a2));   // FREE_ETA: a^2 itself
             f32[m] = make_float4((float)dx, (float)dy, (float)dz, 0.f);
             double R = 0.0;
             for (int r = 0; r < nr; ++r) {
@@ -311,10 +311,16 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_fo
         double dfc = (-2.0 * p.k2) * (Cc * Sc);        // fc'(c)/c
         if (!active || !(c2 < p.rc2)) { fcc = 0.0; dfc = 0.0; }   // exact cutoff (the masks were screened in FP32)
         double Y[Spec::NETA];
-        Y[0] = (J.e0 * ek) * (tiny ? exp_tiny(-eta0 * c2) : exp_small(-eta0 * c2));
-        if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
-        if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
-        if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
+        if constexpr (Spec::FREE_ETA) {
+            const double r2 = (J.e0 + ek) + c2;                // a^2 + b^2 + c^2
+#pragma unroll
+            for (int e = 0; e < Spec::NETA; ++e) Y[e] = exp_small(-eta[e] * r2);
+        } else {
+            Y[0] = (J.e0 * ek) * (tiny ? exp_tiny(-eta0 * c2) : exp_small(-eta0 * c2));
+            if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
+            if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
+            if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
+        }
         const double iab = J.ia * k1.y;
         const double cosv = fma(J.ux, k0.x, fma(J.uy, k0.y, J.uz * k1.x)) * iab;
         // pw[l][b] = (1 +- cos)^(2^b) ; pd[l][b] = (1 +- cos)^(2^b - 1)  (REGC: times zeta = 2^b)
@@ -458,7 +464,7 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.dEdG = w.dEdG; p.f_sorted = w.f_sorted;
     p.word_off = w.word_off; p.gmask = w.gmask; p.gmask_cap = w.gmask_cap;
-    bool use[3][2] = {{false, false}, {false, false}, {false, false}};   // [variant][tiny_exp]
+    bool use[ANG_NVARIANT][2] = {};                                       // [variant][tiny_exp]
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
         p.variant[e] = e < n_elem ? (variant[e] & 255) : -1;                 // bit 8 of variant[] = tiny_exp of the element
@@ -469,6 +475,7 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
     if (use[ANG_BASE12][0]) launches += launch_one2<SpecBase12, false>(p, st);
     if (use[ANG_WIDE32][1]) launches += launch_one2<SpecWide32, true>(p, st);
     if (use[ANG_WIDE32][0]) launches += launch_one2<SpecWide32, false>(p, st);
+    if (use[ANG_FREE32][0]) launches += launch_one2<SpecFree32, false>(p, st);
     return launches;
 }
 

@@ -219,14 +219,14 @@ int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const El
     for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.G = w.G;
-    bool use[3] = {false, false, false};
+    bool use[ANG_NVARIANT] = {};
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
         p.variant[e] = e < n_elem ? (variant[e] & 255) : -1;      // bit 8 = tiny_exp flag (fast launchers)
         if (e < n_elem) use[variant[e] & 255] = true;
     }
     int launches = 0;
-    if (use[ANG_BASE12] || use[ANG_WIDE32])     // specialised tables: lane-owned design (k_sf2.cu)
+    if (use[ANG_BASE12] || use[ANG_WIDE32] || use[ANG_FREE32])     // specialised tables: lane-owned design (k_sf2.cu)
         launches += launch_sf2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, st);
     if (use[ANG_GENERIC]) launches += launch_one<SpecGeneric>(p, st);
     return launches;

@@ -94,7 +94,8 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
         const double Ca = cos_only(a2 * p.k2);
         p0[m] = make_double2(dx, dy);
         p1[m] = make_double2(dz, ia);
-        p2[m] = make_double2((tiny ? exp_tiny(-eta0 * a2) : exp_small(-eta0 * a2)), Ca * Ca);
+        // first component: exp(-eta_0 a^2), or a^2 itself where every eta gets its own exponential (FREE_ETA)
+        p2[m] = make_double2(Spec::FREE_ETA ? a2 : (tiny ? exp_tiny(-eta0 * a2) : exp_small(-eta0 * a2)), Ca * Ca);
         ra[m] = a2 * ia;
         f32[m] = make_float4((float)dx, (float)dy, (float)dz, 0.f);
     }
@@ -181,10 +182,16 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
         double Cf = (jfa * k2v.y) * (Cc * Cc);      // fc(a) fc(b) fc(c), fc(c) = cos^2(pi c / (2 rc))
         if (!active || !(c2 < p.rc2)) Cf = 0.0;     // exact cutoff (the masks were screened in FP32)
         double Y[Spec::NETA];
-        Y[0] = (je0 * k2v.x) * (tiny ? exp_tiny(-eta0 * c2) : exp_small(-eta0 * c2));
-        if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
-        if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
-        if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
+        if constexpr (Spec::FREE_ETA) {
+            const double r2 = (je0 + k2v.x) + c2;              // a^2 + b^2 + c^2
+#pragma unroll
+            for (int e = 0; e < Spec::NETA; ++e) Y[e] = exp_small(-prog->ang_eta[e] * r2);
+        } else {
+            Y[0] = (je0 * k2v.x) * (tiny ? exp_tiny(-eta0 * c2) : exp_small(-eta0 * c2));
+            if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
+            if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
+            if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
+        }
         const double cosv = fma(jx, k0.x, fma(jy, k0.y, jz * k1.x)) * (jia * k1.y);
         double pw[2][Spec::MAXBIT + 1];
         pw[0][0] = 1.0 + cosv;
@@ -306,7 +313,7 @@ int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const E
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.G = w.G;
     p.word_off = w.word_off; p.gmask = w.gmask; p.gmask_cap = w.gmask_cap;
-    bool use[3][2] = {{false, false}, {false, false}, {false, false}};   // [variant][tiny_exp]
+    bool use[ANG_NVARIANT][2] = {};                                       // [variant][tiny_exp]
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
         p.variant[e] = e < n_elem ? (variant[e] & 255) : -1;                 // bit 8 of variant[] = tiny_exp of the element
@@ -317,6 +324,7 @@ int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const E
     if (use[ANG_BASE12][0]) launches += launch_one_sf2<SpecBase12, false>(p, st);
     if (use[ANG_WIDE32][1]) launches += launch_one_sf2<SpecWide32, true>(p, st);
     if (use[ANG_WIDE32][0]) launches += launch_one_sf2<SpecWide32, false>(p, st);
+    if (use[ANG_FREE32][0]) launches += launch_one_sf2<SpecFree32, false>(p, st);
     return launches;
 }
 

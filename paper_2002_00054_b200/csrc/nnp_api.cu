@@ -191,6 +191,43 @@ static bool match_spec(const std::vector<std::vector<AngularSF>>& groups, ElemPr
     return true;
 }
 
+// Any table with <= 4 distinct eta values, lambda = +-1, zeta in {1, 2, 4, 16} and no (eta, lambda, zeta) twice in a pair
+// group runs on SpecFree32: the eta slots are the sorted distinct values (padded with the last one), missing menu
+// entries get no G index (the kernels then skip them / use a zero coefficient).
+static bool match_free32(const std::vector<std::vector<AngularSF>>& groups, ElemProgram* P) {
+    std::vector<double> etas;
+    for (const auto& grp : groups)
+        for (const auto& f : grp) {
+            bool seen = false;
+            for (double e : etas) seen |= (e == f.eta);
+            if (!seen) etas.push_back(f.eta);
+        }
+    if (etas.empty() || (int)etas.size() > SpecFree32::NETA) return false;
+    for (size_t a = 0; a < etas.size(); ++a)
+        for (size_t b = a + 1; b < etas.size(); ++b)
+            if (etas[b] < etas[a]) std::swap(etas[a], etas[b]);
+    for (int e = 0; e < MAX_ETA; ++e) P->ang_eta[e] = e < (int)etas.size() ? etas[e] : etas.back();
+    for (size_t p = 0; p < groups.size(); ++p) {
+        for (int e = 0; e < MAX_ETA; ++e)
+            for (int b = 0; b < 16; ++b) P->ang_g[p][e][b] = -1;
+        unsigned seen[MAX_ETA] = {0, 0, 0, 0};
+        for (const auto& f : groups[p]) {
+            int e = -1;
+            for (int q = (int)etas.size() - 1; q >= 0; --q)
+                if (etas[q] == f.eta) e = q;
+            int bit = -1;
+            for (int b = 0; b < 7; ++b)
+                if (f.izeta == (1 << b)) bit = b;
+            if (e < 0 || bit < 0) return false;
+            if (f.lam < 0) bit += 8;
+            if (!(SpecFree32::mask(e) >> bit & 1u) || (seen[e] >> bit & 1u)) return false;
+            seen[e] |= 1u << bit;
+            P->ang_g[p][e][bit] = (int16_t)f.g;
+        }
+    }
+    return true;
+}
+
 extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* const* elem_names, double rc,
                                  int32_t n_sf, const nnp_sf* sf, const int32_t* n_layers,
                                  const int32_t* const* layer_sizes, const double* const* weights,
@@ -279,13 +316,14 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
             const bool in_range = !any_wide && eta_max * 3.0 * rc * rc <= 700.0;
             if (in_range && match_spec<SpecBase12>(ang[c], &P)) P.variant = ANG_BASE12;
             else if (in_range && match_spec<SpecWide32>(ang[c], &P)) P.variant = ANG_WIDE32;
+            else if (in_range && match_free32(ang[c], &P)) P.variant = ANG_FREE32;
             else {
                 for (int p = 0; p < npair; ++p)
                     if (P.n_ang[p] > 64)
                         return bail(NNP_ERR_INVALID_ARG, "generic angular path supports <= 64 SFs per pair group");
             }
         }
-        P.tiny_exp = (P.variant != ANG_GENERIC && P.ang_eta[0] * rc * rc * (1.0 + 1e-5) <= 0.05) ? 1 : 0;
+        P.tiny_exp = (P.variant != ANG_GENERIC && P.variant != ANG_FREE32 && P.ang_eta[0] * rc * rc * (1.0 + 1e-5) <= 0.05) ? 1 : 0;
         m->variant[c] = P.variant | (P.tiny_exp << 8);      // bit 8: host-side copy of tiny_exp for the launchers
     }
 

@@ -132,6 +132,38 @@ def test_fast_path_one_and_three_elements(elements):
     _check_full(model, sysm)
 
 
+@pytest.mark.parametrize("n_elem", [1, 2, 3])
+def test_fast_path_free_eta_menu(n_elem):
+    # tables that are NOT BASELINE.json's: up to four unrelated eta values, any subset of lambda = +-1 x zeta in
+    # {1, 2, 4, 16}, different subsets per pair group, one group empty -> the lane-owned kernels with per-eta
+    # exponentials and missing menu entries (SpecFree32), not the generic ones
+    etas = (0.0007, 0.003, 0.02, 0.0451)
+    menu = ((1.0, 1.0), (-1.0, 2.0), (1.0, 4.0), (1.0, 16.0), (-1.0, 16.0), (-1.0, 1.0), (1.0, 2.0), (-1.0, 4.0))
+    rows = []
+    pairs = [(a, b) for a in range(n_elem) for b in range(a, n_elem)]
+    for c in range(n_elem):
+        for e1 in range(n_elem):
+            rows.append((c, 2, e1, 0, 0.05 + 0.01 * c, 0.5 * e1, 0.0, 0.0))
+            rows.append((c, 2, e1, 0, 0.3, 1.0, 0.0, 0.0))
+        for ip, (e1, e2) in enumerate(pairs):
+            if n_elem == 3 and ip == 2:
+                continue                                     # an absent pair group
+            for ie, eta in enumerate(etas[:4 - (c % 2)]):   # odd elements use three eta values only
+                for im, (lam, zeta) in enumerate(menu):
+                    if (im + ie + ip + c) % 3 == 0:
+                        continue                             # holes in the menu, different per group and eta
+                    rows.append((c, 3, e1, e2, eta, 0.0, lam, zeta))
+    model = tiny_model(rows, n_elem=n_elem, hidden=(6, 4), seed=13)
+    sysm = W.make_water(120, 5, L=15.0)
+    sysm.types = (np.arange(sysm.n_atoms) % n_elem).astype(np.int32)
+    from paper_2002_00054_b200 import NNP
+    nnp = NNP.from_model(model)
+    assert nnp.uses_fast_path()
+    nnp.close()
+    _check_full(model, sysm)
+    _check_full(model, sysm, max_neighbors=255)
+
+
 def test_fast_path_large_cutoff_general_exp():
     # rc = 8 A: eta_0 rc^2 = 0.064 > 0.05, so the fast kernels take the range-reduced exp (the water-like
     # configs, rc = 6 A, run on the small-argument polynomial exp_tiny)
