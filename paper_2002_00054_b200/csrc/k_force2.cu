@@ -156,6 +156,7 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_fo
     const double xi = p.sx[i], yi = p.sy[i], zi = p.sz[i];
     const int32_t* row = p.nbr + (size_t)i * p.stride;
     const double eta0 = prog->ang_eta[0];
+    const int neta = Spec::FREE_ETA ? prog->n_eta : Spec::NETA;
     constexpr bool tiny = TINY;                      // exp(-eta_0 r^2) without range reduction (mathfn.cuh exp_tiny)
     if ((prog->tiny_exp != 0) != TINY) return;       // uniform per CTA: the other instantiation owns this element
     for (int e = 0; e < p.n_elem; ++e) {
@@ -311,11 +312,8 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_fo
         double dfc = (-2.0 * p.k2) * (Cc * Sc);        // fc'(c)/c
         if (!active || !(c2 < p.rc2)) { fcc = 0.0; dfc = 0.0; }   // exact cutoff (the masks were screened in FP32)
         double Y[Spec::NETA];
-        if constexpr (Spec::FREE_ETA) {
-            const double r2 = (J.e0 + ek) + c2;                // a^2 + b^2 + c^2
-#pragma unroll
-            for (int e = 0; e < Spec::NETA; ++e) Y[e] = exp_small(-eta[e] * r2);
-        } else {
+        const double r2 = (J.e0 + ek) + c2;                    // FREE_ETA: a^2 + b^2 + c^2 (the staged value is a^2)
+        if constexpr (!Spec::FREE_ETA) {
             Y[0] = (J.e0 * ek) * (tiny ? exp_tiny(-eta0 * c2) : exp_small(-eta0 * c2));
             if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
             if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
@@ -343,6 +341,8 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_fo
         double Z0 = 0.0, Z1 = 0.0, Z2 = 0.0;
 #pragma unroll
         for (int e = 0; e < Spec::NETA; ++e) {
+            if (Spec::FREE_ETA && e >= neta) break;            // uniform per CTA: eta slots the table does not use
+            if constexpr (Spec::FREE_ETA) Y[e] = exp_small(-eta[e] * r2);
             double T0 = 0.0, T1 = 0.0;
             // the coefficients of eta_e sit at consecutive (even-aligned) accumulator indices
             constexpr int NE = 16;

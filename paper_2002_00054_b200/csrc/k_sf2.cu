@@ -82,6 +82,10 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
     const double xi = p.sx[i], yi = p.sy[i], zi = p.sz[i];
     const int32_t* row = p.nbr + (size_t)i * p.stride;
     const double eta0 = prog->ang_eta[0];
+    const int neta = Spec::FREE_ETA ? prog->n_eta : Spec::NETA;
+    double etav[Spec::FREE_ETA ? Spec::NETA : 1];
+    if constexpr (Spec::FREE_ETA)
+        for (int e = 0; e < Spec::NETA; ++e) etav[e] = prog->ang_eta[e];
     constexpr bool tiny = TINY;                      // exp(-eta_0 r^2) without range reduction (mathfn.cuh exp_tiny)
     if ((prog->tiny_exp != 0) != TINY) return;       // uniform per CTA: the other instantiation owns this element
     for (int m = tid; m < ntot; m += NT) {
@@ -182,11 +186,8 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
         double Cf = (jfa * k2v.y) * (Cc * Cc);      // fc(a) fc(b) fc(c), fc(c) = cos^2(pi c / (2 rc))
         if (!active || !(c2 < p.rc2)) Cf = 0.0;     // exact cutoff (the masks were screened in FP32)
         double Y[Spec::NETA];
-        if constexpr (Spec::FREE_ETA) {
-            const double r2 = (je0 + k2v.x) + c2;              // a^2 + b^2 + c^2
-#pragma unroll
-            for (int e = 0; e < Spec::NETA; ++e) Y[e] = exp_small(-prog->ang_eta[e] * r2);
-        } else {
+        const double r2 = (je0 + k2v.x) + c2;                  // FREE_ETA: a^2 + b^2 + c^2 (the staged value is a^2)
+        if constexpr (!Spec::FREE_ETA) {
             Y[0] = (je0 * k2v.x) * (tiny ? exp_tiny(-eta0 * c2) : exp_small(-eta0 * c2));
             if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
             if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
@@ -203,6 +204,8 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
         }
 #pragma unroll
         for (int e = 0; e < Spec::NETA; ++e) {
+            if (Spec::FREE_ETA && e >= neta) break;            // uniform per CTA: eta slots the table does not use
+            if constexpr (Spec::FREE_ETA) Y[e] = exp_small(-etav[e] * r2);
             const double xc = Y[e] * Cf;
 #pragma unroll
             for (int b = 0; b <= Spec::MAXBIT; ++b) {

@@ -207,6 +207,7 @@ static bool match_free32(const std::vector<std::vector<AngularSF>>& groups, Elem
         for (size_t b = a + 1; b < etas.size(); ++b)
             if (etas[b] < etas[a]) std::swap(etas[a], etas[b]);
     for (int e = 0; e < MAX_ETA; ++e) P->ang_eta[e] = e < (int)etas.size() ? etas[e] : etas.back();
+    P->n_eta = (int)etas.size();
     for (size_t p = 0; p < groups.size(); ++p) {
         for (int e = 0; e < MAX_ETA; ++e)
             for (int b = 0; b < 16; ++b) P->ang_g[p][e][b] = -1;

@@ -55,7 +55,7 @@ struct ElemProgram {
     int32_t variant;                 // AngVariant
     int32_t tiny_exp;                // specialised path: eta_0 rc^2 <= 0.05 -> exp_tiny() for exp(-eta_0 r^2)
     int32_t per_sf_rc;               // 1: some SF of this element has its own cutoff radius (nnp_set_sf_cutoffs); generic kernels
-    int32_t pad0;
+    int32_t n_eta;                   // SpecFree32: distinct eta values in use (the slots beyond are skipped)
     int32_t n_rad[MAX_ELEM];         // radial SFs for neighbour element e
     int32_t rad_off[MAX_ELEM];       // first index into rad[]
     int32_t n_ang[MAX_PAIR];         // angular SFs of pair group p
