@@ -133,17 +133,6 @@ nnp_status nnp_set_sf_scaling(nnp_model* m, int32_t elem, const double* h_shift,
 nnp_status nnp_set_activation(nnp_model* m, int32_t kind);
 nnp_status nnp_set_sf_cutoffs(nnp_model* m, int32_t n_sf, const double* h_rc);
 
-/* ---- mixed precision: NNP_FORCE_MIXED runs the per-triplet arithmetic of the force kernel
- * (the angular part of step 3, PAPER.md L40 -- 58 % of an evaluation) in FP32 and keeps every accumulation in FP64;
- * symmetry functions, networks, energies and the radial forces stay FP64, so energies are unchanged and forces
- * carry a relative error of ~1e-6 of the largest triplet term (measured: DESIGN.md 2a) -- outside BASELINE.json's
- * 1e-8 eV/A, hence off by default.  Available for models whose every element uses BASELINE.json's base
- * 12-function angular table and for max_neighbors in 129..160; otherwise NNP_ERR_INVALID_ARG (here, or from
- * nnp_compute if the table / max_neighbors changed afterwards).  There is no silent fallback. */
-#define NNP_FORCE_FP64 0
-#define NNP_FORCE_MIXED 1
-nnp_status nnp_set_force_precision(nnp_model* m, int32_t mode);
-
 /* ---- MD loop around the path (the implementation is checked by energy
  * conservation in an NVE run).  Velocity Verlet, everything on the device:
  *     v += (dt/2) F/m ;  x += dt v ;  F = nnp_compute(x) ;  v += (dt/2) F/m

@@ -81,10 +81,10 @@ __host__ __device__ constexpr int acc_index(int e, int bit) {
     return n;
 }
 
-template <int K, class T>
-__device__ __forceinline__ T ipow(T x) {
+template <int K>
+__device__ __forceinline__ double ipow(double x) {
     if constexpr (K <= 1) return x;
-    else if constexpr (K % 2 == 0) { const T h = ipow<K / 2>(x); return h * h; }
+    else if constexpr (K % 2 == 0) { const double h = ipow<K / 2>(x); return h * h; }
     else return x * ipow<K - 1>(x);
 }
 

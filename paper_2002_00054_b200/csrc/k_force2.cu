@@ -101,9 +101,7 @@ struct JData {
 #ifndef F2_MINB1
 #define F2_MINB1 20          // resident CTAs per SM asked of the one-warp-per-centre instantiation (metals: 5.2 vs 5.65 ms at 14)
 #endif
-// MIXED (S:8(f)3, nnp_set_force_precision): the per-triplet arithmetic in FP32 (Taylor cutoff pair, __expf / short
-// polynomial, powers, menu sums, slot scalars), every accumulation (slot sums, j-side sums, flush) in FP64.
-template <class Spec, int WPC, int CAPA, bool TINY, bool MIXED = false>
+template <class Spec, int WPC, int CAPA, bool TINY>
 __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_force2(const __grid_constant__ Force2Params p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NT = WPC * 32;
@@ -262,13 +260,6 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_fo
 #pragma unroll
     for (int a = 0; a < (REGC ? Spec::NACC : 1); ++a) cf[a] = 0.0;
     uint32_t dcur = 0xffffffffu;
-    float jf[MIXED ? 7 : 1];                          // MIXED: FP32 copy of J
-    float cff[MIXED ? Spec::NACC : 1];                // MIXED: FP32 copy of the group's coefficients
-    if constexpr (MIXED) {
-        jf[0] = jf[1] = jf[2] = 1.0f; jf[3] = 1.0f; jf[4] = 0.0f; jf[5] = 0.0f; jf[6] = 1.0f;
-#pragma unroll
-        for (int a = 0; a < Spec::NACC; ++a) cff[a] = 0.0f;
-    }
     for (int it = 0; it < quota; ++it) {
         const bool active = wk.cnt > 0;
         wk.advance();
@@ -290,10 +281,6 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_fo
                 jcur = jn;
                 const double2 a0 = p0[jcur], a1 = p1[jcur], a2 = p2[jcur];
                 J.ux = a0.x; J.uy = a0.y; J.uz = a1.x; J.ia = a1.y; J.fa = a2.x; J.dfa = a2.y; J.e0 = e0[jcur];
-                if constexpr (MIXED) {
-                    jf[0] = (float)J.ux; jf[1] = (float)J.uy; jf[2] = (float)J.uz; jf[3] = (float)J.ia;
-                    jf[4] = (float)J.fa; jf[5] = (float)J.dfa; jf[6] = (float)J.e0;
-                }
                 Aj = 0.0; Vx = 0.0; Vy = 0.0; Vz = 0.0;
             }
             const int pr = p.n_elem <= 2 ? wk.pair2() : pair_of_slots(jn, wk.first_partner(), seg, p.n_elem);
@@ -307,10 +294,6 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_fo
                         cf[2 * a] = c.x; cf[2 * a + 1] = c.y;
                     }
                     if constexpr (Spec::NACC & 1) cf[Spec::NACC - 1] = btc[pr * 2 * bt2_stride<Spec>() + Spec::NACC - 1];
-                    if constexpr (MIXED) {
-#pragma unroll
-                        for (int a = 0; a < Spec::NACC; ++a) cff[a] = (float)cf[a];
-                    }
                 }
             }
         }
@@ -321,84 +304,6 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_fo
         const int rank = conflict_rank(k, active, lane);       // issued early: its latency hides behind the FP64 work
         const double2 k0 = p0[k], k1 = p1[k], k2v = p2[k];
         const double ek = e0[k];
-        if constexpr (MIXED) {
-            static_assert(!MIXED || (REGC && !Spec::FREE_ETA), "mixed precision: register-coefficient specs only");
-            const float kx = (float)k0.x, ky = (float)k0.y, kz = (float)k1.x, kia = (float)k1.y;
-            const float kfa = (float)k2v.x, kdfa = (float)k2v.y;
-            const float wxf = kx - jf[0], wyf = ky - jf[1], wzf = kz - jf[2];
-            const float c2f = fmaf(wxf, wxf, fmaf(wyf, wyf, wzf * wzf));
-            const float k2f = (float)p.k2;
-            const float z = c2f * k2f;
-            // cos(sqrt z) and sin(sqrt z)/sqrt z on [0, (pi/2)^2]: Taylor in z, truncation < 1e-8
-            float Cc = fmaf(z, fmaf(z, fmaf(z, fmaf(z, fmaf(z, fmaf(z, 2.08767570e-9f, -2.75573192e-7f), 2.48015873e-5f),
-                                                     -1.38888889e-3f), 4.16666667e-2f), -0.5f), 1.0f);
-            float Sc = fmaf(z, fmaf(z, fmaf(z, fmaf(z, fmaf(z, -2.50521084e-8f, 2.75573192e-6f), -1.98412698e-4f),
-                                            8.33333333e-3f), -1.66666667e-1f), 1.0f);
-            float fccf = Cc * Cc, dfcf = (-2.0f * k2f) * (Cc * Sc);
-            if (!active || !(c2f < (float)p.rc2)) { fccf = 0.0f; dfcf = 0.0f; }
-            float Yf[Spec::NETA];
-            {
-                const float y = -(float)eta0 * c2f;
-                float ex;
-                if constexpr (tiny) ex = fmaf(y, fmaf(y, fmaf(y, fmaf(y, 4.16666667e-2f, 1.66666667e-1f), 0.5f), 1.0f), 1.0f);
-                else ex = __expf(y);
-                Yf[0] = (jf[6] * (float)ek) * ex;
-            }
-            if constexpr (Spec::NETA > 1) Yf[1] = ipow<Spec::ratio(1)>(Yf[Spec::rbase(1)]);
-            const float iabf = jf[3] * kia;
-            const float cosf_ = fmaf(jf[0], kx, fmaf(jf[1], ky, jf[2] * kz)) * iabf;
-            float pwf[2][Spec::MAXBIT + 1], pdf[2][Spec::MAXBIT + 1];
-            pwf[0][0] = 1.0f + cosf_; pwf[1][0] = 1.0f - cosf_;
-            pdf[0][0] = 1.0f; pdf[1][0] = 1.0f;
-#pragma unroll
-            for (int b = 1; b <= Spec::MAXBIT; ++b) {
-#pragma unroll
-                for (int l = 0; l < 2; ++l) {
-                    pwf[l][b] = pwf[l][b - 1] * pwf[l][b - 1];
-                    pdf[l][b] = pdf[l][b - 1] * pwf[l][b - 1];
-                }
-            }
-#pragma unroll
-            for (int b = 1; b <= Spec::MAXBIT; ++b) {
-                pdf[0][b] *= (float)(1 << b);
-                pdf[1][b] *= (float)(1 << b);
-            }
-            float Z0f = 0.0f, Z1f = 0.0f, Z2f = 0.0f;
-#pragma unroll
-            for (int e = 0; e < Spec::NETA; ++e) {
-                float T0 = 0.0f, T1 = 0.0f;
-#pragma unroll
-                for (int b = 0; b <= Spec::MAXBIT; ++b) {
-#pragma unroll
-                    for (int l = 0; l < 2; ++l)
-                        if (Spec::mask(e) >> (8 * l + b) & 1u) {
-                            const float c = cff[acc_index<Spec>(e, 8 * l + b)];
-                            T0 = fmaf(c, pwf[l][b], T0);
-                            T1 = l == 0 ? fmaf(c, pdf[l][b], T1) : fmaf(-c, pdf[l][b], T1);
-                        }
-                }
-                const float A = T0 * Yf[e];
-                Z0f += A;
-                Z1f = fmaf(T1, Yf[e], Z1f);
-                Z2f = fmaf((float)eta[e], A, Z2f);
-            }
-            const float fab = jf[4] * kfa;
-            const float Cf = fab * fccf;
-            const float t2 = (Cf + Cf) * Z2f;
-            const float f_w = fmaf(fab * dfcf, Z0f, -t2);
-            const float q = Z1f * Cf;
-            const float qc = q * cosf_;
-            const float f_uu = fmaf(-qc, jf[3] * jf[3], fmaf((jf[5] * kfa) * fccf, Z0f, -t2));
-            const float f_vv = fmaf(-qc, kia * kia, fmaf((jf[4] * kdfa) * fccf, Z0f, -t2));
-            const float s1 = f_uu + f_w, s2 = f_vv + f_w, s3 = fmaf(-q, iabf, f_w);
-            Aj += (double)s1;
-            Vx += (double)(s3 * kx);
-            Vy += (double)(s3 * ky);
-            Vz += (double)(s3 * kz);
-            slot_add(acc, k, active, rank, (double)fmaf(s3, jf[0], -s2 * kx), (double)fmaf(s3, jf[1], -s2 * ky),
-                     (double)fmaf(s3, jf[2], -s2 * kz));
-            continue;
-        }
         const double wx = k0.x - J.ux, wy = k0.y - J.uy, wz = k1.x - J.uz;
         const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
         double Cc, Sc;
@@ -547,19 +452,6 @@ static int launch_one2(const Force2Params& p, cudaStream_t st) {
     return launch_capa<Spec, 256, TINY>(p, st);
 }
 
-// FP32 triplet arithmetic, FP64 accumulation (nnp_set_force_precision): base-12 table, 160 slots
-template <bool TINY>
-static int launch_mixed(const Force2Params& p, cudaStream_t st) {
-    const size_t smem = force2_smem<SpecBase12>(160, p.g_stride, p.n_elem, F2_WPC);
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k_force2<SpecBase12, F2_WPC, 160, TINY, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        configured = true;
-    }
-    k_force2<SpecBase12, F2_WPC, 160, TINY, true><<<(unsigned)p.n, F2_WPC * 32, smem, st>>>(p);
-    return 1;
-}
-
 // launches the fast kernels for the specialised variants in use; the caller has zeroed f_sorted
 int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
                   const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st) {
@@ -579,11 +471,6 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
         if (e < n_elem) use[variant[e] & 255][(variant[e] >> 8) & 1] = true;
     }
     int launches = 0;
-    if (n_elem > 0 && (variant[0] >> 9 & 1)) {      // bit 9: mixed-precision force kernel (nnp_api.cu validated table and capacity)
-        if (use[ANG_BASE12][1]) launches += launch_mixed<true>(p, st);
-        if (use[ANG_BASE12][0]) launches += launch_mixed<false>(p, st);
-        return launches;
-    }
     if (use[ANG_BASE12][1]) launches += launch_one2<SpecBase12, true>(p, st);
     if (use[ANG_BASE12][0]) launches += launch_one2<SpecBase12, false>(p, st);
     if (use[ANG_WIDE32][1]) launches += launch_one2<SpecWide32, true>(p, st);

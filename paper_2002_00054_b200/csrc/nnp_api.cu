@@ -18,7 +18,6 @@ struct nnp_model {
     int device = 0;
     int max_nbr = 160;
     int g_stride = 0;
-    int force_mixed = 0;            // nnp_set_force_precision
     int na_max = 0;                 // largest angular pair group (SF count) of any element
     int n_sf_elem[MAX_ELEM] = {0, 0, 0, 0};
     ElemProgram* d_prog[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
@@ -528,22 +527,6 @@ extern "C" nnp_status nnp_set_activation(nnp_model* m, int32_t kind) {
     return NNP_OK;
 }
 
-// The mixed kernel exists for the base-12 table at 160 slots (the BASELINE.json workloads); anything else is refused.
-static bool mixed_ok(const nnp_model* m) {
-    for (int c = 0; c < m->n_elem; ++c)
-        if ((m->variant[c] & 255) != ANG_BASE12) return false;
-    return m->max_nbr > 128 && m->max_nbr <= 160;
-}
-
-extern "C" nnp_status nnp_set_force_precision(nnp_model* m, int32_t mode) {
-    if (!m) return NNP_ERR_INVALID_ARG;
-    if (mode != NNP_FORCE_FP64 && mode != NNP_FORCE_MIXED) return fail(m, NNP_ERR_INVALID_ARG, "unknown force precision");
-    if (mode == NNP_FORCE_MIXED && !mixed_ok(m))
-        return fail(m, NNP_ERR_INVALID_ARG, "mixed force precision needs the base-12 angular table on every element and max_neighbors in 129..160");
-    m->force_mixed = mode;
-    return NNP_OK;
-}
-
 extern "C" nnp_status nnp_set_max_neighbors(nnp_model* m, int32_t max_neighbors) {
     if (!m) return NNP_ERR_INVALID_ARG;
     if (max_neighbors < 32 || max_neighbors > 255) return fail(m, NNP_ERR_INVALID_ARG, "max_neighbors must be 32..255");
@@ -584,8 +567,6 @@ extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d
         if (!std::isfinite(box[c]) || !(box[c] > 0.0)) return fail(m, NNP_ERR_INVALID_ARG, "box length must be finite and > 0");
         if (box[c] < 2.0 * m->rc) return fail(m, NNP_ERR_BOX_TOO_SMALL, "box length < 2*rc");
     }
-    if (m->force_mixed && !mixed_ok(m))
-        return fail(m, NNP_ERR_INVALID_ARG, "mixed force precision no longer applies (table or max_neighbors changed); reset it with nnp_set_force_precision");
     const int stride = row_stride(m);
     Workspace w;
     const size_t need = ws_layout(&w, d_workspace, n_atoms, m->n_elem, stride, m->g_stride);
@@ -621,9 +602,7 @@ extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d
     mark(3);
     launches += launch_mlp(w, n_atoms, m->n_elem, g.ncell, m->nets, m->g_stride, st);
     mark(4);
-    int fvar[MAX_ELEM];
-    for (int c = 0; c < MAX_ELEM; ++c) fvar[c] = m->variant[c] | (m->force_mixed ? 1 << 9 : 0);   // bit 9: mixed-precision force kernel
-    launches += launch_force(w, g, n_atoms, m->n_elem, m->d_prog, fvar, m->rc, stride, m->max_nbr, m->g_stride, st);
+    launches += launch_force(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->rc, stride, m->max_nbr, m->g_stride, st);
     mark(5);
     launches += launch_finalize(w, n_atoms, d_e_atom, d_e_total, d_force, st);
     mark(6);
