@@ -19,10 +19,25 @@ N_STAGES = 6
 STAGE_NAMES = ("sort", "neighbors", "symmetry_functions", "networks", "forces", "finalize")
 
 # every symbol include/nnp.h declares
-EXPORTS = ("nnp_create", "nnp_destroy", "nnp_set_max_neighbors", "nnp_workspace_bytes", "nnp_compute",
+EXPORTS = ("nnp_create", "nnp_table_kernels", "nnp_destroy", "nnp_set_max_neighbors", "nnp_workspace_bytes", "nnp_compute",
            "nnp_compute_host", "nnp_set_sf_scaling", "nnp_set_activation", "nnp_set_sf_cutoffs", "nnp_md_run", "nnp_md_kinetic_energy", "nnp_sync_status", "nnp_get_neighbor_counts", "nnp_get_neighbors", "nnp_get_sf",
            "nnp_get_dedg", "nnp_g_stride", "nnp_set_timing", "nnp_get_timings", "nnp_last_launch_count",
            "nnp_uses_fast_path", "nnp_measure_fp64_peak", "nnp_last_error", "nnp_version")
+
+
+KERNEL_NAMES = ("generic", "base12", "wide32", "free32")
+
+
+def table_kernels(model):
+    """Which kernels each element of `model` would run on (host only, no GPU needed) -> tuple of KERNEL_NAMES."""
+    L = load_library()
+    sf = np.ascontiguousarray(model.sf)
+    out = np.zeros(len(model.elements), dtype=np.int32)
+    st = L.nnp_table_kernels(len(model.elements), float(model.rc), int(sf.shape[0]), sf.ctypes.data_as(C.c_void_p),
+                             out.ctypes.data_as(C.c_void_p))
+    if st != 0:
+        raise NNPError(st, L.nnp_last_error(None).decode())
+    return tuple(KERNEL_NAMES[k] for k in out)
 
 
 class NNPError(RuntimeError):
@@ -52,6 +67,8 @@ def load_library():
     L.nnp_create.restype = C.c_int
     L.nnp_create.argtypes = [C.POINTER(vp), i32, C.POINTER(C.c_char_p), dbl, i32, vp, vp, C.POINTER(vp),
                              C.POINTER(vp), i32]
+    L.nnp_table_kernels.restype = C.c_int
+    L.nnp_table_kernels.argtypes = [i32, dbl, i32, vp, vp]
     L.nnp_destroy.restype = None
     L.nnp_destroy.argtypes = [vp]
     L.nnp_set_max_neighbors.restype = C.c_int

@@ -229,81 +229,66 @@ static bool match_free32(const std::vector<std::vector<AngularSF>>& groups, Elem
     return true;
 }
 
-extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* const* elem_names, double rc,
-                                 int32_t n_sf, const nnp_sf* sf, const int32_t* n_layers,
-                                 const int32_t* const* layer_sizes, const double* const* weights,
-                                 int32_t cuda_device) {
-    if (!out) return fail(nullptr, NNP_ERR_INVALID_ARG, "out is NULL");
-    *out = nullptr;
-    if (n_elem < 1 || n_elem > MAX_ELEM) return fail(nullptr, NNP_ERR_INVALID_ARG, "n_elem must be 1..4");
-    if (!(rc > 0.0) || !std::isfinite(rc)) return fail(nullptr, NNP_ERR_INVALID_ARG, "rc must be > 0");
-    if (n_sf < 1 || !sf || !n_layers || !layer_sizes || !weights)
-        return fail(nullptr, NNP_ERR_INVALID_ARG, "null table");
-
-    std::vector<ElemProgram> progs(n_elem);
+// Host side of nnp_create: validate the SF table and build every element's program, including the choice of
+// kernels (ElemProgram::variant).  No CUDA call in here -- nnp_table_kernels exposes the choice to CPU-only tests.
+static nnp_status build_tables(int n_elem, double rc, int n_sf, const nnp_sf* sf, std::vector<ElemProgram>& progs,
+                               int count[MAX_ELEM], int& na_max, std::string& err) {
+    auto tfail = [&](const char* msg) {
+        err = msg;
+        return NNP_ERR_INVALID_ARG;
+    };
+    na_max = 0;
+    progs.assign(n_elem, ElemProgram());
     std::vector<std::vector<std::vector<AngularSF>>> ang(n_elem);   // [central][pair] -> list
     std::vector<std::vector<std::vector<RadialSF>>> rad(n_elem);    // [central][nbr element] -> list
     int npair = n_elem * (n_elem + 1) / 2;
-    int count[MAX_ELEM] = {0, 0, 0, 0};
+    for (int c = 0; c < MAX_ELEM; ++c) count[c] = 0;
     for (int c = 0; c < n_elem; ++c) { ang[c].resize(npair); rad[c].resize(n_elem); }
     for (int q = 0; q < n_sf; ++q) {
         const nnp_sf& f = sf[q];
-        if (f.central < 0 || f.central >= n_elem) return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.central out of range");
-        if (!(f.eta >= 0.0) || !std::isfinite(f.eta)) return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.eta must be >= 0");
+        if (f.central < 0 || f.central >= n_elem) return tfail("sf.central out of range");
+        if (!(f.eta >= 0.0) || !std::isfinite(f.eta)) return tfail("sf.eta must be >= 0");
         const int g = count[f.central]++;
         if (f.kind == 2) {
-            if (f.e1 < 0 || f.e1 >= n_elem) return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.e1 out of range");
-            if (!std::isfinite(f.rs)) return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.rs not finite");
+            if (f.e1 < 0 || f.e1 >= n_elem) return tfail("sf.e1 out of range");
+            if (!std::isfinite(f.rs)) return tfail("sf.rs not finite");
             rad[f.central][f.e1].push_back(RadialSF{f.eta, f.rs, g, 0, rc * rc, k2_of(rc)});
         } else if (f.kind == 3 || f.kind == 9) {
             if (f.e1 < 0 || f.e1 >= n_elem || f.e2 < 0 || f.e2 >= n_elem)
-                return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.e1/e2 out of range");
+                return tfail("sf.e1/e2 out of range");
             if (!(f.lambda == 1.0 || f.lambda == -1.0))
-                return fail(nullptr, NNP_ERR_INVALID_ARG, "angular lambda must be +1 or -1");
+                return tfail("angular lambda must be +1 or -1");
             const int iz = (int)f.zeta;
             if ((double)iz != f.zeta || iz < 1 || iz > 64)
-                return fail(nullptr, NNP_ERR_INVALID_ARG, "angular zeta must be an integer in [1, 64]");
+                return tfail("angular zeta must be an integer in [1, 64]");
             const int a = f.e1 < f.e2 ? f.e1 : f.e2, b = f.e1 < f.e2 ? f.e2 : f.e1;
             ang[f.central][pair_index(a, b, n_elem)].push_back(
                 AngularSF{f.eta, std::exp2(1.0 - f.zeta), g, iz, f.lambda > 0 ? 1 : -1, f.kind == 9 ? 1 : 0, rc * rc,
                           k2_of(rc)});
         } else {
-            return fail(nullptr, NNP_ERR_INVALID_ARG, "sf.kind must be 2 (radial), 3 (angular narrow) or 9 (angular wide)");
+            return tfail("sf.kind must be 2 (radial), 3 (angular narrow) or 9 (angular wide)");
         }
     }
-
-    nnp_model* m = new nnp_model();
-    m->n_elem = n_elem;
-    m->rc = rc;
-    m->device = cuda_device;
-    for (int c = 0; c < n_elem; ++c) m->names.push_back(elem_names && elem_names[c] ? elem_names[c] : "?");
-    auto bail = [&](nnp_status s, const std::string& msg) {
-        g_create_err = msg;
-        nnp_destroy(m);
-        return s;
-    };
 
     for (int c = 0; c < n_elem; ++c) {
         ElemProgram& P = progs[c];
         std::memset(&P, 0, sizeof(P));
         P.n_sf = count[c];
         P.n_elem = n_elem;
-        m->n_sf_elem[c] = count[c];
-        if (count[c] < 1) return bail(NNP_ERR_INVALID_ARG, "an element has no symmetry functions");
-        if (count[c] > m->g_stride) m->g_stride = count[c];
+        if (count[c] < 1) return tfail("an element has no symmetry functions");
         int ro = 0;
         for (int e = 0; e < n_elem; ++e) {
             P.n_rad[e] = (int)rad[c][e].size();
             P.rad_off[e] = ro;
-            if (ro + P.n_rad[e] > MAX_RAD_TOTAL) return bail(NNP_ERR_INVALID_ARG, "too many radial SFs (max 128 per element)");
+            if (ro + P.n_rad[e] > MAX_RAD_TOTAL) return tfail("too many radial SFs (max 128 per element)");
             for (const auto& f : rad[c][e]) P.rad[ro++] = f;
         }
         int ao = 0;
         for (int p = 0; p < npair; ++p) {
             P.n_ang[p] = (int)ang[c][p].size();
-            if (P.n_ang[p] > m->na_max) m->na_max = P.n_ang[p];
+            if (P.n_ang[p] > na_max) na_max = P.n_ang[p];
             P.ang_off[p] = ao;
-            if (ao + P.n_ang[p] > MAX_ANG_TOTAL) return bail(NNP_ERR_INVALID_ARG, "too many angular SFs (max 512 per element)");
+            if (ao + P.n_ang[p] > MAX_ANG_TOTAL) return tfail("too many angular SFs (max 512 per element)");
             for (const auto& f : ang[c][p]) P.ang[ao++] = f;
         }
         bool any_ang = ao > 0;
@@ -321,11 +306,52 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
             else {
                 for (int p = 0; p < npair; ++p)
                     if (P.n_ang[p] > 64)
-                        return bail(NNP_ERR_INVALID_ARG, "generic angular path supports <= 64 SFs per pair group");
+                        return tfail("generic angular path supports <= 64 SFs per pair group");
             }
         }
         P.tiny_exp = (P.variant != ANG_GENERIC && P.variant != ANG_FREE32 && P.ang_eta[0] * rc * rc * (1.0 + 1e-5) <= 0.05) ? 1 : 0;
-        m->variant[c] = P.variant | (P.tiny_exp << 8);      // bit 8: host-side copy of tiny_exp for the launchers
+    }
+    return NNP_OK;
+}
+
+extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* const* elem_names, double rc,
+                                 int32_t n_sf, const nnp_sf* sf, const int32_t* n_layers,
+                                 const int32_t* const* layer_sizes, const double* const* weights,
+                                 int32_t cuda_device) {
+    if (!out) return fail(nullptr, NNP_ERR_INVALID_ARG, "out is NULL");
+    *out = nullptr;
+    if (n_elem < 1 || n_elem > MAX_ELEM) return fail(nullptr, NNP_ERR_INVALID_ARG, "n_elem must be 1..4");
+    if (!(rc > 0.0) || !std::isfinite(rc)) return fail(nullptr, NNP_ERR_INVALID_ARG, "rc must be > 0");
+    if (n_sf < 1 || !sf || !n_layers || !layer_sizes || !weights)
+        return fail(nullptr, NNP_ERR_INVALID_ARG, "null table");
+
+    std::vector<ElemProgram> progs;
+    int count[MAX_ELEM];
+    int na_max_tab = 0;
+    {
+        std::string terr;
+        const nnp_status ts = build_tables(n_elem, rc, n_sf, sf, progs, count, na_max_tab, terr);
+        if (ts != NNP_OK) return fail(nullptr, ts, terr);
+    }
+    const int npair = n_elem * (n_elem + 1) / 2;
+    (void)npair;
+
+    nnp_model* m = new nnp_model();
+    m->n_elem = n_elem;
+    m->rc = rc;
+    m->device = cuda_device;
+    for (int c = 0; c < n_elem; ++c) m->names.push_back(elem_names && elem_names[c] ? elem_names[c] : "?");
+    auto bail = [&](nnp_status s, const std::string& msg) {
+        g_create_err = msg;
+        nnp_destroy(m);
+        return s;
+    };
+
+    m->na_max = na_max_tab;
+    for (int c = 0; c < n_elem; ++c) {
+        m->n_sf_elem[c] = count[c];
+        if (count[c] > m->g_stride) m->g_stride = count[c];
+        m->variant[c] = progs[c].variant | (progs[c].tiny_exp << 8);      // bit 8: host-side copy of tiny_exp for the launchers
     }
 
     // networks: validate and pack everything on the host first, upload afterwards
@@ -448,6 +474,18 @@ extern "C" void nnp_destroy(nnp_model* m) {
     if (m->md_exec) { cudaStreamSynchronize(m->md_exec_stream); cudaGraphExecDestroy(m->md_exec); }
     if (m->hstream) cudaStreamDestroy(m->hstream);
     delete m;
+}
+
+extern "C" nnp_status nnp_table_kernels(int32_t n_elem, double rc, int32_t n_sf, const nnp_sf* sf, int32_t* kernels_out) {
+    if (n_elem < 1 || n_elem > MAX_ELEM || !(rc > 0.0) || !std::isfinite(rc) || n_sf < 1 || !sf || !kernels_out)
+        return fail(nullptr, NNP_ERR_INVALID_ARG, "bad table arguments");
+    std::vector<ElemProgram> progs;
+    int count[MAX_ELEM], na_max = 0;
+    std::string terr;
+    const nnp_status ts = build_tables(n_elem, rc, n_sf, sf, progs, count, na_max, terr);
+    if (ts != NNP_OK) return fail(nullptr, ts, terr);
+    for (int c = 0; c < n_elem; ++c) kernels_out[c] = progs[c].variant;
+    return NNP_OK;
 }
 
 extern "C" nnp_status nnp_set_sf_cutoffs(nnp_model* m, int32_t n_sf, const double* h_rc) {

@@ -75,6 +75,40 @@ def test_create_rejects_bad_arguments(lib):
     assert _create(lib, model, layer_sizes=ls)[0] == INVALID
 
 
+def test_kernel_choice_per_table(lib):
+    """Host logic of nnp_create: which kernels a symmetry-function table runs on (no GPU involved)."""
+    from conftest import tiny_model
+    from paper_2002_00054_b200.binding import table_kernels, NNPError
+    assert table_kernels(W.make_model(False)) == ("base12", "base12")
+    assert table_kernels(W.make_model(True)) == ("wide32", "wide32")
+    assert table_kernels(W.make_model(False, elements=("A", "B", "C"))) == ("base12",) * 3
+    m = W.make_model(False)
+    ang = m.sf["kind"] == 3
+    m.sf["eta"][ang & (m.sf["eta"] == 0.01)] = 0.0123             # eta ratio broken: the free-eta menu kernels
+    assert table_kernels(m) == ("free32", "free32")
+    m.sf["zeta"][ang & (m.sf["zeta"] == 16.0) & (m.sf["central"] == 1)] = 3.0     # zeta outside {1,2,4,16}: generic, that element only
+    assert table_kernels(m) == ("free32", "generic")
+    m = W.make_model(False)
+    m.sf["kind"][np.nonzero(ang)[0][0]] = 9                         # one wide angular SF on element 0
+    assert table_kernels(m) == ("generic", "base12")
+    m = W.make_model(False)
+    q = np.nonzero(ang)[0][:5]
+    m.sf["eta"][q] = [0.002, 0.003, 0.004, 0.005, 0.006]           # more than four eta values
+    assert table_kernels(m)[0] == "generic"
+    m = W.make_model(False)
+    q = np.nonzero(ang)[0]
+    m.sf["zeta"][q[1]] = m.sf["zeta"][q[0]]; m.sf["lam"][q[1]] = m.sf["lam"][q[0]]; m.sf["eta"][q[1]] = m.sf["eta"][q[0]]
+    assert table_kernels(m)[0] == "generic"                         # the same (eta, lambda, zeta) twice in one pair group
+    rows = [(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0), (0, 3, 0, 0, 0.5, 0.0, 1.0, 2.0)]
+    assert table_kernels(tiny_model(rows, rc=6.0)) == ("free32",)
+    assert table_kernels(tiny_model(rows, rc=25.0)) == ("generic",)  # eta 3 rc^2 > 700: exp_small's range
+    assert table_kernels(tiny_model(rows[:1])) == ("generic",)      # radial only
+    bad = W.make_model(False)
+    bad.sf["lam"][np.nonzero(ang)[0][0]] = 0.5
+    with pytest.raises(NNPError):
+        table_kernels(bad)
+
+
 def test_create_without_gpu_reports_cuda_error(lib):
     import torch
     if torch.cuda.is_available():
