@@ -296,11 +296,16 @@ int launch_mlp(const Workspace& w, int64_t n, int n_elem, int ncell, const NetDe
             ++launches;
             continue;
         }
+        // Atoms per CTA: the 256 threads form 256 / TA groups that each own blocks of four outputs, so TA is chosen
+        // to give as many groups as the widest hidden layer has blocks -- 25 wide: 7 blocks, 8 groups, 32 atoms
+        // (4.6 ms against 6.5 ms with 64 atoms at 2.1 M atoms); 64 wide: 16 blocks, 16 groups, 16 atoms (2.0 ms against
+        // 3.2 ms with 32 atoms on configs[4]: half the shared memory per CTA, twice the resident warps)
+        int widest = 1;
+        for (int l = 1; l < p.net.n_layers; ++l) widest = p.net.sizes[l] > widest ? p.net.sizes[l] : widest;
+        const int blocks = (widest + 3) / 4;
         const size_t budget = 100 * 1024;
-        // 32 atoms per CTA: 8 thread groups cover the 7 output blocks of a 25-wide layer in one round
-        // (measured 4.6 ms against 6.5 ms with 64 atoms / 4 groups at 2.1 M atoms)
-        if (mlp_smem_bytes(p.net, 32) <= budget) launch_ta<32>(p, n, mlp_smem_bytes(p.net, 32), st);
-        else if (mlp_smem_bytes(p.net, 16) <= 2 * budget) launch_ta<16>(p, n, mlp_smem_bytes(p.net, 16), st);
+        if (blocks <= 8 && mlp_smem_bytes(p.net, 32) <= budget) launch_ta<32>(p, n, mlp_smem_bytes(p.net, 32), st);
+        else if (blocks <= 16 && mlp_smem_bytes(p.net, 16) <= 2 * budget) launch_ta<16>(p, n, mlp_smem_bytes(p.net, 16), st);
         else launch_ta<8>(p, n, mlp_smem_bytes(p.net, 8), st);
         ++launches;
     }
