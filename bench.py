@@ -204,6 +204,10 @@ def main():
     ap.add_argument("--md", action="store_true",
                     help="time velocity-Verlet MD steps (nnp_md_run: kick+drift, the whole path, kick) instead of bare evaluations")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--table", default="baseline", choices=["baseline", "free", "generic"],
+                    help="SF table probe (not a BASELINE.json workload): 'free' breaks the eta ratio of the angular set "
+                         "(0.01 -> 0.0123: lane-owned kernels with per-eta exponentials), 'generic' also replaces zeta 16 by 3 "
+                         "(queue-based generic kernels); the roofline object is then not meaningful")
     ap.add_argument("--no-probe", action="store_true", help="skip the DFMA issue-rate probe (for ncu runs)")
     args = ap.parse_args()
     if args.warmup < 3:
@@ -216,6 +220,7 @@ def main():
 
     import workloads as W
     from paper_2002_00054_b200 import NNP, measure_fp64_peak
+    from paper_2002_00054_b200.binding import table_kernels
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -229,6 +234,12 @@ def main():
 
     cfg = W.CONFIGS[args.config]
     sysm, model = W.build(cfg)
+    if args.table != "baseline":
+        ang = model.sf["kind"] == 3
+        model.sf["eta"][ang & (model.sf["eta"] == 0.01)] = 0.0123
+        if args.table == "generic":
+            model.sf["zeta"][ang & (model.sf["zeta"] == 16.0)] = 3.0
+        model.name += "+" + args.table
     n = sysm.n_atoms
     nnp = NNP.from_model(model, device=local)
     if cfg.kind == "metal":
@@ -356,7 +367,7 @@ def main():
         "metric": METRIC, "value": job_value(n, args.steps, world, ms), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg.name, "n_atoms": n, "model": model.name, "box": float(sysm.box[0]),
+        "config": {"workload": cfg.name, "n_atoms": n, "model": model.name, "kernels": list(table_kernels(model)), "box": float(sysm.box[0]),
                    "neighbor_rebuild": "every call", "md": bool(args.md), "parallelism": "replicas x%d" % world,
                    "l2": ("working set per step (%.2f GB workspace) %s the 126 MB L2; no flush between steps"
                           % (nnp.workspace_bytes(n) / 1e9, "exceeds" if nnp.workspace_bytes(n) > 126e6 else "FITS IN"))},
