@@ -86,14 +86,16 @@ nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* const* elem_n
 /* Which kernels a symmetry-function table would run on (host only, no CUDA call; nnp_create takes the same
  * decision): kernels_out[c] for every central element c --
  *   NNP_KERNELS_BASE12 / NNP_KERNELS_WIDE32  the lane-owned kernels specialised for BASELINE.json's two angular tables,
- *   NNP_KERNELS_FREE32   the lane-owned kernels for any table with <= 4 distinct angular eta values, lambda = +-1,
- *                        zeta in {1, 2, 4, 16}, narrow (kind 3) functions only, no (eta, lambda, zeta) twice per pair,
+ *   NNP_KERNELS_FREE32 / NNP_KERNELS_FREE16  the lane-owned kernels for any table with <= 4 (FREE16: <= 2) distinct
+ *                        angular eta values, lambda = +-1, zeta in {1, 2, 4, 16}, narrow (kind 3) functions only,
+ *                        no (eta, lambda, zeta) twice per pair group,
  *   NNP_KERNELS_GENERIC  everything else (other zeta, more eta values, kind 9, no angular functions at all).
  * Returns NNP_ERR_INVALID_ARG for a table nnp_create would reject (message: nnp_last_error(NULL)). */
 #define NNP_KERNELS_GENERIC 0
 #define NNP_KERNELS_BASE12 1
 #define NNP_KERNELS_WIDE32 2
 #define NNP_KERNELS_FREE32 3
+#define NNP_KERNELS_FREE16 4
 nnp_status nnp_table_kernels(int32_t n_elem, double rc, int32_t n_sf, const nnp_sf* sf, int32_t* kernels_out);
 
 /* Free the model and everything the library allocated for it.  NULL is allowed. */

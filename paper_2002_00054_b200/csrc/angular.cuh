@@ -69,6 +69,18 @@ struct SpecFree32 {
     __host__ __device__ static constexpr int rbase(int) { return 0; }
 };
 
+// the same for tables with one or two eta values: half the accumulators, more resident CTAs
+struct SpecFree16 {
+    static constexpr int ID = ANG_FREE16;
+    static constexpr int NETA = 2;
+    static constexpr int MAXBIT = 4;
+    static constexpr int NACC = 16;
+    static constexpr bool FREE_ETA = true;
+    __host__ __device__ static constexpr unsigned mask(int e) { return e < 2 ? 0x1717u : 0u; }
+    __host__ __device__ static constexpr int ratio(int) { return 1; }
+    __host__ __device__ static constexpr int rbase(int) { return 0; }
+};
+
 // accumulator slot of menu entry (e, bit) = number of set menu bits before it
 template <class Spec>
 __host__ __device__ constexpr int acc_index(int e, int bit) {

@@ -476,6 +476,7 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
     if (use[ANG_WIDE32][1]) launches += launch_one2<SpecWide32, true>(p, st);
     if (use[ANG_WIDE32][0]) launches += launch_one2<SpecWide32, false>(p, st);
     if (use[ANG_FREE32][0]) launches += launch_one2<SpecFree32, false>(p, st);
+    if (use[ANG_FREE16][0]) launches += launch_one2<SpecFree16, false>(p, st);
     return launches;
 }
 

@@ -226,7 +226,7 @@ int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const El
         if (e < n_elem) use[variant[e] & 255] = true;
     }
     int launches = 0;
-    if (use[ANG_BASE12] || use[ANG_WIDE32] || use[ANG_FREE32])     // specialised tables: lane-owned design (k_sf2.cu)
+    if (use[ANG_BASE12] || use[ANG_WIDE32] || use[ANG_FREE32] || use[ANG_FREE16])     // specialised tables: lane-owned design (k_sf2.cu)
         launches += launch_sf2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, st);
     if (use[ANG_GENERIC]) launches += launch_one<SpecGeneric>(p, st);
     return launches;

@@ -44,7 +44,7 @@ __host__ __device__ constexpr size_t sf2_smem(int capa, int n_elem, int wpc) {
 #define S2_MINB1 24          // resident CTAs per SM asked of the one-warp-per-centre instantiation (12 SFs per group)
 #endif
 template <class Spec, int WPC, int CAPA, bool TINY>
-__global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MINB1 : 16) : (Spec::NACC <= 12 ? 24 : 16) / WPC) k_sf2(const __grid_constant__ Sf2Params p) {
+__global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MINB1 : 16) : (Spec::NACC <= 12 ? 24 : (Spec::NACC <= 16 ? 20 : 16)) / WPC) k_sf2(const __grid_constant__ Sf2Params p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NT = WPC * 32;
     constexpr int NACC = Spec::NACC;
@@ -328,6 +328,7 @@ int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const E
     if (use[ANG_WIDE32][1]) launches += launch_one_sf2<SpecWide32, true>(p, st);
     if (use[ANG_WIDE32][0]) launches += launch_one_sf2<SpecWide32, false>(p, st);
     if (use[ANG_FREE32][0]) launches += launch_one_sf2<SpecFree32, false>(p, st);
+    if (use[ANG_FREE16][0]) launches += launch_one_sf2<SpecFree16, false>(p, st);
     return launches;
 }
 

@@ -302,14 +302,14 @@ static nnp_status build_tables(int n_elem, double rc, int n_sf, const nnp_sf* sf
             const bool in_range = !any_wide && eta_max * 3.0 * rc * rc <= 700.0;
             if (in_range && match_spec<SpecBase12>(ang[c], &P)) P.variant = ANG_BASE12;
             else if (in_range && match_spec<SpecWide32>(ang[c], &P)) P.variant = ANG_WIDE32;
-            else if (in_range && match_free32(ang[c], &P)) P.variant = ANG_FREE32;
+            else if (in_range && match_free32(ang[c], &P)) P.variant = P.n_eta <= SpecFree16::NETA ? ANG_FREE16 : ANG_FREE32;
             else {
                 for (int p = 0; p < npair; ++p)
                     if (P.n_ang[p] > 64)
                         return tfail("generic angular path supports <= 64 SFs per pair group");
             }
         }
-        P.tiny_exp = (P.variant != ANG_GENERIC && P.variant != ANG_FREE32 && P.ang_eta[0] * rc * rc * (1.0 + 1e-5) <= 0.05) ? 1 : 0;
+        P.tiny_exp = (P.variant != ANG_GENERIC && P.variant != ANG_FREE32 && P.variant != ANG_FREE16 && P.ang_eta[0] * rc * rc * (1.0 + 1e-5) <= 0.05) ? 1 : 0;
     }
     return NNP_OK;
 }

@@ -46,7 +46,7 @@ struct AngularSF {
 
 // Angular kernel variants.  Specialised variants bake the (eta ratio, lambda, zeta) structure
 // of a pair group into the kernel; ANG_GENERIC walks the AngularSF list (any table).
-enum AngVariant : int { ANG_GENERIC = 0, ANG_BASE12 = 1, ANG_WIDE32 = 2, ANG_FREE32 = 3, ANG_NVARIANT = 4 };
+enum AngVariant : int { ANG_GENERIC = 0, ANG_BASE12 = 1, ANG_WIDE32 = 2, ANG_FREE32 = 3, ANG_FREE16 = 4, ANG_NVARIANT = 5 };
 
 // Symmetry-function program of ONE central element; lives in device memory (model-owned).
 struct ElemProgram {

@@ -85,9 +85,12 @@ def test_kernel_choice_per_table(lib):
     m = W.make_model(False)
     ang = m.sf["kind"] == 3
     m.sf["eta"][ang & (m.sf["eta"] == 0.01)] = 0.0123             # eta ratio broken: the free-eta menu kernels
-    assert table_kernels(m) == ("free32", "free32")
+    assert table_kernels(m) == ("free16", "free16")                 # two eta values: the 16-accumulator instantiation
+    m3 = W.make_model(True)
+    m3.sf["eta"][(m3.sf["kind"] == 3) & (m3.sf["eta"] == 0.003)] = 0.0041
+    assert table_kernels(m3) == ("free32", "free32")               # four unrelated eta values
     m.sf["zeta"][ang & (m.sf["zeta"] == 16.0) & (m.sf["central"] == 1)] = 3.0     # zeta outside {1,2,4,16}: generic, that element only
-    assert table_kernels(m) == ("free32", "generic")
+    assert table_kernels(m) == ("free16", "generic")
     m = W.make_model(False)
     m.sf["kind"][np.nonzero(ang)[0][0]] = 9                         # one wide angular SF on element 0
     assert table_kernels(m) == ("generic", "base12")
@@ -100,7 +103,7 @@ def test_kernel_choice_per_table(lib):
     m.sf["zeta"][q[1]] = m.sf["zeta"][q[0]]; m.sf["lam"][q[1]] = m.sf["lam"][q[0]]; m.sf["eta"][q[1]] = m.sf["eta"][q[0]]
     assert table_kernels(m)[0] == "generic"                         # the same (eta, lambda, zeta) twice in one pair group
     rows = [(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0), (0, 3, 0, 0, 0.5, 0.0, 1.0, 2.0)]
-    assert table_kernels(tiny_model(rows, rc=6.0)) == ("free32",)
+    assert table_kernels(tiny_model(rows, rc=6.0)) == ("free16",)
     assert table_kernels(tiny_model(rows, rc=25.0)) == ("generic",)  # eta 3 rc^2 > 700: exp_small's range
     assert table_kernels(tiny_model(rows[:1])) == ("generic",)      # radial only
     bad = W.make_model(False)

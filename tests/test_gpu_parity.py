@@ -132,8 +132,8 @@ def test_fast_path_one_and_three_elements(elements):
     _check_full(model, sysm)
 
 
-@pytest.mark.parametrize("n_elem", [1, 2, 3])
-def test_fast_path_free_eta_menu(n_elem):
+@pytest.mark.parametrize("n_elem,n_eta", [(1, 4), (2, 4), (3, 4), (2, 2), (3, 1)])
+def test_fast_path_free_eta_menu(n_elem, n_eta):
     # tables that are NOT BASELINE.json's: up to four unrelated eta values, any subset of lambda = +-1 x zeta in
     # {1, 2, 4, 16}, different subsets per pair group, one group empty -> the lane-owned kernels with per-eta
     # exponentials and missing menu entries (SpecFree32), not the generic ones
@@ -148,7 +148,7 @@ def test_fast_path_free_eta_menu(n_elem):
         for ip, (e1, e2) in enumerate(pairs):
             if n_elem == 3 and ip == 2:
                 continue                                     # an absent pair group
-            for ie, eta in enumerate(etas[:4 - (c % 2)]):   # odd elements use three eta values only
+            for ie, eta in enumerate(etas[:n_eta - (c % 2 if n_eta > 2 else 0)]):   # n_eta = 4: odd elements use three only
                 for im, (lam, zeta) in enumerate(menu):
                     if (im + ie + ip + c) % 3 == 0:
                         continue                             # holes in the menu, different per group and eta
@@ -157,6 +157,8 @@ def test_fast_path_free_eta_menu(n_elem):
     sysm = W.make_water(120, 5, L=15.0)
     sysm.types = (np.arange(sysm.n_atoms) % n_elem).astype(np.int32)
     from paper_2002_00054_b200 import NNP
+    from paper_2002_00054_b200.binding import table_kernels
+    assert set(table_kernels(model)) == {"free32" if n_eta > 2 else "free16"}     # <= 2 eta values: 16 accumulators
     nnp = NNP.from_model(model)
     assert nnp.uses_fast_path()
     nnp.close()
