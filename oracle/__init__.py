@@ -45,6 +45,17 @@ def lib():
         L.oracle_centres.restype = C.c_int32
         L.oracle_centres.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
                                      C.c_int64, C.c_void_p] + [C.c_void_p] * 3 + [C.c_int64] + [C.c_void_p] * 3
+        L.oracle_centres_ex.restype = C.c_int32
+        L.oracle_centres_ex.argtypes = L.oracle_centres.argtypes + [C.c_int32, C.c_void_p, C.c_void_p, C.c_int64]
+        L.oracle_neighbors_of.restype = C.c_int64
+        L.oracle_neighbors_of.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_double, C.c_int64,
+                                          C.c_void_p, C.c_int64]
+        L.oracle_cells_build.restype = C.c_void_p
+        L.oracle_cells_build.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_double]
+        L.oracle_cells_free.restype = None
+        L.oracle_cells_free.argtypes = [C.c_void_p]
+        L.oracle_neighbors_of_cells.restype = C.c_int64
+        L.oracle_neighbors_of_cells.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_int64]
         _lib = L
     return _lib
 
@@ -109,6 +120,31 @@ def neighbor_list(pos, box, rc):
     return off, idx[:total]
 
 
+def neighbor_rows(pos, box, rc, atoms, search="brute"):
+    """Rows N(m) (ascending original indices) of the given atoms.  search = "brute": the O(N) scan per row
+    (the definition); "cells": the cell-prefiltered scan (same predicate, pinned equal to "brute")."""
+    pos = np.ascontiguousarray(pos, dtype=np.float64)
+    box = np.ascontiguousarray(box, dtype=np.float64)
+    n = pos.shape[0]
+    w = wrap(pos, box)
+    L = lib()
+    buf = np.empty(max(n, 1), dtype=np.int32)
+    cells = L.oracle_cells_build(n, _ptr(w), _ptr(box), float(rc)) if search == "cells" else None
+    assert search in ("brute", "cells")
+    rows = []
+    try:
+        for m in atoms:
+            if cells is not None:
+                cnt = L.oracle_neighbors_of_cells(cells, int(m), _ptr(buf), n)
+            else:
+                cnt = L.oracle_neighbors_of(n, _ptr(w), _ptr(box), float(rc), int(m), _ptr(buf), n)
+            rows.append(buf[:cnt].copy())
+    finally:
+        if cells is not None:
+            L.oracle_cells_free(cells)
+    return rows
+
+
 def mlp(layer_sizes, weights, G, want_beta=True):
     sizes = np.asarray(layer_sizes, dtype=np.int32)
     w = np.ascontiguousarray(weights, dtype=np.float64)
@@ -123,12 +159,14 @@ class Result:
     pass
 
 
-def centres(om: OracleModel, pos, types, box, sel=None, forces=True, want_g=True):
+def centres(om: OracleModel, pos, types, box, sel=None, forces=True, want_g=True, search="brute", rows=False):
     """Run the path for the selected centres (None = all atoms).
 
     Returns Result with e_atom[n_sel], G, dEdG [n_sel][g_stride], nbr_count[n_sel],
     F[N][3] (contributions of the selected centres only; total force if sel is None),
-    e_total (sum over selected), timing (s in neighbour search, s in the rest)."""
+    e_total (sum over selected), timing (s in neighbour search, s in the rest).
+    search: "brute" (the definition) or "cells" (cell-prefiltered, same rows; whole-system goldens).
+    rows=True: also row_off int64[n_sel+1], row_idx int32[total]: the neighbour rows of the selected centres."""
     pos = np.ascontiguousarray(pos, dtype=np.float64)
     types = np.ascontiguousarray(types, dtype=np.int32)
     box = np.ascontiguousarray(box, dtype=np.float64)
@@ -145,9 +183,21 @@ def centres(om: OracleModel, pos, types, box, sel=None, forces=True, want_g=True
     r.nbr_count = np.zeros(n_sel, dtype=np.int32)
     r.F = np.zeros((n, 3), dtype=np.float64) if forces else None
     timing = np.zeros(2, dtype=np.float64)
-    rcode = lib().oracle_centres(C.byref(om.c), n, _ptr(pos), _ptr(types), _ptr(box), n_sel, _ptr(sel_a),
-                                 _ptr(r.e_atom), _ptr(r.G), _ptr(r.dEdG), om.g_stride,
-                                 _ptr(r.nbr_count), _ptr(r.F), _ptr(timing))
+    skind = {"brute": 0, "cells": 1}[search]
+    if rows:
+        cap = 256 * max(n_sel, 1)
+        r.row_off = np.zeros(n_sel + 1, dtype=np.int64)
+        r.row_idx = np.empty(cap, dtype=np.int32)
+    else:
+        cap, r.row_off, r.row_idx = 0, None, None
+    rcode = lib().oracle_centres_ex(C.byref(om.c), n, _ptr(pos), _ptr(types), _ptr(box), n_sel, _ptr(sel_a),
+                                    _ptr(r.e_atom), _ptr(r.G), _ptr(r.dEdG), om.g_stride,
+                                    _ptr(r.nbr_count), _ptr(r.F), _ptr(timing), skind,
+                                    _ptr(r.row_off), _ptr(r.row_idx), cap)
+    if rows and rcode == 0:
+        if r.row_off[-1] > cap:
+            raise ValueError("oracle.centres(rows=True): more than 256 neighbours per centre on average")
+        r.row_idx = r.row_idx[:r.row_off[-1]]
     if rcode != 0:
         raise ValueError("oracle_centres: invalid input (type out of range or box < 2 rc)")
     r.e_total = float(np.sum(r.e_atom))
@@ -171,9 +221,6 @@ def forces_on(om: OracleModel, pos, types, box, atoms, offsets=None, idx=None):
     w = wrap(pos, box)
     out_f, out_e, out_g, out_rows = [], [], [], []
     L = lib()
-    L.oracle_neighbors_of.restype = C.c_int64
-    L.oracle_neighbors_of.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_double, C.c_int64,
-                                      C.c_void_p, C.c_int64]
     buf = np.empty(n, dtype=np.int32)
     for m in atoms:
         cnt = L.oracle_neighbors_of(n, _ptr(w), _ptr(box), om.rc, int(m), _ptr(buf), n)

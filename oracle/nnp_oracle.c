@@ -21,7 +21,9 @@
  * boundary, neighbour sets vs scipy's periodic k-d tree, MLP special cases and
  * finite differences in G, central finite differences of E vs analytic forces,
  * sum F = 0, translation / cube-rotation / free-rotation / permutation invariance,
- * and an independent PyTorch-autograd evaluation of the dense formula.
+ * and an independent PyTorch-autograd evaluation of the dense formula; the cell-prefiltered
+ * neighbour search and oracle.forces_on (the glue of the full-size parity tests) against the
+ * brute-force scan and the whole-system run (tests/test_oracle_cells_pins.py).
  * No function here is "parity unpinned".
  *
  * Build: gcc -O2 -ffp-contract=off -fno-fast-math -shared -fPIC (see oracle/build.py).
@@ -135,6 +137,116 @@ int64_t oracle_neighbor_list(int64_t n, const double* pos, const double* box, do
     offsets[n] = total;
     free(w);
     return total;
+}
+
+/* ---- cell-prefiltered search (whole-system goldens only) ------------------------------
+ * The SAME predicate (min_image + norm2 + strict <) applied to a candidate list instead of
+ * to all N atoms: atoms are binned into nc = floor(L / (rc (1 + 1e-9))) >= 1 cells per
+ * dimension (cell width >= rc (1 + 1e-9), so rounding in the bin index cannot matter) and
+ * row i tests the atoms of the cells within +-1 of i's cell in every dimension, each
+ * distinct periodic cell once.  Why this is a superset of N(i): |d| < rc implies
+ * |d_c| < rc <= cell width in every component, and a component that took the +-L branch of
+ * min_image has x_i, x_j within one cell width of opposite box faces -- in both cases the
+ * cell indices differ by at most 1 modulo nc.  The candidates are then sorted ascending, so
+ * the row equals oracle_neighbors_of() element by element.
+ * It exists because the brute-force scan costs 25 ms per centre at 2.1 M atoms (15 core-hours
+ * for the whole system); tests/golden/make_fullsize_golden.py uses it for whole-system sums
+ * and re-checks rows against the brute-force scan while it runs.  Pinned bit-exact against
+ * oracle_neighbors_of in tests/test_oracle_cells_pins.py (2-cell box, 1-cell dimensions,
+ * 2x3x5 cells, atoms on box faces, every atom of configs[0] and of a 10-cell box). */
+typedef struct {
+    int64_t n;
+    int32_t nc[3];
+    int32_t* start;      /* [ncell + 1] */
+    int32_t* items;      /* [n] atom indices, grouped by cell, ascending inside a cell */
+    const double* w;     /* wrapped positions (not owned) */
+    double box[3], rc;
+} oracle_cells;
+
+static int32_t cell_coord(double x, double L, int32_t nc) {
+    int32_t c = (int32_t)floor(x / L * (double)nc);
+    if (c < 0) c = 0;
+    if (c > nc - 1) c = nc - 1;       /* x == L can come out of the wrap by rounding */
+    return c;
+}
+
+oracle_cells* oracle_cells_build(int64_t n, const double* w, const double* box, double rc) {
+    oracle_cells* C = (oracle_cells*)calloc(1, sizeof(oracle_cells));
+    C->n = n; C->w = w; C->rc = rc;
+    int64_t ncell = 1;
+    for (int c = 0; c < 3; ++c) {
+        C->box[c] = box[c];
+        int32_t k = (int32_t)floor(box[c] / (rc * (1.0 + 1e-9)));
+        if (k < 1) k = 1;
+        if (k > 1024) k = 1024;
+        C->nc[c] = k;
+        ncell *= k;
+    }
+    C->start = (int32_t*)calloc((size_t)ncell + 1, sizeof(int32_t));
+    C->items = (int32_t*)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+    int32_t* cid = (int32_t*)malloc(sizeof(int32_t) * (size_t)(n > 0 ? n : 1));
+    for (int64_t i = 0; i < n; ++i) {
+        int32_t cx = cell_coord(w[3 * i], box[0], C->nc[0]);
+        int32_t cy = cell_coord(w[3 * i + 1], box[1], C->nc[1]);
+        int32_t cz = cell_coord(w[3 * i + 2], box[2], C->nc[2]);
+        cid[i] = (cz * C->nc[1] + cy) * C->nc[0] + cx;
+        C->start[cid[i] + 1] += 1;
+    }
+    for (int64_t c = 0; c < ncell; ++c) C->start[c + 1] += C->start[c];
+    int32_t* fill = (int32_t*)calloc((size_t)ncell, sizeof(int32_t));
+    for (int64_t i = 0; i < n; ++i) C->items[C->start[cid[i]] + fill[cid[i]]++] = (int32_t)i;
+    free(fill); free(cid);
+    return C;
+}
+
+void oracle_cells_free(oracle_cells* C) {
+    if (!C) return;
+    free(C->start); free(C->items); free(C);
+}
+
+static int cmp_i32(const void* a, const void* b) {
+    int32_t x = *(const int32_t*)a, y = *(const int32_t*)b;
+    return (x > y) - (x < y);
+}
+
+/* the distinct cell coordinates within +-1 of c (periodic) along a dimension of nc cells */
+static int stencil_1d(int32_t c, int32_t nc, int32_t* out) {
+    if (nc <= 3) {                        /* 1, 2 or 3 cells: all of them, once */
+        for (int32_t k = 0; k < nc; ++k) out[k] = k;
+        return nc;
+    }
+    out[0] = (c + nc - 1) % nc; out[1] = c; out[2] = (c + 1) % nc;
+    return 3;
+}
+
+/* Row i, same contract as oracle_neighbors_of (ascending j, count returned, first cap written). */
+int64_t oracle_neighbors_of_cells(const oracle_cells* C, int64_t i, int32_t* out, int64_t cap) {
+    const double* w = C->w;
+    double rc2 = C->rc * C->rc, d[3];
+    int32_t sx[3], sy[3], sz[3];
+    int nx = stencil_1d(cell_coord(w[3 * i], C->box[0], C->nc[0]), C->nc[0], sx);
+    int ny = stencil_1d(cell_coord(w[3 * i + 1], C->box[1], C->nc[1]), C->nc[1], sy);
+    int nz = stencil_1d(cell_coord(w[3 * i + 2], C->box[2], C->nc[2]), C->nc[2], sz);
+    int64_t cnt = 0, room = 64;
+    int32_t* tmp = (int32_t*)malloc(sizeof(int32_t) * (size_t)room);
+    for (int a = 0; a < nz; ++a)
+        for (int b = 0; b < ny; ++b)
+            for (int c = 0; c < nx; ++c) {
+                int64_t cell = ((int64_t)sz[a] * C->nc[1] + sy[b]) * C->nc[0] + sx[c];
+                for (int32_t q = C->start[cell]; q < C->start[cell + 1]; ++q) {
+                    int64_t j = C->items[q];
+                    if (j == i) continue;
+                    min_image(w + 3 * i, w + 3 * j, C->box, d);
+                    if (norm2(d) < rc2) {
+                        if (cnt == room) { room *= 2; tmp = (int32_t*)realloc(tmp, sizeof(int32_t) * (size_t)room); }
+                        tmp[cnt++] = (int32_t)j;
+                    }
+                }
+            }
+    qsort(tmp, (size_t)cnt, sizeof(int32_t), cmp_i32);
+    for (int64_t k = 0; k < cnt && k < cap; ++k) out[k] = tmp[k];
+    free(tmp);
+    return cnt;
 }
 
 /* ---- cutoff (reading 2) ------------------------------------------------------- */
@@ -328,11 +440,15 @@ int32_t oracle_n_sf_of(const oracle_model* M, int e) {
  * Outputs (any may be NULL): e_atom[n_sel], G[n_sel][g_stride], dEdG[n_sel][g_stride],
  * nbr_count[n_sel], F[n][3] (accumulated into - caller zeroes), timing[2] =
  * {seconds in neighbour search, seconds in SF + NN + forces}.
+ * search / row_off / row_idx: see the parameter comments (row_idx holds at most row_cap entries; row_off is
+ * always complete, so a second call with a big enough buffer gets every row).
  * Returns 0, or -1 if a type is out of range / box < 2 rc. */
-int32_t oracle_centres(const oracle_model* M, int64_t n, const double* pos, const int32_t* type,
-                       const double* box, int64_t n_sel, const int64_t* sel,
-                       double* e_atom, double* G, double* dEdG, int64_t g_stride,
-                       int32_t* nbr_count, double* F, double* timing) {
+int32_t oracle_centres_ex(const oracle_model* M, int64_t n, const double* pos, const int32_t* type,
+                          const double* box, int64_t n_sel, const int64_t* sel,
+                          double* e_atom, double* G, double* dEdG, int64_t g_stride,
+                          int32_t* nbr_count, double* F, double* timing,
+                          int32_t search /* 0 brute-force scan (the definition), 1 cell-prefiltered (same rows) */,
+                          int64_t* row_off /* [n_sel + 1] or NULL */, int32_t* row_idx /* or NULL */, int64_t row_cap) {
     for (int c = 0; c < 3; ++c)
         if (!(box[c] >= 2.0 * M->rc)) return -1;
     for (int64_t i = 0; i < n; ++i)
@@ -340,6 +456,8 @@ int32_t oracle_centres(const oracle_model* M, int64_t n, const double* pos, cons
     double* w = (double*)malloc(sizeof(double) * 3 * (size_t)n);
     oracle_wrap(n, pos, box, w);
     int32_t* nb = (int32_t*)malloc(sizeof(int32_t) * (size_t)n);
+    oracle_cells* cells = search == 1 ? oracle_cells_build(n, w, box, M->rc) : NULL;
+    int64_t row_total = 0;
     double t_nbr = 0.0, t_rest = 0.0;
     int maxsf = 0;
     for (int e = 0; e < M->n_elem; ++e) {
@@ -351,7 +469,13 @@ int32_t oracle_centres(const oracle_model* M, int64_t n, const double* pos, cons
     for (int64_t q = 0; q < n_sel; ++q) {
         int64_t i = sel ? sel[q] : q;
         double t0 = now_s();
-        int64_t nn = oracle_neighbors_of(n, w, box, M->rc, i, nb, n);
+        int64_t nn = cells ? oracle_neighbors_of_cells(cells, i, nb, n) : oracle_neighbors_of(n, w, box, M->rc, i, nb, n);
+        if (row_off) {                        /* the neighbour rows of the selected centres, CSR */
+            row_off[q] = row_total;
+            for (int64_t m = 0; m < nn; ++m)
+                if (row_idx && row_total + m < row_cap) row_idx[row_total + m] = nb[m];
+            row_total += nn;
+        }
         double* u = (double*)malloc(sizeof(double) * 3 * (size_t)(nn + 1));
         int32_t* tn = (int32_t*)malloc(sizeof(int32_t) * (size_t)(nn + 1));
         for (int64_t m = 0; m < nn; ++m) {
@@ -387,7 +511,18 @@ int32_t oracle_centres(const oracle_model* M, int64_t n, const double* pos, cons
         t_nbr += t1 - t0;
         t_rest += t2 - t1;
     }
+    if (row_off) row_off[n_sel] = row_total;
     if (timing) { timing[0] = t_nbr; timing[1] = t_rest; }
+    oracle_cells_free(cells);
     free(Gi); free(bi); free(nb); free(w);
     return 0;
+}
+
+/* the definition: brute-force neighbour scan, no row export */
+int32_t oracle_centres(const oracle_model* M, int64_t n, const double* pos, const int32_t* type,
+                       const double* box, int64_t n_sel, const int64_t* sel,
+                       double* e_atom, double* G, double* dEdG, int64_t g_stride,
+                       int32_t* nbr_count, double* F, double* timing) {
+    return oracle_centres_ex(M, n, pos, type, box, n_sel, sel, e_atom, G, dEdG, g_stride, nbr_count, F, timing,
+                             0, NULL, NULL, 0);
 }
