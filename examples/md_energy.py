@@ -1,5 +1,5 @@
 """Energy-conservation table of an NVE run (the check the paper uses for its own
-implementation, PAPER.md L80 / Suppl. S2): `python -m paper_2002_00054_b200.md_energy [--molecules M] [--fs T]`.
+implementation, PAPER.md L80 / Suppl. S2): `python examples/md_energy.py [--molecules M] [--fs T]`.
 
 For each time step dt the same start state is integrated for T fs with `nnp_md_run` (velocity Verlet on the
 device, neighbour list rebuilt every step) and the total energy E = E_pot + E_kin is sampled; forces that are
@@ -7,9 +7,13 @@ the exact gradient of the energy give a bounded fluctuation of E that shrinks as
 Prints a markdown table; every number comes from the CUDA path (no oracle, no CPU fallback).
 """
 import argparse
+import os
+import sys
 
 import numpy as np
 import torch
+
+sys.path.insert(0, os.path.dirname(os.path.dirname(os.path.abspath(__file__))))
 
 import workloads as W
 from paper_2002_00054_b200 import NNP

@@ -19,7 +19,8 @@
  *   - nothing here allocates per call except nnp_compute_host (library-owned, cached).
  *   - every function returns an nnp_status; no exceptions, no abort() across the ABI.
  *     Argument errors are returned synchronously.  Errors detected on the device
- *     (neighbour overflow, non-finite input) are reported by nnp_sync_status().
+ *     (neighbour overflow, non-finite input) are reported by nnp_sync_status(), for every
+ *     evaluation since the previous nnp_sync_status().
  *   - nnp_compute enqueues work on the caller's stream and returns without
  *     synchronising.  There is no CPU fallback: without a CUDA device every entry
  *     point that needs one returns NNP_ERR_CUDA.
@@ -45,8 +46,17 @@ typedef enum {
     NNP_ERR_NEIGHBOR_OVERFLOW = 4, /* an atom has more neighbours than max_neighbors (device-detected) */
     NNP_ERR_WORKSPACE = 5,         /* workspace pointer null / misaligned / too small */
     NNP_ERR_CUDA = 6,              /* CUDA runtime error; see nnp_last_error */
-    NNP_ERR_NONFINITE = 7          /* NaN/Inf in positions (device-detected) */
+    NNP_ERR_NONFINITE = 7,         /* NaN/Inf in positions (device-detected) */
+    NNP_ERR_LIMIT = 8              /* a well-formed request beyond a compile-time limit of this build: more than
+                                      NNP_MAX_ELEMENTS elements, max_neighbors > NNP_MAX_NEIGHBORS, a hidden layer wider
+                                      than NNP_MAX_HIDDEN_WIDTH, more than 8 weight layers, more than 128 radial / 512
+                                      angular symmetry functions per element; nnp_last_error names the limit */
 } nnp_status;
+
+/* compile-time limits (NNP_ERR_LIMIT) */
+#define NNP_MAX_ELEMENTS 4
+#define NNP_MAX_NEIGHBORS 255
+#define NNP_MAX_HIDDEN_WIDTH 256
 
 /* One symmetry function of central element `central` (n2p2 numbering, C2-C5).
  *   kind 2 (radial):  G = sum_{j in N(i), t_j = e1} exp(-eta (r_ij - rs)^2) fc(r_ij)
@@ -67,8 +77,9 @@ typedef struct {
     double eta, rs, lambda, zeta;
 } nnp_sf;
 
-/* Create a model on CUDA device `cuda_device`.
- *   n_elem        number of elements (1..4); atom types are indices into elem_names.
+/* Create a model on CUDA device `cuda_device` ("potential parameters, masses, symmetry-function
+ * parameters, NN weights and biases" are per-type tables; L58: n2p2-based initialisation is replaced by these arguments).
+ *   n_elem        number of elements (1..NNP_MAX_ELEMENTS, more: NNP_ERR_LIMIT); atom types are indices into elem_names.
  *   elem_names    [n_elem] NUL-terminated names (copied; informational).
  *   rc            cutoff radius (> 0), one for all symmetry functions.
  *   sf            [n_sf] symmetry functions, all elements together (copied).
@@ -101,11 +112,15 @@ nnp_status nnp_table_kernels(int32_t n_elem, double rc, int32_t n_sf, const nnp_
 /* Free the model and everything the library allocated for it.  NULL is allowed. */
 void nnp_destroy(nnp_model* m);
 
-/* Upper bound on neighbours per atom the kernels provision for (default 160; the
- * water-like workloads average 91, Poisson tail < 150 at 2.1 M atoms).  Range 32..255. */
+/* Upper bound on neighbours per atom the kernels provision for (PAPER.md L48 / L116: the per-atom neighbour list;
+ * default 160 -- the water-like workloads average 91, Poisson tail < 150 at 2.1 M atoms).  Range 32..NNP_MAX_NEIGHBORS
+ * (below 32: NNP_ERR_INVALID_ARG; above 255: NNP_ERR_LIMIT -- the kernels address neighbour slots with 8 bits). */
 nnp_status nnp_set_max_neighbors(nnp_model* m, int32_t max_neighbors);
 
-/* Bytes of device workspace nnp_compute needs for n_atoms (0 on error). */
+/* Bytes of device workspace nnp_compute needs for n_atoms (0 on error): sorted coordinates, neighbour rows, G and
+ * dE/dG rows, screening masks -- about 2.9 KB per atom for the base-52 model.  The derivative tensor dG/dr is never
+ * stored ("store and move as little data as possible, recomputing where necessary"; L82: what lets
+ * 2 M atoms fit one GPU), so this is the whole memory footprint of an evaluation. */
 size_t nnp_workspace_bytes(const nnp_model* m, int64_t n_atoms);
 
 /* One energy + force evaluation (Fig. 1(b) steps 1-3 after the neighbour build).
@@ -173,11 +188,16 @@ nnp_status nnp_md_kinetic_energy(nnp_model* m, const double* h_mass, int64_t n_a
                                  const int32_t* d_type, double* d_ekin, void* d_workspace, size_t workspace_bytes,
                                  void* cuda_stream);
 
-/* Synchronise the stream of the last nnp_compute and return its device-side status. */
+/* Synchronise the stream of the last nnp_compute / nnp_md_run and return the device-side status of EVERY
+ * evaluation enqueued since the previous nnp_sync_status (a sticky device word owned by the model: a neighbour
+ * overflow or a non-finite position in step 3 of a 100-step nnp_md_run, or in the first of several nnp_compute
+ * calls enqueued back to back, is still reported).  Reading clears the word.  Precedence when several flags are
+ * set: NNP_ERR_NONFINITE, NNP_ERR_TYPE_RANGE, NNP_ERR_NEIGHBOR_OVERFLOW. */
 nnp_status nnp_sync_status(nnp_model* m);
 
-/* Debug / parity exports of the LAST nnp_compute (they synchronise its stream first).
- * Atom indices and row order are the CALLER's; all pointers are device memory.
+/* Debug / parity exports of the LAST nnp_compute (they synchronise its stream first): the neighbour list of
+ * PAPER.md L48 / L116 ("random access (neighbor list)"), the descriptors of step 1 and the network gradient
+ * dE/dG of steps 2-3 (L40, Fig. 1(b)).  Atom indices and row order are the CALLER's; all pointers are device memory.
  *   nnp_get_neighbor_counts: d_counts[n_atoms] = |N(i)|.
  *   nnp_get_neighbors: d_offsets[n_atoms+1] (exclusive prefix sum of the counts) and
  *                      d_idx[total] with every row sorted ascending.  d_idx may be NULL to get
@@ -190,21 +210,24 @@ nnp_status nnp_get_sf(nnp_model* m, double* d_G);
 nnp_status nnp_get_dedg(nnp_model* m, double* d_dEdG);
 int32_t nnp_g_stride(const nnp_model* m);
 
-/* Per-stage device times of nnp_compute.  Off by default (no events recorded).
+/* Per-stage device times of nnp_compute: the time split the paper reports per step (Fig. 5:
+ * symmetry functions / network / force; force "up to 60 %", network "a minor part").  Off by default (no events recorded).
  * ms[NNP_N_STAGES]: 0 wrap+bin+sort, 1 neighbour list, 2 symmetry functions,
  * 3 networks fwd+bwd, 4 forces, 5 reduce+un-permute.  Synchronises the stream. */
 #define NNP_N_STAGES 6
 nnp_status nnp_set_timing(nnp_model* m, int32_t enabled);
 nnp_status nnp_get_timings(nnp_model* m, double* ms);
 
-/* Number of kernels the last nnp_compute launched (for launch accounting). */
+/* Number of kernels the last nnp_compute / nnp_md_run launched (launch accounting of the benchmark; every
+ * PAPER.md L98 "parallel_for" of the reference is a launch here too). */
 int32_t nnp_last_launch_count(const nnp_model* m);
 
 /* 1 if the model's angular symmetry functions run on a specialised kernel, 0 if on the
  * generic (slower, any-table) kernel. */
 int32_t nnp_uses_fast_path(const nnp_model* m);
 
-/* Measure the FP64 FMA issue rate of the device (independent DFMA chains on every SM):
+/* Measure the FP64 FMA issue rate of the device (independent DFMA chains on every SM; the path is bound by the
+ * FP64 ALUs, so this is the measured roofline denominator next to the derived one):
  * thread-level DFMA instructions per second, *dfma_per_s = best 10-launch burst,
  * *dfma_per_s_sustained (may be NULL) = mean over the whole `seconds`.  Roofline denominator. */
 nnp_status nnp_measure_fp64_peak(int32_t cuda_device, double seconds, double* dfma_per_s,

@@ -159,14 +159,16 @@ class Result:
     pass
 
 
-def centres(om: OracleModel, pos, types, box, sel=None, forces=True, want_g=True, search="brute", rows=False):
+def centres(om: OracleModel, pos, types, box, sel=None, forces=True, want_g=True, search="brute", rows=False,
+            F_accum=None):
     """Run the path for the selected centres (None = all atoms).
 
     Returns Result with e_atom[n_sel], G, dEdG [n_sel][g_stride], nbr_count[n_sel],
     F[N][3] (contributions of the selected centres only; total force if sel is None),
     e_total (sum over selected), timing (s in neighbour search, s in the rest).
     search: "brute" (the definition) or "cells" (cell-prefiltered, same rows; whole-system goldens).
-    rows=True: also row_off int64[n_sel+1], row_idx int32[total]: the neighbour rows of the selected centres."""
+    rows=True: also row_off int64[n_sel+1], row_idx int32[total]: the neighbour rows of the selected centres.
+    F_accum: a float64 [N][3] array the force contributions are ADDED to (instead of a fresh zero array)."""
     pos = np.ascontiguousarray(pos, dtype=np.float64)
     types = np.ascontiguousarray(types, dtype=np.int32)
     box = np.ascontiguousarray(box, dtype=np.float64)
@@ -181,7 +183,11 @@ def centres(om: OracleModel, pos, types, box, sel=None, forces=True, want_g=True
     r.G = np.zeros((n_sel, om.g_stride), dtype=np.float64) if want_g else None
     r.dEdG = np.zeros((n_sel, om.g_stride), dtype=np.float64) if want_g else None
     r.nbr_count = np.zeros(n_sel, dtype=np.int32)
-    r.F = np.zeros((n, 3), dtype=np.float64) if forces else None
+    if forces and F_accum is not None:
+        assert F_accum.dtype == np.float64 and F_accum.shape == (n, 3) and F_accum.flags.c_contiguous
+        r.F = F_accum
+    else:
+        r.F = np.zeros((n, 3), dtype=np.float64) if forces else None
     timing = np.zeros(2, dtype=np.float64)
     skind = {"brute": 0, "cells": 1}[search]
     if rows:

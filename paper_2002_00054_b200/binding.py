@@ -14,7 +14,8 @@ LIB_PATH = os.path.join(HERE, "libnnp_b200.so")
 
 NNP_OK = 0
 STATUS_NAMES = {0: "NNP_OK", 1: "NNP_ERR_INVALID_ARG", 2: "NNP_ERR_BOX_TOO_SMALL", 3: "NNP_ERR_TYPE_RANGE",
-                4: "NNP_ERR_NEIGHBOR_OVERFLOW", 5: "NNP_ERR_WORKSPACE", 6: "NNP_ERR_CUDA", 7: "NNP_ERR_NONFINITE"}
+                4: "NNP_ERR_NEIGHBOR_OVERFLOW", 5: "NNP_ERR_WORKSPACE", 6: "NNP_ERR_CUDA", 7: "NNP_ERR_NONFINITE",
+                8: "NNP_ERR_LIMIT"}
 N_STAGES = 6
 STAGE_NAMES = ("sort", "neighbors", "symmetry_functions", "networks", "forces", "finalize")
 

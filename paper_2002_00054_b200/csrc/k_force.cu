@@ -339,11 +339,8 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
 template <class Spec>
 static int launch_one(const ForceParams& p, cudaStream_t st) {
     const size_t smem = FC_WARPS * force_warp_smem<Spec>(p.cap, p.g_stride, p.n_elem);
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k_force<Spec>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        configured = true;
-    }
+    static unsigned long long configured = 0ull;      // per device (opt_in_smem)
+    opt_in_smem(k_force<Spec>, &configured);
     const unsigned nb = (unsigned)((p.n + FC_WARPS - 1) / FC_WARPS);
     k_force<Spec><<<nb, FC_WARPS * 32, smem, st>>>(p);
     return 1;

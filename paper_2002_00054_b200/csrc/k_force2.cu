@@ -433,11 +433,8 @@ constexpr int F2_WPC = NNP_F2_WPC;
 template <class Spec, int CAPA, bool TINY, int WPC = F2_WPC>
 static int launch_capa(const Force2Params& p, cudaStream_t st) {
     const size_t smem = force2_smem<Spec>(CAPA, p.g_stride, p.n_elem, WPC);
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k_force2<Spec, WPC, CAPA, TINY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        configured = true;
-    }
+    static unsigned long long configured = 0ull;      // per device (opt_in_smem)
+    opt_in_smem(k_force2<Spec, WPC, CAPA, TINY>, &configured);
     k_force2<Spec, WPC, CAPA, TINY><<<(unsigned)p.n, WPC * 32, smem, st>>>(p);
     return 1;
 }

@@ -266,11 +266,8 @@ size_t mlp_smem_bytes(const NetDesc& net, int TA) {
 
 template <int TA>
 static void launch_ta(const MlpParams& p, int64_t n, size_t smem, cudaStream_t st) {
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k_mlp<TA>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        configured = true;
-    }
+    static unsigned long long configured = 0ull;      // per device (opt_in_smem)
+    opt_in_smem(k_mlp<TA>, &configured);
     const unsigned nb = (unsigned)((n + TA - 1) / TA);   // upper bound; CTAs past the element's range exit
     k_mlp<TA><<<nb, MLP_THREADS, smem, st>>>(p);
 }

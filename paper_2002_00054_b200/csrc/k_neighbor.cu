@@ -27,7 +27,7 @@ __global__ void __launch_bounds__(NB_WARPS * 32)
 k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
             const double* __restrict__ sx, const double* __restrict__ sy, const double* __restrict__ sz,
             const int32_t* __restrict__ cell_start, int32_t* __restrict__ nbr, int32_t* __restrict__ nbr_cnt,
-            int32_t* __restrict__ status) {
+            int32_t* __restrict__ status, int32_t* __restrict__ sticky) {
     const int lane = threadIdx.x & 31;
     const int64_t i = (int64_t)blockIdx.x * NB_WARPS + (threadIdx.x >> 5);
     if (i >= n) return;
@@ -105,7 +105,7 @@ k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
     }
     if (lane == 0) {
         for (int e = n_elem; e < MAX_ELEM; ++e) nbr_cnt[(size_t)i * MAX_ELEM + e] = 0;
-        if (cnt > max_nbr) atomicOr(status, ST_NBR_OVERFLOW);
+        if (cnt > max_nbr) { atomicOr(status, ST_NBR_OVERFLOW); atomicOr(sticky, ST_NBR_OVERFLOW); }
     }
 }
 
@@ -114,7 +114,7 @@ int launch_neighbors(const Workspace& w, const Grid& g, int64_t n, int n_elem, d
     if (n == 0) return 0;
     const unsigned nb = (unsigned)((n + NB_WARPS - 1) / NB_WARPS);
     k_neighbors<<<nb, NB_WARPS * 32, 0, st>>>(n, n_elem, g, rc2, stride, max_nbr, w.sx, w.sy, w.sz, w.cell_start,
-                                              w.nbr, w.nbr_cnt, w.status);
+                                              w.nbr, w.nbr_cnt, w.status, w.sticky);
     return 1;
 }
 

@@ -198,11 +198,8 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
 template <class Spec>
 static int launch_one(const SfParams& p, cudaStream_t st) {
     const size_t smem = SF_WARPS * sf_warp_smem<Spec>(p.cap, p.na_max);
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k_sf<Spec>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        configured = true;
-    }
+    static unsigned long long configured = 0ull;      // per device (opt_in_smem)
+    opt_in_smem(k_sf<Spec>, &configured);
     const unsigned nb = (unsigned)((p.n + SF_WARPS - 1) / SF_WARPS);
     k_sf<Spec><<<nb, SF_WARPS * 32, smem, st>>>(p);
     return 1;

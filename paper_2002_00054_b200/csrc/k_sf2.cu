@@ -286,11 +286,8 @@ constexpr int SF2_WPC = NNP_SF2_WPC;
 template <class Spec, int CAPA, bool TINY, int WPC = SF2_WPC>
 static int launch_capa_sf(const Sf2Params& p, cudaStream_t st) {
     const size_t smem = sf2_smem<Spec>(CAPA, p.n_elem, WPC);
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(k_sf2<Spec, WPC, CAPA, TINY>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        configured = true;
-    }
+    static unsigned long long configured = 0ull;      // per device (opt_in_smem)
+    opt_in_smem(k_sf2<Spec, WPC, CAPA, TINY>, &configured);
     k_sf2<Spec, WPC, CAPA, TINY><<<(unsigned)p.n, WPC * 32, smem, st>>>(p);
     return 1;
 }

@@ -106,7 +106,7 @@ int launch_scan_i64_from_i32(const int32_t* d_in, int64_t n, int64_t* d_out, int
 // key = element * ncell + cell; rank = arrival order inside the key (made deterministic later).
 __global__ void k_bin(int64_t n, const double* __restrict__ pos, const int32_t* __restrict__ type, Grid g,
                       int n_elem, int32_t* __restrict__ key, int32_t* __restrict__ rank,
-                      int32_t* __restrict__ cell_cnt, int32_t* __restrict__ status) {
+                      int32_t* __restrict__ cell_cnt, int32_t* __restrict__ status, int32_t* __restrict__ sticky) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const double x = pos[3 * i], y = pos[3 * i + 1], z = pos[3 * i + 2];
@@ -114,7 +114,7 @@ __global__ void k_bin(int64_t n, const double* __restrict__ pos, const int32_t* 
     int bad = 0;
     if (!(isfinite(x) && isfinite(y) && isfinite(z))) bad |= ST_NONFINITE;
     if (t < 0 || t >= n_elem) { bad |= ST_TYPE_RANGE; t = 0; }
-    if (bad) atomicOr(status, bad);
+    if (bad) { atomicOr(status, bad); atomicOr(sticky, bad); }
     const double wx = (bad & ST_NONFINITE) ? 0.0 : wrap_coord(x, g.box[0]);
     const double wy = (bad & ST_NONFINITE) ? 0.0 : wrap_coord(y, g.box[1]);
     const double wz = (bad & ST_NONFINITE) ? 0.0 : wrap_coord(z, g.box[2]);
@@ -170,7 +170,7 @@ int launch_sort(const Workspace& w, const Grid& g, int64_t n, int n_elem, const 
     cudaMemsetAsync(w.cell_start, 0, sizeof(int32_t) * (size_t)(n_keys + 1), st);
     cudaMemsetAsync(w.status, 0, sizeof(int32_t) * 4, st);
     const unsigned nb = (unsigned)((n + 255) / 256);
-    k_bin<<<nb, 256, 0, st>>>(n, d_pos, d_type, g, n_elem, w.key, w.rank, w.cell_start, w.status);
+    k_bin<<<nb, 256, 0, st>>>(n, d_pos, d_type, g, n_elem, w.key, w.rank, w.cell_start, w.status, w.sticky);
     ++launches;
     exclusive_scan_i32(w.cell_start, n_keys + 1, w.scan_tmp, st, &launches);
     k_scatter<<<nb, 256, 0, st>>>(n, d_pos, g, w.key, w.rank, w.cell_start, w.tx, w.ty, w.tz, w.tperm, w.tkey);

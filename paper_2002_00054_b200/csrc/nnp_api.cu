@@ -37,6 +37,7 @@ struct nnp_model {
     cudaStream_t last_stream = nullptr;
     int last_launches = 0;
     int32_t* h_status = nullptr;   // pinned
+    int32_t* d_sticky = nullptr;   // device word: OR of the status flags of every call since the last nnp_sync_status
     // timing
     bool timing = false;
     bool timing_valid = false;
@@ -52,7 +53,7 @@ struct nnp_model {
     std::string err;
 };
 
-static std::string g_create_err = "";
+static thread_local std::string g_create_err = "";   // nnp_last_error(NULL): per host thread
 
 // (pi / (2 rc))^2, the argument scale of the cutoff polynomials (same arithmetic as the kernel launchers)
 static double k2_of(double rc) {
@@ -237,6 +238,10 @@ static nnp_status build_tables(int n_elem, double rc, int n_sf, const nnp_sf* sf
         err = msg;
         return NNP_ERR_INVALID_ARG;
     };
+    auto lfail = [&](const char* msg) {
+        err = msg;
+        return NNP_ERR_LIMIT;
+    };
     na_max = 0;
     progs.assign(n_elem, ElemProgram());
     std::vector<std::vector<std::vector<AngularSF>>> ang(n_elem);   // [central][pair] -> list
@@ -280,7 +285,7 @@ static nnp_status build_tables(int n_elem, double rc, int n_sf, const nnp_sf* sf
         for (int e = 0; e < n_elem; ++e) {
             P.n_rad[e] = (int)rad[c][e].size();
             P.rad_off[e] = ro;
-            if (ro + P.n_rad[e] > MAX_RAD_TOTAL) return tfail("too many radial SFs (max 128 per element)");
+            if (ro + P.n_rad[e] > MAX_RAD_TOTAL) return lfail("more than 128 radial SFs for one element");
             for (const auto& f : rad[c][e]) P.rad[ro++] = f;
         }
         int ao = 0;
@@ -288,7 +293,7 @@ static nnp_status build_tables(int n_elem, double rc, int n_sf, const nnp_sf* sf
             P.n_ang[p] = (int)ang[c][p].size();
             if (P.n_ang[p] > na_max) na_max = P.n_ang[p];
             P.ang_off[p] = ao;
-            if (ao + P.n_ang[p] > MAX_ANG_TOTAL) return tfail("too many angular SFs (max 512 per element)");
+            if (ao + P.n_ang[p] > MAX_ANG_TOTAL) return lfail("more than 512 angular SFs for one element");
             for (const auto& f : ang[c][p]) P.ang[ao++] = f;
         }
         bool any_ang = ao > 0;
@@ -306,7 +311,7 @@ static nnp_status build_tables(int n_elem, double rc, int n_sf, const nnp_sf* sf
             else {
                 for (int p = 0; p < npair; ++p)
                     if (P.n_ang[p] > 64)
-                        return tfail("generic angular path supports <= 64 SFs per pair group");
+                        return lfail("generic angular path supports <= 64 SFs per pair group");
             }
         }
         P.tiny_exp = (P.variant != ANG_GENERIC && P.variant != ANG_FREE32 && P.variant != ANG_FREE16 && P.ang_eta[0] * rc * rc * (1.0 + 1e-5) <= 0.05) ? 1 : 0;
@@ -320,7 +325,8 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
                                  int32_t cuda_device) {
     if (!out) return fail(nullptr, NNP_ERR_INVALID_ARG, "out is NULL");
     *out = nullptr;
-    if (n_elem < 1 || n_elem > MAX_ELEM) return fail(nullptr, NNP_ERR_INVALID_ARG, "n_elem must be 1..4");
+    if (n_elem < 1) return fail(nullptr, NNP_ERR_INVALID_ARG, "n_elem must be >= 1");
+    if (n_elem > MAX_ELEM) return fail(nullptr, NNP_ERR_LIMIT, "n_elem > NNP_MAX_ELEMENTS (4): this build keeps 4 element segments per neighbour row");
     if (!(rc > 0.0) || !std::isfinite(rc)) return fail(nullptr, NNP_ERR_INVALID_ARG, "rc must be > 0");
     if (n_sf < 1 || !sf || !n_layers || !layer_sizes || !weights)
         return fail(nullptr, NNP_ERR_INVALID_ARG, "null table");
@@ -358,7 +364,8 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
     std::vector<std::vector<double>> packed_all(n_elem);
     for (int c = 0; c < n_elem; ++c) {
         const int L = n_layers[c];
-        if (L < 1 || L > MAX_LAYERS) return bail(NNP_ERR_INVALID_ARG, "n_layers must be 1..8");
+        if (L < 1) return bail(NNP_ERR_INVALID_ARG, "n_layers must be >= 1");
+        if (L > MAX_LAYERS) return bail(NNP_ERR_LIMIT, "more than 8 weight layers");
         const int32_t* sz = layer_sizes[c];
         if (!sz || !weights[c]) return bail(NNP_ERR_INVALID_ARG, "null layer_sizes/weights");
         if (sz[0] != count[c]) return bail(NNP_ERR_INVALID_ARG, "first layer size must equal the element's SF count");
@@ -367,7 +374,8 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
         std::memset(&nd, 0, sizeof(nd));
         nd.n_layers = L;
         for (int l = 0; l <= L; ++l) {
-            if (sz[l] < 1 || (l > 0 && l < L && sz[l] > MAX_WIDTH)) return bail(NNP_ERR_INVALID_ARG, "bad layer width (hidden <= 256)");
+            if (sz[l] < 1) return bail(NNP_ERR_INVALID_ARG, "layer width < 1");
+            if (l > 0 && l < L && sz[l] > MAX_WIDTH) return bail(NNP_ERR_LIMIT, "hidden layer wider than NNP_MAX_HIDDEN_WIDTH (256)");
             nd.sizes[l] = sz[l];
         }
         auto r4 = [](int x) { return (x + 3) & ~3; };
@@ -393,7 +401,7 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
                 }
             for (int o = 0; o < nout; ++o) packed[nd.b_off[l] + o] = B[o];
         }
-        if (mlp_smem_bytes(nd, 8) > 200 * 1024) return bail(NNP_ERR_INVALID_ARG, "network too large for the shared-memory tile");
+        if (mlp_smem_bytes(nd, 8) > 200 * 1024) return bail(NNP_ERR_LIMIT, "network too large for the shared-memory tile");
         // parameter-block copy for the register kernel: n_in -> n1 -> n2 -> 1 with n1, n2 <= 32
         if (L == 3 && sz[1] <= MLP_REG_H && sz[2] <= MLP_REG_H &&
             (size_t)sz[0] * MLP_REG_H + 2 * MLP_REG_H + MLP_REG_H * MLP_REG_H + MLP_REG_H + 1 <= (size_t)MLP_REG_MAXW) {
@@ -443,6 +451,8 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
         DeviceGuard dg(cuda_device);
         if (cudaMallocHost(&m->h_status, 64) != cudaSuccess) return bail(NNP_ERR_CUDA, "cudaMallocHost failed");
         std::memset(m->h_status, 0, 64);
+        if (cudaMalloc(&m->d_sticky, 64) != cudaSuccess || cudaMemset(m->d_sticky, 0, 64) != cudaSuccess)
+            return bail(NNP_ERR_CUDA, "cudaMalloc failed");
     }
     m->h_prog = progs;
     {
@@ -463,6 +473,7 @@ extern "C" void nnp_destroy(nnp_model* m) {
         delete m->reg_w[c];
     }
     if (m->h_status) cudaFreeHost(m->h_status);
+    if (m->d_sticky) cudaFree(m->d_sticky);
     if (m->ev_created)
         for (int k = 0; k <= NNP_N_STAGES; ++k) cudaEventDestroy(m->ev[k]);
     if (m->h_ws) cudaFree(m->h_ws);
@@ -477,7 +488,8 @@ extern "C" void nnp_destroy(nnp_model* m) {
 }
 
 extern "C" nnp_status nnp_table_kernels(int32_t n_elem, double rc, int32_t n_sf, const nnp_sf* sf, int32_t* kernels_out) {
-    if (n_elem < 1 || n_elem > MAX_ELEM || !(rc > 0.0) || !std::isfinite(rc) || n_sf < 1 || !sf || !kernels_out)
+    if (n_elem > MAX_ELEM) return fail(nullptr, NNP_ERR_LIMIT, "n_elem > NNP_MAX_ELEMENTS (4)");
+    if (n_elem < 1 || !(rc > 0.0) || !std::isfinite(rc) || n_sf < 1 || !sf || !kernels_out)
         return fail(nullptr, NNP_ERR_INVALID_ARG, "bad table arguments");
     std::vector<ElemProgram> progs;
     int count[MAX_ELEM], na_max = 0;
@@ -567,7 +579,9 @@ extern "C" nnp_status nnp_set_activation(nnp_model* m, int32_t kind) {
 
 extern "C" nnp_status nnp_set_max_neighbors(nnp_model* m, int32_t max_neighbors) {
     if (!m) return NNP_ERR_INVALID_ARG;
-    if (max_neighbors < 32 || max_neighbors > 255) return fail(m, NNP_ERR_INVALID_ARG, "max_neighbors must be 32..255");
+    if (max_neighbors < 32) return fail(m, NNP_ERR_INVALID_ARG, "max_neighbors must be >= 32");
+    if (max_neighbors > NNP_MAX_NEIGHBORS)
+        return fail(m, NNP_ERR_LIMIT, "max_neighbors > NNP_MAX_NEIGHBORS (255): the kernels address neighbour slots with 8 bits");
     m->max_nbr = max_neighbors;
     m->have_ws = false;
     return NNP_OK;
@@ -610,6 +624,7 @@ extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d
     const size_t need = ws_layout(&w, d_workspace, n_atoms, m->n_elem, stride, m->g_stride);
     if (!d_workspace || ((uintptr_t)d_workspace & 255u) || workspace_bytes < need)
         return fail(m, NNP_ERR_WORKSPACE, "workspace null, misaligned or too small");
+    w.sticky = m->d_sticky;
     DeviceGuard dg(m->device);
     if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -748,9 +763,13 @@ extern "C" nnp_status nnp_sync_status(nnp_model* m) {
     if (!m) return NNP_ERR_INVALID_ARG;
     if (!m->have_ws) return NNP_OK;
     DeviceGuard dg(m->device);
+    // flags of the last call OR the sticky word (every call since the previous nnp_sync_status: the steps of an
+    // nnp_md_run, or several nnp_compute calls enqueued back to back); reading clears the sticky word
     NNP_CUDA(m, cudaMemcpyAsync(m->h_status, m->ws.status, sizeof(int32_t), cudaMemcpyDeviceToHost, m->last_stream));
+    NNP_CUDA(m, cudaMemcpyAsync(m->h_status + 1, m->d_sticky, sizeof(int32_t), cudaMemcpyDeviceToHost, m->last_stream));
+    NNP_CUDA(m, cudaMemsetAsync(m->d_sticky, 0, sizeof(int32_t), m->last_stream));
     NNP_CUDA(m, cudaStreamSynchronize(m->last_stream));
-    const int s = m->h_status[0];
+    const int s = m->h_status[0] | m->h_status[1];
     if (s & ST_NONFINITE) return fail(m, NNP_ERR_NONFINITE, "non-finite position");
     if (s & ST_TYPE_RANGE) return fail(m, NNP_ERR_TYPE_RANGE, "atom type out of range");
     if (s & ST_NBR_OVERFLOW) return fail(m, NNP_ERR_NEIGHBOR_OVERFLOW, "an atom has more than max_neighbors neighbours");

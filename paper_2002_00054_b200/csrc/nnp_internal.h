@@ -125,12 +125,25 @@ struct Workspace {
     uint32_t *gmask;                 // [gmask_cap]
     int64_t gmask_cap;
     double *partial;                 // [n_partial] block sums of the energy
-    int32_t *status;                 // [4]
+    int32_t *status;                 // [4]; word 0 = flags of this nnp_compute (cleared by launch_sort)
+    int32_t *sticky;                 // model-owned word: flags of every call since the last nnp_sync_status (set by nnp_compute, not by ws_layout)
     int64_t n_keys_cap;
     int64_t scan_tmp_len;
     int64_t n_partial;
     size_t bytes;
 };
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-DEVICE attribute: opt a kernel instantiation in once per
+// device it is launched on (`done` = one static bit mask per instantiation, indexed by the current device).  A
+// failure stays in the runtime's last-error slot and is returned by the cudaGetLastError() at the end of nnp_compute.
+template <class K>
+inline void opt_in_smem(K kernel, unsigned long long* done, int bytes = 200 * 1024) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return;
+    if (dev >= 0 && dev < 64 && ((*done >> dev) & 1ull)) return;
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess && dev >= 0 && dev < 64)
+        *done |= 1ull << dev;
+}
 
 // ---- launchers (each enqueues on `st`; returns the number of kernels launched) ----------
 int launch_sort(const Workspace& w, const Grid& g, int64_t n, int n_elem, const double* d_pos,

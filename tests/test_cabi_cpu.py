@@ -56,7 +56,12 @@ def test_create_rejects_bad_arguments(lib):
     model = W.make_model(False)
     INVALID = 1
     assert _create(lib, model, n_elem=0)[0] == INVALID
-    assert _create(lib, model, n_elem=5)[0] == INVALID
+    assert _create(lib, model, n_elem=5)[0] == 8          # NNP_ERR_LIMIT: a compile-time limit, with its own message
+    assert b"NNP_MAX_ELEMENTS" in lib.nnp_last_error(None)
+    ls = [list(x) for x in model.layer_sizes]; ls[0][1] = 300
+    w = [np.zeros(52 * 300 + 300 + 300 * 25 + 25 + 25 + 1), model.weights[1]]
+    assert _create(lib, model, layer_sizes=ls, weights=w)[0] == 8
+    assert b"256" in lib.nnp_last_error(None)
     assert _create(lib, model, rc=-1.0)[0] == INVALID
     sf = model.sf.copy(); sf["kind"][3] = 7
     assert _create(lib, model, sf=sf)[0] == INVALID

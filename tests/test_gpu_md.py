@@ -84,3 +84,60 @@ def test_md_argument_errors():
     nnp.md_run(0, 0.5, MASS, pos_d, vel_d, typ_d, sysm.box, state)     # zero steps: nothing changes
     assert torch.equal(pos_d.cpu(), torch.tensor(sysm.pos, dtype=torch.float64))
     nnp.close()
+
+
+def _imploding_shell():
+    """One centre atom and 33 atoms on a sphere of radius 8 A around it, flying inwards at 1 A/fs: with
+    max_neighbors = 32 the start (radius 8) and the end (radius 8 on the far side, 16 steps of 1 fs later) are
+    fine, the steps in between overflow (33 neighbours of the centre at radius < 6, all 33 mutual below ~3)."""
+    k = np.arange(33) + 0.5
+    phi = np.arccos(1.0 - 2.0 * k / 33.0)
+    th = np.pi * (1.0 + 5.0 ** 0.5) * k
+    unit = np.stack([np.cos(th) * np.sin(phi), np.sin(th) * np.sin(phi), np.cos(phi)], axis=1)
+    c = np.array([20.0, 20.0, 20.0])
+    pos = np.concatenate([[c], c + 8.0 * unit])
+    vel = np.concatenate([[np.zeros(3)], -1.0 * unit])
+    types = np.zeros(34, dtype=np.int32)
+    return pos, vel, types, np.array([40.0, 40.0, 40.0])
+
+
+@pytest.mark.parametrize("n_steps", [16, 3])     # 16: CUDA-graph replay of steps 2..n; 3: plain launches
+def test_md_run_reports_an_error_of_a_middle_step(n_steps):
+    # ADVICE r1: every step's nnp_compute clears the device status word, so an overflow in steps 5..11 used to be
+    # lost (NNP_OK after the run, wrong forces integrated).  The sticky word keeps it until nnp_sync_status.
+    from paper_2002_00054_b200 import NNP, NNPError
+    model = W.make_model(False, seed=5, elements=("X",), hidden=(6, 4))
+    pos, vel, types, box = _imploding_shell()
+    dev = torch.device("cuda", 0)
+    nnp = NNP.from_model(model)
+    nnp.set_max_neighbors(32)
+    pos_d = torch.tensor(pos, dtype=torch.float64, device=dev)
+    vel_d = torch.tensor(vel, dtype=torch.float64, device=dev)
+    typ_d = torch.tensor(types, dtype=torch.int32, device=dev)
+    heavy = (1.0e6,)                                   # ballistic: the forces do not deflect anything
+    state = nnp.compute(pos_d, typ_d, box)             # radius 8: fine
+    with pytest.raises(NNPError) as ei:                # 16 steps of 1 fs, or 3 steps of 16/3 fs (radius 8, 2.67, -2.67, -8)
+        nnp.md_run(n_steps, 16.0 / n_steps, heavy, pos_d, vel_d, typ_d, box, state)
+    assert ei.value.status == 4                        # NNP_ERR_NEIGHBOR_OVERFLOW, from a middle step
+    r = np.linalg.norm(pos_d.cpu().numpy()[1:] - pos[0], axis=1)
+    assert np.all(np.abs(r - 8.0) < 1e-3)              # the LAST step is fine again
+    nnp.compute(pos_d, typ_d, box)                     # ... and reading cleared the sticky word
+    nnp.close()
+
+
+def test_sync_status_covers_every_call_since_the_last_sync():
+    from paper_2002_00054_b200 import NNP, NNPError
+    sysm, model = W.build(W.CONFIGS[0])
+    dev = torch.device("cuda", 0)
+    nnp = NNP.from_model(model)
+    good = torch.tensor(sysm.pos, dtype=torch.float64, device=dev)
+    bad = good.clone(); bad[17, 2] = float("inf")
+    typ = torch.tensor(sysm.types, dtype=torch.int32, device=dev)
+    nnp.compute(good, typ, sysm.box, sync=False)
+    nnp.compute(bad, typ, sysm.box, sync=False)
+    nnp.compute(good, typ, sysm.box, sync=False)
+    with pytest.raises(NNPError) as ei:
+        nnp.sync_status()
+    assert ei.value.status == 7                        # NNP_ERR_NONFINITE of the middle call
+    nnp.sync_status()                                  # cleared by reading
+    nnp.close()

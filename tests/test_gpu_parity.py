@@ -2,6 +2,10 @@
 same seeded inputs.  Tolerances (BASELINE.json north_star):
   neighbour sets bit-exact (sorted index lists); total energy relative 1e-10;
   force components absolute 1e-8 eV/A; e_atom abs 1e-10*max|E_i|; G abs 1e-11*max(1,|G|)."""
+import json
+import math
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -277,37 +281,112 @@ def test_single_element_radial_only():
     _check_full(model, sysm)
 
 
+# ------------------------------------------------------------------------ full size vs whole-system goldens
+# tests/golden/fullsize_*.json are written by tests/golden/make_fullsize_golden.py from oracle/ + workloads/ alone
+# (every centre of the system through the oracle, sharded over host processes): E_total, per-shard sums of E_i and F,
+# an order-independent hash of every (i, j) neighbour pair per shard, projections of the whole force field, and
+# row / G / E_i / F of >= 64 stratified atoms.
+
+GOLD_DIR = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _golden(cfg, call=0):
+    path = os.path.join(GOLD_DIR, "fullsize_%s%s.json" % (cfg.name, "_call%d" % call if call else ""))
+    assert os.path.exists(path), "missing golden %s (python tests/golden/make_fullsize_golden.py --config k)" % path
+    g = json.load(open(path))
+    assert g["config"] == cfg.name and g["call"] == call
+    return g
+
+
+def _pair_hash(i, j):
+    # the digest of tests/golden/make_fullsize_golden.py: sum over pairs of a 64-bit mix of (i << 32 | j), mod 2^64
+    from workloads import rng
+    key = rng.stream_key(2002_00054, 0x6E6272)
+    c = (i.astype(np.uint64) << np.uint64(32)) | j.astype(np.uint64)
+    with np.errstate(over="ignore"):
+        return int(np.add.reduce(rng.bits(key, c), dtype=np.uint64))
+
+
+def _check_against_golden(g, nnp, n, e_atom, e_total, force, model, types):
+    """Whole-system comparison of one evaluation with a golden file; returns a dict of the measured deviations."""
+    dev = _dev()
+    rep = {}
+    # ---- energies: total (north_star: relative 1e-10) and per shard
+    assert g["n_atoms"] == n
+    rep["dE_rel"] = abs(e_total - g["e_total"]) / abs(g["e_total"])
+    assert rep["dE_rel"] <= E_REL
+    assert abs(g["e_total"]) > 1e-3 * g["e_abs_sum"]                    # no cancellation (reading C16)
+    emax = g["e_atom_max_abs"]
+    bounds = g["shards"]["bounds"]
+    sh_e = np.array([math.fsum(e_atom[bounds[s]:bounds[s + 1]]) for s in range(len(bounds) - 1)])
+    d = np.abs(sh_e - np.array(g["shards"]["e_sum"]))
+    assert np.all(d <= 1e-10 * emax * np.maximum(np.diff(bounds), 1))
+    rep["shard_dE_max"] = float(d.max())
+    # ---- neighbour list of EVERY atom, bit-exact: per-shard pair counts and pair hashes
+    off, idx = nnp.neighbors(n)
+    off = off.cpu().numpy(); idx = idx.cpu().numpy()
+    cnt = np.diff(off)
+    assert int(off[-1]) == g["n_pairs"]
+    assert np.array_equal(np.bincount(cnt), np.array(g["nbr_count_hist"]))
+    for s in range(len(bounds) - 1):
+        lo, hi = bounds[s], bounds[s + 1]
+        assert int(off[hi] - off[lo]) == g["shards"]["n_pairs"][s]
+        owner = np.repeat(np.arange(lo, hi, dtype=np.int64), cnt[lo:hi])
+        assert "%016x" % _pair_hash(owner, idx[off[lo]:off[hi]]) == g["shards"]["nbr_hash"][s], "neighbour rows of shard %d" % s
+    # ---- forces: whole-field projections, per-shard sums, net force (each bound follows from |dF| <= 1e-8 per component)
+    from workloads import rng
+    for k, (ref, l1) in enumerate(zip(g["force_digest"]["values"], g["force_digest"]["q_l1"])):
+        q = rng.normal(rng.stream_key(g["force_digest"]["seed"], 0x646967, k), np.arange(3 * n, dtype=np.uint64)).reshape(n, 3)
+        dd = abs(float(np.sum(force * q)) - ref)
+        assert dd <= F_ABS * l1
+        rep["digest%d_dev_over_bound" % k] = dd / (F_ABS * l1)
+    sh_f = np.array([[math.fsum(force[bounds[s]:bounds[s + 1], c]) for c in range(3)] for s in range(len(bounds) - 1)])
+    d = np.abs(sh_f - np.array(g["shards"]["f_sum"]))
+    assert np.all(d <= F_ABS * np.maximum(np.diff(bounds), 1)[:, None])
+    rep["shard_dF_max"] = float(d.max())
+    assert np.all(np.abs(force.sum(axis=0)) < 1e-7)
+    # ---- stratified atoms: row, G, E_i, F element by element
+    atoms = np.array([a["index"] for a in g["atoms"]])
+    assert len(atoms) >= 64
+    G = nnp.symmetry_functions(n)[torch.tensor(atoms, device=dev)].cpu().numpy()
+    dF = dG = dEa = 0.0
+    for q, a in enumerate(g["atoms"]):
+        m = a["index"]
+        assert np.array_equal(idx[off[m]:off[m + 1]], np.array(a["row"], dtype=idx.dtype)), a["why"]
+        ref_g = np.array(a["G"])
+        assert ref_g.shape[0] == model.n_sf_per_elem[int(types[m])]
+        gg = G[q, :ref_g.shape[0]]
+        assert np.all(np.abs(gg - ref_g) <= 1e-11 * np.maximum(1.0, np.abs(ref_g))), a["why"]
+        assert abs(e_atom[m] - a["e_atom"]) <= 1e-10 * emax, a["why"]
+        assert np.abs(force[m] - np.array(a["F"])).max() <= F_ABS, a["why"]
+        dF = max(dF, float(np.abs(force[m] - np.array(a["F"])).max()))
+        dG = max(dG, float(np.abs(gg - ref_g).max()))
+        dEa = max(dEa, abs(e_atom[m] - a["e_atom"]))
+    rep.update(stratified_atoms=len(atoms), dF_max=dF, dG_max=dG, dEatom_max=dEa)
+    return rep, off, idx
+
+
 @pytest.mark.parametrize("k", [1, 2, 3, 4])
-def test_full_size_configs_sampled(k):
-    """configs[1..4] at full size, in the launch configuration bench.py times: sampled outputs the
-    oracle can compute one by one (neighbour rows, G_i, E_i, F_m) + properties that hold at any size."""
+def test_full_size_configs_vs_golden(k):
+    """configs[1..4] at full size, in the launch configuration bench.py times, against the whole-system oracle
+    results: total energy at relative 1e-10, the neighbour list of every atom (hashes), projections and shard sums of
+    the whole force field, and >= 64 stratified atoms element by element."""
     from paper_2002_00054_b200 import NNP
     cfg = W.CONFIGS[k]
     sysm, model = W.build(cfg)
+    g = _golden(cfg)
     nnp = NNP.from_model(model)
     n = sysm.n_atoms
     e_atom, e_total, force = _run(nnp, sysm.pos, sysm.types, sysm.box)
-    n_samples = {1: 12, 2: 8, 3: 5, 4: 4}[k]
-    rs = np.random.RandomState(1000 + k)
-    samples = np.sort(rs.choice(n, n_samples, replace=False))
-    om = oracle.OracleModel(model)
-    ref = oracle.forces_on(om, sysm.pos, sysm.types, sysm.box, samples)
-    off, idx = nnp.neighbors(n)
-    off = off.cpu().numpy(); idx = idx.cpu().numpy()
-    G = nnp.symmetry_functions(n)[torch.tensor(samples, device=_dev())].cpu().numpy()
-    emax = np.abs(e_atom).max()
-    for q, m in enumerate(samples):
-        assert np.array_equal(idx[off[m]:off[m + 1]], ref.rows[q])          # bit-exact neighbour set
-        assert np.all(np.abs(G[q] - ref.G[q]) <= 1e-11 * np.maximum(1.0, np.abs(ref.G[q])))
-        assert abs(e_atom[m] - ref.e_atom[q]) <= 1e-10 * emax
-        assert np.abs(force[m] - ref.F[q]).max() <= F_ABS
+    rep, off, idx = _check_against_golden(g, nnp, n, e_atom, e_total, force, model, sysm.types)
+    print("full-size parity %s: %s" % (cfg.name, json.dumps(rep)))
     # properties at full size
     assert abs(e_total - e_atom.sum()) <= 1e-11 * np.abs(e_atom).sum()
-    assert np.all(np.abs(force.sum(axis=0)) < 1e-7)
     cnt = np.diff(off)
     assert 85 < cnt.mean() < 97 and cnt.max() < 160
     # neighbour symmetry j in N(i) <=> i in N(j) on a sample of rows
-    for m in samples[:3]:
+    for a in g["atoms"][:3]:
+        m = a["index"]
         for j in idx[off[m]:off[m + 1]][:10]:
             assert m in idx[off[j]:off[j + 1]]
     # repeatability at full size (a shared-memory race in the lane-owned kernels would show up as a run-to-run
@@ -320,7 +399,8 @@ def test_full_size_configs_sampled(k):
 
 def test_config1_displacement_sequence():
     """configs[1]: repeated evaluations with cumulative sigma = 0.01 A kicks (reading C15); positions
-    drift out of the box and are re-wrapped by the library.  Parity at calls 0, 1, 50, 99 (sampled)."""
+    drift out of the box and are re-wrapped by the library.  Parity at calls 0, 1, 50 (three atoms through
+    oracle.forces_on) and at call 99 against the whole-system golden of that call."""
     from paper_2002_00054_b200 import NNP
     cfg = W.CONFIGS[1]
     sysm, model = W.build(cfg)
@@ -331,7 +411,7 @@ def test_config1_displacement_sequence():
     for call in range(100):
         if call >= 1:
             pos = pos + W.displacement(sysm.n_atoms, cfg.seed_disp, call)
-        if call in (0, 1, 50, 99):
+        if call in (0, 1, 50):
             e_atom, e_total, force = _run(nnp, pos, sysm.types, sysm.box)
             ref = oracle.forces_on(om, pos, sysm.types, sysm.box, samples)
             off, idx = nnp.neighbors(sysm.n_atoms)
@@ -340,6 +420,11 @@ def test_config1_displacement_sequence():
                 assert np.array_equal(idx[off[m]:off[m + 1]], ref.rows[q])
                 assert abs(e_atom[m] - ref.e_atom[q]) <= 1e-10 * np.abs(e_atom).max()
                 assert np.abs(force[m] - ref.F[q]).max() <= F_ABS
+        elif call < 99:
+            _run(nnp, pos, sysm.types, sysm.box)        # the library sees every call of the sequence
+    e_atom, e_total, force = _run(nnp, pos, sysm.types, sysm.box)
+    rep, _, _ = _check_against_golden(_golden(cfg, 99), nnp, sysm.n_atoms, e_atom, e_total, force, model, sysm.types)
+    print("configs[1] call 99: %s" % json.dumps(rep))
     nnp.close()
 
 
