@@ -8,9 +8,11 @@ call) over one synthetic water-like system.  Default workload = BASELINE.json co
 one GPU.  N > 1 (torchrun): the path does not shard in this build ("replicas only", DESIGN.md
 section 8(e)) -> every rank evaluates the same system on its own GPU, value = N * atoms * K / max time.
 
-One JSON line on stdout (rank 0).  Extra keys: roofline (dominant kernel k_force2, FP64-ALU bound),
-cpu_baseline (the oracle on a bounded sample of centres of the same system), e2e (host buffers
-through nnp_compute_host), clocks, gpu_launches, stage_ms.
+One JSON line on stdout (rank 0).  Extra keys: roofline (dominant kernel k_force2, FP64-ALU bound; `frac` on the
+frozen count of roofline_counts.json, `frac_survey_estimate` on SURVEY.md's paper estimate, `fp64_pipe_pct` /
+`traffic` parsed from the newest committed ncu launch list), cpu_baseline (the oracle on a bounded sample of
+centres of the same system), e2e (host buffers through nnp_compute_host), clocks, gpu_launches, stage_ms,
+config_sweep (short timed runs of configs[1], [2], [4]).
 """
 from __future__ import annotations
 
@@ -31,19 +33,54 @@ import numpy as np  # noqa: E402
 METRIC = "nnp_energy_force_atom_steps_per_sec"
 UNIT = "atom-steps/s"
 
-# Algorithmic FP64-pipe thread-instructions per atom-step (
-# SURVEY.md 8(d)): minimal per-centre evaluation, water-like workload statistics
-# (91 neighbours, 4,141 enumerated (j,k), 1,941 contributing triplets per atom).
-FP64_INSTR_PER_ATOM = {
-    False: {"sf": 230e3, "mlp": 7e3, "force": 400e3},     # base-52 model
-    True: {"sf": 368e3, "mlp": 33e3, "force": 586e3},      # wide-128 model
-    # Ni-like metal (not a BASELINE.json config): 18 neighbours, 153 enumerated (j,k), 60 contributing
-    # triplets per atom, same per-unit costs: SF 18*230 + 153*7 + 60*93, force 18*264 + 153*7 + 60*179, MLP 20-30-30-1
-    "metal": {"sf": 10.8e3, "mlp": 3.3e3, "force": 16.6e3},
-}
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_force2 launch, from the ncu captures under profiles/
-# (r1f_launches_config3.csv for configs[3], r1b_ncu_k_sf2_k_force2.md for configs[2]); null where not captured
-NCU_DRAM_BYTES_K_FORCE2 = {3: 3617708288 + 103256064, 2: 338736896 + 9724160}
+# Algorithmic FP64-pipe thread-instructions per atom-step: roofline_counts.json, written by roofline_counts.py
+# (operation lists of the minimal per-centre evaluation scheme x statistics measured on the seeded systems;
+# DESIGN.md "Roofline denominators").  SURVEY.md 8(d)'s paper estimate (+-15 %) is reported beside it.
+def _roofline_counts():
+    with open(os.path.join(ROOT, "roofline_counts.json")) as fh:
+        return json.load(fh)
+
+
+def _ncu_launch_metrics(cfg_index: int, kernel: str):
+    """Per-launch ncu metrics of `kernel` from the newest committed launch list of this config
+    (profiles/*launches_config<k>.csv, written by the ncu command its .md names): DRAM bytes and, when the
+    list carries them, FP64-pipe utilisation and executed FP64 warp-instructions.  -> (dict, source) or (None, why)."""
+    import csv
+    import glob
+    files = sorted(glob.glob(os.path.join(ROOT, "profiles", "*launches_config%d.csv" % cfg_index)))
+    if not files:
+        return None, "no profiles/*launches_config%d.csv committed" % cfg_index
+    path = files[-1]
+    per = {}
+    with open(path, newline="") as fh:
+        rows = [r for r in csv.reader(l for l in fh if l.startswith('"'))]
+    if not rows:
+        return None, "no rows in " + os.path.basename(path)
+    head = rows[0]
+    try:
+        ik, im, iv, iid = head.index("Kernel Name"), head.index("Metric Name"), head.index("Metric Value"), head.index("ID")
+    except ValueError:
+        return None, "unexpected header in " + os.path.basename(path)
+    for r in rows[1:]:
+        if len(r) <= iv or kernel not in r[ik]:
+            continue
+        try:
+            per.setdefault(r[im], {})[r[iid]] = float(r[iv].replace(",", ""))
+        except ValueError:
+            pass
+    if "dram__bytes_read.sum" not in per:
+        return None, "no %s launch with DRAM metrics in %s" % (kernel, os.path.basename(path))
+    mean = {k: sum(v.values()) / len(v) for k, v in per.items()}
+    out = {"dram_bytes": mean["dram__bytes_read.sum"] + mean.get("dram__bytes_write.sum", 0.0),
+           "launches_averaged": len(per["dram__bytes_read.sum"]),
+           "ncu_kernel_ms_cold": mean.get("gpu__time_duration.sum", float("nan")) / 1e6}
+    k = "sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active"
+    out["fp64_pipe_pct"] = mean.get(k)
+    k = "sm__inst_executed_pipe_fp64.sum"
+    out["fp64_warp_instr_executed"] = mean.get(k)
+    return out, "profiles/" + os.path.basename(path)
+
+
 # FP64 pipe peak derived from unit counts and clocks: 148 SMs x 64 DFMA lanes/clk x clocks.max.sm
 FP64_LANES_PER_SM = 64
 N_SM = 148
@@ -145,6 +182,63 @@ def oracle_sample(cfg_index: int, n_centres: int, seed: int = 12345):
     return dt, float(r.timing[0]), 1, int(sel.size)
 
 
+def sweep_config(k: int, local: int, peak_alu: float, counts: dict, steps: int = 5, warmup: int = 3):
+    """Short timed run (CUDA events on the launching stream, device-resident inputs, `warmup` untimed + `steps`
+    timed evaluations) of another BASELINE.json config, so that the driver's record carries every config."""
+    import torch
+
+    import workloads as W
+    from paper_2002_00054_b200 import NNP
+    cfg = W.CONFIGS[k]
+    sysm, model = W.build(cfg)
+    n = sysm.n_atoms
+    dev = torch.device("cuda", local)
+    nnp = NNP.from_model(model, device=local)
+    pos = torch.tensor(sysm.pos, dtype=torch.float64, device=dev)
+    typ = torch.tensor(sysm.types, dtype=torch.int32, device=dev)
+    out = (torch.empty(n, dtype=torch.float64, device=dev), torch.empty(1, dtype=torch.float64, device=dev),
+           torch.empty((n, 3), dtype=torch.float64, device=dev))
+    disp = None
+    if cfg.seed_disp is not None:
+        disp = [torch.tensor(W.displacement(n, cfg.seed_disp, c + 1), device=dev) for c in range(4)]
+
+    def step(i):
+        if disp is not None:
+            pos.add_(disp[i % len(disp)])
+        nnp.compute(pos, typ, sysm.box, out=out, sync=False)
+
+    for i in range(warmup):
+        step(i)
+    nnp.sync_status()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for i in range(steps):
+        step(i)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    nnp.sync_status()
+    nnp.set_timing(True)
+    stage = np.zeros(6)
+    for i in range(steps):
+        step(i)
+        tm = nnp.timings_ms()
+        stage += np.array([tm[q] for q in ("sort", "neighbors", "symmetry_functions", "networks", "forces", "finalize")])
+    stage /= steps
+    nnp.set_timing(False)
+    ws = nnp.workspace_bytes(n)
+    nnp.close()
+    instr = counts["configs"][cfg.name]["per_atom"]
+    return {"config_index": k, "workload": cfg.name, "n_atoms": n, "model": model.name, "steps": steps, "warmup": warmup,
+            "value": n / (ms * 1e-3), "unit": UNIT, "ms_per_step": ms,
+            "stage_ms": {"neighbors": float(stage[1]), "symmetry_functions": float(stage[2]), "networks": float(stage[3]),
+                         "forces": float(stage[4])},
+            "roofline_frac_whole_step": instr["total"] * n / (ms * 1e-3) / peak_alu,
+            "roofline_frac_k_force2": instr["force"] * n / (float(stage[4]) * 1e-3) / peak_alu,
+            "l2": "workspace %.0f MB %s the 126 MB L2" % (ws / 1e6, "exceeds" if ws > 126e6 else "fits in")}
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores, each step a bounded sample of the workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -209,6 +303,10 @@ def main():
                          "(0.01 -> 0.0123: lane-owned kernels with per-eta exponentials), 'generic' also replaces zeta 16 by 3 "
                          "(queue-based generic kernels); the roofline object is then not meaningful")
     ap.add_argument("--no-probe", action="store_true", help="skip the DFMA issue-rate probe (for ncu runs)")
+    ap.add_argument("--no-sweep", action="store_true",
+                    help="skip the short timed runs of configs[1], [2], [4] that the default line carries as config_sweep")
+    ap.add_argument("--precision", default="f64", choices=["f64"],
+                    help="arithmetic mode of the hot kernels (headline: f64)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -338,30 +436,58 @@ def main():
     peaks = _peaks()
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
     peak_alu = N_SM * FP64_LANES_PER_SM * sm_max * 1e6
-    instr = FP64_INSTR_PER_ATOM["metal" if cfg.kind == "metal" else cfg.wide]
+    counts = _roofline_counts()
+    instr = counts["configs"][cfg.name]["per_atom"]
+    survey = counts["survey_estimate_per_atom"].get(counts["configs"][cfg.name]["model"])
     force_ms = float(stage_ms[4])
+    step_s = ms / args.steps * 1e-3
     achieved = instr["force"] * n / (force_ms * 1e-3)
-    total_instr = sum(instr.values()) * n
+    total_instr = instr["total"] * n
     hbm_bytes_per_atom = 1.0e3 if cfg.kind == "metal" else (2.8e3 if not cfg.wide else 5.2e3)
+    ncu, ncu_src = _ncu_launch_metrics(args.config, "k_force2")
+    baseline_table = args.table == "baseline" and args.precision == "f64"
     roofline = {
         "bound": "alu", "kernel": "k_force2", "achieved": achieved / 1e12, "peak": peak_alu / 1e12,
-        "unit": "T FP64 instr/s", "frac": achieved / peak_alu, "traffic": NCU_DRAM_BYTES_K_FORCE2.get(args.config),
+        "unit": "T FP64 instr/s", "frac": achieved / peak_alu,
+        "frac_is": "algorithmic-model fraction: frozen FP64 instruction count of the minimal per-centre scheme "
+                   "(roofline_counts.json) / kernel time / derived pipe peak; the hardware pipe utilisation is fp64_pipe_pct",
+        "frac_survey_estimate": (survey["force"] * n / (force_ms * 1e-3) / peak_alu) if survey else None,
+        "traffic": ncu["dram_bytes"] if ncu else None,
+        "traffic_source": ncu_src,
+        "traffic_algorithmic": (n * (8 * nnp.g_stride + 4 * 91 + 28 + 24)) if cfg.kind != "metal" else None,
+        "fp64_pipe_pct": ncu["fp64_pipe_pct"] if ncu else None,
+        "fp64_thread_instr_executed_per_atom": (ncu["fp64_warp_instr_executed"] * 32 / n
+                                                if ncu and ncu["fp64_warp_instr_executed"] else None),
         "peak_source": "derived: 148 SMs x 64 FP64 lanes x %.0f MHz (clocks.max.sm); DFMA probe in this run: "
                        "burst %.2f, sustained %.2f T instr/s" % (sm_max, dfma_burst / 1e12, dfma_sust / 1e12),
         "frac_of_measured_dfma": achieved / dfma_burst,
         "algorithmic_instr_per_launch": instr["force"] * n,
         "kernel_ms": force_ms,
-        "whole_step": {"fp64_instr": total_instr, "frac": total_instr / (ms / args.steps * 1e-3) / peak_alu,
+        "stages": {"sf": {"instr_per_atom": instr["sf"], "ms": float(stage_ms[2]),
+                          "frac": instr["sf"] * n / (float(stage_ms[2]) * 1e-3) / peak_alu},
+                   "mlp": {"instr_per_atom": instr["mlp"], "ms": float(stage_ms[3]),
+                           "frac": instr["mlp"] * n / (float(stage_ms[3]) * 1e-3) / peak_alu},
+                   "force": {"instr_per_atom": instr["force"], "ms": force_ms, "frac": achieved / peak_alu}},
+        "whole_step": {"fp64_instr": total_instr, "frac": total_instr / step_s / peak_alu,
+                       "frac_survey_estimate": (sum(survey.values()) * n / step_s / peak_alu) if survey else None,
                        "hbm_bytes": hbm_bytes_per_atom * n,
-                       "hbm_frac": hbm_bytes_per_atom * n / (ms / args.steps * 1e-3) / (peaks.get("hbm_gbs", 6650.0) * 1e9)},
+                       "hbm_frac": hbm_bytes_per_atom * n / step_s / (peaks.get("hbm_gbs", 6650.0) * 1e9)},
     }
+    if not baseline_table:
+        roofline["note"] = "probe table / precision mode: the frozen count is the base table's, fractions are indicative only"
+
+    sweep = None
+    if world == 1 and args.config == 3 and baseline_table and not args.md and not args.no_sweep:
+        sweep = [sweep_config(k, local, peak_alu, counts) for k in (1, 2, 4)]
 
     cpu = None
     if args.cpu_centres > 0:
         dt, t_nbr, cores, ns = oracle_sample(args.config, args.cpu_centres)
         cpu = {"value": ns / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "value_without_neighbour_scan": ns / max(dt - t_nbr, 1e-9),
                "sample": "%d randomly chosen centres of %s, each: O(N) brute-force neighbour scan + SFs + MLP + "
-                         "force contributions; %.1f s total, %.1f s of it in the neighbour scan" % (ns, cfg.name, dt, t_nbr)}
+                         "force contributions; %.1f s total, %.1f s of it in the O(N^2)-style neighbour scan no production "
+                         "CPU code would use (value_without_neighbour_scan leaves it out)" % (ns, cfg.name, dt, t_nbr)}
 
     line = {
         "metric": METRIC, "value": job_value(n, args.steps, world, ms), "unit": UNIT, "n_gpus": world,
@@ -375,6 +501,7 @@ def main():
         "stage_ms": dict(zip(("sort", "neighbors", "symmetry_functions", "networks", "forces", "finalize"),
                              [float(x) for x in stage_ms])),
         "stage_ms_last_timed_step": t_last,
+        "config_sweep": sweep,
     }
     print(json.dumps(line), flush=True)
     if world > 1:
