@@ -87,15 +87,16 @@ def test_md_argument_errors():
 
 
 def _imploding_shell():
-    """One centre atom and 33 atoms on a sphere of radius 8 A around it, flying inwards at 1 A/fs: with
-    max_neighbors = 32 the start (radius 8) and the end (radius 8 on the far side, 16 steps of 1 fs later) are
-    fine, the steps in between overflow (33 neighbours of the centre at radius < 6, all 33 mutual below ~3)."""
+    """One centre atom and 33 atoms on a sphere of radius 8.5 A around it, flying inwards at 1 A/fs: with
+    max_neighbors = 32 the start (radius 8.5) and the end (radius 7.5 on the far side, 16 fs later) are fine, the
+    steps in between overflow (33 neighbours of the centre at radius < 6, all 33 mutual below ~3).  The shell
+    passes the centre between two steps (radius 0.5 -> -0.5), so no two atoms ever coincide."""
     k = np.arange(33) + 0.5
     phi = np.arccos(1.0 - 2.0 * k / 33.0)
     th = np.pi * (1.0 + 5.0 ** 0.5) * k
     unit = np.stack([np.cos(th) * np.sin(phi), np.sin(th) * np.sin(phi), np.cos(phi)], axis=1)
     c = np.array([20.0, 20.0, 20.0])
-    pos = np.concatenate([[c], c + 8.0 * unit])
+    pos = np.concatenate([[c], c + 8.5 * unit])
     vel = np.concatenate([[np.zeros(3)], -1.0 * unit])
     types = np.zeros(34, dtype=np.int32)
     return pos, vel, types, np.array([40.0, 40.0, 40.0])
@@ -115,12 +116,12 @@ def test_md_run_reports_an_error_of_a_middle_step(n_steps):
     vel_d = torch.tensor(vel, dtype=torch.float64, device=dev)
     typ_d = torch.tensor(types, dtype=torch.int32, device=dev)
     heavy = (1.0e6,)                                   # ballistic: the forces do not deflect anything
-    state = nnp.compute(pos_d, typ_d, box)             # radius 8: fine
-    with pytest.raises(NNPError) as ei:                # 16 steps of 1 fs, or 3 steps of 16/3 fs (radius 8, 2.67, -2.67, -8)
+    state = nnp.compute(pos_d, typ_d, box)             # radius 8.5: fine
+    with pytest.raises(NNPError) as ei:                # 16 steps of 1 fs, or 3 steps of 16/3 fs (radius 8.5, 3.17, -2.17, -7.5)
         nnp.md_run(n_steps, 16.0 / n_steps, heavy, pos_d, vel_d, typ_d, box, state)
     assert ei.value.status == 4                        # NNP_ERR_NEIGHBOR_OVERFLOW, from a middle step
     r = np.linalg.norm(pos_d.cpu().numpy()[1:] - pos[0], axis=1)
-    assert np.all(np.abs(r - 8.0) < 1e-3)              # the LAST step is fine again
+    assert np.all(np.abs(r - 7.5) < 1e-3)              # the LAST step is fine again
     nnp.compute(pos_d, typ_d, box)                     # ... and reading cleared the sticky word
     nnp.close()
 

@@ -274,6 +274,31 @@ def test_sf_cutoff_argument_errors():
     nnp.close()
 
 
+def test_n2p2_model_round_trip(tmp_path):
+    # a model written as n2p2 files (fixture writer of tests/test_n2p2_reader.py), read back by
+    # paper_2002_00054_b200.n2p2.read_model (SFs re-sorted, scaling / atom_energy / normalisation folded) and run on
+    # the GPU: parity with the oracle on the read model, and the energy of the original model plus the offsets
+    import copy
+    from test_n2p2_reader import write_model
+    from paper_2002_00054_b200 import NNP, n2p2
+    model = copy.deepcopy(W.make_model(False))
+    rs = np.random.RandomState(3)
+    model.sf_scaling = [(rs.uniform(0.0, 0.5, n), rs.uniform(0.2, 3.0, n)) for n in model.n_sf_per_elem]
+    model.activation = "tanh"
+    offs = {"H": -0.4581, "O": -2.0413}
+    write_model(str(tmp_path), model, scaling_mode="scalecenter", smin=-0.5, smax=1.5, atom_energy=offs,
+                order=lambda n: list(np.random.RandomState(1).permutation(n)))
+    got = n2p2.read_model(str(tmp_path))
+    sysm = W.make_water(150, 31, L=15.3)
+    ref_read = _check_full(got, sysm)
+    ref = oracle.compute(oracle.OracleModel(model), sysm.pos, sysm.types, sysm.box)
+    e_off = sum(offs[model.elements[t]] for t in sysm.types)
+    assert abs(ref_read.e_total - (ref.e_total + e_off)) <= 1e-11 * abs(ref.e_total + e_off)
+    nnp = NNP.from_model(got)
+    assert nnp.uses_fast_path()                       # the re-sorted base-52 table still matches the base-12 shape
+    nnp.close()
+
+
 def test_single_element_radial_only():
     model = tiny_model([(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0), (0, 2, 0, 0, 0.4, 2.0, 0.0, 0.0)], hidden=(4,))
     sysm = W.make_water(60, 3, L=12.4)
@@ -475,6 +500,9 @@ def test_error_codes():
         nnp.compute(badp, typ, sysm.box)
     assert ei.value.status == 7                       # NNP_ERR_NONFINITE
     # neighbour overflow: 150 atoms in 13^3 have ~60 neighbours each; allow only 32
+    with pytest.raises(NNPError) as ei:
+        nnp.set_max_neighbors(256)
+    assert ei.value.status == 8                       # NNP_ERR_LIMIT (slots are addressed with 8 bits)
     nnp.set_max_neighbors(32)
     with pytest.raises(NNPError) as ei:
         nnp.compute(pos, typ, sysm.box)
