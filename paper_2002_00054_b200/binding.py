@@ -10,7 +10,8 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libnnp_b200.so")
+# the in-tree build; NNP_B200_LIBRARY points at another build of the same sources (kernel-variant comparisons)
+LIB_PATH = os.environ.get("NNP_B200_LIBRARY") or os.path.join(HERE, "libnnp_b200.so")
 
 NNP_OK = 0
 STATUS_NAMES = {0: "NNP_OK", 1: "NNP_ERR_INVALID_ARG", 2: "NNP_ERR_BOX_TOO_SMALL", 3: "NNP_ERR_TYPE_RANGE",

@@ -28,12 +28,14 @@ namespace nnp {
 struct Force2Params {
     int64_t n;
     int n_elem, ncell, stride, cap, g_stride;
+    int nt_lo, nt_hi;                    // this launch owns the centres with nt_lo <= neighbours <= nt_hi (slot-capacity split)
     double rc, rc2, k2;                  // k2 = (pi / (2 rc))^2
     double box[3], half[3];
     const double *sx, *sy, *sz;
     const int32_t *cell_start, *nbr, *nbr_cnt;
     const double* dEdG;
     double* f_sorted;
+    const int32_t *big_list, *big_count; // centres with more than 128 neighbours (k_count_words)
     const int64_t* word_off;             // masks from the SF kernel (see Workspace::gmask)
     const uint32_t* gmask;
     int64_t gmask_cap;
@@ -98,16 +100,17 @@ struct JData {
     double ux, uy, uz, ia, fa, dfa, e0;
 };
 
+#ifndef F2_MINB_128
+#define F2_MINB_128 20       // warps per SM asked of the 128-slot instantiation: 10 CTAs of 2 warps (96 registers, 21.7 KB each)
+#endif
 #ifndef F2_MINB1
 #define F2_MINB1 20          // resident CTAs per SM asked of the one-warp-per-centre instantiation (metals: 5.2 vs 5.65 ms at 14)
 #endif
 template <class Spec, int WPC, int CAPA, bool TINY>
-__global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_force2(const __grid_constant__ Force2Params p) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
+__device__ __forceinline__ void force2_centre(const Force2Params& p, const int64_t i, unsigned char* smem_raw) {
     constexpr int NT = WPC * 32;
     constexpr bool REGC = Spec::NACC <= 12;          // coefficients of the current group in registers
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int64_t i = blockIdx.x;
     int tc = 0;
     for (int e = 1; e < p.n_elem; ++e)
         if (i >= p.cell_start[(size_t)e * p.ncell]) tc = e;
@@ -139,6 +142,7 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_fo
 #pragma unroll
     for (int e = 0; e < MAX_ELEM; ++e) seg[e + 1] = seg[e] + p.nbr_cnt[(size_t)i * MAX_ELEM + e];
     const int ntot = seg[MAX_ELEM];
+    if (ntot < p.nt_lo || ntot > p.nt_hi) return;   // uniform per CTA: another slot-capacity instantiation owns this centre
 
     for (int s = tid; s < p.g_stride; s += NT) brow[s] = p.dEdG[(size_t)i * p.g_stride + s];
     // The SF kernel has screened this centre already (Workspace::gmask): fetch its mask words now, so that
@@ -425,13 +429,32 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : 14 / WPC) k_fo
     }
 }
 
+// one CTA per centre: blockIdx.x = sorted position of the centre
+template <class Spec, int WPC, int CAPA, bool TINY>
+__global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : (CAPA <= 128 ? F2_MINB_128 : 14) / WPC) k_force2(const __grid_constant__ Force2Params p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    force2_centre<Spec, WPC, CAPA, TINY>(p, (int64_t)blockIdx.x, smem_raw);
+}
+
+// the centres of a list (Workspace::big_list: those with more than 128 neighbours), a few CTAs walking it
+template <class Spec, int WPC, int CAPA, bool TINY>
+__global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2_list(const __grid_constant__ Force2Params p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int n_list = *p.big_count;
+    for (int q = blockIdx.x; q < n_list; q += gridDim.x) {
+        force2_centre<Spec, WPC, CAPA, TINY>(p, (int64_t)p.big_list[q], smem_raw);
+        __syncthreads();                             // the next centre reuses the shared memory
+    }
+}
+
 #ifndef NNP_F2_WPC
 #define NNP_F2_WPC 2
 #endif
 constexpr int F2_WPC = NNP_F2_WPC;
 
 template <class Spec, int CAPA, bool TINY, int WPC = F2_WPC>
-static int launch_capa(const Force2Params& p, cudaStream_t st) {
+static int launch_capa(Force2Params p, int nt_lo, int nt_hi, cudaStream_t st) {
+    p.nt_lo = nt_lo; p.nt_hi = nt_hi;
     const size_t smem = force2_smem<Spec>(CAPA, p.g_stride, p.n_elem, WPC);
     static unsigned long long configured = 0ull;      // per device (opt_in_smem)
     opt_in_smem(k_force2<Spec, WPC, CAPA, TINY>, &configured);
@@ -439,14 +462,30 @@ static int launch_capa(const Force2Params& p, cudaStream_t st) {
     return 1;
 }
 
+template <class Spec, int CAPA, bool TINY, int WPC = F2_WPC>
+static int launch_capa_list(Force2Params p, int nt_lo, int nt_hi, cudaStream_t st) {
+    p.nt_lo = nt_lo; p.nt_hi = nt_hi;
+    const size_t smem = force2_smem<Spec>(CAPA, p.g_stride, p.n_elem, WPC);
+    static unsigned long long configured = 0ull;
+    opt_in_smem(k_force2_list<Spec, WPC, CAPA, TINY>, &configured);
+    const unsigned grid = (unsigned)(p.n < 148 * 8 ? p.n : 148 * 8);
+    k_force2_list<Spec, WPC, CAPA, TINY><<<grid, WPC * 32, smem, st>>>(p);
+    return 1;
+}
+
 // slot capacity = smallest instantiated CAPA that holds max_neighbors (nnp_set_max_neighbors: 32..255)
 template <class Spec, bool TINY>
 static int launch_one2(const Force2Params& p, cudaStream_t st) {
     // small neighbourhoods (metals: ~20 neighbours, ~60 triplets per centre): 64 slots, ONE warp per centre
-    if (p.cap <= 64) return launch_capa<Spec, 64, TINY, 1>(p, st);
-    if (p.cap <= 128) return launch_capa<Spec, 128, TINY>(p, st);
-    if (p.cap <= 160) return launch_capa<Spec, 160, TINY>(p, st);
-    return launch_capa<Spec, 256, TINY>(p, st);
+    if (p.cap <= 64) return launch_capa<Spec, 64, TINY, 1>(p, 0, 64, st);
+    // The 128-slot instantiation keeps 10 CTAs per SM resident (21.7 KB, 96 registers) against 8 of the 160-slot one
+    // (27.5 KB, 119 registers): every centre with at most 128 neighbours runs on it (measured on configs[3]: 79.4 ->
+    // 76.8 ms), the few others (water-like systems: 1 centre in ~10^4; listed by k_count_words) on a list-driven launch
+    // of the bigger instantiation -- a second launch over all N centres costs 1.3 ms in CTAs that return at once.
+    int launches = launch_capa<Spec, 128, TINY>(p, 0, 128, st);
+    if (p.cap > 128) launches += p.cap <= 160 ? launch_capa_list<Spec, 160, TINY>(p, 129, 160, st)
+                                              : launch_capa_list<Spec, 256, TINY>(p, 129, 255, st);
+    return launches;
 }
 
 // launches the fast kernels for the specialised variants in use; the caller has zeroed f_sorted
@@ -461,6 +500,7 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.dEdG = w.dEdG; p.f_sorted = w.f_sorted;
     p.word_off = w.word_off; p.gmask = w.gmask; p.gmask_cap = w.gmask_cap;
+    p.big_list = w.big_list; p.big_count = w.status + 2;
     bool use[ANG_NVARIANT][2] = {};                                       // [variant][tiny_exp]
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;

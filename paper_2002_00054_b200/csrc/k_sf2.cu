@@ -254,7 +254,7 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
 __global__ void __launch_bounds__(256)
 k_count_words(int64_t n, int n_elem, int ncell, const int32_t* __restrict__ cell_start,
               const int32_t* __restrict__ nbr_cnt, const ElemProgram* p0, const ElemProgram* p1, const ElemProgram* p2,
-              const ElemProgram* p3, int32_t* __restrict__ nw) {
+              const ElemProgram* p3, int32_t* __restrict__ nw, int32_t* __restrict__ big_list, int32_t* __restrict__ big_count) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     int tc = 0;
@@ -266,6 +266,8 @@ k_count_words(int64_t n, int n_elem, int ncell, const int32_t* __restrict__ cell
 #pragma unroll
     for (int e = 0; e < MAX_ELEM; ++e) seg[e + 1] = seg[e] + nbr_cnt[(size_t)i * MAX_ELEM + e];
     nw[i] = count_words(seg, n_elem, prog->n_ang);
+    // centres that do not fit the 128-slot force kernel (k_force2.cu launch_one2); any order
+    if (seg[MAX_ELEM] > 128) big_list[atomicAdd(big_count, 1)] = (int32_t)i;
 }
 
 int launch_word_offsets(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
@@ -274,7 +276,7 @@ int launch_word_offsets(const Workspace& w, const Grid& g, int64_t n, int n_elem
     const ElemProgram* pr[MAX_ELEM];
     for (int e = 0; e < MAX_ELEM; ++e) pr[e] = e < n_elem ? d_prog[e] : nullptr;
     k_count_words<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(n, n_elem, g.ncell, w.cell_start, w.nbr_cnt, pr[0], pr[1],
-                                                                pr[2], pr[3], w.nw);
+                                                                pr[2], pr[3], w.nw, w.big_list, w.status + 2);
     return 1 + launch_scan_i64_from_i32(w.nw, n, w.word_off, w.word_tmp, st);
 }
 

@@ -111,6 +111,7 @@ static size_t ws_layout(Workspace* w, void* base, int64_t n, int n_elem, int str
     w->dEdG = (double*)take(N * (size_t)g_stride * 8);
     w->e_sorted = (double*)take(N * 8);
     w->f_sorted = (double*)take(N * 3 * 8);
+    w->big_list = (int32_t*)take(N * 4);
     w->nw = (int32_t*)take(N * 4);
     w->word_off = (int64_t*)take((N + 1) * 8);
     w->word_tmp = (int64_t*)take(((N + 1) / 4096 + 2 * 4096 + 16) * 8);

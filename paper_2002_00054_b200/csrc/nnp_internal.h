@@ -119,13 +119,14 @@ struct Workspace {
     // masks handed from the symmetry-function kernel to the force kernel (fast paths): the SF kernel
     // screens the (j,k) candidates of every centre anyway; it stores the mask words of centre i in the
     // force kernel's (j-major) order at gmask[word_off[i] ..), if they fit the budget
+    int32_t *big_list;               // [N] sorted positions of the centres with more than 128 neighbours (count: status[2])
     int32_t *nw;                     // [N] mask words of centre i
     int64_t *word_off;               // [N+1] exclusive prefix of nw
     int64_t *word_tmp;               // scan scratch
     uint32_t *gmask;                 // [gmask_cap]
     int64_t gmask_cap;
     double *partial;                 // [n_partial] block sums of the energy
-    int32_t *status;                 // [4]; word 0 = flags of this nnp_compute (cleared by launch_sort)
+    int32_t *status;                 // [4]; word 0 = flags of this nnp_compute, word 2 = length of big_list (all cleared by launch_sort)
     int32_t *sticky;                 // model-owned word: flags of every call since the last nnp_sync_status (set by nnp_compute, not by ws_layout)
     int64_t n_keys_cap;
     int64_t scan_tmp_len;
