@@ -305,8 +305,9 @@ def main():
     ap.add_argument("--no-probe", action="store_true", help="skip the DFMA issue-rate probe (for ncu runs)")
     ap.add_argument("--no-sweep", action="store_true",
                     help="skip the short timed runs of configs[1], [2], [4] that the default line carries as config_sweep")
-    ap.add_argument("--precision", default="f64", choices=["f64"],
-                    help="arithmetic mode of the hot kernels (headline: f64)")
+    ap.add_argument("--precision", default="f64", choices=["f64", "mixed"],
+                    help="arithmetic mode of the hot kernels: f64 (headline) or the opt-in mixed mode of nnp_set_precision "
+                         "(FP32 staging and per-triplet arithmetic, FP64 accumulation; not a BASELINE.json result)")
     args = ap.parse_args()
     if args.warmup < 3:
         args.warmup = 3
@@ -340,6 +341,8 @@ def main():
         model.name += "+" + args.table
     n = sysm.n_atoms
     nnp = NNP.from_model(model, device=local)
+    if args.precision != "f64":
+        nnp.set_precision(args.precision)
     if cfg.kind == "metal":
         nnp.set_max_neighbors(48)      # 18 neighbours per atom: the 64-slot, one-warp-per-centre kernels
     pos = torch.tensor(sysm.pos, dtype=torch.float64, device=dev)
@@ -492,7 +495,7 @@ def main():
     line = {
         "metric": METRIC, "value": job_value(n, args.steps, world, ms), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
-        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == "f64" else "f32-stage/f64-acc", "data": "synthetic",
         "config": {"workload": cfg.name, "n_atoms": n, "model": model.name, "kernels": list(table_kernels(model)), "box": float(sysm.box[0]),
                    "neighbor_rebuild": "every call", "md": bool(args.md), "parallelism": "replicas x%d" % world,
                    "l2": ("working set per step (%.2f GB workspace) %s the 126 MB L2; no flush between steps"

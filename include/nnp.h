@@ -163,6 +163,18 @@ nnp_status nnp_set_sf_scaling(nnp_model* m, int32_t elem, const double* h_shift,
 nnp_status nnp_set_activation(nnp_model* m, int32_t kind);
 nnp_status nnp_set_sf_cutoffs(nnp_model* m, int32_t n_sf, const double* h_rc);
 
+/* ---- mixed precision (the paper does not state its precision).  OPT-IN, never the default:
+ * NNP_PRECISION_MIXED stages the neighbourhood of a centre in FP32 and evaluates the angular symmetry functions and
+ * their force terms per triplet in FP32 (hardware exponential, degree-5 cutoff polynomials); the neighbour list and
+ * its predicate, the minimum-image geometry, the radial symmetry functions, the networks, the reduction of the
+ * symmetry-function sums over the lanes and every global force / energy accumulation stay FP64.  It applies to elements
+ * whose table has one of BASELINE.json's two angular shapes (NNP_KERNELS_BASE12 / NNP_KERNELS_WIDE32) with
+ * eta_0 rc^2 <= 0.05 and max_neighbors <= 160; every other element silently keeps FP64.  The results no longer meet
+ * BASELINE.json's tolerances (measured on the water-like configs: DESIGN.md section 6c); energies stay bit-reproducible. */
+#define NNP_PRECISION_F64 0
+#define NNP_PRECISION_MIXED 1
+nnp_status nnp_set_precision(nnp_model* m, int32_t mode);
+
 /* ---- MD loop around the path (the implementation is checked by energy
  * conservation in an NVE run).  Velocity Verlet, everything on the device:
  *     v += (dt/2) F/m ;  x += dt v ;  F = nnp_compute(x) ;  v += (dt/2) F/m

@@ -347,7 +347,7 @@ static int launch_one(const ForceParams& p, cudaStream_t st) {
 }
 
 int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                 const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st) {
+                 const int* variant, double rc, int stride, int max_nbr, int g_stride, int precision, cudaStream_t st) {
     if (n == 0) return 0;
     ForceParams p;
     p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride;
@@ -364,7 +364,7 @@ int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const
     cudaMemsetAsync(w.f_sorted, 0, sizeof(double) * 3 * (size_t)n, st);
     int launches = 0;
     if (use[ANG_BASE12] || use[ANG_WIDE32] || use[ANG_FREE32] || use[ANG_FREE16])     // specialised tables: lane-owned design (k_force2.cu)
-        launches += launch_force2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, st);
+        launches += launch_force2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, precision, st);
     if (use[ANG_GENERIC]) launches += launch_one<SpecGeneric>(p, st);
     return launches;
 }

@@ -54,19 +54,29 @@ __host__ __device__ constexpr int bt2_stride() { return Spec::NACC + 1; }   // +
 //   then, at run-time offsets: group table, coefficient tables, scratch, beta row, and the mask words
 //   (mask + descriptor, uint2[mask_words_cap(CAPA, n_elem)])
 template <class Spec>
-__host__ __device__ constexpr size_t force2_smem(int capa, int g_stride, int n_elem, int wpc) {
+__host__ __device__ constexpr size_t force2_smem(int capa, int g_stride, int n_elem, int wpc, size_t real = 8) {
     const size_t npair = (size_t)n_elem * (n_elem + 1) / 2;
-    size_t b = (size_t)capa * (3 * 16 + 2 * 8 + (size_t)wpc * 32);
+    size_t b = (size_t)capa * (3 * 2 * real + 2 * real + (size_t)wpc * 4 * real) + 8;
     b += npair * sizeof(GroupTab);
-    b += npair * bt2_stride<Spec>() * 16;
+    b += npair * bt2_stride<Spec>() * 2 * real;
     b += 64 + (size_t)((g_stride + 1) & ~1) * 8;
     b += (size_t)mask_words_cap(capa, n_elem) * 8;
     return (b + 15) / 16 * 16;
 }
 
+// Arithmetic type of the staged planes, the per-triplet evaluation and the per-slot accumulators: double (the
+// default, BASELINE.json's FP64) or float (nnp_set_precision(NNP_PRECISION_MIXED): FP32 staging and
+// triplet arithmetic, FP64 staging geometry, radial part, networks and global force / energy accumulation).
+template <class R> struct Vec2;
+template <> struct Vec2<double> { using type = double2; };
+template <> struct Vec2<float> { using type = float2; };
+__device__ __forceinline__ double2 mk2(double a, double b) { return make_double2(a, b); }
+__device__ __forceinline__ float2 mk2(float a, float b) { return make_float2(a, b); }
+
+template <class R>
 struct SlotAcc2 {
-    double2* fxy;  // (Fx, Fy)
-    double* fz;    // Fz
+    typename Vec2<R>::type* fxy;  // (Fx, Fy)
+    R* fz;                        // Fz
 };
 
 // rank of the lane among the lanes of its warp that target the same slot (inactive lanes: 0)
@@ -76,11 +86,12 @@ __device__ __forceinline__ int conflict_rank(int slot, bool act, int lane) {
 }
 
 // acc[slot] += (x, y, z) for the lanes with act; lanes that target the same slot take turns
-__device__ __forceinline__ void slot_add(const SlotAcc2& acc, int slot, bool act, int rank, double x, double y, double z) {
+template <class R>
+__device__ __forceinline__ void slot_add(const SlotAcc2<R>& acc, int slot, bool act, int rank, R x, R y, R z) {
     for (int pass = 0; __any_sync(FULL, act && rank >= pass); ++pass) {
         if (act && rank == pass) {
-            double2 p = acc.fxy[slot];
-            double q = acc.fz[slot];
+            typename Vec2<R>::type p = acc.fxy[slot];
+            R q = acc.fz[slot];
             p.x += x; p.y += y; q += z;
             acc.fxy[slot] = p;
             acc.fz[slot] = q;
@@ -94,10 +105,12 @@ __device__ __forceinline__ void slot_add(const SlotAcc2& acc, int slot, bool act
 __device__ __forceinline__ double scale2(double x, int b) {
     return __hiloint2double(__double2hiint(x) + (b << 20), __double2loint(x));
 }
+__device__ __forceinline__ float scale2(float x, int b) { return __int_as_float(__float_as_int(x) + (b << 23)); }
 
 // data of the lane's owner slot j, in registers
+template <class R>
 struct JData {
-    double ux, uy, uz, ia, fa, dfa, e0;
+    R ux, uy, uz, ia, fa, dfa, e0;
 };
 
 #ifndef F2_MINB_128
@@ -106,8 +119,9 @@ struct JData {
 #ifndef F2_MINB1
 #define F2_MINB1 20          // resident CTAs per SM asked of the one-warp-per-centre instantiation (metals: 5.2 vs 5.65 ms at 14)
 #endif
-template <class Spec, int WPC, int CAPA, bool TINY>
+template <class Spec, int WPC, int CAPA, bool TINY, class R>
 __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64_t i, unsigned char* smem_raw) {
+    using R2 = typename Vec2<R>::type;
     constexpr int NT = WPC * 32;
     constexpr bool REGC = Spec::NACC <= 12;          // coefficients of the current group in registers
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
@@ -119,18 +133,18 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
 
     constexpr int capa = CAPA;
     const int npair = p.n_elem * (p.n_elem + 1) / 2;
-    double2* p0 = reinterpret_cast<double2*>(smem_raw);     // (ux, uy)
-    double2* p1 = p0 + capa;                                // (uz, 1/a)
-    double2* p2 = p1 + capa;                                // (fc(a), fc'(a)/a)
-    double2* acc0 = p2 + capa;                              // WPC x (fxy[capa] double2, fz[capa] double, pad)
-    SlotAcc2 acc;
+    R2* p0 = reinterpret_cast<R2*>(smem_raw);               // (ux, uy)
+    R2* p1 = p0 + capa;                                     // (uz, 1/a)
+    R2* p2 = p1 + capa;                                     // (fc(a), fc'(a)/a)
+    R2* acc0 = p2 + capa;                                   // WPC x (fxy[capa] R2, fz[capa] R, pad)
+    SlotAcc2<R> acc;
     acc.fxy = acc0 + (size_t)wid * 2 * capa;
-    acc.fz = reinterpret_cast<double*>(acc.fxy + capa);
-    double* e0 = reinterpret_cast<double*>(acc0 + (size_t)WPC * 2 * capa);   // exp(-eta_0 a^2)
-    double* rad = e0 + capa;                                  // radial scalar R
-    GroupTab* tab = reinterpret_cast<GroupTab*>(rad + capa);
-    double2* bt = reinterpret_cast<double2*>(tab + npair);    // [pair][bt2_stride]: (beta 2^(1-zeta), beta 2^(1-zeta) zeta lambda)
-    double* btc = reinterpret_cast<double*>(bt);              // register-coefficient path: [pair][2 * bt2_stride] doubles, c_b only
+    acc.fz = reinterpret_cast<R*>(acc.fxy + capa);
+    R* e0 = reinterpret_cast<R*>(acc0 + (size_t)WPC * 2 * capa);   // exp(-eta_0 a^2)
+    R* rad = e0 + capa;                                       // radial scalar R
+    GroupTab* tab = reinterpret_cast<GroupTab*>(reinterpret_cast<double*>(rad + capa + (capa & 1)));   // 8-byte aligned for R = float too
+    R2* bt = reinterpret_cast<R2*>(tab + npair);              // [pair][bt2_stride] pairs of c_b = beta_b 2^(1-zeta_b)
+    R* btc = reinterpret_cast<R*>(bt);                        // the same table, entry by entry
     int* wsum = reinterpret_cast<int*>(bt + npair * bt2_stride<Spec>());   // 16 ints of scratch
     double* brow = reinterpret_cast<double*>(wsum + 16);
     uint2* words = reinterpret_cast<uint2*>(brow + ((p.g_stride + 1) & ~1));   // (mask, descriptor)
@@ -177,19 +191,19 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
             cos_sinc(a2 * p.k2, Ca, Sa);
             const double fa = Ca * Ca;                          // fc(a)
             const double dfa_a = (-2.0 * p.k2) * (Ca * Sa);     // fc'(a)/a
-            p0[m] = make_double2(dx, dy);
-            p1[m] = make_double2(dz, ia);
-            p2[m] = make_double2(fa, dfa_a);
-            e0[m] = Spec::FREE_ETA ? a2 : (tiny ? exp_tiny(-eta0 * a2) : exp_small(-eta0 * a2));   // FREE_ETA: a^2 itself
+            p0[m] = mk2((R)dx, (R)dy);
+            p1[m] = mk2((R)dz, (R)ia);
+            p2[m] = mk2((R)fa, (R)dfa_a);
+            e0[m] = (R)(Spec::FREE_ETA ? a2 : (tiny ? exp_tiny(-eta0 * a2) : exp_small(-eta0 * a2)));   // FREE_ETA: a^2 itself
             f32[m] = make_float4((float)dx, (float)dy, (float)dz, 0.f);
-            double R = 0.0;
+            double Rs = 0.0;
             for (int r = 0; r < nr; ++r) {
                 const RadialSF f = prog->rad[off + r];
                 const double d = a - f.rs;
                 const double ex = exp_small(fmax(-f.eta * d * d, -700.0));
-                R = fma(brow[f.g] * ex, fma(-2.0 * f.eta * d, fa * ia, dfa_a), R);
+                Rs = fma(brow[f.g] * ex, fma(-2.0 * f.eta * d, fa * ia, dfa_a), Rs);
             }
-            rad[m] = R;
+            rad[m] = (R)Rs;
         }
     }
     // coefficient tables of all pair groups
@@ -208,7 +222,7 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
                         if (ee < e) a += __popc(mk);
                         else if (ee == e) a += __popc(mk & ((1u << tid) - 1u));
                     }
-                    btc[pr * 2 * bt2_stride<Spec>() + a] = bc;
+                    btc[pr * 2 * bt2_stride<Spec>() + a] = (R)bc;
                     (void)zeta; (void)lam;
                 }
             }
@@ -249,20 +263,21 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
     wk.m = 1u; wk.d = 0u; wk.idx = 0;
     if (wk.cnt > 0) wk.seek(C, NW, tid * quota);
     __syncthreads();
-    for (int m = tid; m < WPC * 2 * capa; m += NT) acc0[m] = make_double2(0.0, 0.0);   // the aliases are dead
+    for (int m = tid; m < WPC * 2 * capa; m += NT) acc0[m] = mk2((R)0, (R)0);   // the aliases are dead
     __syncthreads();
 
     // ---- angular part: every lane walks its range of the stream ---------------------------------------
-    double eta[Spec::NETA];
+    R eta[Spec::NETA];
 #pragma unroll
-    for (int e = 0; e < Spec::NETA; ++e) eta[e] = prog->ang_eta[e];
-    JData J;
-    J.ux = J.uy = J.uz = 1.0; J.ia = 1.0; J.fa = 0.0; J.dfa = 0.0; J.e0 = 1.0;
+    for (int e = 0; e < Spec::NETA; ++e) eta[e] = (R)prog->ang_eta[e];
+    const R eta0r = (R)eta0, k2r = (R)p.k2, rc2r = (R)p.rc2, m2k2 = (R)(-2.0 * p.k2);
+    JData<R> J;
+    J.ux = J.uy = J.uz = (R)1; J.ia = (R)1; J.fa = (R)0; J.dfa = (R)0; J.e0 = (R)1;
     int jcur = -1, paircur = -1;
-    double Aj = 0.0, Vx = 0.0, Vy = 0.0, Vz = 0.0;
-    double cf[REGC ? Spec::NACC : 1];                 // c_b of the lane's current pair group
+    R Aj = (R)0, Vx = (R)0, Vy = (R)0, Vz = (R)0;
+    R cf[REGC ? Spec::NACC : 1];                      // c_b of the lane's current pair group
 #pragma unroll
-    for (int a = 0; a < (REGC ? Spec::NACC : 1); ++a) cf[a] = 0.0;
+    for (int a = 0; a < (REGC ? Spec::NACC : 1); ++a) cf[a] = (R)0;
     uint32_t dcur = 0xffffffffu;
     for (int it = 0; it < quota; ++it) {
         const bool active = wk.cnt > 0;
@@ -276,25 +291,25 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
             const int jn = wk.j();
             if (jn != jcur) {
                 if (jcur >= 0) {
-                    double2 a = acc.fxy[jcur];
-                    double b = acc.fz[jcur];
+                    R2 a = acc.fxy[jcur];
+                    R b = acc.fz[jcur];
                     a.x += fma(-Aj, J.ux, Vx); a.y += fma(-Aj, J.uy, Vy); b += fma(-Aj, J.uz, Vz);
                     acc.fxy[jcur] = a;
                     acc.fz[jcur] = b;
                 }
                 jcur = jn;
-                const double2 a0 = p0[jcur], a1 = p1[jcur], a2 = p2[jcur];
+                const R2 a0 = p0[jcur], a1 = p1[jcur], a2 = p2[jcur];
                 J.ux = a0.x; J.uy = a0.y; J.uz = a1.x; J.ia = a1.y; J.fa = a2.x; J.dfa = a2.y; J.e0 = e0[jcur];
-                Aj = 0.0; Vx = 0.0; Vy = 0.0; Vz = 0.0;
+                Aj = (R)0; Vx = (R)0; Vy = (R)0; Vz = (R)0;
             }
             const int pr = p.n_elem <= 2 ? wk.pair2() : pair_of_slots(jn, wk.first_partner(), seg, p.n_elem);
             if (pr != paircur) {
                 paircur = pr;
                 if constexpr (REGC) {
-                    const double2* src = reinterpret_cast<const double2*>(btc + pr * 2 * bt2_stride<Spec>());
+                    const R2* src = reinterpret_cast<const R2*>(btc + pr * 2 * bt2_stride<Spec>());
 #pragma unroll
                     for (int a = 0; a < Spec::NACC / 2; ++a) {
-                        const double2 c = src[a];
+                        const R2 c = src[a];
                         cf[2 * a] = c.x; cf[2 * a + 1] = c.y;
                     }
                     if constexpr (Spec::NACC & 1) cf[Spec::NACC - 1] = btc[pr * 2 * bt2_stride<Spec>() + Spec::NACC - 1];
@@ -303,32 +318,32 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
         }
         __syncwarp();
         // c_b of the lane's pair group: registers (REGC) or, for the large sets, 128-bit loads of c pairs per eta
-        const double2* btg = bt + max(paircur, 0) * bt2_stride<Spec>();
+        const R2* btg = bt + max(paircur, 0) * bt2_stride<Spec>();
         const int k = active ? wk.pop() : max(jcur, 0);
         const int rank = conflict_rank(k, active, lane);       // issued early: its latency hides behind the FP64 work
-        const double2 k0 = p0[k], k1 = p1[k], k2v = p2[k];
-        const double ek = e0[k];
-        const double wx = k0.x - J.ux, wy = k0.y - J.uy, wz = k1.x - J.uz;
-        const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
-        double Cc, Sc;
-        cos_sinc(c2 * p.k2, Cc, Sc);
-        double fcc = Cc * Cc;                          // fc(c)
-        double dfc = (-2.0 * p.k2) * (Cc * Sc);        // fc'(c)/c
-        if (!active || !(c2 < p.rc2)) { fcc = 0.0; dfc = 0.0; }   // exact cutoff (the masks were screened in FP32)
-        double Y[Spec::NETA];
-        const double r2 = (J.e0 + ek) + c2;                    // FREE_ETA: a^2 + b^2 + c^2 (the staged value is a^2)
+        const R2 k0 = p0[k], k1 = p1[k], k2v = p2[k];
+        const R ek = e0[k];
+        const R wx = k0.x - J.ux, wy = k0.y - J.uy, wz = k1.x - J.uz;
+        const R c2 = fma(wx, wx, fma(wy, wy, wz * wz));
+        R Cc, Sc;
+        cos_sinc(c2 * k2r, Cc, Sc);
+        R fcc = Cc * Cc;                               // fc(c)
+        R dfc = m2k2 * (Cc * Sc);                      // fc'(c)/c
+        if (!active || !(c2 < rc2r)) { fcc = (R)0; dfc = (R)0; }   // cutoff (FP64: exact; the masks were screened in FP32)
+        R Y[Spec::NETA];
+        const R r2 = (J.e0 + ek) + c2;                         // FREE_ETA: a^2 + b^2 + c^2 (the staged value is a^2)
         if constexpr (!Spec::FREE_ETA) {
-            Y[0] = (J.e0 * ek) * (tiny ? exp_tiny(-eta0 * c2) : exp_small(-eta0 * c2));
+            Y[0] = (J.e0 * ek) * (tiny ? exp_tiny(-eta0r * c2) : exp_small(-eta0r * c2));
             if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
             if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
             if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
         }
-        const double iab = J.ia * k1.y;
-        const double cosv = fma(J.ux, k0.x, fma(J.uy, k0.y, J.uz * k1.x)) * iab;
+        const R iab = J.ia * k1.y;
+        const R cosv = fma(J.ux, k0.x, fma(J.uy, k0.y, J.uz * k1.x)) * iab;
         // pw[l][b] = (1 +- cos)^(2^b) ; pd[l][b] = (1 +- cos)^(2^b - 1)  (REGC: times zeta = 2^b)
-        double pw[2][Spec::MAXBIT + 1], pd[2][Spec::MAXBIT + 1];
-        pw[0][0] = 1.0 + cosv; pw[1][0] = 1.0 - cosv;
-        pd[0][0] = 1.0; pd[1][0] = 1.0;
+        R pw[2][Spec::MAXBIT + 1], pd[2][Spec::MAXBIT + 1];
+        pw[0][0] = (R)1 + cosv; pw[1][0] = (R)1 - cosv;
+        pd[0][0] = (R)1; pd[1][0] = (R)1;
 #pragma unroll
         for (int b = 1; b <= Spec::MAXBIT; ++b) {
 #pragma unroll
@@ -342,23 +357,23 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
             pd[0][b] = scale2(pd[0][b], b);
             pd[1][b] = scale2(pd[1][b], b);
         }
-        double Z0 = 0.0, Z1 = 0.0, Z2 = 0.0;
+        R Z0 = (R)0, Z1 = (R)0, Z2 = (R)0;
 #pragma unroll
         for (int e = 0; e < Spec::NETA; ++e) {
             if (Spec::FREE_ETA && e >= neta) break;            // uniform per CTA: eta slots the table does not use
             if constexpr (Spec::FREE_ETA) Y[e] = exp_small(-eta[e] * r2);
-            double T0 = 0.0, T1 = 0.0;
+            R T0 = (R)0, T1 = (R)0;
             // the coefficients of eta_e sit at consecutive (even-aligned) accumulator indices
             constexpr int NE = 16;
-            double ce[REGC ? 1 : NE];
+            R ce[REGC ? 1 : NE];
             if constexpr (!REGC) {
                 const int base = acc_index<Spec>(e, 0) & ~1;
 #pragma unroll
                 for (int q = 0; q < NE / 2; ++q) {
                     if (base + 2 * q < acc_index<Spec>(e + 1, 0)) {          // folds after unrolling: only this eta's pairs
-                        const double2 v = btg[(base >> 1) + q];
+                        const R2 v = btg[(base >> 1) + q];
                         ce[2 * q] = v.x; ce[2 * q + 1] = v.y;
-                    } else { ce[2 * q] = 0.0; ce[2 * q + 1] = 0.0; }
+                    } else { ce[2 * q] = (R)0; ce[2 * q + 1] = (R)0; }
                 }
             }
 #pragma unroll
@@ -366,28 +381,28 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
 #pragma unroll
                 for (int l = 0; l < 2; ++l)
                     if (Spec::mask(e) >> (8 * l + b) & 1u) {
-                        double c;
+                        R c;
                         if constexpr (REGC) c = cf[acc_index<Spec>(e, 8 * l + b)];
                         else c = ce[acc_index<Spec>(e, 8 * l + b) - (acc_index<Spec>(e, 0) & ~1)];
                         T0 = fma(c, pw[l][b], T0);
                         T1 = l == 0 ? fma(c, pd[l][b], T1) : fma(-c, pd[l][b], T1);
                     }
             }
-            const double A = T0 * Y[e];
+            const R A = T0 * Y[e];
             Z0 += A;
             Z1 = fma(T1, Y[e], Z1);
             Z2 = fma(eta[e], A, Z2);
         }
         // slot scalars
-        const double fab = J.fa * k2v.x;
-        const double Cf = fab * fcc;
-        const double t2 = (Cf + Cf) * Z2;
-        const double f_w = fma(fab * dfc, Z0, -t2);
-        const double q = Z1 * Cf;
-        const double qc = q * cosv;
-        const double f_uu = fma(-qc, J.ia * J.ia, fma((J.dfa * k2v.x) * fcc, Z0, -t2));
-        const double f_vv = fma(-qc, k1.y * k1.y, fma((J.fa * k2v.y) * fcc, Z0, -t2));
-        const double s1 = f_uu + f_w, s2 = f_vv + f_w, s3 = fma(-q, iab, f_w);
+        const R fab = J.fa * k2v.x;
+        const R Cf = fab * fcc;
+        const R t2 = (Cf + Cf) * Z2;
+        const R f_w = fma(fab * dfc, Z0, -t2);
+        const R q = Z1 * Cf;
+        const R qc = q * cosv;
+        const R f_uu = fma(-qc, J.ia * J.ia, fma((J.dfa * k2v.x) * fcc, Z0, -t2));
+        const R f_vv = fma(-qc, k1.y * k1.y, fma((J.fa * k2v.y) * fcc, Z0, -t2));
+        const R s1 = f_uu + f_w, s2 = f_vv + f_w, s3 = fma(-q, iab, f_w);
         Aj += s1;
         Vx = fma(s3, k0.x, Vx);
         Vy = fma(s3, k0.y, Vy);
@@ -404,18 +419,19 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
     double fx = 0.0, fy = 0.0, fz = 0.0;
     for (int m = tid; m < ntot; m += NT) {
         const int j = row[m];
-        const double2 u0 = p0[m];
-        const double uz = p1[m].x;
-        double2 fxy = acc0[m];
-        double fzz = reinterpret_cast<const double*>(acc0 + capa)[m];
+        const R2 u0 = p0[m];
+        const R uz = p1[m].x;
+        R2 fxy = acc0[m];
+        R fzz = reinterpret_cast<const R*>(acc0 + capa)[m];
 #pragma unroll
         for (int w = 1; w < WPC; ++w) {
-            const double2 a = acc0[(size_t)w * 2 * capa + m];
+            const R2 a = acc0[(size_t)w * 2 * capa + m];
             fxy.x += a.x; fxy.y += a.y;
-            fzz += reinterpret_cast<const double*>(acc0 + (size_t)w * 2 * capa + capa)[m];
+            fzz += reinterpret_cast<const R*>(acc0 + (size_t)w * 2 * capa + capa)[m];
         }
-        const double R = rad[m];
-        const double ax = fma(-R, u0.x, fxy.x), ay = fma(-R, u0.y, fxy.y), az = fma(-R, uz, fzz);
+        const double Rm = (double)rad[m];
+        const double ax = fma(-Rm, (double)u0.x, (double)fxy.x), ay = fma(-Rm, (double)u0.y, (double)fxy.y),
+                     az = fma(-Rm, (double)uz, (double)fzz);
         atomicAdd(&p.f_sorted[3 * (size_t)j + 0], ax);
         atomicAdd(&p.f_sorted[3 * (size_t)j + 1], ay);
         atomicAdd(&p.f_sorted[3 * (size_t)j + 2], az);
@@ -429,20 +445,30 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
     }
 }
 
+#ifndef F2_MINB_F32
+#define F2_MINB_F32 32       // warps per SM asked of the FP32 instantiations (mixed-precision mode)
+#endif
+template <class Spec, int WPC, int CAPA, class R>
+__host__ __device__ constexpr int f2_min_blocks() {
+    // 10 CTAs per SM only where the coefficients live in registers (NACC <= 12): the wide set at 96 registers
+    // spilled into the loop (configs[4]: 10.38 vs 9.80 ms)
+    return WPC == 1 ? F2_MINB1 : (sizeof(R) == 4 ? F2_MINB_F32 : (CAPA <= 128 && Spec::NACC <= 12 ? F2_MINB_128 : 14)) / WPC;
+}
+
 // one CTA per centre: blockIdx.x = sorted position of the centre
-template <class Spec, int WPC, int CAPA, bool TINY>
-__global__ void __launch_bounds__(WPC * 32, WPC == 1 ? F2_MINB1 : (CAPA <= 128 ? F2_MINB_128 : 14) / WPC) k_force2(const __grid_constant__ Force2Params p) {
+template <class Spec, int WPC, int CAPA, bool TINY, class R>
+__global__ void __launch_bounds__(WPC * 32, f2_min_blocks<Spec, WPC, CAPA, R>()) k_force2(const __grid_constant__ Force2Params p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    force2_centre<Spec, WPC, CAPA, TINY>(p, (int64_t)blockIdx.x, smem_raw);
+    force2_centre<Spec, WPC, CAPA, TINY, R>(p, (int64_t)blockIdx.x, smem_raw);
 }
 
 // the centres of a list (Workspace::big_list: those with more than 128 neighbours), a few CTAs walking it
-template <class Spec, int WPC, int CAPA, bool TINY>
+template <class Spec, int WPC, int CAPA, bool TINY, class R>
 __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2_list(const __grid_constant__ Force2Params p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int n_list = *p.big_count;
     for (int q = blockIdx.x; q < n_list; q += gridDim.x) {
-        force2_centre<Spec, WPC, CAPA, TINY>(p, (int64_t)p.big_list[q], smem_raw);
+        force2_centre<Spec, WPC, CAPA, TINY, R>(p, (int64_t)p.big_list[q], smem_raw);
         __syncthreads();                             // the next centre reuses the shared memory
     }
 }
@@ -452,45 +478,45 @@ __global__ void __launch_bounds__(WPC * 32, 14 / WPC) k_force2_list(const __grid
 #endif
 constexpr int F2_WPC = NNP_F2_WPC;
 
-template <class Spec, int CAPA, bool TINY, int WPC = F2_WPC>
+template <class Spec, int CAPA, bool TINY, class R, int WPC = F2_WPC>
 static int launch_capa(Force2Params p, int nt_lo, int nt_hi, cudaStream_t st) {
     p.nt_lo = nt_lo; p.nt_hi = nt_hi;
-    const size_t smem = force2_smem<Spec>(CAPA, p.g_stride, p.n_elem, WPC);
+    const size_t smem = force2_smem<Spec>(CAPA, p.g_stride, p.n_elem, WPC, sizeof(R));
     static unsigned long long configured = 0ull;      // per device (opt_in_smem)
-    opt_in_smem(k_force2<Spec, WPC, CAPA, TINY>, &configured);
-    k_force2<Spec, WPC, CAPA, TINY><<<(unsigned)p.n, WPC * 32, smem, st>>>(p);
+    opt_in_smem(k_force2<Spec, WPC, CAPA, TINY, R>, &configured);
+    k_force2<Spec, WPC, CAPA, TINY, R><<<(unsigned)p.n, WPC * 32, smem, st>>>(p);
     return 1;
 }
 
-template <class Spec, int CAPA, bool TINY, int WPC = F2_WPC>
+template <class Spec, int CAPA, bool TINY, class R, int WPC = F2_WPC>
 static int launch_capa_list(Force2Params p, int nt_lo, int nt_hi, cudaStream_t st) {
     p.nt_lo = nt_lo; p.nt_hi = nt_hi;
-    const size_t smem = force2_smem<Spec>(CAPA, p.g_stride, p.n_elem, WPC);
+    const size_t smem = force2_smem<Spec>(CAPA, p.g_stride, p.n_elem, WPC, sizeof(R));
     static unsigned long long configured = 0ull;
-    opt_in_smem(k_force2_list<Spec, WPC, CAPA, TINY>, &configured);
+    opt_in_smem(k_force2_list<Spec, WPC, CAPA, TINY, R>, &configured);
     const unsigned grid = (unsigned)(p.n < 148 * 8 ? p.n : 148 * 8);
-    k_force2_list<Spec, WPC, CAPA, TINY><<<grid, WPC * 32, smem, st>>>(p);
+    k_force2_list<Spec, WPC, CAPA, TINY, R><<<grid, WPC * 32, smem, st>>>(p);
     return 1;
 }
 
 // slot capacity = smallest instantiated CAPA that holds max_neighbors (nnp_set_max_neighbors: 32..255)
-template <class Spec, bool TINY>
+template <class Spec, bool TINY, class R = double>
 static int launch_one2(const Force2Params& p, cudaStream_t st) {
-    // small neighbourhoods (metals: ~20 neighbours, ~60 triplets per centre): 64 slots, ONE warp per centre
-    if (p.cap <= 64) return launch_capa<Spec, 64, TINY, 1>(p, 0, 64, st);
+    // small neighbourhoods (metals: ~20 neighbours, ~60 triplets per centre): 64 slots, ONE warp per centre (FP64 only)
+    if (p.cap <= 64) return launch_capa<Spec, 64, TINY, double, 1>(p, 0, 64, st);
     // The 128-slot instantiation keeps 10 CTAs per SM resident (21.7 KB, 96 registers) against 8 of the 160-slot one
     // (27.5 KB, 119 registers): every centre with at most 128 neighbours runs on it (measured on configs[3]: 79.4 ->
     // 76.8 ms), the few others (water-like systems: 1 centre in ~10^4; listed by k_count_words) on a list-driven launch
     // of the bigger instantiation -- a second launch over all N centres costs 1.3 ms in CTAs that return at once.
-    int launches = launch_capa<Spec, 128, TINY>(p, 0, 128, st);
-    if (p.cap > 128) launches += p.cap <= 160 ? launch_capa_list<Spec, 160, TINY>(p, 129, 160, st)
-                                              : launch_capa_list<Spec, 256, TINY>(p, 129, 255, st);
+    int launches = launch_capa<Spec, 128, TINY, R>(p, 0, 128, st);
+    if (p.cap > 128) launches += p.cap <= 160 ? launch_capa_list<Spec, 160, TINY, R>(p, 129, 160, st)
+                                              : launch_capa_list<Spec, 256, TINY, double>(p, 129, 255, st);
     return launches;
 }
 
 // launches the fast kernels for the specialised variants in use; the caller has zeroed f_sorted
 int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                  const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st) {
+                  const int* variant, double rc, int stride, int max_nbr, int g_stride, int precision, cudaStream_t st) {
     if (n == 0) return 0;
     Force2Params p;
     p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride;
@@ -508,9 +534,11 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
         if (e < n_elem) use[variant[e] & 255][(variant[e] >> 8) & 1] = true;
     }
     int launches = 0;
-    if (use[ANG_BASE12][1]) launches += launch_one2<SpecBase12, true>(p, st);
+    // precision 1 (nnp_set_precision: mixed): FP32 instantiations of BASELINE.json's two shapes, water-like exp range
+    const bool f32 = precision == 1;
+    if (use[ANG_BASE12][1]) launches += f32 ? launch_one2<SpecBase12, true, float>(p, st) : launch_one2<SpecBase12, true>(p, st);
     if (use[ANG_BASE12][0]) launches += launch_one2<SpecBase12, false>(p, st);
-    if (use[ANG_WIDE32][1]) launches += launch_one2<SpecWide32, true>(p, st);
+    if (use[ANG_WIDE32][1]) launches += f32 ? launch_one2<SpecWide32, true, float>(p, st) : launch_one2<SpecWide32, true>(p, st);
     if (use[ANG_WIDE32][0]) launches += launch_one2<SpecWide32, false>(p, st);
     if (use[ANG_FREE32][0]) launches += launch_one2<SpecFree32, false>(p, st);
     if (use[ANG_FREE16][0]) launches += launch_one2<SpecFree16, false>(p, st);

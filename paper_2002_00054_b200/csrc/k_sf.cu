@@ -206,7 +206,7 @@ static int launch_one(const SfParams& p, cudaStream_t st) {
 }
 
 int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-              const int* variant, double rc, int stride, int max_nbr, int g_stride, int na_max, cudaStream_t st) {
+              const int* variant, double rc, int stride, int max_nbr, int g_stride, int na_max, int precision, cudaStream_t st) {
     if (n == 0) return 0;
     SfParams p;
     p.na_max = na_max;
@@ -224,7 +224,7 @@ int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const El
     }
     int launches = 0;
     if (use[ANG_BASE12] || use[ANG_WIDE32] || use[ANG_FREE32] || use[ANG_FREE16])     // specialised tables: lane-owned design (k_sf2.cu)
-        launches += launch_sf2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, st);
+        launches += launch_sf2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, precision, st);
     if (use[ANG_GENERIC]) launches += launch_one<SpecGeneric>(p, st);
     return launches;
 }

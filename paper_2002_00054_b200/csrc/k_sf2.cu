@@ -29,10 +29,18 @@ struct Sf2Params {
 // Shared memory of one centre: planes p0 (ux,uy), p1 (uz,1/a), p2 (exp(-eta0 a^2), fc(a)) double2[CAPA];
 // ra (a) double[CAPA]; FP32 screening copy float4[CAPA] (the prefix array aliases it afterwards);
 // then group table, G accumulators [npair][NACC], scratch, mask words (mask + descriptor)
+// arithmetic type R of the staged planes and the per-triplet evaluation (double, or float in the opt-in
+// mixed-precision mode: see k_force2.cu)
+template <class R> struct SfVec2;
+template <> struct SfVec2<double> { using type = double2; };
+template <> struct SfVec2<float> { using type = float2; };
+__device__ __forceinline__ double2 sf_mk2(double a, double b) { return make_double2(a, b); }
+__device__ __forceinline__ float2 sf_mk2(float a, float b) { return make_float2(a, b); }
+
 template <class Spec>
-__host__ __device__ constexpr size_t sf2_smem(int capa, int n_elem, int wpc) {
+__host__ __device__ constexpr size_t sf2_smem(int capa, int n_elem, int wpc, size_t real = 8) {
     const size_t npair = (size_t)n_elem * (n_elem + 1) / 2;
-    size_t b = (size_t)capa * (3 * 16 + 8 + 16);
+    size_t b = (size_t)capa * (3 * 2 * real + 8 + 16);
     b += npair * sizeof(GroupTab);
     b += (size_t)(wpc + 1) * npair * Spec::NACC * 8;
     b += 64;
@@ -43,8 +51,12 @@ __host__ __device__ constexpr size_t sf2_smem(int capa, int n_elem, int wpc) {
 #ifndef S2_MINB1
 #define S2_MINB1 24          // resident CTAs per SM asked of the one-warp-per-centre instantiation (12 SFs per group)
 #endif
-template <class Spec, int WPC, int CAPA, bool TINY>
-__global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MINB1 : 16) : (Spec::NACC <= 12 ? 24 : (Spec::NACC <= 16 ? 20 : 16)) / WPC) k_sf2(const __grid_constant__ Sf2Params p) {
+#ifndef S2_MINB_F32
+#define S2_MINB_F32 32       // warps per SM asked of the FP32 instantiations (mixed-precision mode)
+#endif
+template <class Spec, int WPC, int CAPA, bool TINY, class R>
+__global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MINB1 : 16) : (sizeof(R) == 4 ? (Spec::NACC <= 12 ? S2_MINB_F32 : 20) : (Spec::NACC <= 12 ? 24 : (Spec::NACC <= 16 ? 20 : 16))) / WPC) k_sf2(const __grid_constant__ Sf2Params p) {
+    using R2 = typename SfVec2<R>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NT = WPC * 32;
     constexpr int NACC = Spec::NACC;
@@ -58,10 +70,10 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
 
     constexpr int capa = CAPA;
     const int npair = p.n_elem * (p.n_elem + 1) / 2;
-    double2* p0 = reinterpret_cast<double2*>(smem_raw);     // (ux, uy)
-    double2* p1 = p0 + capa;                                // (uz, 1/a)
-    double2* p2 = p1 + capa;                                // (exp(-eta_0 a^2), fc(a))
-    double* ra = reinterpret_cast<double*>(p2 + capa);      // a
+    R2* p0 = reinterpret_cast<R2*>(smem_raw);               // (ux, uy)
+    R2* p1 = p0 + capa;                                     // (uz, 1/a)
+    R2* p2 = p1 + capa;                                     // (exp(-eta_0 a^2), fc(a))
+    double* ra = reinterpret_cast<double*>(p2 + capa);      // a (FP64 in both modes: the radial block)
     float4* f32 = reinterpret_cast<float4*>(ra + capa);     // screening copy
     uint16_t* C = reinterpret_cast<uint16_t*>(f32);         // alias: prefix of the mask popcounts (after screening)
     GroupTab* tab = reinterpret_cast<GroupTab*>(f32 + capa);
@@ -83,9 +95,10 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
     const int32_t* row = p.nbr + (size_t)i * p.stride;
     const double eta0 = prog->ang_eta[0];
     const int neta = Spec::FREE_ETA ? prog->n_eta : Spec::NETA;
-    double etav[Spec::FREE_ETA ? Spec::NETA : 1];
+    R etav[Spec::FREE_ETA ? Spec::NETA : 1];
     if constexpr (Spec::FREE_ETA)
-        for (int e = 0; e < Spec::NETA; ++e) etav[e] = prog->ang_eta[e];
+        for (int e = 0; e < Spec::NETA; ++e) etav[e] = (R)prog->ang_eta[e];
+    const R eta0r = (R)eta0, k2r = (R)p.k2, rc2r = (R)p.rc2;
     constexpr bool tiny = TINY;                      // exp(-eta_0 r^2) without range reduction (mathfn.cuh exp_tiny)
     if ((prog->tiny_exp != 0) != TINY) return;       // uniform per CTA: the other instantiation owns this element
     for (int m = tid; m < ntot; m += NT) {
@@ -96,10 +109,10 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
         const double a2 = fma(dx, dx, fma(dy, dy, dz * dz));
         const double ia = rsqrt(a2);
         const double Ca = cos_only(a2 * p.k2);
-        p0[m] = make_double2(dx, dy);
-        p1[m] = make_double2(dz, ia);
+        p0[m] = sf_mk2((R)dx, (R)dy);
+        p1[m] = sf_mk2((R)dz, (R)ia);
         // first component: exp(-eta_0 a^2), or a^2 itself where every eta gets its own exponential (FREE_ETA)
-        p2[m] = make_double2(Spec::FREE_ETA ? a2 : (tiny ? exp_tiny(-eta0 * a2) : exp_small(-eta0 * a2)), Ca * Ca);
+        p2[m] = sf_mk2((R)(Spec::FREE_ETA ? a2 : (tiny ? exp_tiny(-eta0 * a2) : exp_small(-eta0 * a2))), (R)(Ca * Ca));
         ra[m] = a2 * ia;
         f32[m] = make_float4((float)dx, (float)dy, (float)dz, 0.f);
     }
@@ -119,7 +132,7 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
             double acc = 0.0;
             for (int m = seg[e] + lane; m < seg[e + 1]; m += 32) {
                 const double d = ra[m] - f.rs;
-                acc = fma(exp_small(fmax(-f.eta * d * d, -700.0)), p2[m].y, acc);
+                acc = fma(exp_small(fmax(-f.eta * d * d, -700.0)), (double)p2[m].y, acc);
             }
             acc = warp_sum(acc);
             if (lane == 0) Grow[f.g] = acc;
@@ -146,12 +159,12 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
     if (wk.cnt > 0) wk.seek(C, NW, tid * quota);
 
     // ---- angular part: every lane walks its range of the stream ---------------------------------------
-    double jx = 1.0, jy = 1.0, jz = 1.0, jia = 1.0, je0 = 1.0, jfa = 0.0;
+    R jx = (R)1, jy = (R)1, jz = (R)1, jia = (R)1, je0 = (R)1, jfa = (R)0;
     int jcur = -1, paircur = -1;
     uint32_t dcur = 0xffffffffu;
-    double acc[NACC];
+    R acc[NACC];                                     // FP32 mode: a lane sums its ~30 triplets in FP32, the lanes are reduced in FP64
 #pragma unroll
-    for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+    for (int a = 0; a < NACC; ++a) acc[a] = (R)0;
     for (int it = 0; it < quota; ++it) {
         const bool active = wk.cnt > 0;
         wk.advance();
@@ -160,7 +173,7 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
             const int jn = wk.j();
             if (jn != jcur) {
                 jcur = jn;
-                const double2 a0 = p0[jcur], a1 = p1[jcur], a2 = p2[jcur];
+                const R2 a0 = p0[jcur], a1 = p1[jcur], a2 = p2[jcur];
                 jx = a0.x; jy = a0.y; jz = a1.x; jia = a1.y; je0 = a2.x; jfa = a2.y;
             }
             const int pr = p.n_elem <= 2 ? wk.pair2() : pair_of_slots(jn, wk.first_partner(), seg, p.n_elem);
@@ -171,32 +184,32 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
                 if (paircur >= 0) {
 #pragma unroll
                     for (int a = 0; a < NACC; ++a) {
-                        gacc[paircur * NACC + a] = acc[a];
-                        acc[a] = 0.0;
+                        gacc[paircur * NACC + a] = (double)acc[a];
+                        acc[a] = (R)0;
                     }
                 }
                 paircur = pr;
             }
         }
         const int k = active ? wk.pop() : max(jcur, 0);
-        const double2 k0 = p0[k], k1 = p1[k], k2v = p2[k];
-        const double wx = k0.x - jx, wy = k0.y - jy, wz = k1.x - jz;
-        const double c2 = fma(wx, wx, fma(wy, wy, wz * wz));
-        const double Cc = cos_only(c2 * p.k2);
-        double Cf = (jfa * k2v.y) * (Cc * Cc);      // fc(a) fc(b) fc(c), fc(c) = cos^2(pi c / (2 rc))
-        if (!active || !(c2 < p.rc2)) Cf = 0.0;     // exact cutoff (the masks were screened in FP32)
-        double Y[Spec::NETA];
-        const double r2 = (je0 + k2v.x) + c2;                  // FREE_ETA: a^2 + b^2 + c^2 (the staged value is a^2)
+        const R2 k0 = p0[k], k1 = p1[k], k2v = p2[k];
+        const R wx = k0.x - jx, wy = k0.y - jy, wz = k1.x - jz;
+        const R c2 = fma(wx, wx, fma(wy, wy, wz * wz));
+        const R Cc = cos_only(c2 * k2r);
+        R Cf = (jfa * k2v.y) * (Cc * Cc);           // fc(a) fc(b) fc(c), fc(c) = cos^2(pi c / (2 rc))
+        if (!active || !(c2 < rc2r)) Cf = (R)0;     // cutoff (FP64: exact; the masks were screened in FP32)
+        R Y[Spec::NETA];
+        const R r2 = (je0 + k2v.x) + c2;                       // FREE_ETA: a^2 + b^2 + c^2 (the staged value is a^2)
         if constexpr (!Spec::FREE_ETA) {
-            Y[0] = (je0 * k2v.x) * (tiny ? exp_tiny(-eta0 * c2) : exp_small(-eta0 * c2));
+            Y[0] = (je0 * k2v.x) * (tiny ? exp_tiny(-eta0r * c2) : exp_small(-eta0r * c2));
             if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);
             if constexpr (Spec::NETA > 2) Y[2] = ipow<Spec::ratio(2)>(Y[Spec::rbase(2)]);
             if constexpr (Spec::NETA > 3) Y[3] = ipow<Spec::ratio(3)>(Y[Spec::rbase(3)]);
         }
-        const double cosv = fma(jx, k0.x, fma(jy, k0.y, jz * k1.x)) * (jia * k1.y);
-        double pw[2][Spec::MAXBIT + 1];
-        pw[0][0] = 1.0 + cosv;
-        pw[1][0] = 1.0 - cosv;
+        const R cosv = fma(jx, k0.x, fma(jy, k0.y, jz * k1.x)) * (jia * k1.y);
+        R pw[2][Spec::MAXBIT + 1];
+        pw[0][0] = (R)1 + cosv;
+        pw[1][0] = (R)1 - cosv;
 #pragma unroll
         for (int b = 1; b <= Spec::MAXBIT; ++b) {
             pw[0][b] = pw[0][b - 1] * pw[0][b - 1];
@@ -206,7 +219,7 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
         for (int e = 0; e < Spec::NETA; ++e) {
             if (Spec::FREE_ETA && e >= neta) break;            // uniform per CTA: eta slots the table does not use
             if constexpr (Spec::FREE_ETA) Y[e] = exp_small(-etav[e] * r2);
-            const double xc = Y[e] * Cf;
+            const R xc = Y[e] * Cf;
 #pragma unroll
             for (int b = 0; b <= Spec::MAXBIT; ++b) {
                 if (Spec::mask(e) >> b & 1u) acc[acc_index<Spec>(e, b)] = fma(pw[0][b], xc, acc[acc_index<Spec>(e, b)]);
@@ -221,7 +234,7 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
         if (!__any_sync(FULL, paircur == pr)) continue;
         double v[NR];
 #pragma unroll
-        for (int a = 0; a < NR; ++a) v[a] = (a < NACC && paircur == pr) ? acc[a < NACC ? a : 0] : 0.0;
+        for (int a = 0; a < NR; ++a) v[a] = (a < NACC && paircur == pr) ? (double)acc[a < NACC ? a : 0] : 0.0;
         warp_reduce_multi<NR>(v, lane);
         const int a = warp_reduce_index<NR>(lane);
         if ((lane & (32 / NR - 1)) == 0 && a < NACC) gacc[((1 + wid) * npair + pr) * NACC + a] = v[0];
@@ -285,27 +298,29 @@ int launch_word_offsets(const Workspace& w, const Grid& g, int64_t n, int n_elem
 #endif
 constexpr int SF2_WPC = NNP_SF2_WPC;
 
-template <class Spec, int CAPA, bool TINY, int WPC = SF2_WPC>
+template <class Spec, int CAPA, bool TINY, class R, int WPC = SF2_WPC>
 static int launch_capa_sf(const Sf2Params& p, cudaStream_t st) {
-    const size_t smem = sf2_smem<Spec>(CAPA, p.n_elem, WPC);
+    const size_t smem = sf2_smem<Spec>(CAPA, p.n_elem, WPC, sizeof(R));
     static unsigned long long configured = 0ull;      // per device (opt_in_smem)
-    opt_in_smem(k_sf2<Spec, WPC, CAPA, TINY>, &configured);
-    k_sf2<Spec, WPC, CAPA, TINY><<<(unsigned)p.n, WPC * 32, smem, st>>>(p);
+    opt_in_smem(k_sf2<Spec, WPC, CAPA, TINY, R>, &configured);
+    k_sf2<Spec, WPC, CAPA, TINY, R><<<(unsigned)p.n, WPC * 32, smem, st>>>(p);
     return 1;
 }
 
-template <class Spec, bool TINY>
+template <class Spec, bool TINY, class R = double>
 static int launch_one_sf2(const Sf2Params& p, cudaStream_t st) {
     // small neighbourhoods (metals: ~20 neighbours, ~60 triplets per centre): 64 slots, ONE warp per centre
-    if (p.cap <= 64) return launch_capa_sf<Spec, 64, TINY, 1>(p, st);
-    if (p.cap <= 128) return launch_capa_sf<Spec, 128, TINY>(p, st);
-    if (p.cap <= 160) return launch_capa_sf<Spec, 160, TINY>(p, st);
-    return launch_capa_sf<Spec, 256, TINY>(p, st);
+    if (p.cap <= 64) return launch_capa_sf<Spec, 64, TINY, double, 1>(p, st);
+    // one launch at the slot capacity of max_neighbors (a 128 / 160 split as in k_force2.cu bought nothing here:
+    // 48.19 vs 48.20 ms on configs[3] at 12 and 14 CTAs per SM -- this kernel is issue-bound, not occupancy-bound)
+    if (p.cap <= 128) return launch_capa_sf<Spec, 128, TINY, R>(p, st);
+    if (p.cap <= 160) return launch_capa_sf<Spec, 160, TINY, R>(p, st);
+    return launch_capa_sf<Spec, 256, TINY, double>(p, st);
 }
 
 // launches the fast kernels for the specialised variants in use
 int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-               const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st) {
+               const int* variant, double rc, int stride, int max_nbr, int g_stride, int precision, cudaStream_t st) {
     if (n == 0) return 0;
     Sf2Params p;
     p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride;
@@ -322,9 +337,10 @@ int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const E
         if (e < n_elem) use[variant[e] & 255][(variant[e] >> 8) & 1] = true;
     }
     int launches = 0;
-    if (use[ANG_BASE12][1]) launches += launch_one_sf2<SpecBase12, true>(p, st);
+    const bool f32 = precision == 1;     // nnp_set_precision: mixed (BASELINE.json's two shapes only)
+    if (use[ANG_BASE12][1]) launches += f32 ? launch_one_sf2<SpecBase12, true, float>(p, st) : launch_one_sf2<SpecBase12, true>(p, st);
     if (use[ANG_BASE12][0]) launches += launch_one_sf2<SpecBase12, false>(p, st);
-    if (use[ANG_WIDE32][1]) launches += launch_one_sf2<SpecWide32, true>(p, st);
+    if (use[ANG_WIDE32][1]) launches += f32 ? launch_one_sf2<SpecWide32, true, float>(p, st) : launch_one_sf2<SpecWide32, true>(p, st);
     if (use[ANG_WIDE32][0]) launches += launch_one_sf2<SpecWide32, false>(p, st);
     if (use[ANG_FREE32][0]) launches += launch_one_sf2<SpecFree32, false>(p, st);
     if (use[ANG_FREE16][0]) launches += launch_one_sf2<SpecFree16, false>(p, st);

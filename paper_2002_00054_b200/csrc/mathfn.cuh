@@ -60,6 +60,28 @@ __device__ __forceinline__ double cos_only(double z) {
     return c;
 }
 
+// ---- FP32 versions for the opt-in mixed-precision mode (nnp_set_precision): degree-5 cutoff
+// polynomials (COSF / SNCF, 3e-8 absolute) and the hardware exponential ex2.approx (2 ulp); errors far below the FP32
+// rounding of the sums they feed.
+__device__ __forceinline__ float exp_small(float y) { return __expf(y); }
+__device__ __forceinline__ float exp_tiny(float y) { return __expf(y); }
+__device__ __forceinline__ void cos_sinc(float z, float& C, float& S) {
+    float c = COSF[5], s = SNCF[5];
+#pragma unroll
+    for (int q = 4; q >= 0; --q) {
+        c = fmaf(c, z, COSF[q]);
+        s = fmaf(s, z, SNCF[q]);
+    }
+    C = c;
+    S = s;
+}
+__device__ __forceinline__ float cos_only(float z) {
+    float c = COSF[5];
+#pragma unroll
+    for (int q = 4; q >= 0; --q) c = fmaf(c, z, COSF[q]);
+    return c;
+}
+
 // Cutoff of an SF with its own radius rc_s (nnp_set_sf_cutoffs), from r^2: fc = cos^2(pi r / (2 rc_s)) for
 // r < rc_s, else 0; rc2 = rc_s^2, k2 = (pi / (2 rc_s))^2.  The polynomial argument is clamped to its range.
 __device__ __forceinline__ double fc_own(double r2, double rc2, double k2) {

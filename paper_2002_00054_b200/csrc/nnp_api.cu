@@ -17,6 +17,7 @@ struct nnp_model {
     double rc = 0.0;
     int device = 0;
     int max_nbr = 160;
+    int precision = 0;              // NNP_PRECISION_F64 / NNP_PRECISION_MIXED (nnp_set_precision)
     int g_stride = 0;
     int na_max = 0;                 // largest angular pair group (SF count) of any element
     int n_sf_elem[MAX_ELEM] = {0, 0, 0, 0};
@@ -578,6 +579,13 @@ extern "C" nnp_status nnp_set_activation(nnp_model* m, int32_t kind) {
     return NNP_OK;
 }
 
+extern "C" nnp_status nnp_set_precision(nnp_model* m, int32_t mode) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    if (mode != NNP_PRECISION_F64 && mode != NNP_PRECISION_MIXED) return fail(m, NNP_ERR_INVALID_ARG, "unknown precision mode");
+    m->precision = mode;
+    return NNP_OK;
+}
+
 extern "C" nnp_status nnp_set_max_neighbors(nnp_model* m, int32_t max_neighbors) {
     if (!m) return NNP_ERR_INVALID_ARG;
     if (max_neighbors < 32) return fail(m, NNP_ERR_INVALID_ARG, "max_neighbors must be >= 32");
@@ -652,11 +660,11 @@ extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d
     launches += launch_neighbors(w, g, n_atoms, m->n_elem, m->rc * m->rc, stride, m->max_nbr, st);
     mark(2);
     launches += launch_word_offsets(w, g, n_atoms, m->n_elem, m->d_prog, st);
-    launches += launch_sf(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->rc, stride, m->max_nbr, m->g_stride, m->na_max, st);
+    launches += launch_sf(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->rc, stride, m->max_nbr, m->g_stride, m->na_max, m->precision, st);
     mark(3);
     launches += launch_mlp(w, n_atoms, m->n_elem, g.ncell, m->nets, m->g_stride, st);
     mark(4);
-    launches += launch_force(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->rc, stride, m->max_nbr, m->g_stride, st);
+    launches += launch_force(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->rc, stride, m->max_nbr, m->g_stride, m->precision, st);
     mark(5);
     launches += launch_finalize(w, n_atoms, d_e_atom, d_e_total, d_force, st);
     mark(6);

@@ -152,21 +152,21 @@ int launch_sort(const Workspace& w, const Grid& g, int64_t n, int n_elem, const 
 int launch_neighbors(const Workspace& w, const Grid& g, int64_t n, int n_elem, double rc2, int stride,
                      int max_nbr, cudaStream_t st);
 int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-              const int* variant, double rc, int stride, int max_nbr, int g_stride, int na_max, cudaStream_t st);
+              const int* variant, double rc, int stride, int max_nbr, int g_stride, int na_max, int precision, cudaStream_t st);
 int launch_mlp(const Workspace& w, int64_t n, int n_elem, int ncell, const NetDesc* nets, int g_stride,
                cudaStream_t st);
 int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                 const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st);
+                 const int* variant, double rc, int stride, int max_nbr, int g_stride, int precision, cudaStream_t st);
 // mask words per centre + their prefix (k_sf2.cu); before launch_sf
 constexpr int WORD_BUDGET = 320;     // gmask capacity = N * WORD_BUDGET words (a water-like centre with 91 neighbours has 152)
 int launch_word_offsets(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
                         cudaStream_t st);
 // fast path of S2 (lane-owned design, k_sf2.cu): specialised variants only
 int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-               const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st);
+               const int* variant, double rc, int stride, int max_nbr, int g_stride, int precision, cudaStream_t st);
 // fast path of S4 (lane-owned design, k_force2.cu): specialised variants only; f_sorted already zeroed
 int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                  const int* variant, double rc, int stride, int max_nbr, int g_stride, cudaStream_t st);
+                  const int* variant, double rc, int stride, int max_nbr, int g_stride, int precision, cudaStream_t st);
 int launch_finalize(const Workspace& w, int64_t n, double* d_e_atom, double* d_e_total, double* d_force,
                     cudaStream_t st);
 
