@@ -239,6 +239,28 @@ def sweep_config(k: int, local: int, peak_alu: float, counts: dict, steps: int =
             "l2": "workspace %.0f MB %s the 126 MB L2" % (ws / 1e6, "exceeds" if ws > 126e6 else "fits in")}
 
 
+def n2p2like_model():
+    """Probe table of `--table n2p2like` (the one tests/test_gpu_parity.py::test_multi_pass_tables checks)."""
+    import workloads as W
+    from workloads.model import Model, mlp_weights
+    rows, rcs = [], []
+    for c in range(2):
+        for e1 in range(2):
+            for (eta, rs, rr) in ((0.003, 0.0, 6.0), (0.03, 0.0, 6.0), (0.2, 1.0, 4.5), (0.6, 2.0, 3.5)):
+                rows.append((c, 2, e1, 0, eta, rs, 0.0, 0.0)); rcs.append(rr)
+        for (e1, e2) in ((0, 0), (0, 1), (1, 1)):
+            for ie, eta in enumerate((0.0005, 0.002, 0.004, 0.008, 0.015, 0.03, 0.07)):
+                for lam in (1.0, -1.0):
+                    for zeta in (1.0, 4.0):
+                        rows.append((c, 3, e1, e2, eta, 0.0, lam, zeta)); rcs.append(6.0 if ie < 5 else 4.8)
+    sf = np.array(rows, dtype=W.SF_DTYPE)
+    n_per = [int(np.sum(sf["central"] == c)) for c in range(2)]
+    layer_sizes = [[n_per[c], 25, 25, 1] for c in range(2)]
+    return Model(elements=("H", "O"), rc=6.0, sf=sf, layer_sizes=layer_sizes,
+                 weights=[mlp_weights(layer_sizes[c], 200200154, c) for c in range(2)], name="n2p2like92",
+                 n_sf_per_elem=n_per, sf_cutoffs=rcs)
+
+
 def run_reference(args):
     """--impl reference: the oracle on the host cores, each step a bounded sample of the workload."""
     rank = int(os.environ.get("RANK", "0"))
@@ -298,10 +320,12 @@ def main():
     ap.add_argument("--md", action="store_true",
                     help="time velocity-Verlet MD steps (nnp_md_run: kick+drift, the whole path, kick) instead of bare evaluations")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--table", default="baseline", choices=["baseline", "free", "generic"],
+    ap.add_argument("--table", default="baseline", choices=["baseline", "free", "generic", "n2p2like"],
                     help="SF table probe (not a BASELINE.json workload): 'free' breaks the eta ratio of the angular set "
                          "(0.01 -> 0.0123: lane-owned kernels with per-eta exponentials), 'generic' also replaces zeta 16 by 3 "
-                         "(queue-based generic kernels); the roofline object is then not meaningful")
+                         "(queue-based generic kernels), 'n2p2like' is a table shaped like published n2p2 models (zeta in {1, 4}, "
+                         "seven eta values, lambda = +-1, angular functions of two cutoff radii: 3 passes of the free-eta "
+                         "kernels); the roofline object is then not meaningful")
     ap.add_argument("--no-probe", action="store_true", help="skip the DFMA issue-rate probe (for ncu runs)")
     ap.add_argument("--no-sweep", action="store_true",
                     help="skip the short timed runs of configs[1], [2], [4] that the default line carries as config_sweep")
@@ -333,7 +357,9 @@ def main():
 
     cfg = W.CONFIGS[args.config]
     sysm, model = W.build(cfg)
-    if args.table != "baseline":
+    if args.table == "n2p2like":
+        model = n2p2like_model()
+    elif args.table != "baseline":
         ang = model.sf["kind"] == 3
         model.sf["eta"][ang & (model.sf["eta"] == 0.01)] = 0.0123
         if args.table == "generic":

@@ -100,13 +100,17 @@ nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* const* elem_n
  *   NNP_KERNELS_FREE32 / NNP_KERNELS_FREE16  the lane-owned kernels for any table with <= 4 (FREE16: <= 2) distinct
  *                        angular eta values, lambda = +-1, zeta in {1, 2, 4, 16}, narrow (kind 3) functions only,
  *                        no (eta, lambda, zeta) twice per pair group,
- *   NNP_KERNELS_GENERIC  everything else (other zeta, more eta values, kind 9, no angular functions at all).
+ *   NNP_KERNELS_MULTI    the same lane-owned free-eta kernels in several passes: any number of eta values (four per pass)
+ *                        and, after nnp_set_sf_cutoffs, angular functions of several cutoff radii (one radius per pass),
+ *                        at most 8 passes; otherwise the conditions of FREE32,
+ *   NNP_KERNELS_GENERIC  everything else (other zeta, kind 9, more passes, no angular functions at all).
  * Returns NNP_ERR_INVALID_ARG for a table nnp_create would reject (message: nnp_last_error(NULL)). */
 #define NNP_KERNELS_GENERIC 0
 #define NNP_KERNELS_BASE12 1
 #define NNP_KERNELS_WIDE32 2
 #define NNP_KERNELS_FREE32 3
 #define NNP_KERNELS_FREE16 4
+#define NNP_KERNELS_MULTI 5
 nnp_status nnp_table_kernels(int32_t n_elem, double rc, int32_t n_sf, const nnp_sf* sf, int32_t* kernels_out);
 
 /* Free the model and everything the library allocated for it.  NULL is allowed. */
@@ -155,7 +159,9 @@ nnp_status nnp_compute_host(nnp_model* m, int64_t n_atoms, const double* h_pos, 
  *   of n_sf radii in the order of the `sf` table of nnp_create, each 0 < h_rc[s] <= rc (else NNP_ERR_INVALID_ARG);
  *   SF s then uses fc(r; h_rc[s]) = (cos(pi r / h_rc[s]) + 1)/2 for r < h_rc[s], else 0 -- for r_ij, r_ik and, in
  *   kind 3, for r_jk (which must be < h_rc[s]) -- on the neighbourhood of the global rc.  NULL = back to the one
- *   global rc.  An element that has an SF with a radius other than rc runs on the generic kernels.
+ *   global rc.  An element whose ANGULAR functions have radii other than rc runs on the multi-pass kernels
+ *   (NNP_KERNELS_MULTI) if its table fits them, else on the generic kernels; radii on radial functions alone leave the
+ *   choice of kernels as it was.
  *   Synchronises the device. */
 #define NNP_ACT_SOFTPLUS 0
 #define NNP_ACT_TANH 1

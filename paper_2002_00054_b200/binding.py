@@ -27,7 +27,7 @@ EXPORTS = ("nnp_create", "nnp_table_kernels", "nnp_destroy", "nnp_set_max_neighb
            "nnp_uses_fast_path", "nnp_measure_fp64_peak", "nnp_last_error", "nnp_version")
 
 
-KERNEL_NAMES = ("generic", "base12", "wide32", "free32", "free16")
+KERNEL_NAMES = ("generic", "base12", "wide32", "free32", "free16", "multi")
 
 
 def table_kernels(model):

@@ -35,6 +35,7 @@ struct ForceParams {
     double* f_sorted;
     const ElemProgram* prog[MAX_ELEM];
     int variant[MAX_ELEM];
+    int radial_only[MAX_ELEM];           // 1: run only the radial block for this element (per-SF radial radii of a lane-owned element)
 };
 
 // per-warp shared-memory footprint (bytes): six double2 planes (geometry, cutoff, Gaussian, two
@@ -224,8 +225,9 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
     int tc = 0;
     for (int e = 1; e < p.n_elem; ++e)
         if (i >= p.cell_start[(size_t)e * p.ncell]) tc = e;
-    if (p.variant[tc] != Spec::ID) return;
+    if (p.variant[tc] != Spec::ID && p.radial_only[tc] == 0) return;
     const ElemProgram* __restrict__ prog = p.prog[tc];
+    const bool radial_only = p.radial_only[tc] != 0;      // see k_sf.cu: the radial forces of a lane-owned element with own radial radii
 
     const int capa = (p.cap + 3) & ~3;
     const int npair = p.n_elem * (p.n_elem + 1) / 2;
@@ -299,7 +301,7 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
 
     // ---- angular part ---------------------------------------------------------------------------
     const float rc2f = screen_rc2(p.rc2);
-    {
+    if (!radial_only) {
         // generic tables: per pair group, walking the SF list; the beta row stays live, so the queue
         // sits in the (unused) p3 plane
         Q.q = reinterpret_cast<uint32_t*>(nb.p3);
@@ -347,7 +349,8 @@ static int launch_one(const ForceParams& p, cudaStream_t st) {
 }
 
 int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                 const int* variant, double rc, int stride, int max_nbr, int g_stride, int precision, cudaStream_t st) {
+                 const int* variant, const PassInfo& passes, double rc, int stride, int max_nbr, int g_stride, int precision,
+                 cudaStream_t st) {
     if (n == 0) return 0;
     ForceParams p;
     p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride;
@@ -359,12 +362,14 @@ int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
         p.variant[e] = e < n_elem ? (variant[e] & 255) : -1;      // bit 8 = tiny_exp flag (fast launchers)
+        p.radial_only[e] = (e < n_elem && (variant[e] & 255) != ANG_GENERIC && passes.radial_own[e]) ? 1 : 0;
         if (e < n_elem) use[variant[e] & 255] = true;
+        if (p.radial_only[e]) use[ANG_GENERIC] = true;
     }
     cudaMemsetAsync(w.f_sorted, 0, sizeof(double) * 3 * (size_t)n, st);
     int launches = 0;
-    if (use[ANG_BASE12] || use[ANG_WIDE32] || use[ANG_FREE32] || use[ANG_FREE16])     // specialised tables: lane-owned design (k_force2.cu)
-        launches += launch_force2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, precision, st);
+    if (use[ANG_BASE12] || use[ANG_WIDE32] || use[ANG_FREE32] || use[ANG_FREE16] || use[ANG_MULTI])     // specialised tables: lane-owned design (k_force2.cu)
+        launches += launch_force2(w, g, n, n_elem, d_prog, variant, passes, rc, stride, max_nbr, g_stride, precision, st);
     if (use[ANG_GENERIC]) launches += launch_one<SpecGeneric>(p, st);
     return launches;
 }

@@ -29,6 +29,7 @@ struct Force2Params {
     int64_t n;
     int n_elem, ncell, stride, cap, g_stride;
     int nt_lo, nt_hi;                    // this launch owns the centres with nt_lo <= neighbours <= nt_hi (slot-capacity split)
+    int pass;                            // free-eta kernels: which AngPass of the element's program this launch evaluates
     double rc, rc2, k2;                  // k2 = (pi / (2 rc))^2
     double box[3], half[3];
     const double *sx, *sy, *sz;
@@ -128,8 +129,17 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
     int tc = 0;
     for (int e = 1; e < p.n_elem; ++e)
         if (i >= p.cell_start[(size_t)e * p.ncell]) tc = e;
-    if (p.variant[tc] != Spec::ID) return;          // uniform per CTA
+    if (p.variant[tc] != Spec::ID && !(Spec::FREE_ETA && p.variant[tc] == ANG_MULTI)) return;          // uniform per CTA
     const ElemProgram* __restrict__ prog = p.prog[tc];
+    // free-eta kernels: one launch per pass (nnp_internal.h AngPass); the forces are additive over the passes
+    const AngPass* __restrict__ ps = &prog->pass[Spec::FREE_ETA ? p.pass : 0];
+    if (Spec::FREE_ETA && (p.pass >= prog->n_pass || ps->spec != Spec::ID)) return;
+    const bool own_rc = Spec::FREE_ETA && ps->own_rc != 0;          // the pass's cutoff is shorter than the neighbour list's
+    const double rc2p = Spec::FREE_ETA ? ps->rc2 : p.rc2, k2p = Spec::FREE_ETA ? ps->k2 : p.k2;
+    const int32_t* __restrict__ n_ang = Spec::FREE_ETA ? ps->n_ang : prog->n_ang;
+    const int neta = Spec::FREE_ETA ? ps->n_eta : Spec::NETA;
+    const bool first_pass = !Spec::FREE_ETA || p.pass == 0;         // the radial forces
+    const bool handover = !Spec::FREE_ETA || (prog->n_pass == 1 && !own_rc);   // masks from the SF kernel
 
     constexpr int capa = CAPA;
     const int npair = p.n_elem * (p.n_elem + 1) / 2;
@@ -164,7 +174,7 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
     constexpr int NPRE = 6;                                   // words per thread kept in registers
     const int64_t moff = p.word_off[i];
     const int nwg = (int)(p.word_off[i + 1] - moff);
-    const bool have_masks = moff + nwg <= p.gmask_cap;
+    const bool have_masks = handover && moff + nwg <= p.gmask_cap;
     uint32_t pre[NPRE];
 #pragma unroll
     for (int r = 0; r < NPRE; ++r) pre[r] = (have_masks && tid + r * NT < nwg) ? p.gmask[moff + tid + r * NT] : 0u;
@@ -174,11 +184,13 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
     const double xi = p.sx[i], yi = p.sy[i], zi = p.sz[i];
     const int32_t* row = p.nbr + (size_t)i * p.stride;
     const double eta0 = prog->ang_eta[0];
-    const int neta = Spec::FREE_ETA ? prog->n_eta : Spec::NETA;
     constexpr bool tiny = TINY;                      // exp(-eta_0 r^2) without range reduction (mathfn.cuh exp_tiny)
     if ((prog->tiny_exp != 0) != TINY) return;       // uniform per CTA: the other instantiation owns this element
+    // radial forces: first pass only; with cutoff radii per symmetry function (ElemProgram::per_sf_rc) they are left to
+    // the generic kernel's radial-only mode (k_force.cu) -- this kernel stages ONE fc per neighbour
+    const bool radial_here = first_pass && prog->per_sf_rc == 0;
     for (int e = 0; e < p.n_elem; ++e) {
-        const int nr = prog->n_rad[e], off = prog->rad_off[e];
+        const int nr = radial_here ? prog->n_rad[e] : 0, off = prog->rad_off[e];
         for (int m = seg[e] + tid; m < seg[e + 1]; m += NT) {
             const int j = row[m];
             const double dx = min_image_1d(xi, p.sx[j], p.box[0], p.half[0]);
@@ -187,15 +199,16 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
             const double a2 = fma(dx, dx, fma(dy, dy, dz * dz));
             const double ia = rsqrt(a2);
             const double a = a2 * ia;
-            double Ca, Sa;
-            cos_sinc(a2 * p.k2, Ca, Sa);
+            const bool in = !own_rc || a2 < rc2p;               // beyond the pass's radius: fc = 0, and out of the screening
+            double Ca = 0.0, Sa = 0.0;
+            if (in) cos_sinc(a2 * k2p, Ca, Sa);
             const double fa = Ca * Ca;                          // fc(a)
-            const double dfa_a = (-2.0 * p.k2) * (Ca * Sa);     // fc'(a)/a
+            const double dfa_a = (-2.0 * k2p) * (Ca * Sa);      // fc'(a)/a
             p0[m] = mk2((R)dx, (R)dy);
             p1[m] = mk2((R)dz, (R)ia);
             p2[m] = mk2((R)fa, (R)dfa_a);
             e0[m] = (R)(Spec::FREE_ETA ? a2 : (tiny ? exp_tiny(-eta0 * a2) : exp_small(-eta0 * a2)));   // FREE_ETA: a^2 itself
-            f32[m] = make_float4((float)dx, (float)dy, (float)dz, 0.f);
+            f32[m] = in ? make_float4((float)dx, (float)dy, (float)dz, 0.f) : make_float4(1e9f * (float)(m + 1), 0.f, 0.f, 0.f);
             double Rs = 0.0;
             for (int r = 0; r < nr; ++r) {
                 const RadialSF f = prog->rad[off + r];
@@ -212,7 +225,7 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
 #pragma unroll
             for (int e = 0; e < Spec::NETA; ++e) {
                 if (Spec::mask(e) >> tid & 1u) {
-                    const int g = prog->ang_g[pr][e][tid];
+                    const int g = Spec::FREE_ETA ? ps->g[pr][e][tid] : prog->ang_g[pr][e][tid];
                     const int zeta = 1 << (tid & 7);
                     const double lam = tid < 8 ? 1.0 : -1.0;
                     const double bc = g >= 0 ? brow[g] * exp2((double)(1 - zeta)) : 0.0;
@@ -229,11 +242,11 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
         }
     }
     int NW = 0;
-    const int ng = build_groups<true>(seg, p.n_elem, prog->n_ang, tab, tid, NW);
+    const int ng = build_groups<true>(seg, p.n_elem, n_ang, tab, tid, NW);
     __syncthreads();
 
     // ---- screening -> masks; prefix; even split of the triplet stream over the NT threads ------------
-    const float rc2f = (float)(p.rc2 * (1.0 + 1e-5));
+    const float rc2f = (float)(rc2p * (1.0 + 1e-5));
     if (have_masks) {
         // masks arrive in the SF kernel's group-major order; place them j-major and rebuild the descriptors
 #pragma unroll
@@ -269,8 +282,8 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
     // ---- angular part: every lane walks its range of the stream ---------------------------------------
     R eta[Spec::NETA];
 #pragma unroll
-    for (int e = 0; e < Spec::NETA; ++e) eta[e] = (R)prog->ang_eta[e];
-    const R eta0r = (R)eta0, k2r = (R)p.k2, rc2r = (R)p.rc2, m2k2 = (R)(-2.0 * p.k2);
+    for (int e = 0; e < Spec::NETA; ++e) eta[e] = (R)(Spec::FREE_ETA ? ps->eta[e] : prog->ang_eta[e]);
+    const R eta0r = (R)eta0, k2r = (R)k2p, rc2r = (R)rc2p, m2k2 = (R)(-2.0 * k2p);
     JData<R> J;
     J.ux = J.uy = J.uz = (R)1; J.ia = (R)1; J.fa = (R)0; J.dfa = (R)0; J.e0 = (R)1;
     int jcur = -1, paircur = -1;
@@ -516,10 +529,11 @@ static int launch_one2(const Force2Params& p, cudaStream_t st) {
 
 // launches the fast kernels for the specialised variants in use; the caller has zeroed f_sorted
 int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                  const int* variant, double rc, int stride, int max_nbr, int g_stride, int precision, cudaStream_t st) {
+                  const int* variant, const PassInfo& passes, double rc, int stride, int max_nbr, int g_stride, int precision,
+                  cudaStream_t st) {
     if (n == 0) return 0;
     Force2Params p;
-    p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride;
+    p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride; p.pass = 0;
     p.rc = rc; p.rc2 = rc * rc;
     p.k2 = (3.14159265358979323846 / (2.0 * rc)) * (3.14159265358979323846 / (2.0 * rc));
     for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
@@ -540,8 +554,15 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
     if (use[ANG_BASE12][0]) launches += launch_one2<SpecBase12, false>(p, st);
     if (use[ANG_WIDE32][1]) launches += f32 ? launch_one2<SpecWide32, true, float>(p, st) : launch_one2<SpecWide32, true>(p, st);
     if (use[ANG_WIDE32][0]) launches += launch_one2<SpecWide32, false>(p, st);
-    if (use[ANG_FREE32][0]) launches += launch_one2<SpecFree32, false>(p, st);
-    if (use[ANG_FREE16][0]) launches += launch_one2<SpecFree16, false>(p, st);
+    // free-eta tables: one launch per pass and kernel (the CTAs of elements without that pass return at once)
+    for (int q = 0; q < MAX_PASS; ++q) {
+        bool f32p = false, f16p = false;
+        for (int e = 0; e < n_elem; ++e)
+            if (q < passes.n_pass[e]) { f32p |= passes.spec[e][q] == ANG_FREE32; f16p |= passes.spec[e][q] == ANG_FREE16; }
+        p.pass = q;
+        if (f32p) launches += launch_one2<SpecFree32, false>(p, st);
+        if (f16p) launches += launch_one2<SpecFree16, false>(p, st);
+    }
     return launches;
 }
 

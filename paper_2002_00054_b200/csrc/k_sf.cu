@@ -24,6 +24,7 @@ struct SfParams {
     double* G;
     const ElemProgram* prog[MAX_ELEM];
     int variant[MAX_ELEM];
+    int radial_only[MAX_ELEM];           // 1: run only the radial block for this element (per-SF radial radii of a lane-owned element)
 };
 
 template <class Spec>
@@ -97,7 +98,10 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
     int tc = 0;
     for (int e = 1; e < p.n_elem; ++e)
         if (i >= p.cell_start[(size_t)e * p.ncell]) tc = e;
-    if (p.variant[tc] != Spec::ID) return;
+    // radial_only: an element of the lane-owned kernels whose RADIAL functions carry their own cutoff radii -- those
+    // kernels then leave the radial block to this one (they stage one fc per neighbour), the angular part stays theirs
+    const bool radial_only = p.radial_only[tc] != 0;
+    if (p.variant[tc] != Spec::ID && !radial_only) return;
     const ElemProgram* __restrict__ prog = p.prog[tc];
 
     const int capa = (p.cap + 3) & ~3;
@@ -148,7 +152,8 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
     __syncwarp();
 
     double* Grow = p.G + (size_t)i * p.g_stride;
-    for (int s = prog->n_sf + lane; s < p.g_stride; s += 32) Grow[s] = 0.0;
+    if (!radial_only)
+        for (int s = prog->n_sf + lane; s < p.g_stride; s += 32) Grow[s] = 0.0;
 
     // ---- radial: G = sum_j exp(-eta (a - rs)^2) fc(a) over the neighbours of element e ----------
     for (int e = 0; e < p.n_elem; ++e) {
@@ -171,6 +176,7 @@ __global__ void __launch_bounds__(SF_WARPS * 32) k_sf(const __grid_constant__ Sf
         }
     }
 
+    if (radial_only) return;                          // warp-uniform
     // ---- angular groups -----------------------------------------------------------------------
     const float rc2f = screen_rc2(p.rc2);
     for (int e1 = 0; e1 < p.n_elem; ++e1)
@@ -206,7 +212,8 @@ static int launch_one(const SfParams& p, cudaStream_t st) {
 }
 
 int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-              const int* variant, double rc, int stride, int max_nbr, int g_stride, int na_max, int precision, cudaStream_t st) {
+              const int* variant, const PassInfo& passes, double rc, int stride, int max_nbr, int g_stride, int na_max,
+              int precision, cudaStream_t st) {
     if (n == 0) return 0;
     SfParams p;
     p.na_max = na_max;
@@ -220,11 +227,13 @@ int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const El
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
         p.variant[e] = e < n_elem ? (variant[e] & 255) : -1;      // bit 8 = tiny_exp flag (fast launchers)
+        p.radial_only[e] = (e < n_elem && (variant[e] & 255) != ANG_GENERIC && passes.radial_own[e]) ? 1 : 0;
         if (e < n_elem) use[variant[e] & 255] = true;
+        if (p.radial_only[e]) use[ANG_GENERIC] = true;
     }
     int launches = 0;
-    if (use[ANG_BASE12] || use[ANG_WIDE32] || use[ANG_FREE32] || use[ANG_FREE16])     // specialised tables: lane-owned design (k_sf2.cu)
-        launches += launch_sf2(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, precision, st);
+    if (use[ANG_BASE12] || use[ANG_WIDE32] || use[ANG_FREE32] || use[ANG_FREE16] || use[ANG_MULTI])     // specialised tables: lane-owned design (k_sf2.cu)
+        launches += launch_sf2(w, g, n, n_elem, d_prog, variant, passes, rc, stride, max_nbr, g_stride, precision, st);
     if (use[ANG_GENERIC]) launches += launch_one<SpecGeneric>(p, st);
     return launches;
 }

@@ -14,6 +14,7 @@ namespace nnp {
 struct Sf2Params {
     int64_t n;
     int n_elem, ncell, stride, cap, g_stride;
+    int pass;                            // free-eta kernels: which AngPass of the element's program this launch evaluates
     double rc, rc2, k2;                  // k2 = (pi / (2 rc))^2
     double box[3], half[3];
     const double *sx, *sy, *sz;
@@ -65,8 +66,16 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
     int tc = 0;
     for (int e = 1; e < p.n_elem; ++e)
         if (i >= p.cell_start[(size_t)e * p.ncell]) tc = e;
-    if (p.variant[tc] != Spec::ID) return;          // uniform per CTA
+    if (p.variant[tc] != Spec::ID && !(Spec::FREE_ETA && p.variant[tc] == ANG_MULTI)) return;          // uniform per CTA
     const ElemProgram* __restrict__ prog = p.prog[tc];
+    // free-eta kernels: one launch per pass (nnp_internal.h AngPass); BASELINE.json's shapes: one sweep at the global rc
+    const AngPass* __restrict__ ps = &prog->pass[Spec::FREE_ETA ? p.pass : 0];
+    if (Spec::FREE_ETA && (p.pass >= prog->n_pass || ps->spec != Spec::ID)) return;
+    const bool own_rc = Spec::FREE_ETA && ps->own_rc != 0;          // the pass's cutoff is shorter than the neighbour list's
+    const double rc2p = Spec::FREE_ETA ? ps->rc2 : p.rc2, k2p = Spec::FREE_ETA ? ps->k2 : p.k2;
+    const int32_t* __restrict__ n_ang = Spec::FREE_ETA ? ps->n_ang : prog->n_ang;
+    const bool first_pass = !Spec::FREE_ETA || p.pass == 0;         // the radial block and the tail of the G row
+    const bool handover = !Spec::FREE_ETA || (prog->n_pass == 1 && !own_rc);   // masks to the force kernel
 
     constexpr int capa = CAPA;
     const int npair = p.n_elem * (p.n_elem + 1) / 2;
@@ -94,11 +103,11 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
     const double xi = p.sx[i], yi = p.sy[i], zi = p.sz[i];
     const int32_t* row = p.nbr + (size_t)i * p.stride;
     const double eta0 = prog->ang_eta[0];
-    const int neta = Spec::FREE_ETA ? prog->n_eta : Spec::NETA;
+    const int neta = Spec::FREE_ETA ? ps->n_eta : Spec::NETA;
     R etav[Spec::FREE_ETA ? Spec::NETA : 1];
     if constexpr (Spec::FREE_ETA)
-        for (int e = 0; e < Spec::NETA; ++e) etav[e] = (R)prog->ang_eta[e];
-    const R eta0r = (R)eta0, k2r = (R)p.k2, rc2r = (R)p.rc2;
+        for (int e = 0; e < Spec::NETA; ++e) etav[e] = (R)ps->eta[e];
+    const R eta0r = (R)eta0, k2r = (R)k2p, rc2r = (R)rc2p;
     constexpr bool tiny = TINY;                      // exp(-eta_0 r^2) without range reduction (mathfn.cuh exp_tiny)
     if ((prog->tiny_exp != 0) != TINY) return;       // uniform per CTA: the other instantiation owns this element
     for (int m = tid; m < ntot; m += NT) {
@@ -108,24 +117,27 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
         const double dz = min_image_1d(zi, p.sz[j], p.box[2], p.half[2]);
         const double a2 = fma(dx, dx, fma(dy, dy, dz * dz));
         const double ia = rsqrt(a2);
-        const double Ca = cos_only(a2 * p.k2);
+        const bool in = !own_rc || a2 < rc2p;                // beyond the pass's radius: fc = 0, and out of the screening
+        const double Ca = in ? cos_only(a2 * k2p) : 0.0;
         p0[m] = sf_mk2((R)dx, (R)dy);
         p1[m] = sf_mk2((R)dz, (R)ia);
         // first component: exp(-eta_0 a^2), or a^2 itself where every eta gets its own exponential (FREE_ETA)
         p2[m] = sf_mk2((R)(Spec::FREE_ETA ? a2 : (tiny ? exp_tiny(-eta0 * a2) : exp_small(-eta0 * a2))), (R)(Ca * Ca));
         ra[m] = a2 * ia;
-        f32[m] = make_float4((float)dx, (float)dy, (float)dz, 0.f);
+        f32[m] = in ? make_float4((float)dx, (float)dy, (float)dz, 0.f) : make_float4(1e9f * (float)(m + 1), 0.f, 0.f, 0.f);
     }
     for (int s = tid; s < (WPC + 1) * npair * NACC; s += NT) gacc[s] = 0.0;
     int NW = 0;
-    const int ng = build_groups<false>(seg, p.n_elem, prog->n_ang, tab, tid, NW);
+    const int ng = build_groups<false>(seg, p.n_elem, n_ang, tab, tid, NW);
     __syncthreads();
 
     double* Grow = p.G + (size_t)i * p.g_stride;
-    for (int s = prog->n_sf + tid; s < p.g_stride; s += NT) Grow[s] = 0.0;
+    if (first_pass)
+        for (int s = prog->n_sf + tid; s < p.g_stride; s += NT) Grow[s] = 0.0;
 
     // ---- radial: G = sum_j exp(-eta (a - rs)^2) fc(a) over the neighbours of element e; one warp per SF
-    for (int e = 0; e < p.n_elem; ++e) {
+    // (first pass only; with cutoff radii per symmetry function the generic kernel's radial-only mode does it, k_sf.cu)
+    for (int e = 0; e < ((first_pass && prog->per_sf_rc == 0) ? p.n_elem : 0); ++e) {
         const int nr = prog->n_rad[e], off = prog->rad_off[e];
         for (int r = wid; r < nr; r += WPC) {
             const RadialSF f = prog->rad[off + r];
@@ -140,13 +152,13 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
     }
 
     // ---- screening -> masks; prefix; even split of the triplet stream over the NT threads ------------
-    const float rc2f = (float)(p.rc2 * (1.0 + 1e-5));
+    const float rc2f = (float)(rc2p * (1.0 + 1e-5));
     for (int g = 0; g < ng; ++g) screen_group(tab[g], f32, words, rc2f, tid, NT);
     __syncthreads();
     // hand the masks to the force kernel (this kernel's group-major order), if they fit the budget
     {
         const int64_t off = p.word_off[i];
-        if (off + NW <= p.gmask_cap)
+        if (handover && off + NW <= p.gmask_cap)
             for (int x = tid; x < NW; x += NT) p.gmask[off + x] = words[x].x;
     }
     const int T = mask_prefix(words, C, NW, tid, NT, wsum);
@@ -252,8 +264,8 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
             if (ee < e) a += __popc(mk);
             else if (ee == e) { a += __popc(mk & ((1u << b) - 1u)); on = (mk >> b) & 1u; }
         }
-        if (!on || prog->n_ang[pr] == 0) continue;
-        const int g = prog->ang_g[pr][e][b];
+        if (!on || n_ang[pr] == 0) continue;
+        const int g = Spec::FREE_ETA ? ps->g[pr][e][b] : prog->ang_g[pr][e][b];
         if (g >= 0) {
             double tot = gacc[pr * NACC + a];
 #pragma unroll
@@ -320,10 +332,11 @@ static int launch_one_sf2(const Sf2Params& p, cudaStream_t st) {
 
 // launches the fast kernels for the specialised variants in use
 int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-               const int* variant, double rc, int stride, int max_nbr, int g_stride, int precision, cudaStream_t st) {
+               const int* variant, const PassInfo& passes, double rc, int stride, int max_nbr, int g_stride, int precision,
+               cudaStream_t st) {
     if (n == 0) return 0;
     Sf2Params p;
-    p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride;
+    p.n = n; p.n_elem = n_elem; p.ncell = g.ncell; p.stride = stride; p.cap = max_nbr; p.g_stride = g_stride; p.pass = 0;
     p.rc = rc; p.rc2 = rc * rc;
     p.k2 = (3.14159265358979323846 / (2.0 * rc)) * (3.14159265358979323846 / (2.0 * rc));
     for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
@@ -342,8 +355,15 @@ int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const E
     if (use[ANG_BASE12][0]) launches += launch_one_sf2<SpecBase12, false>(p, st);
     if (use[ANG_WIDE32][1]) launches += f32 ? launch_one_sf2<SpecWide32, true, float>(p, st) : launch_one_sf2<SpecWide32, true>(p, st);
     if (use[ANG_WIDE32][0]) launches += launch_one_sf2<SpecWide32, false>(p, st);
-    if (use[ANG_FREE32][0]) launches += launch_one_sf2<SpecFree32, false>(p, st);
-    if (use[ANG_FREE16][0]) launches += launch_one_sf2<SpecFree16, false>(p, st);
+    // free-eta tables: one launch per pass and kernel (the CTAs of elements without that pass return at once)
+    for (int q = 0; q < MAX_PASS; ++q) {
+        bool f32p = false, f16p = false;
+        for (int e = 0; e < n_elem; ++e)
+            if (q < passes.n_pass[e]) { f32p |= passes.spec[e][q] == ANG_FREE32; f16p |= passes.spec[e][q] == ANG_FREE16; }
+        p.pass = q;
+        if (f32p) launches += launch_one_sf2<SpecFree32, false>(p, st);
+        if (f16p) launches += launch_one_sf2<SpecFree16, false>(p, st);
+    }
     return launches;
 }
 

@@ -25,6 +25,7 @@ struct nnp_model {
     std::vector<ElemProgram> h_prog;             // host copies as built by nnp_create (global rc, specialised variants)
     std::vector<std::pair<int, int>> sf_loc;     // per SF of the nnp_create table: (central element, position in its G)
     int variant[MAX_ELEM] = {0, 0, 0, 0};
+    PassInfo passes;                 // free-eta passes per element (launchers)
     NetDesc nets[MAX_ELEM];
     double* d_weights[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
     double* d_scaling[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
@@ -60,6 +61,15 @@ static thread_local std::string g_create_err = "";   // nnp_last_error(NULL): pe
 static double k2_of(double rc) {
     const double t = 3.14159265358979323846 / (2.0 * rc);
     return t * t;
+}
+
+static void set_pass_info(nnp_model* m, const std::vector<ElemProgram>& progs) {
+    std::memset(&m->passes, 0, sizeof(m->passes));
+    for (int c = 0; c < m->n_elem; ++c) {
+        m->passes.n_pass[c] = progs[c].n_pass;
+        m->passes.radial_own[c] = progs[c].per_sf_rc;
+        for (int q = 0; q < progs[c].n_pass; ++q) m->passes.spec[c][q] = progs[c].pass[q].spec;
+    }
 }
 
 static nnp_status fail(nnp_model* m, nnp_status s, const std::string& msg) {
@@ -194,42 +204,113 @@ static bool match_spec(const std::vector<std::vector<AngularSF>>& groups, ElemPr
     return true;
 }
 
-// Any table with <= 4 distinct eta values, lambda = +-1, zeta in {1, 2, 4, 16} and no (eta, lambda, zeta) twice in a pair
-// group runs on SpecFree32: the eta slots are the sorted distinct values (padded with the last one), missing menu
-// entries get no G index (the kernels then skip them / use a zero coefficient).
-static bool match_free32(const std::vector<std::vector<AngularSF>>& groups, ElemProgram* P) {
-    std::vector<double> etas;
+// Free-eta passes (nnp_internal.h AngPass): any table of NARROW angular symmetry functions with lambda = +-1,
+// zeta in {1, 2, 4, 16} and no (rc, eta, lambda, zeta) twice in a pair group.  The symmetry functions are split by
+// cutoff radius (descending) and, inside a radius, into chunks of at most four eta values of about equal size; one
+// pass per chunk.  Returns false if the table does not fit (another zeta, a wide SF, more than MAX_PASS passes, an
+// exponent beyond exp_small's range).
+static bool build_passes(const std::vector<std::vector<AngularSF>>& groups, double rc, ElemProgram* P) {
+    struct Key { double rc2, eta, k2; };
+    std::vector<Key> keys;
     for (const auto& grp : groups)
         for (const auto& f : grp) {
+            if (f.wide) return false;
+            bool zok = false;
+            for (int b = 0; b < 7; ++b) zok |= (f.izeta == (1 << b)) && ((SpecFree32::mask(0) >> b) & 1u);
+            if (!zok) return false;
+            if (f.eta * 3.0 * f.rc2 > 700.0) return false;
             bool seen = false;
-            for (double e : etas) seen |= (e == f.eta);
-            if (!seen) etas.push_back(f.eta);
+            for (const Key& k : keys) seen |= (k.rc2 == f.rc2 && k.eta == f.eta);
+            if (!seen) keys.push_back(Key{f.rc2, f.eta, f.k2});
         }
-    if (etas.empty() || (int)etas.size() > SpecFree32::NETA) return false;
-    for (size_t a = 0; a < etas.size(); ++a)
-        for (size_t b = a + 1; b < etas.size(); ++b)
-            if (etas[b] < etas[a]) std::swap(etas[a], etas[b]);
-    for (int e = 0; e < MAX_ETA; ++e) P->ang_eta[e] = e < (int)etas.size() ? etas[e] : etas.back();
-    P->n_eta = (int)etas.size();
-    for (size_t p = 0; p < groups.size(); ++p) {
-        for (int e = 0; e < MAX_ETA; ++e)
-            for (int b = 0; b < 16; ++b) P->ang_g[p][e][b] = -1;
-        unsigned seen[MAX_ETA] = {0, 0, 0, 0};
-        for (const auto& f : groups[p]) {
-            int e = -1;
-            for (int q = (int)etas.size() - 1; q >= 0; --q)
-                if (etas[q] == f.eta) e = q;
-            int bit = -1;
-            for (int b = 0; b < 7; ++b)
-                if (f.izeta == (1 << b)) bit = b;
-            if (e < 0 || bit < 0) return false;
-            if (f.lam < 0) bit += 8;
-            if (!(SpecFree32::mask(e) >> bit & 1u) || (seen[e] >> bit & 1u)) return false;
-            seen[e] |= 1u << bit;
-            P->ang_g[p][e][bit] = (int16_t)f.g;
+    if (keys.empty()) return false;
+    for (size_t x = 0; x < keys.size(); ++x)                  // sort: rc descending, eta ascending
+        for (size_t y = x + 1; y < keys.size(); ++y)
+            if (keys[y].rc2 > keys[x].rc2 || (keys[y].rc2 == keys[x].rc2 && keys[y].eta < keys[x].eta)) std::swap(keys[x], keys[y]);
+    int np = 0;
+    size_t x = 0;
+    while (x < keys.size()) {
+        size_t y = x;
+        while (y < keys.size() && keys[y].rc2 == keys[x].rc2) ++y;
+        const int n = (int)(y - x), chunks = (n + MAX_ETA - 1) / MAX_ETA;
+        const int class_first = np;
+        for (int c = 0; c < chunks; ++c) {
+            if (np >= MAX_PASS) return false;
+            const int lo = (int)x + (n * c) / chunks, hi = (int)x + (n * (c + 1)) / chunks;
+            AngPass& ps = P->pass[np++];
+            std::memset(&ps, 0, sizeof(ps));
+            ps.n_eta = hi - lo;
+            for (int e = 0; e < MAX_ETA; ++e) ps.eta[e] = keys[lo + (e < ps.n_eta ? e : ps.n_eta - 1)].eta;
+            ps.rc2 = keys[lo].rc2;
+            ps.k2 = keys[lo].k2;                            // k2_of(rc_p), as stored with the symmetry function
+            ps.own_rc = ps.rc2 != rc * rc ? 1 : 0;
+            ps.spec = ps.n_eta <= SpecFree16::NETA ? ANG_FREE16 : ANG_FREE32;
+            for (size_t pr = 0; pr < groups.size(); ++pr) {
+                for (int e = 0; e < MAX_ETA; ++e)
+                    for (int b = 0; b < 16; ++b) ps.g[pr][e][b] = -1;
+                for (const auto& f : groups[pr]) {
+                    if (f.rc2 != ps.rc2) continue;
+                    int e = -1;
+                    for (int q = ps.n_eta - 1; q >= 0; --q)
+                        if (ps.eta[q] == f.eta) e = q;
+                    if (e < 0) continue;
+                    int bit = 0;
+                    while ((1 << bit) != f.izeta) ++bit;
+                    if (f.lam < 0) bit += 8;
+                    if (ps.g[pr][e][bit] >= 0) return false;    // the same (rc, eta, lambda, zeta) twice in a pair group
+                    ps.g[pr][e][bit] = (int16_t)f.g;
+                    ps.n_ang[pr] += 1;
+                }
+            }
         }
+        (void)class_first;     // (an in-kernel loop over the passes of one radius was measured: +7 % on single-pass tables for
+                               //  the loop structure, -3 % on a three-pass table -- the triplet loops dominate, not the staging)
+        x = y;
     }
+    P->n_pass = np;
     return true;
+}
+
+// Choice of kernels for one element from its complete program (lists, per-SF radii); nnp_create and
+// nnp_set_sf_cutoffs both end here.  Sets variant, tiny_exp, per_sf_rc and the pass tables.
+static nnp_status select_variant(ElemProgram& P, int n_elem, double rc, std::string& err) {
+    const int npair = n_elem * (n_elem + 1) / 2;
+    std::vector<std::vector<AngularSF>> groups(npair);
+    bool own_ang = false, own_rad = false, any_ang = false;
+    int nr = 0;
+    for (int e = 0; e < n_elem; ++e) nr += P.n_rad[e];
+    for (int r = 0; r < nr; ++r) own_rad |= P.rad[r].rc2 != rc * rc;
+    for (int p = 0; p < npair; ++p)
+        for (int a = 0; a < P.n_ang[p]; ++a) {
+            groups[p].push_back(P.ang[P.ang_off[p] + a]);
+            own_ang |= groups[p].back().rc2 != rc * rc;
+            any_ang = true;
+        }
+    P.per_sf_rc = (own_ang || own_rad) ? 1 : 0;
+    P.variant = ANG_GENERIC;
+    P.n_pass = 0;
+    P.tiny_exp = 0;
+    if (!any_ang) return NNP_OK;
+    // the specialised kernels use exp_small() unclamped: its argument -eta (a^2+b^2+c^2) must stay > -700
+    double eta_max = 0.0;
+    bool any_wide = false;           // wide angular SFs run on the generic kernels only
+    for (int p = 0; p < npair; ++p)
+        for (const auto& f : groups[p]) { eta_max = std::fmax(eta_max, f.eta); any_wide |= f.wide != 0; }
+    const bool in_range = !any_wide && eta_max * 3.0 * rc * rc <= 700.0;
+    if (in_range && !own_ang && match_spec<SpecBase12>(groups, &P)) P.variant = ANG_BASE12;
+    else if (in_range && !own_ang && match_spec<SpecWide32>(groups, &P)) P.variant = ANG_WIDE32;
+    else if (!any_wide && build_passes(groups, rc, &P))
+        P.variant = (P.n_pass == 1 && !P.pass[0].own_rc) ? P.pass[0].spec : ANG_MULTI;
+    else {
+        P.n_pass = 0;
+        for (int p = 0; p < npair; ++p)
+            if (P.n_ang[p] > 64) {
+                err = "generic angular path supports <= 64 SFs per pair group";
+                return NNP_ERR_LIMIT;
+            }
+    }
+    P.tiny_exp = ((P.variant == ANG_BASE12 || P.variant == ANG_WIDE32) && P.ang_eta[0] * rc * rc * (1.0 + 1e-5) <= 0.05) ? 1 : 0;
+    return NNP_OK;
 }
 
 // Host side of nnp_create: validate the SF table and build every element's program, including the choice of
@@ -298,25 +379,8 @@ static nnp_status build_tables(int n_elem, double rc, int n_sf, const nnp_sf* sf
             if (ao + P.n_ang[p] > MAX_ANG_TOTAL) return lfail("more than 512 angular SFs for one element");
             for (const auto& f : ang[c][p]) P.ang[ao++] = f;
         }
-        bool any_ang = ao > 0;
-        P.variant = ANG_GENERIC;
-        if (any_ang) {
-            // the specialised kernels use exp_small() unclamped: its argument -eta (a^2+b^2+c^2) must stay > -700
-            double eta_max = 0.0;
-            bool any_wide = false;           // wide angular SFs run on the generic kernels only
-            for (int p = 0; p < npair; ++p)
-                for (const auto& f : ang[c][p]) { eta_max = std::fmax(eta_max, f.eta); any_wide |= f.wide != 0; }
-            const bool in_range = !any_wide && eta_max * 3.0 * rc * rc <= 700.0;
-            if (in_range && match_spec<SpecBase12>(ang[c], &P)) P.variant = ANG_BASE12;
-            else if (in_range && match_spec<SpecWide32>(ang[c], &P)) P.variant = ANG_WIDE32;
-            else if (in_range && match_free32(ang[c], &P)) P.variant = P.n_eta <= SpecFree16::NETA ? ANG_FREE16 : ANG_FREE32;
-            else {
-                for (int p = 0; p < npair; ++p)
-                    if (P.n_ang[p] > 64)
-                        return lfail("generic angular path supports <= 64 SFs per pair group");
-            }
-        }
-        P.tiny_exp = (P.variant != ANG_GENERIC && P.variant != ANG_FREE32 && P.variant != ANG_FREE16 && P.ang_eta[0] * rc * rc * (1.0 + 1e-5) <= 0.05) ? 1 : 0;
+        const nnp_status vs = select_variant(P, n_elem, rc, err);
+        if (vs != NNP_OK) return vs;
     }
     return NNP_OK;
 }
@@ -457,6 +521,7 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
             return bail(NNP_ERR_CUDA, "cudaMalloc failed");
     }
     m->h_prog = progs;
+    set_pass_info(m, progs);
     {
         int cnt[MAX_ELEM] = {0, 0, 0, 0};
         for (int s = 0; s < n_sf; ++s) m->sf_loc.push_back({sf[s].central, cnt[sf[s].central]++});
@@ -532,13 +597,13 @@ extern "C" nnp_status nnp_set_sf_cutoffs(nnp_model* m, int32_t n_sf, const doubl
             P.ang[a].k2 = k2_of(x);
             own |= x != m->rc;
         }
-        if (own) {             // the specialised kernels stage ONE fc per neighbour: such an element runs on the generic ones
-            for (int p = 0; p < npair; ++p)
-                if (P.n_ang[p] > 64) return fail(m, NNP_ERR_INVALID_ARG, "generic angular path supports <= 64 SFs per pair group");
-            P.per_sf_rc = 1;
-            P.variant = ANG_GENERIC;
-            P.tiny_exp = 0;
-        }
+        (void)own;
+        // radii on angular symmetry functions: free-eta passes, one cutoff radius per pass, if the table fits them,
+        // else the generic kernels; radii on radial functions only: the element keeps its kernels (their radial block
+        // evaluates fc per symmetry function)
+        std::string verr;
+        const nnp_status vs = select_variant(P, m->n_elem, m->rc, verr);
+        if (vs != NNP_OK) return fail(m, vs, verr);
     }
     DeviceGuard dg(m->device);
     if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
@@ -547,6 +612,7 @@ extern "C" nnp_status nnp_set_sf_cutoffs(nnp_model* m, int32_t n_sf, const doubl
         NNP_CUDA(m, cudaMemcpy(m->d_prog[c], &progs[c], sizeof(ElemProgram), cudaMemcpyHostToDevice));
         m->variant[c] = progs[c].variant | (progs[c].tiny_exp << 8);
     }
+    set_pass_info(m, progs);
     return NNP_OK;
 }
 
@@ -660,11 +726,11 @@ extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d
     launches += launch_neighbors(w, g, n_atoms, m->n_elem, m->rc * m->rc, stride, m->max_nbr, st);
     mark(2);
     launches += launch_word_offsets(w, g, n_atoms, m->n_elem, m->d_prog, st);
-    launches += launch_sf(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->rc, stride, m->max_nbr, m->g_stride, m->na_max, m->precision, st);
+    launches += launch_sf(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->passes, m->rc, stride, m->max_nbr, m->g_stride, m->na_max, m->precision, st);
     mark(3);
     launches += launch_mlp(w, n_atoms, m->n_elem, g.ncell, m->nets, m->g_stride, st);
     mark(4);
-    launches += launch_force(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->rc, stride, m->max_nbr, m->g_stride, m->precision, st);
+    launches += launch_force(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->passes, m->rc, stride, m->max_nbr, m->g_stride, m->precision, st);
     mark(5);
     launches += launch_finalize(w, n_atoms, d_e_atom, d_e_total, d_force, st);
     mark(6);

@@ -46,7 +46,30 @@ struct AngularSF {
 
 // Angular kernel variants.  Specialised variants bake the (eta ratio, lambda, zeta) structure
 // of a pair group into the kernel; ANG_GENERIC walks the AngularSF list (any table).
-enum AngVariant : int { ANG_GENERIC = 0, ANG_BASE12 = 1, ANG_WIDE32 = 2, ANG_FREE32 = 3, ANG_FREE16 = 4, ANG_NVARIANT = 5 };
+enum AngVariant : int { ANG_GENERIC = 0, ANG_BASE12 = 1, ANG_WIDE32 = 2, ANG_FREE32 = 3, ANG_FREE16 = 4, ANG_MULTI = 5, ANG_NVARIANT = 6 };
+
+// One sweep of the free-eta lane-owned kernels (SpecFree16 / SpecFree32) over the triplets of a centre: up to four
+// eta values that share ONE cutoff radius.  A table with more eta values, or with angular symmetry functions of
+// several radii (n2p2 gives every symmetry function its own rc), runs as several passes -- G entries are
+// independent and the forces are additive over the symmetry functions.  ANG_FREE16 / ANG_FREE32 = one pass at the
+// global rc; ANG_MULTI = anything else that fits MAX_PASS passes.
+constexpr int MAX_PASS = 8;
+struct AngPass {
+    double eta[MAX_ETA];
+    double rc2, k2;                  // the pass's cutoff: rc_p^2, (pi / (2 rc_p))^2
+    int32_t n_eta;
+    int32_t spec;                    // ANG_FREE16 (<= 2 eta values) or ANG_FREE32
+    int32_t own_rc;                  // 1: rc_p differs from the global rc (slots beyond rc_p are switched off while staging)
+    int32_t pad;
+    int32_t n_ang[MAX_PAIR];         // symmetry functions of pair group p in this pass (0: the group is skipped)
+    int16_t g[MAX_PAIR][MAX_ETA][16];   // G index of menu entry (eta slot, bit); -1 = absent
+};
+// host-side summary for the launchers
+struct PassInfo {
+    int n_pass[MAX_ELEM];
+    int spec[MAX_ELEM][MAX_PASS];
+    int radial_own[MAX_ELEM];        // the element's radial functions carry their own cutoff radii (ElemProgram::per_sf_rc)
+};
 
 // Symmetry-function program of ONE central element; lives in device memory (model-owned).
 struct ElemProgram {
@@ -55,7 +78,8 @@ struct ElemProgram {
     int32_t variant;                 // AngVariant
     int32_t tiny_exp;                // specialised path: eta_0 rc^2 <= 0.05 -> exp_tiny() for exp(-eta_0 r^2)
     int32_t per_sf_rc;               // 1: some SF of this element has its own cutoff radius (nnp_set_sf_cutoffs); generic kernels
-    int32_t n_eta;                   // SpecFree32: distinct eta values in use (the slots beyond are skipped)
+    int32_t n_eta;                   // (unused since the passes; kept for layout)
+    int32_t n_pass;                  // free-eta kernels: passes in use (pass[0 .. n_pass))
     int32_t n_rad[MAX_ELEM];         // radial SFs for neighbour element e
     int32_t rad_off[MAX_ELEM];       // first index into rad[]
     int32_t n_ang[MAX_PAIR];         // angular SFs of pair group p
@@ -66,6 +90,7 @@ struct ElemProgram {
     int16_t ang_g[MAX_PAIR][MAX_ETA][16];
     RadialSF rad[MAX_RAD_TOTAL];
     AngularSF ang[MAX_ANG_TOTAL];
+    AngPass pass[MAX_PASS];
 };
 
 // Small networks (two hidden layers of width <= 32, <= 80 inputs) also travel in the KERNEL PARAMETER block
@@ -152,21 +177,25 @@ int launch_sort(const Workspace& w, const Grid& g, int64_t n, int n_elem, const 
 int launch_neighbors(const Workspace& w, const Grid& g, int64_t n, int n_elem, double rc2, int stride,
                      int max_nbr, cudaStream_t st);
 int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-              const int* variant, double rc, int stride, int max_nbr, int g_stride, int na_max, int precision, cudaStream_t st);
+              const int* variant, const PassInfo& passes, double rc, int stride, int max_nbr, int g_stride, int na_max,
+              int precision, cudaStream_t st);
 int launch_mlp(const Workspace& w, int64_t n, int n_elem, int ncell, const NetDesc* nets, int g_stride,
                cudaStream_t st);
 int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                 const int* variant, double rc, int stride, int max_nbr, int g_stride, int precision, cudaStream_t st);
+                 const int* variant, const PassInfo& passes, double rc, int stride, int max_nbr, int g_stride, int precision,
+                 cudaStream_t st);
 // mask words per centre + their prefix (k_sf2.cu); before launch_sf
 constexpr int WORD_BUDGET = 320;     // gmask capacity = N * WORD_BUDGET words (a water-like centre with 91 neighbours has 152)
 int launch_word_offsets(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
                         cudaStream_t st);
 // fast path of S2 (lane-owned design, k_sf2.cu): specialised variants only
 int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-               const int* variant, double rc, int stride, int max_nbr, int g_stride, int precision, cudaStream_t st);
+               const int* variant, const PassInfo& passes, double rc, int stride, int max_nbr, int g_stride, int precision,
+               cudaStream_t st);
 // fast path of S4 (lane-owned design, k_force2.cu): specialised variants only; f_sorted already zeroed
 int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                  const int* variant, double rc, int stride, int max_nbr, int g_stride, int precision, cudaStream_t st);
+                  const int* variant, const PassInfo& passes, double rc, int stride, int max_nbr, int g_stride, int precision,
+                  cudaStream_t st);
 int launch_finalize(const Workspace& w, int64_t n, double* d_e_atom, double* d_e_total, double* d_force,
                     cudaStream_t st);
 

@@ -101,8 +101,10 @@ def test_kernel_choice_per_table(lib):
     assert table_kernels(m) == ("generic", "base12")
     m = W.make_model(False)
     q = np.nonzero(ang)[0][:5]
-    m.sf["eta"][q] = [0.002, 0.003, 0.004, 0.005, 0.006]           # more than four eta values
-    assert table_kernels(m)[0] == "generic"
+    m.sf["eta"][q] = [0.002, 0.003, 0.004, 0.005, 0.006]           # more than four eta values: several passes of the free-eta kernels
+    assert table_kernels(m)[0] == "multi"
+    rows = [(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0)] + [(0, 3, 0, 0, 0.001 * (k + 1), 0.0, 1.0, 1.0) for k in range(33)]
+    assert table_kernels(tiny_model(rows)) == ("generic",)          # 33 eta values: more than 8 passes of four
     m = W.make_model(False)
     q = np.nonzero(ang)[0]
     m.sf["zeta"][q[1]] = m.sf["zeta"][q[0]]; m.sf["lam"][q[1]] = m.sf["lam"][q[0]]; m.sf["eta"][q[1]] = m.sf["eta"][q[0]]

@@ -170,6 +170,53 @@ def test_fast_path_free_eta_menu(n_elem, n_eta):
     _check_full(model, sysm, max_neighbors=255)
 
 
+def _n2p2_like_model(n_elem=2, seed=41):
+    """A table shaped like published n2p2 models (not one of them): zeta in {1, 4}, lambda = +-1, seven eta values,
+    angular functions of two cutoff radii, radial functions of three radii with shifts."""
+    rows, rcs = [], []
+    pairs = [(a, b) for a in range(n_elem) for b in range(a, n_elem)]
+    for c in range(n_elem):
+        for e1 in range(n_elem):
+            for k, (eta, rs, rr) in enumerate(((0.003, 0.0, 6.0), (0.03, 0.0, 6.0), (0.2, 1.0, 4.5), (0.6, 2.0, 3.5))):
+                rows.append((c, 2, e1, 0, eta, rs, 0.0, 0.0)); rcs.append(rr)
+        for (e1, e2) in pairs:
+            for ie, eta in enumerate((0.0005, 0.002, 0.004, 0.008, 0.015, 0.03, 0.07)):
+                for lam in (1.0, -1.0):
+                    for zeta in (1.0, 4.0):
+                        if (ie + (lam > 0) + int(zeta)) % 5 == 0:
+                            continue                         # holes
+                        rows.append((c, 3, e1, e2, eta, 0.0, lam, zeta)); rcs.append(6.0 if ie < 5 else 4.8)
+    model = tiny_model(rows, n_elem=n_elem, hidden=(12, 9), seed=seed)
+    model.sf_cutoffs = rcs
+    return model
+
+
+@pytest.mark.parametrize("n_elem", [1, 2, 3])
+def test_multi_pass_tables(n_elem):
+    # SURVEY.md 8(f)4: more than four eta values and angular functions of several cutoff radii on the lane-owned
+    # kernels, as several passes (NNP_KERNELS_MULTI) -- not on the queue-based generic ones
+    from paper_2002_00054_b200 import NNP
+    from paper_2002_00054_b200.binding import table_kernels
+    model = _n2p2_like_model(n_elem)
+    sysm = W.make_water(120, 5, L=15.0)
+    sysm.types = (np.arange(sysm.n_atoms) % n_elem).astype(np.int32)
+    import copy
+    plain = copy.deepcopy(model); plain.sf_cutoffs = None
+    assert set(table_kernels(plain)) == {"multi"}             # seven eta values: two passes even at one radius
+    _check_full(plain, sysm)
+    nnp = NNP.from_model(model)
+    assert nnp.uses_fast_path()
+    nnp.close()
+    _check_full(model, sysm)                                  # + radii: 5 eta at 6.0 A (2 passes) and 2 eta at 4.8 A (1 pass)
+    _check_full(model, sysm, max_neighbors=255)
+    # radii on RADIAL functions only: BASELINE.json's table keeps its specialised kernels
+    base = W.make_model(False)
+    rc2 = np.where((base.sf["kind"] == 2) & (np.arange(len(base.sf)) % 3 == 0), 0.7 * base.rc, base.rc)
+    base.sf_cutoffs = list(rc2)
+    s0, _ = W.build(W.CONFIGS[0])
+    _check_full(base, s0)
+
+
 def test_fast_path_large_cutoff_general_exp():
     # rc = 8 A: eta_0 rc^2 = 0.064 > 0.05, so the fast kernels take the range-reduced exp (the water-like
     # configs, rc = 6 A, run on the small-argument polynomial exp_tiny)
