@@ -326,6 +326,10 @@ def main():
                          "(queue-based generic kernels), 'n2p2like' is a table shaped like published n2p2 models (zeta in {1, 4}, "
                          "seven eta values, lambda = +-1, angular functions of two cutoff radii: 3 passes of the free-eta "
                          "kernels); the roofline object is then not meaningful")
+    ap.add_argument("--skin", type=float, default=0.0,
+                    help="probe of what a Verlet-skin neighbour list would cost the hot kernels: the neighbour list is built "
+                         "with rc + SKIN while every symmetry function keeps its cutoff (nnp_set_sf_cutoffs), i.e. exactly the "
+                         "list a skin scheme would hand the kernels on its reuse steps; the list is still rebuilt every call")
     ap.add_argument("--no-probe", action="store_true", help="skip the DFMA issue-rate probe (for ncu runs)")
     ap.add_argument("--no-sweep", action="store_true",
                     help="skip the short timed runs of configs[1], [2], [4] that the default line carries as config_sweep")
@@ -365,6 +369,11 @@ def main():
         if args.table == "generic":
             model.sf["zeta"][ang & (model.sf["zeta"] == 16.0)] = 3.0
         model.name += "+" + args.table
+    if args.skin > 0.0:
+        rc_sf = list(model.sf_cutoffs) if model.sf_cutoffs is not None else [model.rc] * len(model.sf)
+        model.rc = model.rc + args.skin
+        model.sf_cutoffs = rc_sf
+        model.name += "+skin%g" % args.skin
     n = sysm.n_atoms
     nnp = NNP.from_model(model, device=local)
     if args.precision != "f64":
@@ -474,7 +483,7 @@ def main():
     total_instr = instr["total"] * n
     hbm_bytes_per_atom = 1.0e3 if cfg.kind == "metal" else (2.8e3 if not cfg.wide else 5.2e3)
     ncu, ncu_src = _ncu_launch_metrics(args.config, "k_force2")
-    baseline_table = args.table == "baseline" and args.precision == "f64"
+    baseline_table = args.table == "baseline" and args.precision == "f64" and args.skin == 0.0
     roofline = {
         "bound": "alu", "kernel": "k_force2", "achieved": achieved / 1e12, "peak": peak_alu / 1e12,
         "unit": "T FP64 instr/s", "frac": achieved / peak_alu,
