@@ -379,7 +379,7 @@ def main():
     if args.precision != "f64":
         nnp.set_precision(args.precision)
     if cfg.kind == "metal":
-        nnp.set_max_neighbors(48)      # 18 neighbours per atom: the 64-slot, one-warp-per-centre kernels
+        nnp.set_max_neighbors(32)      # 18 neighbours per atom: the 8-lanes-per-centre kernels of k_small.cu
     pos = torch.tensor(sysm.pos, dtype=torch.float64, device=dev)
     typ = torch.tensor(sysm.types, dtype=torch.int32, device=dev)
     out = (torch.empty(n, dtype=torch.float64, device=dev), torch.empty(1, dtype=torch.float64, device=dev),

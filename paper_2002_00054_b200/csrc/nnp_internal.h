@@ -196,6 +196,11 @@ int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const E
 int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
                   const int* variant, const PassInfo& passes, double rc, int stride, int max_nbr, int g_stride, int precision,
                   cudaStream_t st);
+// small neighbourhoods (max_neighbors <= 32; k_small.cu): 8 lanes per centre, SpecBase12 elements
+int launch_sf_small(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
+                    const int* variant, double rc, int stride, int g_stride, bool tiny, cudaStream_t st);
+int launch_force_small(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
+                       const int* variant, double rc, int stride, int g_stride, bool tiny, cudaStream_t st);
 int launch_finalize(const Workspace& w, int64_t n, double* d_e_atom, double* d_e_total, double* d_force,
                     cudaStream_t st);
 

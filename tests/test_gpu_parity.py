@@ -253,6 +253,30 @@ def test_metal_like_small_neighbourhoods():
     sysm, model = W.build(W.Config("fcc6", 6, False, 1, 11, 12, None, "metal"))
     _check_full(model, sysm, max_neighbors=48)
     _check_full(model, sysm)                       # and the default 160-slot kernels on the same system
+    _check_full(model, sysm, max_neighbors=32)     # and the 8-lanes-per-centre kernels of k_small.cu
+
+
+@pytest.mark.parametrize("elements", [("X",), ("H", "O"), ("A", "B", "C")])
+def test_small_neighbourhood_kernels(elements):
+    # k_small.cu (max_neighbors <= 32): four centres per warp, exact pair test + compacted list; 1 - 3 elements, ragged
+    # last CTA (290 atoms are not a multiple of 8), a centre without any neighbour of one element, general exp (rc = 8 would
+    # not fit 32 slots, so the non-tiny variant is forced through eta instead)
+    import copy
+    from paper_2002_00054_b200 import NNP
+    model = W.make_model(False, seed=23, rc=3.2, elements=elements, hidden=(9, 6))
+    sysm = W.make_water(96, 77, L=14.2)
+    sysm.types = (np.arange(sysm.n_atoms) % len(elements)).astype(np.int32)
+    sysm.pos = np.concatenate([sysm.pos, [[7.1, 7.1, 7.1], [7.3, 7.0, 7.2]]])       # 290 atoms, one very close pair
+    sysm.types = np.concatenate([sysm.types, [0, len(elements) - 1]]).astype(np.int32)
+    nnp = NNP.from_model(model)
+    nnp.set_max_neighbors(32)
+    assert nnp.uses_fast_path()
+    nnp.close()
+    _check_full(model, sysm, max_neighbors=32)
+    big = copy.deepcopy(model)                      # eta_0 rc^2 > 0.05: the range-reduced exponential
+    ang = big.sf["kind"] == 3
+    big.sf["eta"][ang] *= 8.0
+    _check_full(big, sysm, max_neighbors=32)
 
 
 def test_wide_angular_mixed_with_narrow():
