@@ -300,8 +300,10 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg.name, "n_atoms": sysm.n_atoms, "model": model.name,
-                   "parallelism": "1 host core (single-threaded oracle)"},
+        # the same keys as the CUDA arm's config (workload, atoms and model are the same; the rest describes this arm)
+        "config": {"workload": cfg.name, "n_atoms": sysm.n_atoms, "model": model.name, "kernels": ["oracle"] * len(model.elements),
+                   "box": float(sysm.box[0]), "neighbor_rebuild": "every call (brute-force scan per centre)", "md": False,
+                   "parallelism": "1 host core (single-threaded oracle)", "l2": "n/a (host)"},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
