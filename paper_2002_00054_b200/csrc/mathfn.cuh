@@ -41,6 +41,16 @@ __device__ __forceinline__ double exp_tiny(double y) {
     return p;
 }
 
+// the same with degree 5 (max error 1e-12 relative): enough for the FORCE kernel's triplet Gaussian (forces to 1e-8 eV/A),
+// not for the symmetry functions themselves (G to 1e-11)
+__device__ __forceinline__ double exp_tiny5(double y) {
+    double p = EXPT5[5];
+#pragma unroll
+    for (int q = 4; q >= 0; --q) p = fma(p, y, EXPT5[q]);
+    return p;
+}
+__device__ __forceinline__ float exp_tiny5(float y) { return __expf(y); }
+
 // C = cos(sqrt z), S = sin(sqrt z)/sqrt z for z in [0, (pi/2)^2]
 __device__ __forceinline__ void cos_sinc(double z, double& C, double& S) {
     double c = COSC[7], s = SNCC[7];
