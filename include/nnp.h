@@ -175,7 +175,8 @@ nnp_status nnp_set_sf_cutoffs(nnp_model* m, int32_t n_sf, const double* h_rc);
  * its predicate, the minimum-image geometry, the radial symmetry functions, the networks, the reduction of the
  * symmetry-function sums over the lanes and every global force / energy accumulation stay FP64.  It applies to elements
  * whose table has one of BASELINE.json's two angular shapes (NNP_KERNELS_BASE12 / NNP_KERNELS_WIDE32) with
- * eta_0 rc^2 <= 0.05 and max_neighbors <= 160; every other element silently keeps FP64.  The results no longer meet
+ * eta_0 rc^2 <= 0.05 and 64 < max_neighbors (centres with more than 160 neighbours stay FP64); every other element
+ * silently keeps FP64.  The results no longer meet
  * BASELINE.json's tolerances (measured on the water-like configs: DESIGN.md section 6c); energies stay bit-reproducible. */
 #define NNP_PRECISION_F64 0
 #define NNP_PRECISION_MIXED 1
