@@ -41,8 +41,8 @@ __device__ __forceinline__ double exp_tiny(double y) {
     return p;
 }
 
-// the same with degree 5 (max error 1e-12 relative): enough for the FORCE kernel's triplet Gaussian (forces to 1e-8 eV/A),
-// not for the symmetry functions themselves (G to 1e-11)
+// the same with degree 5 (max error 1.0e-14 on [-0.05, 0]): the per-triplet Gaussian exp(-eta_0 c^2) of both hot kernels --
+// one DFMA less in the dependent chain of every triplet; the per-neighbour staging keeps degree 6
 __device__ __forceinline__ double exp_tiny5(double y) {
     double p = EXPT5[5];
 #pragma unroll
