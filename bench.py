@@ -487,8 +487,11 @@ def main():
     total_instr = instr["total"] * n
     hbm_bytes_per_atom = 1.0e3 if cfg.kind == "metal" else (2.8e3 if not cfg.wide else 5.2e3)
     # the dominant kernel: k_force2<...> (not its list-driven sibling for the few big centres), k_force_small on the metal workload
-    ncu, ncu_src = _ncu_launch_metrics(args.config, r"k_force2<|k_force_small<")
     baseline_table = args.table == "baseline" and args.precision == "f64" and args.skin == 0.0
+    if baseline_table:
+        ncu, ncu_src = _ncu_launch_metrics(args.config, r"k_force2<|k_force_small<")
+    else:
+        ncu, ncu_src = None, "the committed launch lists are of the FP64 run on BASELINE.json's tables"
     roofline = {
         "bound": "alu", "kernel": "k_force_small" if cfg.kind == "metal" else "k_force2", "achieved": achieved / 1e12, "peak": peak_alu / 1e12,
         "unit": "T FP64 instr/s", "frac": achieved / peak_alu,
