@@ -334,6 +334,8 @@ def main():
                     help="probe of what a Verlet-skin neighbour list would cost the hot kernels: the neighbour list is built "
                          "with rc + SKIN while every symmetry function keeps its cutoff (nnp_set_sf_cutoffs), i.e. exactly the "
                          "list a skin scheme would hand the kernels on its reuse steps; the list is still rebuilt every call")
+    ap.add_argument("--deterministic", action="store_true",
+                    help="nnp_set_deterministic_forces: fixed-point force accumulation (bit-reproducible forces)")
     ap.add_argument("--no-probe", action="store_true", help="skip the DFMA issue-rate probe (for ncu runs)")
     ap.add_argument("--no-sweep", action="store_true",
                     help="skip the short timed runs of configs[1], [2], [4] that the default line carries as config_sweep")
@@ -382,6 +384,8 @@ def main():
     nnp = NNP.from_model(model, device=local)
     if args.precision != "f64":
         nnp.set_precision(args.precision)
+    if args.deterministic:
+        nnp.set_deterministic_forces(True)
     if cfg.kind == "metal":
         nnp.set_max_neighbors(32)      # 18 neighbours per atom: the 8-lanes-per-centre kernels of k_small.cu
     pos = torch.tensor(sysm.pos, dtype=torch.float64, device=dev)
@@ -540,7 +544,8 @@ def main():
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == "f64" else "f32-stage/f64-acc", "data": "synthetic",
         "config": {"workload": cfg.name, "n_atoms": n, "model": model.name, "kernels": list(table_kernels(model)), "box": float(sysm.box[0]),
-                   "neighbor_rebuild": "every call", "md": bool(args.md), "parallelism": "replicas x%d" % world,
+                   "neighbor_rebuild": "every call", "md": bool(args.md),
+                   "force_accumulation": "fixed-point 2^-40 eV/A (bit-reproducible)" if args.deterministic else "FP64 atomics", "parallelism": "replicas x%d" % world,
                    "l2": ("working set per step (%.2f GB workspace) %s the 126 MB L2; no flush between steps"
                           % (nnp.workspace_bytes(n) / 1e9, "exceeds" if nnp.workspace_bytes(n) > 126e6 else "FITS IN"))},
         "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "clocks": clocks, "gpu_launches": launches,

@@ -47,6 +47,8 @@ typedef enum {
     NNP_ERR_WORKSPACE = 5,         /* workspace pointer null / misaligned / too small */
     NNP_ERR_CUDA = 6,              /* CUDA runtime error; see nnp_last_error */
     NNP_ERR_NONFINITE = 7,         /* NaN/Inf in positions (device-detected) */
+    NNP_ERR_FORCE_RANGE = 9,       /* nnp_set_deterministic_forces: a force contribution beyond the fixed-point range
+                                      (device-detected; forces of that call are incomplete) */
     NNP_ERR_LIMIT = 8              /* a well-formed request beyond a compile-time limit of this build: more than
                                       NNP_MAX_ELEMENTS elements, max_neighbors > NNP_MAX_NEIGHBORS, a hidden layer wider
                                       than NNP_MAX_HIDDEN_WIDTH, more than 8 weight layers, more than 128 radial / 512
@@ -182,6 +184,15 @@ nnp_status nnp_set_sf_cutoffs(nnp_model* m, int32_t n_sf, const double* h_rc);
 #define NNP_PRECISION_MIXED 1
 nnp_status nnp_set_precision(nnp_model* m, int32_t mode);
 
+/* ---- bit-reproducible forces (BASELINE.json north_star: forces are accumulated "either atomic-free via per-atom gather or
+ * with warp-aggregated atomics"; "thread-safe atomics as needed for ... force updates").  By default every centre
+ * adds its contributions to the neighbours' forces with FP64 atomics: the ~180 additions per atom happen in an order that
+ * differs from run to run, so forces repeat only to ~1e-13 eV/A (energies are always bit-reproducible).  With
+ * nnp_set_deterministic_forces(m, 1) every contribution is rounded to a multiple of 2^-40 eV/A (9.1e-13) and accumulated as a
+ * 64-bit integer; integer addition is associative, so the forces are the same bits on every run, at the same speed.  A
+ * contribution beyond +-2^22 eV/A (coincident atoms) is reported as NNP_ERR_FORCE_RANGE by nnp_sync_status. */
+nnp_status nnp_set_deterministic_forces(nnp_model* m, int32_t enabled);
+
 /* ---- MD loop around the path (the implementation is checked by energy
  * conservation in an NVE run).  Velocity Verlet, everything on the device:
  *     v += (dt/2) F/m ;  x += dt v ;  F = nnp_compute(x) ;  v += (dt/2) F/m
@@ -211,7 +222,7 @@ nnp_status nnp_md_kinetic_energy(nnp_model* m, const double* h_mass, int64_t n_a
  * evaluation enqueued since the previous nnp_sync_status (a sticky device word owned by the model: a neighbour
  * overflow or a non-finite position in step 3 of a 100-step nnp_md_run, or in the first of several nnp_compute
  * calls enqueued back to back, is still reported).  Reading clears the word.  Precedence when several flags are
- * set: NNP_ERR_NONFINITE, NNP_ERR_TYPE_RANGE, NNP_ERR_NEIGHBOR_OVERFLOW. */
+ * set: NNP_ERR_NONFINITE, NNP_ERR_TYPE_RANGE, NNP_ERR_NEIGHBOR_OVERFLOW, NNP_ERR_FORCE_RANGE. */
 nnp_status nnp_sync_status(nnp_model* m);
 
 /* Debug / parity exports of the LAST nnp_compute (they synchronise its stream first): the neighbour list of

@@ -16,13 +16,13 @@ LIB_PATH = os.environ.get("NNP_B200_LIBRARY") or os.path.join(HERE, "libnnp_b200
 NNP_OK = 0
 STATUS_NAMES = {0: "NNP_OK", 1: "NNP_ERR_INVALID_ARG", 2: "NNP_ERR_BOX_TOO_SMALL", 3: "NNP_ERR_TYPE_RANGE",
                 4: "NNP_ERR_NEIGHBOR_OVERFLOW", 5: "NNP_ERR_WORKSPACE", 6: "NNP_ERR_CUDA", 7: "NNP_ERR_NONFINITE",
-                8: "NNP_ERR_LIMIT"}
+                8: "NNP_ERR_LIMIT", 9: "NNP_ERR_FORCE_RANGE"}
 N_STAGES = 6
 STAGE_NAMES = ("sort", "neighbors", "symmetry_functions", "networks", "forces", "finalize")
 
 # every symbol include/nnp.h declares
 EXPORTS = ("nnp_create", "nnp_table_kernels", "nnp_destroy", "nnp_set_max_neighbors", "nnp_workspace_bytes", "nnp_compute",
-           "nnp_compute_host", "nnp_set_sf_scaling", "nnp_set_activation", "nnp_set_sf_cutoffs", "nnp_set_precision", "nnp_md_run", "nnp_md_kinetic_energy", "nnp_sync_status", "nnp_get_neighbor_counts", "nnp_get_neighbors", "nnp_get_sf",
+           "nnp_compute_host", "nnp_set_sf_scaling", "nnp_set_activation", "nnp_set_sf_cutoffs", "nnp_set_precision", "nnp_set_deterministic_forces", "nnp_md_run", "nnp_md_kinetic_energy", "nnp_sync_status", "nnp_get_neighbor_counts", "nnp_get_neighbors", "nnp_get_sf",
            "nnp_get_dedg", "nnp_g_stride", "nnp_set_timing", "nnp_get_timings", "nnp_last_launch_count",
            "nnp_uses_fast_path", "nnp_measure_fp64_peak", "nnp_last_error", "nnp_version")
 
@@ -89,6 +89,8 @@ def load_library():
     L.nnp_set_sf_cutoffs.argtypes = [vp, i32, vp]
     L.nnp_set_precision.restype = C.c_int
     L.nnp_set_precision.argtypes = [vp, i32]
+    L.nnp_set_deterministic_forces.restype = C.c_int
+    L.nnp_set_deterministic_forces.argtypes = [vp, i32]
     L.nnp_md_run.restype = C.c_int
     L.nnp_md_run.argtypes = [vp, i32, dbl, C.POINTER(dbl), i64, vp, vp, vp, C.POINTER(dbl), vp, vp, vp, vp,
                              C.c_size_t, vp]
@@ -260,6 +262,10 @@ class NNP:
     def set_precision(self, mode):
         """"f64" (default) or "mixed" (FP32 staging and per-triplet arithmetic; include/nnp.h nnp_set_precision)."""
         self._check(self._L.nnp_set_precision(self._h, {"f64": 0, "mixed": 1}[mode]))
+
+    def set_deterministic_forces(self, on: bool):
+        """Fixed-point (2^-40 eV/A) global force accumulation: bit-reproducible forces (include/nnp.h)."""
+        self._check(self._L.nnp_set_deterministic_forces(self._h, 1 if on else 0))
 
     def set_sf_cutoffs(self, rcs):
         """Per-SF cutoff radii in the order of the model's SF table (each <= rc); None = the global rc."""

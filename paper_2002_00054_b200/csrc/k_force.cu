@@ -33,6 +33,8 @@ struct ForceParams {
     const int32_t *cell_start, *nbr, *nbr_cnt;
     const double* dEdG;
     double* f_sorted;
+    int fixed;                           // 1: fixed-point force accumulation (nnp_internal.h force_add)
+    int32_t *status, *sticky;
     const ElemProgram* prog[MAX_ELEM];
     int variant[MAX_ELEM];
     int radial_only[MAX_ELEM];           // 1: run only the radial block for this element (per-SF radial radii of a lane-owned element)
@@ -325,16 +327,16 @@ __global__ void __launch_bounds__(FC_WARPS * 32) k_force(const __grid_constant__
         const double2 u0 = nb.p0[m], av = acc.av[m], yz = acc.yz[m];
         const double uz = nb.p1[m].x;
         const double ax = fma(-av.x, u0.x, av.y), ay = fma(-av.x, u0.y, yz.x), az = fma(-av.x, uz, yz.y);
-        atomicAdd(&p.f_sorted[3 * (size_t)j + 0], ax);
-        atomicAdd(&p.f_sorted[3 * (size_t)j + 1], ay);
-        atomicAdd(&p.f_sorted[3 * (size_t)j + 2], az);
+        force_add(p, 3 * (size_t)j + 0, ax);
+        force_add(p, 3 * (size_t)j + 1, ay);
+        force_add(p, 3 * (size_t)j + 2, az);
         fx -= ax; fy -= ay; fz -= az;
     }
     fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
     if (lane == 0) {
-        atomicAdd(&p.f_sorted[3 * (size_t)i + 0], fx);
-        atomicAdd(&p.f_sorted[3 * (size_t)i + 1], fy);
-        atomicAdd(&p.f_sorted[3 * (size_t)i + 2], fz);
+        force_add(p, 3 * (size_t)i + 0, fx);
+        force_add(p, 3 * (size_t)i + 1, fy);
+        force_add(p, 3 * (size_t)i + 2, fz);
     }
 }
 
@@ -358,6 +360,7 @@ int launch_force(const Workspace& w, const Grid& g, int64_t n, int n_elem, const
     for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.dEdG = w.dEdG; p.f_sorted = w.f_sorted;
+    p.fixed = passes.fixed_forces; p.status = w.status; p.sticky = w.sticky;
     bool use[ANG_NVARIANT] = {};
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;

@@ -36,6 +36,8 @@ struct Force2Params {
     const int32_t *cell_start, *nbr, *nbr_cnt;
     const double* dEdG;
     double* f_sorted;
+    int fixed;                           // 1: fixed-point force accumulation (nnp_internal.h force_add)
+    int32_t *status, *sticky;
     const int32_t *big_list, *big_count; // centres with more than 128 neighbours (k_count_words)
     const int64_t* word_off;             // masks from the SF kernel (see Workspace::gmask)
     const uint32_t* gmask;
@@ -449,16 +451,16 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
         const double Rm = (double)rad[m];
         const double ax = fma(-Rm, (double)u0.x, (double)fxy.x), ay = fma(-Rm, (double)u0.y, (double)fxy.y),
                      az = fma(-Rm, (double)uz, (double)fzz);
-        atomicAdd(&p.f_sorted[3 * (size_t)j + 0], ax);
-        atomicAdd(&p.f_sorted[3 * (size_t)j + 1], ay);
-        atomicAdd(&p.f_sorted[3 * (size_t)j + 2], az);
+        force_add(p, 3 * (size_t)j + 0, ax);
+        force_add(p, 3 * (size_t)j + 1, ay);
+        force_add(p, 3 * (size_t)j + 2, az);
         fx -= ax; fy -= ay; fz -= az;
     }
     fx = warp_sum(fx); fy = warp_sum(fy); fz = warp_sum(fz);
     if (lane == 0) {
-        atomicAdd(&p.f_sorted[3 * (size_t)i + 0], fx);
-        atomicAdd(&p.f_sorted[3 * (size_t)i + 1], fy);
-        atomicAdd(&p.f_sorted[3 * (size_t)i + 2], fz);
+        force_add(p, 3 * (size_t)i + 0, fx);
+        force_add(p, 3 * (size_t)i + 1, fy);
+        force_add(p, 3 * (size_t)i + 2, fz);
     }
 }
 
@@ -543,6 +545,7 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
     for (int c = 0; c < 3; ++c) { p.box[c] = g.box[c]; p.half[c] = g.half[c]; }
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt; p.dEdG = w.dEdG; p.f_sorted = w.f_sorted;
+    p.fixed = passes.fixed_forces; p.status = w.status; p.sticky = w.sticky;
     p.word_off = w.word_off; p.gmask = w.gmask; p.gmask_cap = w.gmask_cap;
     p.big_list = w.big_list; p.big_count = w.status + 2;
     bool use[ANG_NVARIANT][2] = {};                                       // [variant][tiny_exp]
@@ -555,8 +558,8 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
     // precision 1 (nnp_set_precision: mixed): FP32 instantiations of BASELINE.json's two shapes, water-like exp range
     const bool f32 = precision == 1;
     if (max_nbr <= 32) {     // small neighbourhoods (metals): 8 lanes per centre (k_small.cu)
-        if (use[ANG_BASE12][1]) launches += launch_force_small(w, g, n, n_elem, d_prog, variant, rc, stride, g_stride, true, st);
-        if (use[ANG_BASE12][0]) launches += launch_force_small(w, g, n, n_elem, d_prog, variant, rc, stride, g_stride, false, st);
+        if (use[ANG_BASE12][1]) launches += launch_force_small(w, g, n, n_elem, d_prog, variant, rc, stride, g_stride, true, passes.fixed_forces, st);
+        if (use[ANG_BASE12][0]) launches += launch_force_small(w, g, n, n_elem, d_prog, variant, rc, stride, g_stride, false, passes.fixed_forces, st);
         use[ANG_BASE12][0] = use[ANG_BASE12][1] = false;
     }
     if (use[ANG_BASE12][1]) launches += f32 ? launch_one2<SpecBase12, true, float>(p, st) : launch_one2<SpecBase12, true>(p, st);

@@ -12,7 +12,7 @@ constexpr int FIN_THREADS = 256;
 __global__ void __launch_bounds__(FIN_THREADS)
 k_unpermute(int64_t n, const int32_t* __restrict__ perm, const double* __restrict__ e_sorted,
             const double* __restrict__ f_sorted, double* __restrict__ e_atom, double* __restrict__ force,
-            double* __restrict__ partial) {
+            double* __restrict__ partial, int fixed) {
     __shared__ double red[FIN_THREADS];
     const int64_t p = (int64_t)blockIdx.x * FIN_THREADS + threadIdx.x;
     double e = 0.0;
@@ -20,9 +20,16 @@ k_unpermute(int64_t n, const int32_t* __restrict__ perm, const double* __restric
         const int64_t i = perm[p];
         e = e_sorted[p];
         e_atom[i] = e;
-        force[3 * i + 0] = f_sorted[3 * p + 0];
-        force[3 * i + 1] = f_sorted[3 * p + 1];
-        force[3 * i + 2] = f_sorted[3 * p + 2];
+        if (fixed) {        // fixed-point sums of the deterministic mode (nnp_internal.h force_add)
+            const unsigned long long* fb = reinterpret_cast<const unsigned long long*>(f_sorted);
+            force[3 * i + 0] = force_from_fixed(fb[3 * p + 0]);
+            force[3 * i + 1] = force_from_fixed(fb[3 * p + 1]);
+            force[3 * i + 2] = force_from_fixed(fb[3 * p + 2]);
+        } else {
+            force[3 * i + 0] = f_sorted[3 * p + 0];
+            force[3 * i + 1] = f_sorted[3 * p + 1];
+            force[3 * i + 2] = f_sorted[3 * p + 2];
+        }
     }
     red[threadIdx.x] = e;
     __syncthreads();
@@ -47,12 +54,12 @@ __global__ void __launch_bounds__(1024) k_sum_partials(int64_t nb, const double*
     if (threadIdx.x == 0) *e_total = red[0];
 }
 
-int launch_finalize(const Workspace& w, int64_t n, double* d_e_atom, double* d_e_total, double* d_force,
+int launch_finalize(const Workspace& w, int64_t n, double* d_e_atom, double* d_e_total, double* d_force, int fixed_forces,
                     cudaStream_t st) {
     const int64_t nb = (n + FIN_THREADS - 1) / FIN_THREADS;
     int launches = 0;
     if (nb > 0) {
-        k_unpermute<<<(unsigned)nb, FIN_THREADS, 0, st>>>(n, w.perm, w.e_sorted, w.f_sorted, d_e_atom, d_force, w.partial);
+        k_unpermute<<<(unsigned)nb, FIN_THREADS, 0, st>>>(n, w.perm, w.e_sorted, w.f_sorted, d_e_atom, d_force, w.partial, fixed_forces);
         ++launches;
     }
     k_sum_partials<<<1, 1024, 0, st>>>(nb, w.partial, d_e_total);

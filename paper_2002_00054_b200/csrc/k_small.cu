@@ -39,6 +39,8 @@ struct SmallParams {
     double* G;                           // SF kernel: out
     const double* dEdG;                  // force kernel: in
     double* f_sorted;                    // force kernel: accumulated into
+    int fixed;                           // 1: fixed-point force accumulation (nnp_internal.h force_add)
+    int32_t *status, *sticky;
     const ElemProgram* prog[MAX_ELEM];
     int variant[MAX_ELEM];
 };
@@ -296,8 +298,14 @@ __host__ __device__ constexpr size_t sm_force_bytes(int g_stride, int n_elem) {
 // kernels they lost to turn-taking (2.9 lanes per slot and iteration), here 8 consecutive list entries hit distinct
 // slots almost always, the CAS succeeds at once, and no warp-synchronous instruction (match / vote / syncwarp on a
 // group mask: four masks per warp) is left in the triplet loop -- 5.4 instead of 7.5 ms on the Ni-like workload.
-__device__ __forceinline__ void small_slot_add(double* fx, double* fy, double* fz, int slot, bool act, double x, double y, double z) {
-    if (act) {
+__device__ __forceinline__ void small_slot_add(double* fx, double* fy, double* fz, int slot, bool act, double x, double y, double z,
+                                               int fixed) {
+    if (!act) return;
+    if (fixed) {            // deterministic mode: 64-bit integer adds (native shared-memory atomics, any order gives the same bits)
+        atomicAdd(reinterpret_cast<unsigned long long*>(fx) + slot, force_to_fixed(x));
+        atomicAdd(reinterpret_cast<unsigned long long*>(fy) + slot, force_to_fixed(y));
+        atomicAdd(reinterpret_cast<unsigned long long*>(fz) + slot, force_to_fixed(z));
+    } else {
         atomicAdd(&fx[slot], x);
         atomicAdd(&fy[slot], y);
         atomicAdd(&fz[slot], z);
@@ -481,8 +489,8 @@ __global__ void __launch_bounds__(SM_WARPS * 32, 8) k_force_small(const __grid_c
                 const double f_vv = fma(-qc, k1.y * k1.y, fma((a2v.x * k2v.y) * fcc, Z0, -t2));
                 const double s1 = f_uu + f_w, s2 = f_vv + f_w, s3 = fma(-qq, iab, f_w);
                 // F_j = s3 v - s1 u ,  F_k = s3 u - s2 v
-                small_slot_add(fx, fy, fz, j, active, fma(s3, k0.x, -s1 * a0.x), fma(s3, k0.y, -s1 * a0.y), fma(s3, k1.x, -s1 * a1.x));
-                small_slot_add(fx, fy, fz, k, active, fma(s3, a0.x, -s2 * k0.x), fma(s3, a0.y, -s2 * k0.y), fma(s3, a1.x, -s2 * k1.x));
+                small_slot_add(fx, fy, fz, j, active, fma(s3, k0.x, -s1 * a0.x), fma(s3, k0.y, -s1 * a0.y), fma(s3, k1.x, -s1 * a1.x), p.fixed);
+                small_slot_add(fx, fy, fz, k, active, fma(s3, a0.x, -s2 * k0.x), fma(s3, a0.y, -s2 * k0.y), fma(s3, a1.x, -s2 * k1.x), p.fixed);
             }
             __syncwarp();                              // the list is refilled
             }
@@ -494,17 +502,20 @@ __global__ void __launch_bounds__(SM_WARPS * 32, 8) k_force_small(const __grid_c
         const int j = row[m];
         const double2 u0 = p0[m];
         const double uz = p1[m].x, R = rad[m];
-        const double ax = fma(-R, u0.x, fx[m]), ay = fma(-R, u0.y, fy[m]), az = fma(-R, uz, fz[m]);
-        atomicAdd(&p.f_sorted[3 * (size_t)j + 0], ax);
-        atomicAdd(&p.f_sorted[3 * (size_t)j + 1], ay);
-        atomicAdd(&p.f_sorted[3 * (size_t)j + 2], az);
+        const double gx = p.fixed ? force_from_fixed(reinterpret_cast<const unsigned long long*>(fx)[m]) : fx[m];
+        const double gy = p.fixed ? force_from_fixed(reinterpret_cast<const unsigned long long*>(fy)[m]) : fy[m];
+        const double gz = p.fixed ? force_from_fixed(reinterpret_cast<const unsigned long long*>(fz)[m]) : fz[m];
+        const double ax = fma(-R, u0.x, gx), ay = fma(-R, u0.y, gy), az = fma(-R, uz, gz);
+        force_add(p, 3 * (size_t)j + 0, ax);
+        force_add(p, 3 * (size_t)j + 1, ay);
+        force_add(p, 3 * (size_t)j + 2, az);
         sx_ -= ax; sy_ -= ay; sz_ -= az;
     }
     sx_ = group8_sum(sx_); sy_ = group8_sum(sy_); sz_ = group8_sum(sz_);
     if (gl == 0 && live) {
-        atomicAdd(&p.f_sorted[3 * (size_t)i + 0], sx_);
-        atomicAdd(&p.f_sorted[3 * (size_t)i + 1], sy_);
-        atomicAdd(&p.f_sorted[3 * (size_t)i + 2], sz_);
+        force_add(p, 3 * (size_t)i + 0, sx_);
+        force_add(p, 3 * (size_t)i + 1, sy_);
+        force_add(p, 3 * (size_t)i + 2, sz_);
     }
 }
 
@@ -519,6 +530,7 @@ static SmallParams small_params(const Workspace& w, const Grid& g, int64_t n, in
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt;
     p.G = w.G; p.dEdG = w.dEdG; p.f_sorted = w.f_sorted;
+    p.fixed = 0; p.status = w.status; p.sticky = w.sticky;
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
         p.variant[e] = e < n_elem ? (variant[e] & 255) : -1;
@@ -539,9 +551,10 @@ int launch_sf_small(const Workspace& w, const Grid& g, int64_t n, int n_elem, co
 }
 
 int launch_force_small(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                       const int* variant, double rc, int stride, int g_stride, bool tiny, cudaStream_t st) {
+                       const int* variant, double rc, int stride, int g_stride, bool tiny, int fixed_forces, cudaStream_t st) {
     if (n == 0) return 0;
-    const SmallParams p = small_params(w, g, n, n_elem, d_prog, variant, rc, stride, g_stride);
+    SmallParams p = small_params(w, g, n, n_elem, d_prog, variant, rc, stride, g_stride);
+    p.fixed = fixed_forces;
     const unsigned grid = (unsigned)((n + SM_CPC - 1) / SM_CPC);
     const size_t smem = SM_CPC * sm_force_bytes(g_stride, n_elem);
     static unsigned long long c1 = 0ull, c0 = 0ull;      // per device (opt_in_smem): > 48 KB with wide G rows

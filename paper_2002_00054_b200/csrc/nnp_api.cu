@@ -25,7 +25,7 @@ struct nnp_model {
     std::vector<ElemProgram> h_prog;             // host copies as built by nnp_create (global rc, specialised variants)
     std::vector<std::pair<int, int>> sf_loc;     // per SF of the nnp_create table: (central element, position in its G)
     int variant[MAX_ELEM] = {0, 0, 0, 0};
-    PassInfo passes;                 // free-eta passes per element (launchers)
+    PassInfo passes = {};            // free-eta passes per element, force-accumulation mode (launchers)
     NetDesc nets[MAX_ELEM];
     double* d_weights[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
     double* d_scaling[MAX_ELEM] = {nullptr, nullptr, nullptr, nullptr};
@@ -64,7 +64,9 @@ static double k2_of(double rc) {
 }
 
 static void set_pass_info(nnp_model* m, const std::vector<ElemProgram>& progs) {
+    const int fixed = m->passes.fixed_forces;
     std::memset(&m->passes, 0, sizeof(m->passes));
+    m->passes.fixed_forces = fixed;
     for (int c = 0; c < m->n_elem; ++c) {
         m->passes.n_pass[c] = progs[c].n_pass;
         m->passes.radial_own[c] = progs[c].per_sf_rc;
@@ -652,6 +654,12 @@ extern "C" nnp_status nnp_set_precision(nnp_model* m, int32_t mode) {
     return NNP_OK;
 }
 
+extern "C" nnp_status nnp_set_deterministic_forces(nnp_model* m, int32_t enabled) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    m->passes.fixed_forces = enabled != 0 ? 1 : 0;
+    return NNP_OK;
+}
+
 extern "C" nnp_status nnp_set_max_neighbors(nnp_model* m, int32_t max_neighbors) {
     if (!m) return NNP_ERR_INVALID_ARG;
     if (max_neighbors < 32) return fail(m, NNP_ERR_INVALID_ARG, "max_neighbors must be >= 32");
@@ -732,7 +740,7 @@ extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d
     mark(4);
     launches += launch_force(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->passes, m->rc, stride, m->max_nbr, m->g_stride, m->precision, st);
     mark(5);
-    launches += launch_finalize(w, n_atoms, d_e_atom, d_e_total, d_force, st);
+    launches += launch_finalize(w, n_atoms, d_e_atom, d_e_total, d_force, m->passes.fixed_forces, st);
     mark(6);
     m->timing_valid = m->timing;
     m->ws = w;
@@ -848,6 +856,7 @@ extern "C" nnp_status nnp_sync_status(nnp_model* m) {
     if (s & ST_NONFINITE) return fail(m, NNP_ERR_NONFINITE, "non-finite position");
     if (s & ST_TYPE_RANGE) return fail(m, NNP_ERR_TYPE_RANGE, "atom type out of range");
     if (s & ST_NBR_OVERFLOW) return fail(m, NNP_ERR_NEIGHBOR_OVERFLOW, "an atom has more than max_neighbors neighbours");
+    if (s & ST_FORCE_RANGE) return fail(m, NNP_ERR_FORCE_RANGE, "a force contribution beyond +-2^22 eV/A (deterministic fixed-point accumulation)");
     return NNP_OK;
 }
 

@@ -20,7 +20,7 @@ constexpr int MAX_LAYERS = 8;
 constexpr int MAX_WIDTH = 256;
 
 // Device-detected status bits (Workspace::status[0] is an OR of these)
-enum : int { ST_TYPE_RANGE = 1, ST_NBR_OVERFLOW = 2, ST_NONFINITE = 4 };
+enum : int { ST_TYPE_RANGE = 1, ST_NBR_OVERFLOW = 2, ST_NONFINITE = 4, ST_FORCE_RANGE = 8 };
 
 // index of the unordered element pair (a <= b) among E elements
 __host__ __device__ inline int pair_index(int a, int b, int n_elem) {
@@ -69,6 +69,7 @@ struct PassInfo {
     int n_pass[MAX_ELEM];
     int spec[MAX_ELEM][MAX_PASS];
     int radial_own[MAX_ELEM];        // the element's radial functions carry their own cutoff radii (ElemProgram::per_sf_rc)
+    int fixed_forces;                // nnp_set_deterministic_forces: fixed-point global force accumulation (force_add)
 };
 
 // Symmetry-function program of ONE central element; lives in device memory (model-owned).
@@ -171,6 +172,34 @@ inline void opt_in_smem(K kernel, unsigned long long* done, int bytes = 200 * 10
         *done |= 1ull << dev;
 }
 
+// Global force accumulation of the force kernels (their parameter blocks carry f_sorted, fixed, status, sticky).
+// Default: FP64 atomics (RED.ADD.F64) -- the order of the ~180 additions per atom is not fixed, the forces repeat to ~1e-13.
+// fixed = 1 (nnp_set_deterministic_forces): every contribution is rounded to a multiple of 2^-40 eV/A (9.1e-13) and added
+// as a 64-bit INTEGER -- integer addition is associative, so the sums are bit-reproducible whatever the order; range
+// +-2^22 eV/A per contribution (beyond: ST_FORCE_RANGE), +-2^23 per sum.  launch_finalize converts back.
+constexpr double FORCE_FIXED_SCALE = 1099511627776.0;             // 2^40
+constexpr double FORCE_FIXED_INV = 1.0 / 1099511627776.0;
+constexpr double FORCE_FIXED_LIMIT = 4194304.0;                   // 2^22
+#ifdef __CUDACC__
+__device__ __forceinline__ unsigned long long force_to_fixed(double v) {
+    return (unsigned long long)__double2ll_rn(v * FORCE_FIXED_SCALE);
+}
+__device__ __forceinline__ double force_from_fixed(unsigned long long b) { return (double)(long long)b * FORCE_FIXED_INV; }
+template <class P>
+__device__ __forceinline__ void force_add(const P& p, size_t idx, double v) {
+    if (p.fixed) {
+        if (!(fabs(v) < FORCE_FIXED_LIMIT)) {
+            atomicOr(p.status, ST_FORCE_RANGE);
+            atomicOr(p.sticky, ST_FORCE_RANGE);
+            return;
+        }
+        atomicAdd(reinterpret_cast<unsigned long long*>(p.f_sorted) + idx, force_to_fixed(v));
+    } else {
+        atomicAdd(p.f_sorted + idx, v);
+    }
+}
+#endif
+
 // ---- launchers (each enqueues on `st`; returns the number of kernels launched) ----------
 int launch_sort(const Workspace& w, const Grid& g, int64_t n, int n_elem, const double* d_pos,
                 const int32_t* d_type, cudaStream_t st);
@@ -200,8 +229,8 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
 int launch_sf_small(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
                     const int* variant, double rc, int stride, int g_stride, bool tiny, cudaStream_t st);
 int launch_force_small(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                       const int* variant, double rc, int stride, int g_stride, bool tiny, cudaStream_t st);
-int launch_finalize(const Workspace& w, int64_t n, double* d_e_atom, double* d_e_total, double* d_force,
+                       const int* variant, double rc, int stride, int g_stride, bool tiny, int fixed_forces, cudaStream_t st);
+int launch_finalize(const Workspace& w, int64_t n, double* d_e_atom, double* d_e_total, double* d_force, int fixed_forces,
                     cudaStream_t st);
 
 // MD loop (k_md.cu)

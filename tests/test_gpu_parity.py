@@ -656,3 +656,62 @@ def test_timings_and_launch_count():
     assert all(v >= 0.0 for v in t.values()) and t["forces"] > 0.0
     assert nnp.last_launch_count() >= 9
     nnp.close()
+
+
+@pytest.mark.parametrize("which", ["water-fast", "metal-small", "generic"])
+def test_deterministic_forces(which):
+    # nnp_set_deterministic_forces: fixed-point (2^-40 eV/A) global accumulation -> the SAME BITS on every run (the default
+    # FP64 atomics repeat to ~1e-13 only), still within BASELINE.json's 1e-8 of the oracle
+    from paper_2002_00054_b200 import NNP
+    kw = {}
+    if which == "water-fast":
+        sysm, model = W.build(W.CONFIGS[1])                      # 24,576 atoms: thousands of CTAs racing on the atomics
+    elif which == "metal-small":
+        sysm, model = W.build(W.Config("fcc10", 10, False, 1, 11, 12, None, "metal"))
+        kw["max_neighbors"] = 32
+    else:
+        rows = []
+        for c in range(2):
+            for e1 in range(2):
+                rows.append((c, 2, e1, 0, 0.05, 0.0, 0.0, 0.0))
+            for (e1, e2) in ((0, 0), (0, 1), (1, 1)):
+                rows.append((c, 3, e1, e2, 0.004, 0.0, 1.0, 3.0))
+                rows.append((c, 9, e1, e2, 0.010, 0.0, -1.0, 1.0))
+        model = tiny_model(rows, n_elem=2, hidden=(5, 4), seed=21)
+        sysm = W.make_water(700, 4242)
+    nnp = NNP.from_model(model)
+    if "max_neighbors" in kw:
+        nnp.set_max_neighbors(kw["max_neighbors"])
+    nnp.set_deterministic_forces(True)
+    runs = [_run(nnp, sysm.pos, sysm.types, sysm.box) for _ in range(3)]
+    for r in runs[1:]:
+        assert np.array_equal(r[2], runs[0][2]) and np.array_equal(r[0], runs[0][0]) and r[1] == runs[0][1]
+    assert np.all(np.abs(runs[0][2].sum(axis=0)) < 1e-7)
+    nnp.set_deterministic_forces(False)
+    plain = _run(nnp, sysm.pos, sysm.types, sysm.box)
+    assert np.abs(plain[2] - runs[0][2]).max() < 1e-10            # ~180 contributions per atom, each rounded to 9.1e-13
+    if sysm.n_atoms <= 5000:
+        ref = oracle.compute(oracle.OracleModel(model), sysm.pos, sysm.types, sysm.box)
+    else:
+        g = _golden(W.CONFIGS[1])
+        ref = None
+        for a in g["atoms"]:
+            assert np.abs(runs[0][2][a["index"]] - np.array(a["F"])).max() <= F_ABS
+    if ref is not None:
+        assert np.abs(runs[0][2] - ref.F).max() <= F_ABS
+    nnp.close()
+
+
+def test_deterministic_forces_range_error():
+    # a neighbour 1e-9 A from the centre: the 1/a factors of the angular force terms exceed the fixed-point range
+    from paper_2002_00054_b200 import NNP, NNPError
+    model = W.make_model(False)
+    nnp = NNP.from_model(model)
+    nnp.set_deterministic_forces(True)
+    pos = np.array([[5.0, 5.0, 5.0], [5.0 + 1e-9, 5.0, 5.0], [7.0, 6.0, 5.0], [4.0, 7.0, 6.5]])
+    typ = np.array([1, 0, 0, 1], dtype=np.int32)
+    dev = _dev()
+    with pytest.raises(NNPError) as ei:
+        nnp.compute(torch.tensor(pos, device=dev), torch.tensor(typ, device=dev), [20.0, 20.0, 20.0])
+    assert ei.value.status == 9                       # NNP_ERR_FORCE_RANGE
+    nnp.close()
