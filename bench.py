@@ -324,12 +324,13 @@ def main():
     ap.add_argument("--md", action="store_true",
                     help="time velocity-Verlet MD steps (nnp_md_run: kick+drift, the whole path, kick) instead of bare evaluations")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--table", default="baseline", choices=["baseline", "free", "generic", "n2p2like"],
+    ap.add_argument("--table", default="baseline", choices=["baseline", "free", "generic", "n2p2like", "wide9"],
                     help="SF table probe (not a BASELINE.json workload): 'free' breaks the eta ratio of the angular set "
                          "(0.01 -> 0.0123: lane-owned kernels with per-eta exponentials), 'generic' also replaces zeta 16 by 3 "
                          "(queue-based generic kernels), 'n2p2like' is a table shaped like published n2p2 models (zeta in {1, 4}, "
                          "seven eta values, lambda = +-1, angular functions of two cutoff radii: 3 passes of the free-eta "
-                         "kernels); the roofline object is then not meaningful")
+                         "kernels), 'wide9' turns the angular functions of the smaller eta into wide ones (n2p2 kind 9: one narrow and one "
+                         "wide pass); the roofline object is then not meaningful")
     ap.add_argument("--skin", type=float, default=0.0,
                     help="probe of what a Verlet-skin neighbour list would cost the hot kernels: the neighbour list is built "
                          "with rc + SKIN while every symmetry function keeps its cutoff (nnp_set_sf_cutoffs), i.e. exactly the "
@@ -369,6 +370,10 @@ def main():
     sysm, model = W.build(cfg)
     if args.table == "n2p2like":
         model = n2p2like_model()
+    elif args.table == "wide9":
+        ang = model.sf["kind"] == 3
+        model.sf["kind"][ang & (model.sf["eta"] == model.sf["eta"][ang].min())] = 9
+        model.name += "+wide9"
     elif args.table != "baseline":
         ang = model.sf["kind"] == 3
         model.sf["eta"][ang & (model.sf["eta"] == 0.01)] = 0.0123

@@ -67,7 +67,7 @@ typedef enum {
  *               (1 + lambda cos)^zeta  exp(-eta (a^2+b^2+c^2))  fc(a) fc(b) fc(c)
  *   kind 9 (angular, wide): the same without the r_jk terms,
  *       G = 2^(1-zeta) sum_{j<k in N(i), {t_j,t_k} = {e1,e2}} (1 + lambda cos)^zeta  exp(-eta (a^2+b^2))  fc(a) fc(b)
- *       (a table that contains kind 9 runs on the generic kernels)
+ *       (every pair of neighbours is a triplet; such functions run as passes of their own, NNP_KERNELS_MULTI)
  *   fc(r) = (cos(pi r / rc) + 1)/2 for r < rc, else 0;  N(i) = { j != i : r_ij^2 < rc^2 }.
  * Constraints (else NNP_ERR_INVALID_ARG): eta >= 0; kinds 3 and 9 need lambda = +1 or -1 and
  * zeta an integer in [1, 64]; rs is used by kind 2 only.  The order of the entries with
@@ -102,10 +102,10 @@ nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* const* elem_n
  *   NNP_KERNELS_FREE32 / NNP_KERNELS_FREE16  the lane-owned kernels for any table with <= 4 (FREE16: <= 2) distinct
  *                        angular eta values, lambda = +-1, zeta in {1, 2, 4, 16}, narrow (kind 3) functions only,
  *                        no (eta, lambda, zeta) twice per pair group,
- *   NNP_KERNELS_MULTI    the same lane-owned free-eta kernels in several passes: any number of eta values (four per pass)
- *                        and, after nnp_set_sf_cutoffs, angular functions of several cutoff radii (one radius per pass),
- *                        at most 8 passes; otherwise the conditions of FREE32,
- *   NNP_KERNELS_GENERIC  everything else (other zeta, kind 9, more passes, no angular functions at all).
+ *   NNP_KERNELS_MULTI    the same lane-owned free-eta kernels in several passes: any number of eta values (four per pass),
+ *                        wide functions (kind 9; passes of their own) and, after nnp_set_sf_cutoffs, angular functions of
+ *                        several cutoff radii (one radius per pass), at most 8 passes; otherwise the conditions of FREE32,
+ *   NNP_KERNELS_GENERIC  everything else (other zeta, more passes, no angular functions at all).
  * Returns NNP_ERR_INVALID_ARG for a table nnp_create would reject (message: nnp_last_error(NULL)). */
 #define NNP_KERNELS_GENERIC 0
 #define NNP_KERNELS_BASE12 1

@@ -137,11 +137,12 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
     const AngPass* __restrict__ ps = &prog->pass[Spec::FREE_ETA ? p.pass : 0];
     if (Spec::FREE_ETA && (p.pass >= prog->n_pass || ps->spec != Spec::ID)) return;
     const bool own_rc = Spec::FREE_ETA && ps->own_rc != 0;          // the pass's cutoff is shorter than the neighbour list's
+    const bool widep = Spec::FREE_ETA && ps->wide != 0;             // wide angular functions: no r_jk term, every pair counts
     const double rc2p = Spec::FREE_ETA ? ps->rc2 : p.rc2, k2p = Spec::FREE_ETA ? ps->k2 : p.k2;
     const int32_t* __restrict__ n_ang = Spec::FREE_ETA ? ps->n_ang : prog->n_ang;
     const int neta = Spec::FREE_ETA ? ps->n_eta : Spec::NETA;
     const bool first_pass = !Spec::FREE_ETA || p.pass == 0;         // the radial forces
-    const bool handover = !Spec::FREE_ETA || (prog->n_pass == 1 && !own_rc);   // masks from the SF kernel
+    const bool handover = !Spec::FREE_ETA || (prog->n_pass == 1 && !own_rc && !widep);   // masks from the SF kernel
 
     constexpr int capa = CAPA;
     const int npair = p.n_elem * (p.n_elem + 1) / 2;
@@ -251,7 +252,7 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
     __syncthreads();
 
     // ---- screening -> masks; prefix; even split of the triplet stream over the NT threads ------------
-    const float rc2f = (float)(rc2p * (1.0 + 1e-5));
+    const float rc2f = widep ? 3.0e38f : (float)(rc2p * (1.0 + 1e-5));      // wide: no screening (a switched-off slot has fc = 0)
     if (have_masks) {
         // masks arrive in the SF kernel's group-major order; place them j-major and rebuild the descriptors
 #pragma unroll
@@ -347,9 +348,10 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
         cos_sinc(c2 * k2r, Cc, Sc);
         R fcc = Cc * Cc;                               // fc(c)
         R dfc = m2k2 * (Cc * Sc);                      // fc'(c)/c
-        if (!active || !(c2 < rc2r)) { fcc = (R)0; dfc = (R)0; }   // cutoff (FP64: exact; the masks were screened in FP32)
+        if (widep) { fcc = (R)1; dfc = (R)0; }         // wide: no fc(c)
+        if (!active || (!widep && !(c2 < rc2r))) { fcc = (R)0; dfc = (R)0; }   // cutoff (FP64: exact; the masks were screened in FP32)
         R Y[Spec::NETA];
-        const R r2 = (J.e0 + ek) + c2;                         // FREE_ETA: a^2 + b^2 + c^2 (the staged value is a^2)
+        const R r2 = widep ? J.e0 + ek : (J.e0 + ek) + c2;       // FREE_ETA: a^2 + b^2 (+ c^2, narrow) -- the staged value is a^2
         if constexpr (!Spec::FREE_ETA) {
             // (exp_tiny5: degree 5, 1e-14 -- one DFMA per triplet less than the symmetry-function kernel's degree 6; 74.8 -> 73.9 ms)
             Y[0] = (J.e0 * ek) * (tiny ? exp_tiny5(-eta0r * c2) : exp_small(-eta0r * c2));
@@ -416,7 +418,7 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
         const R fab = J.fa * k2v.x;
         const R Cf = fab * fcc;
         const R t2 = (Cf + Cf) * Z2;
-        const R f_w = fma(fab * dfc, Z0, -t2);
+        const R f_w = widep ? (R)0 : fma(fab * dfc, Z0, -t2);      // wide: nothing depends on w
         const R q = Z1 * Cf;
         const R qc = q * cosv;
         const R f_uu = fma(-qc, J.ia * J.ia, fma((J.dfa * k2v.x) * fcc, Z0, -t2));

@@ -72,10 +72,11 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
     const AngPass* __restrict__ ps = &prog->pass[Spec::FREE_ETA ? p.pass : 0];
     if (Spec::FREE_ETA && (p.pass >= prog->n_pass || ps->spec != Spec::ID)) return;
     const bool own_rc = Spec::FREE_ETA && ps->own_rc != 0;          // the pass's cutoff is shorter than the neighbour list's
+    const bool widep = Spec::FREE_ETA && ps->wide != 0;             // wide angular functions: no r_jk term, every pair counts
     const double rc2p = Spec::FREE_ETA ? ps->rc2 : p.rc2, k2p = Spec::FREE_ETA ? ps->k2 : p.k2;
     const int32_t* __restrict__ n_ang = Spec::FREE_ETA ? ps->n_ang : prog->n_ang;
     const bool first_pass = !Spec::FREE_ETA || p.pass == 0;         // the radial block and the tail of the G row
-    const bool handover = !Spec::FREE_ETA || (prog->n_pass == 1 && !own_rc);   // masks to the force kernel
+    const bool handover = !Spec::FREE_ETA || (prog->n_pass == 1 && !own_rc && !widep);   // masks to the force kernel
 
     constexpr int capa = CAPA;
     const int npair = p.n_elem * (p.n_elem + 1) / 2;
@@ -152,7 +153,7 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
     }
 
     // ---- screening -> masks; prefix; even split of the triplet stream over the NT threads ------------
-    const float rc2f = (float)(rc2p * (1.0 + 1e-5));
+    const float rc2f = widep ? 3.0e38f : (float)(rc2p * (1.0 + 1e-5));      // wide: no screening (a switched-off slot has fc = 0)
     for (int g = 0; g < ng; ++g) screen_group(tab[g], f32, words, rc2f, tid, NT);
     __syncthreads();
     // hand the masks to the force kernel (this kernel's group-major order), if they fit the budget
@@ -209,9 +210,10 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
         const R c2 = fma(wx, wx, fma(wy, wy, wz * wz));
         const R Cc = cos_only(c2 * k2r);
         R Cf = (jfa * k2v.y) * (Cc * Cc);           // fc(a) fc(b) fc(c), fc(c) = cos^2(pi c / (2 rc))
-        if (!active || !(c2 < rc2r)) Cf = (R)0;     // cutoff (FP64: exact; the masks were screened in FP32)
+        if (widep) Cf = jfa * k2v.y;                // wide: fc(a) fc(b) only
+        if (!active || (!widep && !(c2 < rc2r))) Cf = (R)0;     // cutoff (FP64: exact; the masks were screened in FP32)
         R Y[Spec::NETA];
-        const R r2 = (je0 + k2v.x) + c2;                       // FREE_ETA: a^2 + b^2 + c^2 (the staged value is a^2)
+        const R r2 = widep ? je0 + k2v.x : (je0 + k2v.x) + c2;   // FREE_ETA: a^2 + b^2 (+ c^2, narrow) -- the staged value is a^2
         if constexpr (!Spec::FREE_ETA) {
             Y[0] = (je0 * k2v.x) * (tiny ? exp_tiny5(-eta0r * c2) : exp_small(-eta0r * c2));   // degree 5: 1e-14 (46.9 -> 46.7 ms)
             if constexpr (Spec::NETA > 1) Y[1] = ipow<Spec::ratio(1)>(Y[Spec::rbase(1)]);

@@ -206,34 +206,38 @@ static bool match_spec(const std::vector<std::vector<AngularSF>>& groups, ElemPr
     return true;
 }
 
-// Free-eta passes (nnp_internal.h AngPass): any table of NARROW angular symmetry functions with lambda = +-1,
-// zeta in {1, 2, 4, 16} and no (rc, eta, lambda, zeta) twice in a pair group.  The symmetry functions are split by
-// cutoff radius (descending) and, inside a radius, into chunks of at most four eta values of about equal size; one
-// pass per chunk.  Returns false if the table does not fit (another zeta, a wide SF, more than MAX_PASS passes, an
-// exponent beyond exp_small's range).
+// Free-eta passes (nnp_internal.h AngPass): any table of angular symmetry functions (narrow, kind 3, and wide, kind 9)
+// with lambda = +-1, zeta in {1, 2, 4, 16} and no (kind, rc, eta, lambda, zeta) twice in a pair group.  The symmetry
+// functions are split by kind and cutoff radius (narrow first, radius descending) and, inside one, into chunks of at
+// most four eta values of about equal size; one pass per chunk.  Returns false if the table does not fit (another zeta,
+// more than MAX_PASS passes, an exponent beyond exp_small's range).
 static bool build_passes(const std::vector<std::vector<AngularSF>>& groups, double rc, ElemProgram* P) {
-    struct Key { double rc2, eta, k2; };
+    struct Key { double rc2, eta, k2; int wide; };
     std::vector<Key> keys;
     for (const auto& grp : groups)
         for (const auto& f : grp) {
-            if (f.wide) return false;
             bool zok = false;
             for (int b = 0; b < 7; ++b) zok |= (f.izeta == (1 << b)) && ((SpecFree32::mask(0) >> b) & 1u);
             if (!zok) return false;
             if (f.eta * 3.0 * f.rc2 > 700.0) return false;
             bool seen = false;
-            for (const Key& k : keys) seen |= (k.rc2 == f.rc2 && k.eta == f.eta);
-            if (!seen) keys.push_back(Key{f.rc2, f.eta, f.k2});
+            for (const Key& k : keys) seen |= (k.rc2 == f.rc2 && k.eta == f.eta && k.wide == f.wide);
+            if (!seen) keys.push_back(Key{f.rc2, f.eta, f.k2, f.wide});
         }
     if (keys.empty()) return false;
-    for (size_t x = 0; x < keys.size(); ++x)                  // sort: rc descending, eta ascending
+    auto before = [](const Key& a, const Key& b) {              // sort: narrow first, rc descending, eta ascending
+        if (a.wide != b.wide) return a.wide < b.wide;
+        if (a.rc2 != b.rc2) return a.rc2 > b.rc2;
+        return a.eta < b.eta;
+    };
+    for (size_t x = 0; x < keys.size(); ++x)
         for (size_t y = x + 1; y < keys.size(); ++y)
-            if (keys[y].rc2 > keys[x].rc2 || (keys[y].rc2 == keys[x].rc2 && keys[y].eta < keys[x].eta)) std::swap(keys[x], keys[y]);
+            if (before(keys[y], keys[x])) std::swap(keys[x], keys[y]);
     int np = 0;
     size_t x = 0;
     while (x < keys.size()) {
         size_t y = x;
-        while (y < keys.size() && keys[y].rc2 == keys[x].rc2) ++y;
+        while (y < keys.size() && keys[y].rc2 == keys[x].rc2 && keys[y].wide == keys[x].wide) ++y;
         const int n = (int)(y - x), chunks = (n + MAX_ETA - 1) / MAX_ETA;
         const int class_first = np;
         for (int c = 0; c < chunks; ++c) {
@@ -246,12 +250,13 @@ static bool build_passes(const std::vector<std::vector<AngularSF>>& groups, doub
             ps.rc2 = keys[lo].rc2;
             ps.k2 = keys[lo].k2;                            // k2_of(rc_p), as stored with the symmetry function
             ps.own_rc = ps.rc2 != rc * rc ? 1 : 0;
+            ps.wide = keys[lo].wide;
             ps.spec = ps.n_eta <= SpecFree16::NETA ? ANG_FREE16 : ANG_FREE32;
             for (size_t pr = 0; pr < groups.size(); ++pr) {
                 for (int e = 0; e < MAX_ETA; ++e)
                     for (int b = 0; b < 16; ++b) ps.g[pr][e][b] = -1;
                 for (const auto& f : groups[pr]) {
-                    if (f.rc2 != ps.rc2) continue;
+                    if (f.rc2 != ps.rc2 || f.wide != ps.wide) continue;
                     int e = -1;
                     for (int q = ps.n_eta - 1; q >= 0; --q)
                         if (ps.eta[q] == f.eta) e = q;
@@ -301,8 +306,8 @@ static nnp_status select_variant(ElemProgram& P, int n_elem, double rc, std::str
     const bool in_range = !any_wide && eta_max * 3.0 * rc * rc <= 700.0;
     if (in_range && !own_ang && match_spec<SpecBase12>(groups, &P)) P.variant = ANG_BASE12;
     else if (in_range && !own_ang && match_spec<SpecWide32>(groups, &P)) P.variant = ANG_WIDE32;
-    else if (!any_wide && build_passes(groups, rc, &P))
-        P.variant = (P.n_pass == 1 && !P.pass[0].own_rc) ? P.pass[0].spec : ANG_MULTI;
+    else if (build_passes(groups, rc, &P))
+        P.variant = (P.n_pass == 1 && !P.pass[0].own_rc && !P.pass[0].wide) ? P.pass[0].spec : ANG_MULTI;
     else {
         P.n_pass = 0;
         for (int p = 0; p < npair; ++p)

@@ -60,7 +60,8 @@ struct AngPass {
     int32_t n_eta;
     int32_t spec;                    // ANG_FREE16 (<= 2 eta values) or ANG_FREE32
     int32_t own_rc;                  // 1: rc_p differs from the global rc (slots beyond rc_p are switched off while staging)
-    int32_t pad;
+    int32_t wide;                    // 1: a pass of WIDE angular functions (n2p2 kind 9): no r_jk term, no r_jk cutoff -- every pair
+                                     // of neighbours of the two elements is a triplet (no screening)
     int32_t n_ang[MAX_PAIR];         // symmetry functions of pair group p in this pass (0: the group is skipped)
     int16_t g[MAX_PAIR][MAX_ETA][16];   // G index of menu entry (eta slot, bit); -1 = absent
 };

@@ -97,7 +97,9 @@ def test_kernel_choice_per_table(lib):
     m.sf["zeta"][ang & (m.sf["zeta"] == 16.0) & (m.sf["central"] == 1)] = 3.0     # zeta outside {1,2,4,16}: generic, that element only
     assert table_kernels(m) == ("free16", "generic")
     m = W.make_model(False)
-    m.sf["kind"][np.nonzero(ang)[0][0]] = 9                         # one wide angular SF on element 0
+    m.sf["kind"][np.nonzero(ang)[0][0]] = 9                         # one wide angular SF on element 0: a pass of its own
+    assert table_kernels(m) == ("multi", "base12")
+    m.sf["zeta"][np.nonzero(ang)[0][0]] = 3.0                       # ... with a zeta outside the menu: generic
     assert table_kernels(m) == ("generic", "base12")
     m = W.make_model(False)
     q = np.nonzero(ang)[0][:5]

@@ -292,8 +292,11 @@ def test_wide_angular_mixed_with_narrow():
             rows.append((c, 3, e1, e2, 0.004, 0.0, 1.0, 4.0))
             rows.append((c, 9, e1, e2, 0.0, 0.0, 1.0, 16.0))
     model = tiny_model(rows, n_elem=2, hidden=(5, 4), seed=21)
+    from paper_2002_00054_b200.binding import table_kernels
+    assert table_kernels(model) == ("multi", "multi")     # zeta in {1, 2, 4, 16}: narrow and wide passes of the lane-owned kernels
     _check_full(model, W.make_water(150, 5, L=16.7))
-    # wide only, one element
+    _check_full(model, W.make_water(80, 21, L=12.2))      # dense: ~115 neighbours, 6,500 pairs per centre in the wide passes
+    # wide only, one element (zeta = 3: the generic kernels)
     rows = [(0, 2, 0, 0, 0.05, 0.0, 0.0, 0.0), (0, 9, 0, 0, 0.02, 0.0, -1.0, 3.0), (0, 9, 0, 0, 0.001, 0.0, 1.0, 1.0)]
     sysm = W.make_water(60, 3, L=12.4)
     sysm.types[:] = 0
