@@ -138,6 +138,7 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
     if (Spec::FREE_ETA && (p.pass >= prog->n_pass || ps->spec != Spec::ID)) return;
     const bool own_rc = Spec::FREE_ETA && ps->own_rc != 0;          // the pass's cutoff is shorter than the neighbour list's
     const bool widep = Spec::FREE_ETA && ps->wide != 0;             // wide angular functions: no r_jk term, every pair counts
+    const int z0 = Spec::FREE_ETA ? ps->zeta0 : 1;                  // menu entry b stands for zeta = z0 * 2^b
     const double rc2p = Spec::FREE_ETA ? ps->rc2 : p.rc2, k2p = Spec::FREE_ETA ? ps->k2 : p.k2;
     const int32_t* __restrict__ n_ang = Spec::FREE_ETA ? ps->n_ang : prog->n_ang;
     const int neta = Spec::FREE_ETA ? ps->n_eta : Spec::NETA;
@@ -232,7 +233,7 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
             for (int e = 0; e < Spec::NETA; ++e) {
                 if (Spec::mask(e) >> tid & 1u) {
                     const int g = Spec::FREE_ETA ? ps->g[pr][e][tid] : prog->ang_g[pr][e][tid];
-                    const int zeta = 1 << (tid & 7);
+                    const int zeta = z0 << (tid & 7);
                     const double lam = tid < 8 ? 1.0 : -1.0;
                     const double bc = g >= 0 ? brow[g] * exp2((double)(1 - zeta)) : 0.0;
                     int a = 0;   // accumulator slot = set bits before (e, tid)
@@ -365,6 +366,11 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
         R pw[2][Spec::MAXBIT + 1], pd[2][Spec::MAXBIT + 1];
         pw[0][0] = (R)1 + cosv; pw[1][0] = (R)1 - cosv;
         pd[0][0] = (R)1; pd[1][0] = (R)1;
+        if (Spec::FREE_ETA && z0 > 1) {                        // uniform per CTA: P = (1 +- cos)^z0, dP/d(1 +- cos) = z0 (1 +- cos)^(z0-1)
+            const R q0 = powi_uniform(pw[0][0], z0 - 1), q1 = powi_uniform(pw[1][0], z0 - 1);
+            pw[0][0] *= q0; pw[1][0] *= q1;
+            pd[0][0] = (R)z0 * q0; pd[1][0] = (R)z0 * q1;
+        }
 #pragma unroll
         for (int b = 1; b <= Spec::MAXBIT; ++b) {
 #pragma unroll

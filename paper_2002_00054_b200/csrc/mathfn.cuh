@@ -108,4 +108,16 @@ __device__ __forceinline__ void fc_dfc_own(double r2, double rc2, double k2, dou
     df = in ? (-2.0 * k2) * (C * S) : 0.0;
 }
 
+// x^n, n >= 1 an integer that is the same in every lane: square-and-multiply in a warp-uniform loop
+// (the base exponent zeta0 of a free-eta pass, nnp_internal.h AngPass)
+template <class R>
+__device__ __forceinline__ R powi_uniform(R x, int n) {
+    R r = (n & 1) ? x : (R)1;
+    for (n >>= 1; n; n >>= 1) {
+        x *= x;
+        if (n & 1) r *= x;
+    }
+    return r;
+}
+
 }  // namespace nnp

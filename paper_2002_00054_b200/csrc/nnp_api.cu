@@ -1,5 +1,6 @@
 // nnp_api.cu -- the C ABI of libnnp_b200 (include/nnp.h): model construction, workspace layout,
 // the nnp_compute pipeline S0..S5, the host-buffer entry point and the debug exports.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -207,27 +208,61 @@ static bool match_spec(const std::vector<std::vector<AngularSF>>& groups, ElemPr
 }
 
 // Free-eta passes (nnp_internal.h AngPass): any table of angular symmetry functions (narrow, kind 3, and wide, kind 9)
-// with lambda = +-1, zeta in {1, 2, 4, 16} and no (kind, rc, eta, lambda, zeta) twice in a pair group.  The symmetry
-// functions are split by kind and cutoff radius (narrow first, radius descending) and, inside one, into chunks of at
-// most four eta values of about equal size; one pass per chunk.  Returns false if the table does not fit (another zeta,
-// more than MAX_PASS passes, an exponent beyond exp_small's range).
+// with lambda = +-1, integer zeta and no (kind, rc, eta, lambda, zeta) twice in a pair group.  The symmetry functions
+// are split by kind, cutoff radius and BASE EXPONENT zeta0 (the kernels' menu holds zeta0 * {1, 2, 4, 16}; inside one
+// (kind, radius) the smallest zeta not yet covered becomes the next zeta0) and, inside one such class, into chunks of
+// at most four eta values of about equal size; one pass per chunk, narrow first, radius descending.  Returns false if
+// the table does not fit (more than MAX_PASS passes, an exponent beyond exp_small's range).
 static bool build_passes(const std::vector<std::vector<AngularSF>>& groups, double rc, ElemProgram* P) {
-    struct Key { double rc2, eta, k2; int wide; };
+    struct Key { double rc2, eta, k2; int wide, z0; };
+    auto menu_bit = [](int zeta, int z0) {                          // b with zeta == z0 * 2^b and b on the menu, else -1
+        if (zeta % z0 != 0) return -1;
+        for (int b = 0; b < 7; ++b)
+            if (zeta / z0 == (1 << b) && ((SpecFree32::mask(0) >> b) & 1u)) return b;
+        return -1;
+    };
+    // base exponents per (kind, radius): the zeta values of the class in ascending order, each joins the first zeta0 that holds it
+    struct Cls { double rc2; int wide; std::vector<int> zetas, z0; };
+    std::vector<Cls> classes;
+    for (const auto& grp : groups)
+        for (const auto& f : grp) {
+            if (f.eta * 3.0 * f.rc2 > 700.0) return false;
+            Cls* c = nullptr;
+            for (auto& q : classes)
+                if (q.rc2 == f.rc2 && q.wide == f.wide) c = &q;
+            if (!c) { classes.push_back(Cls{f.rc2, f.wide, {}, {}}); c = &classes.back(); }
+            bool have = false;
+            for (int z : c->zetas) have |= z == f.izeta;
+            if (!have) c->zetas.push_back(f.izeta);
+        }
+    if (classes.empty()) return false;
+    for (auto& c : classes) {
+        std::sort(c.zetas.begin(), c.zetas.end());
+        for (int z : c.zetas) {
+            bool covered = false;
+            for (int z0 : c.z0) covered |= menu_bit(z, z0) >= 0;
+            if (!covered) c.z0.push_back(z);
+        }
+    }
+    auto base_of = [&](const AngularSF& f) {
+        for (const auto& c : classes)
+            if (c.rc2 == f.rc2 && c.wide == f.wide)
+                for (int z0 : c.z0)
+                    if (menu_bit(f.izeta, z0) >= 0) return z0;
+        return 0;
+    };
     std::vector<Key> keys;
     for (const auto& grp : groups)
         for (const auto& f : grp) {
-            bool zok = false;
-            for (int b = 0; b < 7; ++b) zok |= (f.izeta == (1 << b)) && ((SpecFree32::mask(0) >> b) & 1u);
-            if (!zok) return false;
-            if (f.eta * 3.0 * f.rc2 > 700.0) return false;
+            const int z0 = base_of(f);
             bool seen = false;
-            for (const Key& k : keys) seen |= (k.rc2 == f.rc2 && k.eta == f.eta && k.wide == f.wide);
-            if (!seen) keys.push_back(Key{f.rc2, f.eta, f.k2, f.wide});
+            for (const Key& k : keys) seen |= (k.rc2 == f.rc2 && k.eta == f.eta && k.wide == f.wide && k.z0 == z0);
+            if (!seen) keys.push_back(Key{f.rc2, f.eta, f.k2, f.wide, z0});
         }
-    if (keys.empty()) return false;
-    auto before = [](const Key& a, const Key& b) {              // sort: narrow first, rc descending, eta ascending
+    auto before = [](const Key& a, const Key& b) {              // sort: narrow first, rc descending, zeta0 and eta ascending
         if (a.wide != b.wide) return a.wide < b.wide;
         if (a.rc2 != b.rc2) return a.rc2 > b.rc2;
+        if (a.z0 != b.z0) return a.z0 < b.z0;
         return a.eta < b.eta;
     };
     for (size_t x = 0; x < keys.size(); ++x)
@@ -237,9 +272,8 @@ static bool build_passes(const std::vector<std::vector<AngularSF>>& groups, doub
     size_t x = 0;
     while (x < keys.size()) {
         size_t y = x;
-        while (y < keys.size() && keys[y].rc2 == keys[x].rc2 && keys[y].wide == keys[x].wide) ++y;
+        while (y < keys.size() && keys[y].rc2 == keys[x].rc2 && keys[y].wide == keys[x].wide && keys[y].z0 == keys[x].z0) ++y;
         const int n = (int)(y - x), chunks = (n + MAX_ETA - 1) / MAX_ETA;
-        const int class_first = np;
         for (int c = 0; c < chunks; ++c) {
             if (np >= MAX_PASS) return false;
             const int lo = (int)x + (n * c) / chunks, hi = (int)x + (n * (c + 1)) / chunks;
@@ -251,18 +285,18 @@ static bool build_passes(const std::vector<std::vector<AngularSF>>& groups, doub
             ps.k2 = keys[lo].k2;                            // k2_of(rc_p), as stored with the symmetry function
             ps.own_rc = ps.rc2 != rc * rc ? 1 : 0;
             ps.wide = keys[lo].wide;
+            ps.zeta0 = keys[lo].z0;
             ps.spec = ps.n_eta <= SpecFree16::NETA ? ANG_FREE16 : ANG_FREE32;
             for (size_t pr = 0; pr < groups.size(); ++pr) {
                 for (int e = 0; e < MAX_ETA; ++e)
                     for (int b = 0; b < 16; ++b) ps.g[pr][e][b] = -1;
                 for (const auto& f : groups[pr]) {
-                    if (f.rc2 != ps.rc2 || f.wide != ps.wide) continue;
+                    if (f.rc2 != ps.rc2 || f.wide != ps.wide || base_of(f) != ps.zeta0) continue;
                     int e = -1;
                     for (int q = ps.n_eta - 1; q >= 0; --q)
                         if (ps.eta[q] == f.eta) e = q;
                     if (e < 0) continue;
-                    int bit = 0;
-                    while ((1 << bit) != f.izeta) ++bit;
+                    int bit = menu_bit(f.izeta, ps.zeta0);
                     if (f.lam < 0) bit += 8;
                     if (ps.g[pr][e][bit] >= 0) return false;    // the same (rc, eta, lambda, zeta) twice in a pair group
                     ps.g[pr][e][bit] = (int16_t)f.g;
@@ -270,8 +304,8 @@ static bool build_passes(const std::vector<std::vector<AngularSF>>& groups, doub
                 }
             }
         }
-        (void)class_first;     // (an in-kernel loop over the passes of one radius was measured: +7 % on single-pass tables for
-                               //  the loop structure, -3 % on a three-pass table -- the triplet loops dominate, not the staging)
+        // (an in-kernel loop over the passes of one radius was measured: +7 % on single-pass tables for the loop structure,
+        //  -3 % on a three-pass table -- the triplet loops dominate, not the staging)
         x = y;
     }
     P->n_pass = np;

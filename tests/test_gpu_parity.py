@@ -99,9 +99,11 @@ def test_wide_model_small_system():
     _check_full(W.make_model(True), sysm)
 
 
-def test_generic_table_three_elements():
-    # irregular table: zeta = 3, Rs != 0, a missing pair group, an element with few SFs,
-    # different hidden sizes -> the generic angular kernel and the generic network tiles
+@pytest.mark.parametrize("route", ["multi", "generic"])
+def test_generic_table_three_elements(route):
+    # irregular table: zeta = 3 and 6, Rs != 0, a missing pair group, an element with few SFs, different hidden sizes ->
+    # passes with base exponents 1 and 3 of the lane-owned kernels ("multi"), or -- with one symmetry function listed
+    # twice, which no pass menu can hold -- the generic angular kernels; the generic network tiles either way
     rows = []
     for c in range(3):
         for e1 in range(3):
@@ -111,14 +113,14 @@ def test_generic_table_three_elements():
             rows.append((c, 3, e1, e2, 0.002, 1.0, 3.0))
             rows.append((c, 3, e2, e1, 0.013, -1.0, 1.0))
             rows.append((c, 3, e1, e2, 0.002, -1.0, 6.0))
+        if route == "generic":
+            rows.append((c, 3, 0, 1, 0.002, 1.0, 3.0))
     rows = [r if len(r) == 8 else (r[0], r[1], r[2], r[3], r[4], 0.0, r[5], r[6]) for r in rows]
     model = tiny_model(rows, n_elem=3, hidden=(7, 5, 3), seed=11)
     sysm = W.make_water(120, 5, L=15.0)
     sysm.types = (np.arange(sysm.n_atoms) % 3).astype(np.int32)
-    from paper_2002_00054_b200 import NNP
-    nnp = NNP.from_model(model)
-    assert not nnp.uses_fast_path()
-    nnp.close()
+    from paper_2002_00054_b200.binding import table_kernels
+    assert table_kernels(model) == (route,) * 3
     _check_full(model, sysm)
 
 
@@ -281,7 +283,7 @@ def test_small_neighbourhood_kernels(elements):
 
 def test_wide_angular_mixed_with_narrow():
     # wide angular SFs (n2p2 kind 9: no r_jk term, no r_jk cutoff) next to narrow ones in the
-    # same pair group; a table that holds one runs on the generic kernels with the FP32 r_jk screen disabled
+    # same pair group: passes of their own on the lane-owned kernels, or the generic kernels with the FP32 r_jk screen disabled
     rows = []
     for c in range(2):
         for e1 in range(2):
@@ -296,11 +298,16 @@ def test_wide_angular_mixed_with_narrow():
     assert table_kernels(model) == ("multi", "multi")     # zeta in {1, 2, 4, 16}: narrow and wide passes of the lane-owned kernels
     _check_full(model, W.make_water(150, 5, L=16.7))
     _check_full(model, W.make_water(80, 21, L=12.2))      # dense: ~115 neighbours, 6,500 pairs per centre in the wide passes
-    # wide only, one element (zeta = 3: the generic kernels)
+    # wide only, one element, zeta = 3: a wide pass with base exponent 3; with a function listed twice: the generic kernels
     rows = [(0, 2, 0, 0, 0.05, 0.0, 0.0, 0.0), (0, 9, 0, 0, 0.02, 0.0, -1.0, 3.0), (0, 9, 0, 0, 0.001, 0.0, 1.0, 1.0)]
     sysm = W.make_water(60, 3, L=12.4)
     sysm.types[:] = 0
+    assert table_kernels(tiny_model(rows, hidden=(4,), seed=3)) == ("multi",)
     _check_full(tiny_model(rows, hidden=(4,), seed=3), sysm)
+    assert table_kernels(tiny_model(rows + rows[1:2], hidden=(4,), seed=3)) == ("generic",)
+    _check_full(tiny_model(rows + rows[1:2], hidden=(4,), seed=3), sysm)
+    # narrow and wide in one pair group on the generic kernels (a narrow function listed twice)
+    _check_full(tiny_model(rows + [(0, 3, 0, 0, 0.004, 0.0, 1.0, 2.0)] * 2, hidden=(4,), seed=3), sysm)
 
 
 def test_per_sf_cutoff_radii():
@@ -319,7 +326,7 @@ def test_per_sf_cutoff_radii():
     model = tiny_model(rows, n_elem=2, hidden=(5, 4), seed=31)
     model.sf_cutoffs = rcs
     _check_full(model, W.make_water(150, 5, L=16.7))
-    # only ONE element of the base-52 model gets shorter radii: it moves to the generic kernels, the other
+    # only ONE element of the base-52 model gets shorter radii: it moves to several passes (radial radii: generic radial-only mode), the other
     # stays on the lane-owned fast path; then back to the global rc: bit-identical to a fresh model
     from paper_2002_00054_b200 import NNP
     sysm, base = W.build(W.CONFIGS[0])
@@ -680,7 +687,10 @@ def test_deterministic_forces(which):
             for (e1, e2) in ((0, 0), (0, 1), (1, 1)):
                 rows.append((c, 3, e1, e2, 0.004, 0.0, 1.0, 3.0))
                 rows.append((c, 9, e1, e2, 0.010, 0.0, -1.0, 1.0))
+            rows.append(rows[-1])                                # listed twice: no pass menu holds it -> the generic kernels
         model = tiny_model(rows, n_elem=2, hidden=(5, 4), seed=21)
+        from paper_2002_00054_b200.binding import table_kernels
+        assert table_kernels(model) == ("generic", "generic")
         sysm = W.make_water(700, 4242)
     nnp = NNP.from_model(model)
     if "max_neighbors" in kw:
