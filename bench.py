@@ -336,6 +336,10 @@ def main():
                     help="probe of what a Verlet-skin neighbour list would cost the hot kernels: the neighbour list is built "
                          "with rc + SKIN while every symmetry function keeps its cutoff (nnp_set_sf_cutoffs), i.e. exactly the "
                          "list a skin scheme would hand the kernels on its reuse steps; the list is still rebuilt every call")
+    ap.add_argument("--reuse-skin", type=float, default=0.0,
+                    help="nnp_set_neighbor_skin: keep a candidate list of radius rc + SKIN across calls and filter the exact list "
+                         "from it; rebuilt when an atom has moved SKIN/2 (decided on the device).  Not the headline: BASELINE.json's "
+                         "metric rebuilds the list every call.  With static positions (no --md) no timed call rebuilds")
     ap.add_argument("--deterministic", action="store_true",
                     help="nnp_set_deterministic_forces: fixed-point force accumulation (bit-reproducible forces)")
     ap.add_argument("--no-probe", action="store_true", help="skip the DFMA issue-rate probe (for ncu runs)")
@@ -399,6 +403,8 @@ def main():
         nnp.set_deterministic_forces(True)
     if cfg.kind == "metal":
         nnp.set_max_neighbors(32)      # 18 neighbours per atom: the 8-lanes-per-centre kernels of k_small.cu
+    if args.reuse_skin > 0.0:
+        nnp.set_neighbor_skin(args.reuse_skin)
     pos = torch.tensor(sysm.pos, dtype=torch.float64, device=dev)
     typ = torch.tensor(sysm.types, dtype=torch.int32, device=dev)
     out = (torch.empty(n, dtype=torch.float64, device=dev), torch.empty(1, dtype=torch.float64, device=dev),
@@ -455,6 +461,10 @@ def main():
     nnp.sync_status()
     nnp.set_timing(False)
     ms = max_over_ranks(ms, dev)
+    rebuild_note = "every call"
+    if args.reuse_skin > 0.0:
+        calls, rebuilds = nnp.neighbor_rebuilds()
+        rebuild_note = "skin %.2f A: %d rebuilds in %d calls (warm-up included)" % (args.reuse_skin, rebuilds, calls)
 
     # per-stage average over K more (untimed for the headline) steps, events inside nnp_compute
     nnp.set_timing(True)
@@ -502,7 +512,7 @@ def main():
     total_instr = instr["total"] * n
     hbm_bytes_per_atom = 1.0e3 if cfg.kind == "metal" else (2.8e3 if not cfg.wide else 5.2e3)
     # the dominant kernel: k_force2<...> (not its list-driven sibling for the few big centres), k_force_small on the metal workload
-    baseline_table = args.table == "baseline" and args.precision == "f64" and args.skin == 0.0
+    baseline_table = args.table == "baseline" and args.precision == "f64" and args.skin == 0.0 and args.reuse_skin == 0.0
     if baseline_table:
         ncu, ncu_src = _ncu_launch_metrics(args.config, r"k_force2<|k_force_small<")
     else:
@@ -555,7 +565,7 @@ def main():
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64" if args.precision == "f64" else "f32-stage/f64-acc", "data": "synthetic",
         "config": {"workload": cfg.name, "n_atoms": n, "model": model.name, "kernels": list(table_kernels(model)), "box": float(sysm.box[0]),
-                   "neighbor_rebuild": "every call", "md": bool(args.md),
+                   "neighbor_rebuild": rebuild_note, "md": bool(args.md),
                    "force_accumulation": "fixed-point 2^-40 eV/A (bit-reproducible)" if args.deterministic else "FP64 atomics", "parallelism": "replicas x%d" % world,
                    "l2": ("working set per step (%.2f GB workspace) %s the 126 MB L2; no flush between steps"
                           % (nnp.workspace_bytes(n) / 1e9, "exceeds" if nnp.workspace_bytes(n) > 126e6 else "FITS IN"))},

@@ -124,6 +124,27 @@ void nnp_destroy(nnp_model* m);
  * (below 32: NNP_ERR_INVALID_ARG; above 255: NNP_ERR_LIMIT -- the kernels address neighbour slots with 8 bits). */
 nnp_status nnp_set_max_neighbors(nnp_model* m, int32_t max_neighbors);
 
+/* Neighbour-list reuse with a Verlet skin ("neighbor list", L116; an MD code rebuilds its
+ * list only every few steps).  skin in Angstrom, 0 <= skin <= rc; 0 (the default) = every nnp_compute bins, sorts and
+ * searches the cells again.  With skin > 0 nnp_compute keeps, in the CALLER'S workspace, the sorted order and a
+ * candidate list of radius rc + skin from the last rebuild, and every call
+ *   1. checks on the device whether any atom has moved more than skin/2 since that rebuild (minimum image) or changed
+ *      its type -- then, or when the workspace pointer, n_atoms or the box differ from the last call (host-side check),
+ *      it rebuilds: sort + cell search with rc + skin;
+ *   2. filters the exact list N(i) = { j : r_ij < rc } of THIS call's positions out of the candidate list with the same
+ *      FP64 predicate as a fresh build.
+ * Results are those of skin = 0: the same neighbour sets bit for bit, energies and forces up to summation order.
+ * The decision is taken on the device, so the launch sequence is fixed (nnp_md_run replays it as a CUDA graph).
+ * The caller must leave the workspace content untouched between calls (or call nnp_invalidate_neighbors);
+ * nnp_workspace_bytes grows by the candidate list (about max_neighbors * ((rc+skin)/rc)^3 * 4 B per atom) -- query it
+ * AFTER this call.  Box lengths must be >= 2 (rc + skin).  A candidate row that overflows reports
+ * NNP_ERR_NEIGHBOR_OVERFLOW like an exact row.  Errors: NNP_ERR_INVALID_ARG (skin < 0, not finite, > rc). */
+nnp_status nnp_set_neighbor_skin(nnp_model* m, double skin);
+/* Forget the candidate list: the next nnp_compute rebuilds (use after writing into the workspace). */
+nnp_status nnp_invalidate_neighbors(nnp_model* m);
+/* Calls and rebuilds since nnp_set_neighbor_skin (synchronises the stream of the last call; host pointers). */
+nnp_status nnp_get_neighbor_rebuilds(nnp_model* m, int64_t* n_calls, int64_t* n_rebuilds);
+
 /* Bytes of device workspace nnp_compute needs for n_atoms (0 on error): sorted coordinates, neighbour rows, G and
  * dE/dG rows, screening masks -- about 2.9 KB per atom for the base-52 model.  The derivative tensor dG/dr is never
  * stored ("store and move as little data as possible, recomputing where necessary"; L82: what lets

@@ -22,7 +22,7 @@ STAGE_NAMES = ("sort", "neighbors", "symmetry_functions", "networks", "forces", 
 
 # every symbol include/nnp.h declares
 EXPORTS = ("nnp_create", "nnp_table_kernels", "nnp_destroy", "nnp_set_max_neighbors", "nnp_workspace_bytes", "nnp_compute",
-           "nnp_compute_host", "nnp_set_sf_scaling", "nnp_set_activation", "nnp_set_sf_cutoffs", "nnp_set_precision", "nnp_set_deterministic_forces", "nnp_md_run", "nnp_md_kinetic_energy", "nnp_sync_status", "nnp_get_neighbor_counts", "nnp_get_neighbors", "nnp_get_sf",
+           "nnp_compute_host", "nnp_set_sf_scaling", "nnp_set_activation", "nnp_set_sf_cutoffs", "nnp_set_precision", "nnp_set_deterministic_forces", "nnp_set_neighbor_skin", "nnp_invalidate_neighbors", "nnp_get_neighbor_rebuilds", "nnp_md_run", "nnp_md_kinetic_energy", "nnp_sync_status", "nnp_get_neighbor_counts", "nnp_get_neighbors", "nnp_get_sf",
            "nnp_get_dedg", "nnp_g_stride", "nnp_set_timing", "nnp_get_timings", "nnp_last_launch_count",
            "nnp_uses_fast_path", "nnp_measure_fp64_peak", "nnp_last_error", "nnp_version")
 
@@ -91,6 +91,12 @@ def load_library():
     L.nnp_set_precision.argtypes = [vp, i32]
     L.nnp_set_deterministic_forces.restype = C.c_int
     L.nnp_set_deterministic_forces.argtypes = [vp, i32]
+    L.nnp_set_neighbor_skin.restype = C.c_int
+    L.nnp_set_neighbor_skin.argtypes = [vp, C.c_double]
+    L.nnp_invalidate_neighbors.restype = C.c_int
+    L.nnp_invalidate_neighbors.argtypes = [vp]
+    L.nnp_get_neighbor_rebuilds.restype = C.c_int
+    L.nnp_get_neighbor_rebuilds.argtypes = [vp, vp, vp]
     L.nnp_md_run.restype = C.c_int
     L.nnp_md_run.argtypes = [vp, i32, dbl, C.POINTER(dbl), i64, vp, vp, vp, C.POINTER(dbl), vp, vp, vp, vp,
                              C.c_size_t, vp]
@@ -262,6 +268,21 @@ class NNP:
     def set_precision(self, mode):
         """"f64" (default) or "mixed" (FP32 staging and per-triplet arithmetic; include/nnp.h nnp_set_precision)."""
         self._check(self._L.nnp_set_precision(self._h, {"f64": 0, "mixed": 1}[mode]))
+
+    def set_neighbor_skin(self, skin: float):
+        """nnp_set_neighbor_skin: reuse the neighbour list across calls with a Verlet skin (Angstrom; 0 = off)."""
+        self._check(self._L.nnp_set_neighbor_skin(self._h, float(skin)))
+        self._ws = None            # the workspace grows by the candidate list
+        self._ws_n = -1
+
+    def invalidate_neighbors(self):
+        self._check(self._L.nnp_invalidate_neighbors(self._h))
+
+    def neighbor_rebuilds(self):
+        """(calls, rebuilds) since set_neighbor_skin."""
+        a, b = C.c_int64(0), C.c_int64(0)
+        self._check(self._L.nnp_get_neighbor_rebuilds(self._h, C.byref(a), C.byref(b)))
+        return int(a.value), int(b.value)
 
     def set_deterministic_forces(self, on: bool):
         """Fixed-point (2^-40 eV/A) global force accumulation: bit-reproducible forces (include/nnp.h)."""

@@ -27,7 +27,8 @@ __global__ void __launch_bounds__(NB_WARPS * 32)
 k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
             const double* __restrict__ sx, const double* __restrict__ sy, const double* __restrict__ sz,
             const int32_t* __restrict__ cell_start, int32_t* __restrict__ nbr, int32_t* __restrict__ nbr_cnt,
-            int32_t* __restrict__ status, int32_t* __restrict__ sticky) {
+            int32_t* __restrict__ status, int32_t* __restrict__ sticky, const int32_t* __restrict__ cond) {
+    if (cond && *cond == 0) return;          // neighbour-skin mode: the candidate list of an earlier call still holds
     const int lane = threadIdx.x & 31;
     const int64_t i = (int64_t)blockIdx.x * NB_WARPS + (threadIdx.x >> 5);
     if (i >= n) return;
@@ -109,13 +110,101 @@ k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
     }
 }
 
+// Neighbour-skin mode, every call: the exact list N(i) of THIS call's positions, filtered from the candidate list
+// (radius rc + skin, built by k_neighbors on the last rebuild) with the same FP64 predicate as a fresh build -- the
+// symmetry-function and force kernels never see a slot beyond rc (staging the extra ~27 % of slots cost them 7x what
+// a rebuild costs: DESIGN.md 11a).  A candidate row is grouped by element and so is the filtered row.  LPA lanes per
+// atom, UN candidates per lane in flight (the loop is latency-bound; one chunk covers the short rows of a metal).
+template <int LPA, int UN>
+__global__ void __launch_bounds__(256)
+k_filter(int64_t n, int n_elem, Grid g, double rc2, int sstride, int stride, int max_nbr,
+         const double* __restrict__ sx, const double* __restrict__ sy, const double* __restrict__ sz,
+         const int32_t* __restrict__ snbr, const int32_t* __restrict__ snbr_cnt, int32_t* __restrict__ nbr,
+         int32_t* __restrict__ nbr_cnt, int32_t* __restrict__ status, int32_t* __restrict__ sticky,
+         const int32_t* __restrict__ flag, int32_t* __restrict__ stats) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) {           // [0] calls, [1] rebuilds since nnp_set_neighbor_skin
+        atomicAdd(&stats[0], 1);
+        if (*flag != 0) atomicAdd(&stats[1], 1);
+    }
+    const int sub = threadIdx.x & (LPA - 1);
+    const int64_t i = ((int64_t)blockIdx.x * 256 + threadIdx.x) / LPA;
+    const unsigned gmask = LPA == 32 ? 0xffffffffu : (((1u << LPA) - 1u) << ((threadIdx.x & 31) & ~(LPA - 1)));
+    const bool live = i < n;
+    const int64_t ii = live ? i : n - 1;                 // idle groups of the last warp replay the last atom, writes off
+    const double xi = sx[ii], yi = sy[ii], zi = sz[ii];
+    const int32_t* __restrict__ srow = snbr + (size_t)ii * sstride;
+    int32_t* __restrict__ row = nbr + (size_t)ii * stride;
+    // the candidate row is packed: element e occupies [bnd[e], bnd[e+1])
+    int bnd[MAX_ELEM + 1];
+    bnd[0] = 0;
+#pragma unroll
+    for (int e = 0; e < MAX_ELEM; ++e) bnd[e + 1] = bnd[e] + (e < n_elem ? snbr_cnt[(size_t)ii * MAX_ELEM + e] : 0);
+    const int tot = bnd[MAX_ELEM];
+    int cnt = 0;
+    int below[MAX_ELEM + 1];                             // hits among the candidates before bnd[e]
+#pragma unroll
+    for (int e = 0; e <= MAX_ELEM; ++e) below[e] = 0;
+    // UN candidates per lane in flight: the loop is latency-bound
+    for (int f0 = 0; f0 < tot; f0 += UN * LPA) {
+        int j[UN];
+        double x[UN], y[UN], z[UN];
+#pragma unroll
+        for (int u = 0; u < UN; ++u) {
+            const int f = f0 + u * LPA + sub;
+            j[u] = f < tot ? srow[f] : -1;
+        }
+#pragma unroll
+        for (int u = 0; u < UN; ++u) {
+            x[u] = y[u] = z[u] = 0.0;
+            if (j[u] >= 0) { x[u] = sx[j[u]]; y[u] = sy[j[u]]; z[u] = sz[j[u]]; }
+        }
+#pragma unroll
+        for (int u = 0; u < UN; ++u) {
+            const int f = f0 + u * LPA + sub;
+            const double dx = min_image_1d(xi, x[u], g.box[0], g.half[0]);
+            const double dy = min_image_1d(yi, y[u], g.box[1], g.half[1]);
+            const double dz = min_image_1d(zi, z[u], g.box[2], g.half[2]);
+            const bool hit = j[u] >= 0 && dist2_exact(dx, dy, dz) < rc2;
+            const unsigned m = __ballot_sync(gmask, hit);       // the groups of a warp run different trip counts
+            if (hit && live) {
+                const int p = cnt + __popc(m & ((1u << (threadIdx.x & 31)) - 1u));
+                if (p < max_nbr) row[p] = j[u];
+            }
+            cnt += __popc(m);
+#pragma unroll
+            for (int e = 1; e <= MAX_ELEM; ++e) below[e] += __popc(__ballot_sync(gmask, hit && f < bnd[e]));
+        }
+    }
+    if (sub == 0 && live) {
+#pragma unroll
+        for (int e = 0; e < MAX_ELEM; ++e)
+            nbr_cnt[(size_t)i * MAX_ELEM + e] = min(below[e + 1], max_nbr) - min(below[e], max_nbr);
+        if (cnt > max_nbr) { atomicOr(status, ST_NBR_OVERFLOW); atomicOr(sticky, ST_NBR_OVERFLOW); }
+    }
+}
+
+// skin_mode 0: the exact list straight from the cells.  Otherwise: the candidate list (radius^2 rs2, rows of sstride,
+// at most smax entries) if this call rebuilds, then the filter.
 int launch_neighbors(const Workspace& w, const Grid& g, int64_t n, int n_elem, double rc2, int stride,
-                     int max_nbr, cudaStream_t st) {
+                     int max_nbr, int skin_mode, double rs2, int sstride, int smax, cudaStream_t st) {
     if (n == 0) return 0;
     const unsigned nb = (unsigned)((n + NB_WARPS - 1) / NB_WARPS);
-    k_neighbors<<<nb, NB_WARPS * 32, 0, st>>>(n, n_elem, g, rc2, stride, max_nbr, w.sx, w.sy, w.sz, w.cell_start,
-                                              w.nbr, w.nbr_cnt, w.status, w.sticky);
-    return 1;
+    if (skin_mode == 0) {
+        k_neighbors<<<nb, NB_WARPS * 32, 0, st>>>(n, n_elem, g, rc2, stride, max_nbr, w.sx, w.sy, w.sz, w.cell_start,
+                                                  w.nbr, w.nbr_cnt, w.status, w.sticky, nullptr);
+        return 1;
+    }
+    k_neighbors<<<nb, NB_WARPS * 32, 0, st>>>(n, n_elem, g, rs2, sstride, smax, w.sx, w.sy, w.sz, w.cell_start,
+                                              w.snbr, w.snbr_cnt, w.status, w.sticky, w.skin_flag);
+#define NNP_FILTER(LPA, UN)                                                                                         \
+    k_filter<LPA, UN><<<(unsigned)((n * LPA + 255) / 256), 256, 0, st>>>(n, n_elem, g, rc2, sstride, stride, max_nbr, w.sx, w.sy, \
+                                                                         w.sz, w.snbr, w.snbr_cnt, w.nbr, w.nbr_cnt, w.status,   \
+                                                                         w.sticky, w.skin_flag, w.skin_stats)
+    if (smax <= 64) NNP_FILTER(32, 1);           // metals: ~26 candidates, one chunk
+    else if (smax <= 128) NNP_FILTER(32, 2);
+    else NNP_FILTER(32, 4);                      // water-like: ~120 candidates
+#undef NNP_FILTER
+    return 2;
 }
 
 }  // namespace nnp

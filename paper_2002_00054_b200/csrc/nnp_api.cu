@@ -41,6 +41,13 @@ struct nnp_model {
     int last_launches = 0;
     int32_t* h_status = nullptr;   // pinned
     int32_t* d_sticky = nullptr;   // device word: OR of the status flags of every call since the last nnp_sync_status
+    // neighbour-skin mode (nnp_set_neighbor_skin): what the candidate list in the caller's workspace was built for
+    double skin = 0.0;
+    int32_t* d_skin_stats = nullptr;   // [2]: calls, rebuilds
+    bool skin_valid = false;
+    void* skin_ws = nullptr;
+    int64_t skin_n = 0;
+    double skin_box[3] = {0.0, 0.0, 0.0};
     // timing
     bool timing = false;
     bool timing_valid = false;
@@ -103,7 +110,7 @@ struct DeviceGuard {
 
 static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
-static size_t ws_layout(Workspace* w, void* base, int64_t n, int n_elem, int stride, int g_stride) {
+static size_t ws_layout(Workspace* w, void* base, int64_t n, int n_elem, int stride, int g_stride, int sstride) {
     size_t off = 0;
     auto take = [&](size_t bytes) -> void* {
         void* p = base ? (void*)((char*)base + off) : nullptr;
@@ -121,6 +128,13 @@ static size_t ws_layout(Workspace* w, void* base, int64_t n, int n_elem, int str
     w->scan_tmp = (int32_t*)take((size_t)w->scan_tmp_len * 4);
     w->nbr = (int32_t*)take(N * (size_t)stride * 4);
     w->nbr_cnt = (int32_t*)take(N * MAX_ELEM * 4);
+    w->snbr = nullptr; w->snbr_cnt = nullptr; w->bx = w->by = w->bz = nullptr; w->skin_flag = nullptr; w->skin_stats = nullptr;
+    if (sstride > 0) {
+        w->snbr = (int32_t*)take(N * (size_t)sstride * 4);
+        w->snbr_cnt = (int32_t*)take(N * MAX_ELEM * 4);
+        w->bx = (double*)take(N * 8); w->by = (double*)take(N * 8); w->bz = (double*)take(N * 8);
+        w->skin_flag = (int32_t*)take(64);
+    }
     w->G = (double*)take(N * (size_t)g_stride * 8);
     w->dEdG = (double*)take(N * (size_t)g_stride * 8);
     w->e_sorted = (double*)take(N * 8);
@@ -560,6 +574,7 @@ extern "C" nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* co
         std::memset(m->h_status, 0, 64);
         if (cudaMalloc(&m->d_sticky, 64) != cudaSuccess || cudaMemset(m->d_sticky, 0, 64) != cudaSuccess)
             return bail(NNP_ERR_CUDA, "cudaMalloc failed");
+        m->d_skin_stats = m->d_sticky + 4;       // words 4, 5 of the same allocation
     }
     m->h_prog = progs;
     set_pass_info(m, progs);
@@ -706,15 +721,55 @@ extern "C" nnp_status nnp_set_max_neighbors(nnp_model* m, int32_t max_neighbors)
         return fail(m, NNP_ERR_LIMIT, "max_neighbors > NNP_MAX_NEIGHBORS (255): the kernels address neighbour slots with 8 bits");
     m->max_nbr = max_neighbors;
     m->have_ws = false;
+    m->skin_valid = false;
+    return NNP_OK;
+}
+
+extern "C" nnp_status nnp_set_neighbor_skin(nnp_model* m, double skin) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    if (!(skin >= 0.0) || !std::isfinite(skin)) return fail(m, NNP_ERR_INVALID_ARG, "skin must be finite and >= 0");
+    if (skin > m->rc) return fail(m, NNP_ERR_INVALID_ARG, "skin > rc");
+    DeviceGuard dg(m->device);
+    if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
+    if (m->have_ws) NNP_CUDA(m, cudaStreamSynchronize(m->last_stream));
+    NNP_CUDA(m, cudaMemset(m->d_skin_stats, 0, 2 * sizeof(int32_t)));
+    m->skin = skin;
+    m->skin_valid = false;
+    m->have_ws = false;              // the workspace layout changes
+    return NNP_OK;
+}
+
+extern "C" nnp_status nnp_invalidate_neighbors(nnp_model* m) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    m->skin_valid = false;
+    return NNP_OK;
+}
+
+extern "C" nnp_status nnp_get_neighbor_rebuilds(nnp_model* m, int64_t* n_calls, int64_t* n_rebuilds) {
+    if (!m || !n_calls || !n_rebuilds) return NNP_ERR_INVALID_ARG;
+    DeviceGuard dg(m->device);
+    if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
+    if (m->have_ws) NNP_CUDA(m, cudaStreamSynchronize(m->last_stream));
+    int32_t h[2] = {0, 0};
+    NNP_CUDA(m, cudaMemcpy(h, m->d_skin_stats, sizeof(h), cudaMemcpyDeviceToHost));
+    *n_calls = h[0];
+    *n_rebuilds = h[1];
     return NNP_OK;
 }
 
 static int row_stride(const nnp_model* m) { return (m->max_nbr + 7) & ~7; }
+// neighbour-skin mode: capacity of a candidate row = max_neighbors scaled by the volume ratio of the two spheres, plus slack
+static int skin_max(const nnp_model* m) {
+    if (!(m->skin > 0.0)) return 0;
+    const double r = (m->rc + m->skin) / m->rc;
+    return (int)std::ceil(m->max_nbr * r * r * r) + 16;
+}
+static int skin_stride(const nnp_model* m) { return (skin_max(m) + 7) & ~7; }
 
 extern "C" size_t nnp_workspace_bytes(const nnp_model* m, int64_t n_atoms) {
     if (!m || n_atoms < 0) return 0;
     Workspace w;
-    return ws_layout(&w, nullptr, n_atoms, m->n_elem, row_stride(m), m->g_stride);
+    return ws_layout(&w, nullptr, n_atoms, m->n_elem, row_stride(m), m->g_stride, skin_stride(m));
 }
 
 extern "C" int32_t nnp_g_stride(const nnp_model* m) { return m ? m->g_stride : 0; }
@@ -739,19 +794,25 @@ extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d
     if (n_atoms > 0 && (!d_pos || !d_type || !d_e_atom || !d_force)) return fail(m, NNP_ERR_INVALID_ARG, "null array");
     for (int c = 0; c < 3; ++c) {
         if (!std::isfinite(box[c]) || !(box[c] > 0.0)) return fail(m, NNP_ERR_INVALID_ARG, "box length must be finite and > 0");
-        if (box[c] < 2.0 * m->rc) return fail(m, NNP_ERR_BOX_TOO_SMALL, "box length < 2*rc");
+        if (box[c] < 2.0 * (m->rc + m->skin)) return fail(m, NNP_ERR_BOX_TOO_SMALL, "box length < 2*(rc + skin)");
     }
     const int stride = row_stride(m);
     Workspace w;
-    const size_t need = ws_layout(&w, d_workspace, n_atoms, m->n_elem, stride, m->g_stride);
+    const size_t need = ws_layout(&w, d_workspace, n_atoms, m->n_elem, stride, m->g_stride, skin_stride(m));
     if (!d_workspace || ((uintptr_t)d_workspace & 255u) || workspace_bytes < need)
         return fail(m, NNP_ERR_WORKSPACE, "workspace null, misaligned or too small");
     w.sticky = m->d_sticky;
+    w.skin_stats = m->d_skin_stats;
     DeviceGuard dg(m->device);
     if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
     cudaStream_t st = (cudaStream_t)cuda_stream;
     Grid g;
-    make_grid(&g, box, m->rc, n_atoms);
+    make_grid(&g, box, m->rc + m->skin, n_atoms);
+    // neighbour-skin mode: 1 = this call must rebuild (nothing valid in this workspace for this n and box), 2 = the device decides
+    int skin_mode = 0;
+    if (m->skin > 0.0)
+        skin_mode = (m->skin_valid && m->skin_ws == d_workspace && m->skin_n == n_atoms && m->skin_box[0] == box[0] &&
+                     m->skin_box[1] == box[1] && m->skin_box[2] == box[2]) ? 2 : 1;
     if (m->timing && !m->ev_created) {
         for (int k = 0; k <= NNP_N_STAGES; ++k) NNP_CUDA(m, cudaEventCreate(&m->ev[k]));
         m->ev_created = true;
@@ -765,12 +826,18 @@ extern "C" nnp_status nnp_compute(nnp_model* m, int64_t n_atoms, const double* d
         NNP_CUDA(m, cudaMemsetAsync(w.status, 0, sizeof(int32_t) * 4, st));
         m->timing_valid = false;
         m->ws = w; m->have_ws = true; m->last_n = 0; m->last_stream = st; m->last_launches = 0;
+        m->skin_valid = false;
         return NNP_OK;
     }
     mark(0);
-    launches += launch_sort(w, g, n_atoms, m->n_elem, d_pos, d_type, st);
+    launches += launch_sort(w, g, n_atoms, m->n_elem, d_pos, d_type, skin_mode, m->skin, st);
     mark(1);
-    launches += launch_neighbors(w, g, n_atoms, m->n_elem, m->rc * m->rc, stride, m->max_nbr, st);
+    launches += launch_neighbors(w, g, n_atoms, m->n_elem, m->rc * m->rc, stride, m->max_nbr, skin_mode,
+                                 (m->rc + m->skin) * (m->rc + m->skin), skin_stride(m), skin_max(m), st);
+    if (skin_mode) {
+        m->skin_valid = true; m->skin_ws = d_workspace; m->skin_n = n_atoms;
+        for (int c = 0; c < 3; ++c) m->skin_box[c] = box[c];
+    }
     mark(2);
     launches += launch_word_offsets(w, g, n_atoms, m->n_elem, m->d_prog, st);
     launches += launch_sf(w, g, n_atoms, m->n_elem, m->d_prog, m->variant, m->passes, m->rc, stride, m->max_nbr, m->g_stride, m->na_max, m->precision, st);
@@ -871,7 +938,7 @@ extern "C" nnp_status nnp_md_kinetic_energy(nnp_model* m, const double* h_mass, 
     if (!m) return NNP_ERR_INVALID_ARG;
     if (!h_mass || !d_ekin || n_atoms < 0 || (n_atoms > 0 && (!d_vel || !d_type))) return fail(m, NNP_ERR_INVALID_ARG, "null array");
     Workspace w;
-    const size_t need = ws_layout(&w, d_workspace, n_atoms, m->n_elem, row_stride(m), m->g_stride);
+    const size_t need = ws_layout(&w, d_workspace, n_atoms, m->n_elem, row_stride(m), m->g_stride, skin_stride(m));
     if (!d_workspace || ((uintptr_t)d_workspace & 255u) || workspace_bytes < need)
         return fail(m, NNP_ERR_WORKSPACE, "workspace null, misaligned or too small");
     DeviceGuard dg(m->device);

@@ -143,6 +143,13 @@ struct Workspace {
     int32_t *scan_tmp;               // block sums of the scans
     int32_t *nbr;                    // [N][stride] neighbour positions (sorted space), grouped by element
     int32_t *nbr_cnt;                // [N][MAX_ELEM] neighbours of each element
+    // neighbour-skin mode (nnp_set_neighbor_skin; absent from the layout otherwise).  These, perm and cell_start are the
+    // state a call that does not rebuild relies on: the caller keeps the workspace intact between calls.
+    int32_t *snbr;                   // [N][sstride] candidate list of the last rebuild (radius rc + skin), grouped by element
+    int32_t *snbr_cnt;               // [N][MAX_ELEM]
+    double *bx, *by, *bz;            // [N] wrapped positions at the last rebuild, sorted order
+    int32_t *skin_flag;              // device word: this call rebuilds (set by the host or by k_skin_check)
+    int32_t *skin_stats;             // model-owned: [0] calls, [1] rebuilds since nnp_set_neighbor_skin
     double *G, *dEdG;                // [N][g_stride], sorted order
     double *e_sorted;                // [N]
     double *f_sorted;                // [N][3]
@@ -205,10 +212,11 @@ __device__ __forceinline__ void force_add(const P& p, size_t idx, double v) {
 #endif
 
 // ---- launchers (each enqueues on `st`; returns the number of kernels launched) ----------
+// skin_mode (neighbour-skin mode, k_sort.cu): 0 off, 1 rebuild forced by the host, 2 the device decides
 int launch_sort(const Workspace& w, const Grid& g, int64_t n, int n_elem, const double* d_pos,
-                const int32_t* d_type, cudaStream_t st);
+                const int32_t* d_type, int skin_mode, double skin, cudaStream_t st);
 int launch_neighbors(const Workspace& w, const Grid& g, int64_t n, int n_elem, double rc2, int stride,
-                     int max_nbr, cudaStream_t st);
+                     int max_nbr, int skin_mode, double rs2, int sstride, int smax, cudaStream_t st);
 int launch_sf(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
               const int* variant, const PassInfo& passes, double rc, int stride, int max_nbr, int g_stride, int na_max,
               int precision, cudaStream_t st);
