@@ -1,7 +1,7 @@
 // k_neighbor.cu -- S1: full neighbour list N(i) = { j != i : |r_j - r_i|_min-image^2 < rc^2 }
 // from the (element, cell)-sorted SoA positions ("neighbor list", L116 "random
-// access (neighbor list)").  One warp per atom; the <= 18 contiguous x-runs of the 3x3(x3) cell
-// stencil are walked as one flat candidate range, hits are ballot-compacted and the row written coalesced.  Rows hold
+// access (neighbor list)").  One warp per atom; cells are rc / HW wide and the <= (2 HW + 1)^2 contiguous x-runs of the
+// cell stencil are walked as one flat candidate range, hits are ballot-compacted and the row written coalesced.  Rows hold
 // positions in the SORTED order, grouped by neighbour element (all of element 0, then 1, ...),
 // which is what lets the symmetry-function kernels run type-homogeneous segments.
 #include "geometry.cuh"
@@ -11,16 +11,22 @@ namespace nnp {
 
 constexpr int NB_WARPS = 8;
 
-// distinct periodic cells {c-1, c, c+1} along one dimension (all cells if nc <= 3)
+// distinct periodic cells {c-HW .. c+HW} along one dimension (all cells if nc <= 2 HW + 1)
+constexpr int HW = NNP_CELL_HW;                 // cells are >= rc / HW wide (make_grid)
+constexpr int SW = 2 * HW + 1;
 __device__ __forceinline__ int stencil_1d(int c, int nc, int* out) {
-    if (nc <= 3) {
+    if (nc <= SW) {
         for (int k = 0; k < nc; ++k) out[k] = k;
         return nc;
     }
-    out[0] = (c == 0) ? nc - 1 : c - 1;
-    out[1] = c;
-    out[2] = (c == nc - 1) ? 0 : c + 1;
-    return 3;
+#pragma unroll
+    for (int k = 0; k < SW; ++k) {
+        int q = c + k - HW;
+        if (q < 0) q += nc;
+        if (q >= nc) q -= nc;
+        out[k] = q;
+    }
+    return SW;
 }
 
 __global__ void __launch_bounds__(NB_WARPS * 32)
@@ -37,70 +43,71 @@ k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
     cx = min(max(cx, 0), g.nc[0] - 1);
     cy = min(max(cy, 0), g.nc[1] - 1);
     cz = min(max(cz, 0), g.nc[2] - 1);
-    int ys[3], zs[3];
+    int ys[SW], zs[SW];
     const int ny = stencil_1d(cy, g.nc[1], ys);
     const int nz = stencil_1d(cz, g.nc[2], zs);
     // x-runs: cells contiguous in memory -> at most two [first, last] cell ranges
-    int xr0[2], xr1[2], nxr;
-    if (g.nc[0] <= 3) { xr0[0] = 0; xr1[0] = g.nc[0] - 1; nxr = 1; }
-    else if (cx == 0) { xr0[0] = 0; xr1[0] = 1; xr0[1] = g.nc[0] - 1; xr1[1] = g.nc[0] - 1; nxr = 2; }
-    else if (cx == g.nc[0] - 1) { xr0[0] = 0; xr1[0] = 0; xr0[1] = cx - 1; xr1[1] = cx; nxr = 2; }
-    else { xr0[0] = cx - 1; xr1[0] = cx + 1; nxr = 1; }
+    int xr0[2], xr1[2], nxr = 1;
+    if (g.nc[0] <= SW) { xr0[0] = 0; xr1[0] = g.nc[0] - 1; }
+    else if (cx < HW) { xr0[0] = 0; xr1[0] = cx + HW; xr0[1] = g.nc[0] + cx - HW; xr1[1] = g.nc[0] - 1; nxr = 2; }
+    else if (cx + HW >= g.nc[0]) { xr0[0] = 0; xr1[0] = cx + HW - g.nc[0]; xr0[1] = cx - HW; xr1[1] = g.nc[0] - 1; nxr = 2; }
+    else { xr0[0] = cx - HW; xr1[0] = cx + HW; }
 
-    // An atom of an interior cell (and >= 4 cells along the dimension) never needs the +-L of the minimum
-    // image: its candidates are less than two cell widths <= L/2 away, so both conditions of min_image_1d
+    // An atom whose stencil does not wrap (and >= 2 SW cells along the dimension) never needs the +-L of the minimum
+    // image: its candidates are less than HW + 1 cell widths <= L/2 away, so both conditions of min_image_1d
     // are false and the raw difference IS the result (same bits).  Warp-uniform -> 12 instructions fewer
-    // per chunk of candidates for ~87 % of the atoms (the kernel is issue-bound: ncu, 83 % issue slots).
-    const bool wx = !(g.nc[0] >= 4 && cx >= 1 && cx <= g.nc[0] - 2);
-    const bool wy = !(g.nc[1] >= 4 && cy >= 1 && cy <= g.nc[1] - 2);
-    const bool wz = !(g.nc[2] >= 4 && cz >= 1 && cz <= g.nc[2] - 2);
+    // per chunk of candidates for most of the atoms (the kernel is issue-bound: ncu, 83 % issue slots).
+    const bool wx = !(g.nc[0] >= 2 * SW && cx >= HW && cx + HW < g.nc[0]);
+    const bool wy = !(g.nc[1] >= 2 * SW && cy >= HW && cy + HW < g.nc[1]);
+    const bool wz = !(g.nc[2] >= 2 * SW && cz >= HW && cz + HW < g.nc[2]);
     int32_t* row = nbr + (size_t)i * stride;
     int cnt = 0;
-    const int nrun = nz * ny * nxr;                     // <= 18 contiguous runs of candidates per element
+    const int nyz = nz * ny;                            // <= SW^2 <= 25 contiguous runs of candidates per element and x-range
     for (int e = 0; e < n_elem; ++e) {
         const int32_t* cs = cell_start + (size_t)e * g.ncell;
         const int cnt_before = cnt;
-        // run table: lane r owns run r (its bounds come in ONE round trip instead of one per run), then the
-        // candidates of all runs are walked as one flat index space -> full chunks of 32 whatever the run lengths
-        int j0 = 0, len = 0;
-        if (lane < nrun) {
-            const int r = lane % nxr, ab = lane / nxr;
-            const int b = ab % ny, a = ab / ny;
-            const int rowbase = (zs[a] * g.nc[1] + ys[b]) * g.nc[0];
-            j0 = cs[rowbase + xr0[r]];
-            len = cs[rowbase + xr1[r] + 1] - j0;
-        }
-        int incl = len;
+        for (int r = 0; r < nxr; ++r) {
+            // run table: lane q owns run q (its bounds come in ONE round trip instead of one per run), then the
+            // candidates of all runs are walked as one flat index space -> full chunks of 32 whatever the run lengths
+            int j0 = 0, len = 0;
+            if (lane < nyz) {
+                const int b = lane % ny, a = lane / ny;
+                const int rowbase = (zs[a] * g.nc[1] + ys[b]) * g.nc[0];
+                j0 = cs[rowbase + xr0[r]];
+                len = cs[rowbase + xr1[r] + 1] - j0;
+            }
+            int incl = len;
 #pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const int t = __shfl_up_sync(0xffffffffu, incl, d);
-            if (lane >= d) incl += t;
-        }
-        const int P = incl - len;                       // first flat index of run `lane`
-        const int total = __shfl_sync(0xffffffffu, incl, 31);
-        for (int f0 = 0; f0 < total; f0 += 32) {
-            const int f = f0 + lane;
-            int lo = 0, hi = 31;                        // largest run r with P[r] <= f
+            for (int d = 1; d < 32; d <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += t;
+            }
+            const int P = incl - len;                       // first flat index of run `lane`
+            const int total = __shfl_sync(0xffffffffu, incl, 31);
+            for (int f0 = 0; f0 < total; f0 += 32) {
+                const int f = f0 + lane;
+                int lo = 0, hi = 31;                        // largest run q with P[q] <= f
 #pragma unroll
-            for (int step = 0; step < 5; ++step) {
-                const int mid = (lo + hi + 1) >> 1;
-                const int pm = __shfl_sync(0xffffffffu, P, mid);
-                if (pm <= f) lo = mid; else hi = mid - 1;
+                for (int step = 0; step < 5; ++step) {
+                    const int mid = (lo + hi + 1) >> 1;
+                    const int pm = __shfl_sync(0xffffffffu, P, mid);
+                    if (pm <= f) lo = mid; else hi = mid - 1;
+                }
+                const int j = __shfl_sync(0xffffffffu, j0, lo) + (f - __shfl_sync(0xffffffffu, P, lo));
+                bool hit = false;
+                if (f < total && j != i) {
+                    const double dx = wx ? min_image_1d(xi, sx[j], g.box[0], g.half[0]) : __dsub_rn(sx[j], xi);
+                    const double dy = wy ? min_image_1d(yi, sy[j], g.box[1], g.half[1]) : __dsub_rn(sy[j], yi);
+                    const double dz = wz ? min_image_1d(zi, sz[j], g.box[2], g.half[2]) : __dsub_rn(sz[j], zi);
+                    hit = dist2_exact(dx, dy, dz) < rc2;
+                }
+                const unsigned m = __ballot_sync(0xffffffffu, hit);
+                if (hit) {
+                    const int p = cnt + __popc(m & ((1u << lane) - 1u));
+                    if (p < max_nbr) row[p] = j;
+                }
+                cnt += __popc(m);
             }
-            const int j = __shfl_sync(0xffffffffu, j0, lo) + (f - __shfl_sync(0xffffffffu, P, lo));
-            bool hit = false;
-            if (f < total && j != i) {
-                const double dx = wx ? min_image_1d(xi, sx[j], g.box[0], g.half[0]) : __dsub_rn(sx[j], xi);
-                const double dy = wy ? min_image_1d(yi, sy[j], g.box[1], g.half[1]) : __dsub_rn(sy[j], yi);
-                const double dz = wz ? min_image_1d(zi, sz[j], g.box[2], g.half[2]) : __dsub_rn(sz[j], zi);
-                hit = dist2_exact(dx, dy, dz) < rc2;
-            }
-            const unsigned m = __ballot_sync(0xffffffffu, hit);
-            if (hit) {
-                const int p = cnt + __popc(m & ((1u << lane) - 1u));
-                if (p < max_nbr) row[p] = j;
-            }
-            cnt += __popc(m);
         }
         if (lane == 0) nbr_cnt[(size_t)i * MAX_ELEM + e] = min(cnt, max_nbr) - min(cnt_before, max_nbr);
     }

@@ -153,7 +153,7 @@ static size_t ws_layout(Workspace* w, void* base, int64_t n, int n_elem, int str
 }
 
 static bool make_grid(Grid* g, const double box[3], double rc, int64_t n) {
-    const double cs_min = rc * (1.0 + 1e-9);   // margin: a cell index rounded the wrong way must not hide a neighbour
+    const double cs_min = rc * (1.0 + 1e-9) / NNP_CELL_HW;   // margin: a cell index rounded the wrong way must not hide a neighbour
     int64_t limit = 2 * (n > 0 ? n : 1) + 64;
     double nc[3];
     for (int c = 0; c < 3; ++c) {
@@ -169,7 +169,7 @@ static bool make_grid(Grid* g, const double box[3], double rc, int64_t n) {
         g->half[c] = 0.5 * box[c];
         g->nc[c] = (int)nc[c];
         g->inv_cs[c] = nc[c] / box[c];
-        g->span[c] = g->nc[c] >= 3 ? 1 : 0;
+        g->span[c] = g->nc[c] >= 2 * NNP_CELL_HW + 1 ? NNP_CELL_HW : 0;
     }
     g->ncell = g->nc[0] * g->nc[1] * g->nc[2];
     return true;
