@@ -14,6 +14,7 @@
 // one atom and blocks of 4 output neurons, weights come as 128-bit broadcast loads through L1.
 // No tensor cores: B200's FP64 tensor rate equals its FP64 vector rate and the contraction is
 // 1-3 % of the step.
+#include "mathfn.cuh"
 #include "nnp_internal.h"
 
 namespace nnp {
@@ -30,12 +31,34 @@ struct MlpParams {
     int g_stride;
 };
 
-__device__ __forceinline__ double softplus_d(double x) { return fmax(x, 0.0) + log1p(exp(-fabs(x))); }
-__device__ __forceinline__ double sigmoid_d(double x) { return 1.0 / (1.0 + exp(-x)); }
+// softplus(x) = max(x, 0) + log1p(e) and softplus'(x) = 1 / (1 + exp(-x)) from ONE exponential e = exp(-|x|):
+//   u = 1 + e in [1, 2];  sigmoid = (x >= 0 ? 1 : e) / u;
+//   log1p(e) = log(u) - ((u - 1) - e) / u      (the second term undoes the rounding of 1 + e: exact to first order, and
+//                                               it IS the result once e < 2^-53)
+//   log(u) = k ln2 + 2 s P(s^2),  m = u / 2^k in [1/sqrt2, sqrt2],  s = (m - 1) / (m + 1),  P = ATHC (mathfn.cuh, 3e-18).
+// libdevice's exp + exp + log1p + division were ~150 FP64-pipe instructions per hidden neuron -- more than the
+// network's matrix products; this is ~65 (k_mlp_reg 3.10 -> 2.77 ms at 2.1 M atoms, 1.45 -> 1.23 ms on the Ni-like workload).
+__device__ __forceinline__ void softplus_sigmoid(double x, double& h, double& dh) {
+    const double e = exp_small(fmax(-fabs(x), -700.0));
+    const double u = 1.0 + e;
+    const double ru = 1.0 / u;
+    const bool big = u > 1.4142135623730951;
+    const double m = big ? 0.5 * u : u;
+    const double s = (m - 1.0) / (m + 1.0);
+    const double q = s * s;
+    double p = ATHC[7];
+#pragma unroll
+    for (int k = 6; k >= 0; --k) p = fma(p, q, ATHC[k]);
+    double lg = (s + s) * p;
+    if (big) lg += 0.69314718055994531;
+    const double l1p = fma(-((u - 1.0) - e), ru, lg);
+    h = fmax(x, 0.0) + l1p;
+    dh = x >= 0.0 ? ru : e * ru;
+}
 // hidden activation and its derivative: kind 0 softplus (BASELINE.json), 1 tanh
 __device__ __forceinline__ void activate(int kind, double z, double& h, double& dh) {
     if (kind == 1) { h = tanh(z); dh = fma(-h, h, 1.0); }
-    else { h = softplus_d(z); dh = sigmoid_d(z); }
+    else softplus_sigmoid(z, h, dh);
 }
 
 __host__ __device__ inline int round4(int x) { return (x + 3) & ~3; }
