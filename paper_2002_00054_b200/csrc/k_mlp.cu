@@ -191,8 +191,12 @@ constexpr int MLP_REG_THREADS = 64;
 // [neuron][thread] columns (conflict-free), so no register array is ever indexed dynamically.
 __global__ void __launch_bounds__(MLP_REG_THREADS) k_mlp_reg(const __grid_constant__ MlpRegParams p) {
     constexpr int H = MLP_REG_H, NT = MLP_REG_THREADS;
-    __shared__ double sh_h[H][NT];               // h1, later delta_1
-    __shared__ double sh_s[H][NT];               // act'(z1)
+    // only the rows the network has (25 + 25 of 64 for BASELINE.json's): shared memory bounds the resident CTAs (ncu: 6 of 64-row
+    // CTAs per SM, 19 % of the warp slots)
+    extern __shared__ __align__(16) double sm_reg[];
+    const int nh = p.W.n1 > p.W.n2 ? p.W.n1 : p.W.n2;
+    double (*sh_h)[NT] = reinterpret_cast<double (*)[NT]>(sm_reg);               // [nh]: h1, later z2 / delta_2, delta_1
+    double (*sh_s)[NT] = reinterpret_cast<double (*)[NT]>(sm_reg) + nh;          // [n1]: act'(z1)
     const int t = threadIdx.x;
     const int begin = *p.elem_begin, end = *p.elem_end;
     const int64_t a = (int64_t)begin + (int64_t)blockIdx.x * NT + t;
@@ -218,7 +222,8 @@ __global__ void __launch_bounds__(MLP_REG_THREADS) k_mlp_reg(const __grid_consta
         for (int o = 0; o < H; ++o) acc[o] = fma(W1[i * H + o], x, acc[o]);
     }
 #pragma unroll
-    for (int o = 0; o < H; ++o) sh_h[o][t] = acc[o];
+    for (int o = 0; o < H; ++o)
+        if (o < n1) sh_h[o][t] = acc[o];
 #pragma unroll 1
     for (int o = 0; o < n1; ++o) {               // rolled: ONE copy of the activation code
         double h, d;
@@ -237,7 +242,8 @@ __global__ void __launch_bounds__(MLP_REG_THREADS) k_mlp_reg(const __grid_consta
     }
     double e = W3[H];                            // b3
 #pragma unroll
-    for (int o = 0; o < H; ++o) sh_h[o][t] = acc[o];      // h1 is dead: its columns take z2, then delta_2
+    for (int o = 0; o < H; ++o)
+        if (o < n2) sh_h[o][t] = acc[o];         // h1 is dead: its columns take z2, then delta_2
 #pragma unroll 1
     for (int o = 0; o < n2; ++o) {
         double h, d;
@@ -312,7 +318,9 @@ int launch_mlp(const Workspace& w, int64_t n, int n_elem, int ncell, const NetDe
             q.G = w.G; q.dEdG = w.dEdG; q.e_sorted = w.e_sorted;
             q.sf_shift = nets[e].sf_shift; q.sf_scale = nets[e].sf_scale;
             q.g_stride = g_stride; q.activation = nets[e].activation;
-            k_mlp_reg<<<(unsigned)((n + MLP_REG_THREADS - 1) / MLP_REG_THREADS), MLP_REG_THREADS, 0, st>>>(q);
+            const int nh = q.W.n1 > q.W.n2 ? q.W.n1 : q.W.n2;
+            const size_t smem = (size_t)(nh + q.W.n1) * MLP_REG_THREADS * sizeof(double);      // <= 32 KB
+            k_mlp_reg<<<(unsigned)((n + MLP_REG_THREADS - 1) / MLP_REG_THREADS), MLP_REG_THREADS, smem, st>>>(q);
             ++launches;
             continue;
         }
