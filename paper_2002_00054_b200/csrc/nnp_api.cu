@@ -153,26 +153,32 @@ static size_t ws_layout(Workspace* w, void* base, int64_t n, int n_elem, int str
 }
 
 static bool make_grid(Grid* g, const double box[3], double rc, int64_t n) {
-    const double cs_min = rc * (1.0 + 1e-9) / NNP_CELL_HW;   // margin: a cell index rounded the wrong way must not hide a neighbour
-    int64_t limit = 2 * (n > 0 ? n : 1) + 64;
-    double nc[3];
-    for (int c = 0; c < 3; ++c) {
-        nc[c] = std::floor(box[c] / cs_min);
-        if (nc[c] < 1.0) nc[c] = 1.0;
+    const int64_t limit = 2 * (n > 0 ? n : 1) + 64;
+    for (int hw = 2; hw >= 1; --hw) {
+        const double cs_min = rc * (1.0 + 1e-9) / hw;   // margin: a cell index rounded the wrong way must not hide a neighbour
+        double nc[3];
+        for (int c = 0; c < 3; ++c) {
+            nc[c] = std::floor(box[c] / cs_min);
+            if (nc[c] < 1.0) nc[c] = 1.0;
+        }
+        // cells of rc/2 pay when they hold a few atoms each (one warp per cell, nnp_internal.h Grid)
+        if (hw == 2 && (double)n < 1.5 * nc[0] * nc[1] * nc[2]) continue;
+        while (nc[0] * nc[1] * nc[2] > (double)limit) {
+            const double s = std::cbrt((double)limit / (nc[0] * nc[1] * nc[2])) * 0.999;
+            for (int c = 0; c < 3; ++c) nc[c] = std::fmax(1.0, std::floor(nc[c] * s));
+        }
+        g->hw = hw;
+        for (int c = 0; c < 3; ++c) {
+            g->box[c] = box[c];
+            g->half[c] = 0.5 * box[c];
+            g->nc[c] = (int)nc[c];
+            g->inv_cs[c] = nc[c] / box[c];
+            g->span[c] = g->nc[c] >= 2 * hw + 1 ? hw : 0;
+        }
+        g->ncell = g->nc[0] * g->nc[1] * g->nc[2];
+        return true;
     }
-    while (nc[0] * nc[1] * nc[2] > (double)limit) {
-        const double s = std::cbrt((double)limit / (nc[0] * nc[1] * nc[2])) * 0.999;
-        for (int c = 0; c < 3; ++c) nc[c] = std::fmax(1.0, std::floor(nc[c] * s));
-    }
-    for (int c = 0; c < 3; ++c) {
-        g->box[c] = box[c];
-        g->half[c] = 0.5 * box[c];
-        g->nc[c] = (int)nc[c];
-        g->inv_cs[c] = nc[c] / box[c];
-        g->span[c] = g->nc[c] >= 2 * NNP_CELL_HW + 1 ? NNP_CELL_HW : 0;
-    }
-    g->ncell = g->nc[0] * g->nc[1] * g->nc[2];
-    return true;
+    return false;
 }
 
 // ---------------------------------------------------------------- create / destroy

@@ -127,16 +127,15 @@ struct NetDesc {
 };
 
 // Cell grid of one nnp_compute call (host-built, passed by value).
-// Cells are at least rc / NNP_CELL_HW wide and the neighbour search visits the (2 HW + 1)^3 stencil: HW = 2 cuts the
-// candidates per atom from 27 rc^3 rho to 15.6 rc^3 rho (583 -> 337 for the water-like systems).
-#ifndef NNP_CELL_HW
-#define NNP_CELL_HW 2
-#endif
+// Cells are at least rc / hw wide and the neighbour search visits the (2 hw + 1)^3 stencil: hw = 2 cuts the candidates
+// per atom from 27 rc^3 rho to 15.6 rc^3 rho (583 -> 337 for the water-like systems); make_grid takes hw = 1 when such
+// cells would hold fewer than 1.5 atoms (the search runs one warp per cell and amortises its bookkeeping over the cell's atoms).
 struct Grid {
     double box[3], half[3], inv_cs[3];
     int32_t nc[3];
     int32_t ncell;
-    int32_t span[3];                 // stencil half-width clipped: NNP_CELL_HW if nc >= 2 HW + 1, else 0 (visit all nc cells)
+    int32_t hw;                      // stencil half-width: cells are >= rc / hw wide
+    int32_t span[3];                 // hw if nc >= 2 hw + 1, else 0 (the stencil is all nc cells)
 };
 
 struct Workspace {
