@@ -240,6 +240,21 @@ nnp_status nnp_md_kinetic_energy(nnp_model* m, const double* h_mass, int64_t n_a
                                  const int32_t* d_type, double* d_ekin, void* d_workspace, size_t workspace_bytes,
                                  void* cuda_stream);
 
+/* nnp_md_kinetic_energy for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the same quantity (the energy-conservation check of an NVE
+ * run; same arithmetic and summation order, same bits) WITHOUT a workspace.  The block sums live in a static device
+ * array inside the library: 128 KB that every GPU which loads the library holds until the process exits.  The call
+ * makes no cudaMalloc / cudaFree and calls no allocating library routine; it enqueues two kernels on cuda_stream and
+ * does not synchronise.
+ *   h_mass [n_elem] HOST (amu);  d_vel [n_atoms][3], d_type [n_atoms], d_ekin [1] DEVICE, caller-owned.
+ *   n_atoms <= NNP_NOALLOC_MAX_ATOMS, beyond: NNP_ERR_LIMIT and nothing is launched.
+ * Every call on a device shares the array (a call overwrites what it reads; nothing needs clearing between calls):
+ * calls that OVERLAP on the GPU -- different streams without an ordering between them, also from different models --
+ * race on it.  Errors: NNP_ERR_INVALID_ARG (null pointers, n_atoms < 0, bad masses), NNP_ERR_LIMIT, NNP_ERR_CUDA. */
+#define NNP_NOALLOC_MAX_ATOMS 4194304
+nnp_status nnp_md_kinetic_energy_noalloc(nnp_model* m, const double* h_mass, int64_t n_atoms, const double* d_vel,
+                                         const int32_t* d_type, double* d_ekin, void* cuda_stream);
+
 /* Synchronise the stream of the last nnp_compute / nnp_md_run and return the device-side status of EVERY
  * evaluation enqueued since the previous nnp_sync_status (a sticky device word owned by the model: a neighbour
  * overflow or a non-finite position in step 3 of a 100-step nnp_md_run, or in the first of several nnp_compute

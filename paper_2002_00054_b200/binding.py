@@ -22,7 +22,7 @@ STAGE_NAMES = ("sort", "neighbors", "symmetry_functions", "networks", "forces", 
 
 # every symbol include/nnp.h declares
 EXPORTS = ("nnp_create", "nnp_table_kernels", "nnp_destroy", "nnp_set_max_neighbors", "nnp_workspace_bytes", "nnp_compute",
-           "nnp_compute_host", "nnp_set_sf_scaling", "nnp_set_activation", "nnp_set_sf_cutoffs", "nnp_set_precision", "nnp_set_deterministic_forces", "nnp_set_neighbor_skin", "nnp_invalidate_neighbors", "nnp_get_neighbor_rebuilds", "nnp_md_run", "nnp_md_kinetic_energy", "nnp_sync_status", "nnp_get_neighbor_counts", "nnp_get_neighbors", "nnp_get_sf",
+           "nnp_compute_host", "nnp_set_sf_scaling", "nnp_set_activation", "nnp_set_sf_cutoffs", "nnp_set_precision", "nnp_set_deterministic_forces", "nnp_set_neighbor_skin", "nnp_invalidate_neighbors", "nnp_get_neighbor_rebuilds", "nnp_md_run", "nnp_md_kinetic_energy", "nnp_md_kinetic_energy_noalloc", "nnp_sync_status", "nnp_get_neighbor_counts", "nnp_get_neighbors", "nnp_get_sf",
            "nnp_get_dedg", "nnp_g_stride", "nnp_set_timing", "nnp_get_timings", "nnp_last_launch_count",
            "nnp_uses_fast_path", "nnp_measure_fp64_peak", "nnp_last_error", "nnp_version")
 
@@ -102,6 +102,8 @@ def load_library():
                              C.c_size_t, vp]
     L.nnp_md_kinetic_energy.restype = C.c_int
     L.nnp_md_kinetic_energy.argtypes = [vp, C.POINTER(dbl), i64, vp, vp, vp, vp, C.c_size_t, vp]
+    L.nnp_md_kinetic_energy_noalloc.restype = C.c_int
+    L.nnp_md_kinetic_energy_noalloc.argtypes = [vp, C.POINTER(dbl), i64, vp, vp, vp, vp]
     L.nnp_sync_status.restype = C.c_int
     L.nnp_sync_status.argtypes = [vp]
     L.nnp_get_neighbor_counts.restype = C.c_int
@@ -332,6 +334,17 @@ class NNP:
         self._check(self._L.nnp_md_kinetic_energy(self._h, m, n, C.c_void_p(vel.data_ptr()),
                                                   C.c_void_p(types.data_ptr()), C.c_void_p(out.data_ptr()),
                                                   C.c_void_p(ws_ptr), ws_len, C.c_void_p(stream)))
+        return out
+
+    def kinetic_energy_noalloc(self, masses, vel, types, out, n_atoms=None):
+        """nnp_md_kinetic_energy_noalloc: the same sum with no workspace and no allocation inside the library; the caller
+        owns `out` (cuda f64 [1]).  n_atoms <= 4,194,304; calls that overlap on the GPU race on the library's static scratch."""
+        n = int(vel.shape[0]) if n_atoms is None else int(n_atoms)
+        m = (C.c_double * len(masses))(*[float(x) for x in masses])
+        stream = self._torch.cuda.current_stream(vel.device).cuda_stream
+        self._check(self._L.nnp_md_kinetic_energy_noalloc(self._h, m, n, C.c_void_p(vel.data_ptr()),
+                                                          C.c_void_p(types.data_ptr()), C.c_void_p(out.data_ptr()),
+                                                          C.c_void_p(stream)))
         return out
 
     def compute_host(self, pos, types, box, out=None):

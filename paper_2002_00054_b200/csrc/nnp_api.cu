@@ -954,6 +954,23 @@ extern "C" nnp_status nnp_md_kinetic_energy(nnp_model* m, const double* h_mass, 
     return NNP_OK;
 }
 
+extern "C" nnp_status nnp_md_kinetic_energy_noalloc(nnp_model* m, const double* h_mass, int64_t n_atoms, const double* d_vel,
+                                                    const int32_t* d_type, double* d_ekin, void* cuda_stream) {
+    if (!m) return NNP_ERR_INVALID_ARG;
+    if (!h_mass || !d_ekin || n_atoms < 0 || (n_atoms > 0 && (!d_vel || !d_type))) return fail(m, NNP_ERR_INVALID_ARG, "null array");
+    for (int e = 0; e < m->n_elem; ++e)
+        if (!(h_mass[e] > 0.0) || !std::isfinite(h_mass[e])) return fail(m, NNP_ERR_INVALID_ARG, "mass must be finite and > 0");
+    if (n_atoms > NOALLOC_MAX_ATOMS)
+        return fail(m, NNP_ERR_LIMIT, "n_atoms > NNP_NOALLOC_MAX_ATOMS (4194304): the static scratch array holds 16384 block sums; "
+                                      "use nnp_md_kinetic_energy with a workspace");
+    DeviceGuard dg(m->device);
+    if (!dg.ok) return fail(m, NNP_ERR_CUDA, "cudaSetDevice failed");
+    int launches = 0;
+    const cudaError_t e = launch_ekin_noalloc(n_atoms, m->n_elem, h_mass, d_type, d_vel, d_ekin, (cudaStream_t)cuda_stream, &launches);
+    if (e != cudaSuccess) return fail(m, NNP_ERR_CUDA, std::string("nnp_md_kinetic_energy_noalloc: ") + cudaGetErrorString(e));
+    return NNP_OK;
+}
+
 extern "C" nnp_status nnp_sync_status(nnp_model* m) {
     if (!m) return NNP_ERR_INVALID_ARG;
     if (!m->have_ws) return NNP_OK;

@@ -252,6 +252,11 @@ int launch_finalize(const Workspace& w, int64_t n, double* d_e_atom, double* d_e
 // MD loop (k_md.cu)
 int launch_vv(int64_t n, int n_elem, const double* h_mass, const int32_t* d_type, const double* d_force, double* d_vel,
               double* d_pos, double dt, bool drift, cudaStream_t st);
+// k_noalloc.cu: the kinetic energy with its block sums in a file-scope device array (no workspace, no allocation)
+constexpr int64_t NOALLOC_MAX_ATOMS = NNP_NOALLOC_MAX_ATOMS;
+constexpr int NOALLOC_MAX_PARTIALS = (int)((NOALLOC_MAX_ATOMS + 255) / 256);        // 16,384 doubles = 128 KB
+cudaError_t launch_ekin_noalloc(int64_t n, int n_elem, const double* h_mass, const int32_t* d_type, const double* d_vel,
+                                double* d_out, cudaStream_t st, int* launches);
 int launch_ekin(int64_t n, int n_elem, const double* h_mass, const int32_t* d_type, const double* d_vel, double* d_part,
                 double* d_out, cudaStream_t st);
 
