@@ -634,6 +634,47 @@ def test_dense_cluster_near_max_neighbors():
     _check_full(W.make_model(False), sysm)
 
 
+def test_neighbour_search_crowded_cell_sparse_grid_and_cell_limit():
+    # k_neighbors runs one warp per cell on cells of rc/2 (5^3 stencil) or rc (3^3), chosen by make_grid:
+    # (a) a blob that puts more than 32 atoms into one rc/2 cell: the warp walks the cell's centres in two groups of 32;
+    # (b) 70 atoms in a 41 A box: fewer than 1.5 atoms per rc/2 cell -> cells of rc, and 6^3 = 216 cells exceed the
+    #     workspace's cell budget of 2 n + 64 = 204, so the grid is coarsened as well (cells wider than rc);
+    # (c) 1,300 atoms in a 33 x 14 x 62 A box: 10, 4 and 20 cells of rc/2 -- wrapping x-ranges, a dimension whose stencil is
+    #     all of its cells, and a dimension whose interior cells skip the minimum-image test
+    from workloads import rng
+    model = W.make_model(False)
+    sysm = W.make_water(150, 5, L=16.7)
+    # 36 atoms on a jittered 4 x 3 x 3 lattice of 0.8 A inside the cell [6.68, 10.02) x [6.68, 10.02) x [3.34, 6.68) of the 5^3 grid
+    # (unphysical on purpose: the arithmetic does not care, the forces get large, hence the relative force bound below)
+    u = rng.uniform(rng.stream_key(31, 7), np.arange(3 * 36, dtype=np.uint64)).reshape(36, 3)
+    ijk = np.array([(a, b, c) for a in range(4) for b in range(3) for c in range(3)], dtype=np.float64)
+    blob = np.array([6.85, 6.85, 3.55]) + 0.8 * ijk + 0.1 * (u - 0.5)
+    keep = np.ones(sysm.n_atoms, dtype=bool)
+    for q in blob:                                              # drop the water atoms closer than 0.8 A to a blob atom
+        d = sysm.pos - q
+        d -= sysm.box * np.round(d / sysm.box)
+        keep &= (d ** 2).sum(axis=1) > 0.64
+    pos = np.vstack([sysm.pos[keep], blob])
+    types = np.concatenate([sysm.types[keep], (np.arange(len(blob)) % 2).astype(np.int32)])
+    cell = np.floor(pos / (sysm.box / 5.0)).astype(int)
+    assert np.sum(np.all(cell == np.array([2, 2, 1]), axis=1)) >= 36
+    from paper_2002_00054_b200 import NNP
+    nnp = NNP.from_model(model)
+    nnp.set_max_neighbors(200)
+    e_atom, e_total, force = _run(nnp, pos, types, sysm.box)
+    off, idx = nnp.neighbors(len(types))
+    roff, ridx = oracle.neighbor_list(pos, sysm.box, model.rc)
+    assert np.array_equal(off.cpu().numpy(), roff) and np.array_equal(idx.cpu().numpy(), ridx)
+    ref = oracle.compute(oracle.OracleModel(model), pos, types, sysm.box)
+    assert abs(e_total - ref.e_total) <= E_REL * np.abs(ref.e_atom).sum()
+    assert np.abs(force - ref.F).max() <= F_ABS * max(1.0, np.abs(ref.F).max() / 20.0)
+    nnp.close()
+    for box, n, seed in ((np.array([41.0, 41.0, 41.0]), 70, 3), (np.array([33.0, 14.0, 62.0]), 1300, 4)):
+        p = _uniform_in(box, n, seed)
+        t = (np.arange(n) % 3 != 0).astype(np.int32)
+        _check_full(model, W.WaterSystem(pos=p, types=t, box=box, seed=seed))
+
+
 @pytest.mark.parametrize("max_neighbors", [128, 200])
 def test_slot_capacity_variants(max_neighbors):
     # the fast kernels are instantiated for slot capacities 128 / 160 / 256 (shared-memory layout at
