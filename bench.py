@@ -324,11 +324,12 @@ def main():
     ap.add_argument("--md", action="store_true",
                     help="time velocity-Verlet MD steps (nnp_md_run: kick+drift, the whole path, kick) instead of bare evaluations")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--table", default="baseline", choices=["baseline", "free", "zeta3", "generic", "n2p2like", "wide9"],
+    ap.add_argument("--table", default="baseline", choices=["baseline", "free", "generic", "zeta5", "queue", "n2p2like", "wide9"],
                     help="SF table probe (not a BASELINE.json workload): 'free' breaks the eta ratio of the angular set "
-                         "(0.01 -> 0.0123: lane-owned kernels with per-eta exponentials), 'zeta3' also replaces zeta 16 by 3 "
-                         "(a second pass with base exponent 3), 'generic' also lists one angular function twice, which no "
-                         "pass menu holds (queue-based generic kernels), 'n2p2like' is a table shaped like published n2p2 models (zeta in {1, 4}, "
+                         "(0.01 -> 0.0123: lane-owned kernels with per-eta exponentials), 'generic' also replaces zeta 16 by 3 "
+                         "(round 1: queue-based generic kernels; now one pass with the exponent menu 1, 2, 4; 3), 'zeta5' replaces "
+                         "zeta 4 by 5 as well (two passes), 'queue' also lists one angular function twice, which no "
+                         "pass menu holds (the queue-based generic kernels), 'n2p2like' is a table shaped like published n2p2 models (zeta in {1, 4}, "
                          "seven eta values, lambda = +-1, angular functions of two cutoff radii: 3 passes of the free-eta "
                          "kernels), 'wide9' turns the angular functions of the smaller eta into wide ones (n2p2 kind 9: one narrow and one "
                          "wide pass); the roofline object is then not meaningful")
@@ -382,9 +383,11 @@ def main():
     elif args.table != "baseline":
         ang = model.sf["kind"] == 3
         model.sf["eta"][ang & (model.sf["eta"] == 0.01)] = 0.0123
-        if args.table in ("zeta3", "generic"):
+        if args.table in ("generic", "zeta5", "queue"):
             model.sf["zeta"][ang & (model.sf["zeta"] == 16.0)] = 3.0
-        if args.table == "generic":
+        if args.table == "zeta5":
+            model.sf["zeta"][ang & (model.sf["zeta"] == 4.0)] = 5.0
+        if args.table == "queue":
             for c in range(len(model.elements)):
                 q = np.nonzero(ang & (model.sf["central"] == c))[0]
                 for key in ("eta", "lam", "zeta", "e1", "e2"):

@@ -100,10 +100,11 @@ nnp_status nnp_create(nnp_model** out, int32_t n_elem, const char* const* elem_n
  * decision): kernels_out[c] for every central element c --
  *   NNP_KERNELS_BASE12 / NNP_KERNELS_WIDE32  the lane-owned kernels specialised for BASELINE.json's two angular tables,
  *   NNP_KERNELS_FREE32 / NNP_KERNELS_FREE16  the lane-owned kernels for any table with <= 4 (FREE16: <= 2) distinct
- *                        angular eta values, lambda = +-1, zeta in z0 * {1, 2, 4, 16} for one integer z0, narrow (kind 3)
- *                        functions only, no (eta, lambda, zeta) twice per pair group,
+ *                        angular eta values, lambda = +-1, zeta in one exponent menu {z0, 2 z0, 4 z0, zx} (any integers, e.g.
+ *                        {1, 2, 4, 16}, {1, 4}, {1, 2, 4, 3}), narrow (kind 3) functions only, no (eta, lambda, zeta) twice per
+ *                        pair group,
  *   NNP_KERNELS_MULTI    the same lane-owned free-eta kernels in several passes: any number of eta values (four per pass),
- *                        wide functions (kind 9; passes of their own), any integer zeta (one pass per base exponent z0) and,
+ *                        wide functions (kind 9; passes of their own), any integer zeta (one pass per exponent menu) and,
  *                        after nnp_set_sf_cutoffs, angular functions of several cutoff radii (one radius per pass), at most
  *                        8 passes; otherwise the conditions of FREE32,
  *   NNP_KERNELS_GENERIC  everything else (more passes, a function listed twice, eta * 3 rc^2 > 700, no angular functions).

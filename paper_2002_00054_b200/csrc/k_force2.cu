@@ -138,7 +138,9 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
     if (Spec::FREE_ETA && (p.pass >= prog->n_pass || ps->spec != Spec::ID)) return;
     const bool own_rc = Spec::FREE_ETA && ps->own_rc != 0;          // the pass's cutoff is shorter than the neighbour list's
     const bool widep = Spec::FREE_ETA && ps->wide != 0;             // wide angular functions: no r_jk term, every pair counts
-    const int z0 = Spec::FREE_ETA ? ps->zeta0 : 1;                  // menu entry b stands for zeta = z0 * 2^b
+    const int z0 = Spec::FREE_ETA ? ps->zeta0 : 1;                  // menu bits 0, 1, 2 stand for zeta = z0, 2 z0, 4 z0 ...
+    const int zx = Spec::FREE_ETA ? ps->zeta_x : 16;                // ... and bit 4 for zeta = zx (16 z0: two more squarings)
+    const bool zx_own = Spec::FREE_ETA && zx != 16 * z0;
     const double rc2p = Spec::FREE_ETA ? ps->rc2 : p.rc2, k2p = Spec::FREE_ETA ? ps->k2 : p.k2;
     const int32_t* __restrict__ n_ang = Spec::FREE_ETA ? ps->n_ang : prog->n_ang;
     const int neta = Spec::FREE_ETA ? ps->n_eta : Spec::NETA;
@@ -233,7 +235,7 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
             for (int e = 0; e < Spec::NETA; ++e) {
                 if (Spec::mask(e) >> tid & 1u) {
                     const int g = Spec::FREE_ETA ? ps->g[pr][e][tid] : prog->ang_g[pr][e][tid];
-                    const int zeta = z0 << (tid & 7);
+                    const int zeta = (tid & 7) == Spec::MAXBIT ? zx : z0 << (tid & 7);
                     const double lam = tid < 8 ? 1.0 : -1.0;
                     const double bc = g >= 0 ? brow[g] * exp2((double)(1 - zeta)) : 0.0;
                     int a = 0;   // accumulator slot = set bits before (e, tid)
@@ -366,6 +368,7 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
         R pw[2][Spec::MAXBIT + 1], pd[2][Spec::MAXBIT + 1];
         pw[0][0] = (R)1 + cosv; pw[1][0] = (R)1 - cosv;
         pd[0][0] = (R)1; pd[1][0] = (R)1;
+        const R base0 = pw[0][0], base1 = pw[1][0];
         if (Spec::FREE_ETA && z0 > 1) {                        // uniform per CTA: P = (1 +- cos)^z0, dP/d(1 +- cos) = z0 (1 +- cos)^(z0-1)
             const R q0 = powi_uniform(pw[0][0], z0 - 1), q1 = powi_uniform(pw[1][0], z0 - 1);
             pw[0][0] *= q0; pw[1][0] *= q1;
@@ -383,6 +386,11 @@ __device__ __forceinline__ void force2_centre(const Force2Params& p, const int64
         for (int b = 1; b <= Spec::MAXBIT; ++b) {       // times zeta = 2^b: dP/dcos comes from the SAME coefficients
             pd[0][b] = scale2(pd[0][b], b);
             pd[1][b] = scale2(pd[1][b], b);
+        }
+        if (zx_own) {                                          // uniform per CTA: the top menu entry is an exponent of its own
+            const R q0 = powi_uniform(base0, zx - 1), q1 = powi_uniform(base1, zx - 1);
+            pw[0][Spec::MAXBIT] = base0 * q0; pw[1][Spec::MAXBIT] = base1 * q1;
+            pd[0][Spec::MAXBIT] = (R)zx * q0; pd[1][Spec::MAXBIT] = (R)zx * q1;
         }
         R Z0 = (R)0, Z1 = (R)0, Z2 = (R)0;
 #pragma unroll

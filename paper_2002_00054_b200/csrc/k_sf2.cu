@@ -73,7 +73,9 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
     if (Spec::FREE_ETA && (p.pass >= prog->n_pass || ps->spec != Spec::ID)) return;
     const bool own_rc = Spec::FREE_ETA && ps->own_rc != 0;          // the pass's cutoff is shorter than the neighbour list's
     const bool widep = Spec::FREE_ETA && ps->wide != 0;             // wide angular functions: no r_jk term, every pair counts
-    const int z0 = Spec::FREE_ETA ? ps->zeta0 : 1;                  // menu entry b stands for zeta = z0 * 2^b
+    const int z0 = Spec::FREE_ETA ? ps->zeta0 : 1;                  // menu bits 0, 1, 2 stand for zeta = z0, 2 z0, 4 z0 ...
+    const int zx = Spec::FREE_ETA ? ps->zeta_x : 16;                // ... and bit 4 for zeta = zx (16 z0: two more squarings)
+    const bool zx_own = Spec::FREE_ETA && zx != 16 * z0;
     const double rc2p = Spec::FREE_ETA ? ps->rc2 : p.rc2, k2p = Spec::FREE_ETA ? ps->k2 : p.k2;
     const int32_t* __restrict__ n_ang = Spec::FREE_ETA ? ps->n_ang : prog->n_ang;
     const bool first_pass = !Spec::FREE_ETA || p.pass == 0;         // the radial block and the tail of the G row
@@ -225,6 +227,7 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
         R pw[2][Spec::MAXBIT + 1];
         pw[0][0] = (R)1 + cosv;
         pw[1][0] = (R)1 - cosv;
+        const R base0 = pw[0][0], base1 = pw[1][0];
         if (Spec::FREE_ETA && z0 > 1) {                        // uniform per CTA
             pw[0][0] = powi_uniform(pw[0][0], z0);
             pw[1][0] = powi_uniform(pw[1][0], z0);
@@ -233,6 +236,10 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
         for (int b = 1; b <= Spec::MAXBIT; ++b) {
             pw[0][b] = pw[0][b - 1] * pw[0][b - 1];
             pw[1][b] = pw[1][b - 1] * pw[1][b - 1];
+        }
+        if (zx_own) {                                          // uniform per CTA: the top menu entry is an exponent of its own
+            pw[0][Spec::MAXBIT] = powi_uniform(base0, zx);
+            pw[1][Spec::MAXBIT] = powi_uniform(base1, zx);
         }
 #pragma unroll
         for (int e = 0; e < Spec::NETA; ++e) {
@@ -277,7 +284,7 @@ __global__ void __launch_bounds__(WPC * 32, WPC == 1 ? (Spec::NACC <= 12 ? S2_MI
             double tot = gacc[pr * NACC + a];
 #pragma unroll
             for (int w = 0; w < WPC; ++w) tot += gacc[((1 + w) * npair + pr) * NACC + a];
-            Grow[g] = exp2((double)(1 - z0 * (1 << (b & 7)))) * tot;
+            Grow[g] = exp2((double)(1 - ((b & 7) == Spec::MAXBIT ? zx : z0 << (b & 7)))) * tot;
         }
     }
 }

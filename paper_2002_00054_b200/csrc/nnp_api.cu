@@ -229,20 +229,22 @@ static bool match_spec(const std::vector<std::vector<AngularSF>>& groups, ElemPr
 
 // Free-eta passes (nnp_internal.h AngPass): any table of angular symmetry functions (narrow, kind 3, and wide, kind 9)
 // with lambda = +-1, integer zeta and no (kind, rc, eta, lambda, zeta) twice in a pair group.  The symmetry functions
-// are split by kind, cutoff radius and BASE EXPONENT zeta0 (the kernels' menu holds zeta0 * {1, 2, 4, 16}; inside one
-// (kind, radius) the smallest zeta not yet covered becomes the next zeta0) and, inside one such class, into chunks of
-// at most four eta values of about equal size; one pass per chunk, narrow first, radius descending.  Returns false if
+// are split by kind, cutoff radius and EXPONENT MENU (zeta0, zeta_x): the kernels' menu of a pass holds the exponents
+// {zeta0, 2 zeta0, 4 zeta0, zeta_x}.  Inside one (kind, radius) the smallest zeta not yet covered becomes the next zeta0;
+// its zeta_x is 16 zeta0 if the table has it (the kernels then square on), else the smallest zeta still uncovered (raised
+// by square-and-multiply).  {1, 2, 4, 16}, {1, 4} and {1, 2, 3, 4} are one menu each.  Inside one such class the eta values
+// go in chunks of at most four of about equal size; one pass per chunk, narrow first, radius descending.  Returns false if
 // the table does not fit (more than MAX_PASS passes, an exponent beyond exp_small's range).
 static bool build_passes(const std::vector<std::vector<AngularSF>>& groups, double rc, ElemProgram* P) {
-    struct Key { double rc2, eta, k2; int wide, z0; };
-    auto menu_bit = [](int zeta, int z0) {                          // b with zeta == z0 * 2^b and b on the menu, else -1
-        if (zeta % z0 != 0) return -1;
-        for (int b = 0; b < 7; ++b)
-            if (zeta / z0 == (1 << b) && ((SpecFree32::mask(0) >> b) & 1u)) return b;
-        return -1;
+    struct Key { double rc2, eta, k2; int wide, z0, zx; };
+    static_assert((SpecFree32::mask(0) & 0xffu) == 0x17u && (SpecFree16::mask(0) & 0xffu) == 0x17u, "menu bits 0, 1, 2, 4");
+    auto menu_bit = [](int zeta, int z0, int zx) {                  // menu bit of zeta in the menu (z0, zx), else -1
+        for (int b = 0; b < 3; ++b)
+            if (zeta == (z0 << b)) return b;
+        return zeta == zx ? 4 : -1;
     };
-    // base exponents per (kind, radius): the zeta values of the class in ascending order, each joins the first zeta0 that holds it
-    struct Cls { double rc2; int wide; std::vector<int> zetas, z0; };
+    // menus per (kind, radius): the zeta values of the class in ascending order, see above
+    struct Cls { double rc2; int wide; std::vector<int> zetas, z0, zx; };
     std::vector<Cls> classes;
     for (const auto& grp : groups)
         for (const auto& f : grp) {
@@ -250,7 +252,7 @@ static bool build_passes(const std::vector<std::vector<AngularSF>>& groups, doub
             Cls* c = nullptr;
             for (auto& q : classes)
                 if (q.rc2 == f.rc2 && q.wide == f.wide) c = &q;
-            if (!c) { classes.push_back(Cls{f.rc2, f.wide, {}, {}}); c = &classes.back(); }
+            if (!c) { classes.push_back(Cls{f.rc2, f.wide, {}, {}, {}}); c = &classes.back(); }
             bool have = false;
             for (int z : c->zetas) have |= z == f.izeta;
             if (!have) c->zetas.push_back(f.izeta);
@@ -258,31 +260,54 @@ static bool build_passes(const std::vector<std::vector<AngularSF>>& groups, doub
     if (classes.empty()) return false;
     for (auto& c : classes) {
         std::sort(c.zetas.begin(), c.zetas.end());
-        for (int z : c.zetas) {
-            bool covered = false;
-            for (int z0 : c.z0) covered |= menu_bit(z, z0) >= 0;
-            if (!covered) c.z0.push_back(z);
+        std::vector<int> open = c.zetas;                            // not yet on a menu, ascending
+        auto take = [&](int z) {
+            for (size_t q = 0; q < open.size(); ++q)
+                if (open[q] == z) { open.erase(open.begin() + q); return true; }
+            return false;
+        };
+        // No menu entry, used or not, may overflow: (1 +- cos) <= 2 and the kernels compute EVERY entry of a menu (an unused one
+        // has coefficient 0, and 0 * inf is NaN), in FP32 in the mixed-precision mode.  So zeta0 <= 16 (4 zeta0 <= 64), the
+        // squaring to 16 zeta0 only for zeta0 <= 4, and a larger exponent goes to the zeta_x entry of a menu with zeta0 = 1.
+        while (!open.empty()) {
+            int z0 = open.front(), zx;
+            if (z0 > 16) {
+                zx = z0; z0 = 1;
+                take(zx);
+            } else {
+                take(z0); take(2 * z0); take(4 * z0);
+                zx = 16 * z0;
+                if (!(z0 <= 4 && take(zx))) {
+                    if (!open.empty()) { zx = open.front(); take(zx); }
+                    else if (z0 > 4) zx = z0;                       // unused: a harmless repeat of zeta0
+                }
+            }
+            c.z0.push_back(z0);
+            c.zx.push_back(zx);
         }
     }
-    auto base_of = [&](const AngularSF& f) {
+    // the menu (index into its class) that holds a symmetry function
+    auto menu_of = [&](const AngularSF& f, int& z0, int& zx) {
         for (const auto& c : classes)
             if (c.rc2 == f.rc2 && c.wide == f.wide)
-                for (int z0 : c.z0)
-                    if (menu_bit(f.izeta, z0) >= 0) return z0;
-        return 0;
+                for (size_t q = 0; q < c.z0.size(); ++q)
+                    if (menu_bit(f.izeta, c.z0[q], c.zx[q]) >= 0) { z0 = c.z0[q]; zx = c.zx[q]; return; }
+        z0 = zx = 0;
     };
     std::vector<Key> keys;
     for (const auto& grp : groups)
         for (const auto& f : grp) {
-            const int z0 = base_of(f);
+            int z0, zx;
+            menu_of(f, z0, zx);
             bool seen = false;
-            for (const Key& k : keys) seen |= (k.rc2 == f.rc2 && k.eta == f.eta && k.wide == f.wide && k.z0 == z0);
-            if (!seen) keys.push_back(Key{f.rc2, f.eta, f.k2, f.wide, z0});
+            for (const Key& k : keys) seen |= (k.rc2 == f.rc2 && k.eta == f.eta && k.wide == f.wide && k.z0 == z0 && k.zx == zx);
+            if (!seen) keys.push_back(Key{f.rc2, f.eta, f.k2, f.wide, z0, zx});
         }
     auto before = [](const Key& a, const Key& b) {              // sort: narrow first, rc descending, zeta0 and eta ascending
         if (a.wide != b.wide) return a.wide < b.wide;
         if (a.rc2 != b.rc2) return a.rc2 > b.rc2;
         if (a.z0 != b.z0) return a.z0 < b.z0;
+        if (a.zx != b.zx) return a.zx < b.zx;
         return a.eta < b.eta;
     };
     for (size_t x = 0; x < keys.size(); ++x)
@@ -292,7 +317,8 @@ static bool build_passes(const std::vector<std::vector<AngularSF>>& groups, doub
     size_t x = 0;
     while (x < keys.size()) {
         size_t y = x;
-        while (y < keys.size() && keys[y].rc2 == keys[x].rc2 && keys[y].wide == keys[x].wide && keys[y].z0 == keys[x].z0) ++y;
+        while (y < keys.size() && keys[y].rc2 == keys[x].rc2 && keys[y].wide == keys[x].wide && keys[y].z0 == keys[x].z0 &&
+               keys[y].zx == keys[x].zx) ++y;
         const int n = (int)(y - x), chunks = (n + MAX_ETA - 1) / MAX_ETA;
         for (int c = 0; c < chunks; ++c) {
             if (np >= MAX_PASS) return false;
@@ -306,17 +332,20 @@ static bool build_passes(const std::vector<std::vector<AngularSF>>& groups, doub
             ps.own_rc = ps.rc2 != rc * rc ? 1 : 0;
             ps.wide = keys[lo].wide;
             ps.zeta0 = keys[lo].z0;
+            ps.zeta_x = keys[lo].zx;
             ps.spec = ps.n_eta <= SpecFree16::NETA ? ANG_FREE16 : ANG_FREE32;
             for (size_t pr = 0; pr < groups.size(); ++pr) {
                 for (int e = 0; e < MAX_ETA; ++e)
                     for (int b = 0; b < 16; ++b) ps.g[pr][e][b] = -1;
                 for (const auto& f : groups[pr]) {
-                    if (f.rc2 != ps.rc2 || f.wide != ps.wide || base_of(f) != ps.zeta0) continue;
+                    int fz0, fzx;
+                    menu_of(f, fz0, fzx);
+                    if (f.rc2 != ps.rc2 || f.wide != ps.wide || fz0 != ps.zeta0 || fzx != ps.zeta_x) continue;
                     int e = -1;
                     for (int q = ps.n_eta - 1; q >= 0; --q)
                         if (ps.eta[q] == f.eta) e = q;
                     if (e < 0) continue;
-                    int bit = menu_bit(f.izeta, ps.zeta0);
+                    int bit = menu_bit(f.izeta, ps.zeta0, ps.zeta_x);
                     if (f.lam < 0) bit += 8;
                     if (ps.g[pr][e][bit] >= 0) return false;    // the same (rc, eta, lambda, zeta) twice in a pair group
                     ps.g[pr][e][bit] = (int16_t)f.g;

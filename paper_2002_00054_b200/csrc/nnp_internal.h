@@ -51,7 +51,7 @@ enum AngVariant : int { ANG_GENERIC = 0, ANG_BASE12 = 1, ANG_WIDE32 = 2, ANG_FRE
 // One sweep of the free-eta lane-owned kernels (SpecFree16 / SpecFree32) over the triplets of a centre: up to four
 // eta values that share ONE cutoff radius.  A table with more eta values, or with angular symmetry functions of
 // several radii (n2p2 gives every symmetry function its own rc), with wide functions or with zeta values outside
-// zeta0 * {1, 2, 4, 16} for one zeta0, runs as several passes -- G entries are independent and the forces are additive
+// {zeta0, 2 zeta0, 4 zeta0, zeta_x} for one pair (zeta0, zeta_x), runs as several passes -- G entries are independent and the forces are additive
 // over the symmetry functions.  ANG_FREE16 / ANG_FREE32 = one pass at the
 // global rc; ANG_MULTI = anything else that fits MAX_PASS passes.
 constexpr int MAX_PASS = 8;
@@ -63,8 +63,10 @@ struct AngPass {
     int32_t own_rc;                  // 1: rc_p differs from the global rc (slots beyond rc_p are switched off while staging)
     int32_t wide;                    // 1: a pass of WIDE angular functions (n2p2 kind 9): no r_jk term, no r_jk cutoff -- every pair
                                      // of neighbours of the two elements is a triplet (no screening)
-    int32_t zeta0;                   // menu entry (bit b) of this pass stands for zeta = zeta0 * 2^b: the kernels raise (1 +- cos) to
-                                     // zeta0 first (a warp-uniform square-and-multiply loop) and run the 2^b chain on that
+    int32_t zeta0;                   // menu bits 0, 1, 2 of this pass stand for zeta = zeta0, 2 zeta0, 4 zeta0: the kernels raise
+                                     // (1 +- cos) to zeta0 first (a warp-uniform square-and-multiply loop) and square from there
+    int32_t zeta_x;                  // menu bit 4 stands for zeta = zeta_x: 16 zeta0 (two more squarings) or any other exponent
+                                     // (raised on its own by square-and-multiply)
     int32_t n_ang[MAX_PAIR];         // symmetry functions of pair group p in this pass (0: the group is skipped)
     int16_t g[MAX_PAIR][MAX_ETA][16];   // G index of menu entry (eta slot, bit); -1 = absent
 };

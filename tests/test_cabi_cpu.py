@@ -94,21 +94,25 @@ def test_kernel_choice_per_table(lib):
     m3 = W.make_model(True)
     m3.sf["eta"][(m3.sf["kind"] == 3) & (m3.sf["eta"] == 0.003)] = 0.0041
     assert table_kernels(m3) == ("free32", "free32")               # four unrelated eta values
-    m.sf["zeta"][ang & (m.sf["zeta"] == 16.0) & (m.sf["central"] == 1)] = 3.0     # zeta outside {1,2,4,16}: a pass with base exponent 3, that element only
+    m.sf["zeta"][ang & (m.sf["zeta"] == 16.0) & (m.sf["central"] == 1)] = 3.0     # zeta {1,2,4,3}: still ONE menu (zeta0 = 1, zeta_x = 3), one pass
+    assert table_kernels(m) == ("free16", "free16")
+    m.sf["zeta"][ang & (m.sf["zeta"] == 4.0) & (m.sf["central"] == 1)] = 5.0      # {1,2,5,3}: menus (1; 3) and (5): two passes, that element only
     assert table_kernels(m) == ("free16", "multi")
     m = W.make_model(False)
     m.sf["kind"][np.nonzero(ang)[0][0]] = 9                         # one wide angular SF on element 0: a pass of its own
     assert table_kernels(m) == ("multi", "base12")
-    m.sf["zeta"][np.nonzero(ang)[0][0]] = 3.0                       # ... with zeta = 3: still a pass of its own (base exponent 3)
+    m.sf["zeta"][np.nonzero(ang)[0][0]] = 3.0                       # ... with zeta = 3: still a pass of its own (menu zeta0 = 3)
     assert table_kernels(m) == ("multi", "base12")
     m = W.make_model(False)
     q = np.nonzero(ang)[0][:5]
     m.sf["eta"][q] = [0.002, 0.003, 0.004, 0.005, 0.006]           # more than four eta values: several passes of the free-eta kernels
     assert table_kernels(m)[0] == "multi"
     rows = [(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0)] + [(0, 3, 0, 0, 0.01, 0.0, 1.0, float(z)) for z in (1, 2, 3, 4, 6, 8, 12, 16, 48, 64)]
-    assert table_kernels(tiny_model(rows)) == ("multi",)            # bases 1 (1,2,4,16), 3 (3,6,12,48), 8 (8), 64: four passes
+    assert table_kernels(tiny_model(rows)) == ("multi",)            # menus (1,2,4;16), (3,6,12;48), (8;64): three passes
     rows = [(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0)] + [(0, 3, 0, 0, 0.01, 0.0, 1.0, float(z)) for z in (3, 5, 7, 9, 11, 13, 15, 17, 19)]
-    assert table_kernels(tiny_model(rows)) == ("generic",)          # nine base exponents: more than 8 passes
+    assert table_kernels(tiny_model(rows)) == ("multi",)            # nine odd exponents: five menus of (zeta0; zeta_x)
+    rows = [(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0)] + [(0, 3, 0, 0, 0.01, 0.0, 1.0, float(z)) for z in range(3, 64, 2)]
+    assert table_kernels(tiny_model(rows)) == ("generic",)          # 31 odd exponents: 16 menus, more than 8 passes
     rows = [(0, 2, 0, 0, 0.1, 0.0, 0.0, 0.0)] + [(0, 3, 0, 0, 0.001 * (k + 1), 0.0, 1.0, 1.0) for k in range(33)]
     assert table_kernels(tiny_model(rows)) == ("generic",)          # 33 eta values: more than 8 passes of four
     m = W.make_model(False)

@@ -101,8 +101,8 @@ def test_wide_model_small_system():
 
 @pytest.mark.parametrize("route", ["multi", "generic"])
 def test_generic_table_three_elements(route):
-    # irregular table: zeta = 3 and 6, Rs != 0, a missing pair group, an element with few SFs, different hidden sizes ->
-    # passes with base exponents 1 and 3 of the lane-owned kernels ("multi"), or -- with one symmetry function listed
+    # irregular table: zeta = 1, 3 and 6, Rs != 0, a missing pair group, an element with few SFs, different hidden sizes ->
+    # two passes of the lane-owned kernels, exponent menus (1; 3) and (6) ("multi"), or -- with one symmetry function listed
     # twice, which no pass menu can hold -- the generic angular kernels; the generic network tiles either way
     rows = []
     for c in range(3):
@@ -217,6 +217,39 @@ def test_multi_pass_tables(n_elem):
     base.sf_cutoffs = list(rc2)
     s0, _ = W.build(W.CONFIGS[0])
     _check_full(base, s0)
+
+
+@pytest.mark.parametrize("zetas,kernels", [((1.0, 2.0, 4.0, 3.0), "free16"), ((2.0, 4.0, 8.0, 5.0), "free16"),
+                                           ((1.0, 2.0, 3.0, 4.0, 6.0, 12.0, 48.0, 64.0), "multi")])
+def test_zeta_menus(zetas, kernels):
+    # any integer zeta on the lane-owned kernels: a pass carries the exponent menu {zeta0, 2 zeta0, 4 zeta0, zeta_x};
+    # (1,2,4;3) and (2,4,8;5) are one pass each, the third set is the menus (1,2,4;3), (6,12;48), (64)
+    from paper_2002_00054_b200.binding import table_kernels
+    rows = []
+    for c in range(2):
+        for e1 in range(2):
+            rows.append((c, 2, e1, 0, 0.05, 0.0, 0.0, 0.0))
+        for (e1, e2) in ((0, 0), (0, 1), (1, 1)):
+            for q, z in enumerate(zetas):
+                rows.append((c, 3, e1, e2, 0.004, 0.0, 1.0, z))
+                if q % 2 == 0:
+                    rows.append((c, 3, e1, e2, 0.004, 0.0, -1.0, z))
+                else:
+                    rows.append((c, 3, e1, e2, 0.011, 0.0, -1.0, z))
+    model = tiny_model(rows, n_elem=2, hidden=(6, 5), seed=41)
+    assert table_kernels(model) == (kernels, kernels)
+    sysm = W.make_water(150, 5, L=16.7)
+    ref = _check_full(model, sysm)
+    if kernels == "multi":
+        # the same table in the mixed-precision mode: FP32 powers up to (1 +- cos)^64 <= 2^64 must not overflow, and no unused
+        # menu entry may (0 * inf = NaN)
+        from paper_2002_00054_b200 import NNP
+        nnp = NNP.from_model(model)
+        nnp.set_precision("mixed")
+        e_atom, e_total, force = _run(nnp, sysm.pos, sysm.types, sysm.box)
+        assert np.all(np.isfinite(force)) and np.all(np.isfinite(e_atom))
+        assert np.abs(force - ref.F).max() < 1e-4 and abs(e_total - ref.e_total) < 1e-5 * np.abs(ref.e_atom).sum()
+        nnp.close()
 
 
 def test_fast_path_large_cutoff_general_exp():
