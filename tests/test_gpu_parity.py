@@ -124,10 +124,11 @@ def test_generic_table_three_elements(route):
     _check_full(model, sysm)
 
 
-@pytest.mark.parametrize("elements", [("X",), ("A", "B", "C")])
+@pytest.mark.parametrize("elements", [("X",), ("A", "B", "C"), ("A", "B", "C", "D")])
 def test_fast_path_one_and_three_elements(elements):
-    # the base-12 table on 1 and 3 elements: the lane-owned kernels with a single tournament segment
-    # (1 group) and with 6 pair groups (pair index derived from the slots, not from the descriptor bits)
+    # the base-12 table on 1, 3 and 4 elements: the lane-owned kernels with a single tournament segment
+    # (1 group), with 6 and with 10 pair groups (pair index derived from the slots, not from the descriptor bits);
+    # 4 = NNP_MAX_ELEMENTS: every per-element array of the kernels at its full length
     model = W.make_model(False, seed=77, elements=elements, hidden=(9, 6))
     sysm = W.make_water(120, 9, L=15.0)
     sysm.types = (np.arange(sysm.n_atoms) % len(elements)).astype(np.int32)
