@@ -341,6 +341,7 @@ def main():
                     help="nnp_set_neighbor_skin: keep a candidate list of radius rc + SKIN across calls and filter the exact list "
                          "from it; rebuilt when an atom has moved SKIN/2 (decided on the device).  Not the headline: BASELINE.json's "
                          "metric rebuilds the list every call.  With static positions (no --md) no timed call rebuilds")
+    ap.add_argument("--max-neighbors", type=int, default=0, help="nnp_set_max_neighbors (0: the default; the Ni-like config 5 uses 24)")
     ap.add_argument("--deterministic", action="store_true",
                     help="nnp_set_deterministic_forces: fixed-point force accumulation (bit-reproducible forces)")
     ap.add_argument("--no-probe", action="store_true", help="skip the DFMA issue-rate probe (for ncu runs)")
@@ -405,7 +406,7 @@ def main():
     if args.deterministic:
         nnp.set_deterministic_forces(True)
     if cfg.kind == "metal":
-        nnp.set_max_neighbors(32)      # 18 neighbours per atom: the 8-lanes-per-centre kernels of k_small.cu
+        nnp.set_max_neighbors(args.max_neighbors or 24)      # 18 neighbours per atom: the 8-lanes-per-centre kernels of k_small.cu (24 slots)
     if args.reuse_skin > 0.0:
         nnp.set_neighbor_skin(args.reuse_skin)
     pos = torch.tensor(sysm.pos, dtype=torch.float64, device=dev)

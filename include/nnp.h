@@ -121,8 +121,10 @@ nnp_status nnp_table_kernels(int32_t n_elem, double rc, int32_t n_sf, const nnp_
 void nnp_destroy(nnp_model* m);
 
 /* Upper bound on neighbours per atom the kernels provision for (PAPER.md L48 / L116: the per-atom neighbour list;
- * default 160 -- the water-like workloads average 91, Poisson tail < 150 at 2.1 M atoms).  Range 32..NNP_MAX_NEIGHBORS
- * (below 32: NNP_ERR_INVALID_ARG; above 255: NNP_ERR_LIMIT -- the kernels address neighbour slots with 8 bits). */
+ * default 160 -- the water-like workloads average 91, Poisson tail < 150 at 2.1 M atoms).  Range 16..NNP_MAX_NEIGHBORS
+ * (below 16: NNP_ERR_INVALID_ARG; above 255: NNP_ERR_LIMIT -- the kernels address neighbour slots with 8 bits).  The value
+ * also selects kernels: up to 32 the small-neighbourhood kernels (eight lanes per centre; up to 24 with smaller per-centre
+ * shared memory -- the paper's Ni system has 18 neighbours, PAPER.md L70 / L96), up to 64 one warp per centre, else two. */
 nnp_status nnp_set_max_neighbors(nnp_model* m, int32_t max_neighbors);
 
 /* Neighbour-list reuse with a Verlet skin ("neighbor list", L116; an MD code rebuilds its

@@ -574,8 +574,8 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
     // precision 1 (nnp_set_precision: mixed): FP32 instantiations of BASELINE.json's two shapes, water-like exp range
     const bool f32 = precision == 1;
     if (max_nbr <= 32) {     // small neighbourhoods (metals): 8 lanes per centre (k_small.cu)
-        if (use[ANG_BASE12][1]) launches += launch_force_small(w, g, n, n_elem, d_prog, variant, rc, stride, g_stride, true, passes.fixed_forces, st);
-        if (use[ANG_BASE12][0]) launches += launch_force_small(w, g, n, n_elem, d_prog, variant, rc, stride, g_stride, false, passes.fixed_forces, st);
+        if (use[ANG_BASE12][1]) launches += launch_force_small(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, true, passes.fixed_forces, st);
+        if (use[ANG_BASE12][0]) launches += launch_force_small(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, false, passes.fixed_forces, st);
         use[ANG_BASE12][0] = use[ANG_BASE12][1] = false;
     }
     if (use[ANG_BASE12][1]) launches += f32 ? launch_one2<SpecBase12, true, float>(p, st) : launch_one2<SpecBase12, true>(p, st);

@@ -366,8 +366,8 @@ int launch_sf2(const Workspace& w, const Grid& g, int64_t n, int n_elem, const E
     int launches = 0;
     const bool f32 = precision == 1;     // nnp_set_precision: mixed (BASELINE.json's two shapes only)
     if (max_nbr <= 32) {     // small neighbourhoods (metals): 8 lanes per centre (k_small.cu)
-        if (use[ANG_BASE12][1]) launches += launch_sf_small(w, g, n, n_elem, d_prog, variant, rc, stride, g_stride, true, st);
-        if (use[ANG_BASE12][0]) launches += launch_sf_small(w, g, n, n_elem, d_prog, variant, rc, stride, g_stride, false, st);
+        if (use[ANG_BASE12][1]) launches += launch_sf_small(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, true, st);
+        if (use[ANG_BASE12][0]) launches += launch_sf_small(w, g, n, n_elem, d_prog, variant, rc, stride, max_nbr, g_stride, false, st);
         use[ANG_BASE12][0] = use[ANG_BASE12][1] = false;
     }
     if (use[ANG_BASE12][1]) launches += f32 ? launch_one_sf2<SpecBase12, true, float>(p, st) : launch_one_sf2<SpecBase12, true>(p, st);

@@ -23,7 +23,8 @@
 
 namespace nnp {
 
-constexpr int SM_SLOTS = 32;                              // neighbour slots per centre
+constexpr int SM_SLOTS = 32;                              // neighbour slots per centre: template parameter SLOTS = 32, or 24 for
+                                                          // max_neighbors <= 24 (10 instead of 8 resident CTAs of k_force_small)
 constexpr int SM_CPW = 4;                                 // centres per warp (8 lanes each)
 constexpr int SM_WARPS = 2;                               // warps per CTA
 constexpr int SM_CPC = SM_CPW * SM_WARPS;                 // centres per CTA
@@ -144,10 +145,10 @@ struct SmallPairs {
 
 // ---------------------------------------------------------------------------------------------- S2
 // shared memory per centre: p0 (ux,uy), p1 (uz,1/a), p2 (exp(-eta0 a^2), fc(a)) double2[32]; ra double[32]; list u16[SM_LIST]
-constexpr size_t SM_SF_BYTES = 3 * SM_SLOTS * 16 + SM_SLOTS * 8 + SM_LIST * 2;
+__host__ __device__ constexpr size_t sm_sf_bytes(int slots) { return (size_t)3 * slots * 16 + (size_t)slots * 8 + SM_LIST * 2; }
 
-template <class Spec, bool TINY>
-__global__ void __launch_bounds__(SM_WARPS * 32, 9) k_sf_small(const __grid_constant__ SmallParams p) {
+template <class Spec, bool TINY, int SLOTS>
+__global__ void __launch_bounds__(SM_WARPS * 32, 12) k_sf_small(const __grid_constant__ SmallParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NACC = Spec::NACC;
     static_assert(NACC <= 16 && !Spec::FREE_ETA, "k_sf_small: BASELINE.json's 12-function shape (<= 16 accumulators)");
@@ -161,12 +162,12 @@ __global__ void __launch_bounds__(SM_WARPS * 32, 9) k_sf_small(const __grid_cons
     // a group without work (past the end, or an element of another kernel) stays in the warp's loops with empty ranges
     const bool live = i0 < p.n && p.variant[tc] == Spec::ID && (prog->tiny_exp != 0) == TINY;
 
-    unsigned char* base = smem_raw + (size_t)(wid * SM_CPW + grp) * SM_SF_BYTES;
+    unsigned char* base = smem_raw + (size_t)(wid * SM_CPW + grp) * sm_sf_bytes(SLOTS);
     double2* p0 = reinterpret_cast<double2*>(base);
-    double2* p1 = p0 + SM_SLOTS;
-    double2* p2 = p1 + SM_SLOTS;
-    double* ra = reinterpret_cast<double*>(p2 + SM_SLOTS);
-    uint16_t* list = reinterpret_cast<uint16_t*>(ra + SM_SLOTS);
+    double2* p1 = p0 + SLOTS;
+    double2* p2 = p1 + SLOTS;
+    double* ra = reinterpret_cast<double*>(p2 + SLOTS);
+    uint16_t* list = reinterpret_cast<uint16_t*>(ra + SLOTS);
 
     int seg[MAX_ELEM + 1];
     seg[0] = 0;
@@ -179,14 +180,14 @@ __global__ void __launch_bounds__(SM_WARPS * 32, 9) k_sf_small(const __grid_cons
     const int32_t* row = p.nbr + (size_t)i * p.stride;
     const double eta0 = prog->ang_eta[0];
     // (the <= 4 slots of a lane: all neighbour indices first, then all coordinates -- two round trips instead of eight)
-    int jn[SM_SLOTS / 8];
-    double xj[SM_SLOTS / 8], yj[SM_SLOTS / 8], zj[SM_SLOTS / 8];
+    int jn[SLOTS / 8];
+    double xj[SLOTS / 8], yj[SLOTS / 8], zj[SLOTS / 8];
 #pragma unroll
-    for (int q = 0; q < SM_SLOTS / 8; ++q) jn[q] = gl + 8 * q < ntot ? row[gl + 8 * q] : (int)i;
+    for (int q = 0; q < SLOTS / 8; ++q) jn[q] = gl + 8 * q < ntot ? row[gl + 8 * q] : (int)i;
 #pragma unroll
-    for (int q = 0; q < SM_SLOTS / 8; ++q) { xj[q] = p.sx[jn[q]]; yj[q] = p.sy[jn[q]]; zj[q] = p.sz[jn[q]]; }
+    for (int q = 0; q < SLOTS / 8; ++q) { xj[q] = p.sx[jn[q]]; yj[q] = p.sy[jn[q]]; zj[q] = p.sz[jn[q]]; }
 #pragma unroll
-    for (int q = 0; q < SM_SLOTS / 8; ++q) {
+    for (int q = 0; q < SLOTS / 8; ++q) {
         const int m = gl + 8 * q;
         if (m >= ntot) continue;
         const double dx = min_image_1d(xi, xj[q], p.box[0], p.half[0]);
@@ -289,8 +290,8 @@ __global__ void __launch_bounds__(SM_WARPS * 32, 9) k_sf_small(const __grid_cons
 // ---------------------------------------------------------------------------------------------- S4
 // shared memory per centre: p0 (ux,uy), p1 (uz,1/a), p2 (fc(a), fc'(a)/a) double2[32]; e0, rad, fx, fy, fz double[32];
 // beta row double[g_stride]; coefficients c_b = beta_b 2^(1-zeta_b) double[npair][16]; list u16[SM_LIST]
-__host__ __device__ constexpr size_t sm_force_bytes(int g_stride, int n_elem) {
-    return (size_t)3 * SM_SLOTS * 16 + 5 * SM_SLOTS * 8 + (size_t)((g_stride + 1) & ~1) * 8 +
+__host__ __device__ constexpr size_t sm_force_bytes(int g_stride, int n_elem, int slots) {
+    return (size_t)3 * slots * 16 + (size_t)5 * slots * 8 + (size_t)((g_stride + 1) & ~1) * 8 +
            (size_t)(n_elem * (n_elem + 1) / 2) * 16 * 8 + SM_LIST * 2;
 }
 
@@ -312,8 +313,8 @@ __device__ __forceinline__ void small_slot_add(double* fx, double* fy, double* f
     }
 }
 
-template <class Spec, bool TINY>
-__global__ void __launch_bounds__(SM_WARPS * 32, 8) k_force_small(const __grid_constant__ SmallParams p) {
+template <class Spec, bool TINY, int SLOTS>
+__global__ void __launch_bounds__(SM_WARPS * 32, SLOTS <= 24 ? 10 : 8) k_force_small(const __grid_constant__ SmallParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int NACC = Spec::NACC;
     static_assert(NACC <= 16 && !Spec::FREE_ETA, "k_force_small: BASELINE.json's 12-function shape (<= 16 accumulators)");
@@ -328,16 +329,16 @@ __global__ void __launch_bounds__(SM_WARPS * 32, 8) k_force_small(const __grid_c
     const bool live = i0 < p.n && p.variant[tc] == Spec::ID && (prog->tiny_exp != 0) == TINY;
 
     const int npair = p.n_elem * (p.n_elem + 1) / 2;
-    unsigned char* base = smem_raw + (size_t)(wid * SM_CPW + grp) * sm_force_bytes(p.g_stride, p.n_elem);
+    unsigned char* base = smem_raw + (size_t)(wid * SM_CPW + grp) * sm_force_bytes(p.g_stride, p.n_elem, SLOTS);
     double2* p0 = reinterpret_cast<double2*>(base);
-    double2* p1 = p0 + SM_SLOTS;
-    double2* p2 = p1 + SM_SLOTS;
-    double* e0 = reinterpret_cast<double*>(p2 + SM_SLOTS);
-    double* rad = e0 + SM_SLOTS;
-    double* fx = rad + SM_SLOTS;
-    double* fy = fx + SM_SLOTS;
-    double* fz = fy + SM_SLOTS;
-    double* brow = fz + SM_SLOTS;
+    double2* p1 = p0 + SLOTS;
+    double2* p2 = p1 + SLOTS;
+    double* e0 = reinterpret_cast<double*>(p2 + SLOTS);
+    double* rad = e0 + SLOTS;
+    double* fx = rad + SLOTS;
+    double* fy = fx + SLOTS;
+    double* fz = fy + SLOTS;
+    double* brow = fz + SLOTS;
     double* cft = brow + ((p.g_stride + 1) & ~1);
     uint16_t* list = reinterpret_cast<uint16_t*>(cft + npair * 16);
 
@@ -354,14 +355,14 @@ __global__ void __launch_bounds__(SM_WARPS * 32, 8) k_force_small(const __grid_c
     const double xi = p.sx[i], yi = p.sy[i], zi = p.sz[i];
     const int32_t* row = p.nbr + (size_t)i * p.stride;
     const double eta0 = prog->ang_eta[0];
-    int jn[SM_SLOTS / 8];
-    double xj[SM_SLOTS / 8], yj[SM_SLOTS / 8], zj[SM_SLOTS / 8];
+    int jn[SLOTS / 8];
+    double xj[SLOTS / 8], yj[SLOTS / 8], zj[SLOTS / 8];
 #pragma unroll
-    for (int q = 0; q < SM_SLOTS / 8; ++q) jn[q] = gl + 8 * q < ntot ? row[gl + 8 * q] : (int)i;
+    for (int q = 0; q < SLOTS / 8; ++q) jn[q] = gl + 8 * q < ntot ? row[gl + 8 * q] : (int)i;
 #pragma unroll
-    for (int q = 0; q < SM_SLOTS / 8; ++q) { xj[q] = p.sx[jn[q]]; yj[q] = p.sy[jn[q]]; zj[q] = p.sz[jn[q]]; }
+    for (int q = 0; q < SLOTS / 8; ++q) { xj[q] = p.sx[jn[q]]; yj[q] = p.sy[jn[q]]; zj[q] = p.sz[jn[q]]; }
 #pragma unroll
-    for (int q = 0; q < SM_SLOTS / 8; ++q) {
+    for (int q = 0; q < SLOTS / 8; ++q) {
         const int m = gl + 8 * q;
         if (m >= ntot) continue;
         int e = 0;                                           // element of slot m
@@ -538,33 +539,47 @@ static SmallParams small_params(const Workspace& w, const Grid& g, int64_t n, in
     return p;
 }
 
-// SpecBase12 elements with max_neighbors <= 32; tiny = the element's exp variant (bit 8 of variant[])
+// SpecBase12 elements with max_neighbors <= 32; tiny = the element's exp variant (bit 8 of variant[]); 24 neighbour slots per
+// centre if max_neighbors <= 24 (rows never hold more than max_neighbors entries), else 32
+template <int SLOTS>
+static void launch_sf_small_slots(const SmallParams& p, unsigned grid, bool tiny, cudaStream_t st) {
+    const size_t smem = SM_CPC * sm_sf_bytes(SLOTS);
+    if (tiny) k_sf_small<SpecBase12, true, SLOTS><<<grid, SM_WARPS * 32, smem, st>>>(p);
+    else k_sf_small<SpecBase12, false, SLOTS><<<grid, SM_WARPS * 32, smem, st>>>(p);
+}
+
 int launch_sf_small(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                    const int* variant, double rc, int stride, int g_stride, bool tiny, cudaStream_t st) {
+                    const int* variant, double rc, int stride, int max_nbr, int g_stride, bool tiny, cudaStream_t st) {
     if (n == 0) return 0;
     const SmallParams p = small_params(w, g, n, n_elem, d_prog, variant, rc, stride, g_stride);
     const unsigned grid = (unsigned)((n + SM_CPC - 1) / SM_CPC);
-    const size_t smem = SM_CPC * SM_SF_BYTES;
-    if (tiny) k_sf_small<SpecBase12, true><<<grid, SM_WARPS * 32, smem, st>>>(p);
-    else k_sf_small<SpecBase12, false><<<grid, SM_WARPS * 32, smem, st>>>(p);
+    if (max_nbr <= 24) launch_sf_small_slots<24>(p, grid, tiny, st);
+    else launch_sf_small_slots<32>(p, grid, tiny, st);
     return 1;
 }
 
+template <int SLOTS>
+static void launch_force_small_slots(const SmallParams& p, unsigned grid, bool tiny, cudaStream_t st) {
+    const size_t smem = SM_CPC * sm_force_bytes(p.g_stride, p.n_elem, SLOTS);
+    static unsigned long long c1 = 0ull, c0 = 0ull;      // per device and instantiation (opt_in_smem): > 48 KB with wide G rows
+    if (tiny) {
+        opt_in_smem(k_force_small<SpecBase12, true, SLOTS>, &c1);
+        k_force_small<SpecBase12, true, SLOTS><<<grid, SM_WARPS * 32, smem, st>>>(p);
+    } else {
+        opt_in_smem(k_force_small<SpecBase12, false, SLOTS>, &c0);
+        k_force_small<SpecBase12, false, SLOTS><<<grid, SM_WARPS * 32, smem, st>>>(p);
+    }
+}
+
 int launch_force_small(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                       const int* variant, double rc, int stride, int g_stride, bool tiny, int fixed_forces, cudaStream_t st) {
+                       const int* variant, double rc, int stride, int max_nbr, int g_stride, bool tiny, int fixed_forces,
+                       cudaStream_t st) {
     if (n == 0) return 0;
     SmallParams p = small_params(w, g, n, n_elem, d_prog, variant, rc, stride, g_stride);
     p.fixed = fixed_forces;
     const unsigned grid = (unsigned)((n + SM_CPC - 1) / SM_CPC);
-    const size_t smem = SM_CPC * sm_force_bytes(g_stride, n_elem);
-    static unsigned long long c1 = 0ull, c0 = 0ull;      // per device (opt_in_smem): > 48 KB with wide G rows
-    if (tiny) {
-        opt_in_smem(k_force_small<SpecBase12, true>, &c1);
-        k_force_small<SpecBase12, true><<<grid, SM_WARPS * 32, smem, st>>>(p);
-    } else {
-        opt_in_smem(k_force_small<SpecBase12, false>, &c0);
-        k_force_small<SpecBase12, false><<<grid, SM_WARPS * 32, smem, st>>>(p);
-    }
+    if (max_nbr <= 24) launch_force_small_slots<24>(p, grid, tiny, st);
+    else launch_force_small_slots<32>(p, grid, tiny, st);
     return 1;
 }
 

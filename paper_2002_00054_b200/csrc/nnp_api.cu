@@ -751,7 +751,7 @@ extern "C" nnp_status nnp_set_deterministic_forces(nnp_model* m, int32_t enabled
 
 extern "C" nnp_status nnp_set_max_neighbors(nnp_model* m, int32_t max_neighbors) {
     if (!m) return NNP_ERR_INVALID_ARG;
-    if (max_neighbors < 32) return fail(m, NNP_ERR_INVALID_ARG, "max_neighbors must be >= 32");
+    if (max_neighbors < 16) return fail(m, NNP_ERR_INVALID_ARG, "max_neighbors must be >= 16");
     if (max_neighbors > NNP_MAX_NEIGHBORS)
         return fail(m, NNP_ERR_LIMIT, "max_neighbors > NNP_MAX_NEIGHBORS (255): the kernels address neighbour slots with 8 bits");
     m->max_nbr = max_neighbors;

@@ -245,9 +245,10 @@ int launch_force2(const Workspace& w, const Grid& g, int64_t n, int n_elem, cons
                   cudaStream_t st);
 // small neighbourhoods (max_neighbors <= 32; k_small.cu): 8 lanes per centre, SpecBase12 elements
 int launch_sf_small(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                    const int* variant, double rc, int stride, int g_stride, bool tiny, cudaStream_t st);
+                    const int* variant, double rc, int stride, int max_nbr, int g_stride, bool tiny, cudaStream_t st);
 int launch_force_small(const Workspace& w, const Grid& g, int64_t n, int n_elem, const ElemProgram* const* d_prog,
-                       const int* variant, double rc, int stride, int g_stride, bool tiny, int fixed_forces, cudaStream_t st);
+                       const int* variant, double rc, int stride, int max_nbr, int g_stride, bool tiny, int fixed_forces,
+                       cudaStream_t st);
 int launch_finalize(const Workspace& w, int64_t n, double* d_e_atom, double* d_e_total, double* d_force, int fixed_forces,
                     cudaStream_t st);
 

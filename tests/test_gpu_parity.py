@@ -290,6 +290,16 @@ def test_metal_like_small_neighbourhoods():
     _check_full(model, sysm, max_neighbors=48)
     _check_full(model, sysm)                       # and the default 160-slot kernels on the same system
     _check_full(model, sysm, max_neighbors=32)     # and the 8-lanes-per-centre kernels of k_small.cu
+    _check_full(model, sysm, max_neighbors=24)     # ... with 24 slots per centre (18 neighbours fit)
+    from paper_2002_00054_b200 import NNP, NNPError
+    nnp = NNP.from_model(model)
+    nnp.set_max_neighbors(16)                      # 18 neighbours do not fit 16: reported, not silently truncated
+    with pytest.raises(NNPError) as ei:
+        _run(nnp, sysm.pos, sysm.types, sysm.box)
+    assert ei.value.status == 4                    # NNP_ERR_NEIGHBOR_OVERFLOW
+    with pytest.raises(NNPError):
+        nnp.set_max_neighbors(15)
+    nnp.close()
 
 
 @pytest.mark.parametrize("elements", [("X",), ("H", "O"), ("A", "B", "C")])
@@ -313,6 +323,10 @@ def test_small_neighbourhood_kernels(elements):
     ang = big.sf["kind"] == 3
     big.sf["eta"][ang] *= 8.0
     _check_full(big, sysm, max_neighbors=32)
+    roff, _ = oracle.neighbor_list(sysm.pos, sysm.box, model.rc)
+    assert 16 < np.diff(roff).max() <= 24            # at most 22 neighbours: the same cases on the 24-slot instantiation
+    _check_full(model, sysm, max_neighbors=24)
+    _check_full(big, sysm, max_neighbors=24)
 
 
 def test_wide_angular_mixed_with_narrow():
