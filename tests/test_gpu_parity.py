@@ -327,6 +327,11 @@ def test_small_neighbourhood_kernels(elements):
     assert 16 < np.diff(roff).max() <= 24            # at most 22 neighbours: the same cases on the 24-slot instantiation
     _check_full(model, sysm, max_neighbors=24)
     _check_full(big, sysm, max_neighbors=24)
+    free = copy.deepcopy(model)                     # a table that is not BASELINE.json's: the lane-owned kernels, one warp per
+    free.sf["eta"][ang & (free.sf["eta"] == free.sf["eta"][ang].max())] *= 1.23      # centre, rows of 24 in 64 slots
+    from paper_2002_00054_b200.binding import table_kernels
+    assert set(table_kernels(free)) == {"free16"}
+    _check_full(free, sysm, max_neighbors=24)
 
 
 def test_wide_angular_mixed_with_narrow():
