@@ -173,7 +173,8 @@ def stratify(pos, types, box, rc, cnt, cnt0, n_random, seed):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("--config", type=int, required=True, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--config", type=int, required=True, choices=[0, 1, 2, 3, 4, 5],
+                    help="index into workloads.CONFIGS: 0-4 = BASELINE.json configs, 5 = the Ni-like workload (SURVEY.md 8(f)2)")
     ap.add_argument("--call", type=int, default=0, help="configs[1]: index of the call in the displacement sequence")
     ap.add_argument("--procs", type=int, default=os.cpu_count())
     ap.add_argument("--search", default="cells", choices=["cells", "brute"])

@@ -588,6 +588,30 @@ def test_full_size_configs_vs_golden(k):
     nnp.close()
 
 
+@pytest.mark.parametrize("max_neighbors", [24, 32])
+def test_full_size_ni_like_workload_vs_golden(max_neighbors):
+    """The Ni-like workload (workloads.CONFIGS[5]: 1,492,992 atoms, 18 neighbours each) at full size, in the
+    launch configurations bench.py --config 5 times (the small-neighbourhood kernels of csrc/k_small.cu with 24 and with 32
+    slots per centre), against the whole-system oracle results of tests/golden/fullsize_nickel1.5M.json."""
+    from paper_2002_00054_b200 import NNP
+    cfg = W.CONFIGS[5]
+    sysm, model = W.build(cfg)
+    g = _golden(cfg)
+    nnp = NNP.from_model(model)
+    nnp.set_max_neighbors(max_neighbors)
+    n = sysm.n_atoms
+    e_atom, e_total, force = _run(nnp, sysm.pos, sysm.types, sysm.box)
+    rep, off, idx = _check_against_golden(g, nnp, n, e_atom, e_total, force, model, sysm.types)
+    print("full-size parity %s (max_neighbors %d): %s" % (cfg.name, max_neighbors, json.dumps(rep)))
+    assert abs(e_total - e_atom.sum()) <= 1e-11 * np.abs(e_atom).sum()
+    cnt = np.diff(off)
+    assert 17.9 < cnt.mean() < 18.1 and cnt.max() <= 24
+    e_atom2, e_total2, force2 = _run(nnp, sysm.pos, sysm.types, sysm.box)
+    assert e_total2 == e_total and np.array_equal(e_atom2, e_atom)
+    assert np.abs(force2 - force).max() < 1e-11
+    nnp.close()
+
+
 def test_config1_displacement_sequence():
     """configs[1]: repeated evaluations with cumulative sigma = 0.01 A kicks (reading C15); positions
     drift out of the box and are re-wrapped by the library.  Parity at calls 0, 1, 50 (three atoms through
