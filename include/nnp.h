@@ -225,7 +225,8 @@ nnp_status nnp_set_deterministic_forces(nnp_model* m, int32_t enabled);
  *
  * nnp_md_run advances n_steps steps.  On entry d_force must hold the forces of d_pos (call nnp_compute
  * first); on return d_pos / d_vel / d_force / d_e_atom / d_e_total belong to the last step.  Positions are
- * NOT wrapped (nnp_compute wraps internally).  The neighbour list is rebuilt every step.
+ * NOT wrapped (nnp_compute wraps internally).  The neighbour list is rebuilt every step, or -- after
+ * nnp_set_neighbor_skin -- when an atom has moved half the skin (decided on the device, also inside the graph replay).
  *   h_mass   [n_elem] HOST, masses in amu, by element index
  *   d_vel    [n_atoms][3] device, in/out, A/fs
  * Everything is enqueued on cuda_stream; no synchronisation inside (except once at the start if the graph of a
