@@ -32,7 +32,8 @@ __device__ __forceinline__ int stencil_1d(int c, int nc, int* out) {
 // One warp per CELL: the atoms of a cell (all elements) share their stencil, so the run table, the flat candidate
 // index and the candidate loads are done once per chunk of 32 candidates and every centre of the cell tests the chunk
 // from registers (one atom per warp spent ~2/3 of its instructions on exactly that bookkeeping: 4.5 ms at 2.1 M atoms).
-// Lane a of a group of 32 centres keeps centre a's counters; its coordinates are broadcast from shared memory.
+// The centres' coordinates, row offsets and running counts sit in shared memory and are read as broadcasts.  A cell whose stencil
+// does not wrap (87 % of the cells of a 2.1 M-atom box) takes a branch-free test on raw differences (4.5 -> 3.33 -> 2.63 ms).
 template <int HW>
 __global__ void __launch_bounds__(NB_WARPS * 32)
 k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
@@ -43,6 +44,8 @@ k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
     constexpr int SW = 2 * HW + 1;
     __shared__ double cpos[NB_WARPS][3][32];
     __shared__ int32_t cidx[NB_WARPS][32];
+    __shared__ int32_t ccnt[NB_WARPS][32];       // neighbours found so far, per centre of the group
+    __shared__ size_t crow[NB_WARPS][32];        // first entry of the centre's row
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
     const int64_t c = (int64_t)blockIdx.x * NB_WARPS + wid;
     if (c >= g.ncell) return;
@@ -90,8 +93,10 @@ k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
             cpos[wid][0][lane] = sx[my]; cpos[wid][1][lane] = sy[my]; cpos[wid][2][lane] = sz[my];
         }
         cidx[wid][lane] = my;
+        ccnt[wid][lane] = 0;
+        crow[wid][lane] = (size_t)(my >= 0 ? my : 0) * stride;
         __syncwarp();
-        int cnt = 0;
+        int cnt = 0;                                    // lane a: neighbours of centre a found so far (copied from ccnt per element)
         for (int e = 0; e < n_elem; ++e) {
             const int32_t* cs = cell_start + (size_t)e * g.ncell;
             const int cnt_before = cnt;
@@ -126,6 +131,24 @@ k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
                     const bool have = f < total;
                     double xj = 0.0, yj = 0.0, zj = 0.0;
                     if (have) { xj = sx[j]; yj = sy[j]; zj = sz[j]; }
+                    const unsigned lt = (1u << lane) - 1u;
+                    if (!(wx || wy || wz)) {
+                        // a cell whose stencil does not wrap: raw differences, no branch in the test (a lane without a
+                        // candidate holds (0, 0, 0): whatever it computes is masked by `have`)
+                        for (int a = 0; a < ng; ++a) {
+                            const int i = cidx[wid][a];
+                            const double dx = __dsub_rn(xj, cpos[wid][0][a]), dy = __dsub_rn(yj, cpos[wid][1][a]),
+                                         dz = __dsub_rn(zj, cpos[wid][2][a]);
+                            const bool hit = have & (j != i) & (dist2_exact(dx, dy, dz) < rc2);
+                            const unsigned m = __ballot_sync(0xffffffffu, hit);
+                            const int base = ccnt[wid][a];
+                            const int p = base + __popc(m & lt);
+                            if (hit && p < max_nbr) nbr[crow[wid][a] + p] = j;
+                            __syncwarp();
+                            if (lane == 0) ccnt[wid][a] = base + __popc(m);
+                        }
+                        __syncwarp();
+                    } else
                     for (int a = 0; a < ng; ++a) {              // every centre of the group against this chunk
                         const int i = cidx[wid][a];
                         const double xi = cpos[wid][0][a], yi = cpos[wid][1][a], zi = cpos[wid][2][a];
@@ -137,15 +160,18 @@ k_neighbors(int64_t n, int n_elem, Grid g, double rc2, int stride, int max_nbr,
                             hit = dist2_exact(dx, dy, dz) < rc2;
                         }
                         const unsigned m = __ballot_sync(0xffffffffu, hit);
-                        const int base = __shfl_sync(0xffffffffu, cnt, a);
+                        const int base = ccnt[wid][a];
                         if (hit) {
                             const int p = base + __popc(m & ((1u << lane) - 1u));
                             if (p < max_nbr) nbr[(size_t)i * stride + p] = j;
                         }
-                        if (lane == a) cnt += __popc(m);
+                        __syncwarp();
+                        if (lane == 0) ccnt[wid][a] = base + __popc(m);
+                        __syncwarp();
                     }
                 }
             }
+            cnt = ccnt[wid][lane];
             if (my >= 0) nbr_cnt[(size_t)my * MAX_ELEM + e] = min(cnt, max_nbr) - min(cnt_before, max_nbr);
         }
         if (my >= 0) {
