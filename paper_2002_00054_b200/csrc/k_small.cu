@@ -41,6 +41,7 @@ struct SmallParams {
     const double* dEdG;                  // force kernel: in
     double* f_sorted;                    // force kernel: accumulated into
     int fixed;                           // 1: fixed-point force accumulation (nnp_internal.h force_add)
+    uint16_t* slist;                     // [N][SMALL_LIST_U16] pair lists handed from the SF kernel to the force kernel (or null)
     int32_t *status, *sticky;
     const ElemProgram* prog[MAX_ELEM];
     int variant[MAX_ELEM];
@@ -223,19 +224,37 @@ __global__ void __launch_bounds__(SM_WARPS * 32, 12) k_sf_small(const __grid_con
         }
     }
 
-    // ---- angular: pair group by pair group
+    // ---- angular: pair group by pair group.  The compacted (j, k) list of a group goes to the force kernel as well (it
+    // would enumerate and test the same 153 pairs again: ~16 % of its instructions on the Ni-like workload), if every
+    // group of the centre fits one fill and all of them together the per-centre budget; [0] = 0 marks a valid hand-over.
+    uint16_t* hlist = (p.slist && live) ? p.slist + (size_t)i * SMALL_LIST_U16 : nullptr;
+    bool ho_ok = hlist != nullptr;
+    int ho_off = 0;
     for (int e1 = 0; e1 < p.n_elem; ++e1)
         for (int e2 = e1; e2 < p.n_elem; ++e2) {
             const int pr = pair_index(e1, e2, p.n_elem);
             const bool on = live && prog->n_ang[pr] != 0;
+            if (hlist && gl == 0) hlist[1 + pr] = 0;
             if (!__any_sync(FULL, on)) continue;
             SmallPairs sp;
             sp.start(seg[e1], on ? seg[e1 + 1] - seg[e1] : 0, seg[e2], on ? seg[e2 + 1] - seg[e2] : 0, e1 == e2, gl);
             double acc[NACC];
 #pragma unroll
             for (int a = 0; a < NACC; ++a) acc[a] = 0.0;
+            int fills = 0;
             while (__any_sync(FULL, !sp.done())) {
+            const bool had_work = !sp.done();
             const int cnt = sp.fill(p0, p1, p.rc2, list, SM_LIST, gl, grp);
+            if (had_work) {
+                ++fills;
+                if (ho_ok && fills == 1 && sp.done() && ho_off + cnt <= SMALL_LIST_U16 - SMALL_LIST_HDR) {
+                    for (int t = gl; t < cnt; t += 8) hlist[SMALL_LIST_HDR + ho_off + t] = list[t];
+                    if (gl == 0) hlist[1 + pr] = (uint16_t)cnt;
+                    ho_off += cnt;
+                } else {
+                    ho_ok = false;
+                }
+            }
             for (int t = gl; t < cnt; t += 8) {
                 const int jk = list[t], j = jk >> 8, k = jk & 255;
                 const double2 a0 = p0[j], a1 = p1[j], a2 = p2[j], k0 = p0[k], k1 = p1[k], k2v = p2[k];
@@ -285,6 +304,7 @@ __global__ void __launch_bounds__(SM_WARPS * 32, 12) k_sf_small(const __grid_con
             }
             __syncwarp();                              // the list is reused by the next pair group
         }
+    if (hlist && gl == 0) hlist[0] = ho_ok ? 0 : 1;
 }
 
 // ---------------------------------------------------------------------------------------------- S4
@@ -414,19 +434,35 @@ __global__ void __launch_bounds__(SM_WARPS * 32, SLOTS <= 24 ? 10 : 8) k_force_s
 #pragma unroll
     for (int e = 0; e < Spec::NETA; ++e) eta[e] = prog->ang_eta[e];
 
+    // the pair lists of the symmetry-function kernel, if it handed them over for this centre (k_sf_small)
+    const uint16_t* hlist = (p.slist && live) ? p.slist + (size_t)i * SMALL_LIST_U16 : nullptr;
+    const bool use_ho = hlist != nullptr && hlist[0] == 0;
+    int ho_off = 0;
+
     // ---- angular part: pair group by pair group
     for (int e1 = 0; e1 < p.n_elem; ++e1)
         for (int e2 = e1; e2 < p.n_elem; ++e2) {
             const int pr = pair_index(e1, e2, p.n_elem);
             const bool on = live && prog->n_ang[pr] != 0;
             if (!__any_sync(FULL, on)) continue;
+            // a centre whose lists came from the SF kernel enumerates nothing (empty ranges: it idles through fill())
+            const bool mine = on && !use_ho;
             SmallPairs sp;
-            sp.start(seg[e1], on ? seg[e1 + 1] - seg[e1] : 0, seg[e2], on ? seg[e2 + 1] - seg[e2] : 0, e1 == e2, gl);
+            sp.start(seg[e1], mine ? seg[e1 + 1] - seg[e1] : 0, seg[e2], mine ? seg[e2 + 1] - seg[e2] : 0, e1 == e2, gl);
+            const int hc = (on && use_ho) ? (int)hlist[1 + pr] : 0;
+            bool pend = hc > 0;
             double cf[NACC];
 #pragma unroll
             for (int a = 0; a < NACC; ++a) cf[a] = cft[pr * 16 + a];
-            while (__any_sync(FULL, !sp.done())) {
-            const int cnt = sp.fill(p0, p1, p.rc2, list, SM_LIST, gl, grp);
+            while (__any_sync(FULL, !sp.done() || pend)) {
+            int cnt = sp.fill(p0, p1, p.rc2, list, SM_LIST, gl, grp);
+            if (pend) {
+                for (int t = gl; t < hc; t += 8) list[t] = hlist[SMALL_LIST_HDR + ho_off + t];
+                cnt = hc;
+                ho_off += hc;
+                pend = false;
+            }
+            __syncwarp();
             const int rounds = (cnt + 7) >> 3;
             for (int q = 0; q < rounds; ++q) {
                 const int t = q * 8 + gl;
@@ -531,7 +567,7 @@ static SmallParams small_params(const Workspace& w, const Grid& g, int64_t n, in
     p.sx = w.sx; p.sy = w.sy; p.sz = w.sz;
     p.cell_start = w.cell_start; p.nbr = w.nbr; p.nbr_cnt = w.nbr_cnt;
     p.G = w.G; p.dEdG = w.dEdG; p.f_sorted = w.f_sorted;
-    p.fixed = 0; p.status = w.status; p.sticky = w.sticky;
+    p.fixed = 0; p.status = w.status; p.sticky = w.sticky; p.slist = w.slist;
     for (int e = 0; e < MAX_ELEM; ++e) {
         p.prog[e] = e < n_elem ? d_prog[e] : nullptr;
         p.variant[e] = e < n_elem ? (variant[e] & 255) : -1;

@@ -135,6 +135,7 @@ static size_t ws_layout(Workspace* w, void* base, int64_t n, int n_elem, int str
         w->bx = (double*)take(N * 8); w->by = (double*)take(N * 8); w->bz = (double*)take(N * 8);
         w->skin_flag = (int32_t*)take(64);
     }
+    w->slist = stride <= 32 ? (uint16_t*)take(N * (size_t)SMALL_LIST_U16 * 2) : nullptr;
     w->G = (double*)take(N * (size_t)g_stride * 8);
     w->dEdG = (double*)take(N * (size_t)g_stride * 8);
     w->e_sorted = (double*)take(N * 8);

@@ -54,6 +54,9 @@ enum AngVariant : int { ANG_GENERIC = 0, ANG_BASE12 = 1, ANG_WIDE32 = 2, ANG_FRE
 // {zeta0, 2 zeta0, 4 zeta0, zeta_x} for one pair (zeta0, zeta_x), runs as several passes -- G entries are independent and the forces are additive
 // over the symmetry functions.  ANG_FREE16 / ANG_FREE32 = one pass at the
 // global rc; ANG_MULTI = anything else that fits MAX_PASS passes.
+// hand-over of the pair lists in k_small.cu: per centre [0] = 0 if valid, [1 + pair group] = entries of the group, [16 ..) the entries
+constexpr int SMALL_LIST_U16 = 256;
+constexpr int SMALL_LIST_HDR = 16;
 constexpr int MAX_PASS = 8;
 struct AngPass {
     double eta[MAX_ETA];
@@ -156,6 +159,8 @@ struct Workspace {
     double *bx, *by, *bz;            // [N] wrapped positions at the last rebuild, sorted order
     int32_t *skin_flag;              // device word: this call rebuilds (set by the host or by k_skin_check)
     int32_t *skin_stats;             // model-owned: [0] calls, [1] rebuilds since nnp_set_neighbor_skin
+    uint16_t *slist;                 // small-neighbourhood kernels only (row stride <= 32, else null): [N][SMALL_LIST_U16] the compacted
+                                     // (j, k) lists of a centre, handed from k_sf_small to k_force_small (k_small.cu)
     double *G, *dEdG;                // [N][g_stride], sorted order
     double *e_sorted;                // [N]
     double *f_sorted;                // [N][3]

@@ -327,6 +327,12 @@ def test_small_neighbourhood_kernels(elements):
     assert 16 < np.diff(roff).max() <= 24            # at most 22 neighbours: the same cases on the 24-slot instantiation
     _check_full(model, sysm, max_neighbors=24)
     _check_full(big, sysm, max_neighbors=24)
+    if len(elements) <= 2:
+        # rc = 3.6 A: up to 29 neighbours; with one element 27 of the 290 centres have more than 120 contributing pairs, so their
+        # lists are NOT handed from k_sf_small to k_force_small (which enumerates them itself) while their warp-mates' lists are;
+        # with two elements the three groups of a centre share the 240-entry budget
+        wider = W.make_model(False, seed=23, rc=3.6, elements=elements, hidden=(9, 6))
+        _check_full(wider, sysm, max_neighbors=32)
     free = copy.deepcopy(model)                     # a table that is not BASELINE.json's: the lane-owned kernels, one warp per
     free.sf["eta"][ang & (free.sf["eta"] == free.sf["eta"][ang].max())] *= 1.23      # centre, rows of 24 in 64 slots
     from paper_2002_00054_b200.binding import table_kernels
